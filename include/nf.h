@@ -1,0 +1,155 @@
+/* nf.h -- C ABI of the B200-native NeuralFluid pressure projection (forward + adjoint), MGPCG solver,
+ * face-weight builder and semi-Lagrangian advection.
+ *
+ * Paper: arXiv 2405.14903 (NeuralFluid); cited below as PAPER.md:Lnnn.  Readings of silent / garbled
+ * passages are listed in DESIGN.md section 3 and cited as R<n>.
+ *
+ * Conventions ("pressures stored at cell centers and velocities at cell faces"):
+ *   - All field arrays are float32, C-ordered [k][j][i] with x (i) fastest.
+ *       p   : cells  nz * ny * nx
+ *       u   : x-faces nz * ny * (nx+1)      u[k][j][i] is the face between cells i-1 and i
+ *       v   : y-faces nz * (ny+1) * nx
+ *       w   : z-faces (nz+1) * ny * nx
+ *       sdf : nodes  (nz+1) * (ny+1) * (nx+1), > 0 in fluid (R1, R2)
+ *   - G  (cells -> faces): (G p)_u[i] = p[i] - p[i-1];  G^T f = f_u[i]-f_u[i+1] + f_v[j]-f_v[j+1] + f_w[k]-f_w[k+1];
+ *     -(1/dx) G^T is the divergence.  S = diag(alpha), c = dt_over_rho/dx, A = c G^T S G
+ *     (Eq. 4).
+ *   - Domain faces are numbered 0..5 = -x,+x,-y,+y,-z,+z.
+ *
+ * Pointers: unless a function name ends in `_host`, EVERY array pointer is a DEVICE pointer owned by the
+ * caller (e.g. a contiguous float32 torch tensor).  The library never frees or retains a caller pointer
+ * after the call returns; it copies what it needs.  `_host` entry points take HOST pointers (pageable or
+ * pinned) and perform the host<->device copies themselves on the handle's stream.
+ *
+ * Execution: all kernels are enqueued on the handle's stream (nf_set_stream).  Calls that contain a
+ * solve (nf_solve, nf_project, nf_project_adjoint) return once the iteration count is known (the host
+ * polls a mapped status word; it never calls cudaDeviceSynchronize); results are ordered on the stream.
+ * Every other call only enqueues work.  There is NO CPU fallback: every step runs in CUDA kernels.
+ *
+ * Errors: functions return an int status.  Negative = error, nothing useful written; NF_NOT_CONVERGED = the
+ * best iterate was written but maxit was hit.  No exceptions, no exit(), no stdout.
+ */
+#ifndef NF_H_
+#define NF_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nf_grid nf_grid; /* opaque: owns face weights, multigrid hierarchy, solver scratch */
+
+enum {
+  NF_OK = 0,
+  NF_NOT_CONVERGED = 1,
+  NF_ERR_INVALID = -1, /* NULL handle / pointer, non-positive size, bad enum value          */
+  NF_ERR_ALLOC = -2,   /* device or host allocation failed                                   */
+  NF_ERR_CUDA = -3,    /* a CUDA runtime call failed; see nf_last_error                      */
+  NF_ERR_STATE = -4    /* weights not set yet (call nf_set_solid or nf_set_weights first)    */
+};
+
+enum { NF_BC_CLOSED = 0, NF_BC_DIRICHLET = 1 };
+
+/* Library version string, e.g. "nf-b200 0.1 (sm_100a)". */
+const char *nf_version(void);
+
+/* Create a handle for an nx*ny*nz MAC grid with spacing dx.  Allocates the multigrid
+ * hierarchy ("hierarchical grid data structure") and all solver scratch on the current
+ * CUDA device.  Defaults: six closed walls, dt_over_rho = 1, stream 0. */
+int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out);
+void nf_grid_destroy(nf_grid *g);
+
+/* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy stream 0. */
+int nf_set_stream(nf_grid *g, void *cuda_stream);
+
+/* Delta t / rho of Eqs. 4-5 (R5).  c = dt_over_rho/dx. */
+int nf_set_dt_rho(nf_grid *g, float dt_over_rho);
+
+/* Domain boundary condition of face 0..5 (R6, R19): NF_BC_CLOSED = wall at rest, alpha forced to 0;
+ * NF_BC_DIRICHLET = a ghost cell one dx outside holds p_value (Eq. 15a generalised).
+ * Must be called BEFORE nf_set_solid / nf_set_weights; changing it afterwards invalidates the weights. */
+int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value);
+
+/* Solver options (PAPER.md:L230 names only "MGPCG"; every parameter is this library's choice, R13):
+ *   nu_pre / nu_post: red-black Gauss-Seidel sweeps before / after the coarse correction (default 1, 1);
+ *   refine: 0 = plain fp32 PCG (default), 1 = fp64 solution accumulator with true-residual restarts. */
+int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int refine);
+
+/* a-1  Face weights from the solid SDF: per face, the fluid area fraction alpha from
+ * the 4 node values at its corners (marching-squares area; the printed one-fluid-corner formula
+ * 1/2 * phi_A/(phi_A-phi_B) * phi_A/(phi_A-phi_D) and its companions, R3; alpha < 1e-4 -> 0, R4); closed
+ * domain walls get 0 (R19).  Builds the coarse-level weights of the hierarchy.  us/vs/ws: solid velocity
+ * on faces (same layout as u/v/w), any of them NULL = zero.  Copied; closed-wall faces are at rest. */
+int nf_set_solid(nf_grid *g, const float *sdf_nodes, const float *us, const float *vs, const float *ws);
+
+/* Test / power-user hook: install face weights directly (MAC face layout), bypassing the builder.
+ * Closed-wall faces are forced to 0.  The solid velocity is kept (zero if never set). */
+int nf_set_weights(nf_grid *g, const float *au, const float *av, const float *aw);
+int nf_get_weights(nf_grid *g, float *au, float *av, float *aw);
+/* Install only the solid velocity (NULL = zero), keeping the weights. */
+int nf_set_solid_velocity(nf_grid *g, const float *us, const float *vs, const float *ws);
+
+/* a-3..a-5  Solve A p = rhs with MGPCG, A = c G^T S G with homogeneous ghosts.
+ * Convergence (R11): ||r||_2 <= tol ||rhs||_2, x0 = 0.  rhs is taken as 0 on inactive cells (sum of the 6
+ * face weights = 0), where p = 0.  If no Dirichlet domain face carries an open weight the system is
+ * singular (R12): the mean of rhs over active cells is removed and p has zero mean over active cells.
+ * rhs is not modified.  p may not alias rhs. */
+int nf_solve(nf_grid *g, const float *rhs, float *p, float tol, int maxit);
+
+/* a-2, a-3..5, a-6  Pressure projection (Eqs. 4-5).  In: u,v,w = Uhat.  Out: u,v,w =
+ * U^{n+1} = Uhat - c G p on faces with alpha > 0 and = U_s on faces with alpha = 0 (R7, R19); p = P^{n+1}
+ * (scaled by dt_over_rho as set).  b = G^T (S Uhat + (I-S) U_s) + c alpha p_D on Dirichlet ghosts. */
+int nf_project(nf_grid *g, float *u, float *v, float *w, float *p, float tol, int maxit);
+
+/* a-7  Adjoint projection (Eqs. 6-7; L134-139 Eq. 9 in the derived forms R9, R10).
+ * In: gu,gv,gw = dJ/dU^{n+1}; p_saved = P^{n+1}; uhat_* = the projection's input velocity.
+ * Solves A y = -c G^T (M g), M = [alpha > 0], with the same hierarchy.
+ * Out: gu,gv,gw (in place) = dJ/dUhat = M g + S G y;
+ *      galpha_* (may be NULL) = dJ/dalpha_f = (G y)_f [ (Uhat - U_s)_f - c (G p)_f ];
+ *      gus_*    (may be NULL) = dJ/dU_s = (I-M) g + (I-S) G y;  both 0 on closed walls (R19);
+ *      y_out    (may be NULL) = the adjoint variable y (cell array). */
+int nf_project_adjoint(nf_grid *g, float *gu, float *gv, float *gw, const float *p_saved,
+                       const float *uhat_u, const float *uhat_v, const float *uhat_w,
+                       float *galpha_u, float *galpha_v, float *galpha_w,
+                       float *gus_u, float *gus_v, float *gus_w, float *y_out, float tol, int maxit);
+
+/* a-8  Semi-Lagrangian advection (Eq. 2; L353-357 Eqs. 11-12; R14, R20): for every face
+ * position x of component c: v0 = U(x); x_m = x - dt/2 v0; v_m = U(x_m); x_b = x - dt v_m;
+ * out_c = U_c(x_b), U(.) = per-component trilinear interpolation, positions clamped to the lattice.
+ * In place (the library reads from an internal copy). */
+int nf_advect(nf_grid *g, float *u, float *v, float *w, float dt);
+
+/* a-9  Adjoint of nf_advect (Eq. 8).  u0,v0,w0 = the saved pre-advection U^n;
+ * in: gu,gv,gw = dJ/dUtilde; out (in place): dJ/dU^n. */
+int nf_advect_adjoint(nf_grid *g, const float *u0, const float *v0, const float *w0,
+                      float *gu, float *gv, float *gw, float dt);
+
+/* a-10  dJ/dalpha -> dJ/dphi at nodes, for the sdf last given to nf_set_solid.
+ * gsdf_nodes is overwritten. */
+int nf_weights_adjoint(nf_grid *g, const float *galpha_u, const float *galpha_v, const float *galpha_w,
+                       float *gsdf_nodes);
+
+/* Apply A to a cell array (q = A p, homogeneous ghosts) -- exposed for tests and kernel benchmarks. */
+int nf_apply_A(nf_grid *g, const float *p, float *q);
+/* One V-cycle z = M^{-1} r (zero initial guess) -- exposed for tests and kernel benchmarks. */
+int nf_vcycle(nf_grid *g, const float *r, float *z);
+
+/* Host-buffer variants: the same operations through HOST pointers; the host->device and device->host
+ * copies run on the handle's stream inside the call, which returns after the results are in host memory. */
+int nf_project_host(nf_grid *g, float *u, float *v, float *w, float *p, float tol, int maxit);
+int nf_project_adjoint_host(nf_grid *g, float *gu, float *gv, float *gw, const float *p_saved,
+                            const float *uhat_u, const float *uhat_v, const float *uhat_w, float tol, int maxit);
+
+/* Info about the last solve on this handle.  Synchronises the handle's stream.
+ * relres = ||r||_2/||rhs||_2 as tracked by the solver; ms = device time of the solve (CUDA events). */
+int nf_last_solve_info(nf_grid *g, int *iters, float *relres, float *ms);
+/* Number of multigrid levels; number of active cells; 1 if the current system is singular (R12). */
+int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, int *singular);
+/* Kernels launched by this handle since creation (for bench.py's gpu_launches). */
+long long nf_launch_count(nf_grid *g);
+/* Last error message of this handle (static storage inside the handle; "" if none). */
+const char *nf_last_error(nf_grid *g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NF_H_ */

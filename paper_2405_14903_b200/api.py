@@ -1,0 +1,264 @@
+"""Thin ctypes binding of the C-ABI library (include/nf.h).  Argument marshalling only: every step of the hot
+path runs in the CUDA kernels of csrc/.  torch is used for device memory and streams (PAPER.md:L145 exposes the
+simulator to PyTorch the same way).  There is no CPU fallback: if libnf_b200.so is missing this module raises.
+
+Function names follow include/nf.h one to one (`Grid.project` -> nf_project, ...)."""
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnf_b200.so")
+
+NF_OK, NF_NOT_CONVERGED = 0, 1
+NF_ERR_INVALID, NF_ERR_ALLOC, NF_ERR_CUDA, NF_ERR_STATE = -1, -2, -3, -4
+BC_CLOSED, BC_DIRICHLET = 0, 1
+
+_c_float_p = ctypes.c_void_p  # raw device (or host) addresses
+_SIGNATURES = {
+    "nf_version": (ctypes.c_char_p, []),
+    "nf_grid_create": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_float,
+                                      ctypes.POINTER(ctypes.c_void_p)]),
+    "nf_grid_destroy": (None, [ctypes.c_void_p]),
+    "nf_set_stream": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "nf_set_dt_rho": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
+    "nf_set_domain_bc": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_float]),
+    "nf_set_solver_options": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "nf_set_solid": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
+    "nf_set_weights": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3),
+    "nf_get_weights": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3),
+    "nf_set_solid_velocity": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3),
+    "nf_solve": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p, ctypes.c_float, ctypes.c_int]),
+    "nf_project": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4 + [ctypes.c_float, ctypes.c_int]),
+    "nf_project_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 14 + [ctypes.c_float, ctypes.c_int]),
+    "nf_advect": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.c_float]),
+    "nf_advect_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 6 + [ctypes.c_float]),
+    "nf_weights_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
+    "nf_apply_A": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p]),
+    "nf_vcycle": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p]),
+    "nf_project_host": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4 + [ctypes.c_float, ctypes.c_int]),
+    "nf_project_adjoint_host": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 7 + [ctypes.c_float, ctypes.c_int]),
+    "nf_last_solve_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_int),
+                                          ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
+    "nf_grid_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_int),
+                                    ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_int)]),
+    "nf_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
+    "nf_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
+}
+EXPORTED_SYMBOLS = tuple(_SIGNATURES)
+
+_lib = None
+
+
+def load_library(path=None):
+    """dlopen libnf_b200.so and declare every signature of include/nf.h.  Raises if the library is missing."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise RuntimeError("%s not found: build it with `python -m paper_2405_14903_b200.build` "
+                           "(there is no CPU fallback)" % path)
+    lib = ctypes.CDLL(path)
+    for name, (res, args) in _SIGNATURES.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+class NfError(RuntimeError):
+    pass
+
+
+def _ptr(t):
+    """Device (or host) address of a contiguous float32 torch tensor; None -> NULL."""
+    if t is None:
+        return None
+    import torch
+    if not isinstance(t, torch.Tensor):
+        raise TypeError("expected a torch.Tensor or None")
+    if t.dtype != torch.float32 or not t.is_contiguous():
+        raise ValueError("arrays must be contiguous float32 tensors")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+class Grid:
+    """Owner of one nf_grid handle.  Tensors are passed by address; shapes follow include/nf.h:
+    p (nz,ny,nx), u (nz,ny,nx+1), v (nz,ny+1,nx), w (nz+1,ny,nx), sdf (nz+1,ny+1,nx+1)."""
+
+    def __init__(self, nx, ny, nz, dx, device=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2405_14903_b200 needs a CUDA device (there is no CPU fallback)")
+        self.lib = load_library()
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self.nx, self.ny, self.nz, self.dx = int(nx), int(ny), int(nz), float(dx)
+        h = ctypes.c_void_p()
+        with torch.cuda.device(self.device):
+            rc = self.lib.nf_grid_create(self.nx, self.ny, self.nz, self.dx, ctypes.byref(h))
+        if rc != NF_OK:
+            raise NfError("nf_grid_create failed with %d" % rc)
+        self.h = h
+        self.set_stream(torch.cuda.current_stream(self.device))
+
+    # -- shapes -------------------------------------------------------------------------------------------
+    @property
+    def shape_p(self):
+        return (self.nz, self.ny, self.nx)
+
+    @property
+    def shape_u(self):
+        return (self.nz, self.ny, self.nx + 1)
+
+    @property
+    def shape_v(self):
+        return (self.nz, self.ny + 1, self.nx)
+
+    @property
+    def shape_w(self):
+        return (self.nz + 1, self.ny, self.nx)
+
+    @property
+    def shape_sdf(self):
+        return (self.nz + 1, self.ny + 1, self.nx + 1)
+
+    def _check(self, rc, name, allow_not_converged=True):
+        if rc == NF_OK or (allow_not_converged and rc == NF_NOT_CONVERGED):
+            return rc
+        msg = self.lib.nf_last_error(self.h)
+        raise NfError("%s failed with %d: %s" % (name, rc, msg.decode() if msg else ""))
+
+    def _expect(self, t, shape, name, host=False):
+        if t is None:
+            return
+        if tuple(t.shape) != tuple(shape):
+            raise ValueError("%s has shape %s, expected %s" % (name, tuple(t.shape), tuple(shape)))
+        if host and t.is_cuda:
+            raise ValueError("%s must be a host tensor" % name)
+        if not host and not t.is_cuda:
+            raise ValueError("%s must be a CUDA tensor" % name)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.nf_grid_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- configuration ------------------------------------------------------------------------------------
+    def set_stream(self, stream):
+        self._check(self.lib.nf_set_stream(self.h, ctypes.c_void_p(stream.cuda_stream)), "nf_set_stream")
+
+    def set_dt_rho(self, dt_over_rho):
+        self._check(self.lib.nf_set_dt_rho(self.h, float(dt_over_rho)), "nf_set_dt_rho")
+
+    def set_domain_bc(self, face, bc_type, p_value=0.0):
+        self._check(self.lib.nf_set_domain_bc(self.h, int(face), int(bc_type), float(p_value)), "nf_set_domain_bc")
+
+    def set_solver_options(self, nu_pre=1, nu_post=1, refine=0):
+        self._check(self.lib.nf_set_solver_options(self.h, nu_pre, nu_post, refine), "nf_set_solver_options")
+
+    def set_solid(self, sdf, us=None, vs=None, ws=None):
+        self._expect(sdf, self.shape_sdf, "sdf")
+        self._expect(us, self.shape_u, "us"); self._expect(vs, self.shape_v, "vs"); self._expect(ws, self.shape_w, "ws")
+        self._check(self.lib.nf_set_solid(self.h, _ptr(sdf), _ptr(us), _ptr(vs), _ptr(ws)), "nf_set_solid")
+
+    def set_weights(self, au, av, aw):
+        self._expect(au, self.shape_u, "au"); self._expect(av, self.shape_v, "av"); self._expect(aw, self.shape_w, "aw")
+        self._check(self.lib.nf_set_weights(self.h, _ptr(au), _ptr(av), _ptr(aw)), "nf_set_weights")
+
+    def get_weights(self):
+        import torch
+        au = torch.empty(self.shape_u, dtype=torch.float32, device=self.device)
+        av = torch.empty(self.shape_v, dtype=torch.float32, device=self.device)
+        aw = torch.empty(self.shape_w, dtype=torch.float32, device=self.device)
+        self._check(self.lib.nf_get_weights(self.h, _ptr(au), _ptr(av), _ptr(aw)), "nf_get_weights")
+        return au, av, aw
+
+    def set_solid_velocity(self, us=None, vs=None, ws=None):
+        self._expect(us, self.shape_u, "us"); self._expect(vs, self.shape_v, "vs"); self._expect(ws, self.shape_w, "ws")
+        self._check(self.lib.nf_set_solid_velocity(self.h, _ptr(us), _ptr(vs), _ptr(ws)), "nf_set_solid_velocity")
+
+    # -- hot path -----------------------------------------------------------------------------------------
+    def solve(self, rhs, p, tol=1e-6, maxit=200):
+        self._expect(rhs, self.shape_p, "rhs"); self._expect(p, self.shape_p, "p")
+        return self._check(self.lib.nf_solve(self.h, _ptr(rhs), _ptr(p), float(tol), int(maxit)), "nf_solve")
+
+    def project(self, u, v, w, p, tol=1e-6, maxit=200):
+        self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
+        self._expect(p, self.shape_p, "p")
+        return self._check(self.lib.nf_project(self.h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), float(tol), int(maxit)),
+                           "nf_project")
+
+    def project_adjoint(self, gu, gv, gw, p_saved=None, uhat=None, galpha=None, gus=None, y_out=None, tol=1e-6,
+                        maxit=200):
+        self._expect(gu, self.shape_u, "gu"); self._expect(gv, self.shape_v, "gv"); self._expect(gw, self.shape_w, "gw")
+        self._expect(p_saved, self.shape_p, "p_saved"); self._expect(y_out, self.shape_p, "y_out")
+        uh = uhat if uhat is not None else (None, None, None)
+        ga = galpha if galpha is not None else (None, None, None)
+        gs = gus if gus is not None else (None, None, None)
+        for trip, nm in ((uh, "uhat"), (ga, "galpha"), (gs, "gus")):
+            self._expect(trip[0], self.shape_u, nm + "_u"); self._expect(trip[1], self.shape_v, nm + "_v")
+            self._expect(trip[2], self.shape_w, nm + "_w")
+        rc = self.lib.nf_project_adjoint(self.h, _ptr(gu), _ptr(gv), _ptr(gw), _ptr(p_saved), _ptr(uh[0]), _ptr(uh[1]),
+                                         _ptr(uh[2]), _ptr(ga[0]), _ptr(ga[1]), _ptr(ga[2]), _ptr(gs[0]), _ptr(gs[1]),
+                                         _ptr(gs[2]), _ptr(y_out), float(tol), int(maxit))
+        return self._check(rc, "nf_project_adjoint")
+
+    def advect(self, u, v, w, dt):
+        self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
+        self._check(self.lib.nf_advect(self.h, _ptr(u), _ptr(v), _ptr(w), float(dt)), "nf_advect")
+
+    def advect_adjoint(self, u0, v0, w0, gu, gv, gw, dt):
+        for t, s, n in ((u0, self.shape_u, "u0"), (v0, self.shape_v, "v0"), (w0, self.shape_w, "w0"),
+                        (gu, self.shape_u, "gu"), (gv, self.shape_v, "gv"), (gw, self.shape_w, "gw")):
+            self._expect(t, s, n)
+        self._check(self.lib.nf_advect_adjoint(self.h, _ptr(u0), _ptr(v0), _ptr(w0), _ptr(gu), _ptr(gv), _ptr(gw),
+                                               float(dt)), "nf_advect_adjoint")
+
+    def weights_adjoint(self, gau, gav, gaw, gsdf):
+        self._expect(gau, self.shape_u, "gau"); self._expect(gav, self.shape_v, "gav")
+        self._expect(gaw, self.shape_w, "gaw"); self._expect(gsdf, self.shape_sdf, "gsdf")
+        self._check(self.lib.nf_weights_adjoint(self.h, _ptr(gau), _ptr(gav), _ptr(gaw), _ptr(gsdf)),
+                    "nf_weights_adjoint")
+
+    def apply_A(self, p, q):
+        self._expect(p, self.shape_p, "p"); self._expect(q, self.shape_p, "q")
+        self._check(self.lib.nf_apply_A(self.h, _ptr(p), _ptr(q)), "nf_apply_A")
+
+    def vcycle(self, r, z):
+        self._expect(r, self.shape_p, "r"); self._expect(z, self.shape_p, "z")
+        self._check(self.lib.nf_vcycle(self.h, _ptr(r), _ptr(z)), "nf_vcycle")
+
+    # -- host-buffer variants (e2e timing) ------------------------------------------------------------------
+    def project_host(self, u, v, w, p, tol=1e-6, maxit=200):
+        self._expect(u, self.shape_u, "u", host=True); self._expect(v, self.shape_v, "v", host=True)
+        self._expect(w, self.shape_w, "w", host=True); self._expect(p, self.shape_p, "p", host=True)
+        return self._check(self.lib.nf_project_host(self.h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), float(tol),
+                                                    int(maxit)), "nf_project_host")
+
+    def project_adjoint_host(self, gu, gv, gw, tol=1e-6, maxit=200):
+        self._expect(gu, self.shape_u, "gu", host=True); self._expect(gv, self.shape_v, "gv", host=True)
+        self._expect(gw, self.shape_w, "gw", host=True)
+        return self._check(self.lib.nf_project_adjoint_host(self.h, _ptr(gu), _ptr(gv), _ptr(gw), None, None, None,
+                                                            None, float(tol), int(maxit)), "nf_project_adjoint_host")
+
+    # -- info -------------------------------------------------------------------------------------------------
+    def last_solve_info(self):
+        it, rr, ms = ctypes.c_int(), ctypes.c_float(), ctypes.c_float()
+        self._check(self.lib.nf_last_solve_info(self.h, ctypes.byref(it), ctypes.byref(rr), ctypes.byref(ms)),
+                    "nf_last_solve_info")
+        return dict(iters=it.value, relres=rr.value, ms=ms.value)
+
+    def info(self):
+        lv, na, sg = ctypes.c_int(), ctypes.c_longlong(), ctypes.c_int()
+        self._check(self.lib.nf_grid_info(self.h, ctypes.byref(lv), ctypes.byref(na), ctypes.byref(sg)), "nf_grid_info")
+        return dict(levels=lv.value, active_cells=na.value, singular=sg.value)
+
+    def launch_count(self):
+        return int(self.lib.nf_launch_count(self.h))

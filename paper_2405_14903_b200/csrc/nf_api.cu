@@ -1,0 +1,337 @@
+// nf_api.cu -- the C ABI (include/nf.h): handle management, argument checking, and the composition of the
+// hot-path calls from the kernels in nf_weights.cu / nf_solver.cu / nf_project.cu / nf_advect.cu.
+#include <new>
+
+#include "nf_internal.cuh"
+
+#define NF_CHECK_HANDLE(g) \
+  do {                     \
+    if (!(g)) return NF_ERR_INVALID; \
+    (g)->err.clear();      \
+  } while (0)
+#define NF_TRY(expr)            \
+  do {                          \
+    int rc_ = (expr);           \
+    if (rc_ < 0) return rc_;    \
+  } while (0)
+
+extern "C" const char *nf_version(void) { return "nf-b200 0.1 (sm_100a)"; }
+
+template <typename T>
+static cudaError_t dalloc(T **p, size_t n) {
+  return cudaMalloc((void **)p, (n ? n : 1) * sizeof(T));
+}
+
+static void free_all(nf_grid *g) {
+  for (int l = 0; l < NF_MAX_LEVELS; ++l) {
+    NfLevel &L = g->lv[l];
+    cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.z); cudaFree(L.r);
+  }
+  cudaFree(g->us); cudaFree(g->vs); cudaFree(g->ws); cudaFree(g->sdf);
+  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->xd);
+  cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
+  cudaFree(g->st); cudaFree(g->d_counts);
+  if (g->hst) cudaFreeHost((void *)g->hst);
+  if (g->h_counts) cudaFreeHost(g->h_counts);
+  if (g->ev0) cudaEventDestroy(g->ev0);
+  if (g->ev1) cudaEventDestroy(g->ev1);
+  cudaFree(g->hs_u); cudaFree(g->hs_v); cudaFree(g->hs_w); cudaFree(g->hs_p);
+  cudaFree(g->hs_a); cudaFree(g->hs_b); cudaFree(g->hs_c); cudaFree(g->hs_d);
+}
+
+extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
+  if (!out) return NF_ERR_INVALID;
+  *out = nullptr;
+  if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0f)) return NF_ERR_INVALID;
+  if ((long long)(nx + 1) * (ny + 1) * (long long)(nz + 1) > (1LL << 31) * 4) return NF_ERR_INVALID;
+  nf_grid *g = new (std::nothrow) nf_grid();
+  if (!g) return NF_ERR_ALLOC;
+  g->nx = nx; g->ny = ny; g->nz = nz; g->dx = dx; g->dt_over_rho = 1.0f;
+  for (int f = 0; f < 6; ++f) { g->bc_type[f] = NF_BC_CLOSED; g->bc_val[f] = 0.0f; }
+  g->stream = 0;
+  g->nu_pre = 1; g->nu_post = 1; g->refine = 0;
+  g->weights_set = g->have_sdf = g->have_us = false;
+  g->singular = 1; g->nact = 0;
+  g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
+  for (int l = 0; l < NF_MAX_LEVELS; ++l) g->lv[l] = NfLevel{};
+  // hierarchy: halve while every extent is even and stays >= 4
+  int lx = nx, ly = ny, lz = nz, nl = 0;
+  float c = g->dt_over_rho / dx;
+  bool ok = true;
+  for (;;) {
+    NfLevel &L = g->lv[nl];
+    L.nx = lx; L.ny = ly; L.nz = lz;
+    L.pax = (lx + 1 + 3) & ~3;
+    L.ncell = (long long)lx * ly * lz;
+    L.c = c;
+    ok = ok && dalloc(&L.ax, (size_t)lz * ly * L.pax) == cudaSuccess;
+    ok = ok && dalloc(&L.ay, (size_t)lz * (ly + 1) * lx) == cudaSuccess;
+    ok = ok && dalloc(&L.az, (size_t)(lz + 1) * ly * lx) == cudaSuccess;
+    ok = ok && dalloc(&L.z, (size_t)L.ncell) == cudaSuccess;
+    ok = ok && dalloc(&L.r, (size_t)L.ncell) == cudaSuccess;
+    if (ok) ok = cudaMemset(L.ax, 0, (size_t)lz * ly * L.pax * sizeof(float)) == cudaSuccess;
+    ++nl;
+    if (!ok || nl >= NF_MAX_LEVELS) break;
+    if ((lx | ly | lz) & 1) break;
+    if (lx / 2 < 4 || ly / 2 < 4 || lz / 2 < 4) break;
+    lx /= 2; ly /= 2; lz /= 2;
+    c *= 0.25f;
+  }
+  g->nlev = nl;
+  const size_t nc = nf_nc(g);
+  ok = ok && dalloc(&g->us, nf_nu(g)) == cudaSuccess && dalloc(&g->vs, nf_nv(g)) == cudaSuccess &&
+       dalloc(&g->ws, nf_nw(g)) == cudaSuccess && dalloc(&g->sdf, nf_nn(g)) == cudaSuccess;
+  ok = ok && dalloc(&g->p, nc) == cudaSuccess && dalloc(&g->q, nc) == cudaSuccess &&
+       dalloc(&g->xtmp, nc) == cudaSuccess && dalloc(&g->xd, nc) == cudaSuccess;
+  ok = ok && dalloc(&g->fu, nf_nu(g)) == cudaSuccess && dalloc(&g->fv, nf_nv(g)) == cudaSuccess &&
+       dalloc(&g->fw, nf_nw(g)) == cudaSuccess;
+  ok = ok && dalloc(&g->st, 1) == cudaSuccess && dalloc(&g->d_counts, 2) == cudaSuccess;
+  ok = ok && cudaHostAlloc((void **)&g->hst, NF_RING * sizeof(NfHostStatus), cudaHostAllocMapped) == cudaSuccess;
+  ok = ok && cudaHostGetDevicePointer((void **)&g->hst_dev, (void *)g->hst, 0) == cudaSuccess;
+  ok = ok && cudaHostAlloc((void **)&g->h_counts, 2 * sizeof(double), cudaHostAllocDefault) == cudaSuccess;
+  ok = ok && cudaEventCreate(&g->ev0) == cudaSuccess && cudaEventCreate(&g->ev1) == cudaSuccess;
+  if (ok) {
+    for (int s = 0; s < NF_RING; ++s) { g->hst[s].seq = 0; g->hst[s].done = 0; g->hst[s].converged = 0; }
+    ok = nf_solver_init(g) == NF_OK;
+  }
+  if (!ok) {
+    cudaGetLastError();
+    free_all(g);
+    delete g;
+    return NF_ERR_ALLOC;
+  }
+  *out = g;
+  return NF_OK;
+}
+
+extern "C" void nf_grid_destroy(nf_grid *g) {
+  if (!g) return;
+  cudaStreamSynchronize(g->stream);
+  free_all(g);
+  delete g;
+}
+
+extern "C" int nf_set_stream(nf_grid *g, void *cuda_stream) {
+  NF_CHECK_HANDLE(g);
+  g->stream = (cudaStream_t)cuda_stream;
+  return NF_OK;
+}
+
+extern "C" int nf_set_dt_rho(nf_grid *g, float dt_over_rho) {
+  NF_CHECK_HANDLE(g);
+  if (!(dt_over_rho > 0.0f)) return NF_ERR_INVALID;
+  g->dt_over_rho = dt_over_rho;
+  float c = dt_over_rho / g->dx;
+  for (int l = 0; l < g->nlev; ++l) { g->lv[l].c = c; c *= 0.25f; }
+  return NF_OK;
+}
+
+extern "C" int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value) {
+  NF_CHECK_HANDLE(g);
+  if (face < 0 || face > 5 || (type != NF_BC_CLOSED && type != NF_BC_DIRICHLET)) return NF_ERR_INVALID;
+  g->bc_type[face] = type;
+  g->bc_val[face] = p_value;
+  g->weights_set = false;  // closed walls force alpha = 0: the weights must be rebuilt
+  return NF_OK;
+}
+
+extern "C" int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int refine) {
+  NF_CHECK_HANDLE(g);
+  if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || refine < 0 || refine > 1) return NF_ERR_INVALID;
+  g->nu_pre = nu_pre; g->nu_post = nu_post; g->refine = refine;
+  return NF_OK;
+}
+
+extern "C" int nf_set_solid(nf_grid *g, const float *sdf_nodes, const float *us, const float *vs, const float *ws) {
+  NF_CHECK_HANDLE(g);
+  if (!sdf_nodes) return NF_ERR_INVALID;
+  NF_TRY(nf_weights_from_sdf(g, sdf_nodes));
+  NF_TRY(nf_store_solid_velocity(g, us, vs, ws));
+  return nf_build_hierarchy(g);
+}
+
+extern "C" int nf_set_weights(nf_grid *g, const float *au, const float *av, const float *aw) {
+  NF_CHECK_HANDLE(g);
+  if (!au || !av || !aw) return NF_ERR_INVALID;
+  NF_TRY(nf_weights_from_user(g, au, av, aw));
+  return nf_build_hierarchy(g);
+}
+
+extern "C" int nf_get_weights(nf_grid *g, float *au, float *av, float *aw) {
+  NF_CHECK_HANDLE(g);
+  if (!g->weights_set) return NF_ERR_STATE;
+  return nf_weights_to_user(g, au, av, aw);
+}
+
+extern "C" int nf_set_solid_velocity(nf_grid *g, const float *us, const float *vs, const float *ws) {
+  NF_CHECK_HANDLE(g);
+  return nf_store_solid_velocity(g, us, vs, ws);
+}
+
+static int solve_timed(nf_grid *g, const float *src, float *x, float tol, int maxit) {
+  if (!(tol > 0.0f) || maxit < 1) return NF_ERR_INVALID;
+  NF_CUDA(g, cudaEventRecord(g->ev0, g->stream));
+  NF_TRY(nf_solve_prepare_from(g, src, tol, maxit));
+  int rc = nf_solve_run(g, x, tol, maxit);
+  if (rc < 0) return rc;
+  NF_CUDA(g, cudaEventRecord(g->ev1, g->stream));
+  g->last_timed = true;
+  return rc;
+}
+
+extern "C" int nf_solve(nf_grid *g, const float *rhs, float *p, float tol, int maxit) {
+  NF_CHECK_HANDLE(g);
+  if (!rhs || !p || rhs == p) return NF_ERR_INVALID;
+  if (!g->weights_set) return NF_ERR_STATE;
+  return solve_timed(g, rhs, p, tol, maxit);
+}
+
+extern "C" int nf_project(nf_grid *g, float *u, float *v, float *w, float *p, float tol, int maxit) {
+  NF_CHECK_HANDLE(g);
+  if (!u || !v || !w || !p) return NF_ERR_INVALID;
+  if (!g->weights_set) return NF_ERR_STATE;
+  NF_TRY(nf_rhs_impl(g, u, v, w));
+  int rc = solve_timed(g, nullptr, p, tol, maxit);
+  if (rc < 0) return rc;
+  NF_TRY(nf_grad_subtract_impl(g, u, v, w, p));
+  return rc;
+}
+
+extern "C" int nf_project_adjoint(nf_grid *g, float *gu, float *gv, float *gw, const float *p_saved,
+                                  const float *uhat_u, const float *uhat_v, const float *uhat_w, float *galpha_u,
+                                  float *galpha_v, float *galpha_w, float *gus_u, float *gus_v, float *gus_w,
+                                  float *y_out, float tol, int maxit) {
+  NF_CHECK_HANDLE(g);
+  if (!gu || !gv || !gw) return NF_ERR_INVALID;
+  const bool want_ga = galpha_u || galpha_v || galpha_w;
+  if (want_ga && !(galpha_u && galpha_v && galpha_w && p_saved && uhat_u && uhat_v && uhat_w)) return NF_ERR_INVALID;
+  const bool want_gs = gus_u || gus_v || gus_w;
+  if (want_gs && !(gus_u && gus_v && gus_w)) return NF_ERR_INVALID;
+  if (!g->weights_set) return NF_ERR_STATE;
+  float *y = y_out ? y_out : g->xtmp;
+  NF_TRY(nf_adjoint_rhs_impl(g, gu, gv, gw));
+  int rc = solve_timed(g, nullptr, y, tol, maxit);
+  if (rc < 0) return rc;
+  NF_TRY(nf_adjoint_finish_impl(g, gu, gv, gw, y, p_saved, uhat_u, uhat_v, uhat_w, galpha_u, galpha_v, galpha_w,
+                                gus_u, gus_v, gus_w));
+  return rc;
+}
+
+extern "C" int nf_advect(nf_grid *g, float *u, float *v, float *w, float dt) {
+  NF_CHECK_HANDLE(g);
+  if (!u || !v || !w) return NF_ERR_INVALID;
+  return nf_advect_impl(g, u, v, w, dt);
+}
+
+extern "C" int nf_advect_adjoint(nf_grid *g, const float *u0, const float *v0, const float *w0, float *gu, float *gv,
+                                 float *gw, float dt) {
+  NF_CHECK_HANDLE(g);
+  if (!u0 || !v0 || !w0 || !gu || !gv || !gw) return NF_ERR_INVALID;
+  return nf_advect_adjoint_impl(g, u0, v0, w0, gu, gv, gw, dt);
+}
+
+extern "C" int nf_weights_adjoint(nf_grid *g, const float *galpha_u, const float *galpha_v, const float *galpha_w,
+                                  float *gsdf_nodes) {
+  NF_CHECK_HANDLE(g);
+  if (!galpha_u || !galpha_v || !galpha_w || !gsdf_nodes) return NF_ERR_INVALID;
+  if (!g->have_sdf) return NF_ERR_STATE;
+  return nf_weights_adjoint_impl(g, galpha_u, galpha_v, galpha_w, gsdf_nodes);
+}
+
+extern "C" int nf_apply_A(nf_grid *g, const float *p, float *q) {
+  NF_CHECK_HANDLE(g);
+  if (!p || !q || p == q) return NF_ERR_INVALID;
+  if (!g->weights_set) return NF_ERR_STATE;
+  return nf_apply_A_impl(g, p, q);
+}
+
+extern "C" int nf_vcycle(nf_grid *g, const float *r, float *z) {
+  NF_CHECK_HANDLE(g);
+  if (!r || !z) return NF_ERR_INVALID;
+  if (!g->weights_set) return NF_ERR_STATE;
+  const size_t bytes = nf_nc(g) * sizeof(float);
+  NF_CUDA(g, cudaMemcpyAsync(g->lv[0].r, r, bytes, cudaMemcpyDeviceToDevice, g->stream));
+  NF_TRY(nf_vcycle_impl(g, false, 0));
+  NF_CUDA(g, cudaMemcpyAsync(z, g->lv[0].z, bytes, cudaMemcpyDeviceToDevice, g->stream));
+  return NF_OK;
+}
+
+// ---- host-buffer variants ------------------------------------------------------------------------------------
+static int ensure_host_staging(nf_grid *g) {
+  if (g->hs_u) return NF_OK;
+  // device staging for the host entry points (the caller's arrays live in host memory)
+  if (dalloc(&g->hs_u, nf_nu(g)) != cudaSuccess || dalloc(&g->hs_v, nf_nv(g)) != cudaSuccess ||
+      dalloc(&g->hs_w, nf_nw(g)) != cudaSuccess || dalloc(&g->hs_p, nf_nc(g)) != cudaSuccess ||
+      dalloc(&g->hs_a, nf_nu(g)) != cudaSuccess || dalloc(&g->hs_b, nf_nv(g)) != cudaSuccess ||
+      dalloc(&g->hs_c, nf_nw(g)) != cudaSuccess || dalloc(&g->hs_d, nf_nc(g)) != cudaSuccess) {
+    g->err = "host-variant staging allocation failed";
+    return NF_ERR_ALLOC;
+  }
+  return NF_OK;
+}
+
+extern "C" int nf_project_host(nf_grid *g, float *u, float *v, float *w, float *p, float tol, int maxit) {
+  NF_CHECK_HANDLE(g);
+  if (!u || !v || !w || !p) return NF_ERR_INVALID;
+  if (!g->weights_set) return NF_ERR_STATE;
+  NF_TRY(ensure_host_staging(g));
+  const size_t bu = nf_nu(g) * sizeof(float), bv = nf_nv(g) * sizeof(float), bw = nf_nw(g) * sizeof(float);
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_u, u, bu, cudaMemcpyHostToDevice, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_v, v, bv, cudaMemcpyHostToDevice, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_w, w, bw, cudaMemcpyHostToDevice, g->stream));
+  int rc = nf_project(g, g->hs_u, g->hs_v, g->hs_w, g->hs_p, tol, maxit);
+  if (rc < 0) return rc;
+  NF_CUDA(g, cudaMemcpyAsync(u, g->hs_u, bu, cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(v, g->hs_v, bv, cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(w, g->hs_w, bw, cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(p, g->hs_p, nf_nc(g) * sizeof(float), cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaStreamSynchronize(g->stream));
+  return rc;
+}
+
+extern "C" int nf_project_adjoint_host(nf_grid *g, float *gu, float *gv, float *gw, const float *p_saved,
+                                       const float *uhat_u, const float *uhat_v, const float *uhat_w, float tol,
+                                       int maxit) {
+  NF_CHECK_HANDLE(g);
+  (void)p_saved; (void)uhat_u; (void)uhat_v; (void)uhat_w;  // only needed for dJ/dalpha, not produced here
+  if (!gu || !gv || !gw) return NF_ERR_INVALID;
+  if (!g->weights_set) return NF_ERR_STATE;
+  NF_TRY(ensure_host_staging(g));
+  const size_t bu = nf_nu(g) * sizeof(float), bv = nf_nv(g) * sizeof(float), bw = nf_nw(g) * sizeof(float);
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_a, gu, bu, cudaMemcpyHostToDevice, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_b, gv, bv, cudaMemcpyHostToDevice, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_c, gw, bw, cudaMemcpyHostToDevice, g->stream));
+  int rc = nf_project_adjoint(g, g->hs_a, g->hs_b, g->hs_c, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+                              nullptr, nullptr, nullptr, nullptr, nullptr, tol, maxit);
+  if (rc < 0) return rc;
+  NF_CUDA(g, cudaMemcpyAsync(gu, g->hs_a, bu, cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(gv, g->hs_b, bv, cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(gw, g->hs_c, bw, cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaStreamSynchronize(g->stream));
+  return rc;
+}
+
+extern "C" int nf_last_solve_info(nf_grid *g, int *iters, float *relres, float *ms) {
+  NF_CHECK_HANDLE(g);
+  float t = 0.0f;
+  if (g->last_timed) {
+    NF_CUDA(g, cudaEventSynchronize(g->ev1));
+    NF_CUDA(g, cudaEventElapsedTime(&t, g->ev0, g->ev1));
+  }
+  if (iters) *iters = g->last_iters;
+  if (relres) *relres = g->last_relres;
+  if (ms) *ms = t;
+  return NF_OK;
+}
+
+extern "C" int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, int *singular) {
+  NF_CHECK_HANDLE(g);
+  if (levels) *levels = g->nlev;
+  if (active_cells) *active_cells = g->weights_set ? g->nact : -1;
+  if (singular) *singular = g->weights_set ? g->singular : -1;
+  return NF_OK;
+}
+
+extern "C" long long nf_launch_count(nf_grid *g) { return g ? g->launches : 0; }
+
+extern "C" const char *nf_last_error(nf_grid *g) { return g ? g->err.c_str() : "null handle"; }

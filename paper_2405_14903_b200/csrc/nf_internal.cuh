@@ -1,0 +1,167 @@
+// nf_internal.cuh -- internal declarations of the CUDA path (sm_100a).  Not part of the C ABI (include/nf.h).
+// Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "nf.h"
+
+#define NF_MAX_LEVELS 12
+#define NF_RING 64          // mapped host status ring (power of two)
+#define NF_ALPHA_EPS 1e-4f  // R4: alpha < 1e-4 -> 0
+
+// One multigrid level ("hierarchical grid data structure").  Level 0 is the simulation grid.
+// Face weights are stored per level in MAC face layout, except that x-face rows are padded to a multiple of
+// 4 floats (pax) so that every row of every array starts 16-byte aligned:
+//   ax[(k*ny + j)*pax + i], i in [0, nx]   weight of the x-face between cells i-1 and i
+//   ay[(k*(ny+1) + j)*nx + i], j in [0, ny]
+//   az[(k*ny + j)*nx + i], k in [0, nz]
+struct NfLevel {
+  int nx, ny, nz, pax;
+  long long ncell;
+  float c;  // c_l = (dt_over_rho/dx) / 4^l  (rediscretised operator on spacing 2^l dx)
+  float *ax, *ay, *az;
+  float *z, *r;  // level 0: CG vectors z and r; level > 0: coarse correction and restricted residual
+};
+
+// Device-resident PCG scalars.  Slots [2] alternate with the iteration parity so that no kernel has to
+// reset a value another kernel of the same iteration still reads.
+struct NfSolveState {
+  double pq[2], rr[2], rz[2];
+  double bb;    // ||b||^2 after masking / mean removal
+  double sum;   // scratch: sum over active cells
+  double tol2;  // tol^2
+  double relres;  // sqrt(rr/bb) at the last executed iteration
+  int iter, maxit, done, converged;
+};
+
+struct NfHostStatus {  // written by the device into mapped pinned memory
+  volatile int seq;    // iteration number + 1 once written (0 = not yet)
+  volatile int iter;   // iterations actually executed so far
+  volatile int done;
+  volatile int converged;
+  volatile float relres;
+};
+
+struct nf_grid {
+  int nx, ny, nz;
+  float dx, dt_over_rho;
+  int bc_type[6];
+  float bc_val[6];
+  cudaStream_t stream;
+  int nlev;
+  NfLevel lv[NF_MAX_LEVELS];
+  bool weights_set, have_sdf, have_us;
+  int singular;
+  long long nact;
+  int nu_pre, nu_post, refine;
+  // solid velocity (MAC layout, closed walls at rest) and the last SDF
+  float *us, *vs, *ws, *sdf;
+  // CG vectors on level 0 (r and z live in lv[0])
+  float *p, *q, *xtmp;
+  double *xd;  // fp64 solution accumulator (refine mode)
+  // scratch face arrays (advection copy / adjoint staging)
+  float *fu, *fv, *fw;
+  NfSolveState *st;      // device
+  NfHostStatus *hst;     // mapped pinned host ring
+  NfHostStatus *hst_dev; // device alias of hst
+  double *d_counts;      // device: [0] active cells, [1] open faces on Dirichlet domain faces
+  double *h_counts;      // pinned host copy
+  cudaEvent_t ev0, ev1;
+  int last_iters;
+  float last_relres;
+  bool last_timed;
+  long long launches;
+  std::string err;
+  // host staging for the *_host entry points
+  float *hs_u, *hs_v, *hs_w, *hs_p, *hs_a, *hs_b, *hs_c, *hs_d;
+};
+
+#define NF_CUDA(g, call)                                                            \
+  do {                                                                              \
+    cudaError_t e_ = (call);                                                        \
+    if (e_ != cudaSuccess) {                                                        \
+      (g)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                \
+      return NF_ERR_CUDA;                                                           \
+    }                                                                               \
+  } while (0)
+
+static inline size_t nf_nu(const nf_grid *g) { return (size_t)g->nz * g->ny * (g->nx + 1); }
+static inline size_t nf_nv(const nf_grid *g) { return (size_t)g->nz * (g->ny + 1) * g->nx; }
+static inline size_t nf_nw(const nf_grid *g) { return (size_t)(g->nz + 1) * g->ny * g->nx; }
+static inline size_t nf_nc(const nf_grid *g) { return (size_t)g->nz * g->ny * g->nx; }
+static inline size_t nf_nn(const nf_grid *g) { return (size_t)(g->nz + 1) * (g->ny + 1) * (g->nx + 1); }
+
+// Launch geometry for a logical (tx, ty, tz) thread lattice: 256 threads per block, x fastest.
+struct NfDims {
+  dim3 grid, block;
+};
+static inline NfDims nf_dims(int tx, int ty, int tz) {
+  int bx = 4;
+  while (bx < tx && bx < 128) bx <<= 1;
+  int by = 1;
+  while (by < ty && bx * by < 256) by <<= 1;
+  int bz = 1;
+  while (bz < tz && bx * by * bz < 256) bz <<= 1;
+  NfDims d;
+  d.block = dim3(bx, by, bz);
+  d.grid = dim3((tx + bx - 1) / bx, (ty + by - 1) / by, (tz + bz - 1) / bz);
+  return d;
+}
+
+// ---- kernels / host launchers implemented across the .cu files -------------------------------------------
+// nf_weights.cu
+int nf_weights_from_sdf(nf_grid *g, const float *sdf);
+int nf_weights_from_user(nf_grid *g, const float *au, const float *av, const float *aw);
+int nf_weights_to_user(nf_grid *g, float *au, float *av, float *aw);
+int nf_build_hierarchy(nf_grid *g);  // coarse weights + active count + singular flag
+int nf_store_solid_velocity(nf_grid *g, const float *us, const float *vs, const float *ws);
+int nf_weights_adjoint_impl(nf_grid *g, const float *gau, const float *gav, const float *gaw, float *gsdf);
+// nf_solver.cu
+int nf_apply_A_impl(nf_grid *g, const float *p, float *q);
+int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot);  // z = M^{-1} r on lv[0].r -> lv[0].z
+// Solve A x = lv[0].r (already masked; mean removed if singular; st->bb set by nf_solve_prepare).
+int nf_solver_init(nf_grid *g);                          // kernel attributes (once per process)
+int nf_solve_prepare(nf_grid *g, float tol, int maxit);  // from lv[0].r: mask, mean removal, bb
+int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit);
+int nf_solve_run(nf_grid *g, float *x, float tol, int maxit);
+// nf_project.cu
+int nf_rhs_impl(nf_grid *g, const float *u, const float *v, const float *w);  // -> lv[0].r
+int nf_grad_subtract_impl(nf_grid *g, float *u, float *v, float *w, const float *p);
+int nf_adjoint_rhs_impl(nf_grid *g, const float *gu, const float *gv, const float *gw);  // -> lv[0].r
+int nf_adjoint_finish_impl(nf_grid *g, float *gu, float *gv, float *gw, const float *y, const float *p_saved,
+                           const float *uu, const float *uv, const float *uw, float *gau, float *gav, float *gaw,
+                           float *gsu, float *gsv, float *gsw);
+// nf_advect.cu
+int nf_advect_impl(nf_grid *g, float *u, float *v, float *w, float dt);
+int nf_advect_adjoint_impl(nf_grid *g, const float *u0, const float *v0, const float *w0, float *gu, float *gv,
+                           float *gw, float dt);
+
+// ---- device helpers ---------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ double nf_warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+// Block reduction (warp shuffles, then one warp over the per-warp partials) followed by ONE fp64 atomicAdd
+// per block.  Every thread of the block must call it.  blockDim total <= 1024.
+__device__ __forceinline__ void nf_block_atomic_add(double v, double *dst) {
+  __shared__ double s_part[32];
+  const int tid = (threadIdx.z * blockDim.y + threadIdx.y) * blockDim.x + threadIdx.x;
+  const int nthr = blockDim.x * blockDim.y * blockDim.z;
+  const int lane = tid & 31, wid = tid >> 5;
+  v = nf_warp_sum(v);
+  if (lane == 0) s_part[wid] = v;
+  __syncthreads();
+  if (wid == 0) {
+    const int nw = (nthr + 31) >> 5;
+    double t = lane < nw ? s_part[lane] : 0.0;
+    t = nf_warp_sum(t);
+    if (lane == 0) atomicAdd(dst, t);
+  }
+  __syncthreads();
+}
+#endif

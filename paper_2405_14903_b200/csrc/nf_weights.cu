@@ -1,0 +1,389 @@
+// nf_weights.cu -- a-1 face-weight builder, coarse-level weights of the hierarchy
+// (PAPER.md:L230), active-cell / singularity classification (R12) and a-10 the weights adjoint.
+#include "nf_internal.cuh"
+
+// ------------------------------------------------------------------------------------------------------------
+// Marching-squares fluid area fraction of a unit face with corner SDF values P[0..3] in cyclic order.
+// phi > 0 is fluid, phi == 0 counts as solid (R1).  If GRAD, d[q] = d alpha / d P[q].
+// tri(a; b, d) = 1/2 * a/(a-b) * a/(a-d): the paper's printed one-fluid-corner formula.
+// ------------------------------------------------------------------------------------------------------------
+template <bool GRAD>
+__device__ __forceinline__ float nf_tri(float a, float b, float d, float &da, float &db, float &dd) {
+  const float iab = 1.0f / (a - b), iad = 1.0f / (a - d);
+  const float fb = a * iab, fd = a * iad;
+  if (GRAD) {
+    const float fb_a = -b * iab * iab, fb_b = a * iab * iab;
+    const float fd_a = -d * iad * iad, fd_d = a * iad * iad;
+    da = 0.5f * (fb_a * fd + fb * fd_a);
+    db = 0.5f * fb_b * fd;
+    dd = 0.5f * fb * fd_d;
+  }
+  return 0.5f * fb * fd;
+}
+
+template <bool GRAD>
+__device__ __forceinline__ float nf_area_fraction(const float P0, const float P1, const float P2, const float P3,
+                                                  float *d /*[4] if GRAD*/) {
+  const float P[4] = {P0, P1, P2, P3};
+  const bool F[4] = {P0 > 0.0f, P1 > 0.0f, P2 > 0.0f, P3 > 0.0f};
+  const int s = (int)F[0] + (int)F[1] + (int)F[2] + (int)F[3];
+  float out = 0.0f;
+  float g[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+  if (s == 4) {
+    out = 1.0f;
+  } else if (s == 1 || s == 3) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int qb = (q + 1) & 3, qd = (q + 3) & 3;
+      const bool hit = (s == 1) ? F[q] : !F[q];
+      if (hit) {
+        float da, db, dd;
+        const float t = nf_tri<GRAD>(P[q], P[qb], P[qd], da, db, dd);
+        if (s == 1) {
+          out = t;
+          if (GRAD) { g[q] = da; g[qb] = db; g[qd] = dd; }
+        } else {
+          out = 1.0f - t;
+          if (GRAD) { g[q] = -da; g[qb] = -db; g[qd] = -dd; }
+        }
+      }
+    }
+  } else if (s == 2) {
+    bool adjacent = false;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int q1 = (q + 1) & 3, q2 = (q + 2) & 3, q3 = (q + 3) & 3;
+      if (F[q] && F[q1]) {  // fluid corners q, q+1; solid neighbours q-1 (of q) and q+2 (of q+1)
+        adjacent = true;
+        const float A = P[q], B = P[q1], C = P[q2], D = P[q3];
+        const float iad = 1.0f / (A - D), ibc = 1.0f / (B - C);
+        out = 0.5f * (A * iad + B * ibc);
+        if (GRAD) {
+          g[q] = 0.5f * (-D * iad * iad);
+          g[q3] = 0.5f * (A * iad * iad);
+          g[q1] = 0.5f * (-C * ibc * ibc);
+          g[q2] = 0.5f * (B * ibc * ibc);
+        }
+      }
+    }
+    if (!adjacent) {  // diagonal: tie-break on the mean of the four values (R3)
+      const float mean = 0.25f * (P[0] + P[1] + P[2] + P[3]);
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        const int q1 = q + 1, q2 = (q + 2) & 3, q3 = (q + 3) & 3;
+        if (F[q] && F[q2]) {
+          const float A = P[q], B = P[q1], C = P[q2], D = P[q3];
+          float a1, b1, c1, a2, b2, c2;
+          if (mean > 0.0f) {  // fluid joined: 1 - two solid triangles at B and D
+            const float t1 = nf_tri<GRAD>(B, C, A, a1, b1, c1);  // corner B, neighbours C and A
+            const float t2 = nf_tri<GRAD>(D, A, C, a2, b2, c2);  // corner D, neighbours A and C
+            out = 1.0f - t1 - t2;
+            if (GRAD) {
+              g[q1] = -a1; g[q2] = -b1 - c2; g[q] = -c1 - b2; g[q3] = -a2;
+            }
+          } else {  // fluid separated: two fluid triangles at A and C
+            const float t1 = nf_tri<GRAD>(A, B, D, a1, b1, c1);
+            const float t2 = nf_tri<GRAD>(C, D, B, a2, b2, c2);
+            out = t1 + t2;
+            if (GRAD) {
+              g[q] = a1; g[q1] = b1 + c2; g[q3] = c1 + b2; g[q2] = a2;
+            }
+          }
+        }
+      }
+    }
+  }
+  if (out < NF_ALPHA_EPS) {  // R4
+    out = 0.0f;
+    if (GRAD) { g[0] = g[1] = g[2] = g[3] = 0.0f; }
+  }
+  if (GRAD) { d[0] = g[0]; d[1] = g[1]; d[2] = g[2]; d[3] = g[3]; }
+  return out;
+}
+
+struct NfBc6 {
+  int t[6];
+};
+
+// One thread per "extended cell" (i <= nx, j <= ny, k <= nz): it owns the low x-, y- and z-face of that cell.
+__global__ void __launch_bounds__(256) k_weights_from_sdf(const float *__restrict__ phi, float *__restrict__ ax,
+                                                          float *__restrict__ ay, float *__restrict__ az, int nx,
+                                                          int ny, int nz, int pax, NfBc6 bc) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i > nx || j > ny || k > nz) return;
+  const size_t sx = 1, sy = (size_t)nx + 1, sz = (size_t)(nx + 1) * (ny + 1);
+  const size_t n0 = (size_t)k * sz + (size_t)j * sy + i;
+  const bool hi = i < nx, hj = j < ny, hk = k < nz;
+  const float p000 = __ldg(phi + n0);
+  const float p001 = hi ? __ldg(phi + n0 + sx) : 0.0f;
+  const float p010 = hj ? __ldg(phi + n0 + sy) : 0.0f;
+  const float p100 = hk ? __ldg(phi + n0 + sz) : 0.0f;
+  if (hj && hk) {  // x-face: corners (k,j),(k,j+1),(k+1,j+1),(k+1,j) at node column i
+    const float p110 = __ldg(phi + n0 + sy + sz);
+    float a = nf_area_fraction<false>(p000, p010, p110, p100, nullptr);
+    if ((i == 0 && bc.t[0] == NF_BC_CLOSED) || (i == nx && bc.t[1] == NF_BC_CLOSED)) a = 0.0f;
+    ax[((size_t)k * ny + j) * pax + i] = a;
+  }
+  if (hi && hk) {  // y-face: corners (k,i),(k,i+1),(k+1,i+1),(k+1,i)
+    const float p101 = __ldg(phi + n0 + sx + sz);
+    float a = nf_area_fraction<false>(p000, p001, p101, p100, nullptr);
+    if ((j == 0 && bc.t[2] == NF_BC_CLOSED) || (j == ny && bc.t[3] == NF_BC_CLOSED)) a = 0.0f;
+    ay[((size_t)k * (ny + 1) + j) * nx + i] = a;
+  }
+  if (hi && hj) {  // z-face: corners (j,i),(j,i+1),(j+1,i+1),(j+1,i)
+    const float p011 = __ldg(phi + n0 + sx + sy);
+    float a = nf_area_fraction<false>(p000, p001, p011, p010, nullptr);
+    if ((k == 0 && bc.t[4] == NF_BC_CLOSED) || (k == nz && bc.t[5] == NF_BC_CLOSED)) a = 0.0f;
+    az[((size_t)k * ny + j) * nx + i] = a;
+  }
+}
+
+// a-10: scatter dJ/dalpha * d alpha/d phi to the four corner nodes of every face.
+__global__ void __launch_bounds__(256) k_weights_adjoint(const float *__restrict__ phi, const float *__restrict__ gau,
+                                                         const float *__restrict__ gav, const float *__restrict__ gaw,
+                                                         float *__restrict__ gphi, int nx, int ny, int nz, NfBc6 bc) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i > nx || j > ny || k > nz) return;
+  const size_t sx = 1, sy = (size_t)nx + 1, sz = (size_t)(nx + 1) * (ny + 1);
+  const size_t n0 = (size_t)k * sz + (size_t)j * sy + i;
+  const bool hi = i < nx, hj = j < ny, hk = k < nz;
+  const float p000 = __ldg(phi + n0);
+  const float p001 = hi ? __ldg(phi + n0 + sx) : 0.0f;
+  const float p010 = hj ? __ldg(phi + n0 + sy) : 0.0f;
+  const float p100 = hk ? __ldg(phi + n0 + sz) : 0.0f;
+  float d[4];
+  if (hj && hk && !((i == 0 && bc.t[0] == NF_BC_CLOSED) || (i == nx && bc.t[1] == NF_BC_CLOSED))) {
+    const float p110 = __ldg(phi + n0 + sy + sz);
+    const bool any = (p000 > 0) | (p010 > 0) | (p110 > 0) | (p100 > 0);
+    const bool all = (p000 > 0) & (p010 > 0) & (p110 > 0) & (p100 > 0);
+    if (any && !all) {
+      nf_area_fraction<true>(p000, p010, p110, p100, d);
+      const float ga = __ldg(gau + ((size_t)k * ny + j) * (nx + 1) + i);
+      if (d[0] != 0.0f) atomicAdd(gphi + n0, ga * d[0]);
+      if (d[1] != 0.0f) atomicAdd(gphi + n0 + sy, ga * d[1]);
+      if (d[2] != 0.0f) atomicAdd(gphi + n0 + sy + sz, ga * d[2]);
+      if (d[3] != 0.0f) atomicAdd(gphi + n0 + sz, ga * d[3]);
+    }
+  }
+  if (hi && hk && !((j == 0 && bc.t[2] == NF_BC_CLOSED) || (j == ny && bc.t[3] == NF_BC_CLOSED))) {
+    const float p101 = __ldg(phi + n0 + sx + sz);
+    const bool any = (p000 > 0) | (p001 > 0) | (p101 > 0) | (p100 > 0);
+    const bool all = (p000 > 0) & (p001 > 0) & (p101 > 0) & (p100 > 0);
+    if (any && !all) {
+      nf_area_fraction<true>(p000, p001, p101, p100, d);
+      const float ga = __ldg(gav + ((size_t)k * (ny + 1) + j) * nx + i);
+      if (d[0] != 0.0f) atomicAdd(gphi + n0, ga * d[0]);
+      if (d[1] != 0.0f) atomicAdd(gphi + n0 + sx, ga * d[1]);
+      if (d[2] != 0.0f) atomicAdd(gphi + n0 + sx + sz, ga * d[2]);
+      if (d[3] != 0.0f) atomicAdd(gphi + n0 + sz, ga * d[3]);
+    }
+  }
+  if (hi && hj && !((k == 0 && bc.t[4] == NF_BC_CLOSED) || (k == nz && bc.t[5] == NF_BC_CLOSED))) {
+    const float p011 = __ldg(phi + n0 + sx + sy);
+    const bool any = (p000 > 0) | (p001 > 0) | (p011 > 0) | (p010 > 0);
+    const bool all = (p000 > 0) & (p001 > 0) & (p011 > 0) & (p010 > 0);
+    if (any && !all) {
+      nf_area_fraction<true>(p000, p001, p011, p010, d);
+      const float ga = __ldg(gaw + ((size_t)k * ny + j) * nx + i);
+      if (d[0] != 0.0f) atomicAdd(gphi + n0, ga * d[0]);
+      if (d[1] != 0.0f) atomicAdd(gphi + n0 + sx, ga * d[1]);
+      if (d[2] != 0.0f) atomicAdd(gphi + n0 + sx + sy, ga * d[2]);
+      if (d[3] != 0.0f) atomicAdd(gphi + n0 + sy, ga * d[3]);
+    }
+  }
+}
+
+// Copy user MAC-layout weights into the internal layout (x rows padded to pax), forcing closed walls to 0.
+__global__ void __launch_bounds__(256) k_weights_import(const float *__restrict__ au, const float *__restrict__ av,
+                                                        const float *__restrict__ aw, float *__restrict__ ax,
+                                                        float *__restrict__ ay, float *__restrict__ az, int nx, int ny,
+                                                        int nz, int pax, NfBc6 bc) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i > nx || j > ny || k > nz) return;
+  if (j < ny && k < nz) {
+    float a = au[((size_t)k * ny + j) * (nx + 1) + i];
+    if ((i == 0 && bc.t[0] == NF_BC_CLOSED) || (i == nx && bc.t[1] == NF_BC_CLOSED)) a = 0.0f;
+    ax[((size_t)k * ny + j) * pax + i] = a;
+  }
+  if (i < nx && k < nz) {
+    float a = av[((size_t)k * (ny + 1) + j) * nx + i];
+    if ((j == 0 && bc.t[2] == NF_BC_CLOSED) || (j == ny && bc.t[3] == NF_BC_CLOSED)) a = 0.0f;
+    ay[((size_t)k * (ny + 1) + j) * nx + i] = a;
+  }
+  if (i < nx && j < ny) {
+    float a = aw[((size_t)k * ny + j) * nx + i];
+    if ((k == 0 && bc.t[4] == NF_BC_CLOSED) || (k == nz && bc.t[5] == NF_BC_CLOSED)) a = 0.0f;
+    az[((size_t)k * ny + j) * nx + i] = a;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_weights_export(const float *__restrict__ ax, float *__restrict__ au, int nx,
+                                                        int ny, int nz, int pax) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i > nx || j >= ny || k >= nz) return;
+  au[((size_t)k * ny + j) * (nx + 1) + i] = ax[((size_t)k * ny + j) * pax + i];
+}
+
+// Coarse face weight = arithmetic mean of the four coincident fine face weights (R13).
+__global__ void __launch_bounds__(256) k_coarsen_weights(const float *__restrict__ fax, const float *__restrict__ fay,
+                                                         const float *__restrict__ faz, float *__restrict__ cax,
+                                                         float *__restrict__ cay, float *__restrict__ caz, int fnx,
+                                                         int fny, int fnz, int fpax, int cnx, int cny, int cnz,
+                                                         int cpax) {
+  const int I = blockIdx.x * blockDim.x + threadIdx.x;
+  const int J = blockIdx.y * blockDim.y + threadIdx.y;
+  const int K = blockIdx.z * blockDim.z + threadIdx.z;
+  if (I > cnx || J > cny || K > cnz) return;
+  const int i = 2 * I, j = 2 * J, k = 2 * K;
+  if (J < cny && K < cnz) {
+    const float *b = fax + ((size_t)k * fny + j) * fpax + i;
+    const size_t sj = fpax, sk = (size_t)fny * fpax;
+    cax[((size_t)K * cny + J) * cpax + I] = 0.25f * ((b[0] + b[sj]) + (b[sk] + b[sk + sj]));
+  }
+  if (I < cnx && K < cnz) {
+    const float *b = fay + ((size_t)k * (fny + 1) + j) * fnx + i;
+    const size_t sk = (size_t)(fny + 1) * fnx;
+    cay[((size_t)K * (cny + 1) + J) * cnx + I] = 0.25f * ((b[0] + b[1]) + (b[sk] + b[sk + 1]));
+  }
+  if (I < cnx && J < cny) {
+    const float *b = faz + ((size_t)k * fny + j) * fnx + i;
+    const size_t sj = fnx;
+    caz[((size_t)K * cny + J) * cnx + I] = 0.25f * ((b[0] + b[1]) + (b[sj] + b[sj + 1]));
+  }
+}
+
+// counts[0] += active cells (sum of six weights > 0); counts[1] += open faces on Dirichlet domain faces (R12).
+__global__ void __launch_bounds__(256) k_classify(const float *__restrict__ ax, const float *__restrict__ ay,
+                                                  const float *__restrict__ az, int nx, int ny, int nz, int pax,
+                                                  NfBc6 bc, double *__restrict__ counts) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  double act = 0.0, dir = 0.0;
+  if (i < nx && j < ny && k < nz) {
+    const float xl = ax[((size_t)k * ny + j) * pax + i], xh = ax[((size_t)k * ny + j) * pax + i + 1];
+    const float yl = ay[((size_t)k * (ny + 1) + j) * nx + i], yh = ay[((size_t)k * (ny + 1) + j + 1) * nx + i];
+    const float zl = az[((size_t)k * ny + j) * nx + i], zh = az[((size_t)(k + 1) * ny + j) * nx + i];
+    if (xl + xh + yl + yh + zl + zh > 0.0f) act = 1.0;
+    if (i == 0 && bc.t[0] == NF_BC_DIRICHLET && xl > 0.0f) dir += 1.0;
+    if (i == nx - 1 && bc.t[1] == NF_BC_DIRICHLET && xh > 0.0f) dir += 1.0;
+    if (j == 0 && bc.t[2] == NF_BC_DIRICHLET && yl > 0.0f) dir += 1.0;
+    if (j == ny - 1 && bc.t[3] == NF_BC_DIRICHLET && yh > 0.0f) dir += 1.0;
+    if (k == 0 && bc.t[4] == NF_BC_DIRICHLET && zl > 0.0f) dir += 1.0;
+    if (k == nz - 1 && bc.t[5] == NF_BC_DIRICHLET && zh > 0.0f) dir += 1.0;
+  }
+  nf_block_atomic_add(act, counts + 0);
+  nf_block_atomic_add(dir, counts + 1);
+}
+
+// Copy a MAC face array (or zero it when src == nullptr) and put closed walls at rest (R19).
+__global__ void __launch_bounds__(256) k_store_us(const float *__restrict__ src, float *__restrict__ dst, int ex, int ey,
+                                                  int ez, int axis, int closed_lo, int closed_hi) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i >= ex || j >= ey || k >= ez) return;
+  const size_t id = ((size_t)k * ey + j) * ex + i;
+  float v = src ? src[id] : 0.0f;
+  const int c = axis == 0 ? i : (axis == 1 ? j : k);
+  const int e = axis == 0 ? ex : (axis == 1 ? ey : ez);
+  if ((c == 0 && closed_lo) || (c == e - 1 && closed_hi)) v = 0.0f;
+  dst[id] = v;
+}
+
+static NfBc6 bc6(const nf_grid *g) {
+  NfBc6 b;
+  for (int f = 0; f < 6; ++f) b.t[f] = g->bc_type[f];
+  return b;
+}
+
+int nf_weights_from_sdf(nf_grid *g, const float *sdf) {
+  NfLevel &L = g->lv[0];
+  NfDims d = nf_dims(g->nx + 1, g->ny + 1, g->nz + 1);
+  NF_CUDA(g, cudaMemcpyAsync(g->sdf, sdf, nf_nn(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
+  k_weights_from_sdf<<<d.grid, d.block, 0, g->stream>>>(g->sdf, L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g));
+  g->launches += 1;
+  g->have_sdf = true;
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
+int nf_weights_from_user(nf_grid *g, const float *au, const float *av, const float *aw) {
+  NfLevel &L = g->lv[0];
+  NfDims d = nf_dims(g->nx + 1, g->ny + 1, g->nz + 1);
+  k_weights_import<<<d.grid, d.block, 0, g->stream>>>(au, av, aw, L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g));
+  g->launches += 1;
+  g->have_sdf = false;
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
+int nf_weights_to_user(nf_grid *g, float *au, float *av, float *aw) {
+  NfLevel &L = g->lv[0];
+  if (au) {
+    NfDims d = nf_dims(g->nx + 1, g->ny, g->nz);
+    k_weights_export<<<d.grid, d.block, 0, g->stream>>>(L.ax, au, g->nx, g->ny, g->nz, L.pax);
+    g->launches += 1;
+  }
+  if (av) NF_CUDA(g, cudaMemcpyAsync(av, L.ay, nf_nv(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
+  if (aw) NF_CUDA(g, cudaMemcpyAsync(aw, L.az, nf_nw(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
+int nf_build_hierarchy(nf_grid *g) {
+  for (int l = 0; l + 1 < g->nlev; ++l) {
+    NfLevel &F = g->lv[l], &C = g->lv[l + 1];
+    NfDims d = nf_dims(C.nx + 1, C.ny + 1, C.nz + 1);
+    k_coarsen_weights<<<d.grid, d.block, 0, g->stream>>>(F.ax, F.ay, F.az, C.ax, C.ay, C.az, F.nx, F.ny, F.nz, F.pax,
+                                                         C.nx, C.ny, C.nz, C.pax);
+    g->launches += 1;
+  }
+  NfLevel &L = g->lv[0];
+  double *cnt = g->d_counts;
+  NF_CUDA(g, cudaMemsetAsync(cnt, 0, 2 * sizeof(double), g->stream));
+  NfDims d = nf_dims(g->nx, g->ny, g->nz);
+  k_classify<<<d.grid, d.block, 0, g->stream>>>(L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g), cnt);
+  g->launches += 1;
+  NF_CUDA(g, cudaGetLastError());
+  NF_CUDA(g, cudaMemcpyAsync(g->h_counts, cnt, 2 * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaStreamSynchronize(g->stream));
+  const double *hc = g->h_counts;
+  g->nact = (long long)hc[0];
+  g->singular = hc[1] > 0.0 ? 0 : 1;
+  g->weights_set = true;
+  return NF_OK;
+}
+
+int nf_store_solid_velocity(nf_grid *g, const float *us, const float *vs, const float *ws) {
+  g->have_us = (us || vs || ws);
+  if (!g->have_us) return NF_OK;  // kernels treat U_s as identically zero
+  const int cl[6] = {g->bc_type[0] == NF_BC_CLOSED, g->bc_type[1] == NF_BC_CLOSED, g->bc_type[2] == NF_BC_CLOSED,
+                     g->bc_type[3] == NF_BC_CLOSED, g->bc_type[4] == NF_BC_CLOSED, g->bc_type[5] == NF_BC_CLOSED};
+  NfDims d = nf_dims(g->nx + 1, g->ny, g->nz);
+  k_store_us<<<d.grid, d.block, 0, g->stream>>>(us, g->us, g->nx + 1, g->ny, g->nz, 0, cl[0], cl[1]);
+  d = nf_dims(g->nx, g->ny + 1, g->nz);
+  k_store_us<<<d.grid, d.block, 0, g->stream>>>(vs, g->vs, g->nx, g->ny + 1, g->nz, 1, cl[2], cl[3]);
+  d = nf_dims(g->nx, g->ny, g->nz + 1);
+  k_store_us<<<d.grid, d.block, 0, g->stream>>>(ws, g->ws, g->nx, g->ny, g->nz + 1, 2, cl[4], cl[5]);
+  g->launches += 3;
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
+int nf_weights_adjoint_impl(nf_grid *g, const float *gau, const float *gav, const float *gaw, float *gsdf) {
+  NF_CUDA(g, cudaMemsetAsync(gsdf, 0, nf_nn(g) * sizeof(float), g->stream));
+  NfDims d = nf_dims(g->nx + 1, g->ny + 1, g->nz + 1);
+  k_weights_adjoint<<<d.grid, d.block, 0, g->stream>>>(g->sdf, gau, gav, gaw, gsdf, g->nx, g->ny, g->nz, bc6(g));
+  g->launches += 1;
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}

@@ -1,0 +1,374 @@
+"""GPU parity: the CUDA path (through the C ABI / ctypes binding) against the fp64 oracle, element by element,
+on the same seeded inputs.  Tolerances: BASELINE.json north_star -- relative L2 <= 1e-4 on velocity and pressure
+after both sides solve to 1e-6 (the oracle solves to 1e-12); 1e-3 on end-to-end gradients; alpha abs 1e-5
+(SURVEY.md 7.1 step 4); integer / index work bit-exact."""
+import numpy as np
+import pytest
+
+from oracle import nf_oracle as orc
+from paper_2405_14903_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_FIELD = 1e-4  # north_star: relative L2 on velocity and pressure
+TOL_GRAD = 1e-3   # north_star: end-to-end gradients
+TOL_ALPHA = 1e-5  # fp32 evaluation of the area formulas vs fp64
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available()
+    return t
+
+
+@pytest.fixture(scope="module")
+def api():
+    from paper_2405_14903_b200 import api as a
+    a.load_library()  # fails loudly if the CUDA library is missing
+    return a
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy().astype(np.float64)
+
+
+def rel(a, b):
+    a, b = np.asarray(a, np.float64), np.asarray(b, np.float64)
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / (nb if nb > 0 else 1.0)
+
+
+def rel3(A, B):
+    num = np.sqrt(sum(np.sum((np.asarray(a, np.float64) - b) ** 2) for a, b in zip(A, B)))
+    den = np.sqrt(sum(np.sum(np.asarray(b, np.float64) ** 2) for b in B))
+    return num / (den if den > 0 else 1.0)
+
+
+def make_grid(api, nx, ny, nz, dx, dt_over_rho=1.0, bc_types=(0,) * 6, bc_values=(0.0,) * 6):
+    g = api.Grid(nx, ny, nz, dx)
+    g.set_dt_rho(dt_over_rho)
+    for f in range(6):
+        g.set_domain_bc(f, bc_types[f], bc_values[f])
+    return g
+
+
+def blob_sdf(nx, ny, nz, seed, nblobs=6):
+    """Smooth SDF-like field: union of a few spheres (phi > 0 fluid)."""
+    rng = np.random.default_rng(seed)
+    x, y, z = wl.node_coords(nx, ny, nz)
+    phi = np.full((nz + 1, ny + 1, nx + 1), 1e9)
+    for _ in range(nblobs):
+        c = rng.uniform(0, 1, 3) * np.array([nx, ny, nz])
+        r = rng.uniform(1.5, 0.25 * min(nx, ny, nz) + 1.5)
+        phi = np.minimum(phi, wl.sdf_sphere(x, y, z, c, r))
+    return phi.astype(np.float32)
+
+
+def ragged_case(seed, nx=20, ny=18, nz=14, dirichlet=True, with_us=True):
+    rng = np.random.default_rng(seed)
+    bc_types = (1, 0, 0, 1, 0, 0) if dirichlet else (0,) * 6
+    bc_values = (0.7, 0, 0, -0.3, 0, 0) if dirichlet else (0.0,) * 6
+    phi = blob_sdf(nx, ny, nz, seed)
+    U = wl.random_velocity(rng, nx, ny, nz, "uniform")
+    G = wl.random_velocity(rng, nx, ny, nz, "normal")
+    us = wl.random_velocity(rng, nx, ny, nz, "uniform") if with_us else None
+    return dict(nx=nx, ny=ny, nz=nz, dx=1.0 / nx, dt_over_rho=0.8, bc_types=bc_types, bc_values=bc_values, phi=phi,
+                U=U, g=G, us=us)
+
+
+def single_component(alpha, bc):
+    """Keep the largest fluid component (R12: the library removes the null space globally)."""
+    au, av, aw, _ = wl.keep_largest_component(*[np.asarray(a, np.float32) for a in alpha])
+    return [au, av, aw]
+
+
+# ---------------------------------------------------------------------------------------------------------
+# a-1 face weights
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", ["config1", "ragged_dirichlet", "ragged_closed", "config5_64"])
+def test_face_weights_match_oracle(torch, api, case):
+    if case == "config1":
+        c = wl.config1()
+        nx = ny = nz = 32; phi = c["phi"]; bt = c["bc_types"]
+    elif case == "config5_64":
+        nx = ny = nz = 64; phi = wl.config5_phi(64); bt = (0,) * 6
+    else:
+        c = ragged_case(11, dirichlet=(case == "ragged_dirichlet"))
+        nx, ny, nz, phi, bt = c["nx"], c["ny"], c["nz"], c["phi"], c["bc_types"]
+    g = make_grid(api, nx, ny, nz, 1.0 / nx, bc_types=bt)
+    g.set_solid(dev(torch, phi))
+    got = [host(a) for a in g.get_weights()]
+    ref = orc.face_weights(phi, orc.BC(bt))
+    nbad = 0
+    for a, b in zip(got, ref):
+        assert a.shape == b.shape
+        d = np.abs(a - b)
+        nbad += int(np.count_nonzero(d > TOL_ALPHA))
+        # classification (open / closed / full) must agree exactly: it decides active cells and M = [alpha>0]
+        assert np.array_equal(a > 0, b > 0)
+        assert np.array_equal(a == 1, b == 1)
+    assert nbad == 0
+    info = g.info()
+    assert info["active_cells"] == int(orc.active_cells(ref).sum())
+    assert info["singular"] == int(orc.is_singular(ref, orc.BC(bt)))
+    g.close()
+
+
+def test_weights_roundtrip_and_wall_zeroing(torch, api):
+    rng = np.random.default_rng(5)
+    nx, ny, nz = 9, 6, 5
+    bt = (1, 0, 0, 0, 0, 1)
+    a = [rng.uniform(0, 1, s).astype(np.float32) for s in wl.face_shapes(nx, ny, nz)]
+    g = make_grid(api, nx, ny, nz, 0.1, bc_types=bt)
+    g.set_weights(*[dev(torch, x) for x in a])
+    got = [host(x) for x in g.get_weights()]
+    exp = [x.astype(np.float64).copy() for x in a]
+    orc.apply_wall_bc(*exp, orc.BC(bt))
+    for x, y in zip(got, exp):
+        assert np.array_equal(x, y)  # a copy: bit exact
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# a-3 operator
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape", [(32, 32, 32), (20, 18, 14), (5, 3, 2), (1, 1, 7)])
+def test_apply_A_matches_oracle(torch, api, shape):
+    nx, ny, nz = shape
+    rng = np.random.default_rng(3)
+    bt = (1, 1, 0, 0, 1, 0)
+    alpha = [np.where(rng.uniform(size=s) < 0.2, 0.0, rng.uniform(0, 1, s)).astype(np.float32)
+             for s in wl.face_shapes(nx, ny, nz)]
+    a64 = [x.astype(np.float64) for x in alpha]
+    orc.apply_wall_bc(*a64, orc.BC(bt))
+    p = rng.standard_normal((nz, ny, nx)).astype(np.float32)
+    g = make_grid(api, nx, ny, nz, 0.05, dt_over_rho=0.3, bc_types=bt)
+    g.set_weights(*[dev(torch, x) for x in alpha])
+    q = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    g.apply_A(dev(torch, p), q)
+    ref = orc.apply_A(p.astype(np.float64), a64, 0.3 / 0.05)
+    assert rel(host(q), ref) < 2e-6
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# a-3..a-5 solve
+# ---------------------------------------------------------------------------------------------------------
+def _solve_case(torch, api, nx, ny, nz, bt, seed, phi=None):
+    rng = np.random.default_rng(seed)
+    bc = orc.BC(bt)
+    phi = blob_sdf(nx, ny, nz, seed) if phi is None else phi
+    alpha = orc.face_weights(phi, bc)
+    alpha = single_component(alpha, bc)
+    a64 = [x.astype(np.float64) for x in alpha]
+    act = orc.active_cells(a64)
+    b = np.where(act, rng.standard_normal((nz, ny, nx)), 0.0).astype(np.float32)
+    dx, dtr = 1.0 / nx, 0.6
+    g = make_grid(api, nx, ny, nz, dx, dt_over_rho=dtr, bc_types=bt)
+    g.set_weights(*[dev(torch, x) for x in alpha])
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    rc = g.solve(dev(torch, b), p, tol=1e-6, maxit=200)
+    info = g.last_solve_info()
+    ref = orc.solve(b.astype(np.float64), a64, dtr / dx, bc, tol=1e-12)
+    g.close()
+    return rc, info, host(p), ref, a64, b.astype(np.float64), dtr / dx, bc
+
+
+@pytest.mark.parametrize("shape,bt", [((32, 32, 32), (0,) * 6), ((32, 32, 32), (0, 1, 0, 0, 0, 0)),
+                                       ((40, 36, 28), (1, 0, 0, 0, 0, 1)), ((20, 18, 14), (0,) * 6),
+                                       ((6, 5, 4), (0,) * 6), ((64, 64, 64), (0,) * 6)])
+def test_solve_matches_oracle(torch, api, shape, bt):
+    rc, info, p, ref, a64, b, c, bc = _solve_case(torch, api, *shape, bt, seed=21)
+    assert rc == 0, info
+    assert 0 < info["iters"] <= 60, info
+    assert info["relres"] <= 1e-6
+    assert rel(p, ref) < TOL_FIELD
+    # the fp64 true residual of the fp32 answer (fp32 storage floor: DESIGN.md section 7)
+    bb = np.where(orc.active_cells(a64), b, 0.0)
+    if orc.is_singular(a64, bc):
+        bb = np.where(orc.active_cells(a64), bb - bb.sum() / orc.active_cells(a64).sum(), 0.0)
+    assert np.linalg.norm(bb - orc.apply_A(p, a64, c)) / np.linalg.norm(bb) < 5e-6
+
+
+def test_solve_zero_rhs_and_maxit(torch, api):
+    nx = ny = nz = 16
+    phi = blob_sdf(nx, ny, nz, 2)
+    g = make_grid(api, nx, ny, nz, 1.0 / nx)
+    g.set_solid(dev(torch, phi))
+    p = torch.full(g.shape_p, 7.0, dtype=torch.float32, device="cuda")
+    rc = g.solve(torch.zeros(g.shape_p, dtype=torch.float32, device="cuda"), p)
+    assert rc == 0 and g.last_solve_info()["iters"] == 0
+    assert float(p.abs().max()) == 0.0
+    b = torch.randn(g.shape_p, dtype=torch.float32, device="cuda")
+    rc = g.solve(b, p, tol=1e-7, maxit=2)
+    assert rc == api.NF_NOT_CONVERGED and g.last_solve_info()["iters"] == 2
+    g.close()
+
+
+def test_vcycle_is_symmetric_and_positive(torch, api):
+    """M^{-1} must be symmetric positive (semi-)definite for PCG: <M r1, r2> = <r1, M r2>, <M r, r> > 0."""
+    nx, ny, nz = 24, 20, 16
+    phi = blob_sdf(nx, ny, nz, 8)
+    g = make_grid(api, nx, ny, nz, 1.0 / nx, bc_types=(0, 1, 0, 0, 0, 0))
+    g.set_solid(dev(torch, phi))
+    au, av, aw = g.get_weights()
+    act = (au[:, :, :-1] + au[:, :, 1:] + av[:, :-1] + av[:, 1:] + aw[:-1] + aw[1:]) > 0
+    r1 = torch.randn(g.shape_p, device="cuda") * act
+    r2 = torch.randn(g.shape_p, device="cuda") * act
+    z1, z2 = torch.empty_like(r1), torch.empty_like(r2)
+    g.vcycle(r1, z1); g.vcycle(r2, z2)
+    d12 = float((z1.double() * r2.double()).sum()); d21 = float((z2.double() * r1.double()).sum())
+    assert abs(d12 - d21) <= 1e-4 * max(abs(d12), abs(d21), 1e-30)
+    assert float((z1.double() * r1.double()).sum()) > 0
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# a-2, a-6, a-7 projection forward + adjoint
+# ---------------------------------------------------------------------------------------------------------
+def _projection_case(torch, api, c, want_geom_grads=True):
+    nx, ny, nz = c["nx"], c["ny"], c["nz"]
+    bc = orc.BC(c["bc_types"], c["bc_values"])
+    g = make_grid(api, nx, ny, nz, c["dx"], c["dt_over_rho"], c["bc_types"], c["bc_values"])
+    us = c.get("us")
+    g.set_solid(dev(torch, c["phi"]), *([dev(torch, a) for a in us] if us is not None else [None] * 3))
+    # stage by stage: alpha parity is tested separately; keep one fluid component (R12) via the weights hook
+    alpha32 = single_component([a.cpu().numpy() for a in g.get_weights()], bc)
+    g.set_weights(*[dev(torch, a) for a in alpha32])
+    alpha = [a.astype(np.float64) for a in alpha32]
+    U = [dev(torch, a) for a in c["U"]]
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    rc = g.project(*U, p, tol=1e-6, maxit=200)
+    assert rc == 0
+    it_f = g.last_solve_info()["iters"]
+    Uref, pref = orc.project(c["U"], alpha, us, c["dx"], c["dt_over_rho"], bc, tol=1e-12)
+    out = dict(p=(host(p), pref), U=([host(a) for a in U], Uref), it_f=it_f)
+    # adjoint
+    G = [dev(torch, a) for a in c["g"]]
+    uhat = [dev(torch, a) for a in c["U"]]
+    ga = [torch.empty_like(a) for a in G]
+    gs = [torch.empty_like(a) for a in G]
+    y = torch.empty_like(p)
+    rc = g.project_adjoint(*G, p_saved=p, uhat=uhat, galpha=ga if want_geom_grads else None,
+                           gus=gs if want_geom_grads else None, y_out=y, tol=1e-6, maxit=200)
+    assert rc == 0
+    out["it_a"] = g.last_solve_info()["iters"]
+    gU, gA, gS, yref = orc.project_adjoint(c["g"], alpha, pref, c["U"], us, c["dx"], c["dt_over_rho"], bc, tol=1e-12)
+    out["gU"] = ([host(a) for a in G], gU)
+    out["y"] = (host(y), yref)
+    if want_geom_grads:
+        out["gA"] = ([host(a) for a in ga], gA)
+        out["gS"] = ([host(a) for a in gs], gS)
+    out["div"] = orc.weighted_divergence(out["U"][0], alpha, us, bc)
+    out["b"] = orc.rhs([a.astype(np.float64) for a in c["U"]], alpha,
+                       orc.effective_solid_velocity(us, [a.shape for a in c["U"]], bc), c["dt_over_rho"] / c["dx"], bc)
+    g.close()
+    return out
+
+
+@pytest.mark.parametrize("case", ["config1", "ragged_dirichlet_us", "ragged_closed", "tiny"])
+def test_project_and_adjoint_match_oracle(torch, api, case):
+    if case == "config1":
+        c = wl.config1()
+    elif case == "ragged_dirichlet_us":
+        c = ragged_case(31, 40, 36, 28, dirichlet=True, with_us=True)
+    elif case == "ragged_closed":
+        c = ragged_case(32, 20, 18, 14, dirichlet=False, with_us=False)
+    else:
+        c = ragged_case(33, 6, 5, 4, dirichlet=True, with_us=True)
+    o = _projection_case(torch, api, c)
+    assert rel(*o["p"]) < TOL_FIELD
+    assert rel3(*o["U"]) < TOL_FIELD
+    assert rel(*o["y"]) < TOL_FIELD
+    assert rel3(*o["gU"]) < TOL_FIELD
+    assert rel3(*o["gA"]) < TOL_GRAD
+    assert rel3(*o["gS"]) < TOL_GRAD
+    # zero weighted divergence after projection (follows from Eqs. 4-5), at the solver tolerance
+    nb = np.linalg.norm(o["b"])
+    assert np.linalg.norm(o["div"]) <= 2e-5 * nb
+    assert o["it_f"] <= 60 and o["it_a"] <= 60
+
+
+def test_adjoint_dot_product_on_gpu(torch, api):
+    """<P x, y> = <x, P^T y> with U_s = 0 (north_star), both solves at 1e-7 in fp32: agreement ~1e-5."""
+    c = wl.config1()
+    g = make_grid(api, 32, 32, 32, c["dx"])
+    g.set_solid(dev(torch, c["phi"]))
+    x = [dev(torch, a) for a in c["U"]]
+    y = [dev(torch, a) for a in c["g"]]
+    Px = [a.clone() for a in x]
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    g.project(*Px, p, tol=1e-7)
+    PTy = [a.clone() for a in y]
+    g.project_adjoint(*PTy, tol=1e-7)
+    lhs = sum(float((a.double() * b.double()).sum()) for a, b in zip(Px, y))
+    rhs = sum(float((a.double() * b.double()).sum()) for a, b in zip(x, PTy))
+    assert abs(lhs - rhs) <= 2e-5 * max(abs(lhs), abs(rhs))
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# a-8, a-9 advection
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,cfl", [((20, 18, 14), 1.5), ((33, 7, 12), 0.7), ((6, 5, 4), 2.5)])
+def test_advect_and_adjoint_match_oracle(torch, api, shape, cfl):
+    nx, ny, nz = shape
+    rng = np.random.default_rng(41)
+    dx = 1.0 / nx
+    U = wl.random_velocity(rng, nx, ny, nz, "uniform")
+    G = wl.random_velocity(rng, nx, ny, nz, "normal")
+    dt = cfl * dx  # |u| <= 1
+    g = make_grid(api, nx, ny, nz, dx)
+    Ud = [dev(torch, a) for a in U]
+    g.advect(*Ud, dt)
+    ref = orc.advect(U, dt, dx)
+    assert rel3([host(a) for a in Ud], ref) < 1e-5
+    Gd = [dev(torch, a) for a in G]
+    g.advect_adjoint(*[dev(torch, a) for a in U], *Gd, dt)
+    gref = orc.advect_adjoint(U, G, dt, dx)
+    assert rel3([host(a) for a in Gd], gref) < TOL_GRAD
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# a-10 weights adjoint
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dirichlet", [False, True])
+def test_weights_adjoint_matches_oracle(torch, api, dirichlet):
+    c = ragged_case(51, dirichlet=dirichlet)
+    nx, ny, nz = c["nx"], c["ny"], c["nz"]
+    rng = np.random.default_rng(52)
+    ga = [rng.standard_normal(s).astype(np.float32) for s in wl.face_shapes(nx, ny, nz)]
+    g = make_grid(api, nx, ny, nz, c["dx"], bc_types=c["bc_types"])
+    g.set_solid(dev(torch, c["phi"]))
+    out = torch.empty(g.shape_sdf, dtype=torch.float32, device="cuda")
+    g.weights_adjoint(*[dev(torch, a) for a in ga], out)
+    ref = orc.weights_adjoint(c["phi"], *ga, orc.BC(c["bc_types"]))
+    assert rel(host(out), ref) < TOL_GRAD
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# error behaviour of the boundary
+# ---------------------------------------------------------------------------------------------------------
+def test_error_codes(torch, api):
+    g = api.Grid(8, 8, 8, 0.125)
+    u = torch.zeros(g.shape_u, device="cuda"); v = torch.zeros(g.shape_v, device="cuda")
+    w = torch.zeros(g.shape_w, device="cuda"); p = torch.zeros(g.shape_p, device="cuda")
+    with pytest.raises(api.NfError):
+        g.project(u, v, w, p)  # NF_ERR_STATE: weights not set
+    lib = api.load_library()
+    assert lib.nf_project(None, None, None, None, None, 1e-6, 10) == api.NF_ERR_INVALID
+    assert lib.nf_project(g.h, None, None, None, None, 1e-6, 10) == api.NF_ERR_INVALID
+    import ctypes
+    h = ctypes.c_void_p()
+    assert lib.nf_grid_create(0, 8, 8, 0.1, ctypes.byref(h)) == api.NF_ERR_INVALID
+    g.set_solid(torch.ones(g.shape_sdf, device="cuda"))
+    assert lib.nf_solve(g.h, ctypes.c_void_p(p.data_ptr()), ctypes.c_void_p(p.data_ptr()), 1e-6, 10) == api.NF_ERR_INVALID
+    assert g.project(u, v, w, p) == 0
+    g.close()
