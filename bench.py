@@ -1,0 +1,402 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200-native NeuralFluid pressure projection (forward + adjoint).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n 256]
+
+Metric (BASELINE.json): ms per forward + adjoint pressure projection at 256^3, both MGPCG solves to a relative
+residual of 1e-6, plus achieved HBM GB/s vs the measured peak.  Workload: BASELINE.json configs[3], the 256^3
+channel-gate (Dirichlet p = 1 / 0 on -x / +x, closed y/z walls, a 4-cell plate rotating about y, alpha rebuilt every
+step), synthetic and seeded (paper_2405_14903_b200/workloads.py).
+
+A "step" is one pass of the whole hot path (SURVEY.md 8a rows a-1 .. a-10):
+  forward : nf_advect -> nf_set_solid(phi^{n+1}, u_s^{n+1}) -> nf_project
+  backward: nf_project_adjoint (dJ/dUhat, dJ/dalpha, dJ/dU_s) -> nf_weights_adjoint -> nf_advect_adjoint
+`value` is the device time of that step with every input resident in HBM; `projection_ms` is the part of it spent
+in nf_project + nf_project_adjoint (the metric's literal scope).  `e2e` repeats set_solid + project + adjoint through
+the C ABI's host-buffer entry points with pinned host arrays, copies inside the timed region.
+
+Multi-GPU (torchrun): replicas only -- every rank runs its own simulation, no collective on
+the data path; value = max-over-ranks time / (K * N).
+
+--impl reference: the fp64 CPU oracle (oracle/nf_oracle.py, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ms per fwd+adjoint pressure projection at 256^3 (1e-6 resid)"
+TOL, MAXIT = 1e-6, 400
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            pk = json.load(f)
+        return float(pk["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------------------------
+# workload: BASELINE.json configs[3]
+# --------------------------------------------------------------------------------------------------------------
+class GateWorkload:
+    """Device-resident inputs of the channel-gate rollout.  Geometry of `nsteps` consecutive time levels is
+    precomputed on the host (closed-form SDF and rigid velocity, workloads.config4_solid) and kept in HBM."""
+
+    def __init__(self, n, nsteps, seed_shift=0):
+        import numpy as np
+        import torch
+        from paper_2405_14903_b200 import api, workloads as wl
+        self.torch, self.np = torch, np
+        P = wl.config4_params(n, seed=1004 + seed_shift)
+        self.P, self.n = P, n
+        self.g = api.Grid(n, n, n, P["dx"])
+        self.g.set_dt_rho(P["dt_over_rho"])
+        for f in range(6):
+            self.g.set_domain_bc(f, P["bc_types"][f], P["bc_values"][f])
+        d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        self.U0 = [d(a) for a in wl.config4_initial_velocity(P)]
+        self.geom = []
+        for s in range(1, nsteps + 1):
+            phi, us = wl.config4_solid(P, s)
+            self.geom.append((d(phi), [d(a) for a in us]))
+        rng = np.random.default_rng(77 + seed_shift)
+        self.gin = [d(rng.standard_normal(a.shape).astype(np.float32)) for a in self.U0]  # dJ/dU^{n+1}
+        self.U = [a.clone() for a in self.U0]
+        self.Uprev = [torch.empty_like(a) for a in self.U0]
+        self.Uhat = [torch.empty_like(a) for a in self.U0]
+        self.G = [torch.empty_like(a) for a in self.U0]
+        self.ga = [torch.empty_like(a) for a in self.U0]
+        self.gs = [torch.empty_like(a) for a in self.U0]
+        self.p = torch.empty(self.g.shape_p, dtype=torch.float32, device="cuda")
+        self.gphi = torch.empty(self.g.shape_sdf, dtype=torch.float32, device="cuda")
+        self.iters = []
+        self.ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        self.proj_ms = 0.0
+        self.step_no = 0
+
+    def step(self, record=False):
+        """One pass of the whole hot path (rows a-1 .. a-10)."""
+        g, P = self.g, self.P
+        phi, us = self.geom[self.step_no % len(self.geom)]
+        self.step_no += 1
+        for a, b in zip(self.Uprev, self.U):
+            a.copy_(b)                                            # saved U^n (back-prop state)
+        g.advect(*self.U, P["dt"])                                # a-8
+        g.set_solid(phi, *us)                                     # a-1 (+ hierarchy)
+        for a, b in zip(self.Uhat, self.U):
+            a.copy_(b)                                            # saved Uhat
+        if record:
+            self.ev[0].record()
+        rc1 = g.project(*self.U, self.p, tol=TOL, maxit=MAXIT)    # a-2 .. a-6
+        if record:
+            self.ev[1].record()
+        it_f = g.last_solve_info()["iters"] if record else -1
+        for a, b in zip(self.G, self.gin):
+            a.copy_(b)
+        if record:
+            self.ev[2].record()
+        rc2 = g.project_adjoint(*self.G, p_saved=self.p, uhat=self.Uhat, galpha=self.ga, gus=self.gs, tol=TOL,
+                                maxit=MAXIT)                      # a-7
+        if record:
+            self.ev[3].record()
+        it_a = g.last_solve_info()["iters"] if record else -1
+        g.weights_adjoint(*self.ga, self.gphi)                    # a-10
+        g.advect_adjoint(*self.Uprev, *self.G, P["dt"])           # a-9
+        if record:
+            self.torch.cuda.synchronize()
+            self.proj_ms += self.ev[0].elapsed_time(self.ev[1]) + self.ev[2].elapsed_time(self.ev[3])
+            self.iters.append((it_f, it_a))
+        if rc1 != 0 or rc2 != 0:
+            raise RuntimeError("solver did not converge (rc %d / %d)" % (rc1, rc2))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2405_14903_b200 import api
+    api.load_library()  # fail loudly if the CUDA extension is missing: there is no fallback
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    n, K, W = args.n, args.steps, max(args.warmup, 3)
+    wlk = GateWorkload(n, min(K + W, 20), seed_shift=rank)
+    g = wlk.g
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(W):
+        wlk.step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(K):
+        wlk.step()
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = g.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    ms_per_step = ms_total / K
+    value = ms_total / (K * world)
+
+    # ---- extra (untimed-for-the-headline) passes: projection share, iteration counts, per-kernel roofline ----
+    nrec = min(K, 3)
+    for _ in range(nrec):
+        wlk.step(record=True)
+    proj_ms = wlk.proj_ms / nrec
+    g.profile_enable(True)
+    wlk.step()
+    prof = g.profile()
+    g.profile_enable(False)
+    ninfo = g.info()
+    ncell = n ** 3
+    peak, peak_src = _peaks()
+    # algorithmic bytes per fine cell per launch (DESIGN.md section 8 / SURVEY.md 8d.2), fp32
+    BYTES = {"apply_A": 20.0, "cg_update": 24.0, "cg_pupdate": 12.0, "rbgs_fine": 24.0, "restrict_fine": 20.5,
+             "prolong_fine": 8.5, "vdown_fine": 20.5, "vup_fine": 24.5}
+    kern = {}
+    for name, (ms, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        kk = {"ms_total": round(ms, 4), "launches": cnt, "us_per_launch": round(1e3 * ms / cnt, 2)}
+        if name in BYTES:
+            kk["gbs"] = round(BYTES[name] * ncell / (ms / cnt * 1e-3) / 1e9, 1)
+            kk["frac_of_peak"] = round(kk["gbs"] / peak, 3)
+        kern[name] = kk
+    dom = max((k for k in kern if k in BYTES), key=lambda k: kern[k]["ms_total"])
+    roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
+            "frac": round(kern[dom]["gbs"] / peak, 4), "traffic": None, "peak_source": peak_src,
+            "algorithmic_bytes_per_cell": BYTES[dom], "cells_per_launch": ncell,
+            "share_of_step": round(kern[dom]["ms_total"] / sum(v["ms_total"] for v in kern.values()), 3)}
+    its = wlk.iters
+    mcell_it = (ninfo["active_cells"] * sum(a + b for a, b in its) / len(its)) / (proj_ms * 1e-3) / 1e6
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region --------------------------------
+    e2e = None
+    if rank == 0 or world > 1:
+        pin = lambda t_: t_.detach().cpu().pin_memory()
+        hU = [pin(a) for a in wlk.U0]
+        hG = [pin(a) for a in wlk.gin]
+        hUw = [torch.empty_like(a).pin_memory() for a in hU]
+        hGw = [torch.empty_like(a).pin_memory() for a in hG]
+        hp = torch.empty(g.shape_p, dtype=torch.float32).pin_memory()
+        hphi = pin(wlk.geom[0][0]); hus = [pin(a) for a in wlk.geom[0][1]]
+        dphi = torch.empty_like(wlk.geom[0][0]); dus = [torch.empty_like(a) for a in wlk.geom[0][1]]
+
+        def e2e_step():
+            for a, b in zip(hUw, hU):
+                a.copy_(b)  # fresh host inputs (host-side memcpy, part of the user's step)
+            for a, b in zip(hGw, hG):
+                a.copy_(b)
+            dphi.copy_(hphi, non_blocking=True)
+            for a, b in zip(dus, hus):
+                a.copy_(b, non_blocking=True)
+            g.set_solid(dphi, *dus)
+            g.project_host(*hUw, hp, tol=TOL, maxit=MAXIT)
+            g.project_adjoint_host(*hGw, tol=TOL, maxit=MAXIT)
+            return float(hp[0, 0, 0])  # the step's result is read on the host
+
+        ke = max(2, min(K, 5))
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            e2e_step()
+        torch.cuda.synchronize()
+        dt_ms = (time.perf_counter() - t0) * 1e3
+        t = torch.tensor([dt_ms], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        h2d = sum(a.numel() for a in hU + hG + hus) * 4 + hphi.numel() * 4
+        d2h = sum(a.numel() for a in hU + hG) * 4 + hp.numel() * 4
+        e2e = {"value": round(float(t.item()) / (ke * world), 3), "unit": "ms", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": ke,
+               "scope": "H2D(phi,u_s,Uhat,g) + nf_set_solid + nf_project_host + nf_project_adjoint_host + D2H(U,p,dJ/dUhat)"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(args.cpu_n)
+    if rank == 0:
+        line = {"metric": METRIC, "value": round(value, 3), "unit": "ms", "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": round(ms_per_step, 3), "higher_is_better": False, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "configs[3] channel-gate %d^3, 20-step geometry cycle, fwd+adjoint full step "
+                                       "(advect, set_solid, project, project_adjoint, weights_adjoint, advect_adjoint)" % n,
+                           "grid": [n, n, n], "tol": TOL, "l2_policy": "inputs exceed L2 (>1 GB working set per step)",
+                           "parallelism": "replicas x%d" % world, "levels": ninfo["levels"],
+                           "active_cells": ninfo["active_cells"]},
+                "projection_ms": round(proj_ms, 3), "iters_fwd_adj": its, "mcell_iters_per_s": round(mcell_it, 1),
+                "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "roofline": roof, "kernels": kern,
+                "cpu_baseline": cpu,
+                "paper_context": "RTX A6000 whole step (advect+viscosity+project) at 64^3: 0.105 s fwd / 0.117-0.301 s "
+                                 "bwd (PAPER.md Tables 2-3); no projection-only number is published"}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# --------------------------------------------------------------------------------------------------------------
+# the oracle, timed (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------------------------
+def _oracle_case(n):
+    from paper_2405_14903_b200 import workloads as wl
+    import numpy as np
+    P = wl.config4_params(n)
+    U = wl.config4_initial_velocity(P)
+    phi, us = wl.config4_solid(P, 1)
+    rng = np.random.default_rng(77)
+    gin = [rng.standard_normal(a.shape).astype(np.float32) for a in U]
+    return P, U, phi, us, gin
+
+
+def _oracle_step(case):
+    """set_solid + project + project_adjoint with the oracle as it stands, tol = 1e-6 (the metric's tolerance)."""
+    from oracle import nf_oracle as orc
+    P, U, phi, us, gin = case
+    bc = orc.BC(P["bc_types"], P["bc_values"])
+    alpha = orc.face_weights(phi, bc)
+    Un, p = orc.project(U, alpha, us, P["dx"], P["dt_over_rho"], bc, tol=TOL)
+    orc.project_adjoint(gin, alpha, p, U, us, P["dx"], P["dt_over_rho"], bc, tol=TOL)
+
+
+def _threads_used():
+    try:
+        from threadpoolctl import threadpool_info
+        return max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:
+        return 1
+
+
+def cpu_baseline(n):
+    case = _oracle_case(n)
+    t0 = time.perf_counter()
+    _oracle_step(case)
+    ms = (time.perf_counter() - t0) * 1e3
+    return {"value": round(ms, 1), "unit": "ms", "cores": _threads_used(), "host_cores": os.cpu_count(),
+            "kind": "oracle",
+            "sample": "channel-gate shape at %d^3 (%.4f of the 256^3 cells): fp64 NumPy face weights + Jacobi-PCG "
+                      "projection + adjoint, both to 1e-6; one pass" % (n, (n / 256.0) ** 3)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank != 0:
+        return
+    K, W = args.steps, args.warmup
+    n = 64 if (K + W) <= 16 else 48
+    case = _oracle_case(n)
+    for _ in range(W):
+        _oracle_step(case)
+    t0 = time.perf_counter()
+    for _ in range(K):
+        _oracle_step(case)
+    ms = (time.perf_counter() - t0) * 1e3 / K
+    sample = ("channel-gate shape at %d^3 (%.4f of the 256^3 cells) per step: fp64 NumPy oracle, set_solid + "
+              "project + project_adjoint to 1e-6" % (n, (n / 256.0) ** 3))
+    line = {"impl": "reference", "metric": METRIC, "value": round(ms, 1), "unit": "ms", "n_gpus": world, "steps": K,
+            "warmup": W, "ms_per_step": round(ms, 1), "higher_is_better": False, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[3] channel-gate, bounded sample %d^3" % n, "grid": [n, n, n], "tol": TOL},
+            "cpu_baseline": {"value": round(ms, 1), "unit": "ms", "cores": _threads_used(),
+                             "host_cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": round(ms, 1), "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=256, help="grid size (the metric is quoted at 256)")
+    ap.add_argument("--cpu-n", type=int, default=80, help="grid size of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

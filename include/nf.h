@@ -144,6 +144,12 @@ int nf_project_adjoint_host(nf_grid *g, float *gu, float *gv, float *gw, const f
 int nf_last_solve_info(nf_grid *g, int *iters, float *relres, float *ms);
 /* Number of multigrid levels; number of active cells; 1 if the current system is singular (R12). */
 int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, int *singular);
+/* Per-kernel-class device timing (CUDA events around every launch on the handle's stream; adds launch overhead, so
+ * use it on extra steps, not on timed ones).  nf_profile_enable(g,1) clears the counters and starts recording;
+ * nf_profile_get synchronises the stream and returns the accumulated milliseconds and launch count of class idx
+ * (0 <= idx < number of classes; NF_ERR_INVALID beyond).  *name points to static storage. */
+int nf_profile_enable(nf_grid *g, int on);
+int nf_profile_get(nf_grid *g, int idx, const char **name, double *ms, long long *launches);
 /* Kernels launched by this handle since creation (for bench.py's gpu_launches). */
 long long nf_launch_count(nf_grid *g);
 /* Last error message of this handle (static storage inside the handle; "" if none). */

@@ -41,6 +41,9 @@ _SIGNATURES = {
                                           ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
     "nf_grid_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_int),
                                     ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_int)]),
+    "nf_profile_enable": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
+    "nf_profile_get": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_char_p),
+                                      ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)]),
     "nf_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
     "nf_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
 }
@@ -259,6 +262,21 @@ class Grid:
         lv, na, sg = ctypes.c_int(), ctypes.c_longlong(), ctypes.c_int()
         self._check(self.lib.nf_grid_info(self.h, ctypes.byref(lv), ctypes.byref(na), ctypes.byref(sg)), "nf_grid_info")
         return dict(levels=lv.value, active_cells=na.value, singular=sg.value)
+
+    def profile_enable(self, on=True):
+        self._check(self.lib.nf_profile_enable(self.h, 1 if on else 0), "nf_profile_enable")
+
+    def profile(self):
+        """{class name: (ms, launches)} accumulated since profile_enable(True)."""
+        out, idx = {}, 0
+        while True:
+            nm, ms, n = ctypes.c_char_p(), ctypes.c_double(), ctypes.c_longlong()
+            rc = self.lib.nf_profile_get(self.h, idx, ctypes.byref(nm), ctypes.byref(ms), ctypes.byref(n))
+            if rc != NF_OK:
+                break
+            out[nm.value.decode()] = (ms.value, n.value)
+            idx += 1
+        return out
 
     def launch_count(self):
         return int(self.lib.nf_launch_count(self.h))

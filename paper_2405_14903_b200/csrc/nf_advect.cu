@@ -163,9 +163,8 @@ int nf_advect_impl(nf_grid *g, float *u, float *v, float *w, float dt) {
   NF_CUDA(g, cudaMemcpyAsync(g->fv, v, nf_nv(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
   NF_CUDA(g, cudaMemcpyAsync(g->fw, w, nf_nw(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
   NfDims d = nf_dims(g->nx + 1, g->ny + 1, g->nz + 1);
-  k_advect<<<d.grid, d.block, 0, g->stream>>>(make_lat(g, g->fu, g->fv, g->fw), u, v, w, g->nx, g->ny, g->nz,
-                                              dt / g->dx);
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_ADVECT, k_advect<<<d.grid, d.block, 0, g->stream>>>(make_lat(g, g->fu, g->fv, g->fw), u, v, w, g->nx, g->ny, g->nz,
+                                              dt / g->dx));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -181,9 +180,8 @@ int nf_advect_adjoint_impl(nf_grid *g, const float *u0, const float *v0, const f
   NfGrad3 G;
   G.g[0] = gu; G.g[1] = gv; G.g[2] = gw;
   NfDims d = nf_dims(g->nx + 1, g->ny + 1, g->nz + 1);
-  k_advect_adjoint<<<d.grid, d.block, 0, g->stream>>>(make_lat(g, u0, v0, w0), G, g->fu, g->fv, g->fw, g->nx, g->ny,
-                                                      g->nz, dt / g->dx);
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_ADVECT_ADJ, k_advect_adjoint<<<d.grid, d.block, 0, g->stream>>>(make_lat(g, u0, v0, w0), G, g->fu, g->fv, g->fw, g->nx, g->ny,
+                                                      g->nz, dt / g->dx));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }

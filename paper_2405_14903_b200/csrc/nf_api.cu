@@ -35,6 +35,7 @@ static void free_all(nf_grid *g) {
   if (g->h_counts) cudaFreeHost(g->h_counts);
   if (g->ev0) cudaEventDestroy(g->ev0);
   if (g->ev1) cudaEventDestroy(g->ev1);
+  for (cudaEvent_t e : g->prof_pool) cudaEventDestroy(e);
   cudaFree(g->hs_u); cudaFree(g->hs_v); cudaFree(g->hs_w); cudaFree(g->hs_p);
   cudaFree(g->hs_a); cudaFree(g->hs_b); cudaFree(g->hs_c); cudaFree(g->hs_d);
 }
@@ -53,6 +54,8 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->nact = 0;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
+  g->prof_on = false;
+  for (int c = 0; c < NFK_COUNT; ++c) { g->prof_ms[c] = 0.0; g->prof_n[c] = 0; }
   for (int l = 0; l < NF_MAX_LEVELS; ++l) g->lv[l] = NfLevel{};
   // hierarchy: halve while every extent is even and stays >= 4
   int lx = nx, ly = ny, lz = nz, nl = 0;
@@ -329,6 +332,60 @@ extern "C" int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, in
   if (levels) *levels = g->nlev;
   if (active_cells) *active_cells = g->weights_set ? g->nact : -1;
   if (singular) *singular = g->weights_set ? g->singular : -1;
+  return NF_OK;
+}
+
+// ---- per-class kernel timing -------------------------------------------------------------------------------------
+static const char *kClassNames[NFK_COUNT] = {
+    "apply_A", "cg_update", "cg_check", "cg_pupdate", "rbgs_fine", "rbgs_coarse", "restrict_fine", "restrict_coarse",
+    "prolong_fine", "prolong_coarse", "bottom", "solve_setup", "rhs", "grad_subtract", "adjoint_rhs", "adjoint_finish",
+    "weights", "coarsen", "classify", "store_us", "advect", "advect_adjoint", "weights_adjoint", "misc"};
+
+void nf_prof_begin(nf_grid *g, int cls) {
+  const size_t r = g->prof_cls.size();
+  if (g->prof_pool.size() < 2 * (r + 1)) {
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { g->prof_on = false; return; }
+    g->prof_pool.push_back(a);
+    g->prof_pool.push_back(b);
+  }
+  g->prof_cls.push_back(cls);
+  cudaEventRecord(g->prof_pool[2 * r], g->stream);
+}
+void nf_prof_end(nf_grid *g) {
+  const size_t r = g->prof_cls.size() - 1;
+  cudaEventRecord(g->prof_pool[2 * r + 1], g->stream);
+}
+static void prof_collect(nf_grid *g) {
+  if (g->prof_cls.empty()) return;
+  cudaStreamSynchronize(g->stream);
+  for (size_t r = 0; r < g->prof_cls.size(); ++r) {
+    float ms = 0.0f;
+    if (cudaEventElapsedTime(&ms, g->prof_pool[2 * r], g->prof_pool[2 * r + 1]) == cudaSuccess) {
+      g->prof_ms[g->prof_cls[r]] += ms;
+      g->prof_n[g->prof_cls[r]] += 1;
+    }
+  }
+  g->prof_cls.clear();
+}
+
+extern "C" int nf_profile_enable(nf_grid *g, int on) {
+  NF_CHECK_HANDLE(g);
+  prof_collect(g);
+  if (on) {
+    for (int c = 0; c < NFK_COUNT; ++c) { g->prof_ms[c] = 0.0; g->prof_n[c] = 0; }
+  }
+  g->prof_on = on != 0;
+  return NF_OK;
+}
+
+extern "C" int nf_profile_get(nf_grid *g, int idx, const char **name, double *ms, long long *launches) {
+  NF_CHECK_HANDLE(g);
+  if (idx < 0 || idx >= NFK_COUNT) return NF_ERR_INVALID;
+  prof_collect(g);
+  if (name) *name = kClassNames[idx];
+  if (ms) *ms = g->prof_ms[idx];
+  if (launches) *launches = g->prof_n[idx];
   return NF_OK;
 }
 

@@ -45,6 +45,14 @@ struct NfHostStatus {  // written by the device into mapped pinned memory
   volatile float relres;
 };
 
+// Kernel classes for the per-class device timing of nf_profile_* (bench.py's roofline leg).
+enum {
+  NFK_APPLY = 0, NFK_UPDATE, NFK_CHECK, NFK_PUPDATE, NFK_RBGS0, NFK_RBGS_C, NFK_RESTRICT0, NFK_RESTRICT_C,
+  NFK_PROLONG0, NFK_PROLONG_C, NFK_BOTTOM, NFK_SETUP, NFK_RHS, NFK_GRADSUB, NFK_ADJ_RHS, NFK_ADJ_FINISH,
+  NFK_WEIGHTS, NFK_COARSEN, NFK_CLASSIFY, NFK_STORE_US, NFK_ADVECT, NFK_ADVECT_ADJ, NFK_WEIGHTS_ADJ, NFK_MISC,
+  NFK_COUNT
+};
+
 struct nf_grid {
   int nx, ny, nz;
   float dx, dt_over_rho;
@@ -75,9 +83,27 @@ struct nf_grid {
   bool last_timed;
   long long launches;
   std::string err;
+  // per-class kernel timing (off by default)
+  bool prof_on;
+  std::vector<cudaEvent_t> prof_pool;  // event pairs: [2*r], [2*r+1]
+  std::vector<int> prof_cls;           // class of record r
+  double prof_ms[NFK_COUNT];
+  long long prof_n[NFK_COUNT];
   // host staging for the *_host entry points
   float *hs_u, *hs_v, *hs_w, *hs_p, *hs_a, *hs_b, *hs_c, *hs_d;
 };
+
+void nf_prof_begin(nf_grid *g, int cls);
+void nf_prof_end(nf_grid *g);
+// Every kernel launch of the library goes through this macro: it counts the launch and, when profiling is on,
+// brackets it with CUDA events on the handle's stream.
+#define NF_LAUNCH(g, cls, ...)              \
+  do {                                      \
+    if ((g)->prof_on) nf_prof_begin(g, cls); \
+    __VA_ARGS__;                            \
+    if ((g)->prof_on) nf_prof_end(g);       \
+    (g)->launches += 1;                     \
+  } while (0)
 
 #define NF_CUDA(g, call)                                                            \
   do {                                                                              \

@@ -180,9 +180,8 @@ int nf_rhs_impl(nf_grid *g, const float *u, const float *v, const float *w) {
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(L.nx, L.ny, L.nz);
   const bool hu = g->have_us;
-  k_rhs<<<d.grid, d.block, 0, g->stream>>>(u, v, w, hu ? g->us : nullptr, hu ? g->vs : nullptr, hu ? g->ws : nullptr,
-                                           L.ax, L.ay, L.az, L.r, L.c, L.nx, L.ny, L.nz, L.pax, bcv(g));
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_RHS, k_rhs<<<d.grid, d.block, 0, g->stream>>>(u, v, w, hu ? g->us : nullptr, hu ? g->vs : nullptr, hu ? g->ws : nullptr,
+                                           L.ax, L.ay, L.az, L.r, L.c, L.nx, L.ny, L.nz, L.pax, bcv(g)));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -191,10 +190,9 @@ int nf_grad_subtract_impl(nf_grid *g, float *u, float *v, float *w, const float 
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(L.nx + 1, L.ny + 1, L.nz + 1);
   const bool hu = g->have_us;
-  k_grad_subtract<<<d.grid, d.block, 0, g->stream>>>(u, v, w, p, hu ? g->us : nullptr, hu ? g->vs : nullptr,
+  NF_LAUNCH(g, NFK_GRADSUB, k_grad_subtract<<<d.grid, d.block, 0, g->stream>>>(u, v, w, p, hu ? g->us : nullptr, hu ? g->vs : nullptr,
                                                      hu ? g->ws : nullptr, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz,
-                                                     L.pax, bcv(g));
-  g->launches += 1;
+                                                     L.pax, bcv(g)));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -202,8 +200,7 @@ int nf_grad_subtract_impl(nf_grid *g, float *u, float *v, float *w, const float 
 int nf_adjoint_rhs_impl(nf_grid *g, const float *gu, const float *gv, const float *gw) {
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(L.nx, L.ny, L.nz);
-  k_adjoint_rhs<<<d.grid, d.block, 0, g->stream>>>(gu, gv, gw, L.ax, L.ay, L.az, L.r, L.c, L.nx, L.ny, L.nz, L.pax);
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_ADJ_RHS, k_adjoint_rhs<<<d.grid, d.block, 0, g->stream>>>(gu, gv, gw, L.ax, L.ay, L.az, L.r, L.c, L.nx, L.ny, L.nz, L.pax));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -214,11 +211,10 @@ int nf_adjoint_finish_impl(nf_grid *g, float *gu, float *gv, float *gw, const fl
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(L.nx + 1, L.ny + 1, L.nz + 1);
   const bool hu = g->have_us;
-  k_adjoint_finish<<<d.grid, d.block, 0, g->stream>>>(gu, gv, gw, y, p_saved, uu, uv, uw, hu ? g->us : nullptr,
+  NF_LAUNCH(g, NFK_ADJ_FINISH, k_adjoint_finish<<<d.grid, d.block, 0, g->stream>>>(gu, gv, gw, y, p_saved, uu, uv, uw, hu ? g->us : nullptr,
                                                       hu ? g->vs : nullptr, hu ? g->ws : nullptr, L.ax, L.ay, L.az,
                                                       gau, gav, gaw, gsu, gsv, gsw, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                      bcv(g));
-  g->launches += 1;
+                                                      bcv(g)));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }

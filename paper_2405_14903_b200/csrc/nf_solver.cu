@@ -391,24 +391,23 @@ int nf_solver_init(nf_grid *g) {
 int nf_apply_A_impl(nf_grid *g, const float *p, float *q) {
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(L.nx, L.ny, L.nz);
-  k_apply_A<false><<<d.grid, d.block, 0, g->stream>>>(p, L.ax, L.ay, L.az, q, L.c, L.nx, L.ny, L.nz, L.pax, nullptr, 0);
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_APPLY, k_apply_A<false><<<d.grid, d.block, 0, g->stream>>>(p, L.ax, L.ay, L.az, q, L.c, L.nx, L.ny, L.nz, L.pax, nullptr, 0));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
 
 static void smooth_half(nf_grid *g, NfLevel &L, int color, bool zero, bool dot, NfSolveState *st, int slot) {
   NfDims d = nf_dims((L.nx + 1) / 2, L.ny, L.nz);
+  const bool lvl0 = (&L == &g->lv[0]);
   if (zero)
-    k_rbgs<true, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                           color, st, slot);
+    NF_LAUNCH(g, (lvl0 ? NFK_RBGS0 : NFK_RBGS_C), k_rbgs<true, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
+                                                           color, st, slot));
   else if (dot)
-    k_rbgs<false, true><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                           color, st, slot);
+    NF_LAUNCH(g, (lvl0 ? NFK_RBGS0 : NFK_RBGS_C), k_rbgs<false, true><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
+                                                           color, st, slot));
   else
-    k_rbgs<false, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                            color, st, slot);
-  g->launches += 1;
+    NF_LAUNCH(g, (lvl0 ? NFK_RBGS0 : NFK_RBGS_C), k_rbgs<false, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
+                                                            color, st, slot));
 }
 
 static int bottom_sweeps(const NfLevel &L) {
@@ -428,17 +427,15 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
       smooth_half(g, L, 1, false, false, st, slot);
     }
     NfDims d = nf_dims(C.nx, C.ny, C.nz);
-    k_residual_restrict<<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                           C.r, C.nx, C.ny, C.nz, st);
-    g->launches += 1;
+    NF_LAUNCH(g, (l == 0 ? NFK_RESTRICT0 : NFK_RESTRICT_C), k_residual_restrict<<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
+                                                           C.r, C.nx, C.ny, C.nz, st));
   }
   {
     NfLevel &B = g->lv[nl - 1];
     if (B.ncell <= NF_BOTTOM_MAX_CELLS) {
       const size_t smem = (size_t)9 * B.ncell * sizeof(float);
-      k_bottom<<<1, 256, smem, g->stream>>>(B.z, B.r, B.ax, B.ay, B.az, B.c, B.nx, B.ny, B.nz, B.pax, bottom_sweeps(B),
-                                            st);
-      g->launches += 1;
+      NF_LAUNCH(g, NFK_BOTTOM, k_bottom<<<1, 256, smem, g->stream>>>(B.z, B.r, B.ax, B.ay, B.az, B.c, B.nx, B.ny, B.nz, B.pax, bottom_sweeps(B),
+                                            st));
     } else {  // coarsest level too large for one CTA (odd sizes): a few symmetric sweeps in global memory
       const int nb = 4;
       for (int s = 0; s < nb; ++s) {
@@ -451,15 +448,13 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
       }
     }
     if (nl == 1 && with_dot) {
-      k_dot<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(B.r, B.z, (size_t)B.ncell, &g->st->rz[slot], st);
-      g->launches += 1;
+      NF_LAUNCH(g, NFK_MISC, k_dot<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(B.r, B.z, (size_t)B.ncell, &g->st->rz[slot], st));
     }
   }
   for (int l = nl - 2; l >= 0; --l) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
     NfDims d = nf_dims(L.nx, L.ny, L.nz);
-    k_prolong_add<<<d.grid, d.block, 0, g->stream>>>(L.z, C.z, L.nx, L.ny, L.nz, C.nx, C.ny, st);
-    g->launches += 1;
+    NF_LAUNCH(g, (l == 0 ? NFK_PROLONG0 : NFK_PROLONG_C), k_prolong_add<<<d.grid, d.block, 0, g->stream>>>(L.z, C.z, L.nx, L.ny, L.nz, C.nx, C.ny, st));
     for (int s = 0; s < g->nu_post; ++s) {
       smooth_half(g, L, 1, false, false, st, slot);
       smooth_half(g, L, 0, false, with_dot && l == 0 && s == g->nu_post - 1, st, slot);
@@ -474,14 +469,13 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
 int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit) {
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(L.nx, L.ny, L.nz);
-  k_init_state<<<1, 32, 0, g->stream>>>(g->st, (double)tol, maxit);
-  k_mask_sum<<<d.grid, d.block, 0, g->stream>>>(src ? src : L.r, L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax,
-                                                &g->st->sum);
+  NF_LAUNCH(g, NFK_SETUP, k_init_state<<<1, 32, 0, g->stream>>>(g->st, (double)tol, maxit));
+  NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<d.grid, d.block, 0, g->stream>>>(src ? src : L.r, L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax,
+                                                &g->st->sum));
   const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
-  k_sub_mean<<<d.grid, d.block, 0, g->stream>>>(L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv,
-                                                g->singular, &g->st->bb);
-  k_start_state<<<1, 32, 0, g->stream>>>(g->st);
-  g->launches += 4;
+  NF_LAUNCH(g, NFK_SETUP, k_sub_mean<<<d.grid, d.block, 0, g->stream>>>(L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv,
+                                                g->singular, &g->st->bb));
+  NF_LAUNCH(g, NFK_SETUP, k_start_state<<<1, 32, 0, g->stream>>>(g->st));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -523,23 +517,20 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
   NF_CUDA(g, cudaMemsetAsync(x, 0, n * sizeof(float), g->stream));
   int rc = nf_vcycle_impl(g, true, 0);
   if (rc != NF_OK) return rc;
-  k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, 0, 1);
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, 0, 1));
   int it = 0, last_seen = -1, done = 0, converged = 0;
   float relres = 0.0f;
   if (maxit < 1) maxit = 1;
   for (it = 0; it < maxit && !done; ++it) {
     const int slot = it & 1;
-    k_apply_A<true><<<dc.grid, dc.block, 0, g->stream>>>(g->p, L.ax, L.ay, L.az, g->q, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                         g->st, slot);
-    k_cg_update<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, g->p, g->q, n, v4, g->st, slot);
-    k_cg_check<<<1, 32, 0, g->stream>>>(g->st, slot, &g->hst_dev[it & (NF_RING - 1)], it + 1);
-    g->launches += 3;
+    NF_LAUNCH(g, NFK_APPLY, k_apply_A<true><<<dc.grid, dc.block, 0, g->stream>>>(g->p, L.ax, L.ay, L.az, g->q, L.c, L.nx, L.ny, L.nz, L.pax,
+                                                         g->st, slot));
+    NF_LAUNCH(g, NFK_UPDATE, k_cg_update<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, g->p, g->q, n, v4, g->st, slot));
+    NF_LAUNCH(g, NFK_CHECK, k_cg_check<<<1, 32, 0, g->stream>>>(g->st, slot, &g->hst_dev[it & (NF_RING - 1)], it + 1));
     if (it + 1 < maxit) {
       rc = nf_vcycle_impl(g, true, 1 - slot);
       if (rc != NF_OK) return rc;
-      k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, slot, 0);
-      g->launches += 1;
+      NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, slot, 0));
     }
     NF_CUDA(g, cudaGetLastError());
     const int look = it - NF_LOOKAHEAD;
@@ -567,11 +558,10 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
   }
   // gauge: zero mean over active cells on a singular system (R12)
   if (g->singular) {
-    k_mask_sum<<<dc.grid, dc.block, 0, g->stream>>>(x, x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum);
+    NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<dc.grid, dc.block, 0, g->stream>>>(x, x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum));
     const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
-    k_sub_mean<<<dc.grid, dc.block, 0, g->stream>>>(x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv, 1,
-                                                    nullptr);
-    g->launches += 2;
+    NF_LAUNCH(g, NFK_SETUP, k_sub_mean<<<dc.grid, dc.block, 0, g->stream>>>(x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv, 1,
+                                                    nullptr));
   }
   NF_CUDA(g, cudaGetLastError());
   // iteration count: read back from the device state lazily in nf_last_solve_info; keep the host view here

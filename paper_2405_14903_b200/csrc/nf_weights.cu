@@ -309,8 +309,7 @@ int nf_weights_from_sdf(nf_grid *g, const float *sdf) {
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(g->nx + 1, g->ny + 1, g->nz + 1);
   NF_CUDA(g, cudaMemcpyAsync(g->sdf, sdf, nf_nn(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
-  k_weights_from_sdf<<<d.grid, d.block, 0, g->stream>>>(g->sdf, L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g));
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_WEIGHTS, k_weights_from_sdf<<<d.grid, d.block, 0, g->stream>>>(g->sdf, L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g)));
   g->have_sdf = true;
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
@@ -319,8 +318,7 @@ int nf_weights_from_sdf(nf_grid *g, const float *sdf) {
 int nf_weights_from_user(nf_grid *g, const float *au, const float *av, const float *aw) {
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(g->nx + 1, g->ny + 1, g->nz + 1);
-  k_weights_import<<<d.grid, d.block, 0, g->stream>>>(au, av, aw, L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g));
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_WEIGHTS, k_weights_import<<<d.grid, d.block, 0, g->stream>>>(au, av, aw, L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g)));
   g->have_sdf = false;
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
@@ -330,8 +328,7 @@ int nf_weights_to_user(nf_grid *g, float *au, float *av, float *aw) {
   NfLevel &L = g->lv[0];
   if (au) {
     NfDims d = nf_dims(g->nx + 1, g->ny, g->nz);
-    k_weights_export<<<d.grid, d.block, 0, g->stream>>>(L.ax, au, g->nx, g->ny, g->nz, L.pax);
-    g->launches += 1;
+    NF_LAUNCH(g, NFK_MISC, k_weights_export<<<d.grid, d.block, 0, g->stream>>>(L.ax, au, g->nx, g->ny, g->nz, L.pax));
   }
   if (av) NF_CUDA(g, cudaMemcpyAsync(av, L.ay, nf_nv(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
   if (aw) NF_CUDA(g, cudaMemcpyAsync(aw, L.az, nf_nw(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
@@ -343,16 +340,14 @@ int nf_build_hierarchy(nf_grid *g) {
   for (int l = 0; l + 1 < g->nlev; ++l) {
     NfLevel &F = g->lv[l], &C = g->lv[l + 1];
     NfDims d = nf_dims(C.nx + 1, C.ny + 1, C.nz + 1);
-    k_coarsen_weights<<<d.grid, d.block, 0, g->stream>>>(F.ax, F.ay, F.az, C.ax, C.ay, C.az, F.nx, F.ny, F.nz, F.pax,
-                                                         C.nx, C.ny, C.nz, C.pax);
-    g->launches += 1;
+    NF_LAUNCH(g, NFK_COARSEN, k_coarsen_weights<<<d.grid, d.block, 0, g->stream>>>(F.ax, F.ay, F.az, C.ax, C.ay, C.az, F.nx, F.ny, F.nz, F.pax,
+                                                         C.nx, C.ny, C.nz, C.pax));
   }
   NfLevel &L = g->lv[0];
   double *cnt = g->d_counts;
   NF_CUDA(g, cudaMemsetAsync(cnt, 0, 2 * sizeof(double), g->stream));
   NfDims d = nf_dims(g->nx, g->ny, g->nz);
-  k_classify<<<d.grid, d.block, 0, g->stream>>>(L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g), cnt);
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_CLASSIFY, k_classify<<<d.grid, d.block, 0, g->stream>>>(L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g), cnt));
   NF_CUDA(g, cudaGetLastError());
   NF_CUDA(g, cudaMemcpyAsync(g->h_counts, cnt, 2 * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
   NF_CUDA(g, cudaStreamSynchronize(g->stream));
@@ -369,12 +364,11 @@ int nf_store_solid_velocity(nf_grid *g, const float *us, const float *vs, const 
   const int cl[6] = {g->bc_type[0] == NF_BC_CLOSED, g->bc_type[1] == NF_BC_CLOSED, g->bc_type[2] == NF_BC_CLOSED,
                      g->bc_type[3] == NF_BC_CLOSED, g->bc_type[4] == NF_BC_CLOSED, g->bc_type[5] == NF_BC_CLOSED};
   NfDims d = nf_dims(g->nx + 1, g->ny, g->nz);
-  k_store_us<<<d.grid, d.block, 0, g->stream>>>(us, g->us, g->nx + 1, g->ny, g->nz, 0, cl[0], cl[1]);
+  NF_LAUNCH(g, NFK_STORE_US, k_store_us<<<d.grid, d.block, 0, g->stream>>>(us, g->us, g->nx + 1, g->ny, g->nz, 0, cl[0], cl[1]));
   d = nf_dims(g->nx, g->ny + 1, g->nz);
-  k_store_us<<<d.grid, d.block, 0, g->stream>>>(vs, g->vs, g->nx, g->ny + 1, g->nz, 1, cl[2], cl[3]);
+  NF_LAUNCH(g, NFK_STORE_US, k_store_us<<<d.grid, d.block, 0, g->stream>>>(vs, g->vs, g->nx, g->ny + 1, g->nz, 1, cl[2], cl[3]));
   d = nf_dims(g->nx, g->ny, g->nz + 1);
-  k_store_us<<<d.grid, d.block, 0, g->stream>>>(ws, g->ws, g->nx, g->ny, g->nz + 1, 2, cl[4], cl[5]);
-  g->launches += 3;
+  NF_LAUNCH(g, NFK_STORE_US, k_store_us<<<d.grid, d.block, 0, g->stream>>>(ws, g->ws, g->nx, g->ny, g->nz + 1, 2, cl[4], cl[5]));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -382,8 +376,7 @@ int nf_store_solid_velocity(nf_grid *g, const float *us, const float *vs, const 
 int nf_weights_adjoint_impl(nf_grid *g, const float *gau, const float *gav, const float *gaw, float *gsdf) {
   NF_CUDA(g, cudaMemsetAsync(gsdf, 0, nf_nn(g) * sizeof(float), g->stream));
   NfDims d = nf_dims(g->nx + 1, g->ny + 1, g->nz + 1);
-  k_weights_adjoint<<<d.grid, d.block, 0, g->stream>>>(g->sdf, gau, gav, gaw, gsdf, g->nx, g->ny, g->nz, bc6(g));
-  g->launches += 1;
+  NF_LAUNCH(g, NFK_WEIGHTS_ADJ, k_weights_adjoint<<<d.grid, d.block, 0, g->stream>>>(g->sdf, gau, gav, gaw, gsdf, g->nx, g->ny, g->nz, bc6(g)));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
