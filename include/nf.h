@@ -70,9 +70,11 @@ int nf_set_dt_rho(nf_grid *g, float dt_over_rho);
 int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value);
 
 /* Solver options (PAPER.md:L230 names only "MGPCG"; every parameter is this library's choice, R13):
- *   nu_pre / nu_post: red-black Gauss-Seidel sweeps before / after the coarse correction (default 1, 1);
- *   refine: 0 = plain fp32 PCG (default), 1 = fp64 solution accumulator with true-residual restarts. */
-int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int refine);
+ *   nu_pre / nu_post: red-black Gauss-Seidel sweeps before / after the coarse correction (default 1, 1; the fused
+ *     4-cells-per-thread V-cycle kernels exist for (1, 1) only, other values run the generic kernels);
+ *   flags: bit 0 = iterative refinement (fp64 true-residual restarts; default off),
+ *          bit 1 = test hook: force the generic kernels (fp32 weights, one colour per launch) on every level. */
+int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags);
 
 /* a-1  Face weights from the solid SDF: per face, the fluid area fraction alpha from
  * the 4 node values at its corners (marching-squares area; the printed one-fluid-corner formula

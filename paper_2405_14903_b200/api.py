@@ -163,8 +163,8 @@ class Grid:
     def set_domain_bc(self, face, bc_type, p_value=0.0):
         self._check(self.lib.nf_set_domain_bc(self.h, int(face), int(bc_type), float(p_value)), "nf_set_domain_bc")
 
-    def set_solver_options(self, nu_pre=1, nu_post=1, refine=0):
-        self._check(self.lib.nf_set_solver_options(self.h, nu_pre, nu_post, refine), "nf_set_solver_options")
+    def set_solver_options(self, nu_pre=1, nu_post=1, flags=0):
+        self._check(self.lib.nf_set_solver_options(self.h, nu_pre, nu_post, flags), "nf_set_solver_options")
 
     def set_solid(self, sdf, us=None, vs=None, ws=None):
         self._expect(sdf, self.shape_sdf, "sdf")

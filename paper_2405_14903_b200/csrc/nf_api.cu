@@ -25,10 +25,10 @@ static cudaError_t dalloc(T **p, size_t n) {
 static void free_all(nf_grid *g) {
   for (int l = 0; l < NF_MAX_LEVELS; ++l) {
     NfLevel &L = g->lv[l];
-    cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.z); cudaFree(L.r);
+    cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.code); cudaFree(L.z); cudaFree(L.r);
   }
   cudaFree(g->us); cudaFree(g->vs); cudaFree(g->ws); cudaFree(g->sdf);
-  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->xd);
+  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->xd); cudaFree(g->tailpack);
   cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
   cudaFree(g->st); cudaFree(g->d_counts);
   if (g->hst) cudaFreeHost((void *)g->hst);
@@ -50,7 +50,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->nx = nx; g->ny = ny; g->nz = nz; g->dx = dx; g->dt_over_rho = 1.0f;
   for (int f = 0; f < 6; ++f) { g->bc_type[f] = NF_BC_CLOSED; g->bc_val[f] = 0.0f; }
   g->stream = 0;
-  g->nu_pre = 1; g->nu_post = 1; g->refine = 0;
+  g->nu_pre = 1; g->nu_post = 1; g->refine = 0; g->force_generic = false;
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->nact = 0;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
@@ -70,6 +70,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     ok = ok && dalloc(&L.ax, (size_t)lz * ly * L.pax) == cudaSuccess;
     ok = ok && dalloc(&L.ay, (size_t)lz * (ly + 1) * lx) == cudaSuccess;
     ok = ok && dalloc(&L.az, (size_t)(lz + 1) * ly * lx) == cudaSuccess;
+    ok = ok && dalloc(&L.code, (size_t)L.ncell + 16) == cudaSuccess;
     ok = ok && dalloc(&L.z, (size_t)L.ncell) == cudaSuccess;
     ok = ok && dalloc(&L.r, (size_t)L.ncell) == cudaSuccess;
     if (ok) ok = cudaMemset(L.ax, 0, (size_t)lz * ly * L.pax * sizeof(float)) == cudaSuccess;
@@ -81,6 +82,12 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     c *= 0.25f;
   }
   g->nlev = nl;
+  nf_mg_plan(g);
+  {
+    size_t tc = 0;
+    for (int l = g->tail; l < nl; ++l) tc += (size_t)g->lv[l].ncell;
+    ok = ok && dalloc(&g->tailpack, 8 * tc) == cudaSuccess;
+  }
   const size_t nc = nf_nc(g);
   ok = ok && dalloc(&g->us, nf_nu(g)) == cudaSuccess && dalloc(&g->vs, nf_nv(g)) == cudaSuccess &&
        dalloc(&g->ws, nf_nw(g)) == cudaSuccess && dalloc(&g->sdf, nf_nn(g)) == cudaSuccess;
@@ -138,10 +145,10 @@ extern "C" int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value) {
   return NF_OK;
 }
 
-extern "C" int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int refine) {
+extern "C" int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags) {
   NF_CHECK_HANDLE(g);
-  if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || refine < 0 || refine > 1) return NF_ERR_INVALID;
-  g->nu_pre = nu_pre; g->nu_post = nu_post; g->refine = refine;
+  if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || flags < 0 || flags > 3) return NF_ERR_INVALID;
+  g->nu_pre = nu_pre; g->nu_post = nu_post; g->refine = flags & 1; g->force_generic = (flags & 2) != 0;
   return NF_OK;
 }
 
@@ -337,9 +344,10 @@ extern "C" int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, in
 
 // ---- per-class kernel timing -------------------------------------------------------------------------------------
 static const char *kClassNames[NFK_COUNT] = {
-    "apply_A", "cg_update", "cg_check", "cg_pupdate", "rbgs_fine", "rbgs_coarse", "restrict_fine", "restrict_coarse",
-    "prolong_fine", "prolong_coarse", "bottom", "solve_setup", "rhs", "grad_subtract", "adjoint_rhs", "adjoint_finish",
-    "weights", "coarsen", "classify", "store_us", "advect", "advect_adjoint", "weights_adjoint", "misc"};
+    "apply_A", "cg_update", "cg_check", "cg_pupdate", "down1_fine", "down2_fine", "up1_fine", "up2_fine", "vec_coarse",
+    "rbgs_fine", "rbgs_coarse", "restrict_fine", "restrict_coarse", "prolong_fine", "prolong_coarse", "tail",
+    "solve_setup", "rhs", "grad_subtract", "adjoint_rhs", "adjoint_finish", "weights", "coarsen", "encode", "store_us",
+    "advect", "advect_adjoint", "weights_adjoint", "misc"};
 
 void nf_prof_begin(nf_grid *g, int cls) {
   const size_t r = g->prof_cls.size();

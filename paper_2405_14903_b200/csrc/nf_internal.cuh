@@ -18,13 +18,37 @@
 //   ax[(k*ny + j)*pax + i], i in [0, nx]   weight of the x-face between cells i-1 and i
 //   ay[(k*(ny+1) + j)*nx + i], j in [0, ny]
 //   az[(k*ny + j)*nx + i], k in [0, nz]
+//
+// Cell code (one byte per cell): bits 0..5 = face -x,+x,-y,+y,-z,+z has alpha == 1 exactly,
+// bit 6 (NF_CODE_MIXED) = some face of the cell is fractional (0 < alpha < 1), in which case the six fp32 weights
+// are read instead.  code == 0  <=>  the cell is inactive (sum of its six weights is 0).
+#define NF_CODE_MIXED 64u
+// bit 7 (NF_CODE_DEEP): the cell has six fully open faces and so has each of its six neighbours that lies inside the
+// grid -- the pre-smoother's fast path needs no neighbour code (every diagonal involved is 6c).
+#define NF_CODE_DEEP 128u
 struct NfLevel {
   int nx, ny, nz, pax;
   long long ncell;
   float c;  // c_l = (dt_over_rho/dx) / 4^l  (rediscretised operator on spacing 2^l dx)
   float *ax, *ay, *az;
+  uint8_t *code;
   float *z, *r;  // level 0: CG vectors z and r; level > 0: coarse correction and restricted residual
+  int vec;       // 1: nx % 4 == 0 and a coarser level exists -> the float4 / code kernels run on this level
 };
+
+// Kernel-side view of a level (passed by value).  ic = 1/c.
+struct NfLvK {
+  const float *ax, *ay, *az;
+  const uint8_t *code;
+  float c, ic;
+  int nx, ny, nz, pax;
+};
+static inline NfLvK nf_lvk(const NfLevel &L) {
+  NfLvK K;
+  K.ax = L.ax; K.ay = L.ay; K.az = L.az; K.code = L.code;
+  K.c = L.c; K.ic = 1.0f / L.c; K.nx = L.nx; K.ny = L.ny; K.nz = L.nz; K.pax = L.pax;
+  return K;
+}
 
 // Device-resident PCG scalars.  Slots [2] alternate with the iteration parity so that no kernel has to
 // reset a value another kernel of the same iteration still reads.
@@ -47,10 +71,10 @@ struct NfHostStatus {  // written by the device into mapped pinned memory
 
 // Kernel classes for the per-class device timing of nf_profile_* (bench.py's roofline leg).
 enum {
-  NFK_APPLY = 0, NFK_UPDATE, NFK_CHECK, NFK_PUPDATE, NFK_RBGS0, NFK_RBGS_C, NFK_RESTRICT0, NFK_RESTRICT_C,
-  NFK_PROLONG0, NFK_PROLONG_C, NFK_BOTTOM, NFK_SETUP, NFK_RHS, NFK_GRADSUB, NFK_ADJ_RHS, NFK_ADJ_FINISH,
-  NFK_WEIGHTS, NFK_COARSEN, NFK_CLASSIFY, NFK_STORE_US, NFK_ADVECT, NFK_ADVECT_ADJ, NFK_WEIGHTS_ADJ, NFK_MISC,
-  NFK_COUNT
+  NFK_APPLY = 0, NFK_UPDATE, NFK_CHECK, NFK_PUPDATE, NFK_DOWN1_0, NFK_DOWN2_0, NFK_UP1_0, NFK_UP2_0, NFK_VEC_C,
+  NFK_RBGS0, NFK_RBGS_C, NFK_RESTRICT0, NFK_RESTRICT_C, NFK_PROLONG0, NFK_PROLONG_C, NFK_BOTTOM, NFK_SETUP, NFK_RHS,
+  NFK_GRADSUB, NFK_ADJ_RHS, NFK_ADJ_FINISH, NFK_WEIGHTS, NFK_COARSEN, NFK_CLASSIFY, NFK_STORE_US, NFK_ADVECT,
+  NFK_ADVECT_ADJ, NFK_WEIGHTS_ADJ, NFK_MISC, NFK_COUNT
 };
 
 struct nf_grid {
@@ -60,15 +84,18 @@ struct nf_grid {
   float bc_val[6];
   cudaStream_t stream;
   int nlev;
+  int tail;  // first level of the shared-memory tail of the V-cycle (levels tail .. nlev-1 run in one CTA); nlev if none
   NfLevel lv[NF_MAX_LEVELS];
   bool weights_set, have_sdf, have_us;
   int singular;
   long long nact;
   int nu_pre, nu_post, refine;
+  bool force_generic;  // test hook: run the generic (fp32-weight, one colour per launch) kernels everywhere
   // solid velocity (MAC layout, closed walls at rest) and the last SDF
   float *us, *vs, *ws, *sdf;
   // CG vectors on level 0 (r and z live in lv[0])
   float *p, *q, *xtmp;
+  float *tailpack;  // 8 floats per cell of the tail levels (nf_mg.cu)
   double *xd;  // fp64 solution accumulator (refine mode)
   // scratch face arrays (advection copy / adjoint staging)
   float *fu, *fv, *fw;
@@ -147,6 +174,10 @@ int nf_store_solid_velocity(nf_grid *g, const float *us, const float *vs, const 
 int nf_weights_adjoint_impl(nf_grid *g, const float *gau, const float *gav, const float *gaw, float *gsdf);
 // nf_solver.cu
 int nf_apply_A_impl(nf_grid *g, const float *p, float *q);
+// nf_mg.cu
+void nf_mg_plan(nf_grid *g);      // choose the shared-memory tail and the vec levels (after the level extents are known)
+int nf_mg_init(nf_grid *g);       // kernel attributes
+int nf_mg_pack_tail(nf_grid *g);  // packed operator of the tail levels from the current weights
 int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot);  // z = M^{-1} r on lv[0].r -> lv[0].z
 // Solve A x = lv[0].r (already masked; mean removed if singular; st->bb set by nf_solve_prepare).
 int nf_solver_init(nf_grid *g);                          // kernel attributes (once per process)

@@ -1,0 +1,655 @@
+// nf_mg.cu -- a-5 the multigrid V-cycle preconditioner z = M^{-1} r of MGPCG ("MGPCG ... hierarchical
+// grid data structure, with custom CUDA kernels for prolongation and restriction").  Everything the paper leaves
+// open (R13) is this library's choice: V(1,1), red-black Gauss-Seidel (pre: red->black from a
+// zero guess, post: black->red), piecewise-constant prolongation P, restriction P^T/8, rediscretised coarse operators.
+//
+// Three families of kernels:
+//   * "vec" kernels (levels with nx % 4 == 0): 4 cells per thread, float4 rows, weights from the 1-byte cell code.
+//     One level of the V-cycle is 4 launches, none of them a single-colour pass over the arrays:
+//       k_down1  z = pre-smooth(r)            red: z = r/diag;  black: z = (r + c sum a z_red)/diag, red values
+//                                             recomputed on the fly from r (no second pass, no halo exchange)
+//       k_down2  r_coarse = P^T/8 (r - A z)   only the red children contribute (the residual is zero on the cells
+//                                             the last half sweep updated); for them r - A z = c sum a z_black
+//       k_up1    black half sweep of the post-smoother on z + P z_coarse, prolongation evaluated on the fly
+//       k_up2    red half sweep (+ r.z on level 0)
+//   * generic kernels (any extents): one colour per launch, fp32 weights -- the v1 path, kept for ragged levels.
+//   * k_tail: all levels that fit one CTA's shared memory (<= 5632 cells in total), whole sub-V-cycle in one launch.
+#include "nf_stencil.cuh"
+
+#define NF_VEC_BLOCKS (148 * 8)
+#define NF_TAIL_MAX_CELLS 5632  // 10 floats per cell of shared memory: 225,280 B <= 227 KB
+#define NF_TAIL_THREADS 1024
+
+// ------------------------------------------------------------------------------------------------------------
+// vec kernels
+// ------------------------------------------------------------------------------------------------------------
+struct NfRow4 {  // one row segment of 4 cells: values and codes, with the idiag-scaled value on demand
+  float v[4];
+  unsigned c4;
+};
+__device__ __forceinline__ NfRow4 nf_row(const float *__restrict__ f, const uint8_t *__restrict__ code, size_t id,
+                                         bool ok) {
+  NfRow4 R;
+  nf_unpack4(nf_ld4(f, id, ok), R.v);
+  R.c4 = nf_ldc4(code, id, ok);
+  return R;
+}
+
+// PAR = (i0 + j + k) & 1 = colour of the first of the 4 cells; cell q is red iff ((q + PAR) & 1) == 0.
+template <int PAR>
+__device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *__restrict__ r, float *__restrict__ z,
+                                              int i0, int j, int k) {
+  const int nx = L.nx, ny = L.ny, nz = L.nz;
+  const size_t sy = nx, sz = (size_t)nx * ny;
+  const size_t id = ((size_t)k * ny + j) * nx + i0;
+  const NfRow4 C = nf_row(r, L.code, id, true);
+  float out[4];
+  if ((C.c4 & 0x80808080u) == 0x80808080u) {
+    // all four cells are deep interior (NF_CODE_DEEP): every diagonal involved is 6c, every weight is 1, and no
+    // neighbour code is needed
+    float yl[4], yh[4], zl[4], zh[4];
+    nf_unpack4(nf_ld4(r, id - sy, j > 0), yl);
+    nf_unpack4(nf_ld4(r, id + sy, j + 1 < ny), yh);
+    nf_unpack4(nf_ld4(r, id - sz, k > 0), zl);
+    nf_unpack4(nf_ld4(r, id + sz, k + 1 < nz), zh);
+    const float g6 = L.ic * (1.0f / 6.0f);
+    const float te = PAR ? nf_ld1(r, id - 1, i0 > 0) : nf_ld1(r, id + 4, i0 + 4 < nx);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      if (((q + PAR) & 1) == 0) {
+        out[q] = C.v[q] * g6;
+      } else {
+        const float tl = q > 0 ? C.v[q - 1] : te, th = q < 3 ? C.v[q + 1] : te;
+        const float sum = ((tl + th) + (yl[q] + yh[q])) + (zl[q] + zh[q]);
+        out[q] = (C.v[q] + (1.0f / 6.0f) * sum) * g6;
+      }
+    }
+    *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
+    return;
+  }
+  const NfRow4 Yl = nf_row(r, L.code, id - sy, j > 0), Yh = nf_row(r, L.code, id + sy, j + 1 < ny);
+  const NfRow4 Zl = nf_row(r, L.code, id - sz, k > 0), Zh = nf_row(r, L.code, id + sz, k + 1 < nz);
+  float idg[4], t[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    idg[q] = nf_code_idiag(L, nf_code_at(C.c4, q), i0 + q, j, k);
+    t[q] = C.v[q] * idg[q];
+  }
+  // the x-neighbour outside the segment that a black cell needs: left of q = 0 (PAR = 1) or right of q = 3 (PAR = 0)
+  float te;
+  if (PAR) {
+    const bool ok = i0 > 0;
+    te = nf_ld1(r, id - 1, ok) * nf_code_idiag(L, nf_ldc1(L.code, id - 1, ok), i0 - 1, j, k);
+  } else {
+    const bool ok = i0 + 4 < nx;
+    te = nf_ld1(r, id + 4, ok) * nf_code_idiag(L, nf_ldc1(L.code, id + 4, ok), i0 + 4, j, k);
+  }
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (((q + PAR) & 1) == 0) {
+      out[q] = t[q];  // red: z = r / diag
+    } else {          // black: its six neighbours are red
+      const NfW6 w = nf_code_w6(L, nf_code_at(C.c4, q), i0 + q, j, k);
+      const float tl = q > 0 ? t[q - 1] : te, th = q < 3 ? t[q + 1] : te;
+      float s = w.xl * tl + w.xh * th;
+      s += w.yl * (Yl.v[q] * nf_code_idiag(L, nf_code_at(Yl.c4, q), i0 + q, j - 1, k));
+      s += w.yh * (Yh.v[q] * nf_code_idiag(L, nf_code_at(Yh.c4, q), i0 + q, j + 1, k));
+      s += w.zl * (Zl.v[q] * nf_code_idiag(L, nf_code_at(Zl.c4, q), i0 + q, j, k - 1));
+      s += w.zh * (Zh.v[q] * nf_code_idiag(L, nf_code_at(Zh.c4, q), i0 + q, j, k + 1));
+      out[q] = (C.v[q] + L.c * s) * idg[q];
+    }
+  }
+  *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
+}
+
+__global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restrict__ r, float *__restrict__ z,
+                                               const NfSolveState *st) {
+  if (st && st->done) return;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i0 >= L.nx || j >= L.ny || k >= L.nz) return;
+  if ((j + k) & 1)
+    nf_down1_body<1>(L, r, z, i0, j, k);
+  else
+    nf_down1_body<0>(L, r, z, i0, j, k);
+}
+
+// One thread per pair of coarse cells (I0, I0+1) = fine cells i0..i0+3 of the rows (2J+dj, 2K+dk).
+__global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restrict__ z, float *__restrict__ rc, int cnx,
+                                               int cny, int cnz, const NfSolveState *st) {
+  if (st && st->done) return;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int J = blockIdx.y * blockDim.y + threadIdx.y;
+  const int K = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i0 >= L.nx || J >= cny || K >= cnz) return;
+  const int nx = L.nx, ny = L.ny, nz = L.nz;
+  const size_t sy = nx, sz = (size_t)nx * ny;
+  const int j0 = 2 * J, k0 = 2 * K;
+  float zc[2][2][4];  // [dk][dj][q]
+  unsigned cc[2][2];
+#pragma unroll
+  for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+    for (int dj = 0; dj < 2; ++dj) {
+      const size_t id = ((size_t)(k0 + dk) * ny + (j0 + dj)) * nx + i0;
+      nf_unpack4(nf_ld4(z, id, true), zc[dk][dj]);
+      cc[dk][dj] = nf_ldc4(L.code, id, true);
+    }
+  float acc0 = 0.0f, acc1 = 0.0f;
+#pragma unroll
+  for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+    for (int dj = 0; dj < 2; ++dj) {
+      const int j = j0 + dj, k = k0 + dk;
+      const size_t id = ((size_t)k * ny + j) * nx + i0;
+      const int par = (dj + dk) & 1;  // colour of q = 0 in this row (i0, j0, k0 are even)
+      // the y / z neighbour rows: inside the 2x2 block or one row outside it
+      float yo[4], zo[4];
+      nf_unpack4(dj == 0 ? nf_ld4(z, id - sy, j > 0) : nf_ld4(z, id + sy, j + 1 < ny), yo);
+      nf_unpack4(dk == 0 ? nf_ld4(z, id - sz, k > 0) : nf_ld4(z, id + sz, k + 1 < nz), zo);
+      const float xe = par == 0 ? nf_ld1(z, id - 1, i0 > 0) : nf_ld1(z, id + 4, i0 + 4 < nx);
+      const bool open4 = (cc[dk][dj] & 0x7f7f7f7fu) == 0x3f3f3f3fu;  // all four cells: six open faces
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        if (((q + par) & 1) != 0) continue;  // red children only
+        const float xl = q > 0 ? zc[dk][dj][q - 1] : xe, xh = q < 3 ? zc[dk][dj][q + 1] : xe;
+        const float yl = dj == 0 ? yo[q] : zc[dk][0][q], yh = dj == 0 ? zc[dk][1][q] : yo[q];
+        const float zl = dk == 0 ? zo[q] : zc[0][dj][q], zh = dk == 0 ? zc[1][dj][q] : zo[q];
+        float s;
+        if (open4) {
+          s = ((xl + xh) + (yl + yh)) + (zl + zh);
+        } else {
+          const NfW6 w = nf_code_w6(L, nf_code_at(cc[dk][dj], q), i0 + q, j, k);
+          s = ((w.xl * xl + w.xh * xh) + (w.yl * yl + w.yh * yh)) + (w.zl * zl + w.zh * zh);
+        }
+        if (q < 2) acc0 += s; else acc1 += s;
+      }
+    }
+  const float f = 0.125f * L.c;
+  *reinterpret_cast<float2 *>(rc + ((size_t)K * cny + J) * cnx + (i0 >> 1)) = make_float2(f * acc0, f * acc1);
+}
+
+// z + P z_coarse on a row of 4 fine cells
+__device__ __forceinline__ void nf_row_prolonged(const float *z, const float *__restrict__ zc, size_t id, size_t cid,
+                                                 bool ok, float o[4]) {
+  if (ok) {
+    const float4 a = *reinterpret_cast<const float4 *>(z + id);
+    const float2 b = __ldg(reinterpret_cast<const float2 *>(zc + cid));
+    o[0] = a.x + b.x; o[1] = a.y + b.x; o[2] = a.z + b.y; o[3] = a.w + b.y;
+  } else {
+    o[0] = o[1] = o[2] = o[3] = 0.0f;
+  }
+}
+
+// Black half sweep on z + P zc (in place: only black cells change; red cells keep the un-prolonged value, which
+// k_up2 overwrites without reading).
+template <int PAR>
+__device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const float *__restrict__ r,
+                                            const float *__restrict__ zc, int cnx, int cny, int i0, int j, int k) {
+  const int nx = L.nx, ny = L.ny, nz = L.nz;
+  const size_t sy = nx, sz = (size_t)nx * ny;
+  const size_t id = ((size_t)k * ny + j) * nx + i0;
+  const size_t scy = cnx, scz = (size_t)cnx * cny;
+  const size_t cid = ((size_t)(k >> 1) * cny + (j >> 1)) * cnx + (i0 >> 1);
+  const float4 zold = *reinterpret_cast<const float4 *>(z + id);
+  float zp[4], yl[4], yh[4], zl[4], zh[4], rr[4], out[4];
+  {
+    const float2 b = __ldg(reinterpret_cast<const float2 *>(zc + cid));
+    zp[0] = zold.x + b.x; zp[1] = zold.y + b.x; zp[2] = zold.z + b.y; zp[3] = zold.w + b.y;
+  }
+  // parent row of j-1 is the same as j's iff j is odd; of j+1 iff j is even (same in z)
+  nf_row_prolonged(z, zc, id - sy, (j & 1) ? cid : cid - scy, j > 0, yl);
+  nf_row_prolonged(z, zc, id + sy, (j & 1) ? cid + scy : cid, j + 1 < ny, yh);
+  nf_row_prolonged(z, zc, id - sz, (k & 1) ? cid : cid - scz, k > 0, zl);
+  nf_row_prolonged(z, zc, id + sz, (k & 1) ? cid + scz : cid, k + 1 < nz, zh);
+  nf_unpack4(nf_ld4(r, id, true), rr);
+  const unsigned c4 = nf_ldc4(L.code, id, true);
+  float xe;
+  if (PAR) {
+    const bool ok = i0 > 0;
+    xe = ok ? z[id - 1] + __ldg(zc + cid - 1) : 0.0f;
+  } else {
+    const bool ok = i0 + 4 < nx;
+    xe = ok ? z[id + 4] + __ldg(zc + cid + 2) : 0.0f;
+  }
+  out[0] = zold.x; out[1] = zold.y; out[2] = zold.z; out[3] = zold.w;
+  const bool open4 = (c4 & 0x7f7f7f7fu) == 0x3f3f3f3fu;
+  const float g6 = L.ic * (1.0f / 6.0f);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (((q + PAR) & 1) == 0) continue;
+    const float xl = q > 0 ? zp[q - 1] : xe, xh = q < 3 ? zp[q + 1] : xe;
+    if (open4) {
+      const float s = ((xl + xh) + (yl[q] + yh[q])) + (zl[q] + zh[q]);
+      out[q] = (rr[q] + L.c * s) * g6;
+    } else {
+      const unsigned code = nf_code_at(c4, q);
+      const NfW6 w = nf_code_w6(L, code, i0 + q, j, k);
+      const float s = ((w.xl * xl + w.xh * xh) + (w.yl * yl[q] + w.yh * yh[q])) + (w.zl * zl[q] + w.zh * zh[q]);
+      out[q] = (rr[q] + L.c * s) * nf_code_idiag(L, code, i0 + q, j, k);
+    }
+  }
+  *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
+}
+
+__global__ void __launch_bounds__(256, 4) k_up1(NfLvK L, float *z, const float *__restrict__ r,
+                                             const float *__restrict__ zc, int cnx, int cny, const NfSolveState *st) {
+  if (st && st->done) return;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i0 >= L.nx || j >= L.ny || k >= L.nz) return;
+  if ((j + k) & 1)
+    nf_up1_body<1>(L, z, r, zc, cnx, cny, i0, j, k);
+  else
+    nf_up1_body<0>(L, z, r, zc, cnx, cny, i0, j, k);
+}
+
+// Red half sweep in place (black neighbours are final); returns r.z over the 4 cells.
+template <int PAR>
+__device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const float *__restrict__ r, int i0, int j,
+                                             int k) {
+  const int nx = L.nx, ny = L.ny, nz = L.nz;
+  const size_t sy = nx, sz = (size_t)nx * ny;
+  const size_t id = ((size_t)k * ny + j) * nx + i0;
+  float zc[4], yl[4], yh[4], zl[4], zh[4], rr[4];
+  nf_unpack4(nf_ld4(z, id, true), zc);
+  nf_unpack4(nf_ld4(z, id - sy, j > 0), yl);
+  nf_unpack4(nf_ld4(z, id + sy, j + 1 < ny), yh);
+  nf_unpack4(nf_ld4(z, id - sz, k > 0), zl);
+  nf_unpack4(nf_ld4(z, id + sz, k + 1 < nz), zh);
+  nf_unpack4(nf_ld4(r, id, true), rr);
+  const unsigned c4 = nf_ldc4(L.code, id, true);
+  // red q = 0 needs its left neighbour (PAR = 0), red q = 3 its right neighbour (PAR = 1)
+  const float xe = PAR == 0 ? nf_ld1(z, id - 1, i0 > 0) : nf_ld1(z, id + 4, i0 + 4 < nx);
+  float dot = 0.0f;
+  const bool open4 = (c4 & 0x7f7f7f7fu) == 0x3f3f3f3fu;
+  const float g6 = L.ic * (1.0f / 6.0f);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (((q + PAR) & 1) == 0) {
+      const float xl = q > 0 ? zc[q - 1] : xe, xh = q < 3 ? zc[q + 1] : xe;
+      if (open4) {
+        const float s = ((xl + xh) + (yl[q] + yh[q])) + (zl[q] + zh[q]);
+        zc[q] = (rr[q] + L.c * s) * g6;
+      } else {
+        const unsigned code = nf_code_at(c4, q);
+        const NfW6 w = nf_code_w6(L, code, i0 + q, j, k);
+        const float s = ((w.xl * xl + w.xh * xh) + (w.yl * yl[q] + w.yh * yh[q])) + (w.zl * zl[q] + w.zh * zh[q]);
+        zc[q] = (rr[q] + L.c * s) * nf_code_idiag(L, code, i0 + q, j, k);
+      }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < 4; ++q) dot += rr[q] * zc[q];
+  *reinterpret_cast<float4 *>(z + id) = make_float4(zc[0], zc[1], zc[2], zc[3]);
+  return dot;
+}
+
+template <bool DOT>
+__global__ void __launch_bounds__(256, 4) k_up2(NfLvK L, float *z, const float *__restrict__ r, NfSolveState *st,
+                                             int slot) {
+  if (st && st->done) return;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  float dot = 0.0f;
+  if (i0 < L.nx && j < L.ny && k < L.nz)
+    dot = ((j + k) & 1) ? nf_up2_body<1>(L, z, r, i0, j, k) : nf_up2_body<0>(L, z, r, i0, j, k);
+  if (DOT) nf_block_atomic_add((double)dot, &st->rz[slot]);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// generic kernels (any extents, fp32 weights, one colour per launch)
+// ------------------------------------------------------------------------------------------------------------
+// Red-black Gauss-Seidel half sweep on the cells with (i+j+k) % 2 == color.  One thread per x-pair of cells.
+// ZERO: the initial guess is zero (neighbours are not read).  DOT: also accumulate r.z over BOTH cells of the pair
+// (used on the last half sweep of the V-cycle on level 0, where z is final).
+template <bool ZERO, bool DOT>
+__global__ void __launch_bounds__(256) k_rbgs(float *__restrict__ z, const float *__restrict__ r,
+                                              const float *__restrict__ ax, const float *__restrict__ ay,
+                                              const float *__restrict__ az, float c, int nx, int ny, int nz, int pax,
+                                              int color, NfSolveState *st, int slot) {
+  if (st && st->done) return;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  double part = 0.0;
+  if (j < ny && k < nz) {
+    const int par = (j + k + color) & 1;
+    const int i = 2 * t + par;
+    if (i < nx) {
+      const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
+      const size_t id = ((size_t)k * ny + j) * nx + i;
+      const float d = nf_w6_sum(w);
+      float zn = 0.0f;
+      const float rv = r[id];
+      if (d > 0.0f) {
+        float s = rv;
+        if (!ZERO) s += c * nf_nb_sum(z, w, i, j, k, nx, ny, nz);
+        zn = s / (c * d);
+      }
+      z[id] = zn;
+      if (DOT) part = (double)rv * (double)zn;
+    }
+    if (DOT) {
+      const int io = 2 * t + 1 - par;
+      if (io < nx) {
+        const size_t ido = ((size_t)k * ny + j) * nx + io;
+        part += (double)r[ido] * (double)z[ido];
+      }
+    }
+  }
+  if (DOT) nf_block_atomic_add(part, &st->rz[slot]);
+}
+
+// r_c = (1/8) sum over the 8 children of (r_f - A_f z_f)   (R = P^T / 8, P = piecewise-constant prolongation)
+__global__ void __launch_bounds__(256) k_residual_restrict(const float *__restrict__ z, const float *__restrict__ r,
+                                                           const float *__restrict__ ax, const float *__restrict__ ay,
+                                                           const float *__restrict__ az, float c, int nx, int ny,
+                                                           int nz, int pax, float *__restrict__ rc, int cnx, int cny,
+                                                           int cnz, const NfSolveState *st) {
+  if (st && st->done) return;
+  const int I = blockIdx.x * blockDim.x + threadIdx.x;
+  const int J = blockIdx.y * blockDim.y + threadIdx.y;
+  const int K = blockIdx.z * blockDim.z + threadIdx.z;
+  if (I >= cnx || J >= cny || K >= cnz) return;
+  float acc = 0.0f;
+#pragma unroll
+  for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+    for (int dj = 0; dj < 2; ++dj)
+#pragma unroll
+      for (int di = 0; di < 2; ++di) {
+        const int i = 2 * I + di, j = 2 * J + dj, k = 2 * K + dk;
+        const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
+        const size_t id = ((size_t)k * ny + j) * nx + i;
+        acc += r[id] - c * (nf_w6_sum(w) * z[id] - nf_nb_sum(z, w, i, j, k, nx, ny, nz));
+      }
+  rc[((size_t)K * cny + J) * cnx + I] = 0.125f * acc;
+}
+
+// z_f += z_c[parent]   (piecewise-constant prolongation)
+__global__ void __launch_bounds__(256) k_prolong_add(float *__restrict__ z, const float *__restrict__ zc, int nx,
+                                                     int ny, int nz, int cnx, int cny, const NfSolveState *st) {
+  if (st && st->done) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i >= nx || j >= ny || k >= nz) return;
+  z[((size_t)k * ny + j) * nx + i] += __ldg(zc + ((size_t)(k >> 1) * cny + (j >> 1)) * cnx + (i >> 1));
+}
+
+__global__ void __launch_bounds__(256) k_dot_rz(const float *__restrict__ a, const float *__restrict__ b, size_t n,
+                                                double *dst, const NfSolveState *st) {
+  if (st && st->done) return;
+  double part = 0.0;
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = tid; t < n; t += nth) part += (double)a[t] * (double)b[t];
+  nf_block_atomic_add(part, dst);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// tail: levels tail .. nlev-1 inside one CTA, everything in shared memory
+// ------------------------------------------------------------------------------------------------------------
+// Per level the hierarchy build packs (k_tail_pack): idg[n] = 1/(c diag) (0 inactive), wg[f][n] = c alpha_f with
+// faces towards the outside of the grid zeroed, col[n] = (i+j+k) & 1 as float.  8n floats per level.
+struct NfTailK {
+  int nlev, sweeps;
+  int n[NF_MAX_LEVELS], nx[NF_MAX_LEVELS], ny[NF_MAX_LEVELS], nz[NF_MAX_LEVELS];
+  int off[NF_MAX_LEVELS];  // offset (in cells) of the level in the packed arrays
+};
+
+__global__ void __launch_bounds__(256) k_tail_pack(const float *__restrict__ ax, const float *__restrict__ ay,
+                                                   const float *__restrict__ az, float c, int nx, int ny, int nz,
+                                                   int pax, float *__restrict__ pack) {
+  const int n = nx * ny * nz;
+  const int id = blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= n) return;
+  const int i = id % nx, j = (id / nx) % ny, k = id / (nx * ny);
+  const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
+  const float d = nf_w6_sum(w);
+  pack[id] = d > 0.0f ? 1.0f / (c * d) : 0.0f;
+  pack[1 * n + id] = i > 0 ? c * w.xl : 0.0f;
+  pack[2 * n + id] = i + 1 < nx ? c * w.xh : 0.0f;
+  pack[3 * n + id] = j > 0 ? c * w.yl : 0.0f;
+  pack[4 * n + id] = j + 1 < ny ? c * w.yh : 0.0f;
+  pack[5 * n + id] = k > 0 ? c * w.zl : 0.0f;
+  pack[6 * n + id] = k + 1 < nz ? c * w.zh : 0.0f;
+  pack[7 * n + id] = (float)((i + j + k) & 1);
+}
+
+// smem per level (offset 10*off[l] floats): z[n], r[n], pack[8n]
+__device__ __forceinline__ void nf_tail_half(float *__restrict__ z, const float *__restrict__ r,
+                                             const float *__restrict__ pk, int n, int sy, int sz, float color,
+                                             bool zero) {
+  for (int id = threadIdx.x; id < n; id += blockDim.x) {
+    if (pk[7 * n + id] != color) continue;
+    float a = r[id];
+    if (!zero) {
+      a += pk[1 * n + id] * z[max(id - 1, 0)];
+      a += pk[2 * n + id] * z[min(id + 1, n - 1)];
+      a += pk[3 * n + id] * z[max(id - sy, 0)];
+      a += pk[4 * n + id] * z[min(id + sy, n - 1)];
+      a += pk[5 * n + id] * z[max(id - sz, 0)];
+      a += pk[6 * n + id] * z[min(id + sz, n - 1)];
+    }
+    z[id] = a * pk[id];
+  }
+  __syncthreads();
+}
+
+__global__ void __launch_bounds__(NF_TAIL_THREADS) k_tail(NfTailK T, const float *__restrict__ pack_g,
+                                                           const float *__restrict__ rg, float *__restrict__ zg,
+                                                           const NfSolveState *st) {
+  if (st && st->done) return;
+  extern __shared__ float sm[];
+  const int nl = T.nlev;
+  // load the packs, the first level's right-hand side, zero every z
+  for (int l = 0; l < nl; ++l) {
+    const int n = T.n[l];
+    float *base = sm + 10 * (size_t)T.off[l];
+    const float *src = pack_g + 8 * (size_t)T.off[l];
+    for (int t = threadIdx.x; t < 8 * n; t += blockDim.x) base[2 * n + t] = src[t];
+    for (int t = threadIdx.x; t < n; t += blockDim.x) {
+      base[t] = 0.0f;
+      base[n + t] = l == 0 ? rg[t] : 0.0f;
+    }
+  }
+  __syncthreads();
+  // down
+  for (int l = 0; l + 1 < nl; ++l) {
+    const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
+    float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
+    nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, true);
+    nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+    // residual + restriction: r_c = 1/8 sum children (r - A z), A z = z/idg - sum wg z_nb on active cells
+    const int cn = T.n[l + 1], cnx = T.nx[l + 1], cny = T.ny[l + 1];
+    float *rc = sm + 10 * (size_t)T.off[l + 1] + cn;
+    const int sy = nx, sz = nx * ny;
+    for (int cidx = threadIdx.x; cidx < cn; cidx += blockDim.x) {
+      const int I = cidx % cnx, J = (cidx / cnx) % cny, K = cidx / (cnx * cny);
+      float acc = 0.0f;
+#pragma unroll
+      for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+        for (int dj = 0; dj < 2; ++dj)
+#pragma unroll
+          for (int di = 0; di < 2; ++di) {
+            const int id = ((2 * K + dk) * ny + (2 * J + dj)) * nx + 2 * I + di;
+            const float s = pk[1 * n + id] * z[max(id - 1, 0)] + pk[2 * n + id] * z[min(id + 1, n - 1)] +
+                      pk[3 * n + id] * z[max(id - sy, 0)] + pk[4 * n + id] * z[min(id + sy, n - 1)] +
+                      pk[5 * n + id] * z[max(id - sz, 0)] + pk[6 * n + id] * z[min(id + sz, n - 1)];
+            const float idg = pk[id];
+            // c*diag = 1/idg on active cells (includes faces towards Dirichlet ghosts); inactive: r = 0, z = 0
+            if (idg > 0.0f) acc += r[id] - (z[id] / idg - s);
+          }
+      rc[cidx] = 0.125f * acc;
+    }
+    __syncthreads();
+  }
+  // coarsest level: `sweeps` red->black sweeps from a zero guess, then `sweeps` black->red sweeps (symmetric)
+  {
+    const int l = nl - 1;
+    const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
+    float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
+    for (int s = 0; s < T.sweeps; ++s) {
+      nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, s == 0);
+      nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+    }
+    for (int s = 0; s < T.sweeps; ++s) {
+      nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+      nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, false);
+    }
+  }
+  // up
+  for (int l = nl - 2; l >= 0; --l) {
+    const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
+    float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
+    const int cnx = T.nx[l + 1], cny = T.ny[l + 1];
+    const float *zc = sm + 10 * (size_t)T.off[l + 1];
+    for (int id = threadIdx.x; id < n; id += blockDim.x) {
+      const int i = id % nx, j = (id / nx) % ny, k = id / (nx * ny);
+      z[id] += zc[((k >> 1) * cny + (j >> 1)) * cnx + (i >> 1)];
+    }
+    __syncthreads();
+    nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+    nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, false);
+  }
+  for (int t = threadIdx.x; t < T.n[0]; t += blockDim.x) zg[t] = sm[t];
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------------------
+static size_t tail_smem_bytes(const nf_grid *g) {
+  size_t cells = 0;
+  for (int l = g->tail; l < g->nlev; ++l) cells += (size_t)g->lv[l].ncell;
+  return cells * 10 * sizeof(float);
+}
+
+// Decide which levels form the shared-memory tail and which run the vec kernels (called from nf_grid_create).
+void nf_mg_plan(nf_grid *g) {
+  const int nl = g->nlev;
+  long long cells = 0;
+  int tail = nl;
+  for (int l = nl - 1; l >= 0; --l) {
+    if (cells + g->lv[l].ncell > NF_TAIL_MAX_CELLS) break;
+    cells += g->lv[l].ncell;
+    tail = l;
+  }
+  g->tail = tail;
+  const int nb = tail < nl ? tail : nl - 1;  // levels [0, nb) have a coarser level below them
+  for (int l = 0; l < nl; ++l) g->lv[l].vec = (l < nb && (g->lv[l].nx & 3) == 0) ? 1 : 0;
+}
+
+int nf_mg_init(nf_grid *g) {
+  NF_CUDA(g, cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  NF_TAIL_MAX_CELLS * 10 * (int)sizeof(float)));
+  return NF_OK;
+}
+
+// (re)build the packed tail arrays from the current weights
+int nf_mg_pack_tail(nf_grid *g) {
+  size_t off = 0;
+  for (int l = g->tail; l < g->nlev; ++l) {
+    NfLevel &L = g->lv[l];
+    const int n = (int)L.ncell;
+    NF_LAUNCH(g, NFK_COARSEN, k_tail_pack<<<(n + 255) / 256, 256, 0, g->stream>>>(L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->tailpack + 8 * off));
+    off += (size_t)n;
+  }
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
+static void smooth_half(nf_grid *g, NfLevel &L, int color, bool zero, bool dot, NfSolveState *st, int slot) {
+  NfDims d = nf_dims((L.nx + 1) / 2, L.ny, L.nz);
+  const int cls = (&L == &g->lv[0]) ? NFK_RBGS0 : NFK_RBGS_C;
+  if (zero)
+    NF_LAUNCH(g, cls, k_rbgs<true, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot));
+  else if (dot)
+    NF_LAUNCH(g, cls, k_rbgs<false, true><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot));
+  else
+    NF_LAUNCH(g, cls, k_rbgs<false, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot));
+}
+
+// z = M^{-1} r on level 0 (lv[0].r -> lv[0].z).  with_dot: accumulate r.z into st->rz[slot] and honour st->done.
+int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
+  NfSolveState *st = with_dot ? g->st : nullptr;
+  const int nl = g->nlev;
+  const bool has_tail = g->tail < nl;
+  const int nb = has_tail ? g->tail : nl - 1;
+  const bool fused = g->nu_pre == 1 && g->nu_post == 1 && !g->force_generic;
+  bool dot_done = false;
+  for (int l = 0; l < nb; ++l) {
+    NfLevel &L = g->lv[l], &C = g->lv[l + 1];
+    if (L.vec && fused) {
+      NfDims d = nf_dims(L.nx / 4, L.ny, L.nz);
+      NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), k_down1<<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.r, L.z, st));
+      NfDims d2 = nf_dims(L.nx / 4, C.ny, C.nz);
+      NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), k_down2<<<d2.grid, d2.block, 0, g->stream>>>(nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, st));
+    } else {
+      for (int s = 0; s < g->nu_pre; ++s) {
+        smooth_half(g, L, 0, s == 0, false, st, slot);
+        smooth_half(g, L, 1, false, false, st, slot);
+      }
+      NfDims d = nf_dims(C.nx, C.ny, C.nz);
+      NF_LAUNCH(g, (l == 0 ? NFK_RESTRICT0 : NFK_RESTRICT_C), k_residual_restrict<<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, C.r, C.nx, C.ny, C.nz, st));
+    }
+  }
+  if (has_tail) {
+    NfTailK T;
+    T.nlev = nl - g->tail;
+    int off = 0, m = 1;
+    for (int l = g->tail; l < nl; ++l) {
+      const NfLevel &L = g->lv[l];
+      const int t = l - g->tail;
+      T.n[t] = (int)L.ncell; T.nx[t] = L.nx; T.ny[t] = L.ny; T.nz[t] = L.nz; T.off[t] = off;
+      off += (int)L.ncell;
+      if (l == nl - 1) m = L.nx > L.ny ? (L.nx > L.nz ? L.nx : L.nz) : (L.ny > L.nz ? L.ny : L.nz);
+    }
+    T.sweeps = 2 * m;
+    NfLevel &F = g->lv[g->tail];
+    NF_LAUNCH(g, NFK_BOTTOM, k_tail<<<1, NF_TAIL_THREADS, tail_smem_bytes(g), g->stream>>>(T, g->tailpack, F.r, F.z, st));
+  } else {  // coarsest level too large for one CTA (odd extents): a few symmetric sweeps in global memory
+    NfLevel &B = g->lv[nl - 1];
+    const int nsw = 4;
+    for (int s = 0; s < nsw; ++s) {
+      smooth_half(g, B, 0, s == 0, false, st, slot);
+      smooth_half(g, B, 1, false, false, st, slot);
+    }
+    for (int s = 0; s < nsw; ++s) {
+      smooth_half(g, B, 1, false, false, st, slot);
+      smooth_half(g, B, 0, false, false, st, slot);
+    }
+  }
+  for (int l = nb - 1; l >= 0; --l) {
+    NfLevel &L = g->lv[l], &C = g->lv[l + 1];
+    if (L.vec && fused) {
+      NfDims d = nf_dims(L.nx / 4, L.ny, L.nz);
+      NF_LAUNCH(g, (l == 0 ? NFK_UP1_0 : NFK_VEC_C), k_up1<<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, C.z, C.nx, C.ny, st));
+      if (l == 0 && with_dot) {
+        NF_LAUNCH(g, NFK_UP2_0, k_up2<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, g->st, slot));
+        dot_done = true;
+      } else {
+        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), k_up2<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, st, slot));
+      }
+    } else {
+      NfDims d = nf_dims(L.nx, L.ny, L.nz);
+      NF_LAUNCH(g, (l == 0 ? NFK_PROLONG0 : NFK_PROLONG_C), k_prolong_add<<<d.grid, d.block, 0, g->stream>>>(L.z, C.z, L.nx, L.ny, L.nz, C.nx, C.ny, st));
+      for (int s = 0; s < g->nu_post; ++s) {
+        const bool dot = with_dot && l == 0 && s == g->nu_post - 1;
+        smooth_half(g, L, 1, false, false, st, slot);
+        smooth_half(g, L, 0, false, dot, st, slot);
+        dot_done = dot_done || dot;
+      }
+    }
+  }
+  if (with_dot && !dot_done) {
+    NfLevel &L = g->lv[0];
+    NF_LAUNCH(g, NFK_MISC, k_dot_rz<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(L.r, L.z, (size_t)L.ncell, &g->st->rz[slot], st));
+  }
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}

@@ -5,46 +5,10 @@
 #include <chrono>
 #include <thread>
 
-#include "nf_internal.cuh"
+#include "nf_stencil.cuh"
 
 #define NF_VEC_BLOCKS (148 * 8)
-#define NF_BOTTOM_MAX_CELLS 4096
 #define NF_LOOKAHEAD 2
-
-// ------------------------------------------------------------------------------------------------------------
-// cell-local helpers
-// ------------------------------------------------------------------------------------------------------------
-struct NfW6 {
-  float xl, xh, yl, yh, zl, zh;
-};
-__device__ __forceinline__ NfW6 nf_load_w6(const float *__restrict__ ax, const float *__restrict__ ay,
-                                           const float *__restrict__ az, int i, int j, int k, int nx, int ny, int pax) {
-  NfW6 w;
-  const size_t rx = ((size_t)k * ny + j) * pax + i;
-  w.xl = __ldg(ax + rx);
-  w.xh = __ldg(ax + rx + 1);
-  const size_t ry = ((size_t)k * (ny + 1) + j) * nx + i;
-  w.yl = __ldg(ay + ry);
-  w.yh = __ldg(ay + ry + nx);
-  const size_t rz = ((size_t)k * ny + j) * nx + i;
-  w.zl = __ldg(az + rz);
-  w.zh = __ldg(az + rz + (size_t)ny * nx);
-  return w;
-}
-// sum over the six neighbours of alpha_f * v_nb with homogeneous ghosts (v = 0 outside the grid)
-__device__ __forceinline__ float nf_nb_sum(const float *__restrict__ v, const NfW6 &w, int i, int j, int k, int nx,
-                                           int ny, int nz) {
-  const size_t id = ((size_t)k * ny + j) * nx + i;
-  const size_t sy = nx, sz = (size_t)nx * ny;
-  float s = 0.0f;
-  if (i > 0) s += w.xl * v[id - 1];
-  if (i + 1 < nx) s += w.xh * v[id + 1];
-  if (j > 0) s += w.yl * v[id - sy];
-  if (j + 1 < ny) s += w.yh * v[id + sy];
-  if (k > 0) s += w.zl * v[id - sz];
-  if (k + 1 < nz) s += w.zh * v[id + sz];
-  return s;
-}
 
 // ------------------------------------------------------------------------------------------------------------
 // a-3  q = A p = c (sum_f alpha_f (p - p_nb)), fused p.q partial sums
@@ -69,6 +33,47 @@ __global__ void __launch_bounds__(256) k_apply_A(const float *__restrict__ p, co
     part = (double)pc * (double)qv;
   }
   if (DOT) nf_block_atomic_add(part, &st->pq[slot]);
+}
+
+// The same operator, 4 cells per thread on float4 rows with the weights taken from the 1-byte cell code
+// (DESIGN.md section 2): 9 B/cell (p, code in; q out) instead of 20.  Needs nx % 4 == 0 and 16-byte aligned p, q.
+template <bool DOT>
+__global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restrict__ p, float *__restrict__ q,
+                                                NfSolveState *st, int slot) {
+  if (DOT && st->done) return;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  float part = 0.0f;
+  if (i0 < L.nx && j < L.ny && k < L.nz) {
+    const int nx = L.nx, ny = L.ny, nz = L.nz;
+    const size_t sy = nx, sz = (size_t)nx * ny;
+    const size_t id = ((size_t)k * ny + j) * nx + i0;
+    float pc[4], yl[4], yh[4], zl[4], zh[4], out[4];
+    nf_unpack4(nf_ld4(p, id, true), pc);
+    nf_unpack4(nf_ld4(p, id - sy, j > 0), yl);
+    nf_unpack4(nf_ld4(p, id + sy, j + 1 < ny), yh);
+    nf_unpack4(nf_ld4(p, id - sz, k > 0), zl);
+    nf_unpack4(nf_ld4(p, id + sz, k + 1 < nz), zh);
+    const float xl = nf_ld1(p, id - 1, i0 > 0), xh = nf_ld1(p, id + 4, i0 + 4 < nx);
+    const unsigned c4 = nf_ldc4(L.code, id, true);
+    const bool open4 = (c4 & 0x7f7f7f7fu) == 0x3f3f3f3fu;  // all four cells: six open faces
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      const float l = t > 0 ? pc[t - 1] : xl, h = t < 3 ? pc[t + 1] : xh;
+      if (open4) {
+        const float s = ((l + h) + (yl[t] + yh[t])) + (zl[t] + zh[t]);
+        out[t] = L.c * (6.0f * pc[t] - s);
+      } else {
+        const NfW6 w = nf_code_w6(L, nf_code_at(c4, t), i0 + t, j, k);
+        const float s = ((w.xl * l + w.xh * h) + (w.yl * yl[t] + w.yh * yh[t])) + (w.zl * zl[t] + w.zh * zh[t]);
+        out[t] = L.c * (nf_w6_sum(w) * pc[t] - s);
+      }
+      part += pc[t] * out[t];
+    }
+    *reinterpret_cast<float4 *>(q + id) = make_float4(out[0], out[1], out[2], out[3]);
+  }
+  if (DOT) nf_block_atomic_add((double)part, &st->pq[slot]);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -245,136 +250,6 @@ __global__ void k_start_state(NfSolveState *st) {
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// a-5  V-cycle pieces
-// ------------------------------------------------------------------------------------------------------------
-// Red-black Gauss-Seidel half sweep on the cells with (i+j+k) % 2 == color.  One thread per x-pair of cells.
-// ZERO: the initial guess is zero (neighbours are not read).  DOT: also accumulate r.z over BOTH cells of the pair
-// (used on the last half sweep of the V-cycle on level 0, where z is final).
-template <bool ZERO, bool DOT>
-__global__ void __launch_bounds__(256) k_rbgs(float *__restrict__ z, const float *__restrict__ r,
-                                              const float *__restrict__ ax, const float *__restrict__ ay,
-                                              const float *__restrict__ az, float c, int nx, int ny, int nz, int pax,
-                                              int color, NfSolveState *st, int slot) {
-  if (st && st->done) return;
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
-  double part = 0.0;
-  if (j < ny && k < nz) {
-    const int par = (j + k + color) & 1;
-    const int i = 2 * t + par;
-    if (i < nx) {
-      const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
-      const size_t id = ((size_t)k * ny + j) * nx + i;
-      const float d = ((w.xl + w.xh) + (w.yl + w.yh)) + (w.zl + w.zh);
-      float zn = 0.0f;
-      const float rv = r[id];
-      if (d > 0.0f) {
-        float s = rv;
-        if (!ZERO) s += c * nf_nb_sum(z, w, i, j, k, nx, ny, nz);
-        zn = s / (c * d);
-      }
-      z[id] = zn;
-      if (DOT) part = (double)rv * (double)zn;
-    }
-    if (DOT) {
-      const int io = 2 * t + 1 - par;
-      if (io < nx) {
-        const size_t ido = ((size_t)k * ny + j) * nx + io;
-        part += (double)r[ido] * (double)z[ido];
-      }
-    }
-  }
-  if (DOT) nf_block_atomic_add(part, &st->rz[slot]);
-}
-
-// r_c = (1/8) sum over the 8 children of (r_f - A_f z_f)   (R = P^T / 8, P = piecewise-constant prolongation)
-__global__ void __launch_bounds__(256) k_residual_restrict(const float *__restrict__ z, const float *__restrict__ r,
-                                                           const float *__restrict__ ax, const float *__restrict__ ay,
-                                                           const float *__restrict__ az, float c, int nx, int ny,
-                                                           int nz, int pax, float *__restrict__ rc, int cnx, int cny,
-                                                           int cnz, const NfSolveState *st) {
-  if (st && st->done) return;
-  const int I = blockIdx.x * blockDim.x + threadIdx.x;
-  const int J = blockIdx.y * blockDim.y + threadIdx.y;
-  const int K = blockIdx.z * blockDim.z + threadIdx.z;
-  if (I >= cnx || J >= cny || K >= cnz) return;
-  float acc = 0.0f;
-#pragma unroll
-  for (int dk = 0; dk < 2; ++dk)
-#pragma unroll
-    for (int dj = 0; dj < 2; ++dj)
-#pragma unroll
-      for (int di = 0; di < 2; ++di) {
-        const int i = 2 * I + di, j = 2 * J + dj, k = 2 * K + dk;
-        const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
-        const size_t id = ((size_t)k * ny + j) * nx + i;
-        const float d = ((w.xl + w.xh) + (w.yl + w.yh)) + (w.zl + w.zh);
-        acc += r[id] - c * (d * z[id] - nf_nb_sum(z, w, i, j, k, nx, ny, nz));
-      }
-  rc[((size_t)K * cny + J) * cnx + I] = 0.125f * acc;
-}
-
-// z_f += z_c[parent]   (piecewise-constant prolongation)
-__global__ void __launch_bounds__(256) k_prolong_add(float *__restrict__ z, const float *__restrict__ zc, int nx,
-                                                     int ny, int nz, int cnx, int cny, const NfSolveState *st) {
-  if (st && st->done) return;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
-  if (i >= nx || j >= ny || k >= nz) return;
-  z[((size_t)k * ny + j) * nx + i] += __ldg(zc + ((size_t)(k >> 1) * cny + (j >> 1)) * cnx + (i >> 1));
-}
-
-// Coarsest level in ONE CTA, all data in shared memory: `sweeps` red->black sweeps from a zero guess followed by
-// `sweeps` black->red sweeps (a symmetric positive semi-definite approximate inverse).
-// smem layout: z[n], r[n], idiag[n], wgt[6][n]
-__global__ void __launch_bounds__(256) k_bottom(float *__restrict__ zg, const float *__restrict__ rg,
-                                                const float *__restrict__ ax, const float *__restrict__ ay,
-                                                const float *__restrict__ az, float c, int nx, int ny, int nz, int pax,
-                                                int sweeps, const NfSolveState *st) {
-  if (st && st->done) return;
-  extern __shared__ float sm[];
-  const int n = nx * ny * nz;
-  float *z = sm, *r = sm + n, *idg = sm + 2 * n, *wg = sm + 3 * n;
-  const int sy = nx, sz = nx * ny;
-  for (int id = threadIdx.x; id < n; id += blockDim.x) {
-    const int i = id % nx, j = (id / nx) % ny, k = id / sz;
-    const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
-    const float d = ((w.xl + w.xh) + (w.yl + w.yh)) + (w.zl + w.zh);
-    idg[id] = d > 0.0f ? 1.0f / (c * d) : 0.0f;
-    wg[0 * n + id] = i > 0 ? c * w.xl : 0.0f;
-    wg[1 * n + id] = i + 1 < nx ? c * w.xh : 0.0f;
-    wg[2 * n + id] = j > 0 ? c * w.yl : 0.0f;
-    wg[3 * n + id] = j + 1 < ny ? c * w.yh : 0.0f;
-    wg[4 * n + id] = k > 0 ? c * w.zl : 0.0f;
-    wg[5 * n + id] = k + 1 < nz ? c * w.zh : 0.0f;
-    r[id] = rg[id];
-    z[id] = 0.0f;
-  }
-  __syncthreads();
-  for (int s = 0; s < 4 * sweeps; ++s) {
-    // half sweeps: forward part = red, black, red, black ...; backward part = black, red, ...
-    const int half = s & 1;
-    const int color = (s < 2 * sweeps) ? half : 1 - half;
-    for (int id = threadIdx.x; id < n; id += blockDim.x) {
-      const int i = id % nx, j = (id / nx) % ny, k = id / sz;
-      if (((i + j + k) & 1) != color) continue;
-      float a = r[id];
-      a += wg[0 * n + id] * z[i > 0 ? id - 1 : id];
-      a += wg[1 * n + id] * z[i + 1 < nx ? id + 1 : id];
-      a += wg[2 * n + id] * z[j > 0 ? id - sy : id];
-      a += wg[3 * n + id] * z[j + 1 < ny ? id + sy : id];
-      a += wg[4 * n + id] * z[k > 0 ? id - sz : id];
-      a += wg[5 * n + id] * z[k + 1 < nz ? id + sz : id];
-      z[id] = a * idg[id];
-    }
-    __syncthreads();
-  }
-  for (int id = threadIdx.x; id < n; id += blockDim.x) zg[id] = z[id];
-}
-
-// ------------------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------------------
 static inline int vec_ok(const void *a, const void *b, const void *c, const void *d, size_t n) {
@@ -382,84 +257,32 @@ static inline int vec_ok(const void *a, const void *b, const void *c, const void
   return ((m & 15) == 0 && (n & 3) == 0) ? 1 : 0;
 }
 
-int nf_solver_init(nf_grid *g) {
-  NF_CUDA(g, cudaFuncSetAttribute(k_bottom, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  9 * NF_BOTTOM_MAX_CELLS * (int)sizeof(float)));
-  return NF_OK;
+int nf_solver_init(nf_grid *g) { return nf_mg_init(g); }
+
+static inline bool apply_vec_ok(const NfLevel &L, const float *p, const float *q) {
+  return (L.nx & 3) == 0 && vec_ok(p, q, p, q, 4);
+}
+
+// q = A p on level 0; dot: accumulate p.q into st->pq[slot] and honour st->done
+static void launch_apply(nf_grid *g, const float *p, float *q, bool dot, int slot) {
+  NfLevel &L = g->lv[0];
+  if (!g->force_generic && apply_vec_ok(L, p, q)) {
+    NfDims d = nf_dims(L.nx / 4, L.ny, L.nz);
+    if (dot)
+      NF_LAUNCH(g, NFK_APPLY, k_apply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, g->st, slot));
+    else
+      NF_LAUNCH(g, NFK_APPLY, k_apply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, nullptr, 0));
+  } else {
+    NfDims d = nf_dims(L.nx, L.ny, L.nz);
+    if (dot)
+      NF_LAUNCH(g, NFK_APPLY, k_apply_A<true><<<d.grid, d.block, 0, g->stream>>>(p, L.ax, L.ay, L.az, q, L.c, L.nx, L.ny, L.nz, L.pax, g->st, slot));
+    else
+      NF_LAUNCH(g, NFK_APPLY, k_apply_A<false><<<d.grid, d.block, 0, g->stream>>>(p, L.ax, L.ay, L.az, q, L.c, L.nx, L.ny, L.nz, L.pax, nullptr, 0));
+  }
 }
 
 int nf_apply_A_impl(nf_grid *g, const float *p, float *q) {
-  NfLevel &L = g->lv[0];
-  NfDims d = nf_dims(L.nx, L.ny, L.nz);
-  NF_LAUNCH(g, NFK_APPLY, k_apply_A<false><<<d.grid, d.block, 0, g->stream>>>(p, L.ax, L.ay, L.az, q, L.c, L.nx, L.ny, L.nz, L.pax, nullptr, 0));
-  NF_CUDA(g, cudaGetLastError());
-  return NF_OK;
-}
-
-static void smooth_half(nf_grid *g, NfLevel &L, int color, bool zero, bool dot, NfSolveState *st, int slot) {
-  NfDims d = nf_dims((L.nx + 1) / 2, L.ny, L.nz);
-  const bool lvl0 = (&L == &g->lv[0]);
-  if (zero)
-    NF_LAUNCH(g, (lvl0 ? NFK_RBGS0 : NFK_RBGS_C), k_rbgs<true, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                           color, st, slot));
-  else if (dot)
-    NF_LAUNCH(g, (lvl0 ? NFK_RBGS0 : NFK_RBGS_C), k_rbgs<false, true><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                           color, st, slot));
-  else
-    NF_LAUNCH(g, (lvl0 ? NFK_RBGS0 : NFK_RBGS_C), k_rbgs<false, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                            color, st, slot));
-}
-
-static int bottom_sweeps(const NfLevel &L) {
-  int m = L.nx > L.ny ? L.nx : L.ny;
-  m = m > L.nz ? m : L.nz;
-  return 4 * m;
-}
-
-// z = M^{-1} r on level 0 (lv[0].r -> lv[0].z).  st may be null (no early exit, no dot).
-int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
-  NfSolveState *st = with_dot ? g->st : nullptr;
-  const int nl = g->nlev;
-  for (int l = 0; l + 1 < nl; ++l) {
-    NfLevel &L = g->lv[l], &C = g->lv[l + 1];
-    for (int s = 0; s < g->nu_pre; ++s) {
-      smooth_half(g, L, 0, s == 0, false, st, slot);
-      smooth_half(g, L, 1, false, false, st, slot);
-    }
-    NfDims d = nf_dims(C.nx, C.ny, C.nz);
-    NF_LAUNCH(g, (l == 0 ? NFK_RESTRICT0 : NFK_RESTRICT_C), k_residual_restrict<<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                           C.r, C.nx, C.ny, C.nz, st));
-  }
-  {
-    NfLevel &B = g->lv[nl - 1];
-    if (B.ncell <= NF_BOTTOM_MAX_CELLS) {
-      const size_t smem = (size_t)9 * B.ncell * sizeof(float);
-      NF_LAUNCH(g, NFK_BOTTOM, k_bottom<<<1, 256, smem, g->stream>>>(B.z, B.r, B.ax, B.ay, B.az, B.c, B.nx, B.ny, B.nz, B.pax, bottom_sweeps(B),
-                                            st));
-    } else {  // coarsest level too large for one CTA (odd sizes): a few symmetric sweeps in global memory
-      const int nb = 4;
-      for (int s = 0; s < nb; ++s) {
-        smooth_half(g, B, 0, s == 0, false, st, slot);
-        smooth_half(g, B, 1, false, false, st, slot);
-      }
-      for (int s = 0; s < nb; ++s) {
-        smooth_half(g, B, 1, false, false, st, slot);
-        smooth_half(g, B, 0, false, false, st, slot);
-      }
-    }
-    if (nl == 1 && with_dot) {
-      NF_LAUNCH(g, NFK_MISC, k_dot<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(B.r, B.z, (size_t)B.ncell, &g->st->rz[slot], st));
-    }
-  }
-  for (int l = nl - 2; l >= 0; --l) {
-    NfLevel &L = g->lv[l], &C = g->lv[l + 1];
-    NfDims d = nf_dims(L.nx, L.ny, L.nz);
-    NF_LAUNCH(g, (l == 0 ? NFK_PROLONG0 : NFK_PROLONG_C), k_prolong_add<<<d.grid, d.block, 0, g->stream>>>(L.z, C.z, L.nx, L.ny, L.nz, C.nx, C.ny, st));
-    for (int s = 0; s < g->nu_post; ++s) {
-      smooth_half(g, L, 1, false, false, st, slot);
-      smooth_half(g, L, 0, false, with_dot && l == 0 && s == g->nu_post - 1, st, slot);
-    }
-  }
+  launch_apply(g, p, q, false, 0);
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -523,8 +346,7 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
   if (maxit < 1) maxit = 1;
   for (it = 0; it < maxit && !done; ++it) {
     const int slot = it & 1;
-    NF_LAUNCH(g, NFK_APPLY, k_apply_A<true><<<dc.grid, dc.block, 0, g->stream>>>(g->p, L.ax, L.ay, L.az, g->q, L.c, L.nx, L.ny, L.nz, L.pax,
-                                                         g->st, slot));
+    launch_apply(g, g->p, g->q, true, slot);
     NF_LAUNCH(g, NFK_UPDATE, k_cg_update<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, g->p, g->q, n, v4, g->st, slot));
     NF_LAUNCH(g, NFK_CHECK, k_cg_check<<<1, 32, 0, g->stream>>>(g->st, slot, &g->hst_dev[it & (NF_RING - 1)], it + 1));
     if (it + 1 < maxit) {

@@ -260,28 +260,62 @@ __global__ void __launch_bounds__(256) k_coarsen_weights(const float *__restrict
   }
 }
 
-// counts[0] += active cells (sum of six weights > 0); counts[1] += open faces on Dirichlet domain faces (R12).
-__global__ void __launch_bounds__(256) k_classify(const float *__restrict__ ax, const float *__restrict__ ay,
-                                                  const float *__restrict__ az, int nx, int ny, int nz, int pax,
-                                                  NfBc6 bc, double *__restrict__ counts) {
+// Cell codes of one level from its fp32 weights: bits 0..5 = face is fully open, bit 6 = the
+// cell has a fractional face.  With counts != nullptr (level 0) also: counts[0] += active cells (sum of six
+// weights > 0); counts[1] += open faces on Dirichlet domain faces (R12).
+__global__ void __launch_bounds__(256) k_encode(const float *__restrict__ ax, const float *__restrict__ ay,
+                                                const float *__restrict__ az, uint8_t *__restrict__ code, int nx,
+                                                int ny, int nz, int pax, NfBc6 bc, double *__restrict__ counts) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z * blockDim.z + threadIdx.z;
   double act = 0.0, dir = 0.0;
   if (i < nx && j < ny && k < nz) {
-    const float xl = ax[((size_t)k * ny + j) * pax + i], xh = ax[((size_t)k * ny + j) * pax + i + 1];
-    const float yl = ay[((size_t)k * (ny + 1) + j) * nx + i], yh = ay[((size_t)k * (ny + 1) + j + 1) * nx + i];
-    const float zl = az[((size_t)k * ny + j) * nx + i], zh = az[((size_t)(k + 1) * ny + j) * nx + i];
-    if (xl + xh + yl + yh + zl + zh > 0.0f) act = 1.0;
-    if (i == 0 && bc.t[0] == NF_BC_DIRICHLET && xl > 0.0f) dir += 1.0;
-    if (i == nx - 1 && bc.t[1] == NF_BC_DIRICHLET && xh > 0.0f) dir += 1.0;
-    if (j == 0 && bc.t[2] == NF_BC_DIRICHLET && yl > 0.0f) dir += 1.0;
-    if (j == ny - 1 && bc.t[3] == NF_BC_DIRICHLET && yh > 0.0f) dir += 1.0;
-    if (k == 0 && bc.t[4] == NF_BC_DIRICHLET && zl > 0.0f) dir += 1.0;
-    if (k == nz - 1 && bc.t[5] == NF_BC_DIRICHLET && zh > 0.0f) dir += 1.0;
+    float w[6];
+    w[0] = ax[((size_t)k * ny + j) * pax + i];
+    w[1] = ax[((size_t)k * ny + j) * pax + i + 1];
+    w[2] = ay[((size_t)k * (ny + 1) + j) * nx + i];
+    w[3] = ay[((size_t)k * (ny + 1) + j + 1) * nx + i];
+    w[4] = az[((size_t)k * ny + j) * nx + i];
+    w[5] = az[((size_t)(k + 1) * ny + j) * nx + i];
+    unsigned c = 0;
+    bool mixed = false;
+#pragma unroll
+    for (int f = 0; f < 6; ++f) {
+      if (w[f] == 1.0f) c |= 1u << f;
+      else if (w[f] != 0.0f) mixed = true;
+    }
+    if (mixed) c |= NF_CODE_MIXED;
+    code[((size_t)k * ny + j) * nx + i] = (uint8_t)c;
+    if (counts) {
+      if (w[0] + w[1] + w[2] + w[3] + w[4] + w[5] > 0.0f) act = 1.0;
+      if (i == 0 && bc.t[0] == NF_BC_DIRICHLET && w[0] > 0.0f) dir += 1.0;
+      if (i == nx - 1 && bc.t[1] == NF_BC_DIRICHLET && w[1] > 0.0f) dir += 1.0;
+      if (j == 0 && bc.t[2] == NF_BC_DIRICHLET && w[2] > 0.0f) dir += 1.0;
+      if (j == ny - 1 && bc.t[3] == NF_BC_DIRICHLET && w[3] > 0.0f) dir += 1.0;
+      if (k == 0 && bc.t[4] == NF_BC_DIRICHLET && w[4] > 0.0f) dir += 1.0;
+      if (k == nz - 1 && bc.t[5] == NF_BC_DIRICHLET && w[5] > 0.0f) dir += 1.0;
+    }
   }
-  nf_block_atomic_add(act, counts + 0);
-  nf_block_atomic_add(dir, counts + 1);
+  if (counts) {
+    nf_block_atomic_add(act, counts + 0);
+    nf_block_atomic_add(dir, counts + 1);
+  }
+}
+
+// Second pass of the encoding: set NF_CODE_DEEP (in place: the bit is not an input of this kernel).
+__global__ void __launch_bounds__(256) k_encode_deep(uint8_t *code, int nx, int ny, int nz) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i >= nx || j >= ny || k >= nz) return;
+  const size_t id = ((size_t)k * ny + j) * nx + i, sy = nx, sz = (size_t)nx * ny;
+  const unsigned full = 63u, m = 127u;
+  bool deep = (code[id] & m) == full;
+  deep = deep && (i == 0 || (code[id - 1] & m) == full) && (i + 1 == nx || (code[id + 1] & m) == full);
+  deep = deep && (j == 0 || (code[id - sy] & m) == full) && (j + 1 == ny || (code[id + sy] & m) == full);
+  deep = deep && (k == 0 || (code[id - sz] & m) == full) && (k + 1 == nz || (code[id + sz] & m) == full);
+  if (deep) code[id] = (uint8_t)(full | NF_CODE_DEEP);
 }
 
 // Copy a MAC face array (or zero it when src == nullptr) and put closed walls at rest (R19).
@@ -343,12 +377,19 @@ int nf_build_hierarchy(nf_grid *g) {
     NF_LAUNCH(g, NFK_COARSEN, k_coarsen_weights<<<d.grid, d.block, 0, g->stream>>>(F.ax, F.ay, F.az, C.ax, C.ay, C.az, F.nx, F.ny, F.nz, F.pax,
                                                          C.nx, C.ny, C.nz, C.pax));
   }
-  NfLevel &L = g->lv[0];
   double *cnt = g->d_counts;
   NF_CUDA(g, cudaMemsetAsync(cnt, 0, 2 * sizeof(double), g->stream));
-  NfDims d = nf_dims(g->nx, g->ny, g->nz);
-  NF_LAUNCH(g, NFK_CLASSIFY, k_classify<<<d.grid, d.block, 0, g->stream>>>(L.ax, L.ay, L.az, g->nx, g->ny, g->nz, L.pax, bc6(g), cnt));
+  for (int l = 0; l < g->nlev; ++l) {
+    NfLevel &L = g->lv[l];
+    NfDims d = nf_dims(L.nx, L.ny, L.nz);
+    NF_LAUNCH(g, NFK_CLASSIFY, k_encode<<<d.grid, d.block, 0, g->stream>>>(L.ax, L.ay, L.az, L.code, L.nx, L.ny, L.nz, L.pax, bc6(g), l == 0 ? cnt : nullptr));
+    if (L.vec) NF_LAUNCH(g, NFK_CLASSIFY, k_encode_deep<<<d.grid, d.block, 0, g->stream>>>(L.code, L.nx, L.ny, L.nz));
+  }
   NF_CUDA(g, cudaGetLastError());
+  {
+    int rc = nf_mg_pack_tail(g);
+    if (rc != NF_OK) return rc;
+  }
   NF_CUDA(g, cudaMemcpyAsync(g->h_counts, cnt, 2 * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
   NF_CUDA(g, cudaStreamSynchronize(g->stream));
   const double *hc = g->h_counts;

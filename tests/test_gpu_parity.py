@@ -137,7 +137,7 @@ def test_weights_roundtrip_and_wall_zeroing(torch, api):
 # ---------------------------------------------------------------------------------------------------------
 # a-3 operator
 # ---------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("shape", [(32, 32, 32), (20, 18, 14), (5, 3, 2), (1, 1, 7)])
+@pytest.mark.parametrize("shape", [(32, 32, 32), (20, 18, 14), (5, 3, 2), (1, 1, 7), (136, 10, 6), (4, 4, 4)])
 def test_apply_A_matches_oracle(torch, api, shape):
     nx, ny, nz = shape
     rng = np.random.default_rng(3)
@@ -181,7 +181,8 @@ def _solve_case(torch, api, nx, ny, nz, bt, seed, phi=None):
 
 @pytest.mark.parametrize("shape,bt", [((32, 32, 32), (0,) * 6), ((32, 32, 32), (0, 1, 0, 0, 0, 0)),
                                        ((40, 36, 28), (1, 0, 0, 0, 0, 1)), ((20, 18, 14), (0,) * 6),
-                                       ((6, 5, 4), (0,) * 6), ((64, 64, 64), (0,) * 6)])
+                                       ((6, 5, 4), (0,) * 6), ((64, 64, 64), (0,) * 6), ((16, 16, 16), (0,) * 6),
+                                       ((96, 64, 32), (0, 0, 0, 0, 1, 0)), ((50, 30, 22), (0,) * 6)])
 def test_solve_matches_oracle(torch, api, shape, bt):
     rc, info, p, ref, a64, b, c, bc = _solve_case(torch, api, *shape, bt, seed=21)
     assert rc == 0, info
@@ -210,9 +211,53 @@ def test_solve_zero_rhs_and_maxit(torch, api):
     g.close()
 
 
-def test_vcycle_is_symmetric_and_positive(torch, api):
+@pytest.mark.parametrize("shape", [(32, 32, 32), (24, 20, 16), (64, 48, 32), (136, 12, 8)])
+def test_apply_A_code_path_equals_weight_path(torch, api, shape):
+    """The 1-byte cell-code kernels compute the same operator as the fp32-weight kernels:
+    pure cells multiply by exactly 0 / 1, mixed cells read the same fp32 weights (difference: summation order)."""
+    nx, ny, nz = shape
+    phi = blob_sdf(nx, ny, nz, 13)
+    g = make_grid(api, nx, ny, nz, 1.0 / nx, dt_over_rho=0.7, bc_types=(1, 0, 0, 1, 0, 0))
+    g.set_solid(dev(torch, phi))
+    p = torch.randn(g.shape_p, device="cuda")
+    q1, q2 = torch.empty_like(p), torch.empty_like(p)
+    g.apply_A(p, q1)
+    g.set_solver_options(1, 1, 2)  # force the generic kernels
+    g.apply_A(p, q2)
+    assert rel(host(q1), host(q2)) < 1e-6
+    ref = orc.apply_A(host(p), [host(a) for a in g.get_weights()], 0.7 * nx)
+    assert rel(host(q1), ref) < 2e-6
+    g.close()
+
+
+@pytest.mark.parametrize("shape,bt", [((32, 32, 32), (0,) * 6), ((24, 20, 16), (0, 1, 0, 0, 0, 0)),
+                                       ((64, 64, 64), (1, 1, 0, 0, 0, 0)), ((128, 64, 32), (0,) * 6),
+                                       ((40, 36, 28), (0, 0, 1, 0, 0, 0))])
+def test_vcycle_fused_equals_generic(torch, api, shape, bt):
+    """The 4-launch-per-level V-cycle (k_down1/k_down2/k_up1/k_up2: red values recomputed on the fly, residual of
+    the red children only, prolongation folded into the black half sweep) is the same operator, in exact
+    arithmetic, as the one-colour-per-launch V-cycle on fp32 weights."""
+    nx, ny, nz = shape
+    phi = blob_sdf(nx, ny, nz, 9)
+    g = make_grid(api, nx, ny, nz, 1.0 / nx, dt_over_rho=0.5, bc_types=bt)
+    g.set_solid(dev(torch, phi))
+    au, av, aw = g.get_weights()
+    act = (au[:, :, :-1] + au[:, :, 1:] + av[:, :-1] + av[:, 1:] + aw[:-1] + aw[1:]) > 0
+    r = torch.randn(g.shape_p, device="cuda") * act
+    z1, z2 = torch.empty_like(r), torch.empty_like(r)
+    g.vcycle(r, z1)
+    g.set_solver_options(1, 1, 2)
+    g.vcycle(r, z2)
+    assert float(z2.abs().max()) > 0
+    assert rel(host(z1), host(z2)) < 2e-5
+    assert float((z1 * (~act)).abs().max()) == 0.0  # inactive cells stay 0
+    g.close()
+
+
+@pytest.mark.parametrize("shape", [(24, 20, 16), (64, 64, 64), (16, 16, 16)])
+def test_vcycle_is_symmetric_and_positive(torch, api, shape):
     """M^{-1} must be symmetric positive (semi-)definite for PCG: <M r1, r2> = <r1, M r2>, <M r, r> > 0."""
-    nx, ny, nz = 24, 20, 16
+    nx, ny, nz = shape
     phi = blob_sdf(nx, ny, nz, 8)
     g = make_grid(api, nx, ny, nz, 1.0 / nx, bc_types=(0, 1, 0, 0, 0, 0))
     g.set_solid(dev(torch, phi))
