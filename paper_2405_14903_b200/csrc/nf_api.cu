@@ -25,10 +25,10 @@ static cudaError_t dalloc(T **p, size_t n) {
 static void free_all(nf_grid *g) {
   for (int l = 0; l < NF_MAX_LEVELS; ++l) {
     NfLevel &L = g->lv[l];
-    cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.code); cudaFree(L.z); cudaFree(L.r);
+    cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.code); cudaFree(L.idg); cudaFree(L.z); cudaFree(L.r);
   }
   cudaFree(g->us); cudaFree(g->vs); cudaFree(g->ws); cudaFree(g->sdf);
-  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->xd); cudaFree(g->tailpack);
+  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->tailpack);
   cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
   cudaFree(g->st); cudaFree(g->d_counts);
   if (g->hst) cudaFreeHost((void *)g->hst);
@@ -71,6 +71,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     ok = ok && dalloc(&L.ay, (size_t)lz * (ly + 1) * lx) == cudaSuccess;
     ok = ok && dalloc(&L.az, (size_t)(lz + 1) * ly * lx) == cudaSuccess;
     ok = ok && dalloc(&L.code, (size_t)L.ncell + 16) == cudaSuccess;
+    ok = ok && dalloc(&L.idg, (size_t)L.ncell) == cudaSuccess;
     ok = ok && dalloc(&L.z, (size_t)L.ncell) == cudaSuccess;
     ok = ok && dalloc(&L.r, (size_t)L.ncell) == cudaSuccess;
     if (ok) ok = cudaMemset(L.ax, 0, (size_t)lz * ly * L.pax * sizeof(float)) == cudaSuccess;
@@ -92,7 +93,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   ok = ok && dalloc(&g->us, nf_nu(g)) == cudaSuccess && dalloc(&g->vs, nf_nv(g)) == cudaSuccess &&
        dalloc(&g->ws, nf_nw(g)) == cudaSuccess && dalloc(&g->sdf, nf_nn(g)) == cudaSuccess;
   ok = ok && dalloc(&g->p, nc) == cudaSuccess && dalloc(&g->q, nc) == cudaSuccess &&
-       dalloc(&g->xtmp, nc) == cudaSuccess && dalloc(&g->xd, nc) == cudaSuccess;
+       dalloc(&g->xtmp, nc) == cudaSuccess && dalloc(&g->p2, nc) == cudaSuccess;
   ok = ok && dalloc(&g->fu, nf_nu(g)) == cudaSuccess && dalloc(&g->fv, nf_nv(g)) == cudaSuccess &&
        dalloc(&g->fw, nf_nw(g)) == cudaSuccess;
   ok = ok && dalloc(&g->st, 1) == cudaSuccess && dalloc(&g->d_counts, 2) == cudaSuccess;
@@ -132,7 +133,10 @@ extern "C" int nf_set_dt_rho(nf_grid *g, float dt_over_rho) {
   if (!(dt_over_rho > 0.0f)) return NF_ERR_INVALID;
   g->dt_over_rho = dt_over_rho;
   float c = dt_over_rho / g->dx;
-  for (int l = 0; l < g->nlev; ++l) { g->lv[l].c = c; c *= 0.25f; }
+  bool changed = false;
+  for (int l = 0; l < g->nlev; ++l) { changed = changed || g->lv[l].c != c; g->lv[l].c = c; c *= 0.25f; }
+  // the inverse diagonals and the packed tail operator carry c: rebuild them from the current weights
+  if (changed && g->weights_set) return nf_build_hierarchy(g);
   return NF_OK;
 }
 

@@ -32,6 +32,7 @@ struct NfLevel {
   float c;  // c_l = (dt_over_rho/dx) / 4^l  (rediscretised operator on spacing 2^l dx)
   float *ax, *ay, *az;
   uint8_t *code;
+  float *idg;    // 1 / (c_l * sum of the six weights), 0 on inactive cells (written with the codes)
   float *z, *r;  // level 0: CG vectors z and r; level > 0: coarse correction and restricted residual
   int vec;       // 1: nx % 4 == 0 and a coarser level exists -> the float4 / code kernels run on this level
 };
@@ -40,25 +41,31 @@ struct NfLevel {
 struct NfLvK {
   const float *ax, *ay, *az;
   const uint8_t *code;
+  const float *idg;
   float c, ic;
   int nx, ny, nz, pax;
 };
 static inline NfLvK nf_lvk(const NfLevel &L) {
   NfLvK K;
-  K.ax = L.ax; K.ay = L.ay; K.az = L.az; K.code = L.code;
+  K.ax = L.ax; K.ay = L.ay; K.az = L.az; K.code = L.code; K.idg = L.idg;
   K.c = L.c; K.ic = 1.0f / L.c; K.nx = L.nx; K.ny = L.ny; K.nz = L.nz; K.pax = L.pax;
   return K;
 }
 
 // Device-resident PCG scalars.  Slots [2] alternate with the iteration parity so that no kernel has to
-// reset a value another kernel of the same iteration still reads.
-struct NfSolveState {
-  double pq[2], rr[2], rz[2];
+// reset a value another kernel of the same iteration still reads.  The control words every CTA reads on entry
+// (done) live in their own 128-byte line, and each accumulator pair in its own line, so that the fp64 atomics of
+// the CTAs that finish do not queue in front of the flag reads of the CTAs that start.
+struct alignas(128) NfSolveState {
+  int iter, maxit, done, converged;
+  unsigned ticket;  // CTAs of k_cg_update that have finished (the last one runs the convergence check)
   double bb;    // ||b||^2 after masking / mean removal
-  double sum;   // scratch: sum over active cells
   double tol2;  // tol^2
   double relres;  // sqrt(rr/bb) at the last executed iteration
-  int iter, maxit, done, converged;
+  alignas(128) double pq[2];
+  alignas(128) double rr[2];
+  alignas(128) double rz[2];
+  alignas(128) double sum;   // scratch: sum over active cells
 };
 
 struct NfHostStatus {  // written by the device into mapped pinned memory
@@ -84,6 +91,7 @@ struct nf_grid {
   float bc_val[6];
   cudaStream_t stream;
   int nlev;
+  int coarse_ctas;  // > 0: CTAs of the cooperative coarse kernel k_vcoarse (nf_mg.cu); 0 = per-level launches
   int tail;  // first level of the shared-memory tail of the V-cycle (levels tail .. nlev-1 run in one CTA); nlev if none
   NfLevel lv[NF_MAX_LEVELS];
   bool weights_set, have_sdf, have_us;
@@ -94,9 +102,8 @@ struct nf_grid {
   // solid velocity (MAC layout, closed walls at rest) and the last SDF
   float *us, *vs, *ws, *sdf;
   // CG vectors on level 0 (r and z live in lv[0])
-  float *p, *q, *xtmp;
+  float *p, *p2, *q, *xtmp;  // p / p2: the search direction ping-pongs between two buffers (k_papply4)
   float *tailpack;  // 8 floats per cell of the tail levels (nf_mg.cu)
-  double *xd;  // fp64 solution accumulator (refine mode)
   // scratch face arrays (advection copy / adjoint staging)
   float *fu, *fv, *fw;
   NfSolveState *st;      // device
@@ -161,6 +168,23 @@ static inline NfDims nf_dims(int tx, int ty, int tz) {
   NfDims d;
   d.block = dim3(bx, by, bz);
   d.grid = dim3((tx + bx - 1) / bx, (ty + by - 1) / by, (tz + bz - 1) / bz);
+  return d;
+}
+
+// Launch geometry of the 4-cells-per-thread ("vec") stencil kernels: thread lattice (nx/4, rows_y), CTAs of up to
+// 64 x 4 threads, and every CTA marches through `kch` consecutive z-planes (blockIdx.z = chunk): 8x fewer CTAs (and
+// reduction atomics) than one plane per CTA, and the z-neighbour rows of one plane are the L1-resident centre rows
+// of the next.
+#define NF_KCH_MG 4  // planes per CTA: V-cycle kernels (measured in situ at 256^3: 1 -> 4 saves 10-20 % per kernel)
+#define NF_KCH_AP 8  // planes per CTA: A-apply (z-neighbour rows rotate through registers)
+static inline NfDims nf_vdims(int tx, int ty, int tz, int kch) {
+  int bx = 1;
+  while (bx < tx && bx < 64) bx <<= 1;  // whole 256-cell rows per CTA: contiguous DRAM segments beat square tiles
+  int by = 1;
+  while (by < ty && bx * by < 256) by <<= 1;
+  NfDims d;
+  d.block = dim3(bx, by, 1);
+  d.grid = dim3((tx + bx - 1) / bx, (ty + by - 1) / by, (tz + kch - 1) / kch);
   return d;
 }
 

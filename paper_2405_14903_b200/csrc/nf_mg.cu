@@ -14,7 +14,11 @@
 //       k_up2    red half sweep (+ r.z on level 0)
 //   * generic kernels (any extents): one colour per launch, fp32 weights -- the v1 path, kept for ragged levels.
 //   * k_tail: all levels that fit one CTA's shared memory (<= 5632 cells in total), whole sub-V-cycle in one launch.
+#include <cooperative_groups.h>
+
 #include "nf_stencil.cuh"
+
+namespace cg = cooperative_groups;
 
 #define NF_VEC_BLOCKS (148 * 8)
 #define NF_TAIL_MAX_CELLS 5632  // 10 floats per cell of shared memory: 225,280 B <= 227 KB
@@ -27,7 +31,7 @@ struct NfRow4 {  // one row segment of 4 cells: values and codes, with the idiag
   float v[4];
   unsigned c4;
 };
-__device__ __forceinline__ NfRow4 nf_row(const float *__restrict__ f, const uint8_t *__restrict__ code, size_t id,
+__device__ __forceinline__ NfRow4 nf_row(const float *f, const uint8_t *__restrict__ code, size_t id,
                                          bool ok) {
   NfRow4 R;
   nf_unpack4(nf_ld4(f, id, ok), R.v);
@@ -37,23 +41,23 @@ __device__ __forceinline__ NfRow4 nf_row(const float *__restrict__ f, const uint
 
 // PAR = (i0 + j + k) & 1 = colour of the first of the 4 cells; cell q is red iff ((q + PAR) & 1) == 0.
 template <int PAR>
-__device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *__restrict__ r, float *__restrict__ z,
-                                              int i0, int j, int k) {
+__device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, float *z, int i0, int j, int k) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const size_t sy = nx, sz = (size_t)nx * ny;
   const size_t id = ((size_t)k * ny + j) * nx + i0;
+  // every load of r is issued before the branch on the code (one round trip for the common, deep path)
   const NfRow4 C = nf_row(r, L.code, id, true);
-  float out[4];
+  float out[4], yl[4], yh[4], zl[4], zh[4];
+  nf_unpack4(nf_ld4(r, id - sy, j > 0), yl);
+  nf_unpack4(nf_ld4(r, id + sy, j + 1 < ny), yh);
+  nf_unpack4(nf_ld4(r, id - sz, k > 0), zl);
+  nf_unpack4(nf_ld4(r, id + sz, k + 1 < nz), zh);
+  const float re = PAR ? nf_ld1(r, id - 1, i0 > 0) : nf_ld1(r, id + 4, i0 + 4 < nx);
   if ((C.c4 & 0x80808080u) == 0x80808080u) {
     // all four cells are deep interior (NF_CODE_DEEP): every diagonal involved is 6c, every weight is 1, and no
     // neighbour code is needed
-    float yl[4], yh[4], zl[4], zh[4];
-    nf_unpack4(nf_ld4(r, id - sy, j > 0), yl);
-    nf_unpack4(nf_ld4(r, id + sy, j + 1 < ny), yh);
-    nf_unpack4(nf_ld4(r, id - sz, k > 0), zl);
-    nf_unpack4(nf_ld4(r, id + sz, k + 1 < nz), zh);
     const float g6 = L.ic * (1.0f / 6.0f);
-    const float te = PAR ? nf_ld1(r, id - 1, i0 > 0) : nf_ld1(r, id + 4, i0 + 4 < nx);
+    const float te = re;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       if (((q + PAR) & 1) == 0) {
@@ -67,23 +71,18 @@ __device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *__res
     *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
     return;
   }
-  const NfRow4 Yl = nf_row(r, L.code, id - sy, j > 0), Yh = nf_row(r, L.code, id + sy, j + 1 < ny);
-  const NfRow4 Zl = nf_row(r, L.code, id - sz, k > 0), Zh = nf_row(r, L.code, id + sz, k + 1 < nz);
-  float idg[4], t[4];
+  // general path: the red neighbours' values r/diag from the inverse-diagonal rows (one more round trip, no
+  // dependence on the codes), the six weights of a black cell from its code
+  float gyl[4], gyh[4], gzl[4], gzh[4], idg[4], t[4];
+  nf_unpack4(nf_ld4(L.idg, id - sy, j > 0), gyl);
+  nf_unpack4(nf_ld4(L.idg, id + sy, j + 1 < ny), gyh);
+  nf_unpack4(nf_ld4(L.idg, id - sz, k > 0), gzl);
+  nf_unpack4(nf_ld4(L.idg, id + sz, k + 1 < nz), gzh);
+  nf_unpack4(nf_ld4(L.idg, id, true), idg);
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    idg[q] = nf_code_idiag(L, nf_code_at(C.c4, q), i0 + q, j, k);
-    t[q] = C.v[q] * idg[q];
-  }
+  for (int q = 0; q < 4; ++q) t[q] = C.v[q] * idg[q];
   // the x-neighbour outside the segment that a black cell needs: left of q = 0 (PAR = 1) or right of q = 3 (PAR = 0)
-  float te;
-  if (PAR) {
-    const bool ok = i0 > 0;
-    te = nf_ld1(r, id - 1, ok) * nf_code_idiag(L, nf_ldc1(L.code, id - 1, ok), i0 - 1, j, k);
-  } else {
-    const bool ok = i0 + 4 < nx;
-    te = nf_ld1(r, id + 4, ok) * nf_code_idiag(L, nf_ldc1(L.code, id + 4, ok), i0 + 4, j, k);
-  }
+  const float te = re * (PAR ? nf_ld1(L.idg, id - 1, i0 > 0) : nf_ld1(L.idg, id + 4, i0 + 4 < nx));
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     if (((q + PAR) & 1) == 0) {
@@ -92,37 +91,34 @@ __device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *__res
       const NfW6 w = nf_code_w6(L, nf_code_at(C.c4, q), i0 + q, j, k);
       const float tl = q > 0 ? t[q - 1] : te, th = q < 3 ? t[q + 1] : te;
       float s = w.xl * tl + w.xh * th;
-      s += w.yl * (Yl.v[q] * nf_code_idiag(L, nf_code_at(Yl.c4, q), i0 + q, j - 1, k));
-      s += w.yh * (Yh.v[q] * nf_code_idiag(L, nf_code_at(Yh.c4, q), i0 + q, j + 1, k));
-      s += w.zl * (Zl.v[q] * nf_code_idiag(L, nf_code_at(Zl.c4, q), i0 + q, j, k - 1));
-      s += w.zh * (Zh.v[q] * nf_code_idiag(L, nf_code_at(Zh.c4, q), i0 + q, j, k + 1));
+      s += w.yl * (yl[q] * gyl[q]);
+      s += w.yh * (yh[q] * gyh[q]);
+      s += w.zl * (zl[q] * gzl[q]);
+      s += w.zh * (zh[q] * gzh[q]);
       out[q] = (C.v[q] + L.c * s) * idg[q];
     }
   }
   *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
 }
 
-__global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restrict__ r, float *__restrict__ z,
+__global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restrict__ r, float *__restrict__ z, int kch,
                                                const NfSolveState *st) {
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
-  if (i0 >= L.nx || j >= L.ny || k >= L.nz) return;
-  if ((j + k) & 1)
-    nf_down1_body<1>(L, r, z, i0, j, k);
-  else
-    nf_down1_body<0>(L, r, z, i0, j, k);
+  if (i0 >= L.nx || j >= L.ny) return;
+  const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, L.nz);
+  for (int k = k0; k < k1; ++k) {
+    if ((j + k) & 1)
+      nf_down1_body<1>(L, r, z, i0, j, k);
+    else
+      nf_down1_body<0>(L, r, z, i0, j, k);
+  }
 }
 
 // One thread per pair of coarse cells (I0, I0+1) = fine cells i0..i0+3 of the rows (2J+dj, 2K+dk).
-__global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restrict__ z, float *__restrict__ rc, int cnx,
-                                               int cny, int cnz, const NfSolveState *st) {
-  if (st && st->done) return;
-  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
-  const int J = blockIdx.y * blockDim.y + threadIdx.y;
-  const int K = blockIdx.z * blockDim.z + threadIdx.z;
-  if (i0 >= L.nx || J >= cny || K >= cnz) return;
+__device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, float *rc, int cnx, int cny, int i0,
+                                              int J, int K) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const size_t sy = nx, sz = (size_t)nx * ny;
   const int j0 = 2 * J, k0 = 2 * K;
@@ -170,12 +166,22 @@ __global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restri
   *reinterpret_cast<float2 *>(rc + ((size_t)K * cny + J) * cnx + (i0 >> 1)) = make_float2(f * acc0, f * acc1);
 }
 
+__global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restrict__ z, float *__restrict__ rc, int cnx,
+                                               int cny, int cnz, int kch, const NfSolveState *st) {
+  if (st && st->done) return;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int J = blockIdx.y * blockDim.y + threadIdx.y;
+  if (i0 >= L.nx || J >= cny) return;
+  const int K0 = blockIdx.z * kch, K1 = min(K0 + kch, cnz);
+  for (int K = K0; K < K1; ++K) nf_down2_body(L, z, rc, cnx, cny, i0, J, K);
+}
+
 // z + P z_coarse on a row of 4 fine cells
-__device__ __forceinline__ void nf_row_prolonged(const float *z, const float *__restrict__ zc, size_t id, size_t cid,
-                                                 bool ok, float o[4]) {
+__device__ __forceinline__ void nf_row_prolonged(const float *z, const float *zc, size_t id, size_t cid, bool ok,
+                                                 float o[4]) {
   if (ok) {
     const float4 a = *reinterpret_cast<const float4 *>(z + id);
-    const float2 b = __ldg(reinterpret_cast<const float2 *>(zc + cid));
+    const float2 b = *reinterpret_cast<const float2 *>(zc + cid);
     o[0] = a.x + b.x; o[1] = a.y + b.x; o[2] = a.z + b.y; o[3] = a.w + b.y;
   } else {
     o[0] = o[1] = o[2] = o[3] = 0.0f;
@@ -185,8 +191,8 @@ __device__ __forceinline__ void nf_row_prolonged(const float *z, const float *__
 // Black half sweep on z + P zc (in place: only black cells change; red cells keep the un-prolonged value, which
 // k_up2 overwrites without reading).
 template <int PAR>
-__device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const float *__restrict__ r,
-                                            const float *__restrict__ zc, int cnx, int cny, int i0, int j, int k) {
+__device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const float *r, const float *zc, int cnx,
+                                            int cny, int i0, int j, int k) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const size_t sy = nx, sz = (size_t)nx * ny;
   const size_t id = ((size_t)k * ny + j) * nx + i0;
@@ -195,7 +201,7 @@ __device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const floa
   const float4 zold = *reinterpret_cast<const float4 *>(z + id);
   float zp[4], yl[4], yh[4], zl[4], zh[4], rr[4], out[4];
   {
-    const float2 b = __ldg(reinterpret_cast<const float2 *>(zc + cid));
+    const float2 b = *reinterpret_cast<const float2 *>(zc + cid);
     zp[0] = zold.x + b.x; zp[1] = zold.y + b.x; zp[2] = zold.z + b.y; zp[3] = zold.w + b.y;
   }
   // parent row of j-1 is the same as j's iff j is odd; of j+1 iff j is even (same in z)
@@ -208,14 +214,16 @@ __device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const floa
   float xe;
   if (PAR) {
     const bool ok = i0 > 0;
-    xe = ok ? z[id - 1] + __ldg(zc + cid - 1) : 0.0f;
+    xe = ok ? z[id - 1] + zc[cid - 1] : 0.0f;
   } else {
     const bool ok = i0 + 4 < nx;
-    xe = ok ? z[id + 4] + __ldg(zc + cid + 2) : 0.0f;
+    xe = ok ? z[id + 4] + zc[cid + 2] : 0.0f;
   }
   out[0] = zold.x; out[1] = zold.y; out[2] = zold.z; out[3] = zold.w;
   const bool open4 = (c4 & 0x7f7f7f7fu) == 0x3f3f3f3fu;
   const float g6 = L.ic * (1.0f / 6.0f);
+  float ig[4];
+  nf_unpack4(nf_ld4(L.idg, id, !open4), ig);
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     if (((q + PAR) & 1) == 0) continue;
@@ -227,29 +235,31 @@ __device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const floa
       const unsigned code = nf_code_at(c4, q);
       const NfW6 w = nf_code_w6(L, code, i0 + q, j, k);
       const float s = ((w.xl * xl + w.xh * xh) + (w.yl * yl[q] + w.yh * yh[q])) + (w.zl * zl[q] + w.zh * zh[q]);
-      out[q] = (rr[q] + L.c * s) * nf_code_idiag(L, code, i0 + q, j, k);
+      out[q] = (rr[q] + L.c * s) * ig[q];
     }
   }
   *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
 }
 
 __global__ void __launch_bounds__(256, 4) k_up1(NfLvK L, float *z, const float *__restrict__ r,
-                                             const float *__restrict__ zc, int cnx, int cny, const NfSolveState *st) {
+                                             const float *__restrict__ zc, int cnx, int cny, int kch,
+                                             const NfSolveState *st) {
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
-  if (i0 >= L.nx || j >= L.ny || k >= L.nz) return;
-  if ((j + k) & 1)
-    nf_up1_body<1>(L, z, r, zc, cnx, cny, i0, j, k);
-  else
-    nf_up1_body<0>(L, z, r, zc, cnx, cny, i0, j, k);
+  if (i0 >= L.nx || j >= L.ny) return;
+  const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, L.nz);
+  for (int k = k0; k < k1; ++k) {
+    if ((j + k) & 1)
+      nf_up1_body<1>(L, z, r, zc, cnx, cny, i0, j, k);
+    else
+      nf_up1_body<0>(L, z, r, zc, cnx, cny, i0, j, k);
+  }
 }
 
 // Red half sweep in place (black neighbours are final); returns r.z over the 4 cells.
 template <int PAR>
-__device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const float *__restrict__ r, int i0, int j,
-                                             int k) {
+__device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const float *r, int i0, int j, int k) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const size_t sy = nx, sz = (size_t)nx * ny;
   const size_t id = ((size_t)k * ny + j) * nx + i0;
@@ -266,6 +276,8 @@ __device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const flo
   float dot = 0.0f;
   const bool open4 = (c4 & 0x7f7f7f7fu) == 0x3f3f3f3fu;
   const float g6 = L.ic * (1.0f / 6.0f);
+  float ig[4];
+  nf_unpack4(nf_ld4(L.idg, id, !open4), ig);
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     if (((q + PAR) & 1) == 0) {
@@ -277,7 +289,7 @@ __device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const flo
         const unsigned code = nf_code_at(c4, q);
         const NfW6 w = nf_code_w6(L, code, i0 + q, j, k);
         const float s = ((w.xl * xl + w.xh * xh) + (w.yl * yl[q] + w.yh * yh[q])) + (w.zl * zl[q] + w.zh * zh[q]);
-        zc[q] = (rr[q] + L.c * s) * nf_code_idiag(L, code, i0 + q, j, k);
+        zc[q] = (rr[q] + L.c * s) * ig[q];
       }
     }
   }
@@ -288,15 +300,17 @@ __device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const flo
 }
 
 template <bool DOT>
-__global__ void __launch_bounds__(256, 4) k_up2(NfLvK L, float *z, const float *__restrict__ r, NfSolveState *st,
-                                             int slot) {
+__global__ void __launch_bounds__(256, 4) k_up2(NfLvK L, float *z, const float *__restrict__ r, int kch,
+                                             NfSolveState *st, int slot) {
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
   float dot = 0.0f;
-  if (i0 < L.nx && j < L.ny && k < L.nz)
-    dot = ((j + k) & 1) ? nf_up2_body<1>(L, z, r, i0, j, k) : nf_up2_body<0>(L, z, r, i0, j, k);
+  if (i0 < L.nx && j < L.ny) {
+    const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, L.nz);
+    for (int k = k0; k < k1; ++k)
+      dot += ((j + k) & 1) ? nf_up2_body<1>(L, z, r, i0, j, k) : nf_up2_body<0>(L, z, r, i0, j, k);
+  }
   if (DOT) nf_block_atomic_add((double)dot, &st->rz[slot]);
 }
 
@@ -440,23 +454,88 @@ __device__ __forceinline__ void nf_tail_half(float *__restrict__ z, const float 
   __syncthreads();
 }
 
-__global__ void __launch_bounds__(NF_TAIL_THREADS) k_tail(NfTailK T, const float *__restrict__ pack_g,
-                                                           const float *__restrict__ rg, float *__restrict__ zg,
-                                                           const NfSolveState *st) {
-  if (st && st->done) return;
-  extern __shared__ float sm[];
+// the same half sweep by one warp (coarsest level: a few dozen cells, many sweeps -- warp barriers instead of CTA
+// barriers)
+__device__ __forceinline__ void nf_tail_half_warp(float *z, const float *r, const float *pk, int n, int sy, int sz,
+                                                  float color, bool zero) {
+  for (int id = threadIdx.x; id < n; id += 32) {
+    if (pk[7 * n + id] != color) continue;
+    float a = r[id];
+    if (!zero) {
+      a += pk[1 * n + id] * z[max(id - 1, 0)];
+      a += pk[2 * n + id] * z[min(id + 1, n - 1)];
+      a += pk[3 * n + id] * z[max(id - sy, 0)];
+      a += pk[4 * n + id] * z[min(id + sy, n - 1)];
+      a += pk[5 * n + id] * z[max(id - sz, 0)];
+      a += pk[6 * n + id] * z[min(id + sz, n - 1)];
+    }
+    z[id] = a * pk[id];
+  }
+  __syncwarp();
+}
+
+// The sub-V-cycle of the tail levels by ONE CTA (all of its threads must call it); rg / zg: right-hand side and
+// result of the first tail level in global memory (plain loads: rg may have been written in this very kernel).
+// Packed operator of the tail levels, global -> shared, by the bulk-copy engine (cp.async.bulk + mbarrier): one
+// thread issues it, no registers are staged, and in k_vcoarse it overlaps the whole down sweep of the levels above.
+// Needs every level's cell count to be a multiple of 4 (16-byte chunks); otherwise nf_tail_run loads with plain loops.
+__device__ __forceinline__ bool nf_tail_bulk_ok(const NfTailK &T) {
+  bool ok = true;
+  for (int l = 0; l < T.nlev; ++l) ok = ok && (T.n[l] & 3) == 0;
+  return ok;
+}
+__device__ __forceinline__ void nf_tail_prefetch(const NfTailK &T, const float *__restrict__ pack_g, float *sm,
+                                                 unsigned long long *mbar) {  // called by ONE thread
+  const unsigned bar = (unsigned)__cvta_generic_to_shared(mbar);
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  unsigned total = 0;
+  for (int l = 0; l < T.nlev; ++l) total += 32u * (unsigned)T.n[l];
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(total) : "memory");
+  for (int l = 0; l < T.nlev; ++l) {
+    const unsigned n = (unsigned)T.n[l];
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(sm + 10 * (size_t)T.off[l] + 2 * n);
+    const char *src = (const char *)(pack_g + 8 * (size_t)T.off[l]);
+    for (unsigned o = 0; o < 32u * n; o += 32768u) {
+      const unsigned bytes = min(32768u, 32u * n - o);
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst + o),
+                   "l"(src + o), "r"(bytes), "r"(bar)
+                   : "memory");
+    }
+  }
+}
+__device__ __forceinline__ void nf_tail_wait(unsigned long long *mbar) {
+  const unsigned bar = (unsigned)__cvta_generic_to_shared(mbar);
+  unsigned done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\nselp.u32 %0, 1, 0, p;\n}"
+        : "=r"(done)
+        : "r"(bar)
+        : "memory");
+  }
+}
+
+// The sub-V-cycle of the tail levels by ONE CTA (all of its threads must call it); rg / zg: right-hand side and
+// result of the first tail level in global memory (plain loads: rg may have been written in this very kernel).
+// mbar != nullptr: the packs are arriving through nf_tail_prefetch -- wait for them instead of loading.
+__device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__restrict__ pack_g, const float *rg,
+                                            float *zg, float *sm, unsigned long long *mbar) {
   const int nl = T.nlev;
-  // load the packs, the first level's right-hand side, zero every z
+  // the first level's right-hand side, zero every z (and the packs unless prefetched)
   for (int l = 0; l < nl; ++l) {
     const int n = T.n[l];
     float *base = sm + 10 * (size_t)T.off[l];
-    const float *src = pack_g + 8 * (size_t)T.off[l];
-    for (int t = threadIdx.x; t < 8 * n; t += blockDim.x) base[2 * n + t] = src[t];
+    if (!mbar) {
+      const float *src = pack_g + 8 * (size_t)T.off[l];
+      for (int t = threadIdx.x; t < 8 * n; t += blockDim.x) base[2 * n + t] = src[t];
+    }
     for (int t = threadIdx.x; t < n; t += blockDim.x) {
       base[t] = 0.0f;
       base[n + t] = l == 0 ? rg[t] : 0.0f;
     }
   }
+  if (mbar) nf_tail_wait(mbar);
   __syncthreads();
   // down
   for (int l = 0; l + 1 < nl; ++l) {
@@ -494,14 +573,26 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS) k_tail(NfTailK T, const float
     const int l = nl - 1;
     const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
     float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
-    for (int s = 0; s < T.sweeps; ++s) {
-      nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, s == 0);
-      nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+    if (n > 256) {  // (a one-level tail: the CTA-wide sweeps)
+      for (int s = 0; s < T.sweeps; ++s) {
+        nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, s == 0);
+        nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+      }
+      for (int s = 0; s < T.sweeps; ++s) {
+        nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+        nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, false);
+      }
+    } else if (threadIdx.x < 32) {
+      for (int s = 0; s < T.sweeps; ++s) {
+        nf_tail_half_warp(z, r, pk, n, nx, nx * ny, 0.0f, s == 0);
+        nf_tail_half_warp(z, r, pk, n, nx, nx * ny, 1.0f, false);
+      }
+      for (int s = 0; s < T.sweeps; ++s) {
+        nf_tail_half_warp(z, r, pk, n, nx, nx * ny, 1.0f, false);
+        nf_tail_half_warp(z, r, pk, n, nx, nx * ny, 0.0f, false);
+      }
     }
-    for (int s = 0; s < T.sweeps; ++s) {
-      nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
-      nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, false);
-    }
+    __syncthreads();
   }
   // up
   for (int l = nl - 2; l >= 0; --l) {
@@ -518,6 +609,102 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS) k_tail(NfTailK T, const float
     nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, false);
   }
   for (int t = threadIdx.x; t < T.n[0]; t += blockDim.x) zg[t] = sm[t];
+}
+
+__global__ void __launch_bounds__(NF_TAIL_THREADS) k_tail(NfTailK T, const float *__restrict__ pack_g,
+                                                           const float *__restrict__ rg, float *__restrict__ zg,
+                                                           const NfSolveState *st) {
+  if (st && st->done) return;
+  extern __shared__ __align__(16) float sm[];
+  __shared__ unsigned long long mbar;
+  const bool bulk = nf_tail_bulk_ok(T);
+  if (bulk && threadIdx.x == 0) nf_tail_prefetch(T, pack_g, sm, &mbar);
+  __syncthreads();
+  nf_tail_run(T, pack_g, rg, zg, sm, bulk ? &mbar : nullptr);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// persistent coarse part of the V-cycle: every level below the finest one in ONE cooperative launch
+// ------------------------------------------------------------------------------------------------------------
+// Levels first .. nb-1 run the vec bodies with grid-stride loops over the (4-cell row, j, k) tasks; phases are
+// separated by grid barriers instead of kernel boundaries (all of these levels are L2-resident at 256^3: 128^3 and
+// below), and CTA 0 runs the shared-memory tail between the down and the up sweep.
+struct NfCoarseK {
+  int first, nb, has_tail;
+  NfLvK lv[NF_MAX_LEVELS];
+  float *z[NF_MAX_LEVELS], *r[NF_MAX_LEVELS];
+  NfTailK T;
+  const float *pack;
+};
+
+__global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_constant__ NfCoarseK P,
+                                                                 const NfSolveState *st) {
+  if (st && st->done) return;  // (uniform over the grid: written by an earlier kernel)
+  extern __shared__ __align__(16) float sm[];
+  __shared__ unsigned long long mbar;
+  const bool bulk = P.has_tail && nf_tail_bulk_ok(P.T);
+  if (bulk && blockIdx.x == 0 && threadIdx.x == 0) nf_tail_prefetch(P.T, P.pack, sm, &mbar);
+  cg::grid_group grid = cg::this_grid();
+  // task index: warps are dealt round-robin over the CTAs so that a small level still spreads over every SM
+  const int gn = gridDim.x * blockDim.x;  // (tasks < 2^31)
+  const int gt = ((threadIdx.x >> 5) * gridDim.x + blockIdx.x) * 32 + (threadIdx.x & 31);
+  // The static data of the small levels (codes, inverse diagonals, fp32 weights) was evicted from L2 by the fine
+  // level's streaming passes: pull it back with L2 prefetches now, off the critical path of the phases below.
+  for (int l = P.first; l < P.nb; ++l) {
+    const NfLvK &L = P.lv[l];
+    const size_t nc = (size_t)L.nx * L.ny * L.nz;
+    for (size_t o = (size_t)gt * 128; o < nc; o += (size_t)gn * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.code + o));
+    if (l >= 2) {
+      const size_t nxf = (size_t)L.nz * L.ny * L.pax, nyf = (size_t)L.nz * (L.ny + 1) * L.nx, nzf = (size_t)(L.nz + 1) * L.ny * L.nx;
+      for (size_t o = (size_t)gt * 32; o < nc; o += (size_t)gn * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.idg + o));
+      for (size_t o = (size_t)gt * 32; o < nxf; o += (size_t)gn * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.ax + o));
+      for (size_t o = (size_t)gt * 32; o < nyf; o += (size_t)gn * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.ay + o));
+      for (size_t o = (size_t)gt * 32; o < nzf; o += (size_t)gn * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.az + o));
+    }
+  }
+  for (int l = P.first; l < P.nb; ++l) {
+    const NfLvK &L = P.lv[l];
+    const int nx4 = L.nx >> 2, ny = L.ny, nz = L.nz;
+    const int cnx = P.lv[l + 1].nx, cny = P.lv[l + 1].ny, cnz = P.lv[l + 1].nz;
+    for (int t = gt; t < nx4 * ny * nz; t += gn) {
+      const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
+      if ((j + k) & 1)
+        nf_down1_body<1>(L, P.r[l], P.z[l], i0, j, k);
+      else
+        nf_down1_body<0>(L, P.r[l], P.z[l], i0, j, k);
+    }
+    grid.sync();
+    for (int t = gt; t < nx4 * cny * cnz; t += gn) {
+      const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
+      nf_down2_body(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
+    }
+    grid.sync();
+  }
+  if (P.has_tail) {
+    if (blockIdx.x == 0) nf_tail_run(P.T, P.pack, P.r[P.nb], P.z[P.nb], sm, bulk ? &mbar : nullptr);
+    grid.sync();
+  }
+  for (int l = P.nb - 1; l >= P.first; --l) {
+    const NfLvK &L = P.lv[l];
+    const int nx4 = L.nx >> 2, ny = L.ny, nz = L.nz;
+    const int cnx = P.lv[l + 1].nx, cny = P.lv[l + 1].ny;
+    for (int t = gt; t < nx4 * ny * nz; t += gn) {
+      const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
+      if ((j + k) & 1)
+        nf_up1_body<1>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+      else
+        nf_up1_body<0>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+    }
+    grid.sync();
+    for (int t = gt; t < nx4 * ny * nz; t += gn) {
+      const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
+      if ((j + k) & 1)
+        nf_up2_body<1>(L, P.z[l], P.r[l], i0, j, k);
+      else
+        nf_up2_body<0>(L, P.z[l], P.r[l], i0, j, k);
+    }
+    if (l > P.first) grid.sync();
+  }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -545,8 +732,23 @@ void nf_mg_plan(nf_grid *g) {
 }
 
 int nf_mg_init(nf_grid *g) {
-  NF_CUDA(g, cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  NF_TAIL_MAX_CELLS * 10 * (int)sizeof(float)));
+  const int smem = NF_TAIL_MAX_CELLS * 10 * (int)sizeof(float);
+  NF_CUDA(g, cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  // the cooperative coarse kernel: one CTA per SM; needs a tail, at least one vec level below the finest one, and
+  // every level between the finest one and the tail to be a vec level
+  g->coarse_ctas = 0;
+  const int nl = g->nlev;
+  if (g->tail < nl && g->tail >= 2) {
+    bool all_vec = true;
+    for (int l = 1; l < g->tail; ++l) all_vec = all_vec && g->lv[l].vec;
+    int dev = 0, sms = 0, coop = 0, per_sm = 0;
+    NF_CUDA(g, cudaGetDevice(&dev));
+    NF_CUDA(g, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    NF_CUDA(g, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    NF_CUDA(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_vcoarse, NF_TAIL_THREADS, tail_smem_bytes(g)));
+    if (all_vec && coop && per_sm >= 1) g->coarse_ctas = sms;
+  }
   return NF_OK;
 }
 
@@ -582,13 +784,14 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
   const int nb = has_tail ? g->tail : nl - 1;
   const bool fused = g->nu_pre == 1 && g->nu_post == 1 && !g->force_generic;
   bool dot_done = false;
-  for (int l = 0; l < nb; ++l) {
+  const bool coop = fused && g->coarse_ctas > 0 && g->lv[0].vec;
+  for (int l = 0; l < (coop ? 1 : nb); ++l) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
     if (L.vec && fused) {
-      NfDims d = nf_dims(L.nx / 4, L.ny, L.nz);
-      NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), k_down1<<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.r, L.z, st));
-      NfDims d2 = nf_dims(L.nx / 4, C.ny, C.nz);
-      NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), k_down2<<<d2.grid, d2.block, 0, g->stream>>>(nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, st));
+      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+      NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), k_down1<<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.r, L.z, NF_KCH_MG, st));
+      NfDims d2 = nf_vdims(L.nx / 4, C.ny, C.nz, 1);
+      NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), k_down2<<<d2.grid, d2.block, 0, g->stream>>>(nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, 1, st));
     } else {
       for (int s = 0; s < g->nu_pre; ++s) {
         smooth_half(g, L, 0, s == 0, false, st, slot);
@@ -598,7 +801,29 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
       NF_LAUNCH(g, (l == 0 ? NFK_RESTRICT0 : NFK_RESTRICT_C), k_residual_restrict<<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, C.r, C.nx, C.ny, C.nz, st));
     }
   }
-  if (has_tail) {
+  if (coop) {
+    NfCoarseK P;
+    P.first = 1; P.nb = nb; P.has_tail = 1;
+    for (int l = 0; l < nl; ++l) {
+      P.lv[l] = nf_lvk(g->lv[l]);
+      P.z[l] = g->lv[l].z;
+      P.r[l] = g->lv[l].r;
+    }
+    int off = 0, m = 1;
+    P.T.nlev = nl - g->tail;
+    for (int l = g->tail; l < nl; ++l) {
+      const NfLevel &L = g->lv[l];
+      const int t = l - g->tail;
+      P.T.n[t] = (int)L.ncell; P.T.nx[t] = L.nx; P.T.ny[t] = L.ny; P.T.nz[t] = L.nz; P.T.off[t] = off;
+      off += (int)L.ncell;
+      if (l == nl - 1) m = L.nx > L.ny ? (L.nx > L.nz ? L.nx : L.nz) : (L.ny > L.nz ? L.ny : L.nz);
+    }
+    P.T.sweeps = 2 * m;
+    P.pack = g->tailpack;
+    const NfSolveState *stc = st;
+    void *args[] = {(void *)&P, (void *)&stc};
+    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel((void *)k_vcoarse, dim3(g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
+  } else if (has_tail) {
     NfTailK T;
     T.nlev = nl - g->tail;
     int off = 0, m = 1;
@@ -624,16 +849,16 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
       smooth_half(g, B, 0, false, false, st, slot);
     }
   }
-  for (int l = nb - 1; l >= 0; --l) {
+  for (int l = (coop ? 0 : nb - 1); l >= 0; --l) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
     if (L.vec && fused) {
-      NfDims d = nf_dims(L.nx / 4, L.ny, L.nz);
-      NF_LAUNCH(g, (l == 0 ? NFK_UP1_0 : NFK_VEC_C), k_up1<<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, C.z, C.nx, C.ny, st));
+      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+      NF_LAUNCH(g, (l == 0 ? NFK_UP1_0 : NFK_VEC_C), k_up1<<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, C.z, C.nx, C.ny, NF_KCH_MG, st));
       if (l == 0 && with_dot) {
-        NF_LAUNCH(g, NFK_UP2_0, k_up2<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, g->st, slot));
+        NF_LAUNCH(g, NFK_UP2_0, k_up2<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, NF_KCH_MG, g->st, slot));
         dot_done = true;
       } else {
-        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), k_up2<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, st, slot));
+        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), k_up2<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, NF_KCH_MG, st, slot));
       }
     } else {
       NfDims d = nf_dims(L.nx, L.ny, L.nz);

@@ -38,52 +38,158 @@ __global__ void __launch_bounds__(256) k_apply_A(const float *__restrict__ p, co
 // The same operator, 4 cells per thread on float4 rows with the weights taken from the 1-byte cell code
 // (DESIGN.md section 2): 9 B/cell (p, code in; q out) instead of 20.  Needs nx % 4 == 0 and 16-byte aligned p, q.
 template <bool DOT>
-__global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restrict__ p, float *__restrict__ q,
+__global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restrict__ p, float *__restrict__ q, int kch,
                                                 NfSolveState *st, int slot) {
   if (DOT && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
   float part = 0.0f;
-  if (i0 < L.nx && j < L.ny && k < L.nz) {
+  if (i0 < L.nx && j < L.ny) {
     const int nx = L.nx, ny = L.ny, nz = L.nz;
     const size_t sy = nx, sz = (size_t)nx * ny;
-    const size_t id = ((size_t)k * ny + j) * nx + i0;
-    float pc[4], yl[4], yh[4], zl[4], zh[4], out[4];
-    nf_unpack4(nf_ld4(p, id, true), pc);
-    nf_unpack4(nf_ld4(p, id - sy, j > 0), yl);
-    nf_unpack4(nf_ld4(p, id + sy, j + 1 < ny), yh);
-    nf_unpack4(nf_ld4(p, id - sz, k > 0), zl);
-    nf_unpack4(nf_ld4(p, id + sz, k + 1 < nz), zh);
-    const float xl = nf_ld1(p, id - 1, i0 > 0), xh = nf_ld1(p, id + 4, i0 + 4 < nx);
-    const unsigned c4 = nf_ldc4(L.code, id, true);
-    const bool open4 = (c4 & 0x7f7f7f7fu) == 0x3f3f3f3fu;  // all four cells: six open faces
+    const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, nz);
+    size_t id = ((size_t)k0 * ny + j) * nx + i0;
+    // the z-neighbour rows rotate through registers: one new row of p per plane
+    float4 lo = nf_ld4(p, id - sz, k0 > 0), ce = nf_ld4(p, id, true);
+    for (int k = k0; k < k1; ++k, id += sz) {
+      const float4 hi = nf_ld4(p, id + sz, k + 1 < nz);
+      float pc[4], yl[4], yh[4], zl[4], zh[4], out[4];
+      nf_unpack4(ce, pc);
+      nf_unpack4(lo, zl);
+      nf_unpack4(hi, zh);
+      nf_unpack4(nf_ld4(p, id - sy, j > 0), yl);
+      nf_unpack4(nf_ld4(p, id + sy, j + 1 < ny), yh);
+      const float xl = nf_ld1(p, id - 1, i0 > 0), xh = nf_ld1(p, id + 4, i0 + 4 < nx);
+      const unsigned c4 = nf_ldc4(L.code, id, true);
+      const bool open4 = (c4 & 0x7f7f7f7fu) == 0x3f3f3f3fu;  // all four cells: six open faces
 #pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      const float l = t > 0 ? pc[t - 1] : xl, h = t < 3 ? pc[t + 1] : xh;
-      if (open4) {
-        const float s = ((l + h) + (yl[t] + yh[t])) + (zl[t] + zh[t]);
-        out[t] = L.c * (6.0f * pc[t] - s);
-      } else {
-        const NfW6 w = nf_code_w6(L, nf_code_at(c4, t), i0 + t, j, k);
-        const float s = ((w.xl * l + w.xh * h) + (w.yl * yl[t] + w.yh * yh[t])) + (w.zl * zl[t] + w.zh * zh[t]);
-        out[t] = L.c * (nf_w6_sum(w) * pc[t] - s);
+      for (int t = 0; t < 4; ++t) {
+        const float l = t > 0 ? pc[t - 1] : xl, h = t < 3 ? pc[t + 1] : xh;
+        if (open4) {
+          const float s = ((l + h) + (yl[t] + yh[t])) + (zl[t] + zh[t]);
+          out[t] = L.c * (6.0f * pc[t] - s);
+        } else {
+          const NfW6 w = nf_code_w6(L, nf_code_at(c4, t), i0 + t, j, k);
+          const float s = ((w.xl * l + w.xh * h) + (w.yl * yl[t] + w.yh * yh[t])) + (w.zl * zl[t] + w.zh * zh[t]);
+          out[t] = L.c * (nf_w6_sum(w) * pc[t] - s);
+        }
+        part += pc[t] * out[t];
       }
-      part += pc[t] * out[t];
+      *reinterpret_cast<float4 *>(q + id) = make_float4(out[0], out[1], out[2], out[3]);
+      lo = ce;
+      ce = hi;
     }
-    *reinterpret_cast<float4 *>(q + id) = make_float4(out[0], out[1], out[2], out[3]);
   }
   if (DOT) nf_block_atomic_add((double)part, &st->pq[slot]);
+}
+
+// a-4 + a-3 fused: p' = z + beta p (beta = rz_new / rz_old from device memory; FIRST: p' = z) evaluated on the fly
+// for the cell's own row and its neighbour rows, q = A p', p.q partial sums.  17 B/cell (z, p, code in; p', q out)
+// instead of 12 + 9 for the two separate passes.  p' goes to a second buffer: the neighbours' threads still read p.
+template <bool FIRST>
+__global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__restrict__ z, const float *__restrict__ pold,
+                                                 float *__restrict__ pnew, float *__restrict__ q, int kch,
+                                                 NfSolveState *st, int slot) {
+  if (st->done) return;
+  float beta = 0.0f;
+  if (!FIRST) {
+    const double rz_old = st->rz[1 - slot];
+    beta = rz_old != 0.0 ? (float)(st->rz[slot] / rz_old) : 0.0f;
+  }
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  float part = 0.0f;
+  if (i0 < L.nx && j < L.ny) {
+    const int nx = L.nx, ny = L.ny, nz = L.nz;
+    const size_t sy = nx, sz = (size_t)nx * ny;
+    const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, nz);
+    size_t id = ((size_t)k0 * ny + j) * nx + i0;
+    auto row4 = [&](size_t at, bool ok) -> float4 {
+      float4 a = nf_ld4(z, at, ok);
+      if (!FIRST) {
+        const float4 b = nf_ld4(pold, at, ok);
+        a.x += beta * b.x; a.y += beta * b.y; a.z += beta * b.z; a.w += beta * b.w;
+      }
+      return a;
+    };
+    auto one = [&](size_t at, bool ok) -> float {
+      float a = nf_ld1(z, at, ok);
+      if (!FIRST) a += beta * nf_ld1(pold, at, ok);
+      return a;
+    };
+    float4 lo = row4(id - sz, k0 > 0), ce = row4(id, true);
+    for (int k = k0; k < k1; ++k, id += sz) {
+      const float4 hi = row4(id + sz, k + 1 < nz);
+      float pc[4], yl[4], yh[4], zl[4], zh[4], out[4];
+      nf_unpack4(ce, pc);
+      nf_unpack4(lo, zl);
+      nf_unpack4(hi, zh);
+      nf_unpack4(row4(id - sy, j > 0), yl);
+      nf_unpack4(row4(id + sy, j + 1 < ny), yh);
+      const float xl = one(id - 1, i0 > 0), xh = one(id + 4, i0 + 4 < nx);
+      const unsigned c4 = nf_ldc4(L.code, id, true);
+      const bool open4 = (c4 & 0x7f7f7f7fu) == 0x3f3f3f3fu;
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        const float l = t > 0 ? pc[t - 1] : xl, h = t < 3 ? pc[t + 1] : xh;
+        if (open4) {
+          const float s = ((l + h) + (yl[t] + yh[t])) + (zl[t] + zh[t]);
+          out[t] = L.c * (6.0f * pc[t] - s);
+        } else {
+          const NfW6 w = nf_code_w6(L, nf_code_at(c4, t), i0 + t, j, k);
+          const float s = ((w.xl * l + w.xh * h) + (w.yl * yl[t] + w.yh * yh[t])) + (w.zl * zl[t] + w.zh * zh[t]);
+          out[t] = L.c * (nf_w6_sum(w) * pc[t] - s);
+        }
+        part += pc[t] * out[t];
+      }
+      *reinterpret_cast<float4 *>(pnew + id) = ce;
+      *reinterpret_cast<float4 *>(q + id) = make_float4(out[0], out[1], out[2], out[3]);
+      lo = ce;
+      ce = hi;
+    }
+  }
+  nf_block_atomic_add((double)part, &st->pq[slot]);
 }
 
 // ------------------------------------------------------------------------------------------------------------
 // a-4  CG vector ops
 // ------------------------------------------------------------------------------------------------------------
-// x += a p ; r -= a q ; rr += r.r      a = rz/pq read from device memory
+// Advance the iteration counter, decide convergence (R11), publish the status to the mapped host ring, and clear
+// the accumulators of the other parity slot.  One thread, after rr[slot] is complete.
+__device__ __forceinline__ void nf_cg_check(NfSolveState *st, int slot, NfHostStatus *hs, int seq) {
+  if (!st->done) {
+    st->iter += 1;
+    const double rr = *(volatile double *)&st->rr[slot];
+    if (!(rr == rr) || rr <= st->tol2 * st->bb) {
+      st->done = 1;
+      st->converged = (rr == rr) ? 1 : 0;
+    } else if (st->iter >= st->maxit) {
+      st->done = 1;
+      st->converged = 0;
+    }
+    st->pq[1 - slot] = 0.0;
+    st->rr[1 - slot] = 0.0;
+    st->rz[1 - slot] = 0.0;
+    st->relres = st->bb > 0.0 ? sqrt(rr / st->bb) : 0.0;
+  }
+  hs->relres = (float)st->relres;
+  hs->iter = st->iter;
+  hs->done = st->done;
+  hs->converged = st->converged;
+  __threadfence_system();
+  hs->seq = seq;
+  __threadfence_system();
+}
+
+// x += a p ; r -= a q ; rr += r.r      a = rz/pq read from device memory.  The last CTA to finish (ticket counter)
+// runs the convergence check: no separate one-thread kernel between the update and the V-cycle.
 __global__ void __launch_bounds__(256) k_cg_update(float *__restrict__ x, float *__restrict__ r,
                                                    const float *__restrict__ p, const float *__restrict__ q, size_t n,
-                                                   int vec4, NfSolveState *st, int slot) {
-  if (st->done) return;
+                                                   int vec4, NfSolveState *st, int slot, NfHostStatus *hs, int seq) {
+  if (st->done) {  // (uniform: done is only ever set by the last CTA of an earlier launch)
+    if (blockIdx.x == 0 && threadIdx.x == 0) nf_cg_check(st, slot, hs, seq);
+    return;
+  }
   const double pq = st->pq[slot];
   const float a = (pq > 0.0) ? (float)(st->rz[slot] / pq) : 0.0f;
   double part = 0.0;
@@ -110,34 +216,22 @@ __global__ void __launch_bounds__(256) k_cg_update(float *__restrict__ x, float 
     }
   }
   nf_block_atomic_add(part, &st->rr[slot]);
+  if (threadIdx.x == 0) {
+    __threadfence();
+    const unsigned t = atomicAdd(&st->ticket, 1u);
+    if (t == gridDim.x - 1) {
+      st->ticket = 0;
+      __threadfence();
+      // (rr[slot] is read through the atomic unit's view: every CTA's add happened before its ticket)
+      nf_cg_check(st, slot, hs, seq);
+    }
+  }
 }
 
-// One thread: advance the iteration counter, decide convergence (R11), publish the status to the mapped host
-// ring, and clear the accumulators of the other parity slot.
+// The same check as a kernel of its own (generic path).
 __global__ void k_cg_check(NfSolveState *st, int slot, NfHostStatus *hs, int seq) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
-  if (!st->done) {
-    st->iter += 1;
-    const double rr = st->rr[slot];
-    if (!(rr == rr) || rr <= st->tol2 * st->bb) {
-      st->done = 1;
-      st->converged = (rr == rr) ? 1 : 0;
-    } else if (st->iter >= st->maxit) {
-      st->done = 1;
-      st->converged = 0;
-    }
-    st->pq[1 - slot] = 0.0;
-    st->rr[1 - slot] = 0.0;
-    st->rz[1 - slot] = 0.0;
-    st->relres = st->bb > 0.0 ? sqrt(rr / st->bb) : 0.0;
-  }
-  hs->relres = (float)st->relres;
-  hs->iter = st->iter;
-  hs->done = st->done;
-  hs->converged = st->converged;
-  __threadfence_system();
-  hs->seq = seq;
-  __threadfence_system();
+  nf_cg_check(st, slot, hs, seq);
 }
 
 // p = z + beta p,  beta = rz_new/rz_old (first: p = z)
@@ -235,6 +329,7 @@ __global__ void k_init_state(NfSolveState *st, double tol, int maxit) {
   st->tol2 = tol * tol;
   st->relres = 0.0;
   st->iter = 0;
+  st->ticket = 0;
   st->maxit = maxit;
   st->done = 0;
   st->converged = 0;
@@ -267,11 +362,11 @@ static inline bool apply_vec_ok(const NfLevel &L, const float *p, const float *q
 static void launch_apply(nf_grid *g, const float *p, float *q, bool dot, int slot) {
   NfLevel &L = g->lv[0];
   if (!g->force_generic && apply_vec_ok(L, p, q)) {
-    NfDims d = nf_dims(L.nx / 4, L.ny, L.nz);
+    NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
     if (dot)
-      NF_LAUNCH(g, NFK_APPLY, k_apply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, g->st, slot));
+      NF_LAUNCH(g, NFK_APPLY, k_apply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, NF_KCH_AP, g->st, slot));
     else
-      NF_LAUNCH(g, NFK_APPLY, k_apply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, nullptr, 0));
+      NF_LAUNCH(g, NFK_APPLY, k_apply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, NF_KCH_AP, nullptr, 0));
   } else {
     NfDims d = nf_dims(L.nx, L.ny, L.nz);
     if (dot)
@@ -340,19 +435,36 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
   NF_CUDA(g, cudaMemsetAsync(x, 0, n * sizeof(float), g->stream));
   int rc = nf_vcycle_impl(g, true, 0);
   if (rc != NF_OK) return rc;
-  NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, 0, 1));
+  // fused path: p' = z + beta p folded into the A-apply (p ping-pongs between g->p and g->p2), convergence check
+  // folded into the x / r update
+  const bool fusedp = !g->force_generic && apply_vec_ok(L, g->p, g->q) && apply_vec_ok(L, g->p2, L.z);
+  if (!fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, 0, 1));
   int it = 0, last_seen = -1, done = 0, converged = 0;
   float relres = 0.0f;
   if (maxit < 1) maxit = 1;
   for (it = 0; it < maxit && !done; ++it) {
     const int slot = it & 1;
-    launch_apply(g, g->p, g->q, true, slot);
-    NF_LAUNCH(g, NFK_UPDATE, k_cg_update<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, g->p, g->q, n, v4, g->st, slot));
-    NF_LAUNCH(g, NFK_CHECK, k_cg_check<<<1, 32, 0, g->stream>>>(g->st, slot, &g->hst_dev[it & (NF_RING - 1)], it + 1));
-    if (it + 1 < maxit) {
-      rc = nf_vcycle_impl(g, true, 1 - slot);
-      if (rc != NF_OK) return rc;
-      NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, slot, 0));
+    NfHostStatus *hs = &g->hst_dev[it & (NF_RING - 1)];
+    if (fusedp) {
+      float *pnew = (it & 1) ? g->p2 : g->p, *pold = (it & 1) ? g->p : g->p2;
+      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
+      if (it == 0)
+        NF_LAUNCH(g, NFK_APPLY, k_papply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, pold, pnew, g->q, NF_KCH_AP, g->st, slot));
+      else
+        NF_LAUNCH(g, NFK_APPLY, k_papply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, pold, pnew, g->q, NF_KCH_AP, g->st, slot));
+      NF_LAUNCH(g, NFK_UPDATE, k_cg_update<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, pnew, g->q, n, v4, g->st, slot, hs, it + 1));
+      if (it + 1 < maxit) {
+        rc = nf_vcycle_impl(g, true, 1 - slot);
+        if (rc != NF_OK) return rc;
+      }
+    } else {
+      launch_apply(g, g->p, g->q, true, slot);
+      NF_LAUNCH(g, NFK_UPDATE, k_cg_update<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, g->p, g->q, n, v4, g->st, slot, hs, it + 1));
+      if (it + 1 < maxit) {
+        rc = nf_vcycle_impl(g, true, 1 - slot);
+        if (rc != NF_OK) return rc;
+        NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, slot, 0));
+      }
     }
     NF_CUDA(g, cudaGetLastError());
     const int look = it - NF_LOOKAHEAD;

@@ -70,13 +70,15 @@ __device__ __forceinline__ float nf_code_diag(const NfLvK &L, unsigned code, int
 
 // Row loads for the 4-cells-per-thread kernels (rows are 16-byte aligned: nx % 4 == 0).  `ok` false = the row lies
 // outside the grid: homogeneous ghost values.
-__device__ __forceinline__ float4 nf_ld4(const float *__restrict__ p, size_t id, bool ok) {
+// (plain loads, no __restrict__ / __ldg: inside the persistent coarse kernel these arrays are written by other CTAs
+// in earlier phases, so they must not take the non-coherent path)
+__device__ __forceinline__ float4 nf_ld4(const float *p, size_t id, bool ok) {
   return ok ? *reinterpret_cast<const float4 *>(p + id) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
 }
 __device__ __forceinline__ unsigned nf_ldc4(const uint8_t *__restrict__ c, size_t id, bool ok) {
   return ok ? __ldg(reinterpret_cast<const unsigned *>(c + id)) : 0u;
 }
-__device__ __forceinline__ float nf_ld1(const float *__restrict__ p, size_t id, bool ok) { return ok ? p[id] : 0.0f; }
+__device__ __forceinline__ float nf_ld1(const float *p, size_t id, bool ok) { return ok ? p[id] : 0.0f; }
 __device__ __forceinline__ unsigned nf_ldc1(const uint8_t *__restrict__ c, size_t id, bool ok) {
   return ok ? (unsigned)__ldg(c + id) : 0u;
 }

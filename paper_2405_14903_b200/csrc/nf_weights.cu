@@ -264,8 +264,9 @@ __global__ void __launch_bounds__(256) k_coarsen_weights(const float *__restrict
 // cell has a fractional face.  With counts != nullptr (level 0) also: counts[0] += active cells (sum of six
 // weights > 0); counts[1] += open faces on Dirichlet domain faces (R12).
 __global__ void __launch_bounds__(256) k_encode(const float *__restrict__ ax, const float *__restrict__ ay,
-                                                const float *__restrict__ az, uint8_t *__restrict__ code, int nx,
-                                                int ny, int nz, int pax, NfBc6 bc, double *__restrict__ counts) {
+                                                const float *__restrict__ az, uint8_t *__restrict__ code,
+                                                float *__restrict__ idg, float ic, int nx, int ny, int nz, int pax,
+                                                NfBc6 bc, double *__restrict__ counts) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z * blockDim.z + threadIdx.z;
@@ -287,6 +288,11 @@ __global__ void __launch_bounds__(256) k_encode(const float *__restrict__ ax, co
     }
     if (mixed) c |= NF_CODE_MIXED;
     code[((size_t)k * ny + j) * nx + i] = (uint8_t)c;
+    {  // the smoother's inverse diagonal, in the arithmetic of nf_code_idiag (nf_stencil.cuh)
+      const float d = ((w[0] + w[1]) + (w[2] + w[3])) + (w[4] + w[5]);
+      const float inv_count[8] = {0.0f, 1.0f, 0.5f, 1.0f / 3.0f, 0.25f, 0.2f, 1.0f / 6.0f, 0.0f};
+      idg[((size_t)k * ny + j) * nx + i] = mixed ? (d > 0.0f ? ic / d : 0.0f) : ic * inv_count[__popc(c & 63u)];
+    }
     if (counts) {
       if (w[0] + w[1] + w[2] + w[3] + w[4] + w[5] > 0.0f) act = 1.0;
       if (i == 0 && bc.t[0] == NF_BC_DIRICHLET && w[0] > 0.0f) dir += 1.0;
@@ -382,7 +388,7 @@ int nf_build_hierarchy(nf_grid *g) {
   for (int l = 0; l < g->nlev; ++l) {
     NfLevel &L = g->lv[l];
     NfDims d = nf_dims(L.nx, L.ny, L.nz);
-    NF_LAUNCH(g, NFK_CLASSIFY, k_encode<<<d.grid, d.block, 0, g->stream>>>(L.ax, L.ay, L.az, L.code, L.nx, L.ny, L.nz, L.pax, bc6(g), l == 0 ? cnt : nullptr));
+    NF_LAUNCH(g, NFK_CLASSIFY, k_encode<<<d.grid, d.block, 0, g->stream>>>(L.ax, L.ay, L.az, L.code, L.idg, 1.0f / L.c, L.nx, L.ny, L.nz, L.pax, bc6(g), l == 0 ? cnt : nullptr));
     if (L.vec) NF_LAUNCH(g, NFK_CLASSIFY, k_encode_deep<<<d.grid, d.block, 0, g->stream>>>(L.code, L.nx, L.ny, L.nz));
   }
   NF_CUDA(g, cudaGetLastError());
