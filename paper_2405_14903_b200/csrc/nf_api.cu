@@ -44,7 +44,8 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   if (!out) return NF_ERR_INVALID;
   *out = nullptr;
   if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0f)) return NF_ERR_INVALID;
-  if ((long long)(nx + 1) * (ny + 1) * (long long)(nz + 1) > (1LL << 31) * 4) return NF_ERR_INVALID;
+  // every array is addressed with 32-bit offsets (x rows padded to a multiple of 4): < 2^32 slots
+  if ((long long)(nx + 8) * (ny + 1) * (long long)(nz + 1) >= (1LL << 32)) return NF_ERR_INVALID;
   nf_grid *g = new (std::nothrow) nf_grid();
   if (!g) return NF_ERR_ALLOC;
   g->nx = nx; g->ny = ny; g->nz = nz; g->dx = dx; g->dt_over_rho = 1.0f;

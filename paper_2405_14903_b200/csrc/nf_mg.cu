@@ -31,7 +31,7 @@ struct NfRow4 {  // one row segment of 4 cells: values and codes, with the idiag
   float v[4];
   unsigned c4;
 };
-__device__ __forceinline__ NfRow4 nf_row(const float *f, const uint8_t *__restrict__ code, size_t id,
+__device__ __forceinline__ NfRow4 nf_row(const float *f, const uint8_t *__restrict__ code, nf_idx id,
                                          bool ok) {
   NfRow4 R;
   nf_unpack4(nf_ld4(f, id, ok), R.v);
@@ -43,8 +43,8 @@ __device__ __forceinline__ NfRow4 nf_row(const float *f, const uint8_t *__restri
 template <int PAR>
 __device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, float *z, int i0, int j, int k) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
-  const size_t sy = nx, sz = (size_t)nx * ny;
-  const size_t id = ((size_t)k * ny + j) * nx + i0;
+  const nf_idx sy = nx, sz = (nf_idx)nx * ny;
+  const nf_idx id = ((nf_idx)k * ny + j) * nx + i0;
   // every load of r is issued before the branch on the code (one round trip for the common, deep path)
   const NfRow4 C = nf_row(r, L.code, id, true);
   float out[4], yl[4], yh[4], zl[4], zh[4];
@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restri
 __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, float *rc, int cnx, int cny, int i0,
                                               int J, int K) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
-  const size_t sy = nx, sz = (size_t)nx * ny;
+  const nf_idx sy = nx, sz = (nf_idx)nx * ny;
   const int j0 = 2 * J, k0 = 2 * K;
   float zc[2][2][4];  // [dk][dj][q]
   unsigned cc[2][2];
@@ -128,7 +128,7 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
   for (int dk = 0; dk < 2; ++dk)
 #pragma unroll
     for (int dj = 0; dj < 2; ++dj) {
-      const size_t id = ((size_t)(k0 + dk) * ny + (j0 + dj)) * nx + i0;
+      const nf_idx id = ((nf_idx)(k0 + dk) * ny + (j0 + dj)) * nx + i0;
       nf_unpack4(nf_ld4(z, id, true), zc[dk][dj]);
       cc[dk][dj] = nf_ldc4(L.code, id, true);
     }
@@ -138,7 +138,7 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
 #pragma unroll
     for (int dj = 0; dj < 2; ++dj) {
       const int j = j0 + dj, k = k0 + dk;
-      const size_t id = ((size_t)k * ny + j) * nx + i0;
+      const nf_idx id = ((nf_idx)k * ny + j) * nx + i0;
       const int par = (dj + dk) & 1;  // colour of q = 0 in this row (i0, j0, k0 are even)
       // the y / z neighbour rows: inside the 2x2 block or one row outside it
       float yo[4], zo[4];
@@ -163,7 +163,7 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
       }
     }
   const float f = 0.125f * L.c;
-  *reinterpret_cast<float2 *>(rc + ((size_t)K * cny + J) * cnx + (i0 >> 1)) = make_float2(f * acc0, f * acc1);
+  *reinterpret_cast<float2 *>(rc + ((nf_idx)K * cny + J) * cnx + (i0 >> 1)) = make_float2(f * acc0, f * acc1);
 }
 
 __global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restrict__ z, float *__restrict__ rc, int cnx,
@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restri
 }
 
 // z + P z_coarse on a row of 4 fine cells
-__device__ __forceinline__ void nf_row_prolonged(const float *z, const float *zc, size_t id, size_t cid, bool ok,
+__device__ __forceinline__ void nf_row_prolonged(const float *z, const float *zc, nf_idx id, nf_idx cid, bool ok,
                                                  float o[4]) {
   if (ok) {
     const float4 a = *reinterpret_cast<const float4 *>(z + id);
@@ -194,10 +194,10 @@ template <int PAR>
 __device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const float *r, const float *zc, int cnx,
                                             int cny, int i0, int j, int k) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
-  const size_t sy = nx, sz = (size_t)nx * ny;
-  const size_t id = ((size_t)k * ny + j) * nx + i0;
-  const size_t scy = cnx, scz = (size_t)cnx * cny;
-  const size_t cid = ((size_t)(k >> 1) * cny + (j >> 1)) * cnx + (i0 >> 1);
+  const nf_idx sy = nx, sz = (nf_idx)nx * ny;
+  const nf_idx id = ((nf_idx)k * ny + j) * nx + i0;
+  const nf_idx scy = cnx, scz = (nf_idx)cnx * cny;
+  const nf_idx cid = ((nf_idx)(k >> 1) * cny + (j >> 1)) * cnx + (i0 >> 1);
   const float4 zold = *reinterpret_cast<const float4 *>(z + id);
   float zp[4], yl[4], yh[4], zl[4], zh[4], rr[4], out[4];
   {
@@ -261,8 +261,8 @@ __global__ void __launch_bounds__(256, 4) k_up1(NfLvK L, float *z, const float *
 template <int PAR>
 __device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const float *r, int i0, int j, int k) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
-  const size_t sy = nx, sz = (size_t)nx * ny;
-  const size_t id = ((size_t)k * ny + j) * nx + i0;
+  const nf_idx sy = nx, sz = (nf_idx)nx * ny;
+  const nf_idx id = ((nf_idx)k * ny + j) * nx + i0;
   float zc[4], yl[4], yh[4], zl[4], zh[4], rr[4];
   nf_unpack4(nf_ld4(z, id, true), zc);
   nf_unpack4(nf_ld4(z, id - sy, j > 0), yl);
@@ -728,7 +728,12 @@ void nf_mg_plan(nf_grid *g) {
   }
   g->tail = tail;
   const int nb = tail < nl ? tail : nl - 1;  // levels [0, nb) have a coarser level below them
-  for (int l = 0; l < nl; ++l) g->lv[l].vec = (l < nb && (g->lv[l].nx & 3) == 0) ? 1 : 0;
+  for (int l = 0; l < nl; ++l) {
+    const NfLevel &L = g->lv[l];
+    const double slots = (double)(L.nz + 1) * (L.ny + 1) * (L.pax + 4);  // largest face array of the level
+    g->lv[l].vec_idx32 = slots < 4.0e9 ? 1 : 0;
+    g->lv[l].vec = (l < nb && (L.nx & 3) == 0 && g->lv[l].vec_idx32) ? 1 : 0;
+  }
 }
 
 int nf_mg_init(nf_grid *g) {

@@ -46,9 +46,9 @@ __global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restr
   float part = 0.0f;
   if (i0 < L.nx && j < L.ny) {
     const int nx = L.nx, ny = L.ny, nz = L.nz;
-    const size_t sy = nx, sz = (size_t)nx * ny;
+    const nf_idx sy = nx, sz = (nf_idx)nx * ny;
     const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, nz);
-    size_t id = ((size_t)k0 * ny + j) * nx + i0;
+    nf_idx id = ((nf_idx)k0 * ny + j) * nx + i0;
     // the z-neighbour rows rotate through registers: one new row of p per plane
     float4 lo = nf_ld4(p, id - sz, k0 > 0), ce = nf_ld4(p, id, true);
     for (int k = k0; k < k1; ++k, id += sz) {
@@ -101,10 +101,10 @@ __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__rest
   float part = 0.0f;
   if (i0 < L.nx && j < L.ny) {
     const int nx = L.nx, ny = L.ny, nz = L.nz;
-    const size_t sy = nx, sz = (size_t)nx * ny;
+    const nf_idx sy = nx, sz = (nf_idx)nx * ny;
     const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, nz);
-    size_t id = ((size_t)k0 * ny + j) * nx + i0;
-    auto row4 = [&](size_t at, bool ok) -> float4 {
+    nf_idx id = ((nf_idx)k0 * ny + j) * nx + i0;
+    auto row4 = [&](nf_idx at, bool ok) -> float4 {
       float4 a = nf_ld4(z, at, ok);
       if (!FIRST) {
         const float4 b = nf_ld4(pold, at, ok);
@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__rest
       }
       return a;
     };
-    auto one = [&](size_t at, bool ok) -> float {
+    auto one = [&](nf_idx at, bool ok) -> float {
       float a = nf_ld1(z, at, ok);
       if (!FIRST) a += beta * nf_ld1(pold, at, ok);
       return a;
@@ -355,7 +355,7 @@ static inline int vec_ok(const void *a, const void *b, const void *c, const void
 int nf_solver_init(nf_grid *g) { return nf_mg_init(g); }
 
 static inline bool apply_vec_ok(const NfLevel &L, const float *p, const float *q) {
-  return (L.nx & 3) == 0 && vec_ok(p, q, p, q, 4);
+  return L.vec_idx32 && (L.nx & 3) == 0 && vec_ok(p, q, p, q, 4);
 }
 
 // q = A p on level 0; dot: accumulate p.q into st->pq[slot] and honour st->done

@@ -4,6 +4,9 @@
 #pragma once
 #include "nf_internal.cuh"
 
+// 32-bit cell / face offsets in the stencil kernels (levels with >= 2^32 face slots do not take the vec path: nf_mg_plan)
+typedef unsigned int nf_idx;
+
 struct NfW6 {
   float xl, xh, yl, yh, zl, zh;
 };
@@ -11,15 +14,15 @@ struct NfW6 {
 __device__ __forceinline__ NfW6 nf_load_w6(const float *__restrict__ ax, const float *__restrict__ ay,
                                            const float *__restrict__ az, int i, int j, int k, int nx, int ny, int pax) {
   NfW6 w;
-  const size_t rx = ((size_t)k * ny + j) * pax + i;
+  const nf_idx rx = ((nf_idx)k * ny + j) * pax + i;
   w.xl = __ldg(ax + rx);
   w.xh = __ldg(ax + rx + 1);
-  const size_t ry = ((size_t)k * (ny + 1) + j) * nx + i;
+  const nf_idx ry = ((nf_idx)k * (ny + 1) + j) * nx + i;
   w.yl = __ldg(ay + ry);
   w.yh = __ldg(ay + ry + nx);
-  const size_t rz = ((size_t)k * ny + j) * nx + i;
+  const nf_idx rz = ((nf_idx)k * ny + j) * nx + i;
   w.zl = __ldg(az + rz);
-  w.zh = __ldg(az + rz + (size_t)ny * nx);
+  w.zh = __ldg(az + rz + (nf_idx)ny * nx);
   return w;
 }
 __device__ __forceinline__ float nf_w6_sum(const NfW6 &w) { return ((w.xl + w.xh) + (w.yl + w.yh)) + (w.zl + w.zh); }
@@ -27,8 +30,8 @@ __device__ __forceinline__ float nf_w6_sum(const NfW6 &w) { return ((w.xl + w.xh
 // sum over the six neighbours of alpha_f * v_nb with homogeneous ghosts (v = 0 outside the grid)
 __device__ __forceinline__ float nf_nb_sum(const float *__restrict__ v, const NfW6 &w, int i, int j, int k, int nx,
                                            int ny, int nz) {
-  const size_t id = ((size_t)k * ny + j) * nx + i;
-  const size_t sy = nx, sz = (size_t)nx * ny;
+  const nf_idx id = ((nf_idx)k * ny + j) * nx + i;
+  const nf_idx sy = nx, sz = (nf_idx)nx * ny;
   float s = 0.0f;
   if (i > 0) s += w.xl * v[id - 1];
   if (i + 1 < nx) s += w.xh * v[id + 1];
@@ -72,14 +75,14 @@ __device__ __forceinline__ float nf_code_diag(const NfLvK &L, unsigned code, int
 // outside the grid: homogeneous ghost values.
 // (plain loads, no __restrict__ / __ldg: inside the persistent coarse kernel these arrays are written by other CTAs
 // in earlier phases, so they must not take the non-coherent path)
-__device__ __forceinline__ float4 nf_ld4(const float *p, size_t id, bool ok) {
+__device__ __forceinline__ float4 nf_ld4(const float *p, nf_idx id, bool ok) {
   return ok ? *reinterpret_cast<const float4 *>(p + id) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
 }
-__device__ __forceinline__ unsigned nf_ldc4(const uint8_t *__restrict__ c, size_t id, bool ok) {
+__device__ __forceinline__ unsigned nf_ldc4(const uint8_t *__restrict__ c, nf_idx id, bool ok) {
   return ok ? __ldg(reinterpret_cast<const unsigned *>(c + id)) : 0u;
 }
-__device__ __forceinline__ float nf_ld1(const float *p, size_t id, bool ok) { return ok ? p[id] : 0.0f; }
-__device__ __forceinline__ unsigned nf_ldc1(const uint8_t *__restrict__ c, size_t id, bool ok) {
+__device__ __forceinline__ float nf_ld1(const float *p, nf_idx id, bool ok) { return ok ? p[id] : 0.0f; }
+__device__ __forceinline__ unsigned nf_ldc1(const uint8_t *__restrict__ c, nf_idx id, bool ok) {
   return ok ? (unsigned)__ldg(c + id) : 0u;
 }
 __device__ __forceinline__ void nf_unpack4(const float4 v, float o[4]) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
