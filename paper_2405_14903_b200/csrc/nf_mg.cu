@@ -436,10 +436,20 @@ __global__ void __launch_bounds__(256) k_tail_pack(const float *__restrict__ ax,
 
 // smem per level (offset 10*off[l] floats): z[n], r[n], pack[8n]
 __device__ __forceinline__ void nf_tail_half(float *__restrict__ z, const float *__restrict__ r,
-                                             const float *__restrict__ pk, int n, int sy, int sz, float color,
+                                             const float *__restrict__ pk, int n, int nx, int sy, int sz, float color,
                                              bool zero) {
-  for (int id = threadIdx.x; id < n; id += blockDim.x) {
-    if (pk[7 * n + id] != color) continue;
+  // nx even: the cells 2h, 2h+1 lie in one row and have different colours -- every thread updates one cell of the
+  // wanted colour (no idle half); nx odd: scan all cells
+  const bool pairs = (nx & 1) == 0;
+  const int cnt = pairs ? (n >> 1) : n;
+  for (int h = threadIdx.x; h < cnt; h += blockDim.x) {
+    int id = h;
+    if (pairs) {
+      id = 2 * h;
+      if (pk[7 * n + id] != color) id += 1;
+    } else if (pk[7 * n + id] != color) {
+      continue;
+    }
     float a = r[id];
     if (!zero) {
       a += pk[1 * n + id] * z[max(id - 1, 0)];
@@ -454,28 +464,52 @@ __device__ __forceinline__ void nf_tail_half(float *__restrict__ z, const float 
   __syncthreads();
 }
 
-// the same half sweep by one warp (coarsest level: a few dozen cells, many sweeps -- warp barriers instead of CTA
-// barriers)
-__device__ __forceinline__ void nf_tail_half_warp(float *z, const float *r, const float *pk, int n, int sy, int sz,
-                                                  float color, bool zero) {
-  for (int id = threadIdx.x; id < n; id += 32) {
-    if (pk[7 * n + id] != color) continue;
-    float a = r[id];
-    if (!zero) {
-      a += pk[1 * n + id] * z[max(id - 1, 0)];
-      a += pk[2 * n + id] * z[min(id + 1, n - 1)];
-      a += pk[3 * n + id] * z[max(id - sy, 0)];
-      a += pk[4 * n + id] * z[min(id + sy, n - 1)];
-      a += pk[5 * n + id] * z[max(id - sz, 0)];
-      a += pk[6 * n + id] * z[min(id + sz, n - 1)];
-    }
-    z[id] = a * pk[id];
+// Coarsest level (n <= 64 cells) by ONE warp with its operator in registers: lane l owns cells l and l + 32; `sweeps`
+// red->black sweeps from a zero guess, then `sweeps` black->red sweeps (symmetric), warp barriers only.
+__device__ __forceinline__ void nf_tail_coarsest_warp(float *z, const float *r, const float *pk, int n, int sy, int sz,
+                                                      int sweeps) {
+  const int lane = threadIdx.x;
+  float w[2][6], dg[2], rr[2], col[2];
+  int nb[2][6];
+  bool has[2];
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    const int id = lane + 32 * c;
+    has[c] = id < n;
+    const int ic = has[c] ? id : 0;
+    dg[c] = pk[ic];
+    rr[c] = r[ic];
+    col[c] = pk[7 * n + ic];
+#pragma unroll
+    for (int f = 0; f < 6; ++f) w[c][f] = pk[(1 + f) * n + ic];
+    nb[c][0] = max(ic - 1, 0); nb[c][1] = min(ic + 1, n - 1);
+    nb[c][2] = max(ic - sy, 0); nb[c][3] = min(ic + sy, n - 1);
+    nb[c][4] = max(ic - sz, 0); nb[c][5] = min(ic + sz, n - 1);
   }
-  __syncwarp();
+  auto half = [&](float color, bool zero) {
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      if (has[c] && col[c] == color) {
+        float a = rr[c];
+        if (!zero) {
+#pragma unroll
+          for (int f = 0; f < 6; ++f) a += w[c][f] * z[nb[c][f]];
+        }
+        z[lane + 32 * c] = a * dg[c];
+      }
+    }
+    __syncwarp();
+  };
+  for (int s = 0; s < sweeps; ++s) {
+    half(0.0f, s == 0);
+    half(1.0f, false);
+  }
+  for (int s = 0; s < sweeps; ++s) {
+    half(1.0f, false);
+    half(0.0f, false);
+  }
 }
 
-// The sub-V-cycle of the tail levels by ONE CTA (all of its threads must call it); rg / zg: right-hand side and
-// result of the first tail level in global memory (plain loads: rg may have been written in this very kernel).
 // Packed operator of the tail levels, global -> shared, by the bulk-copy engine (cp.async.bulk + mbarrier): one
 // thread issues it, no registers are staged, and in k_vcoarse it overlaps the whole down sweep of the levels above.
 // Needs every level's cell count to be a multiple of 4 (16-byte chunks); otherwise nf_tail_run loads with plain loops.
@@ -541,8 +575,8 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
   for (int l = 0; l + 1 < nl; ++l) {
     const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
     float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
-    nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, true);
-    nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, true);
+    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
     // residual + restriction: r_c = 1/8 sum children (r - A z), A z = z/idg - sum wg z_nb on active cells
     const int cn = T.n[l + 1], cnx = T.nx[l + 1], cny = T.ny[l + 1];
     float *rc = sm + 10 * (size_t)T.off[l + 1] + cn;
@@ -556,6 +590,8 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
         for (int dj = 0; dj < 2; ++dj)
 #pragma unroll
           for (int di = 0; di < 2; ++di) {
+            // (the residual is zero on the black cells: the black half sweep has just solved their equations)
+            if ((di + dj + dk) & 1) continue;
             const int id = ((2 * K + dk) * ny + (2 * J + dj)) * nx + 2 * I + di;
             const float s = pk[1 * n + id] * z[max(id - 1, 0)] + pk[2 * n + id] * z[min(id + 1, n - 1)] +
                       pk[3 * n + id] * z[max(id - sy, 0)] + pk[4 * n + id] * z[min(id + sy, n - 1)] +
@@ -575,21 +611,23 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
     float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
     if (n > 256) {  // (a one-level tail: the CTA-wide sweeps)
       for (int s = 0; s < T.sweeps; ++s) {
-        nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, s == 0);
-        nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
+        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, s == 0);
+        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
       }
       for (int s = 0; s < T.sweeps; ++s) {
-        nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
-        nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, false);
+        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
       }
-    } else if (threadIdx.x < 32) {
+    } else if (n <= 64) {
+      if (threadIdx.x < 32) nf_tail_coarsest_warp(z, r, pk, n, nx, nx * ny, T.sweeps);
+    } else {
       for (int s = 0; s < T.sweeps; ++s) {
-        nf_tail_half_warp(z, r, pk, n, nx, nx * ny, 0.0f, s == 0);
-        nf_tail_half_warp(z, r, pk, n, nx, nx * ny, 1.0f, false);
+        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, s == 0);
+        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
       }
       for (int s = 0; s < T.sweeps; ++s) {
-        nf_tail_half_warp(z, r, pk, n, nx, nx * ny, 1.0f, false);
-        nf_tail_half_warp(z, r, pk, n, nx, nx * ny, 0.0f, false);
+        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
       }
     }
     __syncthreads();
@@ -605,8 +643,8 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
       z[id] += zc[((k >> 1) * cny + (j >> 1)) * cnx + (i >> 1)];
     }
     __syncthreads();
-    nf_tail_half(z, r, pk, n, nx, nx * ny, 1.0f, false);
-    nf_tail_half(z, r, pk, n, nx, nx * ny, 0.0f, false);
+    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
   }
   for (int t = threadIdx.x; t < T.n[0]; t += blockDim.x) zg[t] = sm[t];
 }

@@ -88,13 +88,16 @@ __global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restr
 // instead of 12 + 9 for the two separate passes.  p' goes to a second buffer: the neighbours' threads still read p.
 template <bool FIRST>
 __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__restrict__ z, const float *__restrict__ pold,
-                                                 float *__restrict__ pnew, float *__restrict__ q, int kch,
-                                                 NfSolveState *st, int slot) {
+                                                 float *__restrict__ pnew, float *__restrict__ q, float *__restrict__ x,
+                                                 int kch, NfSolveState *st, int slot) {
   if (st->done) return;
-  float beta = 0.0f;
+  float beta = 0.0f, aprev = 0.0f;
   if (!FIRST) {
     const double rz_old = st->rz[1 - slot];
     beta = rz_old != 0.0 ? (float)(st->rz[slot] / rz_old) : 0.0f;
+    // the previous iteration's x += a p rides on this pass (p is read here anyway): a = rz / pq of that iteration
+    const double pq_old = st->pq[1 - slot];
+    aprev = pq_old > 0.0 ? (float)(rz_old / pq_old) : 0.0f;
   }
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -112,14 +115,29 @@ __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__rest
       }
       return a;
     };
+    // the row k + 1 of this thread's own column: also carries the deferred x update of that row
+    auto row4x = [&](nf_idx at, bool ok) -> float4 {
+      float4 a = nf_ld4(z, at, ok);
+      if (!FIRST) {
+        const float4 b = nf_ld4(pold, at, ok);
+        if (ok) {
+          float4 xv = *reinterpret_cast<const float4 *>(x + at);
+          xv.x += aprev * b.x; xv.y += aprev * b.y; xv.z += aprev * b.z; xv.w += aprev * b.w;
+          *reinterpret_cast<float4 *>(x + at) = xv;
+        }
+        a.x += beta * b.x; a.y += beta * b.y; a.z += beta * b.z; a.w += beta * b.w;
+      }
+      return a;
+    };
     auto one = [&](nf_idx at, bool ok) -> float {
       float a = nf_ld1(z, at, ok);
       if (!FIRST) a += beta * nf_ld1(pold, at, ok);
       return a;
     };
-    float4 lo = row4(id - sz, k0 > 0), ce = row4(id, true);
+    // (the x update belongs to the rows this CTA owns: k0 .. k1-1; the halo rows k0-1 and k1 only feed the stencil)
+    float4 lo = row4(id - sz, k0 > 0), ce = row4x(id, true);
     for (int k = k0; k < k1; ++k, id += sz) {
-      const float4 hi = row4(id + sz, k + 1 < nz);
+      const float4 hi = (k + 1 < k1) ? row4x(id + sz, true) : row4(id + sz, k + 1 < nz);
       float pc[4], yl[4], yh[4], zl[4], zh[4], out[4];
       nf_unpack4(ce, pc);
       nf_unpack4(lo, zl);
@@ -183,6 +201,7 @@ __device__ __forceinline__ void nf_cg_check(NfSolveState *st, int slot, NfHostSt
 
 // x += a p ; r -= a q ; rr += r.r      a = rz/pq read from device memory.  The last CTA to finish (ticket counter)
 // runs the convergence check: no separate one-thread kernel between the update and the V-cycle.
+template <bool XUPD>
 __global__ void __launch_bounds__(256) k_cg_update(float *__restrict__ x, float *__restrict__ r,
                                                    const float *__restrict__ p, const float *__restrict__ q, size_t n,
                                                    int vec4, NfSolveState *st, int slot, NfHostStatus *hs, int seq) {
@@ -199,18 +218,22 @@ __global__ void __launch_bounds__(256) k_cg_update(float *__restrict__ x, float 
     float4 *x4 = (float4 *)x, *r4 = (float4 *)r;
     const float4 *p4 = (const float4 *)p, *q4 = (const float4 *)q;
     for (size_t t = tid; t < n4; t += nth) {
-      float4 xv = x4[t], rv = r4[t];
-      const float4 pv = p4[t], qv = q4[t];
-      xv.x += a * pv.x; xv.y += a * pv.y; xv.z += a * pv.z; xv.w += a * pv.w;
+      float4 rv = r4[t];
+      const float4 qv = q4[t];
+      if (XUPD) {
+        float4 xv = x4[t];
+        const float4 pv = p4[t];
+        xv.x += a * pv.x; xv.y += a * pv.y; xv.z += a * pv.z; xv.w += a * pv.w;
+        x4[t] = xv;
+      }
       rv.x -= a * qv.x; rv.y -= a * qv.y; rv.z -= a * qv.z; rv.w -= a * qv.w;
-      x4[t] = xv;
       r4[t] = rv;
       part += ((double)rv.x * rv.x + (double)rv.y * rv.y) + ((double)rv.z * rv.z + (double)rv.w * rv.w);
     }
   } else {
     for (size_t t = tid; t < n; t += nth) {
       const float rv = r[t] - a * q[t];
-      x[t] += a * p[t];
+      if (XUPD) x[t] += a * p[t];
       r[t] = rv;
       part += (double)rv * rv;
     }
@@ -225,6 +248,26 @@ __global__ void __launch_bounds__(256) k_cg_update(float *__restrict__ x, float 
       // (rr[slot] is read through the atomic unit's view: every CTA's add happened before its ticket)
       nf_cg_check(st, slot, hs, seq);
     }
+  }
+}
+
+// The x update of the LAST executed iteration (fused path: every other one rode on the next k_papply4).
+// p0 / p1: the ping-pong buffers; iteration i wrote p' into p(i & 1) and its scalars into slot i & 1.
+__global__ void __launch_bounds__(256) k_x_final(float *__restrict__ x, const float *__restrict__ p0,
+                                                 const float *__restrict__ p1, size_t n, const NfSolveState *st) {
+  const int it = st->iter - 1;
+  if (it < 0) return;
+  const int slot = it & 1;
+  const double pq = st->pq[slot];
+  const float a = pq > 0.0 ? (float)(st->rz[slot] / pq) : 0.0f;
+  const float4 *p4 = (const float4 *)(slot ? p1 : p0);
+  float4 *x4 = (float4 *)x;
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = tid; t < (n >> 2); t += nth) {
+    float4 xv = x4[t];
+    const float4 pv = p4[t];
+    xv.x += a * pv.x; xv.y += a * pv.y; xv.z += a * pv.z; xv.w += a * pv.w;
+    x4[t] = xv;
   }
 }
 
@@ -437,7 +480,8 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
   if (rc != NF_OK) return rc;
   // fused path: p' = z + beta p folded into the A-apply (p ping-pongs between g->p and g->p2), convergence check
   // folded into the x / r update
-  const bool fusedp = !g->force_generic && apply_vec_ok(L, g->p, g->q) && apply_vec_ok(L, g->p2, L.z);
+  const bool fusedp = !g->force_generic && apply_vec_ok(L, g->p, g->q) && apply_vec_ok(L, g->p2, L.z) &&
+                      apply_vec_ok(L, x, x) && (n & 3) == 0;
   if (!fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, 0, 1));
   int it = 0, last_seen = -1, done = 0, converged = 0;
   float relres = 0.0f;
@@ -449,17 +493,17 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
       float *pnew = (it & 1) ? g->p2 : g->p, *pold = (it & 1) ? g->p : g->p2;
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
       if (it == 0)
-        NF_LAUNCH(g, NFK_APPLY, k_papply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, pold, pnew, g->q, NF_KCH_AP, g->st, slot));
+        NF_LAUNCH(g, NFK_APPLY, k_papply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
       else
-        NF_LAUNCH(g, NFK_APPLY, k_papply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, pold, pnew, g->q, NF_KCH_AP, g->st, slot));
-      NF_LAUNCH(g, NFK_UPDATE, k_cg_update<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, pnew, g->q, n, v4, g->st, slot, hs, it + 1));
+        NF_LAUNCH(g, NFK_APPLY, k_papply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
+      NF_LAUNCH(g, NFK_UPDATE, k_cg_update<false><<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, pnew, g->q, n, v4, g->st, slot, hs, it + 1));
       if (it + 1 < maxit) {
         rc = nf_vcycle_impl(g, true, 1 - slot);
         if (rc != NF_OK) return rc;
       }
     } else {
       launch_apply(g, g->p, g->q, true, slot);
-      NF_LAUNCH(g, NFK_UPDATE, k_cg_update<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, g->p, g->q, n, v4, g->st, slot, hs, it + 1));
+      NF_LAUNCH(g, NFK_UPDATE, k_cg_update<true><<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, g->p, g->q, n, v4, g->st, slot, hs, it + 1));
       if (it + 1 < maxit) {
         rc = nf_vcycle_impl(g, true, 1 - slot);
         if (rc != NF_OK) return rc;
@@ -478,6 +522,7 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
       h->seq = 0;
     }
   }
+  if (fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->p, g->p2, n, g->st));
   // drain: every enqueued check kernel must have reported before the ring is reused
   const int enq = it;  // checks enqueued: 0 .. enq-1
   for (int s = last_seen + 1; s < enq; ++s) {
