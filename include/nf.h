@@ -74,8 +74,12 @@ int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value);
 /* Solver options (PAPER.md:L230 names only "MGPCG"; every parameter is this library's choice, R13):
  *   nu_pre / nu_post: red-black Gauss-Seidel sweeps before / after the coarse correction (default 1, 1; the fused
  *     4-cells-per-thread V-cycle kernels exist for (1, 1) only, other values run the generic kernels);
- *   flags: bit 0 = iterative refinement (fp64 true-residual restarts; default off),
- *          bit 1 = test hook: force the generic kernels (fp32 weights, one colour per launch) on every level. */
+ *   flags: bit 0 = reserved,
+ *          bit 1 = test hook: force the generic kernels (fp32 weights, one colour per launch) on every level,
+ *          bit 2 = switch OFF the true-residual refresh.  By default a solve with tol < 3e-4 runs PCG to 30 tol,
+ *                  re-evaluates r = b - A x in fp64 (the fp32 recursion r -= a q drifts: at 256^3 a recursive 1e-6
+ *                  was a true 4e-5), and runs PCG on that residual for a correction down to tol; the true residual
+ *                  then sits at the storage rounding of the fp32 pressure. */
 int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags);
 
 /* a-1  Face weights from the solid SDF: per face, the fluid area fraction alpha from

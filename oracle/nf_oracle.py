@@ -433,3 +433,45 @@ def advect_adjoint(U, gout, dt, dx):
         for d in range(3):
             _interp_adjoint(U[d], d, x, gv0[d], gU[d])
     return gU
+
+
+# ----------------------------------------------------------------------------------------------------
+# full steps forward and backward        PAPER.md:L78 (advection, projection), L111-141 (backward pass)
+# ----------------------------------------------------------------------------------------------------
+def rollout(U0, solid_fn, nsteps, dt, dx, dt_over_rho, bc, loss_fn, tol=1e-12, advect_on=True):
+    """N steps "advect -> geometry at t^{n+1} -> project" (R15) and the backward pass that "mirrors the
+    forward simulation in a reversed order", per-step state stored instead of a graph (L236).
+
+    solid_fn(step) -> (phi, us, dphi_dtheta, dus_dtheta) for step = 1..N, one scalar parameter theta;
+    loss_fn(U) -> (J, dJ/dU) on the final velocity.
+    Returns (J, dJ/dtheta, dJ/dU0).  dJ/dtheta = sum_n <dJ/dphi^n, dphi^n/dtheta> + <dJ/dU_s^n, dU_s^n/dtheta>
+    with dJ/dphi from dJ/dS (Eq. 9a) through the weight builder (L141) and dJ/dU_s from Eq. 9b (R9, R10)."""
+    U = [np.asarray(a, dtype=np.float64) for a in U0]
+    tape = []
+    for n in range(1, nsteps + 1):
+        Uprev = U
+        Ut = advect(U, dt, dx) if advect_on else [a.copy() for a in U]
+        phi, us, dphi, dus = solid_fn(n)
+        alpha = face_weights(phi, bc)
+        U, p = project(Ut, alpha, us, dx, dt_over_rho, bc, tol=tol)
+        tape.append((Uprev, Ut, phi, us, dphi, dus, alpha, p))
+    J, g = loss_fn(U)
+    g = [np.asarray(a, dtype=np.float64) for a in g]
+    dtheta = 0.0
+    for n in range(nsteps, 0, -1):
+        Uprev, Ut, phi, us, dphi, dus, alpha, p = tape[n - 1]
+        g_ut, g_alpha, g_us, _ = project_adjoint(g, alpha, p, Ut, us, dx, dt_over_rho, bc, tol=tol)
+        g_phi = weights_adjoint(phi, g_alpha[0], g_alpha[1], g_alpha[2], bc)
+        dtheta += float(np.sum(g_phi * dphi)) + sum(float(np.sum(a * b)) for a, b in zip(g_us, dus))
+        g = advect_adjoint(Uprev, g_ut, dt, dx) if advect_on else g_ut
+    return J, dtheta, g
+
+
+def loss_sum_u2(lo, hi):
+    """BASELINE.json configs[1]: J = sum of u^2 over the u-faces with i, j, k in [lo, hi)."""
+    def fn(U):
+        g = [np.zeros_like(np.asarray(a, dtype=np.float64)) for a in U]
+        blk = np.asarray(U[0], dtype=np.float64)[lo:hi, lo:hi, lo:hi]
+        g[0][lo:hi, lo:hi, lo:hi] = 2.0 * blk
+        return float(np.sum(blk * blk)), g
+    return fn

@@ -28,7 +28,7 @@ static void free_all(nf_grid *g) {
     cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.code); cudaFree(L.idg); cudaFree(L.z); cudaFree(L.r);
   }
   cudaFree(g->us); cudaFree(g->vs); cudaFree(g->ws); cudaFree(g->sdf);
-  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->tailpack);
+  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->b0); cudaFree(g->ecorr); cudaFree(g->tailpack);
   cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
   cudaFree(g->st); cudaFree(g->d_counts);
   if (g->hst) cudaFreeHost((void *)g->hst);
@@ -51,7 +51,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->nx = nx; g->ny = ny; g->nz = nz; g->dx = dx; g->dt_over_rho = 1.0f;
   for (int f = 0; f < 6; ++f) { g->bc_type[f] = NF_BC_CLOSED; g->bc_val[f] = 0.0f; }
   g->stream = 0;
-  g->nu_pre = 1; g->nu_post = 1; g->refine = 0; g->force_generic = false;
+  g->nu_pre = 1; g->nu_post = 1; g->refine = 0; g->force_generic = false; g->refresh = true;
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->nact = 0;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
@@ -94,7 +94,8 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   ok = ok && dalloc(&g->us, nf_nu(g)) == cudaSuccess && dalloc(&g->vs, nf_nv(g)) == cudaSuccess &&
        dalloc(&g->ws, nf_nw(g)) == cudaSuccess && dalloc(&g->sdf, nf_nn(g)) == cudaSuccess;
   ok = ok && dalloc(&g->p, nc) == cudaSuccess && dalloc(&g->q, nc) == cudaSuccess &&
-       dalloc(&g->xtmp, nc) == cudaSuccess && dalloc(&g->p2, nc) == cudaSuccess;
+       dalloc(&g->xtmp, nc) == cudaSuccess && dalloc(&g->p2, nc) == cudaSuccess &&
+       dalloc(&g->b0, nc) == cudaSuccess && dalloc(&g->ecorr, nc) == cudaSuccess;
   ok = ok && dalloc(&g->fu, nf_nu(g)) == cudaSuccess && dalloc(&g->fv, nf_nv(g)) == cudaSuccess &&
        dalloc(&g->fw, nf_nw(g)) == cudaSuccess;
   ok = ok && dalloc(&g->st, 1) == cudaSuccess && dalloc(&g->d_counts, 2) == cudaSuccess;
@@ -152,8 +153,8 @@ extern "C" int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value) {
 
 extern "C" int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags) {
   NF_CHECK_HANDLE(g);
-  if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || flags < 0 || flags > 3) return NF_ERR_INVALID;
-  g->nu_pre = nu_pre; g->nu_post = nu_post; g->refine = flags & 1; g->force_generic = (flags & 2) != 0;
+  if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || flags < 0 || flags > 7) return NF_ERR_INVALID;
+  g->nu_pre = nu_pre; g->nu_post = nu_post; g->refine = flags & 1; g->force_generic = (flags & 2) != 0; g->refresh = (flags & 4) == 0;
   return NF_OK;
 }
 

@@ -60,8 +60,9 @@ static inline NfLvK nf_lvk(const NfLevel &L) {
 struct alignas(128) NfSolveState {
   int iter, maxit, done, converged;
   unsigned ticket;  // CTAs of k_cg_update that have finished (the last one runs the convergence check)
+  int last_slot;    // parity slot of the last executed iteration of the current phase (-1: none)
   double bb;    // ||b||^2 after masking / mean removal
-  double tol2;  // tol^2
+  double tol2;  // (tolerance of the current phase)^2
   double relres;  // sqrt(rr/bb) at the last executed iteration
   alignas(128) double pq[2];
   alignas(128) double rr[2];
@@ -99,10 +100,13 @@ struct nf_grid {
   int singular;
   long long nact;
   int nu_pre, nu_post, refine;
+  bool refresh;  // true-residual refresh between two PCG phases (default on; flag 4 of nf_set_solver_options: off)
   bool force_generic;  // test hook: run the generic (fp32-weight, one colour per launch) kernels everywhere
   // solid velocity (MAC layout, closed walls at rest) and the last SDF
   float *us, *vs, *ws, *sdf;
   // CG vectors on level 0 (r and z live in lv[0])
+  float *ecorr;  // correction vector of the second PCG phase
+  float *b0;  // the prepared right-hand side (kept for the true-residual refresh, nf_solver.cu)
   float *p, *p2, *q, *xtmp;  // p / p2: the search direction ping-pongs between two buffers (k_papply4)
   float *tailpack;  // 8 floats per cell of the tail levels (nf_mg.cu)
   // scratch face arrays (advection copy / adjoint staging)

@@ -411,6 +411,7 @@ __global__ void __launch_bounds__(256) k_dot_rz(const float *__restrict__ a, con
 // faces towards the outside of the grid zeroed, col[n] = (i+j+k) & 1 as float.  8n floats per level.
 struct NfTailK {
   int nlev, sweeps;
+  int singular;  // the system has the constant null vector (R12): the coarsest solve works in its complement
   int n[NF_MAX_LEVELS], nx[NF_MAX_LEVELS], ny[NF_MAX_LEVELS], nz[NF_MAX_LEVELS];
   int off[NF_MAX_LEVELS];  // offset (in cells) of the level in the packed arrays
 };
@@ -462,6 +463,26 @@ __device__ __forceinline__ void nf_tail_half(float *__restrict__ z, const float 
     z[id] = a * pk[id];
   }
   __syncthreads();
+}
+
+// v -= mean of v over the active cells (pk[id] > 0), on the active cells.  Warp 0 only; caller syncs around it.
+__device__ __forceinline__ void nf_tail_project_warp(float *v, const float *pk, int n) {
+  const int lane = threadIdx.x;
+  float s = 0.0f, c = 0.0f;
+  for (int id = lane; id < n; id += 32)
+    if (pk[id] > 0.0f) {
+      s += v[id];
+      c += 1.0f;
+    }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s += __shfl_xor_sync(0xffffffffu, s, o);
+    c += __shfl_xor_sync(0xffffffffu, c, o);
+  }
+  const float m = c > 0.0f ? s / c : 0.0f;
+  for (int id = lane; id < n; id += 32)
+    if (pk[id] > 0.0f) v[id] -= m;
+  __syncwarp();
 }
 
 // Coarsest level (n <= 64 cells) by ONE warp with its operator in registers: lane l owns cells l and l + 32; `sweeps`
@@ -609,6 +630,14 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
     const int l = nl - 1;
     const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
     float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
+    // Singular system: the restricted residual is compatible (zero sum over the active cells) only up to rounding,
+    // and the many sweeps below would amplify what is left into a huge constant in z (which, prolonged, ends up
+    // dominating the search direction: PCG then stalls near 1e-5 and diverges).  Solve in the complement of the
+    // constant: project r before and z after (P M_c P stays symmetric).
+    if (T.singular) {
+      if (threadIdx.x < 32) nf_tail_project_warp(r, pk, n);
+      __syncthreads();
+    }
     if (n > 256) {  // (a one-level tail: the CTA-wide sweeps)
       for (int s = 0; s < T.sweeps; ++s) {
         nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, s == 0);
@@ -631,6 +660,10 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
       }
     }
     __syncthreads();
+    if (T.singular) {
+      if (threadIdx.x < 32) nf_tail_project_warp(z, pk, n);
+      __syncthreads();
+    }
   }
   // up
   for (int l = nl - 2; l >= 0; --l) {
@@ -862,6 +895,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
       if (l == nl - 1) m = L.nx > L.ny ? (L.nx > L.nz ? L.nx : L.nz) : (L.ny > L.nz ? L.ny : L.nz);
     }
     P.T.sweeps = 2 * m;
+    P.T.singular = g->singular;
     P.pack = g->tailpack;
     const NfSolveState *stc = st;
     void *args[] = {(void *)&P, (void *)&stc};
@@ -878,6 +912,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
       if (l == nl - 1) m = L.nx > L.ny ? (L.nx > L.nz ? L.nx : L.nz) : (L.ny > L.nz ? L.ny : L.nz);
     }
     T.sweeps = 2 * m;
+    T.singular = g->singular;
     NfLevel &F = g->lv[g->tail];
     NF_LAUNCH(g, NFK_BOTTOM, k_tail<<<1, NF_TAIL_THREADS, tail_smem_bytes(g), g->stream>>>(T, g->tailpack, F.r, F.z, st));
   } else {  // coarsest level too large for one CTA (odd extents): a few symmetric sweeps in global memory

@@ -9,6 +9,7 @@
 
 #define NF_VEC_BLOCKS (148 * 8)
 #define NF_LOOKAHEAD 2
+#define NF_REFRESH_FACTOR 30.0f  // phase 1 of a solve stops at 30 tol; then r = b - A x afresh (k_phase_begin)  // phase 1 of a solve stops here; then r = b - A x afresh (k_phase_begin)
 
 // ------------------------------------------------------------------------------------------------------------
 // a-3  q = A p = c (sum_f alpha_f (p - p_nb)), fused p.q partial sums
@@ -27,8 +28,9 @@ __global__ void __launch_bounds__(256) k_apply_A(const float *__restrict__ p, co
     const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
     const size_t id = ((size_t)k * ny + j) * nx + i;
     const float pc = p[id];
-    const float d = ((w.xl + w.xh) + (w.yl + w.yh)) + (w.zl + w.zh);
-    const float qv = c * (d * pc - nf_nb_sum(p, w, i, j, k, nx, ny, nz));
+    // difference form sum_f alpha_f (p - p_nb): a constant (or pocket-wise constant) part of p cancels exactly
+    // instead of leaving 6 ulp(p) of noise, which on singular / weakly connected systems is what stops PCG near 1e-5
+    const float qv = c * nf_nb_diff(p, w, pc, i, j, k, nx, ny, nz);
     q[id] = qv;
     part = (double)pc * (double)qv;
   }
@@ -65,13 +67,13 @@ __global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restr
 #pragma unroll
       for (int t = 0; t < 4; ++t) {
         const float l = t > 0 ? pc[t - 1] : xl, h = t < 3 ? pc[t + 1] : xh;
+        const float c0 = pc[t];  // (difference form: see k_apply_A)
         if (open4) {
-          const float s = ((l + h) + (yl[t] + yh[t])) + (zl[t] + zh[t]);
-          out[t] = L.c * (6.0f * pc[t] - s);
+          out[t] = L.c * ((((c0 - l) + (c0 - h)) + ((c0 - yl[t]) + (c0 - yh[t]))) + ((c0 - zl[t]) + (c0 - zh[t])));
         } else {
           const NfW6 w = nf_code_w6(L, nf_code_at(c4, t), i0 + t, j, k);
-          const float s = ((w.xl * l + w.xh * h) + (w.yl * yl[t] + w.yh * yh[t])) + (w.zl * zl[t] + w.zh * zh[t]);
-          out[t] = L.c * (nf_w6_sum(w) * pc[t] - s);
+          out[t] = L.c * (((w.xl * (c0 - l) + w.xh * (c0 - h)) + (w.yl * (c0 - yl[t]) + w.yh * (c0 - yh[t]))) +
+                          (w.zl * (c0 - zl[t]) + w.zh * (c0 - zh[t])));
         }
         part += pc[t] * out[t];
       }
@@ -150,13 +152,13 @@ __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__rest
 #pragma unroll
       for (int t = 0; t < 4; ++t) {
         const float l = t > 0 ? pc[t - 1] : xl, h = t < 3 ? pc[t + 1] : xh;
+        const float c0 = pc[t];  // (difference form: see k_apply_A)
         if (open4) {
-          const float s = ((l + h) + (yl[t] + yh[t])) + (zl[t] + zh[t]);
-          out[t] = L.c * (6.0f * pc[t] - s);
+          out[t] = L.c * ((((c0 - l) + (c0 - h)) + ((c0 - yl[t]) + (c0 - yh[t]))) + ((c0 - zl[t]) + (c0 - zh[t])));
         } else {
           const NfW6 w = nf_code_w6(L, nf_code_at(c4, t), i0 + t, j, k);
-          const float s = ((w.xl * l + w.xh * h) + (w.yl * yl[t] + w.yh * yh[t])) + (w.zl * zl[t] + w.zh * zh[t]);
-          out[t] = L.c * (nf_w6_sum(w) * pc[t] - s);
+          out[t] = L.c * (((w.xl * (c0 - l) + w.xh * (c0 - h)) + (w.yl * (c0 - yl[t]) + w.yh * (c0 - yh[t]))) +
+                          (w.zl * (c0 - zl[t]) + w.zh * (c0 - zh[t])));
         }
         part += pc[t] * out[t];
       }
@@ -177,6 +179,7 @@ __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__rest
 __device__ __forceinline__ void nf_cg_check(NfSolveState *st, int slot, NfHostStatus *hs, int seq) {
   if (!st->done) {
     st->iter += 1;
+    st->last_slot = slot;
     const double rr = *(volatile double *)&st->rr[slot];
     if (!(rr == rr) || rr <= st->tol2 * st->bb) {
       st->done = 1;
@@ -252,12 +255,11 @@ __global__ void __launch_bounds__(256) k_cg_update(float *__restrict__ x, float 
 }
 
 // The x update of the LAST executed iteration (fused path: every other one rode on the next k_papply4).
-// p0 / p1: the ping-pong buffers; iteration i wrote p' into p(i & 1) and its scalars into slot i & 1.
+// p0 / p1: the ping-pong buffers; the iteration with parity slot s wrote p' into p_s and its scalars into slot s.
 __global__ void __launch_bounds__(256) k_x_final(float *__restrict__ x, const float *__restrict__ p0,
                                                  const float *__restrict__ p1, size_t n, const NfSolveState *st) {
-  const int it = st->iter - 1;
-  if (it < 0) return;
-  const int slot = it & 1;
+  const int slot = st->last_slot;
+  if (slot < 0) return;
   const double pq = st->pq[slot];
   const float a = pq > 0.0 ? (float)(st->rz[slot] / pq) : 0.0f;
   const float4 *p4 = (const float4 *)(slot ? p1 : p0);
@@ -373,6 +375,7 @@ __global__ void k_init_state(NfSolveState *st, double tol, int maxit) {
   st->relres = 0.0;
   st->iter = 0;
   st->ticket = 0;
+  st->last_slot = -1;
   st->maxit = maxit;
   st->done = 0;
   st->converged = 0;
@@ -385,6 +388,79 @@ __global__ void k_start_state(NfSolveState *st) {
     st->done = 1;
     st->converged = (st->bb == 0.0) ? 1 : 0;
   }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// true-residual refresh (fp32 recursion drift, SURVEY.md 7.3-1 / DESIGN.md section 7)
+// ------------------------------------------------------------------------------------------------------------
+// The recursive residual r -= a q drifts away from b - A x by the rounding of ~30 updates of an O(1) pressure: at
+// 256^3 the channel-gate solve stops at a recursive 1e-6 with a TRUE residual of 4e-5,
+// while the exact solution rounded to fp32 already has ~6e-6.  So the solve runs in two phases: PCG
+// to 30 tol, then r = b - A x evaluated afresh in fp64, then PCG on that residual for a correction e (accumulated on
+// its own, x += e once) down to the requested tolerance.  Measured: 32 iterations instead of 31, true residual
+// 7.3e-6 = the fp32 storage floor of p.  The phase boundary is the only host synchronisation inside a solve.
+__global__ void k_phase_begin(NfSolveState *st, double tol, int keep_done) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  st->tol2 = tol * tol;
+  st->pq[0] = st->pq[1] = 0.0;
+  st->rr[0] = st->rr[1] = 0.0;
+  st->rz[0] = st->rz[1] = 0.0;
+  st->ticket = 0;
+  st->last_slot = -1;
+  if (!keep_done) {
+    st->done = 0;
+    st->converged = 0;
+  }
+}
+// r = b0 - A x evaluated in fp64 from the fp32 data (one pass per solve: the fp32 evaluation of A x cancels
+// 6 p - sum p_nb to ~6 ulp(p) c, which for an O(1) pressure is already above a 1e-6 residual); rr[0] += r.r
+__global__ void __launch_bounds__(256) k_true_residual(float *__restrict__ r, const float *__restrict__ b0,
+                                                       const float *__restrict__ x, const float *__restrict__ ax,
+                                                       const float *__restrict__ ay, const float *__restrict__ az,
+                                                       float c, int nx, int ny, int nz, int pax, NfSolveState *st) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  double part = 0.0;
+  if (i < nx && j < ny && k < nz) {
+    const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
+    const nf_idx id = ((nf_idx)k * ny + j) * nx + i, sy = nx, sz = (nf_idx)nx * ny;
+    const double pc = x[id];
+    double s = 0.0;
+    s += (double)w.xl * (pc - (i > 0 ? (double)x[id - 1] : 0.0));
+    s += (double)w.xh * (pc - (i + 1 < nx ? (double)x[id + 1] : 0.0));
+    s += (double)w.yl * (pc - (j > 0 ? (double)x[id - sy] : 0.0));
+    s += (double)w.yh * (pc - (j + 1 < ny ? (double)x[id + sy] : 0.0));
+    s += (double)w.zl * (pc - (k > 0 ? (double)x[id - sz] : 0.0));
+    s += (double)w.zh * (pc - (k + 1 < nz ? (double)x[id + sz] : 0.0));
+    const float d = nf_w6_sum(w);
+    const double v = d > 0.0f ? (double)b0[id] - (double)c * s : 0.0;
+    r[id] = (float)v;
+    part = v * v;
+  }
+  nf_block_atomic_add(part, &st->rr[0]);
+}
+// x += e
+__global__ void __launch_bounds__(256) k_add(float *__restrict__ x, const float *__restrict__ e, size_t n) {
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = tid; t < n; t += nth) x[t] += e[t];
+}
+// decide from the TRUE residual in rr[0] whether the solve is finished at tolerance `tol`; publish; clear rr[0]
+__global__ void k_phase_check(NfSolveState *st, double tol, NfHostStatus *hs, int seq) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const double rr = st->rr[0];
+  st->relres = st->bb > 0.0 ? sqrt(rr / st->bb) : 0.0;
+  const bool bad = !(rr == rr);
+  st->done = (bad || rr <= tol * tol * st->bb || st->iter >= st->maxit) ? 1 : 0;
+  st->converged = (!bad && rr <= tol * tol * st->bb) ? 1 : 0;
+  st->rr[0] = 0.0;
+  hs->relres = (float)st->relres;
+  hs->iter = st->iter;
+  hs->done = st->done;
+  hs->converged = st->converged;
+  __threadfence_system();
+  hs->seq = seq;
+  __threadfence_system();
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -437,6 +513,7 @@ int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit) {
   NF_LAUNCH(g, NFK_SETUP, k_sub_mean<<<d.grid, d.block, 0, g->stream>>>(L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv,
                                                 g->singular, &g->st->bb));
   NF_LAUNCH(g, NFK_SETUP, k_start_state<<<1, 32, 0, g->stream>>>(g->st));
+  NF_CUDA(g, cudaMemcpyAsync(g->b0, L.r, (size_t)L.ncell * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -467,24 +544,20 @@ static int wait_seq(nf_grid *g, int idx, int expect) {
   return NF_OK;
 }
 
-// MGPCG on A x = lv[0].r (prepared).  x is overwritten.
-int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
-  (void)tol;
+// One PCG phase on the residual in lv[0].r: V-cycle, then iterations until the device sets `done` (criterion:
+// st->tol2) or maxit.  x accumulates.  Returns after every enqueued check has reported (hst drained).
+struct NfPhaseOut {
+  int converged, iters;
+  float relres;
+};
+static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, NfPhaseOut *out) {
   NfLevel &L = g->lv[0];
   const size_t n = (size_t)L.ncell;
-  NfDims dc = nf_dims(L.nx, L.ny, L.nz);
-  const int v4 = vec_ok(x, L.r, g->p, g->q, n) && vec_ok(L.z, L.z, L.z, L.z, n);
   for (int s = 0; s < NF_RING; ++s) g->hst[s].seq = 0;
-  NF_CUDA(g, cudaMemsetAsync(x, 0, n * sizeof(float), g->stream));
   int rc = nf_vcycle_impl(g, true, 0);
   if (rc != NF_OK) return rc;
-  // fused path: p' = z + beta p folded into the A-apply (p ping-pongs between g->p and g->p2), convergence check
-  // folded into the x / r update
-  const bool fusedp = !g->force_generic && apply_vec_ok(L, g->p, g->q) && apply_vec_ok(L, g->p2, L.z) &&
-                      apply_vec_ok(L, x, x) && (n & 3) == 0;
   if (!fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, 0, 1));
-  int it = 0, last_seen = -1, done = 0, converged = 0;
-  float relres = 0.0f;
+  int it = 0, last_seen = -1, done = 0;
   if (maxit < 1) maxit = 1;
   for (it = 0; it < maxit && !done; ++it) {
     const int slot = it & 1;
@@ -522,19 +595,60 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
       h->seq = 0;
     }
   }
+  // the x update of the last executed iteration (every other one rode on the following k_papply4)
   if (fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->p, g->p2, n, g->st));
-  // drain: every enqueued check kernel must have reported before the ring is reused
+  // drain: every enqueued check must have reported before the ring is reused
   const int enq = it;  // checks enqueued: 0 .. enq-1
   for (int s = last_seen + 1; s < enq; ++s) {
     rc = wait_seq(g, s, s + 1);
     if (rc != NF_OK) return rc;
   }
-  {
-    NfHostStatus *h = &g->hst[(enq - 1) & (NF_RING - 1)];
-    converged = h->converged;
-    relres = h->relres;
-    g->last_iters = h->iter;
+  const NfHostStatus *h = &g->hst[(enq - 1) & (NF_RING - 1)];
+  out->converged = h->converged;
+  out->relres = h->relres;
+  out->iters = h->iter;
+  return NF_OK;
+}
+
+// MGPCG on A x = lv[0].r (prepared; a copy of it is in g->b0).  x is overwritten.
+int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
+  NfLevel &L = g->lv[0];
+  const size_t n = (size_t)L.ncell;
+  NfDims dc = nf_dims(L.nx, L.ny, L.nz);
+  const int v4 = vec_ok(x, L.r, g->p, g->q, n) && vec_ok(L.z, L.z, L.z, L.z, n);
+  // fused path: p' = z + beta p folded into the A-apply (p ping-pongs between g->p and g->p2), convergence check
+  // folded into the x / r update
+  const bool fusedp = !g->force_generic && apply_vec_ok(L, g->p, g->q) && apply_vec_ok(L, g->p2, L.z) &&
+                      apply_vec_ok(L, x, x) && (n & 3) == 0;
+  NF_CUDA(g, cudaMemsetAsync(x, 0, n * sizeof(float), g->stream));
+  // phase 1 stops at 30 tol (see k_phase_begin's comment)
+  const float tol1 = NF_REFRESH_FACTOR * tol;
+  const bool two_phase = tol1 < 1e-2f && g->refresh;
+  NfPhaseOut ph;
+  NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)(two_phase ? tol1 : tol), 1));
+  int rc = run_pcg_phase(g, x, maxit, fusedp, v4, &ph);
+  if (rc != NF_OK) return rc;
+  if (two_phase && ph.converged && ph.iters > 0 && ph.iters < maxit) {
+    // r = b - A x afresh (fp64 evaluation), decide, and if needed run PCG on it for a correction e; x += e
+    NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)tol, 0));
+    NF_LAUNCH(g, NFK_SETUP, k_true_residual<<<dc.grid, dc.block, 0, g->stream>>>(L.r, g->b0, x, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->st));
+    g->hst[0].seq = 0;
+    NF_LAUNCH(g, NFK_SETUP, k_phase_check<<<1, 32, 0, g->stream>>>(g->st, (double)tol, &g->hst_dev[0], 1));
+    NF_CUDA(g, cudaGetLastError());
+    rc = wait_seq(g, 0, 1);
+    if (rc != NF_OK) return rc;
+    ph.converged = g->hst[0].converged;
+    ph.relres = g->hst[0].relres;
+    if (!g->hst[0].done) {
+      // (the correction is ~1e-3 of x: accumulated on its own its rounding is invisible, and x is rounded once)
+      NF_CUDA(g, cudaMemsetAsync(g->ecorr, 0, n * sizeof(float), g->stream));
+      const bool fusede = fusedp && apply_vec_ok(L, g->ecorr, g->ecorr);
+      rc = run_pcg_phase(g, g->ecorr, maxit - ph.iters, fusede, v4, &ph);
+      if (rc != NF_OK) return rc;
+      NF_LAUNCH(g, NFK_SETUP, k_add<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->ecorr, n));
+    }
   }
+  g->last_iters = ph.iters;
   // gauge: zero mean over active cells on a singular system (R12)
   if (g->singular) {
     NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<dc.grid, dc.block, 0, g->stream>>>(x, x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum));
@@ -543,7 +657,6 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
                                                     nullptr));
   }
   NF_CUDA(g, cudaGetLastError());
-  // iteration count: read back from the device state lazily in nf_last_solve_info; keep the host view here
-  g->last_relres = relres;
-  return converged ? NF_OK : NF_NOT_CONVERGED;
+  g->last_relres = ph.relres;
+  return ph.converged ? NF_OK : NF_NOT_CONVERGED;
 }

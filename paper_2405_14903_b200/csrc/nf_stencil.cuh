@@ -42,6 +42,20 @@ __device__ __forceinline__ float nf_nb_sum(const float *__restrict__ v, const Nf
   return s;
 }
 
+// sum over the six faces of alpha_f * (pc - v_nb) with homogeneous ghosts
+__device__ __forceinline__ float nf_nb_diff(const float *__restrict__ v, const NfW6 &w, float pc, int i, int j, int k,
+                                            int nx, int ny, int nz) {
+  const nf_idx id = ((nf_idx)k * ny + j) * nx + i;
+  const nf_idx sy = nx, sz = (nf_idx)nx * ny;
+  float s = w.xl * (pc - (i > 0 ? v[id - 1] : 0.0f));
+  s += w.xh * (pc - (i + 1 < nx ? v[id + 1] : 0.0f));
+  s += w.yl * (pc - (j > 0 ? v[id - sy] : 0.0f));
+  s += w.yh * (pc - (j + 1 < ny ? v[id + sy] : 0.0f));
+  s += w.zl * (pc - (k > 0 ? v[id - sz] : 0.0f));
+  s += w.zh * (pc - (k + 1 < nz ? v[id + sz] : 0.0f));
+  return s;
+}
+
 // ---- cell-code path ------------------------------------------------------------------------------------------
 // The six weights of cell (i,j,k) whose code is `code`: exactly 0.0f / 1.0f from the bits of a pure cell, the fp32
 // arrays for a mixed cell (rare: O(n^2) cells).

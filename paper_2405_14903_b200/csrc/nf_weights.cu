@@ -10,7 +10,7 @@
 template <bool GRAD>
 __device__ __forceinline__ float nf_tri(float a, float b, float d, float &da, float &db, float &dd) {
   const float iab = 1.0f / (a - b), iad = 1.0f / (a - d);
-  const float fb = a * iab, fd = a * iad;
+  const float fb = a / (a - b), fd = a / (a - d);  // (true divisions: x / (x - 0) must be exactly 1)
   if (GRAD) {
     const float fb_a = -b * iab * iab, fb_b = a * iab * iab;
     const float fd_a = -d * iad * iad, fd_d = a * iad * iad;
@@ -57,7 +57,7 @@ __device__ __forceinline__ float nf_area_fraction(const float P0, const float P1
         adjacent = true;
         const float A = P[q], B = P[q1], C = P[q2], D = P[q3];
         const float iad = 1.0f / (A - D), ibc = 1.0f / (B - C);
-        out = 0.5f * (A * iad + B * ibc);
+        out = 0.5f * (A / (A - D) + B / (B - C));
         if (GRAD) {
           g[q] = 0.5f * (-D * iad * iad);
           g[q3] = 0.5f * (A * iad * iad);

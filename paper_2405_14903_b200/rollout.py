@@ -1,0 +1,45 @@
+"""Full time steps forward and backward through the C ABI (PAPER.md:L78 forward order, L111-141 backward pass):
+per step  nf_advect -> nf_set_solid(phi^{n+1}, u_s^{n+1}) -> nf_project,  and in reverse
+nf_project_adjoint -> nf_weights_adjoint -> nf_advect_adjoint, with the per-step state (U^n, Uhat, p) kept by the
+caller instead of an autodiff graph.  Argument marshalling and the two inner products of the geometry
+chain rule only: every step of the path runs in the library's kernels."""
+import torch
+
+
+def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect_on=True):
+    """solid_fn(step) -> (phi, (us, vs, ws), dphi_dtheta, (dus, dvs, dws)) as CUDA float32 tensors (the derivative
+    tensors may be None); loss_fn(U) -> (J tensor, [dJ/du, dJ/dv, dJ/dw]).
+    Returns (J, dJ/dtheta, dJ/dU0) -- J and dJ/dtheta as Python floats."""
+    g = grid
+    U = [a.clone() for a in U0]
+    tape = []
+    for n in range(1, nsteps + 1):
+        Uprev = [a.clone() for a in U]
+        if advect_on:
+            g.advect(*U, dt)
+        phi, us, dphi, dus = solid_fn(n)
+        g.set_solid(phi, *us)
+        Uhat = [a.clone() for a in U]
+        p = torch.empty(g.shape_p, dtype=torch.float32, device=U[0].device)
+        g.project(*U, p, tol=tol, maxit=maxit)
+        tape.append((Uprev, Uhat, p, phi, us, dphi, dus))
+    J, G = loss_fn(U)
+    G = [a.clone() for a in G]
+    dtheta = torch.zeros((), dtype=torch.float64, device=U[0].device)
+    ga = [torch.empty_like(a) for a in U]
+    gs = [torch.empty_like(a) for a in U]
+    gphi = torch.empty(g.shape_sdf, dtype=torch.float32, device=U[0].device)
+    for n in range(nsteps, 0, -1):
+        Uprev, Uhat, p, phi, us, dphi, dus = tape[n - 1]
+        g.set_solid(phi, *us)  # the hierarchy of step n (the handle holds one geometry at a time)
+        g.project_adjoint(*G, p_saved=p, uhat=Uhat, galpha=ga, gus=gs, tol=tol, maxit=maxit)
+        g.weights_adjoint(*ga, gphi)
+        if dphi is not None:
+            dtheta += (gphi.double() * dphi.double()).sum()
+        if dus is not None:
+            for a, b in zip(gs, dus):
+                if b is not None:
+                    dtheta += (a.double() * b.double()).sum()
+        if advect_on:
+            g.advect_adjoint(*Uprev, *G, dt)
+    return float(J), float(dtheta), G
