@@ -173,23 +173,20 @@ def run_ours(args):
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2405_14903_b200 import api
+    from paper_2405_14903_b200 import api, replicas
     api.load_library()  # fail loudly if the CUDA extension is missing: there is no fallback
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = replicas.rank_world()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device")
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     n, K, W = args.n, args.steps, max(args.warmup, 3)
-    wlk = GateWorkload(n, min(K + W, 20), seed_shift=rank)
+    wlk = GateWorkload(n, min(K + W, 20), seed_shift=replicas.seed_shift(rank))
     g = wlk.g
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier(dist)
         torch.cuda.synchronize()
 
     for _ in range(W):
@@ -209,12 +206,9 @@ def run_ours(args):
     ms_total = e0.elapsed_time(e1)
     launches = g.launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
+    ms_total = replicas.max_over_ranks(ms_total, dist, device="cuda")
     ms_per_step = ms_total / K
-    value = ms_total / (K * world)
+    value = replicas.job_value_ms(ms_total, K, world)
 
     # ---- extra (untimed-for-the-headline) passes: projection share, iteration counts, per-kernel roofline ----
     nrec = min(K, 3)
@@ -229,6 +223,7 @@ def run_ours(args):
     ncell = n ** 3
     peak, peak_src = _peaks()
     # algorithmic bytes per fine cell per launch (DESIGN.md section 8 / SURVEY.md 8d.2), fp32
+    # fused p-update + A-apply + deferred x update: z, p, x, code in; p', q, x out = 25; r update: r, q in, r out = 12
     BYTES = {"apply_A": 25.0, "cg_update": 12.0, "cg_pupdate": 12.0, "down1_fine": 9.0, "down2_fine": 5.5,
              "up1_fine": 13.5, "up2_fine": 13.0, "rbgs_fine": 24.0, "restrict_fine": 20.5, "prolong_fine": 8.5}
     kern = {}
@@ -241,8 +236,18 @@ def run_ours(args):
             kk["frac_of_peak"] = round(kk["gbs"] / peak, 3)
         kern[name] = kk
     dom = max((k for k in kern if k in BYTES), key=lambda k: kern[k]["ms_total"])
+    # dram bytes per launch of that kernel from the committed ncu --set full capture (profiles/, 256^3 only)
+    traffic = None
+    try:
+        if n == 256:
+            with open(os.path.join(ROOT, "profiles", "r1_v4_traffic.json")) as f:
+                tr = json.load(f)
+            traffic = tr.get({"apply_A": "k_papply4", "cg_update": "k_cg_update", "down1_fine": "k_down1",
+                              "down2_fine": "k_down2", "up1_fine": "k_up1", "up2_fine": "k_up2"}.get(dom, ""))
+    except Exception:
+        traffic = None
     roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
-            "frac": round(kern[dom]["gbs"] / peak, 4), "traffic": None, "peak_source": peak_src,
+            "frac": round(kern[dom]["gbs"] / peak, 4), "traffic": traffic, "peak_source": peak_src,
             "algorithmic_bytes_per_cell": BYTES[dom], "cells_per_launch": ncell,
             "share_of_step": round(kern[dom]["ms_total"] / sum(v["ms_total"] for v in kern.values()), 3)}
     its = wlk.iters
