@@ -364,6 +364,43 @@ __global__ void __launch_bounds__(256) k_sub_mean(float *__restrict__ r, const f
   if (sq) nf_block_atomic_add(part, sq);
 }
 
+// The same two steps on float4 rows with the active mask taken from the 1-byte cell codes (code != 0 <=> active):
+// pass 1: dst = mask(src) (also into dst2 if given), sum += dst, sq += dst^2;  pass 2 (singular systems only):
+// dst -= sum / #active on the active cells (also into dst2), sq += dst^2.
+__global__ void __launch_bounds__(256) k_mask4(const float *src, float *dst, float *dst2,
+                                               const uint8_t *__restrict__ code, size_t n4, double *sum, double *sq) {
+  double s = 0.0, q = 0.0;
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = tid; t < n4; t += nth) {
+    float4 v = reinterpret_cast<const float4 *>(src)[t];
+    const unsigned c = __ldg(reinterpret_cast<const unsigned *>(code) + t);
+    v.x = (c & 0xffu) ? v.x : 0.0f; v.y = (c & 0xff00u) ? v.y : 0.0f;
+    v.z = (c & 0xff0000u) ? v.z : 0.0f; v.w = (c & 0xff000000u) ? v.w : 0.0f;
+    reinterpret_cast<float4 *>(dst)[t] = v;
+    if (dst2) reinterpret_cast<float4 *>(dst2)[t] = v;
+    s += ((double)v.x + v.y) + ((double)v.z + v.w);
+    q += ((double)v.x * v.x + (double)v.y * v.y) + ((double)v.z * v.z + (double)v.w * v.w);
+  }
+  if (sum) nf_block_atomic_add(s, sum);
+  if (sq) nf_block_atomic_add(q, sq);
+}
+__global__ void __launch_bounds__(256) k_center4(float *dst, float *dst2, const uint8_t *__restrict__ code, size_t n4,
+                                                 const double *sum, double inv_nact, double *sq) {
+  const float m = (float)((*sum) * inv_nact);
+  double q = 0.0;
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = tid; t < n4; t += nth) {
+    float4 v = reinterpret_cast<const float4 *>(dst)[t];
+    const unsigned c = __ldg(reinterpret_cast<const unsigned *>(code) + t);
+    v.x -= (c & 0xffu) ? m : 0.0f; v.y -= (c & 0xff00u) ? m : 0.0f;
+    v.z -= (c & 0xff0000u) ? m : 0.0f; v.w -= (c & 0xff000000u) ? m : 0.0f;
+    reinterpret_cast<float4 *>(dst)[t] = v;
+    if (dst2) reinterpret_cast<float4 *>(dst2)[t] = v;
+    q += ((double)v.x * v.x + (double)v.y * v.y) + ((double)v.z * v.z + (double)v.w * v.w);
+  }
+  if (sq) nf_block_atomic_add(q, sq);
+}
+
 __global__ void k_init_state(NfSolveState *st, double tol, int maxit) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   st->pq[0] = st->pq[1] = 0.0;
@@ -507,13 +544,24 @@ int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit) {
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(L.nx, L.ny, L.nz);
   NF_LAUNCH(g, NFK_SETUP, k_init_state<<<1, 32, 0, g->stream>>>(g->st, (double)tol, maxit));
-  NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<d.grid, d.block, 0, g->stream>>>(src ? src : L.r, L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax,
-                                                &g->st->sum));
   const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
-  NF_LAUNCH(g, NFK_SETUP, k_sub_mean<<<d.grid, d.block, 0, g->stream>>>(L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv,
-                                                g->singular, &g->st->bb));
-  NF_LAUNCH(g, NFK_SETUP, k_start_state<<<1, 32, 0, g->stream>>>(g->st));
-  NF_CUDA(g, cudaMemcpyAsync(g->b0, L.r, (size_t)L.ncell * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
+  const float *in = src ? src : L.r;
+  const size_t n = (size_t)L.ncell;
+  if (!g->force_generic && vec_ok(in, L.r, g->b0, g->b0, n)) {
+    if (!g->singular) {
+      NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(in, L.r, g->b0, L.code, n >> 2, nullptr, &g->st->bb));
+    } else {
+      NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(in, L.r, nullptr, L.code, n >> 2, &g->st->sum, nullptr));
+      NF_LAUNCH(g, NFK_SETUP, k_center4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(L.r, g->b0, L.code, n >> 2, &g->st->sum, inv, &g->st->bb));
+    }
+    NF_LAUNCH(g, NFK_SETUP, k_start_state<<<1, 32, 0, g->stream>>>(g->st));
+  } else {
+    NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<d.grid, d.block, 0, g->stream>>>(in, L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum));
+    NF_LAUNCH(g, NFK_SETUP, k_sub_mean<<<d.grid, d.block, 0, g->stream>>>(L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv,
+                                                  g->singular, &g->st->bb));
+    NF_LAUNCH(g, NFK_SETUP, k_start_state<<<1, 32, 0, g->stream>>>(g->st));
+    NF_CUDA(g, cudaMemcpyAsync(g->b0, L.r, n * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
+  }
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -650,7 +698,11 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
   }
   g->last_iters = ph.iters;
   // gauge: zero mean over active cells on a singular system (R12)
-  if (g->singular) {
+  if (g->singular && !g->force_generic && vec_ok(x, x, x, x, n)) {
+    NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, x, nullptr, L.code, n >> 2, &g->st->sum, nullptr));
+    const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
+    NF_LAUNCH(g, NFK_SETUP, k_center4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, nullptr, L.code, n >> 2, &g->st->sum, inv, nullptr));
+  } else if (g->singular) {
     NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<dc.grid, dc.block, 0, g->stream>>>(x, x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum));
     const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
     NF_LAUNCH(g, NFK_SETUP, k_sub_mean<<<dc.grid, dc.block, 0, g->stream>>>(x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv, 1,

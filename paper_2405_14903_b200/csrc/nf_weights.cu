@@ -263,15 +263,17 @@ __global__ void __launch_bounds__(256) k_coarsen_weights(const float *__restrict
 // Cell codes of one level from its fp32 weights: bits 0..5 = face is fully open, bit 6 = the
 // cell has a fractional face.  With counts != nullptr (level 0) also: counts[0] += active cells (sum of six
 // weights > 0); counts[1] += open faces on Dirichlet domain faces (R12).
+#define NF_ENC_KCH 8
 __global__ void __launch_bounds__(256) k_encode(const float *__restrict__ ax, const float *__restrict__ ay,
                                                 const float *__restrict__ az, uint8_t *__restrict__ code,
                                                 float *__restrict__ idg, float ic, int nx, int ny, int nz, int pax,
                                                 NfBc6 bc, double *__restrict__ counts) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z * blockDim.z + threadIdx.z;
   double act = 0.0, dir = 0.0;
-  if (i < nx && j < ny && k < nz) {
+  // (each CTA marches through NF_ENC_KCH planes: 8x fewer same-address fp64 atomics for the two counts)
+  for (int k = blockIdx.z * NF_ENC_KCH; k < min((int)(blockIdx.z + 1) * NF_ENC_KCH, nz); ++k)
+  if (i < nx && j < ny) {
     float w[6];
     w[0] = ax[((size_t)k * ny + j) * pax + i];
     w[1] = ax[((size_t)k * ny + j) * pax + i + 1];
@@ -294,7 +296,7 @@ __global__ void __launch_bounds__(256) k_encode(const float *__restrict__ ax, co
       idg[((size_t)k * ny + j) * nx + i] = mixed ? (d > 0.0f ? ic / d : 0.0f) : ic * inv_count[__popc(c & 63u)];
     }
     if (counts) {
-      if (w[0] + w[1] + w[2] + w[3] + w[4] + w[5] > 0.0f) act = 1.0;
+      if (w[0] + w[1] + w[2] + w[3] + w[4] + w[5] > 0.0f) act += 1.0;
       if (i == 0 && bc.t[0] == NF_BC_DIRICHLET && w[0] > 0.0f) dir += 1.0;
       if (i == nx - 1 && bc.t[1] == NF_BC_DIRICHLET && w[1] > 0.0f) dir += 1.0;
       if (j == 0 && bc.t[2] == NF_BC_DIRICHLET && w[2] > 0.0f) dir += 1.0;
@@ -388,7 +390,9 @@ int nf_build_hierarchy(nf_grid *g) {
   for (int l = 0; l < g->nlev; ++l) {
     NfLevel &L = g->lv[l];
     NfDims d = nf_dims(L.nx, L.ny, L.nz);
-    NF_LAUNCH(g, NFK_CLASSIFY, k_encode<<<d.grid, d.block, 0, g->stream>>>(L.ax, L.ay, L.az, L.code, L.idg, 1.0f / L.c, L.nx, L.ny, L.nz, L.pax, bc6(g), l == 0 ? cnt : nullptr));
+    NfDims de = nf_dims(L.nx, L.ny, 1);
+    de.grid.z = (L.nz + NF_ENC_KCH - 1) / NF_ENC_KCH;
+    NF_LAUNCH(g, NFK_CLASSIFY, k_encode<<<de.grid, de.block, 0, g->stream>>>(L.ax, L.ay, L.az, L.code, L.idg, 1.0f / L.c, L.nx, L.ny, L.nz, L.pax, bc6(g), l == 0 ? cnt : nullptr));
     if (L.vec) NF_LAUNCH(g, NFK_CLASSIFY, k_encode_deep<<<d.grid, d.block, 0, g->stream>>>(L.code, L.nx, L.ny, L.nz));
   }
   NF_CUDA(g, cudaGetLastError());
