@@ -8,6 +8,9 @@
 // stencils it reduces to (same clamping as the general interpolation) instead of three general interpolations;
 // 32-bit index arithmetic throughout (lattices have < 2^31 points).
 #include "nf_internal.cuh"
+#ifndef NF_ADJ_MINB
+#define NF_ADJ_MINB 4
+#endif
 
 struct NfLat {  // the three staggered lattices: extents and data
   const float *f[3];
@@ -155,7 +158,7 @@ __device__ __forceinline__ void nf_self_adjoint(float *__restrict__ g, const int
 
 // a-9: one thread per face of family C; gin = dJ/d(advected field) of that family; G accumulates dJ/dU^n.
 template <int C>
-__global__ void __launch_bounds__(256) k_advect_adjoint(NfLat U, NfGrad3 G, const float *__restrict__ gin, float s) {
+__global__ void __launch_bounds__(256, NF_ADJ_MINB) k_advect_adjoint(NfLat U, NfGrad3 G, const float *__restrict__ gin, float s) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z * blockDim.z + threadIdx.z;

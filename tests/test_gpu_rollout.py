@@ -63,3 +63,81 @@ def test_rollout_loss_and_gradients_match_oracle(torch, api, n, nsteps, u0_amp):
     # the generic initial velocity.
     if u0_amp > 0 and den > 0:
         assert num <= 1e-3 * den, num / den
+
+
+def _rel3(A, B):
+    num = np.sqrt(sum(np.sum((a.cpu().numpy().astype(np.float64) - b) ** 2) for a, b in zip(A, B)))
+    den = np.sqrt(sum(np.sum(np.asarray(b, np.float64) ** 2) for b in B))
+    return num / (den if den > 0 else 1.0)
+
+
+def test_chamber_pump_shape_projection_and_control_gradient(torch, api):
+    """BASELINE.json configs[2] shape at 32^3 (ellipsoid chamber + outlet tube, Dirichlet p = 0 on +x, wall-normal
+    velocity from 16 Gaussian bumps): projection and adjoint against the oracle, and the gradient of
+    J = 1/2 sum u^2 on the +x outlet faces w.r.t. the 16 bump amplitudes (u_s is linear in them: dJ/dtheta_k =
+    <dJ/dU_s, dU_s/dtheta_k>, Eq. 9b in the derived form R10) within 1e-3."""
+    n = 32
+    P = wl.config3_params(n)
+    bc = orc.BC(P["bc_types"], P["bc_values"])
+    phi, us = wl.config3_solid(P, 7)
+    alpha = orc.face_weights(phi, bc)
+    au, av, aw, _ = wl.keep_largest_component(*[a.astype(np.float32) for a in alpha])
+    alpha = [au.astype(np.float64), av.astype(np.float64), aw.astype(np.float64)]
+    U0 = [np.zeros(s, np.float32) for s in wl.face_shapes(n, n, n)]  # fluid at rest
+    Uo, po = orc.project(U0, alpha, us, P["dx"], P["dt_over_rho"], bc, tol=1e-12)
+    g_out = [np.zeros_like(a) for a in Uo]
+    g_out[0][:, :, -1] = Uo[0][:, :, -1]                               # J = 1/2 sum u^2 on the outlet faces
+    gU, gA, gS, _ = orc.project_adjoint(g_out, alpha, po, U0, us, P["dx"], P["dt_over_rho"], bc, tol=1e-12)
+    basis = [wl.config3_us_basis(P, 7, k) for k in range(16)]
+    dJo = np.array([sum(float(np.sum(a * b)) for a, b in zip(gS, bk)) for bk in basis])
+
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    g = api.Grid(n, n, n, P["dx"])
+    g.set_dt_rho(P["dt_over_rho"])
+    for f in range(6):
+        g.set_domain_bc(f, P["bc_types"][f], P["bc_values"][f])
+    g.set_weights(d(au), d(av), d(aw))
+    g.set_solid_velocity(*[d(a) for a in us])
+    U = [d(a) for a in U0]
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    assert g.project(*U, p, tol=1e-6, maxit=400) == 0
+    assert np.linalg.norm(p.cpu().numpy() - po) <= 1e-4 * np.linalg.norm(po)
+    assert _rel3(U, Uo) <= 1e-4
+    G = [torch.zeros_like(a) for a in U]
+    G[0][:, :, -1] = U[0][:, :, -1]
+    ga = [torch.empty_like(a) for a in U]
+    gs = [torch.empty_like(a) for a in U]
+    assert g.project_adjoint(*G, p_saved=p, uhat=[d(a) for a in U0], galpha=ga, gus=gs, tol=1e-6, maxit=400) == 0
+    assert _rel3(G, gU) <= 1e-4
+    assert _rel3(gs, gS) <= 1e-3
+    dJg = np.array([sum(float((a.double() * d(b).double()).sum()) for a, b in zip(gs, bk)) for bk in basis])
+    g.close()
+    assert np.linalg.norm(dJg - dJo) <= 1e-3 * np.linalg.norm(dJo), (dJg, dJo)
+
+
+def test_channel_gate_shape_full_step_matches_oracle(torch, api):
+    """BASELINE.json configs[3] shape at 48^3 (Dirichlet p = 1 / 0 on -x / +x, rotating plate, u_s = omega x r):
+    two full steps (advect, set_solid, project) against the oracle, U and p within 1e-4."""
+    n = 48
+    P = wl.config4_params(n)
+    bc = orc.BC(P["bc_types"], P["bc_values"])
+    U0 = wl.config4_initial_velocity(P)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    g = api.Grid(n, n, n, P["dx"])
+    g.set_dt_rho(P["dt_over_rho"])
+    for f in range(6):
+        g.set_domain_bc(f, P["bc_types"][f], P["bc_values"][f])
+    U = [d(a) for a in U0]
+    Uo = [a.astype(np.float64) for a in U0]
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    for step in (1, 2):
+        phi, us = wl.config4_solid(P, step)
+        g.advect(*U, P["dt"])
+        g.set_solid(d(phi), *[d(a) for a in us])
+        assert g.project(*U, p, tol=1e-6, maxit=400) == 0
+        Ut = orc.advect(Uo, P["dt"], P["dx"])
+        alpha = [a.cpu().numpy().astype(np.float64) for a in g.get_weights()]  # (weights have their own parity test)
+        Uo, po = orc.project(Ut, alpha, us, P["dx"], P["dt_over_rho"], bc, tol=1e-12)
+        assert np.linalg.norm(p.cpu().numpy() - po) <= 1e-4 * np.linalg.norm(po)
+        assert _rel3(U, Uo) <= 1e-4
+    g.close()
