@@ -51,7 +51,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->nx = nx; g->ny = ny; g->nz = nz; g->dx = dx; g->dt_over_rho = 1.0f;
   for (int f = 0; f < 6; ++f) { g->bc_type[f] = NF_BC_CLOSED; g->bc_val[f] = 0.0f; }
   g->stream = 0;
-  g->nu_pre = 1; g->nu_post = 1; g->refine = 0; g->force_generic = false; g->refresh = true;
+  g->nu_pre = 1; g->nu_post = 1; g->refine = 0; g->force_generic = false; g->refresh = true; g->warm = false;
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->nact = 0;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
@@ -153,8 +153,8 @@ extern "C" int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value) {
 
 extern "C" int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags) {
   NF_CHECK_HANDLE(g);
-  if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || flags < 0 || flags > 7) return NF_ERR_INVALID;
-  g->nu_pre = nu_pre; g->nu_post = nu_post; g->refine = flags & 1; g->force_generic = (flags & 2) != 0; g->refresh = (flags & 4) == 0;
+  if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || flags < 0 || flags > 15) return NF_ERR_INVALID;
+  g->nu_pre = nu_pre; g->nu_post = nu_post; g->refine = flags & 1; g->force_generic = (flags & 2) != 0; g->refresh = (flags & 4) == 0; g->warm = (flags & 8) != 0;
   return NF_OK;
 }
 
@@ -184,11 +184,11 @@ extern "C" int nf_set_solid_velocity(nf_grid *g, const float *us, const float *v
   return nf_store_solid_velocity(g, us, vs, ws);
 }
 
-static int solve_timed(nf_grid *g, const float *src, float *x, float tol, int maxit) {
+static int solve_timed(nf_grid *g, const float *src, float *x, float tol, int maxit, bool warm) {
   if (!(tol > 0.0f) || maxit < 1) return NF_ERR_INVALID;
   NF_CUDA(g, cudaEventRecord(g->ev0, g->stream));
   NF_TRY(nf_solve_prepare_from(g, src, tol, maxit));
-  int rc = nf_solve_run(g, x, tol, maxit);
+  int rc = nf_solve_run(g, x, tol, maxit, warm);
   if (rc < 0) return rc;
   NF_CUDA(g, cudaEventRecord(g->ev1, g->stream));
   g->last_timed = true;
@@ -199,7 +199,7 @@ extern "C" int nf_solve(nf_grid *g, const float *rhs, float *p, float tol, int m
   NF_CHECK_HANDLE(g);
   if (!rhs || !p || rhs == p) return NF_ERR_INVALID;
   if (!g->weights_set) return NF_ERR_STATE;
-  return solve_timed(g, rhs, p, tol, maxit);
+  return solve_timed(g, rhs, p, tol, maxit, g->warm);
 }
 
 extern "C" int nf_project(nf_grid *g, float *u, float *v, float *w, float *p, float tol, int maxit) {
@@ -207,7 +207,7 @@ extern "C" int nf_project(nf_grid *g, float *u, float *v, float *w, float *p, fl
   if (!u || !v || !w || !p) return NF_ERR_INVALID;
   if (!g->weights_set) return NF_ERR_STATE;
   NF_TRY(nf_rhs_impl(g, u, v, w));
-  int rc = solve_timed(g, nullptr, p, tol, maxit);
+  int rc = solve_timed(g, nullptr, p, tol, maxit, g->warm);
   if (rc < 0) return rc;
   NF_TRY(nf_grad_subtract_impl(g, u, v, w, p));
   return rc;
@@ -226,7 +226,7 @@ extern "C" int nf_project_adjoint(nf_grid *g, float *gu, float *gv, float *gw, c
   if (!g->weights_set) return NF_ERR_STATE;
   float *y = y_out ? y_out : g->xtmp;
   NF_TRY(nf_adjoint_rhs_impl(g, gu, gv, gw));
-  int rc = solve_timed(g, nullptr, y, tol, maxit);
+  int rc = solve_timed(g, nullptr, y, tol, maxit, g->warm && y_out != nullptr);  // (never from internal scratch)
   if (rc < 0) return rc;
   NF_TRY(nf_adjoint_finish_impl(g, gu, gv, gw, y, p_saved, uhat_u, uhat_v, uhat_w, galpha_u, galpha_v, galpha_w,
                                 gus_u, gus_v, gus_w));

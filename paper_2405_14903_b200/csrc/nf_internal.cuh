@@ -100,6 +100,7 @@ struct nf_grid {
   int singular;
   long long nact;
   int nu_pre, nu_post, refine;
+  bool warm;     // flag 8 of nf_set_solver_options: caller-provided solution arrays hold the initial guess
   bool refresh;  // true-residual refresh between two PCG phases (default on; flag 4 of nf_set_solver_options: off)
   bool force_generic;  // test hook: run the generic (fp32-weight, one colour per launch) kernels everywhere
   // solid velocity (MAC layout, closed walls at rest) and the last SDF
@@ -212,7 +213,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot);  // z = M^{-1} r on lv[
 int nf_solver_init(nf_grid *g);                          // kernel attributes (once per process)
 int nf_solve_prepare(nf_grid *g, float tol, int maxit);  // from lv[0].r: mask, mean removal, bb
 int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit);
-int nf_solve_run(nf_grid *g, float *x, float tol, int maxit);
+int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm);  // warm: x holds the initial guess
 // nf_project.cu
 int nf_rhs_impl(nf_grid *g, const float *u, const float *v, const float *w);  // -> lv[0].r
 int nf_grad_subtract_impl(nf_grid *g, float *u, float *v, float *w, const float *p);

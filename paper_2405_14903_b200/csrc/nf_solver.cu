@@ -477,6 +477,17 @@ __global__ void __launch_bounds__(256) k_true_residual(float *__restrict__ r, co
   }
   nf_block_atomic_add(part, &st->rr[0]);
 }
+// warm start: the initial guess on the active cells only (0 elsewhere), and 0 everywhere when b = 0 (done is then
+// already set by k_start_state: the answer is x = 0)
+__global__ void __launch_bounds__(256) k_warm_mask(float *__restrict__ x, const uint8_t *__restrict__ code, size_t n,
+                                                   const NfSolveState *st) {
+  const bool zero = st->done != 0;
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = tid; t < n; t += nth) {
+    const float v = x[t];
+    x[t] = (zero || code[t] == 0 || !(v == v)) ? 0.0f : v;
+  }
+}
 // x += e
 __global__ void __launch_bounds__(256) k_add(float *__restrict__ x, const float *__restrict__ e, size_t n) {
   const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
@@ -659,7 +670,7 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
 }
 
 // MGPCG on A x = lv[0].r (prepared; a copy of it is in g->b0).  x is overwritten.
-int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
+int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
   NfLevel &L = g->lv[0];
   const size_t n = (size_t)L.ncell;
   NfDims dc = nf_dims(L.nx, L.ny, L.nz);
@@ -668,33 +679,48 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit) {
   // folded into the x / r update
   const bool fusedp = !g->force_generic && apply_vec_ok(L, g->p, g->q) && apply_vec_ok(L, g->p2, L.z) &&
                       apply_vec_ok(L, x, x) && (n & 3) == 0;
-  NF_CUDA(g, cudaMemsetAsync(x, 0, n * sizeof(float), g->stream));
   // phase 1 stops at 30 tol (see k_phase_begin's comment)
   const float tol1 = NF_REFRESH_FACTOR * tol;
   const bool two_phase = tol1 < 1e-2f && g->refresh;
   NfPhaseOut ph;
-  NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)(two_phase ? tol1 : tol), 1));
-  int rc = run_pcg_phase(g, x, maxit, fusedp, v4, &ph);
-  if (rc != NF_OK) return rc;
-  if (two_phase && ph.converged && ph.iters > 0 && ph.iters < maxit) {
-    // r = b - A x afresh (fp64 evaluation), decide, and if needed run PCG on it for a correction e; x += e
-    NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)tol, 0));
+  ph.converged = 0; ph.iters = 0; ph.relres = 0.0f;
+  int rc = NF_OK;
+  // r = b - A x afresh (fp64 evaluation); decide at `tol`; if not done run PCG on it (phase tolerance tolp) for a
+  // correction e accumulated on its own, x += e once.  Used for the refresh and for a warm start.
+  auto correct = [&](float tolp) -> int {
+    NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)tolp, 0));
     NF_LAUNCH(g, NFK_SETUP, k_true_residual<<<dc.grid, dc.block, 0, g->stream>>>(L.r, g->b0, x, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->st));
     g->hst[0].seq = 0;
     NF_LAUNCH(g, NFK_SETUP, k_phase_check<<<1, 32, 0, g->stream>>>(g->st, (double)tol, &g->hst_dev[0], 1));
     NF_CUDA(g, cudaGetLastError());
-    rc = wait_seq(g, 0, 1);
-    if (rc != NF_OK) return rc;
+    int rcc = wait_seq(g, 0, 1);
+    if (rcc != NF_OK) return rcc;
     ph.converged = g->hst[0].converged;
     ph.relres = g->hst[0].relres;
     if (!g->hst[0].done) {
-      // (the correction is ~1e-3 of x: accumulated on its own its rounding is invisible, and x is rounded once)
       NF_CUDA(g, cudaMemsetAsync(g->ecorr, 0, n * sizeof(float), g->stream));
       const bool fusede = fusedp && apply_vec_ok(L, g->ecorr, g->ecorr);
-      rc = run_pcg_phase(g, g->ecorr, maxit - ph.iters, fusede, v4, &ph);
-      if (rc != NF_OK) return rc;
+      rcc = run_pcg_phase(g, g->ecorr, maxit - ph.iters, fusede, v4, &ph);
+      if (rcc != NF_OK) return rcc;
       NF_LAUNCH(g, NFK_SETUP, k_add<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->ecorr, n));
     }
+    return NF_OK;
+  };
+  if (warm) {
+    // x holds the caller's initial guess (masked; zeroed when b = 0 so that the answer is p = 0, R11)
+    NF_LAUNCH(g, NFK_SETUP, k_warm_mask<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.code, n, g->st));
+    rc = correct(two_phase ? tol1 : tol);
+    if (rc != NF_OK) return rc;
+  } else {
+    NF_CUDA(g, cudaMemsetAsync(x, 0, n * sizeof(float), g->stream));
+    NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)(two_phase ? tol1 : tol), 1));
+    rc = run_pcg_phase(g, x, maxit, fusedp, v4, &ph);
+    if (rc != NF_OK) return rc;
+  }
+  if (two_phase && ph.converged && ph.iters > 0 && ph.iters < maxit) {
+    // (the correction is ~1e-4 of x: accumulated on its own its rounding is invisible, and x is rounded once)
+    rc = correct(tol);
+    if (rc != NF_OK) return rc;
   }
   g->last_iters = ph.iters;
   // gauge: zero mean over active cells on a singular system (R12)

@@ -141,3 +141,35 @@ def test_channel_gate_shape_full_step_matches_oracle(torch, api):
         assert np.linalg.norm(p.cpu().numpy() - po) <= 1e-4 * np.linalg.norm(po)
         assert _rel3(U, Uo) <= 1e-4
     g.close()
+
+
+def test_warm_start_option(torch, api):
+    """flag bit 3 of nf_set_solver_options: the pressure array holds the initial guess.  Same answer as the cold
+    solve; starting from the converged pressure needs no iteration; b = 0 still returns p = 0."""
+    c = wl.config1()
+    n = c["nx"]
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    g = api.Grid(n, n, n, c["dx"])
+    g.set_domain_bc(1, 1, 0.0)  # +x Dirichlet: non-singular
+    g.set_solid(d(c["phi"]))
+    U = [d(a) for a in c["U"]]
+    p_cold = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    assert g.project(*U, p_cold, tol=1e-6, maxit=200) == 0
+    it_cold = g.last_solve_info()["iters"]
+    g.set_solver_options(1, 1, 8)
+    U2 = [d(a) for a in c["U"]]
+    p_warm = p_cold.clone()
+    assert g.project(*U2, p_warm, tol=1e-6, maxit=200) == 0
+    assert g.last_solve_info()["iters"] == 0
+    assert float((p_warm - p_cold).norm() / p_cold.norm()) <= 1e-5
+    U3 = [d(a) for a in c["U"]]
+    p_half = 0.5 * p_cold
+    assert g.project(*U3, p_half, tol=1e-6, maxit=200) == 0
+    assert 0 < g.last_solve_info()["iters"] <= it_cold
+    assert float((p_half - p_cold).norm() / p_cold.norm()) <= 1e-5
+    assert float((U3[0] - U[0]).norm() / U[0].norm()) <= 1e-5
+    Z = [torch.zeros_like(a) for a in U]
+    p_junk = p_cold.clone()
+    assert g.project(*Z, p_junk, tol=1e-6, maxit=200) == 0
+    assert float(p_junk.abs().max()) == 0.0
+    g.close()
