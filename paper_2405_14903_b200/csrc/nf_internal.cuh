@@ -226,6 +226,32 @@ int nf_advect_impl(nf_grid *g, float *u, float *v, float *w, float dt);
 int nf_advect_adjoint_impl(nf_grid *g, const float *u0, const float *v0, const float *w0, float *gu, float *gv,
                            float *gw, float dt);
 
+// Programmatic dependent launch (PDL): the kernels of one PCG iteration are launched with the programmatic stream
+// serialisation attribute and start with nf_pdl_enter() -- "my dependents may be scheduled" + "wait until the grids
+// I depend on have completed and flushed".  The next kernel's CTAs are then already resident (launch latency, CTA
+// scheduling and prologue behind them) when the previous kernel's last wave drains: each of the 7 kernels of an
+// iteration otherwise pays a fixed ~15 us of ramp-up and tail on top of its bytes.
+#ifdef __CUDACC__
+template <typename... KArgs, typename... Args>
+static inline cudaError_t nf_launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, cudaStream_t stream, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+__device__ __forceinline__ void nf_pdl_enter() {
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+#endif
+
 // ---- device helpers ---------------------------------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ double nf_warp_sum(double v) {

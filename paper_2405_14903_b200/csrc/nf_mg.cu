@@ -103,6 +103,7 @@ __device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, fl
 
 __global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restrict__ r, float *__restrict__ z, int kch,
                                                const NfSolveState *st) {
+  nf_pdl_enter();
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -168,6 +169,7 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
 
 __global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restrict__ z, float *__restrict__ rc, int cnx,
                                                int cny, int cnz, int kch, const NfSolveState *st) {
+  nf_pdl_enter();
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int J = blockIdx.y * blockDim.y + threadIdx.y;
@@ -244,6 +246,7 @@ __device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const floa
 __global__ void __launch_bounds__(256, 4) k_up1(NfLvK L, float *z, const float *__restrict__ r,
                                              const float *__restrict__ zc, int cnx, int cny, int kch,
                                              const NfSolveState *st) {
+  nf_pdl_enter();
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -302,6 +305,7 @@ __device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const flo
 template <bool DOT>
 __global__ void __launch_bounds__(256, 4) k_up2(NfLvK L, float *z, const float *__restrict__ r, int kch,
                                              NfSolveState *st, int slot) {
+  nf_pdl_enter();
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -865,9 +869,9 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
     if (L.vec && fused) {
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
-      NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), k_down1<<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.r, L.z, NF_KCH_MG, st));
+      NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), nf_launch_pdl(k_down1, d.grid, d.block, g->stream, nf_lvk(L), L.r, L.z, NF_KCH_MG, (const NfSolveState *)st));
       NfDims d2 = nf_vdims(L.nx / 4, C.ny, C.nz, 1);
-      NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), k_down2<<<d2.grid, d2.block, 0, g->stream>>>(nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, 1, st));
+      NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), nf_launch_pdl(k_down2, d2.grid, d2.block, g->stream, nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, 1, (const NfSolveState *)st));
     } else {
       for (int s = 0; s < g->nu_pre; ++s) {
         smooth_half(g, L, 0, s == 0, false, st, slot);
@@ -931,12 +935,12 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
     if (L.vec && fused) {
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
-      NF_LAUNCH(g, (l == 0 ? NFK_UP1_0 : NFK_VEC_C), k_up1<<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, C.z, C.nx, C.ny, NF_KCH_MG, st));
+      NF_LAUNCH(g, (l == 0 ? NFK_UP1_0 : NFK_VEC_C), nf_launch_pdl(k_up1, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, C.z, C.nx, C.ny, NF_KCH_MG, (const NfSolveState *)st));
       if (l == 0 && with_dot) {
-        NF_LAUNCH(g, NFK_UP2_0, k_up2<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, NF_KCH_MG, g->st, slot));
+        NF_LAUNCH(g, NFK_UP2_0, nf_launch_pdl(k_up2<true>, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, NF_KCH_MG, g->st, slot));
         dot_done = true;
       } else {
-        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), k_up2<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, L.r, NF_KCH_MG, st, slot));
+        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), nf_launch_pdl(k_up2<false>, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, NF_KCH_MG, st, slot));
       }
     } else {
       NfDims d = nf_dims(L.nx, L.ny, L.nz);

@@ -92,6 +92,7 @@ template <bool FIRST>
 __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__restrict__ z, const float *__restrict__ pold,
                                                  float *__restrict__ pnew, float *__restrict__ q, float *__restrict__ x,
                                                  int kch, NfSolveState *st, int slot) {
+  nf_pdl_enter();
   if (st->done) return;
   float beta = 0.0f, aprev = 0.0f;
   if (!FIRST) {
@@ -208,6 +209,7 @@ template <bool XUPD>
 __global__ void __launch_bounds__(256) k_cg_update(float *__restrict__ x, float *__restrict__ r,
                                                    const float *__restrict__ p, const float *__restrict__ q, size_t n,
                                                    int vec4, NfSolveState *st, int slot, NfHostStatus *hs, int seq) {
+  nf_pdl_enter();
   if (st->done) {  // (uniform: done is only ever set by the last CTA of an earlier launch)
     if (blockIdx.x == 0 && threadIdx.x == 0) nf_cg_check(st, slot, hs, seq);
     return;
@@ -625,10 +627,10 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
       float *pnew = (it & 1) ? g->p2 : g->p, *pold = (it & 1) ? g->p : g->p2;
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
       if (it == 0)
-        NF_LAUNCH(g, NFK_APPLY, k_papply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
+        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<true>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
       else
-        NF_LAUNCH(g, NFK_APPLY, k_papply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), L.z, pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
-      NF_LAUNCH(g, NFK_UPDATE, k_cg_update<false><<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, pnew, g->q, n, v4, g->st, slot, hs, it + 1));
+        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<false>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
+      NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_cg_update<false>, dim3(NF_VEC_BLOCKS), dim3(256), g->stream, x, L.r, (const float *)pnew, (const float *)g->q, n, v4, g->st, slot, hs, it + 1));
       if (it + 1 < maxit) {
         rc = nf_vcycle_impl(g, true, 1 - slot);
         if (rc != NF_OK) return rc;
