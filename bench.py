@@ -225,8 +225,8 @@ def run_ours(args):
     ncell = n ** 3
     peak, peak_src = _peaks()
     # algorithmic bytes per fine cell per launch (DESIGN.md section 8 / SURVEY.md 8d.2), fp32
-    # fused p-update + A-apply + deferred x update: z, p, x, code in; p', q, x out = 25; r update: r, q in, r out = 12
-    BYTES = {"apply_A": 25.0, "cg_update": 12.0, "cg_pupdate": 12.0, "down1_fine": 9.0, "down2_fine": 5.5,
+    # fused p-update + A-apply + deferred x update: z, p, x, code in; p', q, x out = 25; fused r update + pre-smoother: r, q, code in; r, z out = 17
+    BYTES = {"apply_A": 25.0, "cg_update": 17.0, "cg_pupdate": 12.0, "down1_fine": 9.0, "down2_fine": 5.5,
              "up1_fine": 13.5, "up2_fine": 13.0, "rbgs_fine": 24.0, "restrict_fine": 20.5, "prolong_fine": 8.5}
     kern = {}
     for name, (ms, cnt) in prof.items():

@@ -106,6 +106,7 @@ struct nf_grid {
   // solid velocity (MAC layout, closed walls at rest) and the last SDF
   float *us, *vs, *ws, *sdf;
   // CG vectors on level 0 (r and z live in lv[0])
+  float *r_alt;  // the residual ping-pongs between lv[0].r and this buffer (k_update_down1); both owned by the handle
   float *ecorr;  // correction vector of the second PCG phase
   float *b0;  // the prepared right-hand side (kept for the true-residual refresh, nf_solver.cu)
   float *p, *p2, *q, *xtmp;  // p / p2: the search direction ping-pongs between two buffers (k_papply4)
@@ -208,7 +209,10 @@ int nf_apply_A_impl(nf_grid *g, const float *p, float *q);
 void nf_mg_plan(nf_grid *g);      // choose the shared-memory tail and the vec levels (after the level extents are known)
 int nf_mg_init(nf_grid *g);       // kernel attributes
 int nf_mg_pack_tail(nf_grid *g);  // packed operator of the tail levels from the current weights
-int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot);  // z = M^{-1} r on lv[0].r -> lv[0].z
+int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1 = false);  // z = M^{-1} r on lv[0].r -> lv[0].z
+// fused r' = r - a q + pre-smoother of level 0 (r' into g->r_alt, then the two buffers swap); false if not applicable
+bool nf_update_down1_ok(const nf_grid *g);
+int nf_update_down1(nf_grid *g, int slot, NfHostStatus *hs, int seq);
 // Solve A x = lv[0].r (already masked; mean removed if singular; st->bb set by nf_solve_prepare).
 int nf_solver_init(nf_grid *g);                          // kernel attributes (once per process)
 int nf_solve_prepare(nf_grid *g, float tol, int maxit);  // from lv[0].r: mask, mean removal, bb
@@ -277,4 +281,32 @@ __device__ __forceinline__ void nf_block_atomic_add(double v, double *dst) {
   }
   __syncthreads();
 }
+// Advance the iteration counter, decide convergence (R11), publish the status to the mapped host ring, and clear
+// the accumulators of the other parity slot.  One thread, after rr[slot] is complete.
+__device__ __forceinline__ void nf_cg_check(NfSolveState *st, int slot, NfHostStatus *hs, int seq) {
+  if (!st->done) {
+    st->iter += 1;
+    st->last_slot = slot;
+    const double rr = *(volatile double *)&st->rr[slot];
+    if (!(rr == rr) || rr <= st->tol2 * st->bb) {
+      st->done = 1;
+      st->converged = (rr == rr) ? 1 : 0;
+    } else if (st->iter >= st->maxit) {
+      st->done = 1;
+      st->converged = 0;
+    }
+    st->pq[1 - slot] = 0.0;
+    st->rr[1 - slot] = 0.0;
+    st->rz[1 - slot] = 0.0;
+    st->relres = st->bb > 0.0 ? sqrt(rr / st->bb) : 0.0;
+  }
+  hs->relres = (float)st->relres;
+  hs->iter = st->iter;
+  hs->done = st->done;
+  hs->converged = st->converged;
+  __threadfence_system();
+  hs->seq = seq;
+  __threadfence_system();
+}
+
 #endif

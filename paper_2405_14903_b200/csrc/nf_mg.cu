@@ -40,19 +40,24 @@ __device__ __forceinline__ NfRow4 nf_row(const float *f, const uint8_t *__restri
 }
 
 // PAR = (i0 + j + k) & 1 = colour of the first of the 4 cells; cell q is red iff ((q + PAR) & 1) == 0.
-template <int PAR>
-__device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, float *z, int i0, int j, int k) {
+// R4(at, ok) / R1(at, ok): the right-hand side r on a row of 4 cells / one cell (0 when !ok).  k_down1 reads it from
+// memory; k_update_down1 evaluates r - a q on the fly.  Returns the row of r of the thread's own 4 cells.
+template <int PAR, class F4, class F1>
+__device__ __forceinline__ float4 nf_down1_core(const NfLvK &L, F4 R4, F1 R1, float *z, int i0, int j, int k) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const nf_idx sy = nx, sz = (nf_idx)nx * ny;
   const nf_idx id = ((nf_idx)k * ny + j) * nx + i0;
   // every load of r is issued before the branch on the code (one round trip for the common, deep path)
-  const NfRow4 C = nf_row(r, L.code, id, true);
+  NfRow4 C;
+  const float4 crow = R4(id, true);
+  nf_unpack4(crow, C.v);
+  C.c4 = nf_ldc4(L.code, id, true);
   float out[4], yl[4], yh[4], zl[4], zh[4];
-  nf_unpack4(nf_ld4(r, id - sy, j > 0), yl);
-  nf_unpack4(nf_ld4(r, id + sy, j + 1 < ny), yh);
-  nf_unpack4(nf_ld4(r, id - sz, k > 0), zl);
-  nf_unpack4(nf_ld4(r, id + sz, k + 1 < nz), zh);
-  const float re = PAR ? nf_ld1(r, id - 1, i0 > 0) : nf_ld1(r, id + 4, i0 + 4 < nx);
+  nf_unpack4(R4(id - sy, j > 0), yl);
+  nf_unpack4(R4(id + sy, j + 1 < ny), yh);
+  nf_unpack4(R4(id - sz, k > 0), zl);
+  nf_unpack4(R4(id + sz, k + 1 < nz), zh);
+  const float re = PAR ? R1(id - 1, i0 > 0) : R1(id + 4, i0 + 4 < nx);
   if ((C.c4 & 0x80808080u) == 0x80808080u) {
     // all four cells are deep interior (NF_CODE_DEEP): every diagonal involved is 6c, every weight is 1, and no
     // neighbour code is needed
@@ -69,7 +74,7 @@ __device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, fl
       }
     }
     *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
-    return;
+    return crow;
   }
   // general path: the red neighbours' values r/diag from the inverse-diagonal rows (one more round trip, no
   // dependence on the codes), the six weights of a black cell from its code
@@ -99,6 +104,59 @@ __device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, fl
     }
   }
   *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
+  return crow;
+}
+template <int PAR>
+__device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, float *z, int i0, int j, int k) {
+  nf_down1_core<PAR>(L, [&](nf_idx at, bool ok) { return nf_ld4(r, at, ok); },
+                     [&](nf_idx at, bool ok) { return nf_ld1(r, at, ok); }, z, i0, j, k);
+}
+
+// a-4 + a-5 fused: the residual update r' = r - a q (a = rz / pq from device memory) evaluated on the fly for the row
+// and its neighbour rows, ||r'||^2, and the pre-smoother z = smooth(r') in the same pass: 17 B/cell (r, q, code in;
+// r', z out) instead of 12 + 9, and one kernel's fixed cost less per iteration.  r' goes to a second buffer (the
+// neighbours' threads still read r).  The last CTA to finish runs the convergence check (nf_cg_check).
+__global__ void __launch_bounds__(256, 4) k_update_down1(NfLvK L, const float *__restrict__ rold,
+                                                      const float *__restrict__ q, float *__restrict__ rnew,
+                                                      float *__restrict__ z, int kch, NfSolveState *st, int slot,
+                                                      NfHostStatus *hs, int seq) {
+  nf_pdl_enter();
+  if (st->done) {  // (uniform: done is only ever set by the last CTA of an earlier launch)
+    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && threadIdx.y == 0)
+      nf_cg_check(st, slot, hs, seq);
+    return;
+  }
+  const double pq = st->pq[slot];
+  const float a = (pq > 0.0) ? (float)(st->rz[slot] / pq) : 0.0f;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  float part = 0.0f;
+  if (i0 < L.nx && j < L.ny) {
+    auto R4 = [&](nf_idx at, bool ok) {
+      float4 v = nf_ld4(rold, at, ok);
+      const float4 w = nf_ld4(q, at, ok);
+      v.x -= a * w.x; v.y -= a * w.y; v.z -= a * w.z; v.w -= a * w.w;
+      return v;
+    };
+    auto R1 = [&](nf_idx at, bool ok) { return nf_ld1(rold, at, ok) - a * nf_ld1(q, at, ok); };
+    const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, L.nz);
+    for (int k = k0; k < k1; ++k) {
+      const float4 c = ((j + k) & 1) ? nf_down1_core<1>(L, R4, R1, z, i0, j, k) : nf_down1_core<0>(L, R4, R1, z, i0, j, k);
+      *reinterpret_cast<float4 *>(rnew + ((nf_idx)k * L.ny + j) * L.nx + i0) = c;
+      part += (c.x * c.x + c.y * c.y) + (c.z * c.z + c.w * c.w);
+    }
+  }
+  nf_block_atomic_add((double)part, &st->rr[slot]);
+  if (threadIdx.x == 0 && threadIdx.y == 0) {
+    __threadfence();
+    const unsigned total = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned t = atomicAdd(&st->ticket, 1u);
+    if (t == total - 1) {
+      st->ticket = 0;
+      __threadfence();
+      nf_cg_check(st, slot, hs, seq);
+    }
+  }
 }
 
 __global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restrict__ r, float *__restrict__ z, int kch,
@@ -857,7 +915,21 @@ static void smooth_half(nf_grid *g, NfLevel &L, int color, bool zero, bool dot, 
 }
 
 // z = M^{-1} r on level 0 (lv[0].r -> lv[0].z).  with_dot: accumulate r.z into st->rz[slot] and honour st->done.
-int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
+bool nf_update_down1_ok(const nf_grid *g) {
+  return g->nu_pre == 1 && g->nu_post == 1 && !g->force_generic && g->lv[0].vec && g->nlev > 1;
+}
+int nf_update_down1(nf_grid *g, int slot, NfHostStatus *hs, int seq) {
+  NfLevel &L = g->lv[0];
+  NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+  NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_update_down1, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.r, (const float *)g->q, g->r_alt, L.z, NF_KCH_MG, g->st, slot, hs, seq));
+  float *t = L.r;
+  L.r = g->r_alt;
+  g->r_alt = t;
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
+int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
   NfSolveState *st = with_dot ? g->st : nullptr;
   const int nl = g->nlev;
   const bool has_tail = g->tail < nl;
@@ -869,7 +941,8 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
     if (L.vec && fused) {
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
-      NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), nf_launch_pdl(k_down1, d.grid, d.block, g->stream, nf_lvk(L), L.r, L.z, NF_KCH_MG, (const NfSolveState *)st));
+      if (!(l == 0 && skip_down1))
+        NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), nf_launch_pdl(k_down1, d.grid, d.block, g->stream, nf_lvk(L), L.r, L.z, NF_KCH_MG, (const NfSolveState *)st));
       NfDims d2 = nf_vdims(L.nx / 4, C.ny, C.nz, 1);
       NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), nf_launch_pdl(k_down2, d2.grid, d2.block, g->stream, nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, 1, (const NfSolveState *)st));
     } else {

@@ -175,34 +175,6 @@ __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__rest
 // ------------------------------------------------------------------------------------------------------------
 // a-4  CG vector ops
 // ------------------------------------------------------------------------------------------------------------
-// Advance the iteration counter, decide convergence (R11), publish the status to the mapped host ring, and clear
-// the accumulators of the other parity slot.  One thread, after rr[slot] is complete.
-__device__ __forceinline__ void nf_cg_check(NfSolveState *st, int slot, NfHostStatus *hs, int seq) {
-  if (!st->done) {
-    st->iter += 1;
-    st->last_slot = slot;
-    const double rr = *(volatile double *)&st->rr[slot];
-    if (!(rr == rr) || rr <= st->tol2 * st->bb) {
-      st->done = 1;
-      st->converged = (rr == rr) ? 1 : 0;
-    } else if (st->iter >= st->maxit) {
-      st->done = 1;
-      st->converged = 0;
-    }
-    st->pq[1 - slot] = 0.0;
-    st->rr[1 - slot] = 0.0;
-    st->rz[1 - slot] = 0.0;
-    st->relres = st->bb > 0.0 ? sqrt(rr / st->bb) : 0.0;
-  }
-  hs->relres = (float)st->relres;
-  hs->iter = st->iter;
-  hs->done = st->done;
-  hs->converged = st->converged;
-  __threadfence_system();
-  hs->seq = seq;
-  __threadfence_system();
-}
-
 // x += a p ; r -= a q ; rr += r.r      a = rz/pq read from device memory.  The last CTA to finish (ticket counter)
 // runs the convergence check: no separate one-thread kernel between the update and the V-cycle.
 template <bool XUPD>
@@ -615,6 +587,7 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
   NfLevel &L = g->lv[0];
   const size_t n = (size_t)L.ncell;
   for (int s = 0; s < NF_RING; ++s) g->hst[s].seq = 0;
+  const bool fusedr = fusedp && nf_update_down1_ok(g) && vec_ok(g->r_alt, g->r_alt, g->r_alt, g->r_alt, n);
   int rc = nf_vcycle_impl(g, true, 0);
   if (rc != NF_OK) return rc;
   if (!fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, 0, 1));
@@ -630,10 +603,20 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
         NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<true>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
       else
         NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<false>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
-      NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_cg_update<false>, dim3(NF_VEC_BLOCKS), dim3(256), g->stream, x, L.r, (const float *)pnew, (const float *)g->q, n, v4, g->st, slot, hs, it + 1));
-      if (it + 1 < maxit) {
-        rc = nf_vcycle_impl(g, true, 1 - slot);
+      if (fusedr) {
+        // r' = r - a q, ||r'||^2, the check and the pre-smoother of level 0 in one pass; the V-cycle skips its down1
+        rc = nf_update_down1(g, slot, hs, it + 1);
         if (rc != NF_OK) return rc;
+        if (it + 1 < maxit) {
+          rc = nf_vcycle_impl(g, true, 1 - slot, true);
+          if (rc != NF_OK) return rc;
+        }
+      } else {
+        NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_cg_update<false>, dim3(NF_VEC_BLOCKS), dim3(256), g->stream, x, L.r, (const float *)pnew, (const float *)g->q, n, v4, g->st, slot, hs, it + 1));
+        if (it + 1 < maxit) {
+          rc = nf_vcycle_impl(g, true, 1 - slot);
+          if (rc != NF_OK) return rc;
+        }
       }
     } else {
       launch_apply(g, g->p, g->q, true, slot);
