@@ -242,9 +242,9 @@ def run_ours(args):
     traffic = None
     try:
         if n == 256:
-            with open(os.path.join(ROOT, "profiles", "r1_v4_traffic.json")) as f:
+            with open(os.path.join(ROOT, "profiles", "r1_v5_traffic.json")) as f:
                 tr = json.load(f)
-            traffic = tr.get({"apply_A": "k_papply4", "cg_update": "k_cg_update", "down1_fine": "k_down1",
+            traffic = tr.get({"apply_A": "k_papply4", "cg_update": "k_update_down1", "down1_fine": "k_down1",
                               "down2_fine": "k_down2", "up1_fine": "k_up1", "up2_fine": "k_up2"}.get(dom, ""))
     except Exception:
         traffic = None
