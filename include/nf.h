@@ -130,6 +130,14 @@ int nf_project_adjoint(nf_grid *g, float *gu, float *gv, float *gw, const float 
  * In place (the library reads from an internal copy). */
 int nf_advect(nf_grid *g, float *u, float *v, float *w, float dt);
 
+/* NEXT-1  Explicit viscosity step (Eq. 3; L359-361 Eq. 13):
+ * Uhat = (I - nu dt/dx^2 G^T G) Utilde, per component on that component's own lattice, 7-point, nothing outside
+ * the lattice (R23: the symmetric form).  In place (the library reads from an internal copy).  Every face is
+ * updated; closed ones are overwritten by the projection.  The operator is symmetric: the backward pass (Eq. 8)
+ * is THIS call applied to dJ/dUhat -- there is no separate adjoint entry point.  Explicit: stable for
+ * nu dt/dx^2 <= 1/6 (the caller's responsibility).  nu < 0 or dt < 0: NF_ERR_INVALID. */
+int nf_viscosity(nf_grid *g, float *u, float *v, float *w, float nu, float dt);
+
 /* a-9  Adjoint of nf_advect (Eq. 8).  u0,v0,w0 = the saved pre-advection U^n;
  * in: gu,gv,gw = dJ/dUtilde; out (in place): dJ/dU^n. */
 int nf_advect_adjoint(nf_grid *g, const float *u0, const float *v0, const float *w0,

@@ -436,9 +436,36 @@ def advect_adjoint(U, gout, dt, dx):
 
 
 # ----------------------------------------------------------------------------------------------------
+# viscosity         PAPER.md:L84-87 (Eq. 3), L359-361 (Eq. 13), L126-128 (Eq. 8)
+# ----------------------------------------------------------------------------------------------------
+def viscosity(U, nu, dt, dx):
+    """Eq. 3: Uhat = (I - nu dt/dx^2 G^T G) Utilde, "for each axis, the Laplacian of the corresponding velocity
+    component ... on grid points": per component, the 7-point operator G^T G of that component's own lattice, G
+    = forward differences between lattice neighbours with nothing outside the lattice (reading R23: the paper is
+    silent on the boundary rows; this is the form that keeps G^T G symmetric, which Eq. 8 relies on when it applies
+    the same matrix in the backward pass).  Every face is updated (closed ones are overwritten by the projection,
+    as with advection, R14).  Self-adjoint: the backward pass calls this same function on dJ/dUhat (Eq. 8)."""
+    k = nu * dt / (dx * dx)
+    out = []
+    for f in U:
+        f = np.asarray(f, dtype=np.float64)
+        gtg = np.zeros_like(f)
+        for ax in range(3):
+            if f.shape[ax] < 2:
+                continue
+            d = np.diff(f, axis=ax)                     # G along this axis: f[i+1] - f[i]
+            lo = [slice(None)] * 3; hi = [slice(None)] * 3
+            lo[ax] = slice(0, -1); hi[ax] = slice(1, None)
+            gtg[tuple(lo)] -= d                          # G^T: -d at the lower point, +d at the upper
+            gtg[tuple(hi)] += d
+        out.append(f - k * gtg)
+    return out
+
+
+# ----------------------------------------------------------------------------------------------------
 # full steps forward and backward        PAPER.md:L78 (advection, projection), L111-141 (backward pass)
 # ----------------------------------------------------------------------------------------------------
-def rollout(U0, solid_fn, nsteps, dt, dx, dt_over_rho, bc, loss_fn, tol=1e-12, advect_on=True):
+def rollout(U0, solid_fn, nsteps, dt, dx, dt_over_rho, bc, loss_fn, tol=1e-12, advect_on=True, nu=0.0):
     """N steps "advect -> geometry at t^{n+1} -> project" (R15) and the backward pass that "mirrors the
     forward simulation in a reversed order", per-step state stored instead of a graph (L236).
 
@@ -451,6 +478,8 @@ def rollout(U0, solid_fn, nsteps, dt, dx, dt_over_rho, bc, loss_fn, tol=1e-12, a
     for n in range(1, nsteps + 1):
         Uprev = U
         Ut = advect(U, dt, dx) if advect_on else [a.copy() for a in U]
+        if nu != 0.0:
+            Ut = viscosity(Ut, nu, dt, dx)               # L78: advection, viscosity, projection
         phi, us, dphi, dus = solid_fn(n)
         alpha = face_weights(phi, bc)
         U, p = project(Ut, alpha, us, dx, dt_over_rho, bc, tol=tol)
@@ -463,6 +492,8 @@ def rollout(U0, solid_fn, nsteps, dt, dx, dt_over_rho, bc, loss_fn, tol=1e-12, a
         g_ut, g_alpha, g_us, _ = project_adjoint(g, alpha, p, Ut, us, dx, dt_over_rho, bc, tol=tol)
         g_phi = weights_adjoint(phi, g_alpha[0], g_alpha[1], g_alpha[2], bc)
         dtheta += float(np.sum(g_phi * dphi)) + sum(float(np.sum(a * b)) for a, b in zip(g_us, dus))
+        if nu != 0.0:
+            g_ut = viscosity(g_ut, nu, dt, dx)           # Eq. 8: the same symmetric matrix
         g = advect_adjoint(Uprev, g_ut, dt, dx) if advect_on else g_ut
     return J, dtheta, g
 

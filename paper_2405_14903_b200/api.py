@@ -31,6 +31,7 @@ _SIGNATURES = {
     "nf_project": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4 + [ctypes.c_float, ctypes.c_int]),
     "nf_project_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 14 + [ctypes.c_float, ctypes.c_int]),
     "nf_advect": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.c_float]),
+    "nf_viscosity": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.c_float, ctypes.c_float]),
     "nf_advect_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 6 + [ctypes.c_float]),
     "nf_weights_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
     "nf_apply_A": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p]),
@@ -216,6 +217,11 @@ class Grid:
     def advect(self, u, v, w, dt):
         self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
         self._check(self.lib.nf_advect(self.h, _ptr(u), _ptr(v), _ptr(w), float(dt)), "nf_advect")
+
+    def viscosity(self, u, v, w, nu, dt):
+        """Explicit viscosity step, in place; symmetric, so the backward pass calls it on the gradient (Eq. 8)."""
+        self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
+        self._check(self.lib.nf_viscosity(self.h, _ptr(u), _ptr(v), _ptr(w), float(nu), float(dt)), "nf_viscosity")
 
     def advect_adjoint(self, u0, v0, w0, gu, gv, gw, dt):
         for t, s, n in ((u0, self.shape_u, "u0"), (v0, self.shape_v, "v0"), (w0, self.shape_w, "w0"),

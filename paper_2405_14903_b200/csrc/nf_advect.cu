@@ -237,3 +237,46 @@ int nf_advect_adjoint_impl(nf_grid *g, const float *u0, const float *v0, const f
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
+
+// ------------------------------------------------------------------------------------------------------------
+// NEXT-1: explicit viscosity  Uhat = (I - nu dt/dx^2 G^T G) Utilde   (Eq. 3, L359-361 Eq. 13)
+// ------------------------------------------------------------------------------------------------------------
+// Per component, the 7-point operator of that component's own lattice with nothing outside it (R23: keeps G^T G
+// symmetric, so the backward pass -- Eq. 8 -- is this same kernel applied to the gradient).  One thread per lattice
+// point; neighbours through L1 (24 B/point algorithmic: read + write once).
+__global__ void __launch_bounds__(256) k_viscosity(const float *__restrict__ f, float *__restrict__ out, int ex, int ey,
+                                                   int ez, float kk) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  if (i >= ex || j >= ey || k >= ez) return;
+  const int id = (k * ey + j) * ex + i, sy = ex, sz = ex * ey;
+  const float c = f[id];
+  float gtg = 0.0f;  // (G^T G f) at this point = sum over existing neighbours of (f - f_nb)
+  if (i > 0) gtg += c - f[id - 1];
+  if (i + 1 < ex) gtg += c - f[id + 1];
+  if (j > 0) gtg += c - f[id - sy];
+  if (j + 1 < ey) gtg += c - f[id + sy];
+  if (k > 0) gtg += c - f[id - sz];
+  if (k + 1 < ez) gtg += c - f[id + sz];
+  out[id] = c - kk * gtg;
+}
+
+int nf_viscosity_impl(nf_grid *g, float *u, float *v, float *w, float nu, float dt) {
+  if (nf_nn(g) >= (size_t)1 << 31) {
+    g->err = "nf_viscosity: grid too large for 32-bit lattice indices";
+    return NF_ERR_INVALID;
+  }
+  NF_CUDA(g, cudaMemcpyAsync(g->fu, u, nf_nu(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(g->fv, v, nf_nv(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
+  NF_CUDA(g, cudaMemcpyAsync(g->fw, w, nf_nw(g) * sizeof(float), cudaMemcpyDeviceToDevice, g->stream));
+  const NfLat U = make_lat(g, g->fu, g->fv, g->fw);
+  const float kk = nu * dt / (g->dx * g->dx);
+  float *outs[3] = {u, v, w};
+  for (int c = 0; c < 3; ++c) {
+    NfDims d = nf_dims(U.ex[c], U.ey[c], U.ez[c]);
+    NF_LAUNCH(g, NFK_ADVECT, k_viscosity<<<d.grid, d.block, 0, g->stream>>>(U.f[c], outs[c], U.ex[c], U.ey[c], U.ez[c], kk));
+  }
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}

@@ -233,6 +233,12 @@ extern "C" int nf_project_adjoint(nf_grid *g, float *gu, float *gv, float *gw, c
   return rc;
 }
 
+extern "C" int nf_viscosity(nf_grid *g, float *u, float *v, float *w, float nu, float dt) {
+  NF_CHECK_HANDLE(g);
+  if (!u || !v || !w || !(nu >= 0.0f) || !(dt >= 0.0f)) return NF_ERR_INVALID;
+  return nf_viscosity_impl(g, u, v, w, nu, dt);
+}
+
 extern "C" int nf_advect(nf_grid *g, float *u, float *v, float *w, float dt) {
   NF_CHECK_HANDLE(g);
   if (!u || !v || !w) return NF_ERR_INVALID;

@@ -6,7 +6,7 @@ chain rule only: every step of the path runs in the library's kernels."""
 import torch
 
 
-def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect_on=True):
+def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect_on=True, nu=0.0):
     """solid_fn(step) -> (phi, (us, vs, ws), dphi_dtheta, (dus, dvs, dws)) as CUDA float32 tensors (the derivative
     tensors may be None); loss_fn(U) -> (J tensor, [dJ/du, dJ/dv, dJ/dw]).
     Returns (J, dJ/dtheta, dJ/dU0) -- J and dJ/dtheta as Python floats."""
@@ -17,6 +17,8 @@ def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect
         Uprev = [a.clone() for a in U]
         if advect_on:
             g.advect(*U, dt)
+        if nu != 0.0:
+            g.viscosity(*U, nu, dt)  # advection, viscosity, projection
         phi, us, dphi, dus = solid_fn(n)
         g.set_solid(phi, *us)
         Uhat = [a.clone() for a in U]
@@ -40,6 +42,8 @@ def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect
             for a, b in zip(gs, dus):
                 if b is not None:
                     dtheta += (a.double() * b.double()).sum()
+        if nu != 0.0:
+            g.viscosity(*G, nu, dt)  # Eq. 8: the same symmetric matrix
         if advect_on:
             g.advect_adjoint(*Uprev, *G, dt)
     return float(J), float(dtheta), G

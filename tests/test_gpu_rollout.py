@@ -173,3 +173,60 @@ def test_warm_start_option(torch, api):
     assert g.project(*Z, p_junk, tol=1e-6, maxit=200) == 0
     assert float(p_junk.abs().max()) == 0.0
     g.close()
+
+
+@pytest.mark.parametrize("shape", [(20, 18, 14), (33, 7, 12), (1, 1, 7)])
+def test_viscosity_matches_oracle_and_is_self_adjoint(torch, api, shape):
+    """NEXT-1: nf_viscosity (Eq. 3) against the oracle, and <L a, b> = <a, L b> on the GPU (Eq. 8 reuses the call)."""
+    nx, ny, nz = shape
+    rng = np.random.default_rng(6)
+    A = wl.random_velocity(rng, nx, ny, nz, "normal")
+    B = wl.random_velocity(rng, nx, ny, nz, "normal")
+    dx = 1.0 / nx
+    nu, dt = 0.1 * dx * dx / 0.01, 0.01          # nu dt / dx^2 = 0.1
+    ref = orc.viscosity(A, nu, dt, dx)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    g = api.Grid(nx, ny, nz, dx)
+    LA = [d(a) for a in A]
+    g.viscosity(*LA, nu, dt)
+    for got, r in zip(LA, ref):
+        assert np.max(np.abs(got.cpu().numpy() - r)) <= 2e-6 * max(1.0, np.max(np.abs(r)))
+    LB = [d(b) for b in B]
+    g.viscosity(*LB, nu, dt)
+    lhs = sum(float((x.double() * d(y).double()).sum()) for x, y in zip(LA, B))
+    rhs = sum(float((d(x).double() * y.double()).sum()) for x, y in zip(A, LB))
+    g.close()
+    assert abs(lhs - rhs) <= 1e-5 * max(abs(lhs), 1.0)
+
+
+def test_rollout_with_viscosity_matches_oracle(torch, api):
+    """Full steps advect -> viscosity -> project and the mirrored backward pass (Eq. 8): J, dJ/dtheta
+    and dJ/dU0 against the oracle's rollout."""
+    from paper_2405_14903_b200 import rollout as ro
+    n, nsteps = 24, 3
+    P = wl.config2_params(n)
+    bc = orc.BC(P["bc_types"], P["bc_values"])
+    rng = np.random.default_rng(1002)
+    U0 = [(0.2 * rng.standard_normal(s)).astype(np.float32) for s in wl.face_shapes(n, n, n)]
+    nu = 0.08 * P["dx"] ** 2 / P["dt"]
+    geom = {s: wl.config2_solid(P, s, P["theta"]) for s in range(1, nsteps + 1)}
+    lo, hi = P["loss_lo"], P["loss_hi"]
+    Jo, dJo, gU0o = orc.rollout(U0, lambda s: geom[s], nsteps, P["dt"], P["dx"], P["dt_over_rho"], bc,
+                                orc.loss_sum_u2(lo, hi), nu=nu)
+    d = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    g = api.Grid(n, n, n, P["dx"])
+    g.set_dt_rho(P["dt_over_rho"])
+    dgeom = {s: (d(v[0]), [d(a) for a in v[1]], d(v[2]), [d(a) for a in v[3]]) for s, v in geom.items()}
+
+    def loss(U):
+        blk = U[0][lo:hi, lo:hi, lo:hi].double()
+        G = [torch.zeros_like(a) for a in U]
+        G[0][lo:hi, lo:hi, lo:hi] = (2.0 * blk).float()
+        return (blk * blk).sum(), G
+
+    Jg, dJg, gU0g = ro.rollout(g, [d(a) for a in U0], lambda s: dgeom[s], nsteps, P["dt"], loss, tol=1e-6, maxit=200,
+                               nu=nu)
+    g.close()
+    assert abs(Jg - Jo) <= 1e-4 * abs(Jo), (Jg, Jo)
+    assert abs(dJg - dJo) <= 1e-3 * abs(dJo), (dJg, dJo)
+    assert _rel3(gU0g, gU0o) <= 1e-3
