@@ -138,6 +138,13 @@ int nf_advect(nf_grid *g, float *u, float *v, float *w, float dt);
  * nu dt/dx^2 <= 1/6 (the caller's responsibility).  nu < 0 or dt < 0: NF_ERR_INVALID. */
 int nf_viscosity(nf_grid *g, float *u, float *v, float *w, float nu, float dt);
 
+/* NEXT-1  CFL sub-stepping support (the simulator "adopts CFL condition",
+ * the steps simulated exceed the frames; the constant is not given, R24): *max_abs_host = max over all faces of
+ * |u|, |v|, |w| (device reduction; HOST pointer; this call synchronises the stream).  The policy
+ * dt = min(dt_frame_left, C dx / max) and the loop over sub-steps belong to the caller
+ * (paper_2405_14903_b200/rollout.py: cfl_substeps); dt is a constant of the backward pass. */
+int nf_max_speed(nf_grid *g, const float *u, const float *v, const float *w, float *max_abs_host);
+
 /* a-9  Adjoint of nf_advect (Eq. 8).  u0,v0,w0 = the saved pre-advection U^n;
  * in: gu,gv,gw = dJ/dUtilde; out (in place): dJ/dU^n. */
 int nf_advect_adjoint(nf_grid *g, const float *u0, const float *v0, const float *w0,

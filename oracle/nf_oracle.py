@@ -462,6 +462,11 @@ def viscosity(U, nu, dt, dx):
     return out
 
 
+def max_speed(U):
+    """max over all faces of |u|, |v|, |w| -- the quantity of the CFL condition (R24)."""
+    return max(float(np.max(np.abs(np.asarray(a, dtype=np.float64)))) for a in U)
+
+
 # ----------------------------------------------------------------------------------------------------
 # full steps forward and backward        PAPER.md:L78 (advection, projection), L111-141 (backward pass)
 # ----------------------------------------------------------------------------------------------------

@@ -31,6 +31,7 @@ _SIGNATURES = {
     "nf_project": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4 + [ctypes.c_float, ctypes.c_int]),
     "nf_project_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 14 + [ctypes.c_float, ctypes.c_int]),
     "nf_advect": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.c_float]),
+    "nf_max_speed": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.POINTER(ctypes.c_float)]),
     "nf_viscosity": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.c_float, ctypes.c_float]),
     "nf_advect_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 6 + [ctypes.c_float]),
     "nf_weights_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
@@ -217,6 +218,13 @@ class Grid:
     def advect(self, u, v, w, dt):
         self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
         self._check(self.lib.nf_advect(self.h, _ptr(u), _ptr(v), _ptr(w), float(dt)), "nf_advect")
+
+    def max_speed(self, u, v, w):
+        """max over all faces of |u|, |v|, |w| (synchronises)."""
+        self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
+        out = ctypes.c_float()
+        self._check(self.lib.nf_max_speed(self.h, _ptr(u), _ptr(v), _ptr(w), ctypes.byref(out)), "nf_max_speed")
+        return out.value
 
     def viscosity(self, u, v, w, nu, dt):
         """Explicit viscosity step, in place; symmetric, so the backward pass calls it on the gradient (Eq. 8)."""

@@ -7,6 +7,8 @@
 // the first stage U(x) at the face's own position is lattice-aligned and is evaluated as the fixed 1- and 4-point
 // stencils it reduces to (same clamping as the general interpolation) instead of three general interpolations;
 // 32-bit index arithmetic throughout (lattices have < 2^31 points).
+#include <cstring>
+
 #include "nf_internal.cuh"
 #ifndef NF_ADJ_MINB
 #define NF_ADJ_MINB 4
@@ -278,5 +280,41 @@ int nf_viscosity_impl(nf_grid *g, float *u, float *v, float *w, float nu, float 
     NF_LAUNCH(g, NFK_ADVECT, k_viscosity<<<d.grid, d.block, 0, g->stream>>>(U.f[c], outs[c], U.ex[c], U.ey[c], U.ez[c], kk));
   }
   NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// NEXT-1: CFL sub-stepping support ("adopts CFL condition ... the actual steps simulated are
+// higher than # Frames"; the condition's constant is not given, R24) -- max over all faces of |velocity|.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_max_abs(const float *__restrict__ f, size_t n, unsigned *out) {
+  float m = 0.0f;
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = tid; t < n; t += nth) {
+    const float v = fabsf(f[t]);
+    m = (v > m || v != v) ? v : m;  // (a NaN propagates)
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float t = __shfl_xor_sync(0xffffffffu, m, o);
+    m = (t > m || t != t) ? t : m;
+  }
+  // non-negative floats order like their bit patterns (NaN patterns sort above every finite value)
+  if ((threadIdx.x & 31) == 0) atomicMax(out, __float_as_uint(m));
+}
+
+int nf_max_speed_impl(nf_grid *g, const float *u, const float *v, const float *w, float *out_host) {
+  unsigned *d = reinterpret_cast<unsigned *>(g->d_counts);  // (scratch: two doubles, rewritten by every hierarchy build)
+  NF_CUDA(g, cudaMemsetAsync(d, 0, sizeof(unsigned), g->stream));
+  const float *f[3] = {u, v, w};
+  const size_t n[3] = {nf_nu(g), nf_nv(g), nf_nw(g)};
+  for (int c = 0; c < 3; ++c)
+    NF_LAUNCH(g, NFK_MISC, k_max_abs<<<148 * 8, 256, 0, g->stream>>>(f[c], n[c], d));
+  unsigned bits = 0;
+  NF_CUDA(g, cudaMemcpyAsync(&bits, d, sizeof(unsigned), cudaMemcpyDeviceToHost, g->stream));
+  NF_CUDA(g, cudaStreamSynchronize(g->stream));
+  float r;
+  memcpy(&r, &bits, sizeof(float));
+  *out_host = r;
   return NF_OK;
 }

@@ -239,6 +239,12 @@ extern "C" int nf_viscosity(nf_grid *g, float *u, float *v, float *w, float nu, 
   return nf_viscosity_impl(g, u, v, w, nu, dt);
 }
 
+extern "C" int nf_max_speed(nf_grid *g, const float *u, const float *v, const float *w, float *max_abs_host) {
+  NF_CHECK_HANDLE(g);
+  if (!u || !v || !w || !max_abs_host) return NF_ERR_INVALID;
+  return nf_max_speed_impl(g, u, v, w, max_abs_host);
+}
+
 extern "C" int nf_advect(nf_grid *g, float *u, float *v, float *w, float dt) {
   NF_CHECK_HANDLE(g);
   if (!u || !v || !w) return NF_ERR_INVALID;

@@ -228,6 +228,7 @@ int nf_adjoint_finish_impl(nf_grid *g, float *gu, float *gv, float *gw, const fl
 // nf_advect.cu
 int nf_advect_impl(nf_grid *g, float *u, float *v, float *w, float dt);
 int nf_viscosity_impl(nf_grid *g, float *u, float *v, float *w, float nu, float dt);
+int nf_max_speed_impl(nf_grid *g, const float *u, const float *v, const float *w, float *out_host);
 int nf_advect_adjoint_impl(nf_grid *g, const float *u0, const float *v0, const float *w0, float *gu, float *gv,
                            float *gw, float dt);
 

@@ -47,3 +47,16 @@ def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect
         if advect_on:
             g.advect_adjoint(*Uprev, *G, dt)
     return float(J), float(dtheta), G
+
+
+def cfl_substeps(grid, U, dt_frame, cfl=1.0, max_substeps=64):
+    """Sub-step sizes that advance one frame of length dt_frame under the CFL condition the paper says it adopts
+    (its constant is not given -- R24: dt <= cfl * dx / max|U|): the first sub-step's dt from the
+    current velocity, and the number of equal sub-steps that would cover the frame at that dt.  The caller re-evaluates
+    after every sub-step (the velocity changes).  Returns (dt_sub, n_left)."""
+    import math
+    vmax = grid.max_speed(*U)
+    if not (vmax > 0.0) or math.isinf(vmax):
+        return dt_frame, 1
+    n = max(1, min(max_substeps, int(math.ceil(dt_frame * vmax / (cfl * grid.dx) - 1e-9))))
+    return dt_frame / n, n

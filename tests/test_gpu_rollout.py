@@ -230,3 +230,22 @@ def test_rollout_with_viscosity_matches_oracle(torch, api):
     assert abs(Jg - Jo) <= 1e-4 * abs(Jo), (Jg, Jo)
     assert abs(dJg - dJo) <= 1e-3 * abs(dJo), (dJg, dJo)
     assert _rel3(gU0g, gU0o) <= 1e-3
+
+
+def test_max_speed_and_cfl_substeps(torch, api):
+    """NEXT-1: the device max-|U| reduction (bit-exact against the fp32 inputs) and the sub-step policy."""
+    from paper_2405_14903_b200 import rollout as ro
+    nx, ny, nz = 33, 18, 7
+    rng = np.random.default_rng(3)
+    U = wl.random_velocity(rng, nx, ny, nz, "normal")
+    U[1][3, 5, 2] = -7.25
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    g = api.Grid(nx, ny, nz, 0.5)
+    dU = [d(a) for a in U]
+    assert g.max_speed(*dU) == np.float32(orc.max_speed([a.astype(np.float32) for a in U])) == 7.25
+    dt_sub, n = ro.cfl_substeps(g, dU, dt_frame=1.0, cfl=1.0)
+    assert n == 15 and abs(dt_sub - 1.0 / 15) < 1e-12           # ceil(1.0 * 7.25 / 0.5)
+    assert dt_sub * 7.25 <= 1.0 * 0.5 + 1e-9
+    Z = [torch.zeros_like(a) for a in dU]
+    assert g.max_speed(*Z) == 0.0 and ro.cfl_substeps(g, Z, 0.3) == (0.3, 1)
+    g.close()
