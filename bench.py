@@ -390,6 +390,58 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: MGPCG alone (nf_solve) on cubic all-Neumann grids with 200 random solid spheres,
+    rhs N(0,1) with its mean removed, tol 1e-6: iterations, ms, Mcell-iterations/s, and the fp64 true residual of the
+    answer evaluated on the host (the oracle's operator, one pass; the oracle does not solve at these sizes)."""
+    import numpy as np
+    import torch
+    from oracle import nf_oracle as orc   # (cpu_baseline-style use: residual evaluation only, outside the timed region)
+    from paper_2405_14903_b200 import api, workloads as wl
+    api.load_library()
+    torch.cuda.set_device(0)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    rows = []
+    for n in [int(x) for x in args.sweep.split(",")]:
+        phi = wl.config5_phi(n)
+        g = api.Grid(n, n, n, 1.0 / n)
+        g.set_solid(d(phi))
+        au, av, aw, ncomp = wl.keep_largest_component(*[a.cpu().numpy() for a in g.get_weights()])
+        active = (au[:, :, :-1] + au[:, :, 1:] + av[:, :-1, :] + av[:, 1:, :] + aw[:-1] + aw[1:]) > 0
+        rhs = wl.config5_rhs(n, active)
+        g.set_weights(d(au), d(av), d(aw))
+        drhs = d(rhs)
+        p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+        for _ in range(3):
+            rc = g.solve(drhs, p, tol=TOL, maxit=MAXIT)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 5
+        e0.record()
+        for _ in range(reps):
+            rc = g.solve(drhs, p, tol=TOL, maxit=MAXIT)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        info = g.last_solve_info()
+        nact = int(active.sum())
+        a64 = [a.astype(np.float64) for a in (au, av, aw)]
+        res = rhs.astype(np.float64) - orc.apply_A(p.cpu().numpy().astype(np.float64), a64, float(n))
+        res[~active] = 0.0
+        res[active] -= res[active].mean()
+        rows.append({"n": n, "rc": int(rc), "iters": info["iters"], "ms": round(ms, 3), "active_cells": nact,
+                     "fluid_components_before_filter": int(ncomp), "levels": g.info()["levels"],
+                     "mcell_iters_per_s": round(nact * info["iters"] / (ms * 1e-3) / 1e6, 1),
+                     "us_per_iter": round(1e3 * ms / max(info["iters"], 1), 1),
+                     "recursive_relres": float(info["relres"]),
+                     "true_relres_fp64": float(np.linalg.norm(res) / np.linalg.norm(rhs))})
+        g.close()
+        del p, drhs
+        torch.cuda.empty_cache()
+    print(json.dumps({"workload": "configs[4] pressure-solve sweep (200 random spheres, all-Neumann, rhs N(0,1))",
+                      "tol": TOL, "dtype": "f32", "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -401,7 +453,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--warm-start", action="store_true",
                     help="nf_project starts from the previous step's pressure (default: x0 = 0, as BASELINE's metric)")
+    ap.add_argument("--sweep", default="", help="comma-separated cubic sizes: run the configs[4] pressure-solve sweep "
+                                                 "instead of the headline step, e.g. --sweep 64,128,256,384")
     args = ap.parse_args()
+    if args.sweep:
+        run_sweep(args)
+        return
     if args.impl == "reference":
         run_reference(args)
     else:
