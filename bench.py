@@ -390,13 +390,25 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def _apply_A_fp64(p, au, av, aw, c):
+    """c G^T S G p in fp64 NumPy with homogeneous ghosts (acceptance check of the sweep; closed walls have alpha = 0)."""
+    import numpy as np
+    fu = np.zeros(au.shape); fv = np.zeros(av.shape); fw = np.zeros(aw.shape)
+    fu[:, :, 1:-1] = au[:, :, 1:-1] * (p[:, :, 1:] - p[:, :, :-1])
+    fu[:, :, 0] = au[:, :, 0] * p[:, :, 0]; fu[:, :, -1] = -au[:, :, -1] * p[:, :, -1]
+    fv[:, 1:-1, :] = av[:, 1:-1, :] * (p[:, 1:, :] - p[:, :-1, :])
+    fv[:, 0, :] = av[:, 0, :] * p[:, 0, :]; fv[:, -1, :] = -av[:, -1, :] * p[:, -1, :]
+    fw[1:-1] = aw[1:-1] * (p[1:] - p[:-1])
+    fw[0] = aw[0] * p[0]; fw[-1] = -aw[-1] * p[-1]
+    return c * ((fu[:, :, :-1] - fu[:, :, 1:]) + (fv[:, :-1, :] - fv[:, 1:, :]) + (fw[:-1] - fw[1:]))
+
+
 def run_sweep(args):
     """BASELINE.json configs[4]: MGPCG alone (nf_solve) on cubic all-Neumann grids with 200 random solid spheres,
     rhs N(0,1) with its mean removed, tol 1e-6: iterations, ms, Mcell-iterations/s, and the fp64 true residual of the
     answer evaluated on the host (the oracle's operator, one pass; the oracle does not solve at these sizes)."""
     import numpy as np
     import torch
-    from oracle import nf_oracle as orc   # (cpu_baseline-style use: residual evaluation only, outside the timed region)
     from paper_2405_14903_b200 import api, workloads as wl
     api.load_library()
     torch.cuda.set_device(0)
@@ -425,8 +437,7 @@ def run_sweep(args):
         ms = e0.elapsed_time(e1) / reps
         info = g.last_solve_info()
         nact = int(active.sum())
-        a64 = [a.astype(np.float64) for a in (au, av, aw)]
-        res = rhs.astype(np.float64) - orc.apply_A(p.cpu().numpy().astype(np.float64), a64, float(n))
+        res = rhs.astype(np.float64) - _apply_A_fp64(p.cpu().numpy().astype(np.float64), au, av, aw, float(n))
         res[~active] = 0.0
         res[active] -= res[active].mean()
         rows.append({"n": n, "rc": int(rc), "iters": info["iters"], "ms": round(ms, 3), "active_cells": nact,
