@@ -418,3 +418,32 @@ def test_error_codes(torch, api):
     assert lib.nf_solve(g.h, ctypes.c_void_p(p.data_ptr()), ctypes.c_void_p(p.data_ptr()), 1e-6, 10) == api.NF_ERR_INVALID
     assert g.project(u, v, w, p) == 0
     g.close()
+
+
+def test_degenerate_all_solid_and_single_cell(torch, api):
+    """Degenerate cases: a grid with no fluid at all (every weight 0: p = 0, U = U_s, no iteration), and a 1x1x1 grid."""
+    n = 8
+    phi = np.full((n + 1, n + 1, n + 1), -1.0, np.float32)  # solid everywhere
+    g = make_grid(api, n, n, n, 1.0 / n)
+    us = wl.random_velocity(np.random.default_rng(2), n, n, n, "uniform")
+    g.set_solid(dev(torch, phi), *[dev(torch, a) for a in us])
+    assert g.info()["active_cells"] == 0
+    U = [dev(torch, a) for a in wl.random_velocity(np.random.default_rng(3), n, n, n, "uniform")]
+    p = torch.full(g.shape_p, 7.0, dtype=torch.float32, device="cuda")
+    assert g.project(*U, p, tol=1e-6, maxit=50) == 0
+    assert g.last_solve_info()["iters"] == 0 and float(p.abs().max()) == 0.0
+    ref = orc.effective_solid_velocity(us, [a.shape for a in us], orc.BC())
+    for a, b in zip(U, ref):
+        assert np.array_equal(host(a), b.astype(np.float32).astype(np.float64))
+    G = [dev(torch, a) for a in us]
+    assert g.project_adjoint(*G, tol=1e-6, maxit=50) == 0   # M g = 0: dJ/dUhat = 0
+    assert all(float(a.abs().max()) == 0.0 for a in G)
+    g.close()
+    g = make_grid(api, 1, 1, 1, 1.0, bc_types=(1, 1, 0, 0, 0, 0), bc_values=(2.0, 0.0, 0, 0, 0, 0))
+    g.set_solid(dev(torch, np.ones((2, 2, 2), np.float32)))
+    U = [dev(torch, np.zeros(s, np.float32)) for s in wl.face_shapes(1, 1, 1)]
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    assert g.project(*U, p, tol=1e-6, maxit=50) == 0
+    assert abs(float(p[0, 0, 0]) - 1.0) <= 1e-6              # 2 alpha c (p - mean of the two ghosts) = 0
+    assert abs(float(U[0][0, 0, 0]) - 1.0) <= 1e-6 and abs(float(U[0][0, 0, 1]) - 1.0) <= 1e-6  # u = -c (p - ghost)
+    g.close()
