@@ -25,7 +25,7 @@ static cudaError_t dalloc(T **p, size_t n) {
 static void free_all(nf_grid *g) {
   for (int l = 0; l < NF_MAX_LEVELS; ++l) {
     NfLevel &L = g->lv[l];
-    cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.code); cudaFree(L.idg); cudaFree(L.z); cudaFree(L.r);
+    cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.code); cudaFree(L.idg); cudaFree(L.pk); cudaFree(L.z); cudaFree(L.r);
   }
   cudaFree(g->us); cudaFree(g->vs); cudaFree(g->ws); cudaFree(g->sdf);
   cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->b0); cudaFree(g->ecorr); cudaFree(g->r_alt); cudaFree(g->tailpack);
@@ -85,6 +85,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   }
   g->nlev = nl;
   nf_mg_plan(g);
+  for (int l = 2; l < g->tail && l < nl; ++l) ok = ok && dalloc(&g->lv[l].pk, 8 * (size_t)g->lv[l].ncell) == cudaSuccess;
   {
     size_t tc = 0;
     for (int l = g->tail; l < nl; ++l) tc += (size_t)g->lv[l].ncell;

@@ -762,8 +762,88 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS) k_tail(NfTailK T, const float
 // Levels first .. nb-1 run the vec bodies with grid-stride loops over the (4-cell row, j, k) tasks; phases are
 // separated by grid barriers instead of kernel boundaries (all of these levels are L2-resident at 256^3: 128^3 and
 // below), and CTA 0 runs the shared-memory tail between the down and the up sweep.
+// Per-cell ("dense") phases for the small levels (64^3 and below): one thread per cell, operator from the level's pack
+// (pk[0] = 1/(c diag), pk[1..6] = c alpha_f with faces towards the outside zeroed), every load issued up front -- ONE
+// round trip per phase.  (The 4-cells-per-thread code path costs two to three dependent round trips around a cut cell
+// -- code, then inverse diagonals, then fp32 weights -- and a grid-synchronised phase lasts as long as its slowest warp.)
+// Same arithmetic as the tail (nf_tail_half) and, up to rounding order, as the vec bodies.
+struct NfDenseLv {
+  const float *pk;
+  float *z, *r;
+  int nx, ny, nz, n;
+};
+__device__ __forceinline__ void nf_dense_nb(const NfDenseLv &D, int id, int nb[6]) {
+  const int sy = D.nx, sz = D.nx * D.ny;
+  nb[0] = max(id - 1, 0); nb[1] = min(id + 1, D.n - 1);
+  nb[2] = max(id - sy, 0); nb[3] = min(id + sy, D.n - 1);
+  nb[4] = max(id - sz, 0); nb[5] = min(id + sz, D.n - 1);
+}
+// pre-smooth from a zero guess, both colours in one phase: red z = r idg; black from its red neighbours' r idg
+__device__ __forceinline__ void nf_dense_down1(const NfDenseLv &D, int id) {
+  const int i = id % D.nx, j = (id / D.nx) % D.ny, k = id / (D.nx * D.ny);
+  const float idg = D.pk[id], rv = D.r[id];
+  float a = rv;
+  if ((i + j + k) & 1) {
+    int nb[6];
+    nf_dense_nb(D, id, nb);
+#pragma unroll
+    for (int f = 0; f < 6; ++f) a += D.pk[(1 + f) * D.n + id] * (D.r[nb[f]] * D.pk[nb[f]]);
+  }
+  D.z[id] = a * idg;
+}
+// residual + restriction of the coarse cell cid: red children only (the black residual is zero)
+__device__ __forceinline__ void nf_dense_down2(const NfDenseLv &D, float *rc, int cnx, int cny, int cid) {
+  const int I = cid % cnx, J = (cid / cnx) % cny, K = cid / (cnx * cny);
+  float acc = 0.0f;
+#pragma unroll
+  for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+    for (int dj = 0; dj < 2; ++dj)
+#pragma unroll
+      for (int di = 0; di < 2; ++di) {
+        if ((di + dj + dk) & 1) continue;
+        const int id = ((2 * K + dk) * D.ny + (2 * J + dj)) * D.nx + 2 * I + di;
+        int nb[6];
+        nf_dense_nb(D, id, nb);
+        float s = 0.0f;
+#pragma unroll
+        for (int f = 0; f < 6; ++f) s += D.pk[(1 + f) * D.n + id] * D.z[nb[f]];
+        if (D.pk[id] > 0.0f) acc += s;  // (r - A z = c sum alpha z_nb on a red cell: z = r / diag there)
+      }
+  rc[cid] = 0.125f * acc;
+}
+// black half sweep on z + P zc (red cells keep the un-prolonged value; the red sweep does not read it)
+__device__ __forceinline__ void nf_dense_up1(const NfDenseLv &D, const float *zc, int cnx, int cny, int id) {
+  const int i = id % D.nx, j = (id / D.nx) % D.ny, k = id / (D.nx * D.ny);
+  if (((i + j + k) & 1) == 0) return;
+  int nb[6];
+  nf_dense_nb(D, id, nb);
+  const int di[6] = {-1, 1, 0, 0, 0, 0}, dj[6] = {0, 0, -1, 1, 0, 0}, dk[6] = {0, 0, 0, 0, -1, 1};
+  float a = D.r[id];
+#pragma unroll
+  for (int f = 0; f < 6; ++f) {
+    const int ii = min(max(i + di[f], 0), D.nx - 1), jj = min(max(j + dj[f], 0), D.ny - 1),
+              kk = min(max(k + dk[f], 0), D.nz - 1);
+    a += D.pk[(1 + f) * D.n + id] * (D.z[nb[f]] + zc[((kk >> 1) * cny + (jj >> 1)) * cnx + (ii >> 1)]);
+  }
+  D.z[id] = a * D.pk[id];
+}
+// red half sweep (its black neighbours are final)
+__device__ __forceinline__ void nf_dense_up2(const NfDenseLv &D, int id) {
+  const int i = id % D.nx, j = (id / D.nx) % D.ny, k = id / (D.nx * D.ny);
+  if ((i + j + k) & 1) return;
+  int nb[6];
+  nf_dense_nb(D, id, nb);
+  float a = D.r[id];
+#pragma unroll
+  for (int f = 0; f < 6; ++f) a += D.pk[(1 + f) * D.n + id] * D.z[nb[f]];
+  D.z[id] = a * D.pk[id];
+}
+
 struct NfCoarseK {
   int first, nb, has_tail;
+  int dense_from;  // levels >= dense_from (and < nb) run the per-cell phases
+  const float *pk[NF_MAX_LEVELS];
   NfLvK lv[NF_MAX_LEVELS];
   float *z[NF_MAX_LEVELS], *r[NF_MAX_LEVELS];
   NfTailK T;
@@ -787,7 +867,9 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
     const NfLvK &L = P.lv[l];
     const size_t nc = (size_t)L.nx * L.ny * L.nz;
     for (size_t o = (size_t)gt * 128; o < nc; o += (size_t)gn * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.code + o));
-    if (l >= 2) {
+    if (l >= P.dense_from) {
+      for (size_t o = (size_t)gt * 32; o < 8 * nc; o += (size_t)gn * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.pk[l] + o));
+    } else if (l >= 2) {
       const size_t nxf = (size_t)L.nz * L.ny * L.pax, nyf = (size_t)L.nz * (L.ny + 1) * L.nx, nzf = (size_t)(L.nz + 1) * L.ny * L.nx;
       for (size_t o = (size_t)gt * 32; o < nc; o += (size_t)gn * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.idg + o));
       for (size_t o = (size_t)gt * 32; o < nxf; o += (size_t)gn * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.ax + o));
@@ -799,17 +881,28 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
     const NfLvK &L = P.lv[l];
     const int nx4 = L.nx >> 2, ny = L.ny, nz = L.nz;
     const int cnx = P.lv[l + 1].nx, cny = P.lv[l + 1].ny, cnz = P.lv[l + 1].nz;
-    for (int t = gt; t < nx4 * ny * nz; t += gn) {
-      const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
-      if ((j + k) & 1)
-        nf_down1_body<1>(L, P.r[l], P.z[l], i0, j, k);
-      else
-        nf_down1_body<0>(L, P.r[l], P.z[l], i0, j, k);
+    const bool dense = l >= P.dense_from;
+    NfDenseLv D;
+    D.pk = P.pk[l]; D.z = P.z[l]; D.r = P.r[l]; D.nx = L.nx; D.ny = ny; D.nz = nz; D.n = L.nx * ny * nz;
+    if (dense) {
+      for (int t = gt; t < D.n; t += gn) nf_dense_down1(D, t);
+    } else {
+      for (int t = gt; t < nx4 * ny * nz; t += gn) {
+        const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
+        if ((j + k) & 1)
+          nf_down1_body<1>(L, P.r[l], P.z[l], i0, j, k);
+        else
+          nf_down1_body<0>(L, P.r[l], P.z[l], i0, j, k);
+      }
     }
     grid.sync();
-    for (int t = gt; t < nx4 * cny * cnz; t += gn) {
-      const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
-      nf_down2_body(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
+    if (dense) {
+      for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t);
+    } else {
+      for (int t = gt; t < nx4 * cny * cnz; t += gn) {
+        const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
+        nf_down2_body(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
+      }
     }
     grid.sync();
   }
@@ -821,20 +914,31 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
     const NfLvK &L = P.lv[l];
     const int nx4 = L.nx >> 2, ny = L.ny, nz = L.nz;
     const int cnx = P.lv[l + 1].nx, cny = P.lv[l + 1].ny;
-    for (int t = gt; t < nx4 * ny * nz; t += gn) {
-      const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
-      if ((j + k) & 1)
-        nf_up1_body<1>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
-      else
-        nf_up1_body<0>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+    const bool dense = l >= P.dense_from;
+    NfDenseLv D;
+    D.pk = P.pk[l]; D.z = P.z[l]; D.r = P.r[l]; D.nx = L.nx; D.ny = ny; D.nz = nz; D.n = L.nx * ny * nz;
+    if (dense) {
+      for (int t = gt; t < D.n; t += gn) nf_dense_up1(D, P.z[l + 1], cnx, cny, t);
+    } else {
+      for (int t = gt; t < nx4 * ny * nz; t += gn) {
+        const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
+        if ((j + k) & 1)
+          nf_up1_body<1>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+        else
+          nf_up1_body<0>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+      }
     }
     grid.sync();
-    for (int t = gt; t < nx4 * ny * nz; t += gn) {
-      const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
-      if ((j + k) & 1)
-        nf_up2_body<1>(L, P.z[l], P.r[l], i0, j, k);
-      else
-        nf_up2_body<0>(L, P.z[l], P.r[l], i0, j, k);
+    if (dense) {
+      for (int t = gt; t < D.n; t += gn) nf_dense_up2(D, t);
+    } else {
+      for (int t = gt; t < nx4 * ny * nz; t += gn) {
+        const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
+        if ((j + k) & 1)
+          nf_up2_body<1>(L, P.z[l], P.r[l], i0, j, k);
+        else
+          nf_up2_body<0>(L, P.z[l], P.r[l], i0, j, k);
+      }
     }
     if (l > P.first) grid.sync();
   }
@@ -892,6 +996,12 @@ int nf_mg_init(nf_grid *g) {
 
 // (re)build the packed tail arrays from the current weights
 int nf_mg_pack_tail(nf_grid *g) {
+  for (int l = 2; l < g->tail && l < g->nlev; ++l) {  // the per-cell levels of k_vcoarse
+    NfLevel &L = g->lv[l];
+    if (!L.pk) continue;
+    const int n = (int)L.ncell;
+    NF_LAUNCH(g, NFK_COARSEN, k_tail_pack<<<(n + 255) / 256, 256, 0, g->stream>>>(L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, L.pk));
+  }
   size_t off = 0;
   for (int l = g->tail; l < g->nlev; ++l) {
     NfLevel &L = g->lv[l];
@@ -957,10 +1067,13 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
   if (coop) {
     NfCoarseK P;
     P.first = 1; P.nb = nb; P.has_tail = 1;
+    P.dense_from = NF_MAX_LEVELS;
     for (int l = 0; l < nl; ++l) {
       P.lv[l] = nf_lvk(g->lv[l]);
       P.z[l] = g->lv[l].z;
       P.r[l] = g->lv[l].r;
+      P.pk[l] = g->lv[l].pk;
+      if (l >= 2 && l < nb && g->lv[l].pk && P.dense_from == NF_MAX_LEVELS) P.dense_from = l;
     }
     int off = 0, m = 1;
     P.T.nlev = nl - g->tail;
