@@ -166,6 +166,14 @@ int nf_project_host(nf_grid *g, float *u, float *v, float *w, float *p, float to
 int nf_project_adjoint_host(nf_grid *g, float *gu, float *gv, float *gw, const float *p_saved,
                             const float *uhat_u, const float *uhat_v, const float *uhat_w, float tol, int maxit);
 
+/* The *_host calls copy H2D on one stream, compute on the handle's stream and copy D2H on a third, ordered by
+ * events.  By default they return when the host arrays hold the results.  nf_set_host_async(g, 1): they return as
+ * soon as the work is enqueued (the solve itself still ends before the return: the host drives it), so the D2H of one
+ * call overlaps the H2D and the kernels of the next; the host arrays are valid after nf_host_sync(g), which waits
+ * for every stream of the handle. */
+int nf_set_host_async(nf_grid *g, int on);
+int nf_host_sync(nf_grid *g);
+
 /* Info about the last solve on this handle.  Synchronises the handle's stream.
  * relres = ||r||_2/||rhs||_2 as tracked by the solver; ms = device time of the solve (CUDA events). */
 int nf_last_solve_info(nf_grid *g, int *iters, float *relres, float *ms);

@@ -37,6 +37,8 @@ _SIGNATURES = {
     "nf_weights_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
     "nf_apply_A": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p]),
     "nf_vcycle": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p]),
+    "nf_set_host_async": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
+    "nf_host_sync": (ctypes.c_int, [ctypes.c_void_p]),
     "nf_project_host": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4 + [ctypes.c_float, ctypes.c_int]),
     "nf_project_adjoint_host": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 7 + [ctypes.c_float, ctypes.c_int]),
     "nf_last_solve_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_int),
@@ -264,6 +266,12 @@ class Grid:
         self._expect(gw, self.shape_w, "gw", host=True)
         return self._check(self.lib.nf_project_adjoint_host(self.h, _ptr(gu), _ptr(gv), _ptr(gw), None, None, None,
                                                             None, float(tol), int(maxit)), "nf_project_adjoint_host")
+
+    def set_host_async(self, on=True):
+        self._check(self.lib.nf_set_host_async(self.h, 1 if on else 0), "nf_set_host_async")
+
+    def host_sync(self):
+        self._check(self.lib.nf_host_sync(self.h), "nf_host_sync")
 
     # -- info -------------------------------------------------------------------------------------------------
     def last_solve_info(self):

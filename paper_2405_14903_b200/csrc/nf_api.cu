@@ -36,6 +36,10 @@ static void free_all(nf_grid *g) {
   if (g->ev0) cudaEventDestroy(g->ev0);
   if (g->ev1) cudaEventDestroy(g->ev1);
   for (cudaEvent_t e : g->prof_pool) cudaEventDestroy(e);
+  if (g->hs_u) {
+    cudaStreamDestroy(g->s_h2d); cudaStreamDestroy(g->s_d2h);
+    cudaEventDestroy(g->ev_in); cudaEventDestroy(g->ev_comp); cudaEventDestroy(g->ev_out_proj); cudaEventDestroy(g->ev_out_adj);
+  }
   cudaFree(g->hs_u); cudaFree(g->hs_v); cudaFree(g->hs_w); cudaFree(g->hs_p);
   cudaFree(g->hs_a); cudaFree(g->hs_b); cudaFree(g->hs_c); cudaFree(g->hs_d);
 }
@@ -51,7 +55,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->nx = nx; g->ny = ny; g->nz = nz; g->dx = dx; g->dt_over_rho = 1.0f;
   for (int f = 0; f < 6; ++f) { g->bc_type[f] = NF_BC_CLOSED; g->bc_val[f] = 0.0f; }
   g->stream = 0;
-  g->nu_pre = 1; g->nu_post = 1; g->refine = 0; g->force_generic = false; g->refresh = true; g->warm = false;
+  g->nu_pre = 1; g->nu_post = 1; g->refine = 0; g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->nact = 0;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
@@ -296,25 +300,55 @@ static int ensure_host_staging(nf_grid *g) {
     g->err = "host-variant staging allocation failed";
     return NF_ERR_ALLOC;
   }
+  NF_CUDA(g, cudaStreamCreateWithFlags(&g->s_h2d, cudaStreamNonBlocking));
+  NF_CUDA(g, cudaStreamCreateWithFlags(&g->s_d2h, cudaStreamNonBlocking));
+  NF_CUDA(g, cudaEventCreateWithFlags(&g->ev_in, cudaEventDisableTiming));
+  NF_CUDA(g, cudaEventCreateWithFlags(&g->ev_comp, cudaEventDisableTiming));
+  NF_CUDA(g, cudaEventCreateWithFlags(&g->ev_out_proj, cudaEventDisableTiming));
+  NF_CUDA(g, cudaEventCreateWithFlags(&g->ev_out_adj, cudaEventDisableTiming));
   return NF_OK;
 }
 
+extern "C" int nf_set_host_async(nf_grid *g, int on) {
+  NF_CHECK_HANDLE(g);
+  g->host_async = on != 0;
+  return NF_OK;
+}
+
+extern "C" int nf_host_sync(nf_grid *g) {
+  NF_CHECK_HANDLE(g);
+  if (g->hs_u) {
+    NF_CUDA(g, cudaStreamSynchronize(g->s_d2h));
+    NF_CUDA(g, cudaStreamSynchronize(g->s_h2d));
+  }
+  NF_CUDA(g, cudaStreamSynchronize(g->stream));
+  return NF_OK;
+}
+
+// H2D on its own stream (after the previous D2H out of the same staging buffers), compute on the handle's stream,
+// D2H on a third: the two copy directions and the kernels of neighbouring calls overlap.
 extern "C" int nf_project_host(nf_grid *g, float *u, float *v, float *w, float *p, float tol, int maxit) {
   NF_CHECK_HANDLE(g);
   if (!u || !v || !w || !p) return NF_ERR_INVALID;
   if (!g->weights_set) return NF_ERR_STATE;
   NF_TRY(ensure_host_staging(g));
   const size_t bu = nf_nu(g) * sizeof(float), bv = nf_nv(g) * sizeof(float), bw = nf_nw(g) * sizeof(float);
-  NF_CUDA(g, cudaMemcpyAsync(g->hs_u, u, bu, cudaMemcpyHostToDevice, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(g->hs_v, v, bv, cudaMemcpyHostToDevice, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(g->hs_w, w, bw, cudaMemcpyHostToDevice, g->stream));
+  NF_CUDA(g, cudaStreamWaitEvent(g->s_h2d, g->ev_out_proj, 0));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_u, u, bu, cudaMemcpyHostToDevice, g->s_h2d));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_v, v, bv, cudaMemcpyHostToDevice, g->s_h2d));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_w, w, bw, cudaMemcpyHostToDevice, g->s_h2d));
+  NF_CUDA(g, cudaEventRecord(g->ev_in, g->s_h2d));
+  NF_CUDA(g, cudaStreamWaitEvent(g->stream, g->ev_in, 0));
   int rc = nf_project(g, g->hs_u, g->hs_v, g->hs_w, g->hs_p, tol, maxit);
   if (rc < 0) return rc;
-  NF_CUDA(g, cudaMemcpyAsync(u, g->hs_u, bu, cudaMemcpyDeviceToHost, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(v, g->hs_v, bv, cudaMemcpyDeviceToHost, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(w, g->hs_w, bw, cudaMemcpyDeviceToHost, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(p, g->hs_p, nf_nc(g) * sizeof(float), cudaMemcpyDeviceToHost, g->stream));
-  NF_CUDA(g, cudaStreamSynchronize(g->stream));
+  NF_CUDA(g, cudaEventRecord(g->ev_comp, g->stream));
+  NF_CUDA(g, cudaStreamWaitEvent(g->s_d2h, g->ev_comp, 0));
+  NF_CUDA(g, cudaMemcpyAsync(p, g->hs_p, nf_nc(g) * sizeof(float), cudaMemcpyDeviceToHost, g->s_d2h));
+  NF_CUDA(g, cudaMemcpyAsync(u, g->hs_u, bu, cudaMemcpyDeviceToHost, g->s_d2h));
+  NF_CUDA(g, cudaMemcpyAsync(v, g->hs_v, bv, cudaMemcpyDeviceToHost, g->s_d2h));
+  NF_CUDA(g, cudaMemcpyAsync(w, g->hs_w, bw, cudaMemcpyDeviceToHost, g->s_d2h));
+  NF_CUDA(g, cudaEventRecord(g->ev_out_proj, g->s_d2h));
+  if (!g->host_async) NF_CUDA(g, cudaStreamSynchronize(g->s_d2h));
   return rc;
 }
 
@@ -327,16 +361,22 @@ extern "C" int nf_project_adjoint_host(nf_grid *g, float *gu, float *gv, float *
   if (!g->weights_set) return NF_ERR_STATE;
   NF_TRY(ensure_host_staging(g));
   const size_t bu = nf_nu(g) * sizeof(float), bv = nf_nv(g) * sizeof(float), bw = nf_nw(g) * sizeof(float);
-  NF_CUDA(g, cudaMemcpyAsync(g->hs_a, gu, bu, cudaMemcpyHostToDevice, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(g->hs_b, gv, bv, cudaMemcpyHostToDevice, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(g->hs_c, gw, bw, cudaMemcpyHostToDevice, g->stream));
+  NF_CUDA(g, cudaStreamWaitEvent(g->s_h2d, g->ev_out_adj, 0));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_a, gu, bu, cudaMemcpyHostToDevice, g->s_h2d));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_b, gv, bv, cudaMemcpyHostToDevice, g->s_h2d));
+  NF_CUDA(g, cudaMemcpyAsync(g->hs_c, gw, bw, cudaMemcpyHostToDevice, g->s_h2d));
+  NF_CUDA(g, cudaEventRecord(g->ev_in, g->s_h2d));
+  NF_CUDA(g, cudaStreamWaitEvent(g->stream, g->ev_in, 0));
   int rc = nf_project_adjoint(g, g->hs_a, g->hs_b, g->hs_c, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
                               nullptr, nullptr, nullptr, nullptr, nullptr, tol, maxit);
   if (rc < 0) return rc;
-  NF_CUDA(g, cudaMemcpyAsync(gu, g->hs_a, bu, cudaMemcpyDeviceToHost, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(gv, g->hs_b, bv, cudaMemcpyDeviceToHost, g->stream));
-  NF_CUDA(g, cudaMemcpyAsync(gw, g->hs_c, bw, cudaMemcpyDeviceToHost, g->stream));
-  NF_CUDA(g, cudaStreamSynchronize(g->stream));
+  NF_CUDA(g, cudaEventRecord(g->ev_comp, g->stream));
+  NF_CUDA(g, cudaStreamWaitEvent(g->s_d2h, g->ev_comp, 0));
+  NF_CUDA(g, cudaMemcpyAsync(gu, g->hs_a, bu, cudaMemcpyDeviceToHost, g->s_d2h));
+  NF_CUDA(g, cudaMemcpyAsync(gv, g->hs_b, bv, cudaMemcpyDeviceToHost, g->s_d2h));
+  NF_CUDA(g, cudaMemcpyAsync(gw, g->hs_c, bw, cudaMemcpyDeviceToHost, g->s_d2h));
+  NF_CUDA(g, cudaEventRecord(g->ev_out_adj, g->s_d2h));
+  if (!g->host_async) NF_CUDA(g, cudaStreamSynchronize(g->s_d2h));
   return rc;
 }
 

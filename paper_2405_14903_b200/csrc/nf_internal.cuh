@@ -133,6 +133,10 @@ struct nf_grid {
   long long prof_n[NFK_COUNT];
   // host staging for the *_host entry points
   float *hs_u, *hs_v, *hs_w, *hs_p, *hs_a, *hs_b, *hs_c, *hs_d;
+  // copy streams of the *_host entry points (H2D and D2H run on their own streams, ordered by events)
+  cudaStream_t s_h2d, s_d2h;
+  cudaEvent_t ev_in, ev_comp, ev_out_proj, ev_out_adj;
+  bool host_async;  // nf_set_host_async: *_host calls return before their D2H copies finish (nf_host_sync waits)
 };
 
 void nf_prof_begin(nf_grid *g, int cls);

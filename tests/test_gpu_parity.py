@@ -447,3 +447,29 @@ def test_degenerate_all_solid_and_single_cell(torch, api):
     assert abs(float(p[0, 0, 0]) - 1.0) <= 1e-6              # 2 alpha c (p - mean of the two ghosts) = 0
     assert abs(float(U[0][0, 0, 0]) - 1.0) <= 1e-6 and abs(float(U[0][0, 0, 1]) - 1.0) <= 1e-6  # u = -c (p - ghost)
     g.close()
+
+
+def test_host_buffer_entry_points_sync_and_async(torch, api):
+    """nf_project_host / nf_project_adjoint_host (pinned host arrays in, results out) equal the device-pointer calls,
+    in the default synchronous mode and in host-async mode (+ nf_host_sync)."""
+    c = wl.config1()
+    n = c["nx"]
+    g = make_grid(api, n, n, n, c["dx"])
+    g.set_solid(dev(torch, c["phi"]))
+    U = [dev(torch, a) for a in c["U"]]
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    assert g.project(*U, p, tol=1e-6, maxit=200) == 0
+    G = [dev(torch, a) for a in c["g"]]
+    assert g.project_adjoint(*G, tol=1e-6, maxit=200) == 0
+    for mode in (False, True):
+        g.set_host_async(mode)
+        hU = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in c["U"]]
+        hG = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in c["g"]]
+        hp = torch.empty(g.shape_p, dtype=torch.float32).pin_memory()
+        assert g.project_host(*hU, hp, tol=1e-6, maxit=200) == 0
+        assert g.project_adjoint_host(*hG, tol=1e-6, maxit=200) == 0
+        g.host_sync()
+        assert rel(hp.numpy(), host(p)) <= 1e-5
+        assert rel3([a.numpy() for a in hU], [host(a) for a in U]) <= 1e-5
+        assert rel3([a.numpy() for a in hG], [host(a) for a in G]) <= 1e-5
+    g.close()
