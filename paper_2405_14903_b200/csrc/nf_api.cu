@@ -55,7 +55,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->nx = nx; g->ny = ny; g->nz = nz; g->dx = dx; g->dt_over_rho = 1.0f;
   for (int f = 0; f < 6; ++f) { g->bc_type[f] = NF_BC_CLOSED; g->bc_val[f] = 0.0f; }
   g->stream = 0;
-  g->nu_pre = 1; g->nu_post = 1; g->refine = 0; g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
+  g->nu_pre = 1; g->nu_post = 1; g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->nact = 0;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
@@ -159,7 +159,7 @@ extern "C" int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value) {
 extern "C" int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags) {
   NF_CHECK_HANDLE(g);
   if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || flags < 0 || flags > 15) return NF_ERR_INVALID;
-  g->nu_pre = nu_pre; g->nu_post = nu_post; g->refine = flags & 1; g->force_generic = (flags & 2) != 0; g->refresh = (flags & 4) == 0; g->warm = (flags & 8) != 0;
+  g->nu_pre = nu_pre; g->nu_post = nu_post; g->force_generic = (flags & 2) != 0; g->refresh = (flags & 4) == 0; g->warm = (flags & 8) != 0;
   return NF_OK;
 }
 

@@ -100,7 +100,7 @@ struct nf_grid {
   bool weights_set, have_sdf, have_us;
   int singular;
   long long nact;
-  int nu_pre, nu_post, refine;
+  int nu_pre, nu_post;
   bool warm;     // flag 8 of nf_set_solver_options: caller-provided solution arrays hold the initial guess
   bool refresh;  // true-residual refresh between two PCG phases (default on; flag 4 of nf_set_solver_options: off)
   bool force_generic;  // test hook: run the generic (fp32-weight, one colour per launch) kernels everywhere

@@ -281,15 +281,6 @@ __global__ void __launch_bounds__(256) k_cg_pupdate(float *__restrict__ p, const
   }
 }
 
-__global__ void __launch_bounds__(256) k_dot(const float *__restrict__ a, const float *__restrict__ b, size_t n,
-                                             double *dst, const NfSolveState *st) {
-  if (st && st->done) return;
-  double part = 0.0;
-  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
-  for (size_t t = tid; t < n; t += nth) part += (double)a[t] * (double)b[t];
-  nf_block_atomic_add(part, dst);
-}
-
 // ------------------------------------------------------------------------------------------------------------
 // solve set-up: r = mask(src), sum over active cells; then mean removal (singular, R12) and bb = ||r||^2
 // ------------------------------------------------------------------------------------------------------------
