@@ -54,7 +54,8 @@ const char *nf_version(void);
 
 /* Create a handle for an nx*ny*nz MAC grid with spacing dx.  Allocates the multigrid
  * hierarchy ("hierarchical grid data structure") and all solver scratch on the current
- * CUDA device.  Defaults: six closed walls, dt_over_rho = 1, stream 0.  Arrays are addressed with 32-bit
+ * CUDA device.  Defaults: six closed walls, dt_over_rho = 1, stream 0.  nz == 1 selects 2-D mode (the hierarchy
+ * coarsens x and y only; the two z-walls stay closed).  Arrays are addressed with 32-bit
  * offsets: (nx+8)(ny+1)(nz+1) must stay below 2^32 (about 1600^3), and nf_advect below 2^31 nodes; larger
  * grids return NF_ERR_INVALID. */
 int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out);

@@ -82,9 +82,18 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     if (ok) ok = cudaMemset(L.ax, 0, (size_t)lz * ly * L.pax * sizeof(float)) == cudaSuccess;
     ++nl;
     if (!ok || nl >= NF_MAX_LEVELS) break;
-    if ((lx | ly | lz) & 1) break;
-    if (lx / 2 < 4 || ly / 2 < 4 || lz / 2 < 4) break;
-    lx /= 2; ly /= 2; lz /= 2;
+    // 2-D mode (nz == 1): x and y coarsen, z stays one layer
+    const bool flat = nz == 1;
+    L.fz = flat ? 1 : 2;
+    if (flat) {
+      if ((lx | ly) & 1) break;
+      if (lx / 2 < 4 || ly / 2 < 4) break;
+      lx /= 2; ly /= 2;
+    } else {
+      if ((lx | ly | lz) & 1) break;
+      if (lx / 2 < 4 || ly / 2 < 4 || lz / 2 < 4) break;
+      lx /= 2; ly /= 2; lz /= 2;
+    }
     c *= 0.25f;
   }
   g->nlev = nl;

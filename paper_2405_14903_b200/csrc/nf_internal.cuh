@@ -35,6 +35,7 @@ struct NfLevel {
   float *idg;    // 1 / (c_l * sum of the six weights), 0 on inactive cells (written with the codes)
   float *z, *r;  // level 0: CG vectors z and r; level > 0: coarse correction and restricted residual
   float *pk;     // levels 2 .. tail-1 (k_vcoarse's per-cell phases): idg[n], c*alpha_f[6][n] (0 towards outside), unused[n]
+  int fz;         // z-coarsening factor towards the next level: 2, or 1 in 2-D mode (nz == 1: x and y coarsen only)
   int vec_idx32;  // 1: every array of the level has < 2^32 slots (32-bit offsets in the stencil kernels)
   int vec;       // 1: nx % 4 == 0 and a coarser level exists -> the float4 / code kernels run on this level
 };

@@ -425,7 +425,7 @@ __global__ void __launch_bounds__(256) k_residual_restrict(const float *__restri
                                                            const float *__restrict__ ax, const float *__restrict__ ay,
                                                            const float *__restrict__ az, float c, int nx, int ny,
                                                            int nz, int pax, float *__restrict__ rc, int cnx, int cny,
-                                                           int cnz, const NfSolveState *st) {
+                                                           int cnz, int fz, const NfSolveState *st) {
   if (st && st->done) return;
   const int I = blockIdx.x * blockDim.x + threadIdx.x;
   const int J = blockIdx.y * blockDim.y + threadIdx.y;
@@ -438,23 +438,24 @@ __global__ void __launch_bounds__(256) k_residual_restrict(const float *__restri
     for (int dj = 0; dj < 2; ++dj)
 #pragma unroll
       for (int di = 0; di < 2; ++di) {
-        const int i = 2 * I + di, j = 2 * J + dj, k = 2 * K + dk;
+        if (dk >= fz) continue;  // (2-D mode: the children are the 2 x 2 x 1 cells)
+        const int i = 2 * I + di, j = 2 * J + dj, k = fz * K + dk;
         const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
         const size_t id = ((size_t)k * ny + j) * nx + i;
         acc += r[id] - c * (nf_w6_sum(w) * z[id] - nf_nb_sum(z, w, i, j, k, nx, ny, nz));
       }
-  rc[((size_t)K * cny + J) * cnx + I] = 0.125f * acc;
+  rc[((size_t)K * cny + J) * cnx + I] = (fz == 2 ? 0.125f : 0.25f) * acc;
 }
 
 // z_f += z_c[parent]   (piecewise-constant prolongation)
 __global__ void __launch_bounds__(256) k_prolong_add(float *__restrict__ z, const float *__restrict__ zc, int nx,
-                                                     int ny, int nz, int cnx, int cny, const NfSolveState *st) {
+                                                     int ny, int nz, int cnx, int cny, int fz, const NfSolveState *st) {
   if (st && st->done) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z * blockDim.z + threadIdx.z;
   if (i >= nx || j >= ny || k >= nz) return;
-  z[((size_t)k * ny + j) * nx + i] += __ldg(zc + ((size_t)(k >> 1) * cny + (j >> 1)) * cnx + (i >> 1));
+  z[((size_t)k * ny + j) * nx + i] += __ldg(zc + ((size_t)(fz == 2 ? k >> 1 : k) * cny + (j >> 1)) * cnx + (i >> 1));
 }
 
 __global__ void __launch_bounds__(256) k_dot_rz(const float *__restrict__ a, const float *__restrict__ b, size_t n,
@@ -476,6 +477,7 @@ struct NfTailK {
   int singular;  // the system has the constant null vector (R12): the coarsest solve works in its complement
   int n[NF_MAX_LEVELS], nx[NF_MAX_LEVELS], ny[NF_MAX_LEVELS], nz[NF_MAX_LEVELS];
   int off[NF_MAX_LEVELS];  // offset (in cells) of the level in the packed arrays
+  int fz[NF_MAX_LEVELS];   // z-coarsening factor towards the next level (1 in 2-D mode)
 };
 
 __global__ void __launch_bounds__(256) k_tail_pack(const float *__restrict__ ax, const float *__restrict__ ay,
@@ -661,7 +663,7 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, true);
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
     // residual + restriction: r_c = 1/8 sum children (r - A z), A z = z/idg - sum wg z_nb on active cells
-    const int cn = T.n[l + 1], cnx = T.nx[l + 1], cny = T.ny[l + 1];
+    const int cn = T.n[l + 1], cnx = T.nx[l + 1], cny = T.ny[l + 1], fz = T.fz[l];
     float *rc = sm + 10 * (size_t)T.off[l + 1] + cn;
     const int sy = nx, sz = nx * ny;
     for (int cidx = threadIdx.x; cidx < cn; cidx += blockDim.x) {
@@ -674,8 +676,8 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
 #pragma unroll
           for (int di = 0; di < 2; ++di) {
             // (the residual is zero on the black cells: the black half sweep has just solved their equations)
-            if ((di + dj + dk) & 1) continue;
-            const int id = ((2 * K + dk) * ny + (2 * J + dj)) * nx + 2 * I + di;
+            if (((di + dj + dk) & 1) || dk >= fz) continue;
+            const int id = ((fz * K + dk) * ny + (2 * J + dj)) * nx + 2 * I + di;
             const float s = pk[1 * n + id] * z[max(id - 1, 0)] + pk[2 * n + id] * z[min(id + 1, n - 1)] +
                       pk[3 * n + id] * z[max(id - sy, 0)] + pk[4 * n + id] * z[min(id + sy, n - 1)] +
                       pk[5 * n + id] * z[max(id - sz, 0)] + pk[6 * n + id] * z[min(id + sz, n - 1)];
@@ -683,7 +685,7 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
             // c*diag = 1/idg on active cells (includes faces towards Dirichlet ghosts); inactive: r = 0, z = 0
             if (idg > 0.0f) acc += r[id] - (z[id] / idg - s);
           }
-      rc[cidx] = 0.125f * acc;
+      rc[cidx] = (fz == 2 ? 0.125f : 0.25f) * acc;
     }
     __syncthreads();
   }
@@ -731,11 +733,11 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
   for (int l = nl - 2; l >= 0; --l) {
     const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
     float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
-    const int cnx = T.nx[l + 1], cny = T.ny[l + 1];
+    const int cnx = T.nx[l + 1], cny = T.ny[l + 1], fz = T.fz[l];
     const float *zc = sm + 10 * (size_t)T.off[l + 1];
     for (int id = threadIdx.x; id < n; id += blockDim.x) {
       const int i = id % nx, j = (id / nx) % ny, k = id / (nx * ny);
-      z[id] += zc[((k >> 1) * cny + (j >> 1)) * cnx + (i >> 1)];
+      z[id] += zc[((fz == 2 ? k >> 1 : k) * cny + (j >> 1)) * cnx + (i >> 1)];
     }
     __syncthreads();
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
@@ -969,7 +971,7 @@ void nf_mg_plan(nf_grid *g) {
     const NfLevel &L = g->lv[l];
     const double slots = (double)(L.nz + 1) * (L.ny + 1) * (L.pax + 4);  // largest face array of the level
     g->lv[l].vec_idx32 = slots < 4.0e9 ? 1 : 0;
-    g->lv[l].vec = (l < nb && (L.nx & 3) == 0 && g->lv[l].vec_idx32) ? 1 : 0;
+    g->lv[l].vec = (l < nb && (L.nx & 3) == 0 && g->lv[l].vec_idx32 && L.fz == 2) ? 1 : 0;
   }
 }
 
@@ -1061,7 +1063,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
         smooth_half(g, L, 1, false, false, st, slot);
       }
       NfDims d = nf_dims(C.nx, C.ny, C.nz);
-      NF_LAUNCH(g, (l == 0 ? NFK_RESTRICT0 : NFK_RESTRICT_C), k_residual_restrict<<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, C.r, C.nx, C.ny, C.nz, st));
+      NF_LAUNCH(g, (l == 0 ? NFK_RESTRICT0 : NFK_RESTRICT_C), k_residual_restrict<<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, C.r, C.nx, C.ny, C.nz, L.fz, st));
     }
   }
   if (coop) {
@@ -1080,7 +1082,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
     for (int l = g->tail; l < nl; ++l) {
       const NfLevel &L = g->lv[l];
       const int t = l - g->tail;
-      P.T.n[t] = (int)L.ncell; P.T.nx[t] = L.nx; P.T.ny[t] = L.ny; P.T.nz[t] = L.nz; P.T.off[t] = off;
+      P.T.n[t] = (int)L.ncell; P.T.nx[t] = L.nx; P.T.ny[t] = L.ny; P.T.nz[t] = L.nz; P.T.off[t] = off; P.T.fz[t] = L.fz;
       off += (int)L.ncell;
       if (l == nl - 1) m = L.nx > L.ny ? (L.nx > L.nz ? L.nx : L.nz) : (L.ny > L.nz ? L.ny : L.nz);
     }
@@ -1097,7 +1099,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
     for (int l = g->tail; l < nl; ++l) {
       const NfLevel &L = g->lv[l];
       const int t = l - g->tail;
-      T.n[t] = (int)L.ncell; T.nx[t] = L.nx; T.ny[t] = L.ny; T.nz[t] = L.nz; T.off[t] = off;
+      T.n[t] = (int)L.ncell; T.nx[t] = L.nx; T.ny[t] = L.ny; T.nz[t] = L.nz; T.off[t] = off; T.fz[t] = L.fz;
       off += (int)L.ncell;
       if (l == nl - 1) m = L.nx > L.ny ? (L.nx > L.nz ? L.nx : L.nz) : (L.ny > L.nz ? L.ny : L.nz);
     }
@@ -1130,7 +1132,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
       }
     } else {
       NfDims d = nf_dims(L.nx, L.ny, L.nz);
-      NF_LAUNCH(g, (l == 0 ? NFK_PROLONG0 : NFK_PROLONG_C), k_prolong_add<<<d.grid, d.block, 0, g->stream>>>(L.z, C.z, L.nx, L.ny, L.nz, C.nx, C.ny, st));
+      NF_LAUNCH(g, (l == 0 ? NFK_PROLONG0 : NFK_PROLONG_C), k_prolong_add<<<d.grid, d.block, 0, g->stream>>>(L.z, C.z, L.nx, L.ny, L.nz, C.nx, C.ny, L.fz, st));
       for (int s = 0; s < g->nu_post; ++s) {
         const bool dot = with_dot && l == 0 && s == g->nu_post - 1;
         smooth_half(g, L, 1, false, false, st, slot);

@@ -232,26 +232,29 @@ __global__ void __launch_bounds__(256) k_weights_export(const float *__restrict_
   au[((size_t)k * ny + j) * (nx + 1) + i] = ax[((size_t)k * ny + j) * pax + i];
 }
 
-// Coarse face weight = arithmetic mean of the four coincident fine face weights (R13).
+// Coarse face weight = arithmetic mean of the coincident fine face weights (R13): four of them,
+// or -- in 2-D mode, fz == 1, where z does not coarsen -- the two of an x- or y-face and the four of a z-face.
 __global__ void __launch_bounds__(256) k_coarsen_weights(const float *__restrict__ fax, const float *__restrict__ fay,
                                                          const float *__restrict__ faz, float *__restrict__ cax,
                                                          float *__restrict__ cay, float *__restrict__ caz, int fnx,
                                                          int fny, int fnz, int fpax, int cnx, int cny, int cnz,
-                                                         int cpax) {
+                                                         int cpax, int fz) {
   const int I = blockIdx.x * blockDim.x + threadIdx.x;
   const int J = blockIdx.y * blockDim.y + threadIdx.y;
   const int K = blockIdx.z * blockDim.z + threadIdx.z;
   if (I > cnx || J > cny || K > cnz) return;
-  const int i = 2 * I, j = 2 * J, k = 2 * K;
+  const int i = 2 * I, j = 2 * J, k = fz * K;
   if (J < cny && K < cnz) {
     const float *b = fax + ((size_t)k * fny + j) * fpax + i;
     const size_t sj = fpax, sk = (size_t)fny * fpax;
-    cax[((size_t)K * cny + J) * cpax + I] = 0.25f * ((b[0] + b[sj]) + (b[sk] + b[sk + sj]));
+    cax[((size_t)K * cny + J) * cpax + I] =
+        fz == 2 ? 0.25f * ((b[0] + b[sj]) + (b[sk] + b[sk + sj])) : 0.5f * (b[0] + b[sj]);
   }
   if (I < cnx && K < cnz) {
     const float *b = fay + ((size_t)k * (fny + 1) + j) * fnx + i;
     const size_t sk = (size_t)(fny + 1) * fnx;
-    cay[((size_t)K * (cny + 1) + J) * cnx + I] = 0.25f * ((b[0] + b[1]) + (b[sk] + b[sk + 1]));
+    cay[((size_t)K * (cny + 1) + J) * cnx + I] =
+        fz == 2 ? 0.25f * ((b[0] + b[1]) + (b[sk] + b[sk + 1])) : 0.5f * (b[0] + b[1]);
   }
   if (I < cnx && J < cny) {
     const float *b = faz + ((size_t)k * fny + j) * fnx + i;
@@ -383,7 +386,7 @@ int nf_build_hierarchy(nf_grid *g) {
     NfLevel &F = g->lv[l], &C = g->lv[l + 1];
     NfDims d = nf_dims(C.nx + 1, C.ny + 1, C.nz + 1);
     NF_LAUNCH(g, NFK_COARSEN, k_coarsen_weights<<<d.grid, d.block, 0, g->stream>>>(F.ax, F.ay, F.az, C.ax, C.ay, C.az, F.nx, F.ny, F.nz, F.pax,
-                                                         C.nx, C.ny, C.nz, C.pax));
+                                                         C.nx, C.ny, C.nz, C.pax, F.fz));
   }
   double *cnt = g->d_counts;
   NF_CUDA(g, cudaMemsetAsync(cnt, 0, 2 * sizeof(double), g->stream));

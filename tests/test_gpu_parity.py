@@ -473,3 +473,37 @@ def test_host_buffer_entry_points_sync_and_async(torch, api):
         assert rel3([a.numpy() for a in hU], [host(a) for a in U]) <= 1e-5
         assert rel3([a.numpy() for a in hG], [host(a) for a in G]) <= 1e-5
     g.close()
+
+
+@pytest.mark.parametrize("shape,dirichlet", [((64, 48, 1), True), ((128, 96, 1), False), ((36, 20, 1), True)])
+def test_two_dimensional_mode(torch, api, shape, dirichlet):
+    """NEXT-3: nz = 1 grids -- the hierarchy coarsens x and y only (2 x 2 x 1 children, restriction
+    P^T / 4), so the paper's 2-D tasks get multigrid convergence.  Projection + adjoint against the oracle."""
+    nx, ny, nz = shape
+    rng = np.random.default_rng(21)
+    bt = (1, 1, 0, 0, 0, 0) if dirichlet else (0,) * 6
+    bv = (1.0, 0.0, 0, 0, 0, 0) if dirichlet else (0.0,) * 6
+    x, y, z = wl.node_coords(nx, ny, nz)
+    phi = np.full((nz + 1, ny + 1, nx + 1), 1e9)
+    for c, r in (((0.3 * nx, 0.5 * ny), 0.12 * ny), ((0.65 * nx, 0.35 * ny), 0.1 * ny)):  # two cylinders along z
+        phi = np.minimum(phi, np.sqrt((x - c[0]) ** 2 + (y - c[1]) ** 2) - r)
+    phi = phi.astype(np.float32)
+    bc = orc.BC(bt, bv)
+    U = wl.random_velocity(rng, nx, ny, nz, "uniform")
+    Gin = wl.random_velocity(rng, nx, ny, nz, "normal")
+    g = make_grid(api, nx, ny, nz, 1.0 / nx, bc_types=bt, bc_values=bv)
+    g.set_solid(dev(torch, phi))
+    assert g.info()["levels"] >= 3
+    alpha = [host(a) for a in g.get_weights()]
+    Uo, po = orc.project(U, alpha, None, 1.0 / nx, 1.0, bc, tol=1e-12)
+    dU = [dev(torch, a) for a in U]
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    assert g.project(*dU, p, tol=1e-6, maxit=200) == 0
+    assert g.last_solve_info()["iters"] <= 40       # multigrid-like, not the hundreds of an unpreconditioned solve
+    assert rel(host(p), po) <= TOL_FIELD
+    assert rel3([host(a) for a in dU], Uo) <= TOL_FIELD
+    gref, _, _, _ = orc.project_adjoint(Gin, alpha, po, U, None, 1.0 / nx, 1.0, bc, tol=1e-12)
+    dG = [dev(torch, a) for a in Gin]
+    assert g.project_adjoint(*dG, tol=1e-6, maxit=200) == 0
+    assert rel3([host(a) for a in dG], gref) <= TOL_FIELD
+    g.close()
