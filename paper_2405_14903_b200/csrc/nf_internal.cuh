@@ -188,7 +188,7 @@ static inline NfDims nf_dims(int tx, int ty, int tz) {
 // 64 x 4 threads, and every CTA marches through `kch` consecutive z-planes (blockIdx.z = chunk): 8x fewer CTAs (and
 // reduction atomics) than one plane per CTA, and the z-neighbour rows of one plane are the L1-resident centre rows
 // of the next.
-#define NF_KCH_MG 4  // planes per CTA: V-cycle kernels (measured in situ at 256^3: 1 -> 4 saves 10-20 % per kernel)
+#define NF_KCH_MG 8  // planes per CTA: V-cycle kernels (measured in situ at 256^3: 1 -> 4 saves 10-20 % per kernel, 4 -> 8 another 1-4 %)
 #define NF_KCH_AP 8  // planes per CTA: A-apply (z-neighbour rows rotate through registers)
 static inline NfDims nf_vdims(int tx, int ty, int tz, int kch) {
   int bx = 1;
