@@ -442,6 +442,41 @@ __global__ void __launch_bounds__(256) k_true_residual(float *__restrict__ r, co
   }
   nf_block_atomic_add(part, &st->rr[0]);
 }
+// The same on float4 rows with the weights from the 1-byte codes (4 cells per thread, fp64 arithmetic).
+__global__ void __launch_bounds__(256, 4) k_true_residual4(NfLvK L, float *__restrict__ r, const float *__restrict__ b0,
+                                                        const float *__restrict__ x, NfSolveState *st) {
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z * blockDim.z + threadIdx.z;
+  double part = 0.0;
+  if (i0 < L.nx && j < L.ny && k < L.nz) {
+    const int nx = L.nx, ny = L.ny, nz = L.nz;
+    const nf_idx sy = nx, sz = (nf_idx)nx * ny, id = ((nf_idx)k * ny + j) * nx + i0;
+    float pc[4], yl[4], yh[4], zl[4], zh[4], bb[4], out[4];
+    nf_unpack4(nf_ld4(x, id, true), pc);
+    nf_unpack4(nf_ld4(x, id - sy, j > 0), yl);
+    nf_unpack4(nf_ld4(x, id + sy, j + 1 < ny), yh);
+    nf_unpack4(nf_ld4(x, id - sz, k > 0), zl);
+    nf_unpack4(nf_ld4(x, id + sz, k + 1 < nz), zh);
+    nf_unpack4(nf_ld4(b0, id, true), bb);
+    const float xl = nf_ld1(x, id - 1, i0 > 0), xh = nf_ld1(x, id + 4, i0 + 4 < nx);
+    const unsigned c4 = nf_ldc4(L.code, id, true);
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      const unsigned code = nf_code_at(c4, t);
+      const NfW6 w = nf_code_w6(L, code, i0 + t, j, k);
+      const double c0 = pc[t], l = t > 0 ? pc[t - 1] : xl, h = t < 3 ? pc[t + 1] : xh;
+      const double s = (((double)w.xl * (c0 - l) + (double)w.xh * (c0 - h)) +
+                        ((double)w.yl * (c0 - (double)yl[t]) + (double)w.yh * (c0 - (double)yh[t]))) +
+                       ((double)w.zl * (c0 - (double)zl[t]) + (double)w.zh * (c0 - (double)zh[t]));
+      const double v = code ? (double)bb[t] - (double)L.c * s : 0.0;
+      out[t] = (float)v;
+      part += v * v;
+    }
+    *reinterpret_cast<float4 *>(r + id) = make_float4(out[0], out[1], out[2], out[3]);
+  }
+  nf_block_atomic_add(part, &st->rr[0]);
+}
 // warm start: the initial guess on the active cells only (0 elsewhere), and 0 everywhere when b = 0 (done is then
 // already set by k_start_state: the answer is x = 0)
 __global__ void __launch_bounds__(256) k_warm_mask(float *__restrict__ x, const uint8_t *__restrict__ code, size_t n,
@@ -665,7 +700,12 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
   // correction e accumulated on its own, x += e once.  Used for the refresh and for a warm start.
   auto correct = [&](float tolp) -> int {
     NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)tolp, 0));
-    NF_LAUNCH(g, NFK_SETUP, k_true_residual<<<dc.grid, dc.block, 0, g->stream>>>(L.r, g->b0, x, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->st));
+    if (!g->force_generic && apply_vec_ok(L, x, L.r) && apply_vec_ok(L, g->b0, g->b0)) {
+      NfDims dv = nf_dims(L.nx / 4, L.ny, L.nz);
+      NF_LAUNCH(g, NFK_SETUP, k_true_residual4<<<dv.grid, dv.block, 0, g->stream>>>(nf_lvk(L), L.r, g->b0, x, g->st));
+    } else {
+      NF_LAUNCH(g, NFK_SETUP, k_true_residual<<<dc.grid, dc.block, 0, g->stream>>>(L.r, g->b0, x, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->st));
+    }
     g->hst[0].seq = 0;
     NF_LAUNCH(g, NFK_SETUP, k_phase_check<<<1, 32, 0, g->stream>>>(g->st, (double)tol, &g->hst_dev[0], 1));
     NF_CUDA(g, cudaGetLastError());
