@@ -258,7 +258,8 @@ def _velocity_points(params, pdot, K, N, M, X, Y, z):
     q the closest point of the section's polygon (segment k, parameter tau held fixed) and nh the unit vector from
     q to the point, qdot = (1 - tau) Vdot_k + tau Vdot_{k+1} is q's velocity under params(t) moving at pdot at
     fixed z, and the solid velocity is its normal part (nh . qdot) nh; where the slab term of R28 is the active one
-    the surface is a cap moving at (0, 0, z0dot) or (0, 0, z1dot).  -> (us, vs, ws) arrays like X."""
+    the surface is a cap moving at (0, 0, z0dot) or (0, 0, z1dot).  -> (us, vs, ws, d) arrays like X, d the
+    primitive's signed distance max(d2, slab) there."""
     params = np.asarray(params, dtype=np.float64)
     pdot = np.asarray(pdot, dtype=np.float64)
     z0, z1 = params[0], params[1]
@@ -307,28 +308,36 @@ def _velocity_points(params, pdot, K, N, M, X, Y, z):
     us = np.where(use_slab, 0.0, us)
     vs = np.where(use_slab, 0.0, vs)
     ws = np.where(use_slab, zdot, ws)
-    return us, vs, ws
+    return us, vs, ws, np.maximum(sgn * dist, slab)
 
 
-def solid_velocity_faces(params, pdot, K, N, M, nx, ny, nz, dx):
+def solid_velocity_faces(params, pdot, K, N, M, nx, ny, nz, dx, band=np.inf, out=None):
     """U_s on the MAC faces (layout of nf_oracle: us (nz, ny, nx+1), vs (nz, ny+1, nx), ws (nz+1, ny, nx)): each
-    component sampled at its own face centres."""
-    us = np.zeros((nz, ny, nx + 1)); vs = np.zeros((nz, ny + 1, nx)); ws = np.zeros((nz + 1, ny, nx))
+    component sampled at its own face centres.  Only faces whose distance to the primitive is <= band are written
+    (R30: several moving parts are composed by one call each with a band of a few dx; the default writes all);
+    the others keep `out`'s values (zero if out is None)."""
+    if out is None:
+        us = np.zeros((nz, ny, nx + 1)); vs = np.zeros((nz, ny + 1, nx)); ws = np.zeros((nz + 1, ny, nx))
+    else:
+        us, vs, ws = (np.array(a, dtype=np.float64) for a in out)
     xi, xc = np.arange(nx + 1) * dx, (np.arange(nx) + 0.5) * dx
     yj, yc = np.arange(ny + 1) * dx, (np.arange(ny) + 0.5) * dx
     for k in range(nz):
         z = (k + 0.5) * dx
         X, Y = np.meshgrid(xi, yc, indexing="xy")
-        us[k] = _velocity_points(params, pdot, K, N, M, X, Y, z)[0]
+        r = _velocity_points(params, pdot, K, N, M, X, Y, z)
+        us[k] = np.where(r[3] <= band, r[0], us[k])
         X, Y = np.meshgrid(xc, yj, indexing="xy")
-        vs[k] = _velocity_points(params, pdot, K, N, M, X, Y, z)[1]
+        r = _velocity_points(params, pdot, K, N, M, X, Y, z)
+        vs[k] = np.where(r[3] <= band, r[1], vs[k])
     X, Y = np.meshgrid(xc, yc, indexing="xy")
     for k in range(nz + 1):
-        ws[k] = _velocity_points(params, pdot, K, N, M, X, Y, k * dx)[2]
+        r = _velocity_points(params, pdot, K, N, M, X, Y, k * dx)
+        ws[k] = np.where(r[3] <= band, r[2], ws[k])
     return us, vs, ws
 
 
-def solid_velocity_faces_adjoint(params, K, N, M, nx, ny, nz, dx, gus, gvs, gws):
+def solid_velocity_faces_adjoint(params, K, N, M, nx, ny, nz, dx, gus, gvs, gws, band=np.inf):
     """dJ/dpdot = J_v^T (gus, gvs, gws): U_s is linear in pdot, so the transpose is assembled column by column from
     solid_velocity_faces on the unit vectors (the definition of the transpose; R31: the dependence of U_s on
     params themselves -- through the closest point and the normal -- is not differentiated)."""
@@ -336,6 +345,6 @@ def solid_velocity_faces_adjoint(params, K, N, M, nx, ny, nz, dx, gus, gvs, gws)
     g = np.zeros(P)
     for a in range(P):
         e = np.zeros(P); e[a] = 1.0
-        us, vs, ws = solid_velocity_faces(params, e, K, N, M, nx, ny, nz, dx)
+        us, vs, ws = solid_velocity_faces(params, e, K, N, M, nx, ny, nz, dx, band)
         g[a] = np.sum(us * gus) + np.sum(vs * gvs) + np.sum(ws * gws)
     return g

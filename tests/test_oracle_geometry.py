@@ -229,7 +229,7 @@ def test_velocity_transports_the_distance_field():
     pd[0] = pd[1] = 0.0
     X, Y = rng.uniform(0.1, 0.9, 60), rng.uniform(0.1, 0.9, 60)
     z = 0.37
-    us, vs, _ = G._velocity_points(p, pd, K, N, M, X, Y, z)
+    us, vs, _, _ = G._velocity_points(p, pd, K, N, M, X, Y, z)
     h = 1e-6
 
     def phi(q, X, Y):
@@ -255,3 +255,9 @@ def test_velocity_is_linear_in_pdot_and_adjoint_is_its_transpose():
     gs = [rng.standard_normal(x.shape) for x in va]
     gp = G.solid_velocity_faces_adjoint(p, K, N, M, n, n, n, dx, *gs)
     assert np.isclose(sum(np.sum(x * g) for x, g in zip(va, gs)), gp @ a, rtol=1e-10)
+    # band: faces farther than the band from the primitive keep what they had
+    phi_u = G._velocity_points(p, a, K, N, M, *np.meshgrid(np.arange(n + 1) * dx, (np.arange(n) + 0.5) * dx), 2.5 * dx)[3]
+    keep = [np.full(x.shape, 7.0) for x in va]
+    vb = G.solid_velocity_faces(p, a, K, N, M, n, n, n, dx, band=0.1, out=keep)
+    assert np.array_equal(vb[0][2] == 7.0, phi_u > 0.1) and np.array_equal(vb[0][2][phi_u <= 0.1], va[0][2][phi_u <= 0.1])
+    assert 0 < np.count_nonzero(phi_u <= 0.1) < phi_u.size
