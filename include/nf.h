@@ -156,6 +156,55 @@ int nf_advect_adjoint(nf_grid *g, const float *u0, const float *v0, const float 
 int nf_weights_adjoint(nf_grid *g, const float *galpha_u, const float *galpha_v, const float *galpha_w,
                        float *gsdf_nodes);
 
+/* ---- NEXT-2  Differentiable parametric geometry (section 2.2; L337-347 appendix A) ----
+ * One primitive = one "closed 3-D surface": K key cross-sections, evenly spaced on [z0, z1] along the z axis, each a
+ * closed curve of N cubic Bezier curves in the polar frame of its centre (L339-343).  Parameter vector (HOST pointer,
+ * float32, physical units; node (i,j,k) sits at (i dx, j dx, k dx)):
+ *     params = [z0, z1,  then for key k = 0..K-1:  cx_k, cy_k, rho1_k[0..N-1], rho2_k[0..N-1]]     2 + K (2 + 2N) floats
+ * Curve i of a section spans the polar angles [theta_i, theta_{i+1}], theta_i = 2 pi i / N; its inner control points
+ * sit at radius rho1_i, angle theta_i + 2 pi/(3N), and radius rho2_i, angle theta_{i+1} - 2 pi/(3N) (L341); the shared
+ * endpoint on the ray theta_{i+1} is collinear with its two neighbours: radius 2 cos(2 pi/(3N)) rho2_i rho1_{i+1} /
+ * (rho2_i + rho1_{i+1}) (R25).  Between key sections centre and radii are interpolated piecewise linearly in
+ * s = clamp((z - z0)/(z1 - z0), 0, 1) (Eq. 10 is garbled: R27).  The curve is sampled at M points per Bezier curve and
+ * the distance is the exact signed distance d2 to that closed polygon of N M edges (R26).
+ * Limits: 1 <= K <= 64, 2 <= N <= 64, N M <= 2048, z1 > z0, all radii > 0 (NF_ERR_INVALID otherwise).
+ * params_host / pdot_host / g*_host are HOST arrays (copied before the call returns); every field is a DEVICE array. */
+enum { NF_GEOM_COMPLEMENT = 1 }; /* flags: the primitive is fluid INSIDE its surface (a chamber): phi = -d */
+enum { NF_CSG_UNION = 0, NF_CSG_INTERSECTION = 1 };
+
+/* phi at the nodes (layout of nf_set_solid's sdf_nodes; > 0 in the fluid): phi = d = max(d2(x, y; section(z)),
+ * z0 - z, z - z1), the cross-section intersected with the slab z0 <= z <= z1 (R28); -d with NF_GEOM_COMPLEMENT.
+ * Overwrites sdf_nodes.  Only enqueues work. */
+int nf_geom_sdf(nf_grid *g, const float *params_host, int K, int N, int M, int flags, float *sdf_nodes);
+
+/* gparams_host[a] = sum over nodes of gsdf_nodes * d phi / d params[a] ("back-propagating dJ/dS first
+ * through the SDF phi then through the distance computation"): the reverse of nf_geom_sdf, gsdf_nodes e.g. from
+ * nf_weights_adjoint.  2 + K (2 + 2N) doubles, overwritten.  Synchronises the stream. */
+int nf_geom_sdf_adjoint(nf_grid *g, const float *params_host, int K, int N, int M, int flags, const float *gsdf_nodes,
+                        double *gparams_host);
+
+/* CSG on solids ("Union and intersection"; phi > 0 = fluid, so the union of two solids is min(a, b), the
+ * intersection max(a, b): R29).  Node arrays; out may alias a or b.  The adjoint routes gout to the operand that
+ * supplied the value (ties: a) and writes 0 to the other; ga, gb may alias gout but not each other. */
+int nf_geom_csg(nf_grid *g, int op, const float *a, const float *b, float *out);
+int nf_geom_csg_adjoint(nf_grid *g, int op, const float *a, const float *b, const float *gout, float *ga, float *gb);
+
+/* Solid velocity of the moving geometry params(t), d params / dt = pdot ("SDF phi^{n+1} and velocity
+ * u_s^{n+1} can be derived from the solid geometry", L132): at every face centre of each family, the velocity of the
+ * closest point q of the section's polygon at that height -- q's edge and edge parameter held fixed -- along the
+ * in-plane unit normal nh: U_s = (nh . qdot) nh (x and y components; w = 0); where the slab term of R28 is the active
+ * one the surface is a cap moving at (0, 0, z0dot) or (0, 0, z1dot) (R30).  Only faces with d <= band (physical
+ * units; INFINITY = all) are written, the others keep their values: several moving parts = one call each.
+ * us / vs / ws: MAC face layout, any may be NULL (skipped).  Only enqueues work. */
+int nf_geom_velocity(nf_grid *g, const float *params_host, const float *pdot_host, int K, int N, int M, float band,
+                     float *us, float *vs, float *ws);
+
+/* gpdot_host = J^T (gus, gvs, gws), J = d U_s / d pdot of nf_geom_velocity with the same band (U_s is linear in
+ * pdot; its dependence on params through q and nh is not differentiated: R31).  gus / gvs / gws may be NULL (= 0),
+ * e.g. from nf_project_adjoint's gus_*.  2 + K (2 + 2N) doubles, overwritten.  Synchronises the stream. */
+int nf_geom_velocity_adjoint(nf_grid *g, const float *params_host, int K, int N, int M, float band, const float *gus,
+                             const float *gvs, const float *gws, double *gpdot_host);
+
 /* Apply A to a cell array (q = A p, homogeneous ghosts) -- exposed for tests and kernel benchmarks. */
 int nf_apply_A(nf_grid *g, const float *p, float *q);
 /* One V-cycle z = M^{-1} r (zero initial guess) -- exposed for tests and kernel benchmarks. */

@@ -14,6 +14,8 @@ NF_ERR_INVALID, NF_ERR_ALLOC, NF_ERR_CUDA, NF_ERR_STATE = -1, -2, -3, -4
 BC_CLOSED, BC_DIRICHLET = 0, 1
 
 _c_float_p = ctypes.c_void_p  # raw device (or host) addresses
+_c_host_float_p = ctypes.POINTER(ctypes.c_float)
+_c_host_double_p = ctypes.POINTER(ctypes.c_double)
 _SIGNATURES = {
     "nf_version": (ctypes.c_char_p, []),
     "nf_grid_create": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_float,
@@ -35,6 +37,15 @@ _SIGNATURES = {
     "nf_viscosity": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.c_float, ctypes.c_float]),
     "nf_advect_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 6 + [ctypes.c_float]),
     "nf_weights_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
+    "nf_geom_sdf": (ctypes.c_int, [ctypes.c_void_p, _c_host_float_p] + [ctypes.c_int] * 4 + [_c_float_p]),
+    "nf_geom_sdf_adjoint": (ctypes.c_int, [ctypes.c_void_p, _c_host_float_p] + [ctypes.c_int] * 4 +
+                            [_c_float_p, _c_host_double_p]),
+    "nf_geom_csg": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int] + [_c_float_p] * 3),
+    "nf_geom_csg_adjoint": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int] + [_c_float_p] * 5),
+    "nf_geom_velocity": (ctypes.c_int, [ctypes.c_void_p, _c_host_float_p, _c_host_float_p] + [ctypes.c_int] * 3 +
+                         [ctypes.c_float] + [_c_float_p] * 3),
+    "nf_geom_velocity_adjoint": (ctypes.c_int, [ctypes.c_void_p, _c_host_float_p] + [ctypes.c_int] * 3 +
+                                 [ctypes.c_float] + [_c_float_p] * 3 + [_c_host_double_p]),
     "nf_apply_A": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p]),
     "nf_vcycle": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p]),
     "nf_set_host_async": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
@@ -232,6 +243,68 @@ class Grid:
         """Explicit viscosity step, in place; symmetric, so the backward pass calls it on the gradient (Eq. 8)."""
         self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
         self._check(self.lib.nf_viscosity(self.h, _ptr(u), _ptr(v), _ptr(w), float(nu), float(dt)), "nf_viscosity")
+
+    # ---- NEXT-2: parametric geometry (host parameter vectors: any float sequence / NumPy array) ----
+    @staticmethod
+    def geom_n_params(K, N):
+        return 2 + K * (2 + 2 * N)
+
+    def _geom_vec(self, v, K, N, name):
+        import numpy as np
+        a = np.ascontiguousarray(np.asarray(v, dtype=np.float32))
+        if a.shape != (self.geom_n_params(K, N),):
+            raise ValueError("%s: expected %d values" % (name, self.geom_n_params(K, N)))
+        return a, a.ctypes.data_as(_c_host_float_p)
+
+    def geom_sdf(self, params, K, N, M, sdf, complement=False):
+        self._expect(sdf, self.shape_sdf, "sdf")
+        _keep, pp = self._geom_vec(params, K, N, "params")
+        self._check(self.lib.nf_geom_sdf(self.h, pp, int(K), int(N), int(M), 1 if complement else 0, _ptr(sdf)),
+                    "nf_geom_sdf")
+
+    def geom_sdf_adjoint(self, params, K, N, M, gsdf, complement=False):
+        """-> NumPy float64 vector dJ/dparams (synchronises)."""
+        import numpy as np
+        self._expect(gsdf, self.shape_sdf, "gsdf")
+        _keep, pp = self._geom_vec(params, K, N, "params")
+        out = np.zeros(self.geom_n_params(K, N), dtype=np.float64)
+        self._check(self.lib.nf_geom_sdf_adjoint(self.h, pp, int(K), int(N), int(M), 1 if complement else 0, _ptr(gsdf),
+                                                 out.ctypes.data_as(_c_host_double_p)), "nf_geom_sdf_adjoint")
+        return out
+
+    def geom_csg(self, op, a, b, out):
+        for t, n in ((a, "a"), (b, "b"), (out, "out")):
+            self._expect(t, self.shape_sdf, n)
+        self._check(self.lib.nf_geom_csg(self.h, {"union": 0, "intersection": 1}[op], _ptr(a), _ptr(b), _ptr(out)),
+                    "nf_geom_csg")
+
+    def geom_csg_adjoint(self, op, a, b, gout, ga, gb):
+        for t, n in ((a, "a"), (b, "b"), (gout, "gout"), (ga, "ga"), (gb, "gb")):
+            self._expect(t, self.shape_sdf, n)
+        self._check(self.lib.nf_geom_csg_adjoint(self.h, {"union": 0, "intersection": 1}[op], _ptr(a), _ptr(b),
+                                                 _ptr(gout), _ptr(ga), _ptr(gb)), "nf_geom_csg_adjoint")
+
+    def geom_velocity(self, params, pdot, K, N, M, us, vs, ws, band=float("inf")):
+        for t, s, n in ((us, self.shape_u, "us"), (vs, self.shape_v, "vs"), (ws, self.shape_w, "ws")):
+            if t is not None:
+                self._expect(t, s, n)
+        _k1, pp = self._geom_vec(params, K, N, "params")
+        _k2, pd = self._geom_vec(pdot, K, N, "pdot")
+        self._check(self.lib.nf_geom_velocity(self.h, pp, pd, int(K), int(N), int(M), float(band), _ptr(us), _ptr(vs),
+                                              _ptr(ws)), "nf_geom_velocity")
+
+    def geom_velocity_adjoint(self, params, K, N, M, gus, gvs, gws, band=float("inf")):
+        """-> NumPy float64 vector dJ/dpdot (synchronises)."""
+        import numpy as np
+        for t, s, n in ((gus, self.shape_u, "gus"), (gvs, self.shape_v, "gvs"), (gws, self.shape_w, "gws")):
+            if t is not None:
+                self._expect(t, s, n)
+        _keep, pp = self._geom_vec(params, K, N, "params")
+        out = np.zeros(self.geom_n_params(K, N), dtype=np.float64)
+        self._check(self.lib.nf_geom_velocity_adjoint(self.h, pp, int(K), int(N), int(M), float(band), _ptr(gus),
+                                                      _ptr(gvs), _ptr(gws), out.ctypes.data_as(_c_host_double_p)),
+                    "nf_geom_velocity_adjoint")
+        return out
 
     def advect_adjoint(self, u0, v0, w0, gu, gv, gw, dt):
         for t, s, n in ((u0, self.shape_u, "u0"), (v0, self.shape_v, "v0"), (w0, self.shape_w, "w0"),

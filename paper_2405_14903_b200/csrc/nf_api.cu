@@ -9,11 +9,6 @@
     if (!(g)) return NF_ERR_INVALID; \
     (g)->err.clear();      \
   } while (0)
-#define NF_TRY(expr)            \
-  do {                          \
-    int rc_ = (expr);           \
-    if (rc_ < 0) return rc_;    \
-  } while (0)
 
 extern "C" const char *nf_version(void) { return "nf-b200 0.1 (sm_100a)"; }
 
@@ -30,7 +25,7 @@ static void free_all(nf_grid *g) {
   cudaFree(g->us); cudaFree(g->vs); cudaFree(g->ws); cudaFree(g->sdf);
   cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->b0); cudaFree(g->ecorr); cudaFree(g->r_alt); cudaFree(g->tailpack);
   cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
-  cudaFree(g->st); cudaFree(g->d_counts);
+  cudaFree(g->st); cudaFree(g->d_counts); cudaFree(g->geom_par); cudaFree(g->geom_grad);
   if (g->hst) cudaFreeHost((void *)g->hst);
   if (g->h_counts) cudaFreeHost(g->h_counts);
   if (g->ev0) cudaEventDestroy(g->ev0);
@@ -113,6 +108,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   ok = ok && dalloc(&g->fu, nf_nu(g)) == cudaSuccess && dalloc(&g->fv, nf_nv(g)) == cudaSuccess &&
        dalloc(&g->fw, nf_nw(g)) == cudaSuccess;
   ok = ok && dalloc(&g->st, 1) == cudaSuccess && dalloc(&g->d_counts, 2) == cudaSuccess;
+  ok = ok && dalloc(&g->geom_par, 2 * (size_t)NF_GEOM_MAXP) == cudaSuccess && dalloc(&g->geom_grad, (size_t)NF_GEOM_MAXP) == cudaSuccess;
   ok = ok && cudaHostAlloc((void **)&g->hst, NF_RING * sizeof(NfHostStatus), cudaHostAllocMapped) == cudaSuccess;
   ok = ok && cudaHostGetDevicePointer((void **)&g->hst_dev, (void *)g->hst, 0) == cudaSuccess;
   ok = ok && cudaHostAlloc((void **)&g->h_counts, 2 * sizeof(double), cudaHostAllocDefault) == cudaSuccess;
@@ -257,6 +253,47 @@ extern "C" int nf_max_speed(nf_grid *g, const float *u, const float *v, const fl
   NF_CHECK_HANDLE(g);
   if (!u || !v || !w || !max_abs_host) return NF_ERR_INVALID;
   return nf_max_speed_impl(g, u, v, w, max_abs_host);
+}
+
+// ---- NEXT-2: parametric geometry (nf_geom.cu) ---------------------------------------------------------------------
+extern "C" int nf_geom_sdf(nf_grid *g, const float *params_host, int K, int N, int M, int flags, float *sdf_nodes) {
+  NF_CHECK_HANDLE(g);
+  if (!sdf_nodes || (flags & ~NF_GEOM_COMPLEMENT)) return NF_ERR_INVALID;
+  return nf_geom_sdf_impl(g, params_host, K, N, M, flags, sdf_nodes);
+}
+
+extern "C" int nf_geom_sdf_adjoint(nf_grid *g, const float *params_host, int K, int N, int M, int flags,
+                                   const float *gsdf_nodes, double *gparams_host) {
+  NF_CHECK_HANDLE(g);
+  if (!gsdf_nodes || !gparams_host || (flags & ~NF_GEOM_COMPLEMENT)) return NF_ERR_INVALID;
+  return nf_geom_sdf_adjoint_impl(g, params_host, K, N, M, flags, gsdf_nodes, gparams_host);
+}
+
+extern "C" int nf_geom_velocity(nf_grid *g, const float *params_host, const float *pdot_host, int K, int N, int M,
+                                float band, float *us, float *vs, float *ws) {
+  NF_CHECK_HANDLE(g);
+  if (!pdot_host || band != band) return NF_ERR_INVALID;
+  return nf_geom_velocity_impl(g, params_host, pdot_host, K, N, M, band, us, vs, ws);
+}
+
+extern "C" int nf_geom_velocity_adjoint(nf_grid *g, const float *params_host, int K, int N, int M, float band,
+                                        const float *gus, const float *gvs, const float *gws, double *gpdot_host) {
+  NF_CHECK_HANDLE(g);
+  if (!gpdot_host || band != band) return NF_ERR_INVALID;
+  return nf_geom_velocity_adjoint_impl(g, params_host, K, N, M, band, gus, gvs, gws, gpdot_host);
+}
+
+extern "C" int nf_geom_csg(nf_grid *g, int op, const float *a, const float *b, float *out) {
+  NF_CHECK_HANDLE(g);
+  if (!a || !b || !out || (op != NF_CSG_UNION && op != NF_CSG_INTERSECTION)) return NF_ERR_INVALID;
+  return nf_geom_csg_impl(g, op, a, b, out);
+}
+
+extern "C" int nf_geom_csg_adjoint(nf_grid *g, int op, const float *a, const float *b, const float *gout, float *ga,
+                                   float *gb) {
+  NF_CHECK_HANDLE(g);
+  if (!a || !b || !gout || !ga || !gb || ga == gb || (op != NF_CSG_UNION && op != NF_CSG_INTERSECTION)) return NF_ERR_INVALID;
+  return nf_geom_csg_adjoint_impl(g, op, a, b, gout, ga, gb);
 }
 
 extern "C" int nf_advect(nf_grid *g, float *u, float *v, float *w, float dt) {
@@ -415,7 +452,7 @@ static const char *kClassNames[NFK_COUNT] = {
     "apply_A", "cg_update", "cg_check", "cg_pupdate", "down1_fine", "down2_fine", "up1_fine", "up2_fine", "vec_coarse",
     "rbgs_fine", "rbgs_coarse", "restrict_fine", "restrict_coarse", "prolong_fine", "prolong_coarse", "tail",
     "solve_setup", "rhs", "grad_subtract", "adjoint_rhs", "adjoint_finish", "weights", "coarsen", "encode", "store_us",
-    "advect", "advect_adjoint", "weights_adjoint", "misc"};
+    "advect", "advect_adjoint", "weights_adjoint", "geometry", "misc"};
 
 void nf_prof_begin(nf_grid *g, int cls) {
   const size_t r = g->prof_cls.size();

@@ -80,12 +80,18 @@ struct NfHostStatus {  // written by the device into mapped pinned memory
   volatile float relres;
 };
 
+// limits of the parametric geometry (nf_geom.cu): K key sections, N curves per section, N*M polygon edges
+#define NF_GEOM_MAXK 64
+#define NF_GEOM_MAXN 64
+#define NF_GEOM_MAXNM 2048
+#define NF_GEOM_MAXP (2 + NF_GEOM_MAXK * (2 + 2 * NF_GEOM_MAXN))
+
 // Kernel classes for the per-class device timing of nf_profile_* (bench.py's roofline leg).
 enum {
   NFK_APPLY = 0, NFK_UPDATE, NFK_CHECK, NFK_PUPDATE, NFK_DOWN1_0, NFK_DOWN2_0, NFK_UP1_0, NFK_UP2_0, NFK_VEC_C,
   NFK_RBGS0, NFK_RBGS_C, NFK_RESTRICT0, NFK_RESTRICT_C, NFK_PROLONG0, NFK_PROLONG_C, NFK_BOTTOM, NFK_SETUP, NFK_RHS,
   NFK_GRADSUB, NFK_ADJ_RHS, NFK_ADJ_FINISH, NFK_WEIGHTS, NFK_COARSEN, NFK_CLASSIFY, NFK_STORE_US, NFK_ADVECT,
-  NFK_ADVECT_ADJ, NFK_WEIGHTS_ADJ, NFK_MISC, NFK_COUNT
+  NFK_ADVECT_ADJ, NFK_WEIGHTS_ADJ, NFK_GEOM, NFK_MISC, NFK_COUNT
 };
 
 struct nf_grid {
@@ -118,6 +124,9 @@ struct nf_grid {
   NfSolveState *st;      // device
   NfHostStatus *hst;     // mapped pinned host ring
   NfHostStatus *hst_dev; // device alias of hst
+  // parametric geometry (nf_geom.cu): device copies of params / pdot (2 x NF_GEOM_MAXP floats), the parameter gradient
+  float *geom_par;
+  double *geom_grad;
   double *d_counts;      // device: [0] active cells, [1] open faces on Dirichlet domain faces
   double *h_counts;      // pinned host copy
   cudaEvent_t ev0, ev1;
@@ -159,6 +168,12 @@ void nf_prof_end(nf_grid *g);
       (g)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                \
       return NF_ERR_CUDA;                                                           \
     }                                                                               \
+  } while (0)
+
+#define NF_TRY(expr)            \
+  do {                          \
+    int rc_ = (expr);           \
+    if (rc_ < 0) return rc_;    \
   } while (0)
 
 static inline size_t nf_nu(const nf_grid *g) { return (size_t)g->nz * g->ny * (g->nx + 1); }
@@ -237,6 +252,16 @@ int nf_viscosity_impl(nf_grid *g, float *u, float *v, float *w, float nu, float 
 int nf_max_speed_impl(nf_grid *g, const float *u, const float *v, const float *w, float *out_host);
 int nf_advect_adjoint_impl(nf_grid *g, const float *u0, const float *v0, const float *w0, float *gu, float *gv,
                            float *gw, float dt);
+// nf_geom.cu
+int nf_geom_sdf_impl(nf_grid *g, const float *params, int K, int N, int M, int flags, float *sdf_nodes);
+int nf_geom_sdf_adjoint_impl(nf_grid *g, const float *params, int K, int N, int M, int flags, const float *gsdf_nodes,
+                             double *gparams_host);
+int nf_geom_velocity_impl(nf_grid *g, const float *params, const float *pdot, int K, int N, int M, float band,
+                          float *us, float *vs, float *ws);
+int nf_geom_velocity_adjoint_impl(nf_grid *g, const float *params, int K, int N, int M, float band, const float *gus,
+                                  const float *gvs, const float *gws, double *gpdot_host);
+int nf_geom_csg_impl(nf_grid *g, int op, const float *a, const float *b, float *out);
+int nf_geom_csg_adjoint_impl(nf_grid *g, int op, const float *a, const float *b, const float *gout, float *ga, float *gb);
 
 // Programmatic dependent launch (PDL): the kernels of one PCG iteration are launched with the programmatic stream
 // serialisation attribute and start with nf_pdl_enter() -- "my dependents may be scheduled" + "wait until the grids

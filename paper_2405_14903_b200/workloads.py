@@ -280,3 +280,28 @@ def keep_largest_component(au, av, aw):
     av = np.where(lab[1::2, 0::2, 1::2] == best, av, 0).astype(av.dtype)
     aw = np.where(lab[0::2, 1::2, 1::2] == best, aw, 0).astype(aw.dtype)
     return au, av, aw, ncomp
+
+
+# ------------------------------------------------------------------------------------------------------
+# NEXT-2: seeded parameter vectors of a polar-Bezier primitive (layout of include/nf.h: [z0, z1, K x (cx, cy,
+# rho1[N], rho2[N])]).  Only draws numbers and fills the layout -- none of the geometry's arithmetic lives here.
+# ------------------------------------------------------------------------------------------------------
+def geom_n_params(K, N):
+    return 2 + K * (2 + 2 * N)
+
+
+def geom_random_params(seed, K, N, z0, z1, centre, radius, jitter=0.25, centre_jitter=0.03):
+    """Radii radius * (1 +- jitter) on every control point, centres scattered by centre_jitter * radius."""
+    rng = np.random.default_rng(seed)
+    p = np.zeros(geom_n_params(K, N), dtype=np.float64)
+    p[0], p[1] = z0, z1
+    keys = p[2:].reshape(K, 2 + 2 * N)
+    keys[:, 0] = centre[0] + centre_jitter * radius * rng.standard_normal(K)
+    keys[:, 1] = centre[1] + centre_jitter * radius * rng.standard_normal(K)
+    keys[:, 2:] = radius * (1.0 + jitter * rng.uniform(-1.0, 1.0, (K, 2 * N)))
+    return p.astype(np.float32)
+
+
+def geom_random_rates(seed, K, N, scale=1.0):
+    rng = np.random.default_rng(seed)
+    return (scale * rng.standard_normal(geom_n_params(K, N))).astype(np.float32)
