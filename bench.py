@@ -462,6 +462,83 @@ def run_sweep(args):
                       "tol": TOL, "dtype": "f32", "rows": rows}))
 
 
+def run_geometry(args):
+    """SURVEY.md 8f NEXT-2 at the headline grid size: a solid made of four polar-Bezier primitives (K = 4 key sections,
+    N = 8 curves, M = 16 samples per curve: 128 polygon edges each; "union of four sub-geometries"),
+    phi = union on the nodes, its reverse with dJ/dphi confined to the nodes next to the surface (what
+    nf_weights_adjoint produces), and the solid velocity of one moving primitive with a band of 3 dx + its reverse.
+    roofline: ALU-bound; one (node, edge) pair costs 19.25 SASS instructions in k_geom_sdf's scan loop (77 per 4 points,
+    cuobjdump), so peak = 148 SMs x 128 lanes x SM clock / 19.25 pairs/s."""
+    import numpy as np
+    import torch
+    from paper_2405_14903_b200 import api, workloads as wl
+    api.load_library()
+    torch.cuda.set_device(0)
+    n, K, N, M = args.n, 4, 8, 16
+    g = api.Grid(n, n, n, 1.0 / n)
+    prims = [wl.geom_random_params(40 + i, K, N, 0.15 + 0.05 * i, 0.6 + 0.08 * i,
+                                   (0.35 + 0.3 * (i % 2), 0.35 + 0.3 * (i // 2)), 0.17) for i in range(4)]
+    phis = [torch.empty(g.shape_sdf, dtype=torch.float32, device="cuda") for _ in prims]
+    acc = [torch.empty_like(phis[0]) for _ in range(3)]
+    gacc = [torch.empty_like(phis[0]) for _ in range(8)]
+
+    def forward():
+        for p, f in zip(prims, phis):
+            g.geom_sdf(p, K, N, M, f)
+        g.geom_csg("union", phis[0], phis[1], acc[0])
+        g.geom_csg("union", acc[0], phis[2], acc[1])
+        g.geom_csg("union", acc[1], phis[3], acc[2])
+
+    forward()
+    gphi = torch.where(acc[2].abs() < 2.0 / n, torch.randn_like(acc[2]), torch.zeros_like(acc[2]))
+
+    def backward():
+        g.geom_csg_adjoint("union", acc[1], phis[3], gphi, gacc[0], gacc[1])
+        g.geom_csg_adjoint("union", acc[0], phis[2], gacc[0], gacc[2], gacc[3])
+        g.geom_csg_adjoint("union", phis[0], phis[1], gacc[2], gacc[4], gacc[5])
+        return [g.geom_sdf_adjoint(p, K, N, M, gg) for p, gg in zip(prims, (gacc[4], gacc[5], gacc[3], gacc[1]))]
+
+    pd = wl.geom_random_rates(3, K, N, 0.1)
+    U = [torch.zeros(s, dtype=torch.float32, device="cuda") for s in (g.shape_u, g.shape_v, g.shape_w)]
+    gU = [torch.randn_like(a) for a in U]
+    legs = {"sdf_union_of_4": forward, "sdf_adjoint_4": backward,
+            "velocity_1": lambda: g.geom_velocity(prims[0], pd, K, N, M, *U, band=3.0 / n),
+            "velocity_adjoint_1": lambda: g.geom_velocity_adjoint(prims[0], K, N, M, *gU, band=3.0 / n)}
+    clocks = ClockSampler(0)
+    clocks.start()
+    out = {}
+    for name, fn in legs.items():
+        for _ in range(max(args.warmup, 3)):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        out[name] = round(e0.elapsed_time(e1) / args.steps, 4)
+    ck = clocks.stop()
+    # the dominant kernel alone
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        g.geom_sdf(prims[0], K, N, M, phis[0])
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    pairs = float((n + 1) ** 3) * N * M
+    mhz = ck.get("sm_mhz") or 1900.0
+    peak = 148 * 128 * mhz * 1e6 / 19.25
+    print(json.dumps({"workload": "NEXT-2 parametric geometry, %d^3 grid, 4 primitives x (K=4, N=8, M=16)" % n,
+                      "dtype": "f32", "ms": out, "clocks": ck,
+                      "roofline": {"kernel": "k_geom_sdf", "bound": "alu", "achieved": round(pairs / (ms * 1e-3) / 1e9, 1),
+                                   "peak": round(peak / 1e9, 1), "unit": "G(node,edge)/s",
+                                   "frac": round(pairs / (ms * 1e-3) / peak, 3), "ms_per_launch": round(ms, 4),
+                                   "traffic": None}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -475,9 +552,14 @@ def main():
                     help="nf_project starts from the previous step's pressure (default: x0 = 0, as BASELINE's metric)")
     ap.add_argument("--sweep", default="", help="comma-separated cubic sizes: run the configs[4] pressure-solve sweep "
                                                  "instead of the headline step, e.g. --sweep 64,128,256,384")
+    ap.add_argument("--geometry", action="store_true",
+                    help="time the NEXT-2 parametric-geometry kernels at --n instead of the headline step")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+        return
+    if args.geometry:
+        run_geometry(args)
         return
     if args.impl == "reference":
         run_reference(args)

@@ -3,8 +3,8 @@
 // adjoint to the parameters (L141), CSG (L67) and the solid velocity of a moving geometry (L89, L132).
 // Readings R25-R31.
 //
-// One CTA = one 64 x 16 tile of points of ONE z-plane.  Every point of a plane sees the same cross-section, so the CTA
-// first builds it in shared memory -- the interpolated section, the N M vertices of the sampled Bezier curves (fp64,
+// One CTA = 1024 consecutive points (x fastest) of ONE z-plane.  Every point of a plane sees the same cross-section, so
+// the CTA first builds it in shared memory -- the interpolated section, the N M vertices of the sampled Bezier curves (fp64,
 // N M <= 2048 values: noise), one 6-float record per polygon edge -- and then every thread scans the N M edges for
 // 4 points (distance, closest edge, parity of the +x ray).  ALU-bound: ~20 fp32 instructions per (point, edge).
 // The reverse kernels redo the scan, scatter into per-CTA vertex gradients (shared-memory atomics; only cut-cell
@@ -12,9 +12,9 @@
 // ending in a handful of fp64 atomics on the parameter gradient.
 #include "nf_internal.cuh"
 
-#define NF_GEOM_TX 64
-#define NF_GEOM_TY 4
-#define NF_GEOM_PPT 4  // points per thread: rows ty, ty + 4, ty + 8, ty + 12 of the tile
+#define NF_GEOM_NT 256  // threads per CTA
+#define NF_GEOM_PPT 4   // points per thread: plane offsets base + tid + 256 q (no tile edges: a plane of 257 x 257 nodes
+                        // wastes 0.8 % of the lanes, a 64 x 16 tiling 20 %)
 
 struct NfGeomK {
   const float *par;   // device: [z0, z1, K x (cx, cy, rho1[N], rho2[N])]
@@ -34,6 +34,7 @@ struct NfGeomPlane {
 // shared-memory carve-up (nf_geom_smem_bytes must agree)
 struct NfGeomSm {
   double *sec, *secd, *gsec;  // W = 2 + 2N each: section, its time derivative, its gradient
+  double *cur;                // 16 per curve: cos[4], sin[4] of the control directions, radii[4], their rates[4]
   float *seg;                 // 6 per edge: ax, ay, ex, ey, 1/|e|^2, ex/ey
   float *V, *Vd, *gV;         // 2 per vertex: position, velocity, gradient
   float *ctrl;                // 8 per curve: gradient w.r.t. e0, p0, p1, e1
@@ -41,7 +42,7 @@ struct NfGeomSm {
 };
 static size_t nf_geom_smem_bytes(int N, int M) {
   const size_t W = 2 + 2 * (size_t)N, NM = (size_t)N * M;
-  return 3 * W * sizeof(double) + (6 * NM + 3 * 2 * NM + 8 * (size_t)N + 4) * sizeof(float);
+  return (3 * W + 16 * (size_t)N) * sizeof(double) + (6 * NM + 3 * 2 * NM + 8 * (size_t)N + 4) * sizeof(float);
 }
 __device__ __forceinline__ NfGeomSm nf_geom_carve(unsigned char *raw, int N, int M) {
   const int W = 2 + 2 * N, NM = N * M;
@@ -49,7 +50,8 @@ __device__ __forceinline__ NfGeomSm nf_geom_carve(unsigned char *raw, int N, int
   s.sec = reinterpret_cast<double *>(raw);
   s.secd = s.sec + W;
   s.gsec = s.secd + W;
-  s.seg = reinterpret_cast<float *>(s.gsec + W);
+  s.cur = s.gsec + W;
+  s.seg = reinterpret_cast<float *>(s.cur + 16 * N);
   s.V = s.seg + 6 * NM;
   s.Vd = s.V + 2 * NM;
   s.gV = s.Vd + 2 * NM;
@@ -101,7 +103,7 @@ __device__ __forceinline__ void nf_curve_dirs(int i, int N, double cs[4], double
 
 // Builds the plane's cross-section in shared memory.  All threads of the CTA call it.
 __device__ void nf_geom_setup(const NfGeomK &G, const NfGeomPlane &P, const NfGeomSm &S, bool zero_grad) {
-  const int tid = threadIdx.y * blockDim.x + threadIdx.x, nth = blockDim.x * blockDim.y;
+  const int tid = threadIdx.x, nth = blockDim.x;
   const int N = G.N, M = G.M, W = 2 + 2 * N, NM = N * M;
   const float *k0 = G.par + 2 + (size_t)P.k0 * W, *k1 = G.par + 2 + (size_t)P.k1 * W;
   double sdot = 0.0;
@@ -120,39 +122,48 @@ __device__ void nf_geom_setup(const NfGeomK &G, const NfGeomPlane &P, const NfGe
   }
   if (tid < 3) S.gsl[tid] = 0.0f;
   __syncthreads();
-  const double cdl = cospi(2.0 / (3.0 * (double)N));
-  const double *r1 = S.sec + 2, *r2 = S.sec + 2 + N, *r1d = S.secd + 2, *r2d = S.secd + 2 + N;
+  // per curve: the four control directions, the four radii (R25: endpoint radius 2 cos(delta) a b / (a + b), a = rho2 of
+  // the curve before the endpoint, b = rho1 of the curve after it) and their rates
+  {
+    const double cdl = cospi(2.0 / (3.0 * (double)N));
+    const double *r1 = S.sec + 2, *r2 = S.sec + 2 + N, *r1d = S.secd + 2, *r2d = S.secd + 2 + N;
+    for (int i = tid; i < N; i += nth) {
+      const int im = (i + N - 1) % N, ip = (i + 1) % N;
+      double *c = S.cur + 16 * i;
+      nf_curve_dirs(i, N, c, c + 4);
+      const double a0 = r2[im], b0 = r1[i], a1 = r2[i], b1 = r1[ip];
+      c[8] = 2.0 * cdl * a0 * b0 / (a0 + b0);
+      c[9] = r1[i];
+      c[10] = r2[i];
+      c[11] = 2.0 * cdl * a1 * b1 / (a1 + b1);
+      if (G.pdot) {
+        c[12] = 2.0 * cdl * (b0 * b0 * r2d[im] + a0 * a0 * r1d[i]) / ((a0 + b0) * (a0 + b0));
+        c[13] = r1d[i];
+        c[14] = r2d[i];
+        c[15] = 2.0 * cdl * (b1 * b1 * r2d[i] + a1 * a1 * r1d[ip]) / ((a1 + b1) * (a1 + b1));
+      }
+    }
+  }
+  __syncthreads();
   for (int v = tid; v < NM; v += nth) {
     const int i = v / M, m = v - i * M;
-    const int im = (i + N - 1) % N, ip = (i + 1) % N;
-    double cs[4], sn[4], B[4], rad[4];
-    nf_curve_dirs(i, N, cs, sn);
+    const double *c = S.cur + 16 * i;
+    double B[4];
     nf_bernstein3((double)m / (double)M, B);
-    // R25: endpoint radius 2 cos(delta) a b / (a + b), a = rho2 of the curve before, b = rho1 of the curve after
-    const double a0 = r2[im], b0 = r1[i], a1 = r2[i], b1 = r1[ip];
-    rad[0] = 2.0 * cdl * a0 * b0 / (a0 + b0);
-    rad[1] = r1[i];
-    rad[2] = r2[i];
-    rad[3] = 2.0 * cdl * a1 * b1 / (a1 + b1);
     double x = S.sec[0], y = S.sec[1];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      x += B[c] * rad[c] * cs[c];
-      y += B[c] * rad[c] * sn[c];
+    for (int b = 0; b < 4; ++b) {
+      x += B[b] * c[8 + b] * c[b];
+      y += B[b] * c[8 + b] * c[4 + b];
     }
     S.V[2 * v] = (float)x;
     S.V[2 * v + 1] = (float)y;
     if (G.pdot) {
-      double rd[4];
-      rd[0] = 2.0 * cdl * (b0 * b0 * r2d[im] + a0 * a0 * r1d[i]) / ((a0 + b0) * (a0 + b0));
-      rd[1] = r1d[i];
-      rd[2] = r2d[i];
-      rd[3] = 2.0 * cdl * (b1 * b1 * r2d[i] + a1 * a1 * r1d[ip]) / ((a1 + b1) * (a1 + b1));
       double xd = S.secd[0], yd = S.secd[1];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        xd += B[c] * rd[c] * cs[c];
-        yd += B[c] * rd[c] * sn[c];
+      for (int b = 0; b < 4; ++b) {
+        xd += B[b] * c[12 + b] * c[b];
+        yd += B[b] * c[12 + b] * c[4 + b];
       }
       S.Vd[2 * v] = (float)xd;
       S.Vd[2 * v + 1] = (float)yd;
@@ -173,10 +184,11 @@ __device__ void nf_geom_setup(const NfGeomK &G, const NfGeomPlane &P, const NfGe
   __syncthreads();
 }
 
-// R26: exact distance of NF_GEOM_PPT points (same X, different Y) to the closed polygon, the closest edge and the
-// parameter on it, and the even-odd parity of the ray towards +x.
+// R26: exact distance of NF_GEOM_PPT points to the closed polygon, the closest edge and the parameter on it, and the
+// even-odd parity of the ray towards +x.
 template <bool TRACK>
-__device__ __forceinline__ void nf_geom_scan(const float *__restrict__ seg, int NM, float X, const float (&Y)[NF_GEOM_PPT],
+__device__ __forceinline__ void nf_geom_scan(const float *__restrict__ seg, int NM, const float (&X)[NF_GEOM_PPT],
+                                             const float (&Y)[NF_GEOM_PPT],
                                              float (&d2)[NF_GEOM_PPT], int (&kb)[NF_GEOM_PPT],
                                              float (&tb)[NF_GEOM_PPT], unsigned &inside) {
 #pragma unroll
@@ -186,10 +198,10 @@ __device__ __forceinline__ void nf_geom_scan(const float *__restrict__ seg, int 
     const float2 a = *reinterpret_cast<const float2 *>(seg + 6 * k);
     const float2 e = *reinterpret_cast<const float2 *>(seg + 6 * k + 2);
     const float2 c = *reinterpret_cast<const float2 *>(seg + 6 * k + 4);
-    const float dxp = X - a.x, by = a.y + e.y;
+    const float by = a.y + e.y;
 #pragma unroll
     for (int q = 0; q < NF_GEOM_PPT; ++q) {
-      const float dyp = Y[q] - a.y;
+      const float dxp = X[q] - a.x, dyp = Y[q] - a.y;
       const float tau = __saturatef((dxp * e.x + dyp * e.y) * c.x);
       const float rx = dxp - tau * e.x, ry = dyp - tau * e.y;
       const float d = rx * rx + ry * ry;
@@ -207,7 +219,7 @@ __device__ __forceinline__ void nf_geom_scan(const float *__restrict__ seg, int 
 __device__ void nf_geom_chain(const NfGeomK &G, const NfGeomPlane &P, const NfGeomSm &S, double *gout) {
   __syncthreads();
   if (S.gsl[2] == 0.0f) return;  // (uniform: read after the barrier)
-  const int tid = threadIdx.y * blockDim.x + threadIdx.x, nth = blockDim.x * blockDim.y;
+  const int tid = threadIdx.x, nth = blockDim.x;
   const int N = G.N, M = G.M, W = 2 + 2 * N;
   for (int i = tid; i < N; i += nth) {
     double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -226,8 +238,7 @@ __device__ void nf_geom_chain(const NfGeomK &G, const NfGeomPlane &P, const NfGe
   const double *r1 = S.sec + 2, *r2 = S.sec + 2 + N;
   for (int i = tid; i < N; i += nth) {
     const int im = (i + N - 1) % N, ip = (i + 1) % N;
-    double cs[4], sn[4];
-    nf_curve_dirs(i, N, cs, sn);
+    const double *cs = S.cur + 16 * i, *sn = cs + 4;
     const float *ci = S.ctrl + 8 * i, *cm = S.ctrl + 8 * im, *cp = S.ctrl + 8 * ip;
     // endpoint at theta_i (e1 of the curve before = e0 of this one) and at theta_{i+1}
     const double ge0 = ((double)cm[6] + ci[0]) * cs[0] + ((double)cm[7] + ci[1]) * sn[0];
@@ -266,59 +277,67 @@ __device__ void nf_geom_chain(const NfGeomK &G, const NfGeomPlane &P, const NfGe
 // ------------------------------------------------------------------------------------------------------------
 // phi on the nodes (R28): d = max(d2(x, y; section(z)), z0 - z, z - z1), phi = sign * d
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NF_GEOM_TX *NF_GEOM_TY) k_geom_sdf(NfGeomK G, int nxn, int nyn, float sign,
-                                                                     float *__restrict__ out) {
+// Points of a plane, x fastest: thread t of CTA b owns the offsets 1024 b + t + 256 q.
+struct NfGeomPts {
+  int i[NF_GEOM_PPT], j[NF_GEOM_PPT];
+  bool ok[NF_GEOM_PPT];
+};
+__device__ __forceinline__ NfGeomPts nf_geom_points(int npx, int npy) {
+  NfGeomPts p;
+#pragma unroll
+  for (int q = 0; q < NF_GEOM_PPT; ++q) {
+    const int id = (blockIdx.x * NF_GEOM_PPT + q) * NF_GEOM_NT + threadIdx.x;
+    p.j[q] = id / npx;
+    p.i[q] = id - p.j[q] * npx;
+    p.ok[q] = id < npx * npy;
+  }
+  return p;
+}
+
+__global__ void __launch_bounds__(NF_GEOM_NT) k_geom_sdf(NfGeomK G, int nxn, int nyn, float sign, float *__restrict__ out) {
   extern __shared__ __align__(16) unsigned char nf_geom_raw[];
   const NfGeomSm S = nf_geom_carve(nf_geom_raw, G.N, G.M);
   const NfGeomPlane P = nf_geom_plane(G, (double)blockIdx.z * (double)G.dx);
   nf_geom_setup(G, P, S, false);
-  const int i = blockIdx.x * NF_GEOM_TX + threadIdx.x;
-  const int j0 = blockIdx.y * (NF_GEOM_TY * NF_GEOM_PPT) + threadIdx.y;
-  if (i >= nxn) return;
-  const float X = (float)i * G.dx;
-  float Y[NF_GEOM_PPT], d2[NF_GEOM_PPT], tb[NF_GEOM_PPT];
+  const NfGeomPts pt = nf_geom_points(nxn, nyn);
+  float X[NF_GEOM_PPT], Y[NF_GEOM_PPT], d2[NF_GEOM_PPT], tb[NF_GEOM_PPT];
   int kb[NF_GEOM_PPT];
   unsigned inside;
 #pragma unroll
-  for (int q = 0; q < NF_GEOM_PPT; ++q) Y[q] = (float)(j0 + NF_GEOM_TY * q) * G.dx;
+  for (int q = 0; q < NF_GEOM_PPT; ++q) { X[q] = (float)pt.i[q] * G.dx; Y[q] = (float)pt.j[q] * G.dx; }
   nf_geom_scan<false>(S.seg, G.N * G.M, X, Y, d2, kb, tb, inside);
 #pragma unroll
   for (int q = 0; q < NF_GEOM_PPT; ++q) {
-    const int j = j0 + NF_GEOM_TY * q;
-    if (j < nyn) {
+    if (pt.ok[q]) {
       const float sd = ((inside >> q) & 1u) ? -sqrtf(d2[q]) : sqrtf(d2[q]);
-      out[((size_t)blockIdx.z * nyn + j) * nxn + i] = sign * fmaxf(sd, P.slab);
+      out[((size_t)blockIdx.z * nyn + pt.j[q]) * nxn + pt.i[q]] = sign * fmaxf(sd, P.slab);
     }
   }
 }
 
 // dJ/dphi -> dJ/dparams (L141)
-__global__ void __launch_bounds__(NF_GEOM_TX *NF_GEOM_TY) k_geom_sdf_adjoint(NfGeomK G, int nxn, int nyn, float sign,
-                                                                             const float *__restrict__ gphi,
-                                                                             double *__restrict__ gout) {
+__global__ void __launch_bounds__(NF_GEOM_NT) k_geom_sdf_adjoint(NfGeomK G, int nxn, int nyn, float sign,
+                                                                 const float *__restrict__ gphi, double *__restrict__ gout) {
   extern __shared__ __align__(16) unsigned char nf_geom_raw[];
   const NfGeomSm S = nf_geom_carve(nf_geom_raw, G.N, G.M);
   const NfGeomPlane P = nf_geom_plane(G, (double)blockIdx.z * (double)G.dx);
   nf_geom_setup(G, P, S, true);
   const int NM = G.N * G.M;
-  const int i = blockIdx.x * NF_GEOM_TX + threadIdx.x;
-  const int j0 = blockIdx.y * (NF_GEOM_TY * NF_GEOM_PPT) + threadIdx.y;
+  const NfGeomPts pt = nf_geom_points(nxn, nyn);
   float g[NF_GEOM_PPT];
   bool work = false;
 #pragma unroll
   for (int q = 0; q < NF_GEOM_PPT; ++q) {
-    const int j = j0 + NF_GEOM_TY * q;
-    g[q] = (i < nxn && j < nyn) ? sign * gphi[((size_t)blockIdx.z * nyn + j) * nxn + i] : 0.0f;
+    g[q] = pt.ok[q] ? sign * gphi[((size_t)blockIdx.z * nyn + pt.j[q]) * nxn + pt.i[q]] : 0.0f;
     work = work || g[q] != 0.0f;
   }
   if (work) {
     S.gsl[2] = 1.0f;
-    const float X = (float)i * G.dx;
-    float Y[NF_GEOM_PPT], d2[NF_GEOM_PPT], tb[NF_GEOM_PPT];
+    float X[NF_GEOM_PPT], Y[NF_GEOM_PPT], d2[NF_GEOM_PPT], tb[NF_GEOM_PPT];
     int kb[NF_GEOM_PPT];
     unsigned inside;
 #pragma unroll
-    for (int q = 0; q < NF_GEOM_PPT; ++q) Y[q] = (float)(j0 + NF_GEOM_TY * q) * G.dx;
+    for (int q = 0; q < NF_GEOM_PPT; ++q) { X[q] = (float)pt.i[q] * G.dx; Y[q] = (float)pt.j[q] * G.dx; }
     nf_geom_scan<true>(S.seg, NM, X, Y, d2, kb, tb, inside);
 #pragma unroll
     for (int q = 0; q < NF_GEOM_PPT; ++q) {
@@ -331,7 +350,7 @@ __global__ void __launch_bounds__(NF_GEOM_TX *NF_GEOM_TY) k_geom_sdf_adjoint(NfG
         const float *sg = S.seg + 6 * kb[q];
         const float qx = sg[0] + tb[q] * sg[2], qy = sg[1] + tb[q] * sg[3];
         const float sc = -sgn * g[q] / dist;
-        const float gx = sc * (X - qx), gy = sc * (Y[q] - qy);
+        const float gx = sc * (X[q] - qx), gy = sc * (Y[q] - qy);
         const int k1 = kb[q] + 1 == NM ? 0 : kb[q] + 1;
         atomicAdd(&S.gV[2 * kb[q]], (1.0f - tb[q]) * gx);
         atomicAdd(&S.gV[2 * kb[q] + 1], (1.0f - tb[q]) * gy);
@@ -346,39 +365,25 @@ __global__ void __launch_bounds__(NF_GEOM_TX *NF_GEOM_TY) k_geom_sdf_adjoint(NfG
 // ------------------------------------------------------------------------------------------------------------
 // U_s on the faces of family C (R30): the closest surface point's velocity along the in-plane normal, caps move in z
 // ------------------------------------------------------------------------------------------------------------
-template <int C>
-__device__ __forceinline__ void nf_face_point(int i, int j0, int k, float dx, float &X, float (&Y)[NF_GEOM_PPT], double &z) {
-  X = (C == 0) ? (float)i * dx : ((float)i + 0.5f) * dx;
-#pragma unroll
-  for (int q = 0; q < NF_GEOM_PPT; ++q) {
-    const int j = j0 + NF_GEOM_TY * q;
-    Y[q] = (C == 1) ? (float)j * dx : ((float)j + 0.5f) * dx;
-  }
-  z = (C == 2) ? (double)k * (double)dx : ((double)k + 0.5) * (double)dx;
-}
-
 template <int C, bool ADJ>
-__global__ void __launch_bounds__(NF_GEOM_TX *NF_GEOM_TY) k_geom_velocity(NfGeomK G, int nxf, int nyf, float band,
-                                                                          float *__restrict__ out,
-                                                                          const float *__restrict__ gin,
-                                                                          double *__restrict__ gout) {
+__global__ void __launch_bounds__(NF_GEOM_NT) k_geom_velocity(NfGeomK G, int nxf, int nyf, float band,
+                                                              float *__restrict__ out, const float *__restrict__ gin,
+                                                              double *__restrict__ gout) {
   extern __shared__ __align__(16) unsigned char nf_geom_raw[];
   const NfGeomSm S = nf_geom_carve(nf_geom_raw, G.N, G.M);
-  const int i = blockIdx.x * NF_GEOM_TX + threadIdx.x;
-  const int j0 = blockIdx.y * (NF_GEOM_TY * NF_GEOM_PPT) + threadIdx.y;
-  float X, Y[NF_GEOM_PPT];
-  double z;
-  nf_face_point<C>(i, j0, blockIdx.z, G.dx, X, Y, z);
+  const double z = (C == 2) ? (double)blockIdx.z * (double)G.dx : ((double)blockIdx.z + 0.5) * (double)G.dx;
   const NfGeomPlane P = nf_geom_plane(G, z);
   nf_geom_setup(G, P, S, ADJ);
   const int NM = G.N * G.M;
-  float g[NF_GEOM_PPT];
-  bool work = !ADJ && i < nxf;
+  const NfGeomPts pt = nf_geom_points(nxf, nyf);
+  float X[NF_GEOM_PPT], Y[NF_GEOM_PPT], g[NF_GEOM_PPT];
+  bool work = false;
 #pragma unroll
   for (int q = 0; q < NF_GEOM_PPT; ++q) {
-    const int j = j0 + NF_GEOM_TY * q;
-    g[q] = (ADJ && i < nxf && j < nyf) ? gin[((size_t)blockIdx.z * nyf + j) * nxf + i] : 0.0f;
-    work = work || g[q] != 0.0f;
+    X[q] = (C == 0) ? (float)pt.i[q] * G.dx : ((float)pt.i[q] + 0.5f) * G.dx;
+    Y[q] = (C == 1) ? (float)pt.j[q] * G.dx : ((float)pt.j[q] + 0.5f) * G.dx;
+    g[q] = (ADJ && pt.ok[q]) ? gin[((size_t)blockIdx.z * nyf + pt.j[q]) * nxf + pt.i[q]] : 0.0f;
+    work = work || (ADJ ? g[q] != 0.0f : pt.ok[q]);
   }
   if (work) {
     float d2[NF_GEOM_PPT], tb[NF_GEOM_PPT];
@@ -388,8 +393,7 @@ __global__ void __launch_bounds__(NF_GEOM_TX *NF_GEOM_TY) k_geom_velocity(NfGeom
     const float zcap = ADJ ? 0.0f : G.pdot[P.cap];
 #pragma unroll
     for (int q = 0; q < NF_GEOM_PPT; ++q) {
-      const int j = j0 + NF_GEOM_TY * q;
-      if (j >= nyf || (ADJ && g[q] == 0.0f)) continue;
+      if (!pt.ok[q] || (ADJ && g[q] == 0.0f)) continue;
       const float dist = sqrtf(d2[q]);
       const float sd = ((inside >> q) & 1u) ? -dist : dist;
       if (!(fmaxf(sd, P.slab) <= band)) continue;
@@ -397,7 +401,7 @@ __global__ void __launch_bounds__(NF_GEOM_TX *NF_GEOM_TY) k_geom_velocity(NfGeom
       const float *sg = S.seg + 6 * kb[q];
       const int k1 = kb[q] + 1 == NM ? 0 : kb[q] + 1;
       const float inv = dist > 0.0f ? 1.0f / dist : 0.0f;
-      const float nx_ = (X - (sg[0] + tb[q] * sg[2])) * inv, ny_ = (Y[q] - (sg[1] + tb[q] * sg[3])) * inv;
+      const float nx_ = (X[q] - (sg[0] + tb[q] * sg[2])) * inv, ny_ = (Y[q] - (sg[1] + tb[q] * sg[3])) * inv;
       const float nc = C == 0 ? nx_ : ny_;
       if (!ADJ) {
         float val = 0.0f;
@@ -408,7 +412,7 @@ __global__ void __launch_bounds__(NF_GEOM_TX *NF_GEOM_TY) k_geom_velocity(NfGeom
           const float qdy = (1.0f - tb[q]) * S.Vd[2 * kb[q] + 1] + tb[q] * S.Vd[2 * k1 + 1];
           val = (nx_ * qdx + ny_ * qdy) * nc;
         }
-        out[((size_t)blockIdx.z * nyf + j) * nxf + i] = val;
+        out[((size_t)blockIdx.z * nyf + pt.j[q]) * nxf + pt.i[q]] = val;
       } else {
         if (cap) {
           if (C == 2) { S.gsl[2] = 1.0f; atomicAdd(&S.gsl[P.cap], g[q]); }
@@ -486,7 +490,8 @@ static int geom_smem(nf_grid *g, Kern kern, int N, int M, size_t *bytes) {
 }
 
 static dim3 geom_grid(int npx, int npy, int npz) {
-  return dim3((npx + NF_GEOM_TX - 1) / NF_GEOM_TX, (npy + NF_GEOM_TY * NF_GEOM_PPT - 1) / (NF_GEOM_TY * NF_GEOM_PPT), npz);
+  const long long per = (long long)NF_GEOM_NT * NF_GEOM_PPT;
+  return dim3((unsigned)(((long long)npx * npy + per - 1) / per), 1, npz);
 }
 
 static int geom_download(nf_grid *g, int K, int N, double *gout_host) {
@@ -502,7 +507,7 @@ int nf_geom_sdf_impl(nf_grid *g, const float *params, int K, int N, int M, int f
   NF_TRY(geom_upload(g, params, nullptr, K, N, &G, M));
   size_t sm;
   NF_TRY(geom_smem(g, k_geom_sdf, N, M, &sm));
-  const dim3 block(NF_GEOM_TX, NF_GEOM_TY);
+  const dim3 block(NF_GEOM_NT);
   NF_LAUNCH(g, NFK_GEOM, k_geom_sdf<<<geom_grid(g->nx + 1, g->ny + 1, g->nz + 1), block, sm, g->stream>>>(
                              G, g->nx + 1, g->ny + 1, (flags & NF_GEOM_COMPLEMENT) ? -1.0f : 1.0f, sdf_nodes));
   NF_CUDA(g, cudaGetLastError());
@@ -517,7 +522,7 @@ int nf_geom_sdf_adjoint_impl(nf_grid *g, const float *params, int K, int N, int 
   size_t sm;
   NF_TRY(geom_smem(g, k_geom_sdf_adjoint, N, M, &sm));
   NF_CUDA(g, cudaMemsetAsync(g->geom_grad, 0, NF_GEOM_MAXP * sizeof(double), g->stream));
-  const dim3 block(NF_GEOM_TX, NF_GEOM_TY);
+  const dim3 block(NF_GEOM_NT);
   NF_LAUNCH(g, NFK_GEOM, k_geom_sdf_adjoint<<<geom_grid(g->nx + 1, g->ny + 1, g->nz + 1), block, sm, g->stream>>>(
                              G, g->nx + 1, g->ny + 1, (flags & NF_GEOM_COMPLEMENT) ? -1.0f : 1.0f, gsdf_nodes, g->geom_grad));
   NF_CUDA(g, cudaGetLastError());
@@ -531,7 +536,7 @@ static int geom_velocity_launch(nf_grid *g, const NfGeomK &G, float band, float 
   NF_TRY(geom_smem(g, k_geom_velocity<0, ADJ>, G.N, G.M, &sm));
   NF_TRY(geom_smem(g, k_geom_velocity<1, ADJ>, G.N, G.M, &sm));
   NF_TRY(geom_smem(g, k_geom_velocity<2, ADJ>, G.N, G.M, &sm));
-  const dim3 block(NF_GEOM_TX, NF_GEOM_TY);
+  const dim3 block(NF_GEOM_NT);
   const int nx = g->nx, ny = g->ny, nz = g->nz;
   if (ADJ ? gus != nullptr : us != nullptr)
     NF_LAUNCH(g, NFK_GEOM, k_geom_velocity<0, ADJ><<<geom_grid(nx + 1, ny, nz), block, sm, g->stream>>>(
