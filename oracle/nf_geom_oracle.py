@@ -16,7 +16,8 @@ in physical units; node (i, j, k) of the grid sits at (i dx, j dx, k dx); phi ar
 Sign convention (R2): phi > 0 in the fluid.  A primitive is solid INSIDE its closed surface (phi < 0
 there); `complement=True` flips it (fluid inside: a chamber).
 
-parity unpinned: nothing in this file.  Pins: tests/test_oracle_geometry.py.
+parity unpinned: nothing in this file.  Pins: tests/test_oracle_geometry.py.  rollout_parametric composes this
+file with oracle/nf_oracle.py (the only import between the two oracle modules).
 """
 import numpy as np
 
@@ -348,3 +349,65 @@ def solid_velocity_faces_adjoint(params, K, N, M, nx, ny, nz, dx, gus, gvs, gws,
         us, vs, ws = solid_velocity_faces(params, e, K, N, M, nx, ny, nz, dx, band)
         g[a] = np.sum(us * gus) + np.sum(vs * gvs) + np.sum(ws * gws)
     return g
+
+
+# ----------------------------------------------------------------------------------------------------
+# the co-design loop: parametric geometry inside the time stepping
+# ----------------------------------------------------------------------------------------------------
+def rollout_parametric(U0, prims_fn, nsteps, dt, dx, dt_over_rho, bc, loss_fn, tol=1e-12, advect_on=True, band=np.inf):
+    """N steps "advect -> geometry at t^{n+1} -> project" (R15) with the solid given by parametric primitives, and
+    the backward pass down to the parameters (L132-141).
+
+    prims_fn(step) -> list of (params, pdot or None, K, N, M) for step = 1..N: the solid is the union (R29) of the
+    primitives; a primitive with pdot moves and supplies U_s on the faces within `band` of it (R30), in list order.
+    Returns (J, grads, dJ/dU0), grads[step-1][i] = (dJ/dparams, dJ/dpdot or None) of primitive i at that step:
+    dJ/dparams through phi only (Eq. 9a -> weight builder -> union -> distance, L141), dJ/dpdot the transpose of the
+    velocity map applied to Eq. 9b's dJ/dU_s (R31)."""
+    from . import nf_oracle as orc
+    U = [np.asarray(a, dtype=np.float64) for a in U0]
+    nz, ny, nx = U[0].shape[0], U[0].shape[1], U[0].shape[2] - 1
+    tape = []
+    for n in range(1, nsteps + 1):
+        Uprev = U
+        Ut = orc.advect(U, dt, dx) if advect_on else [a.copy() for a in U]
+        prims = prims_fn(n)
+        phis = [sdf_nodes(p, K, N, M, nx, ny, nz, dx) for (p, pd, K, N, M) in prims]
+        partial = [phis[0]]
+        for f in phis[1:]:
+            partial.append(csg("union", partial[-1], f))
+        phi = partial[-1]
+        us = None
+        for (p, pd, K, N, M) in prims:
+            if pd is not None:
+                us = solid_velocity_faces(p, pd, K, N, M, nx, ny, nz, dx, band, us)
+        alpha = orc.face_weights(phi, bc)
+        U, pr = orc.project(Ut, alpha, us, dx, dt_over_rho, bc, tol=tol)
+        tape.append((Uprev, Ut, prims, phis, partial, us, alpha, pr, phi))
+    J, g = loss_fn(U)
+    g = [np.asarray(a, dtype=np.float64) for a in g]
+    grads = [None] * nsteps
+    for n in range(nsteps, 0, -1):
+        Uprev, Ut, prims, phis, partial, us, alpha, pr, phi = tape[n - 1]
+        g_ut, g_alpha, g_us, _ = orc.project_adjoint(g, alpha, pr, Ut, us, dx, dt_over_rho, bc, tol=tol)
+        g_phi = orc.weights_adjoint(phi, g_alpha[0], g_alpha[1], g_alpha[2], bc)
+        gphis = [None] * len(prims)
+        for i in range(len(prims) - 1, 0, -1):
+            g_phi, gphis[i] = csg_adjoint("union", partial[i - 1], phis[i], g_phi)
+        gphis[0] = g_phi
+        # a face's U_s was written by the LAST moving primitive whose band covers it: walk the list backwards and
+        # clear dJ/dU_s on the faces a primitive owns once it has taken them (its velocity map with pdot = 0 writes 0
+        # exactly there)
+        g_us = [a.copy() for a in g_us]
+        out = [None] * len(prims)
+        for i in range(len(prims) - 1, -1, -1):
+            p, pd, K, N, M = prims[i]
+            gp = sdf_nodes_adjoint(p, K, N, M, nx, ny, nz, dx, gphis[i])
+            gd = None
+            if pd is not None:
+                gd = solid_velocity_faces_adjoint(p, K, N, M, nx, ny, nz, dx, *g_us, band=band)
+                g_us = list(solid_velocity_faces(p, np.zeros_like(np.asarray(p, dtype=np.float64)), K, N, M, nx, ny,
+                                                 nz, dx, band, out=g_us))
+            out[i] = (gp, gd)
+        grads[n - 1] = out
+        g = orc.advect_adjoint(Uprev, g_ut, dt, dx) if advect_on else g_ut
+    return J, grads, g

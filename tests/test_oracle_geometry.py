@@ -261,3 +261,58 @@ def test_velocity_is_linear_in_pdot_and_adjoint_is_its_transpose():
     vb = G.solid_velocity_faces(p, a, K, N, M, n, n, n, dx, band=0.1, out=keep)
     assert np.array_equal(vb[0][2] == 7.0, phi_u > 0.1) and np.array_equal(vb[0][2][phi_u <= 0.1], va[0][2][phi_u <= 0.1])
     assert 0 < np.count_nonzero(phi_u <= 0.1) < phi_u.size
+
+
+# --- the co-design loop: finite differences of the loss through full time steps ---------------------------------------------
+def _rollout_setup():
+    from oracle import nf_oracle as orc
+    n, dx = 10, 0.1
+    bc = orc.BC((1, 1, 0, 0, 0, 0), (1.0, 0.0, 0, 0, 0, 0))
+    rng = np.random.default_rng(21)
+    U0 = [0.2 * rng.standard_normal(s) for s in ((n, n, n + 1), (n, n + 1, n), (n + 1, n, n))]
+    pA = rand_params(rng, 2, 4, z0=0.22, z1=0.77, c=(0.38, 0.5), r=0.17)
+    pB = rand_params(rng, 1, 3, z0=0.31, z1=0.68, c=(0.7, 0.45), r=0.12)
+    dB = 0.3 * rng.standard_normal(pB.shape)
+
+    def loss(U):
+        return 0.5 * sum(float(np.sum(a * a)) for a in U), [a.copy() for a in U]
+    return orc, n, dx, bc, U0, pA, pB, dB, loss
+
+
+def test_design_gradient_of_a_rollout_matches_finite_differences():
+    """dJ/dparams of a static shape (the paper's design tasks) through 2 full steps: sum over steps of the per-step
+    gradient against a central difference of the loss (the paper's own validation method, L430-434)."""
+    orc, n, dx, bc, U0, pA, pB, dB, loss = _rollout_setup()
+    prims = lambda a, b: (lambda step: [(a, None, 2, 4, 5), (b, None, 1, 3, 6)])
+    J, grads, gU0 = G.rollout_parametric(U0, prims(pA, pB), 2, 0.04, dx, 1.0, bc, loss)
+    gA = sum(g[0][0] for g in grads)
+    gB = sum(g[1][0] for g in grads)
+    assert grads[0][0][1] is None
+    rng = np.random.default_rng(2)
+    for _ in range(2):
+        dA, dBdir = rng.standard_normal(pA.shape) * 0.02, rng.standard_normal(pB.shape) * 0.02
+        h = 1e-4
+        Jp = G.rollout_parametric(U0, prims(pA + h * dA, pB + h * dBdir), 2, 0.04, dx, 1.0, bc, loss)[0]
+        Jm = G.rollout_parametric(U0, prims(pA - h * dA, pB - h * dBdir), 2, 0.04, dx, 1.0, bc, loss)[0]
+        fd = (Jp - Jm) / (2 * h)
+        an = gA @ dA + gB @ dBdir
+        assert abs(fd - an) < 2e-3 * max(abs(fd), abs(an)), (fd, an)
+        assert abs(fd) > 1e-4
+
+
+def test_control_gradient_of_a_rollout_matches_finite_differences():
+    """dJ/dpdot of a moving primitive (the paper's control tasks): U_s is linear in pdot and phi does not depend on it,
+    so the transpose is exact and the loss is quadratic in pdot."""
+    orc, n, dx, bc, U0, pA, pB, dB, loss = _rollout_setup()
+    band = 0.15
+    prims = lambda d: (lambda step: [(pA, None, 2, 4, 5), (pB, d * (1.0 if step == 1 else -0.5), 1, 3, 6)])
+    J, grads, _ = G.rollout_parametric(U0, prims(dB), 2, 0.04, dx, 1.0, bc, loss, band=band)
+    rng = np.random.default_rng(3)
+    dd = rng.standard_normal(pB.shape) * 0.1
+    h = 1e-3
+    Jp = G.rollout_parametric(U0, prims(dB + h * dd), 2, 0.04, dx, 1.0, bc, loss, band=band)[0]
+    Jm = G.rollout_parametric(U0, prims(dB - h * dd), 2, 0.04, dx, 1.0, bc, loss, band=band)[0]
+    fd = (Jp - Jm) / (2 * h)
+    an = grads[0][1][1] @ dd - 0.5 * (grads[1][1][1] @ dd)
+    assert abs(fd - an) < 1e-6 * max(abs(fd), abs(an)), (fd, an)
+    assert abs(fd) > 1e-6
