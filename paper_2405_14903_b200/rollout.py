@@ -60,3 +60,76 @@ def cfl_substeps(grid, U, dt_frame, cfl=1.0, max_substeps=64):
         return dt_frame, 1
     n = max(1, min(max_substeps, int(math.ceil(dt_frame * vmax / (cfl * grid.dx) - 1e-9))))
     return dt_frame / n, n
+
+
+def rollout_parametric(grid, U0, prims_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect_on=True, band=float("inf")):
+    """The co-design loop: like rollout(), with the solid of step n given by
+    parametric primitives: prims_fn(step) -> list of (params, pdot or None, K, N, M) (host vectors, layout of
+    include/nf.h).  The solid is the union of the primitives; one with pdot moves and supplies U_s on the faces
+    within `band` of it, in list order.  Backward: nf_project_adjoint -> nf_weights_adjoint -> nf_geom_csg_adjoint ->
+    nf_geom_sdf_adjoint (dJ/dparams, through phi) and nf_geom_velocity_adjoint (dJ/dpdot).
+    Returns (J, grads, dJ/dU0), grads[step-1][i] = (dJ/dparams, dJ/dpdot or None) as float64 NumPy vectors."""
+    import numpy as np
+    g = grid
+    dev = U0[0].device
+    new_nodes = lambda: torch.empty(g.shape_sdf, dtype=torch.float32, device=dev)
+    U = [a.clone() for a in U0]
+    tape = []
+    for n in range(1, nsteps + 1):
+        Uprev = [a.clone() for a in U]
+        if advect_on:
+            g.advect(*U, dt)
+        prims = prims_fn(n)
+        phis, partial = [], []
+        for i, (p, pd, K, N, M) in enumerate(prims):
+            f = new_nodes()
+            g.geom_sdf(p, K, N, M, f)
+            phis.append(f)
+            if i == 0:
+                partial.append(f)
+            else:
+                u = new_nodes()
+                g.geom_csg("union", partial[-1], f, u)
+                partial.append(u)
+        us = None
+        for (p, pd, K, N, M) in prims:
+            if pd is not None:
+                if us is None:
+                    us = [torch.zeros(s, dtype=torch.float32, device=dev) for s in (g.shape_u, g.shape_v, g.shape_w)]
+                g.geom_velocity(p, pd, K, N, M, *us, band=band)
+        g.set_solid(partial[-1], *(us if us is not None else (None, None, None)))
+        Uhat = [a.clone() for a in U]
+        pr = torch.empty(g.shape_p, dtype=torch.float32, device=dev)
+        g.project(*U, pr, tol=tol, maxit=maxit)
+        tape.append((Uprev, Uhat, pr, prims, phis, partial, us))
+    J, G = loss_fn(U)
+    G = [a.clone() for a in G]
+    ga = [torch.empty_like(a) for a in U]
+    gs = [torch.empty_like(a) for a in U]
+    grads = [None] * nsteps
+    for n in range(nsteps, 0, -1):
+        Uprev, Uhat, pr, prims, phis, partial, us = tape[n - 1]
+        g.set_solid(partial[-1], *(us if us is not None else (None, None, None)))
+        g.project_adjoint(*G, p_saved=pr, uhat=Uhat, galpha=ga, gus=gs, tol=tol, maxit=maxit)
+        gphi = new_nodes()
+        g.weights_adjoint(*ga, gphi)
+        gphis = [None] * len(prims)
+        for i in range(len(prims) - 1, 0, -1):
+            ga_i, gb_i = new_nodes(), new_nodes()
+            g.geom_csg_adjoint("union", partial[i - 1], phis[i], gphi, ga_i, gb_i)
+            gphi, gphis[i] = ga_i, gb_i
+        gphis[0] = gphi
+        out = [None] * len(prims)
+        for i in range(len(prims) - 1, -1, -1):
+            p, pd, K, N, M = prims[i]
+            gp = g.geom_sdf_adjoint(p, K, N, M, gphis[i])
+            gd = None
+            if pd is not None:
+                gd = g.geom_velocity_adjoint(p, K, N, M, *gs, band=band)
+                # the faces this primitive owns are taken: its velocity map with pdot = 0 writes 0 exactly there
+                g.geom_velocity(p, np.zeros_like(np.asarray(p, dtype=np.float32)), K, N, M, *gs, band=band)
+            out[i] = (gp, gd)
+        grads[n - 1] = out
+        if advect_on:
+            g.advect_adjoint(*Uprev, *G, dt)
+    return float(J), grads, G

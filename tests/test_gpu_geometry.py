@@ -237,3 +237,46 @@ def test_geometry_error_codes(torch, api):
         g.geom_sdf(wl.geom_random_params(1, 1, 64, 0.2, 0.8, (0.5, 0.5), 0.2), 1, 64, 33, sdf)   # N M > 2048
     g.geom_sdf(p, 1, 4, 8, sdf)
     g.close()
+
+
+def test_parametric_rollout_matches_oracle(torch, api):
+    """Two full time steps with a static and a moving primitive: loss, dJ/dparams and dJ/dpdot of every primitive at
+    every step, dJ/dU0 -- device path (paper_2405_14903_b200/rollout.py: C-ABI calls only) vs the oracle's
+    rollout_parametric; north_star's tolerances (1e-4 loss and fields, 1e-3 gradients)."""
+    from paper_2405_14903_b200 import rollout as ro
+    n, dx = 24, float(np.float32(1.0 / 24))
+    bc_t, bc_v = (1, 1, 0, 0, 0, 0), (1.0, 0.0, 0, 0, 0, 0)
+    bc = orc.BC(bc_t, bc_v)
+    rng = np.random.default_rng(8)
+    U0 = [(0.2 * rng.standard_normal(s)).astype(np.float32) for s in wl.face_shapes(n, n, n)]
+    pA = wl.geom_random_params(51, 2, 5, 0.21, 0.79, (0.36, 0.5), 0.17)
+    pB = wl.geom_random_params(52, 1, 4, 0.3, 0.71, (0.7, 0.46), 0.12)
+    dB = wl.geom_random_rates(53, 1, 4, 0.3)
+    band, dt, nsteps = 3.0 * dx, 0.4 * dx, 2
+    prims = lambda step: [(pA, None, 2, 5, 8), (pB, dB * np.float32(1.0 if step == 1 else -0.5), 1, 4, 10)]
+
+    g = api.Grid(n, n, n, dx)
+    for f in range(6):
+        g.set_domain_bc(f, bc_t[f], bc_v[f])
+
+    def loss_dev(U):
+        return 0.5 * sum((a.double() ** 2).sum() for a in U), [a.clone() for a in U]
+    J, grads, gU0 = ro.rollout_parametric(g, [dev(torch, a) for a in U0], prims, nsteps, dt, loss_dev, tol=1e-7,
+                                          maxit=400, band=band)
+
+    def loss_ref(U):
+        return 0.5 * sum(float(np.sum(a * a)) for a in U), [a.copy() for a in U]
+    p64 = lambda step: [(p.astype(np.float64), None if d is None else d.astype(np.float64), K, N, M)
+                        for (p, d, K, N, M) in prims(step)]
+    Jr, gr, gU0r = G.rollout_parametric(U0, p64, nsteps, dt, dx, 1.0, bc, loss_ref, band=band)
+    assert abs(J - Jr) < 1e-4 * abs(Jr)
+    for s in range(nsteps):
+        for i in range(2):
+            for got, ref in zip(grads[s][i], gr[s][i]):
+                assert (got is None) == (ref is None)
+                if ref is not None:
+                    assert np.max(np.abs(ref)) > 0
+                    assert np.max(np.abs(got - ref)) < 1e-3 * np.max(np.abs(ref)), (s, i)
+    num = np.sqrt(sum(float(((a.cpu().numpy() - b) ** 2).sum()) for a, b in zip(gU0, gU0r)))
+    assert num < 1e-3 * np.sqrt(sum(float((b ** 2).sum()) for b in gU0r))
+    g.close()
