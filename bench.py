@@ -539,6 +539,59 @@ def run_geometry(args):
                                    "traffic": None}}))
 
 
+def run_envs(args):
+    """E concurrent small environments (paper_2405_14903_b200/envs.py: one handle, stream and host
+    thread each) -- aggregate forward + adjoint projection steps per second at the paper's task sizes (PAPER.md:L151-160:
+    40^3-48^3), a step = nf_set_solid + nf_project + nf_project_adjoint to 1e-6 on a sphere-in-channel grid."""
+    import time
+    import numpy as np
+    import torch
+    from paper_2405_14903_b200 import api, envs, workloads as wl
+    api.load_library()
+    torch.cuda.set_device(0)
+    n = args.n
+    i, j, k = wl.node_coords(n, n, n)
+    phi = torch.from_numpy(wl.sdf_sphere(i, j, k, (n / 2 + 0.3, n / 2 - 0.2, n / 2 + 0.1), n / 5).astype(np.float32)).cuda()
+    rows = []
+    for E in [int(x) for x in args.envs.split(",")]:
+        pool = envs.EnvPool(E, n, n, n, 1.0 / n)
+        for g in pool.grids:
+            g.set_domain_bc(0, 1, 1.0)
+            g.set_domain_bc(1, 1, 0.0)
+        rng = np.random.default_rng(1)
+        U0 = [[torch.from_numpy((0.3 * rng.standard_normal(s)).astype(np.float32)).cuda() for s in wl.face_shapes(n, n, n)]
+              for _ in range(E)]
+        torch.cuda.synchronize()
+
+        def work(reps):
+            def fn(e, g):
+                p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+                its = 0
+                for _ in range(reps):
+                    V = [a.clone() for a in U0[e]]
+                    g.set_solid(phi)
+                    g.project(*V, p, tol=TOL, maxit=MAXIT)
+                    its += g.last_solve_info()["iters"]
+                    g.project_adjoint(*V, p_saved=p, uhat=U0[e], tol=TOL, maxit=MAXIT)
+                    its += g.last_solve_info()["iters"]
+                torch.cuda.current_stream().synchronize()
+                return its
+            return fn
+        pool.run(work(max(args.warmup, 3)))
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        its = pool.run(work(args.steps))
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        rows.append({"envs": E, "env_steps_per_s": round(E * args.steps / dt, 1),
+                     "ms_per_env_step": round(1e3 * dt / args.steps, 3),
+                     "iters_per_solve": round(sum(its) / (2.0 * E * args.steps), 1)})
+        pool.close()
+    print(json.dumps({"workload": "NEXT-4 concurrent environments, %d^3 sphere-in-channel, forward + adjoint projection "
+                                  "to %g (wall clock over all environments, host threads included)" % (n, TOL),
+                      "dtype": "f32", "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -554,7 +607,12 @@ def main():
                                                  "instead of the headline step, e.g. --sweep 64,128,256,384")
     ap.add_argument("--geometry", action="store_true",
                     help="time the NEXT-2 parametric-geometry kernels at --n instead of the headline step")
+    ap.add_argument("--envs", default="", help="comma-separated environment counts: aggregate throughput of concurrent "
+                                                "small grids of size --n (e.g. --envs 1,4,8 --n 48) instead of the headline step")
     args = ap.parse_args()
+    if args.envs:
+        run_envs(args)
+        return
     if args.sweep:
         run_sweep(args)
         return

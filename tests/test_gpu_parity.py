@@ -507,3 +507,38 @@ def test_two_dimensional_mode(torch, api, shape, dirichlet):
     assert g.project_adjoint(*dG, tol=1e-6, maxit=200) == 0
     assert rel3([host(a) for a in dG], gref) <= TOL_FIELD
     g.close()
+
+
+def test_concurrent_environments_match_the_oracle(torch, api):
+    """four small environments solved concurrently (one handle, stream and host thread each,
+    paper_2405_14903_b200/envs.py) give, each, the oracle's projection of its own input."""
+    from paper_2405_14903_b200 import envs
+    n, dx = 20, 1.0 / 20
+    bc_t, bc_v = (1, 1, 0, 0, 0, 0), (1.0, 0.0, 0, 0, 0, 0)
+    bc = orc.BC(bc_t, bc_v)
+    i, j, k = wl.node_coords(n, n, n)
+    E = 4
+    phis = [wl.sdf_sphere(i, j, k, (9.3 + e, 10.2, 9.9 - 0.5 * e), 4.0 + 0.4 * e).astype(np.float32) for e in range(E)]
+    rng = np.random.default_rng(17)
+    Us = [[(0.3 * rng.standard_normal(s)).astype(np.float32) for s in wl.face_shapes(n, n, n)] for _ in range(E)]
+    pool = envs.EnvPool(E, n, n, n, dx)
+    for g in pool.grids:
+        for f in range(6):
+            g.set_domain_bc(f, bc_t[f], bc_v[f])
+
+    def fn(e, g):
+        res = None
+        for _ in range(3):   # several rounds so that the solves of different environments really interleave
+            U = [dev(torch, a) for a in Us[e]]
+            p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+            g.set_solid(dev(torch, phis[e]))
+            assert g.project(*U, p, tol=1e-6, maxit=200) == 0
+            res = [host(a) for a in U], host(p)
+        return res
+    out = pool.run(fn)
+    for e in range(E):
+        alpha = orc.face_weights(phis[e], bc)
+        Uref, pref = orc.project(Us[e], alpha, None, dx, 1.0, bc)
+        assert rel(out[e][1], pref) < TOL_FIELD
+        assert rel3(out[e][0], Uref) < TOL_FIELD
+    pool.close()
