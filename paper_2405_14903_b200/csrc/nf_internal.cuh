@@ -216,6 +216,16 @@ static inline NfDims nf_vdims(int tx, int ty, int tz, int kch) {
   return d;
 }
 
+// Planes per CTA for a level: the full chunk (kmax) only where that still leaves >= 4 CTAs per SM; small grids (the
+// paper's 40^3-64^3 tasks) march less and spread over more CTAs instead -- at 48^3 eight planes per CTA meant 18 CTAs
+// on 148 SMs.
+static inline int nf_kch(int tx, int ty, int tz, int kmax) {
+  const NfDims d = nf_vdims(tx, ty, tz, 1);
+  const long long ctas = (long long)d.grid.x * d.grid.y * tz;
+  const long long k = ctas / (148 * 4);  // (measured 48^3 .. 192^3: 2, 4, 8, 16, 32 CTAs per SM; 4 is best at 128^3)
+  return (int)(k < 1 ? 1 : (k > kmax ? kmax : k));
+}
+
 // ---- kernels / host launchers implemented across the .cu files -------------------------------------------
 // nf_weights.cu
 int nf_weights_from_sdf(nf_grid *g, const float *sdf);

@@ -1041,8 +1041,9 @@ bool nf_update_down1_ok(const nf_grid *g) {
 }
 int nf_update_down1(nf_grid *g, int slot, NfHostStatus *hs, int seq) {
   NfLevel &L = g->lv[0];
-  NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
-  NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_update_down1, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.r, (const float *)g->q, g->r_alt, L.z, NF_KCH_MG, g->st, slot, hs, seq));
+  const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+  NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
+  NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_update_down1, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.r, (const float *)g->q, g->r_alt, L.z, kch, g->st, slot, hs, seq));
   float *t = L.r;
   L.r = g->r_alt;
   g->r_alt = t;
@@ -1061,9 +1062,10 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
   for (int l = 0; l < (coop ? 1 : nb); ++l) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
     if (L.vec && fused) {
-      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+      const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
       if (!(l == 0 && skip_down1))
-        NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), nf_launch_pdl(k_down1, d.grid, d.block, g->stream, nf_lvk(L), L.r, L.z, NF_KCH_MG, (const NfSolveState *)st));
+        NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), nf_launch_pdl(k_down1, d.grid, d.block, g->stream, nf_lvk(L), L.r, L.z, kch, (const NfSolveState *)st));
       NfDims d2 = nf_vdims(L.nx / 4, C.ny, C.nz, 1);
       NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), nf_launch_pdl(k_down2, d2.grid, d2.block, g->stream, nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, 1, (const NfSolveState *)st));
     } else {
@@ -1131,13 +1133,14 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
   for (int l = (coop ? 0 : nb - 1); l >= 0; --l) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
     if (L.vec && fused) {
-      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
-      NF_LAUNCH(g, (l == 0 ? NFK_UP1_0 : NFK_VEC_C), nf_launch_pdl(k_up1, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, C.z, C.nx, C.ny, NF_KCH_MG, (const NfSolveState *)st));
+      const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
+      NF_LAUNCH(g, (l == 0 ? NFK_UP1_0 : NFK_VEC_C), nf_launch_pdl(k_up1, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, C.z, C.nx, C.ny, kch, (const NfSolveState *)st));
       if (l == 0 && with_dot) {
-        NF_LAUNCH(g, NFK_UP2_0, nf_launch_pdl(k_up2<true>, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, NF_KCH_MG, g->st, slot));
+        NF_LAUNCH(g, NFK_UP2_0, nf_launch_pdl(k_up2<true>, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, kch, g->st, slot));
         dot_done = true;
       } else {
-        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), nf_launch_pdl(k_up2<false>, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, NF_KCH_MG, st, slot));
+        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), nf_launch_pdl(k_up2<false>, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, kch, st, slot));
       }
     } else {
       NfDims d = nf_dims(L.nx, L.ny, L.nz);

@@ -529,11 +529,12 @@ static inline bool apply_vec_ok(const NfLevel &L, const float *p, const float *q
 static void launch_apply(nf_grid *g, const float *p, float *q, bool dot, int slot) {
   NfLevel &L = g->lv[0];
   if (!g->force_generic && apply_vec_ok(L, p, q)) {
-    NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
+    const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
+    NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
     if (dot)
-      NF_LAUNCH(g, NFK_APPLY, k_apply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, NF_KCH_AP, g->st, slot));
+      NF_LAUNCH(g, NFK_APPLY, k_apply4<true><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, kch, g->st, slot));
     else
-      NF_LAUNCH(g, NFK_APPLY, k_apply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, NF_KCH_AP, nullptr, 0));
+      NF_LAUNCH(g, NFK_APPLY, k_apply4<false><<<d.grid, d.block, 0, g->stream>>>(nf_lvk(L), p, q, kch, nullptr, 0));
   } else {
     NfDims d = nf_dims(L.nx, L.ny, L.nz);
     if (dot)
@@ -624,11 +625,12 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
     NfHostStatus *hs = &g->hst_dev[it & (NF_RING - 1)];
     if (fusedp) {
       float *pnew = (it & 1) ? g->p2 : g->p, *pold = (it & 1) ? g->p : g->p2;
-      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
+      const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
+      NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
       if (it == 0)
-        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<true>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
+        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<true>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, kch, g->st, slot));
       else
-        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<false>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, NF_KCH_AP, g->st, slot));
+        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<false>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, kch, g->st, slot));
       if (fusedr) {
         // r' = r - a q, ||r'||^2, the check and the pre-smoother of level 0 in one pass; the V-cycle skips its down1
         rc = nf_update_down1(g, slot, hs, it + 1);
