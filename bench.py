@@ -592,6 +592,53 @@ def run_envs(args):
                       "dtype": "f32", "rows": rows}))
 
 
+def run_karman(args):
+    """the paper's 2-D validation case (appendix D: flow past a cylinder on a
+    512 x 1024 grid with viscosity) as a timing workload -- nz = 1 grid of 1024 x 512 cells, inflow p = 1 / outflow p = 0,
+    a cylinder of radius 40 cells, nu = 0.01; a step = nf_advect + nf_viscosity + nf_project (the solid is static)."""
+    import numpy as np
+    import torch
+    from paper_2405_14903_b200 import api, workloads as wl
+    api.load_library()
+    torch.cuda.set_device(0)
+    nx, ny = 1024, 512
+    dx = 1.0 / ny
+    g = api.Grid(nx, ny, 1, dx)
+    g.set_domain_bc(0, 1, 1.0)
+    g.set_domain_bc(1, 1, 0.0)
+    i, j, k = wl.node_coords(nx, ny, 1)
+    phi = (np.sqrt((i - 256.3) ** 2 + (j - 255.7) ** 2) - 40.0 + 0 * k).astype(np.float32)
+    g.set_solid(torch.from_numpy(np.ascontiguousarray(phi)).cuda())
+    rng = np.random.default_rng(0)
+    U = [torch.from_numpy(((1.0 if c == 0 else 0.0) + 0.05 * rng.standard_normal(s)).astype(np.float32)).cuda()
+         for c, s in enumerate(wl.face_shapes(nx, ny, 1))]
+    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    dt, nu = 0.5 * dx, 0.01
+    its, pms = [], []
+
+    def step():
+        g.advect(*U, dt)
+        g.viscosity(*U, nu, dt)
+        g.project(*U, p, tol=TOL, maxit=MAXIT)
+        info = g.last_solve_info()
+        its.append(info["iters"])
+        pms.append(info["ms"])
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    del its[:], pms[:]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    print(json.dumps({"workload": "NEXT-3 2-D mode: cylinder in a 1024 x 512 channel, advect + viscosity + projection to %g" % TOL,
+                      "dtype": "f32", "ms_per_step": round(e0.elapsed_time(e1) / args.steps, 3),
+                      "solve_ms": round(sum(pms) / len(pms), 3), "iters_per_solve": round(sum(its) / len(its), 1),
+                      "levels": g.info()["levels"], "active_cells": g.info()["active_cells"]}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -609,7 +656,11 @@ def main():
                     help="time the NEXT-2 parametric-geometry kernels at --n instead of the headline step")
     ap.add_argument("--envs", default="", help="comma-separated environment counts: aggregate throughput of concurrent "
                                                 "small grids of size --n (e.g. --envs 1,4,8 --n 48) instead of the headline step")
+    ap.add_argument("--karman", action="store_true", help="time the 2-D cylinder-in-channel case (1024 x 512, nz = 1)")
     args = ap.parse_args()
+    if args.karman:
+        run_karman(args)
+        return
     if args.envs:
         run_envs(args)
         return

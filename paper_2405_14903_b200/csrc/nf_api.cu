@@ -93,7 +93,8 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   }
   g->nlev = nl;
   nf_mg_plan(g);
-  for (int l = 2; l < g->tail && l < nl; ++l) ok = ok && dalloc(&g->lv[l].pk, 8 * (size_t)g->lv[l].ncell) == cudaSuccess;
+  // (2-D mode runs the 4-cell bodies on every level above the tail: the packed per-cell phases assume 2x2x2 children)
+  for (int l = 2; l < g->tail && l < nl && nz != 1; ++l) ok = ok && dalloc(&g->lv[l].pk, 8 * (size_t)g->lv[l].ncell) == cudaSuccess;
   {
     size_t tc = 0;
     for (int l = g->tail; l < nl; ++l) tc += (size_t)g->lv[l].ncell;

@@ -176,16 +176,18 @@ __global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restri
   }
 }
 
-// One thread per pair of coarse cells (I0, I0+1) = fine cells i0..i0+3 of the rows (2J+dj, 2K+dk).
+// One thread per pair of coarse cells (I0, I0+1) = fine cells i0..i0+3 of the rows (2J+dj, FZ K+dk).  FZ = 2, or 1 in
+// 2-D mode (one layer: 2 x 2 x 1 children, R = P^T / 4).
+template <int FZ>
 __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, float *rc, int cnx, int cny, int i0,
                                               int J, int K) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const nf_idx sy = nx, sz = (nf_idx)nx * ny;
-  const int j0 = 2 * J, k0 = 2 * K;
-  float zc[2][2][4];  // [dk][dj][q]
-  unsigned cc[2][2];
+  const int j0 = 2 * J, k0 = FZ * K;
+  float zc[FZ][2][4];  // [dk][dj][q]
+  unsigned cc[FZ][2];
 #pragma unroll
-  for (int dk = 0; dk < 2; ++dk)
+  for (int dk = 0; dk < FZ; ++dk)
 #pragma unroll
     for (int dj = 0; dj < 2; ++dj) {
       const nf_idx id = ((nf_idx)(k0 + dk) * ny + (j0 + dj)) * nx + i0;
@@ -194,7 +196,7 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
     }
   float acc0 = 0.0f, acc1 = 0.0f;
 #pragma unroll
-  for (int dk = 0; dk < 2; ++dk)
+  for (int dk = 0; dk < FZ; ++dk)
 #pragma unroll
     for (int dj = 0; dj < 2; ++dj) {
       const int j = j0 + dj, k = k0 + dk;
@@ -203,7 +205,10 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
       // the y / z neighbour rows: inside the 2x2 block or one row outside it
       float yo[4], zo[4];
       nf_unpack4(dj == 0 ? nf_ld4(z, id - sy, j > 0) : nf_ld4(z, id + sy, j + 1 < ny), yo);
-      nf_unpack4(dk == 0 ? nf_ld4(z, id - sz, k > 0) : nf_ld4(z, id + sz, k + 1 < nz), zo);
+      if (FZ == 2)
+        nf_unpack4(dk == 0 ? nf_ld4(z, id - sz, k > 0) : nf_ld4(z, id + sz, k + 1 < nz), zo);
+      else
+        zo[0] = zo[1] = zo[2] = zo[3] = 0.0f;  // (one layer between closed walls: both z neighbours are ghosts)
       const float xe = par == 0 ? nf_ld1(z, id - 1, i0 > 0) : nf_ld1(z, id + 4, i0 + 4 < nx);
       const bool open4 = (cc[dk][dj] & 0x7f7f7f7fu) == 0x3f3f3f3fu;  // all four cells: six open faces
 #pragma unroll
@@ -211,7 +216,7 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
         if (((q + par) & 1) != 0) continue;  // red children only
         const float xl = q > 0 ? zc[dk][dj][q - 1] : xe, xh = q < 3 ? zc[dk][dj][q + 1] : xe;
         const float yl = dj == 0 ? yo[q] : zc[dk][0][q], yh = dj == 0 ? zc[dk][1][q] : yo[q];
-        const float zl = dk == 0 ? zo[q] : zc[0][dj][q], zh = dk == 0 ? zc[1][dj][q] : zo[q];
+        const float zl = dk == 0 ? zo[q] : zc[0][dj][q], zh = (FZ == 2 && dk == 0) ? zc[FZ - 1][dj][q] : zo[q];
         float s;
         if (open4) {
           s = ((xl + xh) + (yl + yh)) + (zl + zh);
@@ -222,7 +227,7 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
         if (q < 2) acc0 += s; else acc1 += s;
       }
     }
-  const float f = 0.125f * L.c;
+  const float f = (FZ == 2 ? 0.125f : 0.25f) * L.c;
   *reinterpret_cast<float2 *>(rc + ((nf_idx)K * cny + J) * cnx + (i0 >> 1)) = make_float2(f * acc0, f * acc1);
 }
 
@@ -234,7 +239,11 @@ __global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restri
   const int J = blockIdx.y * blockDim.y + threadIdx.y;
   if (i0 >= L.nx || J >= cny) return;
   const int K0 = blockIdx.z * kch, K1 = min(K0 + kch, cnz);
-  for (int K = K0; K < K1; ++K) nf_down2_body(L, z, rc, cnx, cny, i0, J, K);
+  if (L.fz == 2) {
+    for (int K = K0; K < K1; ++K) nf_down2_body<2>(L, z, rc, cnx, cny, i0, J, K);
+  } else {
+    for (int K = K0; K < K1; ++K) nf_down2_body<1>(L, z, rc, cnx, cny, i0, J, K);
+  }
 }
 
 // z + P z_coarse on a row of 4 fine cells
@@ -251,14 +260,14 @@ __device__ __forceinline__ void nf_row_prolonged(const float *z, const float *zc
 
 // Black half sweep on z + P zc (in place: only black cells change; red cells keep the un-prolonged value, which
 // k_up2 overwrites without reading).
-template <int PAR>
+template <int PAR, int FZ>
 __device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const float *r, const float *zc, int cnx,
                                             int cny, int i0, int j, int k) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const nf_idx sy = nx, sz = (nf_idx)nx * ny;
   const nf_idx id = ((nf_idx)k * ny + j) * nx + i0;
   const nf_idx scy = cnx, scz = (nf_idx)cnx * cny;
-  const nf_idx cid = ((nf_idx)(k >> 1) * cny + (j >> 1)) * cnx + (i0 >> 1);
+  const nf_idx cid = ((nf_idx)(k >> (FZ - 1)) * cny + (j >> 1)) * cnx + (i0 >> 1);  // (FZ == 1: nz == 1, no z rows)
   const float4 zold = *reinterpret_cast<const float4 *>(z + id);
   float zp[4], yl[4], yh[4], zl[4], zh[4], rr[4], out[4];
   {
@@ -312,10 +321,17 @@ __global__ void __launch_bounds__(256, 4) k_up1(NfLvK L, float *z, const float *
   if (i0 >= L.nx || j >= L.ny) return;
   const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, L.nz);
   for (int k = k0; k < k1; ++k) {
-    if ((j + k) & 1)
-      nf_up1_body<1>(L, z, r, zc, cnx, cny, i0, j, k);
-    else
-      nf_up1_body<0>(L, z, r, zc, cnx, cny, i0, j, k);
+    if (L.fz == 2) {
+      if ((j + k) & 1)
+        nf_up1_body<1, 2>(L, z, r, zc, cnx, cny, i0, j, k);
+      else
+        nf_up1_body<0, 2>(L, z, r, zc, cnx, cny, i0, j, k);
+    } else {
+      if ((j + k) & 1)
+        nf_up1_body<1, 1>(L, z, r, zc, cnx, cny, i0, j, k);
+      else
+        nf_up1_body<0, 1>(L, z, r, zc, cnx, cny, i0, j, k);
+    }
   }
 }
 
@@ -904,7 +920,10 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
     } else {
       for (int t = gt; t < nx4 * cny * cnz; t += gn) {
         const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
-        nf_down2_body(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
+        if (L.fz == 2)
+          nf_down2_body<2>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
+        else
+          nf_down2_body<1>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
       }
     }
     grid.sync();
@@ -926,9 +945,9 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
       for (int t = gt; t < nx4 * ny * nz; t += gn) {
         const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
         if ((j + k) & 1)
-          nf_up1_body<1>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+          (L.fz == 2 ? nf_up1_body<1, 2> : nf_up1_body<1, 1>)(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
         else
-          nf_up1_body<0>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+          (L.fz == 2 ? nf_up1_body<0, 2> : nf_up1_body<0, 1>)(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
       }
     }
     grid.sync();
@@ -972,7 +991,7 @@ void nf_mg_plan(nf_grid *g) {
     const NfLevel &L = g->lv[l];
     const double slots = (double)(L.nz + 1) * (L.ny + 1) * (L.pax + 4);  // largest face array of the level
     g->lv[l].vec_idx32 = slots < 4.0e9 ? 1 : 0;
-    g->lv[l].vec = (l < nb && (L.nx & 3) == 0 && g->lv[l].vec_idx32 && L.fz == 2) ? 1 : 0;
+    g->lv[l].vec = (l < nb && (L.nx & 3) == 0 && g->lv[l].vec_idx32) ? 1 : 0;
   }
 }
 

@@ -64,6 +64,10 @@ def blob_sdf(nx, ny, nz, seed, nblobs=6):
     phi = np.full((nz + 1, ny + 1, nx + 1), 1e9)
     for _ in range(nblobs):
         c = rng.uniform(0, 1, 3) * np.array([nx, ny, nz])
+        if nz == 1:  # 2-D mode: discs (cylinders along z)
+            r = rng.uniform(1.5, 0.2 * min(nx, ny) + 1.5)
+            phi = np.minimum(phi, np.sqrt((x - c[0]) ** 2 + (y - c[1]) ** 2) - r + 0 * z)
+            continue
         r = rng.uniform(1.5, 0.25 * min(nx, ny, nz) + 1.5)
         phi = np.minimum(phi, wl.sdf_sphere(x, y, z, c, r))
     return phi.astype(np.float32)
@@ -232,7 +236,10 @@ def test_apply_A_code_path_equals_weight_path(torch, api, shape):
 
 @pytest.mark.parametrize("shape,bt", [((32, 32, 32), (0,) * 6), ((24, 20, 16), (0, 1, 0, 0, 0, 0)),
                                        ((64, 64, 64), (1, 1, 0, 0, 0, 0)), ((128, 64, 32), (0,) * 6),
-                                       ((40, 36, 28), (0, 0, 1, 0, 0, 0))])
+                                       ((40, 36, 28), (0, 0, 1, 0, 0, 0)),
+                                       # 2-D mode (2 x 2 x 1 children): 4-cell bodies + cooperative kernel vs generic
+                                       ((256, 192, 1), (1, 1, 0, 0, 0, 0)), ((512, 256, 1), (0,) * 6),
+                                       ((136, 88, 1), (0, 1, 0, 0, 0, 0))])
 def test_vcycle_fused_equals_generic(torch, api, shape, bt):
     """The 4-launch-per-level V-cycle (k_down1/k_down2/k_up1/k_up2: red values recomputed on the fly, residual of
     the red children only, prolongation folded into the black half sweep) is the same operator, in exact
@@ -475,7 +482,8 @@ def test_host_buffer_entry_points_sync_and_async(torch, api):
     g.close()
 
 
-@pytest.mark.parametrize("shape,dirichlet", [((64, 48, 1), True), ((128, 96, 1), False), ((36, 20, 1), True)])
+@pytest.mark.parametrize("shape,dirichlet", [((64, 48, 1), True), ((128, 96, 1), False), ((36, 20, 1), True),
+                                             ((256, 192, 1), True)])
 def test_two_dimensional_mode(torch, api, shape, dirichlet):
     """NEXT-3: nz = 1 grids -- the hierarchy coarsens x and y only (2 x 2 x 1 children, restriction
     P^T / 4), so the paper's 2-D tasks get multigrid convergence.  Projection + adjoint against the oracle."""
