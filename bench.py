@@ -531,12 +531,18 @@ def run_geometry(args):
     pairs = float((n + 1) ** 3) * N * M
     mhz = ck.get("sm_mhz") or 1900.0
     peak = 148 * 128 * mhz * 1e6 / 19.25
+    traffic = None
+    try:
+        with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r1_geom_traffic.json")) as f:
+            traffic = float(json.load(f)["k_geom_sdf"]["traffic"])
+    except Exception:
+        pass
     print(json.dumps({"workload": "NEXT-2 parametric geometry, %d^3 grid, 4 primitives x (K=4, N=8, M=16)" % n,
                       "dtype": "f32", "ms": out, "clocks": ck,
                       "roofline": {"kernel": "k_geom_sdf", "bound": "alu", "achieved": round(pairs / (ms * 1e-3) / 1e9, 1),
                                    "peak": round(peak / 1e9, 1), "unit": "G(node,edge)/s",
                                    "frac": round(pairs / (ms * 1e-3) / peak, 3), "ms_per_launch": round(ms, 4),
-                                   "traffic": None}}))
+                                   "traffic": traffic}}))
 
 
 def run_envs(args):

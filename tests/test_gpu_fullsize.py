@@ -170,3 +170,61 @@ def test_pressure_solve_sweep_residual(torch, api, n):
     res[active] -= res[active].mean()
     g.close()
     assert np.linalg.norm(res) <= 5e-6 * np.linalg.norm(rhs)
+
+
+def test_parametric_geometry_full_size(torch, api):
+    """NEXT-2 at 256^3 in bench.py --geometry's configuration (K = 4, N = 8, M = 16): phi on sampled planes against the
+    geometry oracle (2e-6), the union of two primitives on the same planes (bit-exact CSG of the device's operands),
+    dJ/dparams for an upstream gradient confined to three planes (the oracle skips the empty ones), and the solid
+    velocity with a band on one plane of each face family."""
+    from oracle import nf_geom_oracle as G
+    K, Nc, M = 4, 8, 16
+    dx = float(np.float32(1.0 / N))
+    g = api.Grid(N, N, N, dx)
+    pA = wl.geom_random_params(40, K, Nc, 0.15, 0.6, (0.35, 0.35), 0.17)
+    pB = wl.geom_random_params(41, K, Nc, 0.2, 0.68, (0.65, 0.35), 0.17)
+    a = torch.empty(g.shape_sdf, dtype=torch.float32, device="cuda")
+    b = torch.empty_like(a)
+    g.geom_sdf(pA, K, Nc, M, a)
+    g.geom_sdf(pB, K, Nc, M, b)
+    u = torch.empty_like(a)
+    g.geom_csg("union", a, b, u)
+    planes = [0, 38, 39, 100, 153, 154, 256]      # outside the slab, at both caps, inside
+    X, Y = np.meshgrid(np.arange(N + 1) * dx, np.arange(N + 1) * dx, indexing="xy")
+    pa64 = pA.astype(np.float64)
+    for k in planes:
+        z = k * dx
+        c, r1, r2 = G.section_at(pa64, K, Nc, z)[:3]
+        ref = np.maximum(G.sdf2d(c, r1, r2, M, X, Y), max(pa64[0] - z, z - pa64[1]))
+        assert np.max(np.abs(a[k].cpu().numpy() - ref)) < 2e-6, k
+        assert np.array_equal(u[k].cpu().numpy(), np.minimum(a[k].cpu().numpy(), b[k].cpu().numpy()))
+    # reverse: upstream gradient on three planes, next to the surface only
+    rng = np.random.default_rng(3)
+    gphi = np.zeros((N + 1, N + 1, N + 1), dtype=np.float32)
+    for k in (45, 100, 152):
+        near = np.abs(a[k].cpu().numpy()) < 2 * dx
+        gphi[k] = np.where(near, rng.standard_normal((N + 1, N + 1)), 0.0)
+    got = g.geom_sdf_adjoint(pA, K, Nc, M, torch.from_numpy(gphi).cuda())
+    ref = G.sdf_nodes_adjoint(pa64, K, Nc, M, N, N, N, dx, gphi.astype(np.float64))
+    assert np.max(np.abs(ref)) > 0
+    assert np.max(np.abs(got - ref)) < 2e-4 * np.max(np.abs(ref))
+    # velocity with a band: one plane of the u family and of the w family
+    pd = wl.geom_random_rates(3, K, Nc, 0.1)
+    band = 3.0 * dx
+    U = [torch.full(s, 7.0, dtype=torch.float32, device="cuda") for s in (g.shape_u, g.shape_v, g.shape_w)]
+    g.geom_velocity(pA, pd, K, Nc, M, *U, band=band)
+    k = 100
+    Xu, Yu = np.meshgrid(np.arange(N + 1) * dx, (np.arange(N) + 0.5) * dx, indexing="xy")
+    ru = G._velocity_points(pa64, pd.astype(np.float64), K, Nc, M, Xu, Yu, (k + 0.5) * dx)
+    gotu = U[0][k].cpu().numpy()
+    sure_in, sure_out = ru[3] < band - 1e-5, ru[3] > band + 1e-5
+    assert np.all(gotu[sure_out] == 7.0) and sure_in.sum() > 100
+    ok = np.abs(gotu - ru[0])[sure_in & (np.abs(ru[3]) > 1e-3)] < 1e-4 * np.max(np.abs(ru[0]))
+    assert ok.mean() > 0.999
+    Xc, Yc = np.meshgrid((np.arange(N) + 0.5) * dx, (np.arange(N) + 0.5) * dx, indexing="xy")
+    kcap = 154   # just above z1 = 0.6 (153.6 dx): inside the outline the cap's velocity z1dot
+    rw = G._velocity_points(pa64, pd.astype(np.float64), K, Nc, M, Xc, Yc, kcap * dx)
+    gotw = U[2][kcap].cpu().numpy()
+    sure_in = rw[3] < band - 1e-5
+    assert np.max(np.abs(gotw - rw[2])[sure_in]) < 1e-6 and np.any(rw[2][sure_in] != 0)
+    g.close()
