@@ -46,6 +46,9 @@ def test_null_handle_is_rejected_without_a_gpu(lib_path):
     assert lib.nf_set_dt_rho(None, 1.0) == api.NF_ERR_INVALID
     assert lib.nf_project(None, None, None, None, None, 1e-6, 10) == api.NF_ERR_INVALID
     assert lib.nf_launch_count(None) == 0
+    assert lib.nf_geom_sdf(None, None, 1, 4, 8, 0, None) == api.NF_ERR_INVALID
+    assert lib.nf_geom_csg(None, 0, None, None, None) == api.NF_ERR_INVALID
+    assert lib.nf_geom_velocity_adjoint(None, None, 1, 4, 8, 1.0, None, None, None, None) == api.NF_ERR_INVALID
 
 
 def test_no_cpu_fallback_in_binding():
