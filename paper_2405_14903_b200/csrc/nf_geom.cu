@@ -39,10 +39,11 @@ struct NfGeomSm {
   float *V, *Vd, *gV;         // 2 per vertex: position, velocity, gradient
   float *ctrl;                // 8 per curve: gradient w.r.t. e0, p0, p1, e1
   float *gsl;                 // [2]: gradient w.r.t. the caps; [2] = "any point of the CTA carried a gradient"
+  int *bb;                    // [4]: bounding box of the polygon as order-preserving ints (velocity kernels' band cull)
 };
 static size_t nf_geom_smem_bytes(int N, int M) {
   const size_t W = 2 + 2 * (size_t)N, NM = (size_t)N * M;
-  return (3 * W + 16 * (size_t)N) * sizeof(double) + (6 * NM + 3 * 2 * NM + 8 * (size_t)N + 4) * sizeof(float);
+  return (3 * W + 16 * (size_t)N) * sizeof(double) + (6 * NM + 3 * 2 * NM + 8 * (size_t)N + 8) * sizeof(float);
 }
 __device__ __forceinline__ NfGeomSm nf_geom_carve(unsigned char *raw, int N, int M) {
   const int W = 2 + 2 * N, NM = N * M;
@@ -57,6 +58,7 @@ __device__ __forceinline__ NfGeomSm nf_geom_carve(unsigned char *raw, int N, int
   s.gV = s.Vd + 2 * NM;
   s.ctrl = s.gV + 2 * NM;
   s.gsl = s.ctrl + 8 * N;
+  s.bb = reinterpret_cast<int *>(s.gsl + 4);
   return s;
 }
 
@@ -365,6 +367,13 @@ __global__ void __launch_bounds__(NF_GEOM_NT) k_geom_sdf_adjoint(NfGeomK G, int 
 // ------------------------------------------------------------------------------------------------------------
 // U_s on the faces of family C (R30): the closest surface point's velocity along the in-plane normal, caps move in z
 // ------------------------------------------------------------------------------------------------------------
+// order-preserving float <-> int (for shared-memory atomicMin / atomicMax on coordinates)
+__device__ __forceinline__ int nf_f2o(float f) {
+  const int i = __float_as_int(f);
+  return i ^ ((i >> 31) & 0x7fffffff);
+}
+__device__ __forceinline__ float nf_o2f(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
+
 template <int C, bool ADJ>
 __global__ void __launch_bounds__(NF_GEOM_NT) k_geom_velocity(NfGeomK G, int nxf, int nyf, float band,
                                                               float *__restrict__ out, const float *__restrict__ gin,
@@ -373,15 +382,31 @@ __global__ void __launch_bounds__(NF_GEOM_NT) k_geom_velocity(NfGeomK G, int nxf
   const NfGeomSm S = nf_geom_carve(nf_geom_raw, G.N, G.M);
   const double z = (C == 2) ? (double)blockIdx.z * (double)G.dx : ((double)blockIdx.z + 0.5) * (double)G.dx;
   const NfGeomPlane P = nf_geom_plane(G, z);
+  // Band cull (exact): d = max(d2, slab) >= slab, and d2 >= the distance to the polygon's bounding box; a plane
+  // farther than the band from the slab, or a point farther than the band from the box, is not written.
+  if (P.slab > band) return;  // (uniform over the CTA; nothing of this plane is within the band)
   nf_geom_setup(G, P, S, ADJ);
   const int NM = G.N * G.M;
-  const NfGeomPts pt = nf_geom_points(nxf, nyf);
+  if (threadIdx.x < 4) S.bb[threadIdx.x] = (threadIdx.x & 1) ? nf_f2o(-INFINITY) : nf_f2o(INFINITY);
+  __syncthreads();
+  for (int v = threadIdx.x; v < NM; v += blockDim.x) {
+    atomicMin(&S.bb[0], nf_f2o(S.V[2 * v]));
+    atomicMax(&S.bb[1], nf_f2o(S.V[2 * v]));
+    atomicMin(&S.bb[2], nf_f2o(S.V[2 * v + 1]));
+    atomicMax(&S.bb[3], nf_f2o(S.V[2 * v + 1]));
+  }
+  __syncthreads();
+  const float bx0 = nf_o2f(S.bb[0]) - band, bx1 = nf_o2f(S.bb[1]) + band;
+  const float by0 = nf_o2f(S.bb[2]) - band, by1 = nf_o2f(S.bb[3]) + band;
+  NfGeomPts pt = nf_geom_points(nxf, nyf);
   float X[NF_GEOM_PPT], Y[NF_GEOM_PPT], g[NF_GEOM_PPT];
   bool work = false;
 #pragma unroll
   for (int q = 0; q < NF_GEOM_PPT; ++q) {
     X[q] = (C == 0) ? (float)pt.i[q] * G.dx : ((float)pt.i[q] + 0.5f) * G.dx;
     Y[q] = (C == 1) ? (float)pt.j[q] * G.dx : ((float)pt.j[q] + 0.5f) * G.dx;
+    // (written with negations so that band = +inf, where the box is (-inf, +inf), keeps every point)
+    pt.ok[q] = pt.ok[q] && !(X[q] < bx0) && !(X[q] > bx1) && !(Y[q] < by0) && !(Y[q] > by1);
     g[q] = (ADJ && pt.ok[q]) ? gin[((size_t)blockIdx.z * nyf + pt.j[q]) * nxf + pt.i[q]] : 0.0f;
     work = work || (ADJ ? g[q] != 0.0f : pt.ok[q]);
   }

@@ -6,7 +6,7 @@ coordinates to fp32 and scans in fp32, so phi carries a few ulp of 1: atol 2e-6.
 with it U_s and the gradients lose relative accuracy like eps / |d| next to the surface: velocities are compared at
 1e-4 relative to max|U_s| where |d| > 1e-3 and at 2e-2 elsewhere.  Where two edges are equidistant (the medial axis)
 the closest edge, hence the normal, is not unique and fp32 may break the tie the other way: up to 0.1 % of the faces
-may disagree (phi itself is continuous there and is compared everywhere)."""
+may disagree, at least 4 on a small grid (phi itself is continuous there and is compared everywhere)."""
 import numpy as np
 import pytest
 
@@ -135,7 +135,7 @@ def test_velocity_matches_oracle(torch, api, name):
         d = face_distance(p64, K, N, M, nx, ny, nz, dx, comp)
         err = np.abs(got - ref[comp])
         bad = np.where(np.abs(d) > 1e-3, err > 1e-4 * scale, err > 2e-2 * scale)
-        assert np.count_nonzero(bad) <= 1e-3 * bad.size, (comp, np.count_nonzero(bad), bad.size)
+        assert np.count_nonzero(bad) <= max(4, 1e-3 * bad.size), (comp, np.count_nonzero(bad), bad.size)
     # band: faces farther than the band keep their value; the others are as before
     band = 2.5 * dx
     keep = [torch.full(s, 7.0, dtype=torch.float32, device="cuda") for s in (g.shape_u, g.shape_v, g.shape_w)]
