@@ -26,6 +26,10 @@
  * polls a mapped status word; it never calls cudaDeviceSynchronize); results are ordered on the stream.
  * Every other call only enqueues work.  There is NO CPU fallback: every step runs in CUDA kernels.
  *
+ * Threads: a handle is used by one host thread at a time; different handles are independent (no shared mutable
+ * state in the library), so several small grids can be driven concurrently, one handle + stream + thread each
+ * (paper_2405_14903_b200/envs.py; the cooperative coarse kernel is sized for its level so that they overlap).
+ *
  * Errors: functions return an int status.  Negative = error, nothing useful written; NF_NOT_CONVERGED = the
  * best iterate was written but maxit was hit.  No exceptions, no exit(), no stdout.
  */
