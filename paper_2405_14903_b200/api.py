@@ -89,6 +89,28 @@ class NfError(RuntimeError):
     pass
 
 
+class NfNotConvergedWarning(RuntimeWarning):
+    """A solve hit maxit: the best iterate was written (NF_NOT_CONVERGED), the caller's tolerance was not met."""
+
+
+def _bound(fn):
+    """Hot-path methods run on the torch stream that is current when they are called (the handle is re-bound if it
+    changed since the last call) and with the handle's device current, so that the library's kernels are ordered with
+    the caller's torch ops on the same stream."""
+    import functools
+
+    @functools.wraps(fn)
+    def wrapper(self, *a, **k):
+        import torch
+        if torch.cuda.current_device() != self.device.index:
+            with torch.cuda.device(self.device):
+                self._bind_stream()
+                return fn(self, *a, **k)
+        self._bind_stream()
+        return fn(self, *a, **k)
+    return wrapper
+
+
 def _ptr(t):
     """Device (or host) address of a contiguous float32 torch tensor; None -> NULL."""
     if t is None:
@@ -118,7 +140,9 @@ class Grid:
         if rc != NF_OK:
             raise NfError("nf_grid_create failed with %d" % rc)
         self.h = h
-        self.set_stream(torch.cuda.current_stream(self.device))
+        self._stream = None
+        self.warn_not_converged = True
+        self._bind_stream()
 
     # -- shapes -------------------------------------------------------------------------------------------
     @property
@@ -141,7 +165,18 @@ class Grid:
     def shape_sdf(self):
         return (self.nz + 1, self.ny + 1, self.nx + 1)
 
+    def _bind_stream(self):
+        import torch
+        s = torch.cuda.current_stream(self.device).cuda_stream
+        if s != self._stream:
+            self._check(self.lib.nf_set_stream(self.h, ctypes.c_void_p(s)), "nf_set_stream")
+            self._stream = s
+
     def _check(self, rc, name, allow_not_converged=True):
+        if rc == NF_NOT_CONVERGED and allow_not_converged and self.warn_not_converged:
+            import warnings
+            warnings.warn("%s: the solve stopped at maxit without reaching the tolerance (NF_NOT_CONVERGED); the "
+                          "result is the best iterate" % name, NfNotConvergedWarning, stacklevel=3)
         if rc == NF_OK or (allow_not_converged and rc == NF_NOT_CONVERGED):
             return rc
         msg = self.lib.nf_last_error(self.h)
@@ -170,8 +205,11 @@ class Grid:
 
     # -- configuration ------------------------------------------------------------------------------------
     def set_stream(self, stream):
+        """Bind the handle to `stream` now (every hot-path call re-binds to the torch stream current at that call)."""
         self._check(self.lib.nf_set_stream(self.h, ctypes.c_void_p(stream.cuda_stream)), "nf_set_stream")
+        self._stream = stream.cuda_stream
 
+    @_bound
     def set_dt_rho(self, dt_over_rho):
         self._check(self.lib.nf_set_dt_rho(self.h, float(dt_over_rho)), "nf_set_dt_rho")
 
@@ -181,15 +219,18 @@ class Grid:
     def set_solver_options(self, nu_pre=1, nu_post=1, flags=0):
         self._check(self.lib.nf_set_solver_options(self.h, nu_pre, nu_post, flags), "nf_set_solver_options")
 
+    @_bound
     def set_solid(self, sdf, us=None, vs=None, ws=None):
         self._expect(sdf, self.shape_sdf, "sdf")
         self._expect(us, self.shape_u, "us"); self._expect(vs, self.shape_v, "vs"); self._expect(ws, self.shape_w, "ws")
         self._check(self.lib.nf_set_solid(self.h, _ptr(sdf), _ptr(us), _ptr(vs), _ptr(ws)), "nf_set_solid")
 
+    @_bound
     def set_weights(self, au, av, aw):
         self._expect(au, self.shape_u, "au"); self._expect(av, self.shape_v, "av"); self._expect(aw, self.shape_w, "aw")
         self._check(self.lib.nf_set_weights(self.h, _ptr(au), _ptr(av), _ptr(aw)), "nf_set_weights")
 
+    @_bound
     def get_weights(self):
         import torch
         au = torch.empty(self.shape_u, dtype=torch.float32, device=self.device)
@@ -198,21 +239,25 @@ class Grid:
         self._check(self.lib.nf_get_weights(self.h, _ptr(au), _ptr(av), _ptr(aw)), "nf_get_weights")
         return au, av, aw
 
+    @_bound
     def set_solid_velocity(self, us=None, vs=None, ws=None):
         self._expect(us, self.shape_u, "us"); self._expect(vs, self.shape_v, "vs"); self._expect(ws, self.shape_w, "ws")
         self._check(self.lib.nf_set_solid_velocity(self.h, _ptr(us), _ptr(vs), _ptr(ws)), "nf_set_solid_velocity")
 
     # -- hot path -----------------------------------------------------------------------------------------
+    @_bound
     def solve(self, rhs, p, tol=1e-6, maxit=200):
         self._expect(rhs, self.shape_p, "rhs"); self._expect(p, self.shape_p, "p")
         return self._check(self.lib.nf_solve(self.h, _ptr(rhs), _ptr(p), float(tol), int(maxit)), "nf_solve")
 
+    @_bound
     def project(self, u, v, w, p, tol=1e-6, maxit=200):
         self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
         self._expect(p, self.shape_p, "p")
         return self._check(self.lib.nf_project(self.h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), float(tol), int(maxit)),
                            "nf_project")
 
+    @_bound
     def project_adjoint(self, gu, gv, gw, p_saved=None, uhat=None, galpha=None, gus=None, y_out=None, tol=1e-6,
                         maxit=200):
         self._expect(gu, self.shape_u, "gu"); self._expect(gv, self.shape_v, "gv"); self._expect(gw, self.shape_w, "gw")
@@ -228,10 +273,12 @@ class Grid:
                                          _ptr(gs[2]), _ptr(y_out), float(tol), int(maxit))
         return self._check(rc, "nf_project_adjoint")
 
+    @_bound
     def advect(self, u, v, w, dt):
         self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
         self._check(self.lib.nf_advect(self.h, _ptr(u), _ptr(v), _ptr(w), float(dt)), "nf_advect")
 
+    @_bound
     def max_speed(self, u, v, w):
         """max over all faces of |u|, |v|, |w| (synchronises)."""
         self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
@@ -239,6 +286,7 @@ class Grid:
         self._check(self.lib.nf_max_speed(self.h, _ptr(u), _ptr(v), _ptr(w), ctypes.byref(out)), "nf_max_speed")
         return out.value
 
+    @_bound
     def viscosity(self, u, v, w, nu, dt):
         """Explicit viscosity step, in place; symmetric, so the backward pass calls it on the gradient (Eq. 8)."""
         self._expect(u, self.shape_u, "u"); self._expect(v, self.shape_v, "v"); self._expect(w, self.shape_w, "w")
@@ -256,12 +304,14 @@ class Grid:
             raise ValueError("%s: expected %d values" % (name, self.geom_n_params(K, N)))
         return a, a.ctypes.data_as(_c_host_float_p)
 
+    @_bound
     def geom_sdf(self, params, K, N, M, sdf, complement=False):
         self._expect(sdf, self.shape_sdf, "sdf")
         _keep, pp = self._geom_vec(params, K, N, "params")
         self._check(self.lib.nf_geom_sdf(self.h, pp, int(K), int(N), int(M), 1 if complement else 0, _ptr(sdf)),
                     "nf_geom_sdf")
 
+    @_bound
     def geom_sdf_adjoint(self, params, K, N, M, gsdf, complement=False):
         """-> NumPy float64 vector dJ/dparams (synchronises)."""
         import numpy as np
@@ -272,18 +322,21 @@ class Grid:
                                                  out.ctypes.data_as(_c_host_double_p)), "nf_geom_sdf_adjoint")
         return out
 
+    @_bound
     def geom_csg(self, op, a, b, out):
         for t, n in ((a, "a"), (b, "b"), (out, "out")):
             self._expect(t, self.shape_sdf, n)
         self._check(self.lib.nf_geom_csg(self.h, {"union": 0, "intersection": 1}[op], _ptr(a), _ptr(b), _ptr(out)),
                     "nf_geom_csg")
 
+    @_bound
     def geom_csg_adjoint(self, op, a, b, gout, ga, gb):
         for t, n in ((a, "a"), (b, "b"), (gout, "gout"), (ga, "ga"), (gb, "gb")):
             self._expect(t, self.shape_sdf, n)
         self._check(self.lib.nf_geom_csg_adjoint(self.h, {"union": 0, "intersection": 1}[op], _ptr(a), _ptr(b),
                                                  _ptr(gout), _ptr(ga), _ptr(gb)), "nf_geom_csg_adjoint")
 
+    @_bound
     def geom_velocity(self, params, pdot, K, N, M, us, vs, ws, band=float("inf")):
         for t, s, n in ((us, self.shape_u, "us"), (vs, self.shape_v, "vs"), (ws, self.shape_w, "ws")):
             if t is not None:
@@ -293,6 +346,7 @@ class Grid:
         self._check(self.lib.nf_geom_velocity(self.h, pp, pd, int(K), int(N), int(M), float(band), _ptr(us), _ptr(vs),
                                               _ptr(ws)), "nf_geom_velocity")
 
+    @_bound
     def geom_velocity_adjoint(self, params, K, N, M, gus, gvs, gws, band=float("inf")):
         """-> NumPy float64 vector dJ/dpdot (synchronises)."""
         import numpy as np
@@ -306,6 +360,7 @@ class Grid:
                     "nf_geom_velocity_adjoint")
         return out
 
+    @_bound
     def advect_adjoint(self, u0, v0, w0, gu, gv, gw, dt):
         for t, s, n in ((u0, self.shape_u, "u0"), (v0, self.shape_v, "v0"), (w0, self.shape_w, "w0"),
                         (gu, self.shape_u, "gu"), (gv, self.shape_v, "gv"), (gw, self.shape_w, "gw")):
@@ -313,27 +368,32 @@ class Grid:
         self._check(self.lib.nf_advect_adjoint(self.h, _ptr(u0), _ptr(v0), _ptr(w0), _ptr(gu), _ptr(gv), _ptr(gw),
                                                float(dt)), "nf_advect_adjoint")
 
+    @_bound
     def weights_adjoint(self, gau, gav, gaw, gsdf):
         self._expect(gau, self.shape_u, "gau"); self._expect(gav, self.shape_v, "gav")
         self._expect(gaw, self.shape_w, "gaw"); self._expect(gsdf, self.shape_sdf, "gsdf")
         self._check(self.lib.nf_weights_adjoint(self.h, _ptr(gau), _ptr(gav), _ptr(gaw), _ptr(gsdf)),
                     "nf_weights_adjoint")
 
+    @_bound
     def apply_A(self, p, q):
         self._expect(p, self.shape_p, "p"); self._expect(q, self.shape_p, "q")
         self._check(self.lib.nf_apply_A(self.h, _ptr(p), _ptr(q)), "nf_apply_A")
 
+    @_bound
     def vcycle(self, r, z):
         self._expect(r, self.shape_p, "r"); self._expect(z, self.shape_p, "z")
         self._check(self.lib.nf_vcycle(self.h, _ptr(r), _ptr(z)), "nf_vcycle")
 
     # -- host-buffer variants (e2e timing) ------------------------------------------------------------------
+    @_bound
     def project_host(self, u, v, w, p, tol=1e-6, maxit=200):
         self._expect(u, self.shape_u, "u", host=True); self._expect(v, self.shape_v, "v", host=True)
         self._expect(w, self.shape_w, "w", host=True); self._expect(p, self.shape_p, "p", host=True)
         return self._check(self.lib.nf_project_host(self.h, _ptr(u), _ptr(v), _ptr(w), _ptr(p), float(tol),
                                                     int(maxit)), "nf_project_host")
 
+    @_bound
     def project_adjoint_host(self, gu, gv, gw, tol=1e-6, maxit=200):
         self._expect(gu, self.shape_u, "gu", host=True); self._expect(gv, self.shape_v, "gv", host=True)
         self._expect(gw, self.shape_w, "gw", host=True)

@@ -56,7 +56,7 @@ class _Project(torch.autograd.Function):
         grid.set_solid(phi_c, *solid)
         uhat = [a.detach().contiguous() for a in (u, v, w)]
         out = [a.clone() for a in uhat]
-        p = torch.empty(grid.shape_p, dtype=torch.float32, device=out[0].device)
+        p = torch.zeros(grid.shape_p, dtype=torch.float32, device=out[0].device)  # (a valid guess under warm start)
         grid.project(*out, p, tol=ctx.tol, maxit=ctx.maxit)
         ctx.has_us = [a is not None for a in solid]
         ctx.save_for_backward(p, phi_c, *uhat, *[a for a in solid if a is not None])

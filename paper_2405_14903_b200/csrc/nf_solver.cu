@@ -9,7 +9,7 @@
 
 #define NF_VEC_BLOCKS (148 * 8)
 #define NF_LOOKAHEAD 2
-#define NF_REFRESH_FACTOR 30.0f  // phase 1 of a solve stops at 30 tol; then r = b - A x afresh (k_phase_begin)  // phase 1 of a solve stops here; then r = b - A x afresh (k_phase_begin)
+#define NF_REFRESH_FACTOR 30.0f  // phase 1 of a solve stops at 30 tol; then r = b - A x afresh (k_phase_begin)
 
 // ------------------------------------------------------------------------------------------------------------
 // a-3  q = A p = c (sum_f alpha_f (p - p_nb)), fused p.q partial sums
@@ -478,14 +478,15 @@ __global__ void __launch_bounds__(256, 4) k_true_residual4(NfLvK L, float *__res
   nf_block_atomic_add(part, &st->rr[0]);
 }
 // warm start: the initial guess on the active cells only (0 elsewhere), and 0 everywhere when b = 0 (done is then
-// already set by k_start_state: the answer is x = 0)
+// already set by k_start_state: the answer is x = 0).  NaN, inf and absurdly large entries (an uninitialised array
+// passed as the guess) count as "no guess": the fp32 residual of a 1e30 pressure could never reach the tolerance.
 __global__ void __launch_bounds__(256) k_warm_mask(float *__restrict__ x, const uint8_t *__restrict__ code, size_t n,
                                                    const NfSolveState *st) {
   const bool zero = st->done != 0;
   const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
   for (size_t t = tid; t < n; t += nth) {
     const float v = x[t];
-    x[t] = (zero || code[t] == 0 || !(v == v)) ? 0.0f : v;
+    x[t] = (zero || code[t] == 0 || !(fabsf(v) < 1e18f)) ? 0.0f : v;
   }
 }
 // x += e

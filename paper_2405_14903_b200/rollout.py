@@ -22,7 +22,7 @@ def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect
         phi, us, dphi, dus = solid_fn(n)
         g.set_solid(phi, *us)
         Uhat = [a.clone() for a in U]
-        p = torch.empty(g.shape_p, dtype=torch.float32, device=U[0].device)
+        p = torch.zeros(g.shape_p, dtype=torch.float32, device=U[0].device)  # (zeros: a valid guess under the warm-start option)
         g.project(*U, p, tol=tol, maxit=maxit)
         tape.append((Uprev, Uhat, p, phi, us, dphi, dus))
     J, G = loss_fn(U)
@@ -70,8 +70,15 @@ def rollout_parametric(grid, U0, prims_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=
     nf_geom_sdf_adjoint (dJ/dparams, through phi) and nf_geom_velocity_adjoint (dJ/dpdot).
     Returns (J, grads, dJ/dU0), grads[step-1][i] = (dJ/dparams, dJ/dpdot or None) as float64 NumPy vectors."""
     import numpy as np
+    import warnings
     g = grid
     dev = U0[0].device
+    if any(pd is not None for (_p, pd, _K, _N, _M) in prims_fn(1)):
+        # R31: U_s is differentiated w.r.t. pdot only.  For a primitive that moves, dJ/dparams below holds the part
+        # through phi (the shape at t^{n+1}) and NOT the part through U_s(params) (closest point and normal).
+        warnings.warn("rollout_parametric: dJ/dparams of a moving primitive (pdot given) omits d U_s / d params "
+                      "(DESIGN.md R31); dJ/dpdot and the gradients of static primitives are complete", RuntimeWarning,
+                      stacklevel=2)
     new_nodes = lambda: torch.empty(g.shape_sdf, dtype=torch.float32, device=dev)
     U = [a.clone() for a in U0]
     tape = []
@@ -99,7 +106,7 @@ def rollout_parametric(grid, U0, prims_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=
                 g.geom_velocity(p, pd, K, N, M, *us, band=band)
         g.set_solid(partial[-1], *(us if us is not None else (None, None, None)))
         Uhat = [a.clone() for a in U]
-        pr = torch.empty(g.shape_p, dtype=torch.float32, device=dev)
+        pr = torch.zeros(g.shape_p, dtype=torch.float32, device=dev)
         g.project(*U, pr, tol=tol, maxit=maxit)
         tape.append((Uprev, Uhat, pr, prims, phis, partial, us))
     J, G = loss_fn(U)

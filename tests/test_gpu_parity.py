@@ -237,6 +237,9 @@ def test_apply_A_code_path_equals_weight_path(torch, api, shape):
 @pytest.mark.parametrize("shape,bt", [((32, 32, 32), (0,) * 6), ((24, 20, 16), (0, 1, 0, 0, 0, 0)),
                                        ((64, 64, 64), (1, 1, 0, 0, 0, 0)), ((128, 64, 32), (0,) * 6),
                                        ((40, 36, 28), (0, 0, 1, 0, 0, 0)),
+                                       # >= 3 cooperative levels: k_vcoarse's packed per-cell phases (levels 2 .. tail-1)
+                                       ((96, 96, 96), (0, 1, 0, 0, 0, 0)), ((160, 160, 160), (1, 1, 0, 0, 0, 0)),
+                                       ((256, 256, 256), (0,) * 6),
                                        # 2-D mode (2 x 2 x 1 children): 4-cell bodies + cooperative kernel vs generic
                                        ((256, 192, 1), (1, 1, 0, 0, 0, 0)), ((512, 256, 1), (0,) * 6),
                                        ((136, 88, 1), (0, 1, 0, 0, 0, 0))])
@@ -259,6 +262,35 @@ def test_vcycle_fused_equals_generic(torch, api, shape, bt):
     assert rel(host(z1), host(z2)) < 2e-5
     assert float((z1 * (~act)).abs().max()) == 0.0  # inactive cells stay 0
     g.close()
+
+
+@pytest.mark.parametrize("shape,bt,seed", [((32, 32, 32), (0,) * 6, 9), ((64, 64, 64), (1, 1, 0, 0, 0, 0), 9),
+                                            ((40, 36, 28), (0, 0, 1, 0, 0, 0), 9), ((96, 96, 96), (0, 1, 0, 0, 0, 0), 9),
+                                            ((128, 128, 128), (1, 1, 0, 0, 0, 0), 9), ((128, 128, 128), (0,) * 6, 2)])
+def test_vcycle_matches_fp64_reference(torch, api, shape, bt, seed):
+    """The CUDA V-cycle (fused fine-level kernels, cooperative coarse kernel incl. its packed per-cell phases at
+    >= 96^3, shared-memory tail) against tests/vcycle_ref.py, the same documented preconditioner in NumPy fp64 on the
+    same fp32 hierarchy.  The fused path evaluates the restricted residual in the cancellation-free form
+    c sum alpha z_black (red children only); the generic one-colour-per-launch path evaluates r - A z, whose
+    rounding noise is amplified by weakly connected coarse cells (inverse diagonals up to 1e4-1e5): blob field 9 at
+    128^3 has such a cell on its top wall, and there the generic path is the inaccurate one (a few 1e-4), not the
+    fused one -- so the fused path is held to 2e-5 and the generic one to 2e-3."""
+    from vcycle_ref import vcycle as vc_ref
+    nx, ny, nz = shape
+    phi = blob_sdf(nx, ny, nz, seed)
+    g = make_grid(api, nx, ny, nz, 1.0 / nx, dt_over_rho=0.5, bc_types=bt)
+    g.set_solid(dev(torch, phi))
+    alpha = [a.cpu().numpy() for a in g.get_weights()]
+    act = orc.active_cells([a.astype(np.float64) for a in alpha])
+    r = (np.random.default_rng(4).standard_normal((nz, ny, nx)) * act).astype(np.float32)
+    ref = vc_ref(r, alpha, 0.5 * nx, bool(g.info()["singular"]))
+    z1, z2 = torch.empty(g.shape_p, device="cuda"), torch.empty(g.shape_p, device="cuda")
+    g.vcycle(dev(torch, r), z1)
+    g.set_solver_options(1, 1, 2)
+    g.vcycle(dev(torch, r), z2)
+    g.close()
+    assert rel(host(z1), ref) < 2e-5
+    assert rel(host(z2), ref) < 2e-3
 
 
 @pytest.mark.parametrize("shape", [(24, 20, 16), (64, 64, 64), (16, 16, 16)])

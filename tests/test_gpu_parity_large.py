@@ -1,0 +1,159 @@
+"""Oracle parity at the sizes the north_star names (BASELINE.json: "forward and adjoint pressure projection at 256^3
+matching the fp64 CPU oracle"), in the launch configuration bench.py times (nf_set_solid alone, fused kernels,
+cooperative coarse kernel with its packed per-cell phases: 96^3 and 128^3 have one such level, 256^3 two):
+
+  * 128^3 channel-gate: the oracle solves LIVE (Jacobi-PCG, fp64, 1e-10) and every array is compared element by element;
+  * 128^3 chamber-pump and 256^3 channel-gate: expected values sampled from an oracle-only solve, stored in
+    tests/golden/*_oracle_samples.txt by tests/golden/make_gate_golden.py (which imports oracle/ and the input
+    generators only) -- 2048 seeded entries per array plus the 2-norm of every full array.
+
+Tolerances (north_star): relative L2 1e-4 on p, U, y, dJ/dUhat; 1e-3 on dJ/dalpha, dJ/dU_s."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import nf_oracle as orc
+from paper_2405_14903_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+TOL_FIELD, TOL_GRAD = 1e-4, 1e-3
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available()
+    return t
+
+
+@pytest.fixture(scope="module")
+def api():
+    from paper_2405_14903_b200 import api as a
+    a.load_library()
+    return a
+
+
+def _case(config, n):
+    """The inputs of tests/golden/make_gate_golden.py (same seeds, same order of draws)."""
+    if config == "gate":
+        P = wl.config4_params(n)
+        U0 = wl.config4_initial_velocity(P)
+        phi, us = wl.config4_solid(P, 3)
+        rng = np.random.default_rng(77)
+    else:
+        P = wl.config3_params(n)
+        phi, us = wl.config3_solid(P, 12)
+        r0 = np.random.default_rng(1003)
+        U0 = [(0.05 * r0.standard_normal(s)).astype(np.float32) for s in wl.face_shapes(n, n, n)]
+        rng = np.random.default_rng(78)
+    g = [rng.standard_normal(a.shape).astype(np.float32) for a in U0]
+    return P, U0, phi, us, g
+
+
+def _gpu_projection(torch, api, P, U0, phi, us, gin):
+    """nf_set_solid -> nf_project -> nf_project_adjoint through the binding; returns host fp64 arrays."""
+    n = P["nx"]
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    g = api.Grid(n, n, n, P["dx"])
+    g.set_dt_rho(P["dt_over_rho"])
+    for f in range(6):
+        g.set_domain_bc(f, P["bc_types"][f], P["bc_values"][f])
+    g.set_solid(d(phi), *[d(a) for a in us])
+    U = [d(a) for a in U0]
+    p = torch.zeros(g.shape_p, dtype=torch.float32, device="cuda")
+    assert g.project(*U, p, tol=1e-6, maxit=400) == 0
+    it_f = g.last_solve_info()["iters"]
+    G = [d(a) for a in gin]
+    ga = [torch.empty_like(a) for a in G]
+    gs = [torch.empty_like(a) for a in G]
+    y = torch.zeros_like(p)
+    assert g.project_adjoint(*G, p_saved=p, uhat=[d(a) for a in U0], galpha=ga, gus=gs, y_out=y, tol=1e-6,
+                             maxit=400) == 0
+    it_a = g.last_solve_info()["iters"]
+    h = lambda t: t.cpu().numpy().astype(np.float64)
+    out = dict(p=h(p), u=h(U[0]), v=h(U[1]), w=h(U[2]), y=h(y), guhat_u=h(G[0]), guhat_v=h(G[1]), guhat_w=h(G[2]),
+               galpha_u=h(ga[0]), galpha_v=h(ga[1]), galpha_w=h(ga[2]), gus_u=h(gs[0]), gus_v=h(gs[1]), gus_w=h(gs[2]),
+               iters=(it_f, it_a), levels=g.info()["levels"])
+    g.close()
+    return out
+
+
+def _rel(groups_got, groups_ref):
+    num = np.sqrt(sum(np.sum((a - b) ** 2) for a, b in zip(groups_got, groups_ref)))
+    den = np.sqrt(sum(np.sum(b ** 2) for b in groups_ref))
+    return num / den
+
+
+def test_gate_128_matches_live_oracle(torch, api):
+    """Channel-gate shape at 128^3 (three cooperative levels: 64^3 vec, 32^3 packed per-cell phases, tail): forward and
+    adjoint projection, every output element by element against a live oracle solve."""
+    n = 128
+    P, U0, phi, us, gin = _case("gate", n)
+    got = _gpu_projection(torch, api, P, U0, phi, us, gin)
+    bc = orc.BC(P["bc_types"], P["bc_values"])
+    alpha = orc.face_weights(phi, bc)
+    Uo, po = orc.project(U0, alpha, us, P["dx"], P["dt_over_rho"], bc, tol=1e-10)
+    gU, gA, gS, yo = orc.project_adjoint(gin, alpha, po, U0, us, P["dx"], P["dt_over_rho"], bc, tol=1e-10)
+    assert _rel([got["p"]], [po]) <= TOL_FIELD
+    assert _rel([got["u"], got["v"], got["w"]], Uo) <= TOL_FIELD
+    assert _rel([got["y"]], [yo]) <= TOL_FIELD
+    assert _rel([got["guhat_u"], got["guhat_v"], got["guhat_w"]], gU) <= TOL_FIELD
+    assert _rel([got["galpha_u"], got["galpha_v"], got["galpha_w"]], gA) <= TOL_GRAD
+    assert _rel([got["gus_u"], got["gus_v"], got["gus_w"]], gS) <= TOL_GRAD
+    assert max(got["iters"]) <= 60, got["iters"]
+
+
+def _load_golden(name):
+    meta, norms, arrays = {}, {}, {}
+    cur = None
+    with open(os.path.join(GOLD, name)) as f:
+        for ln in f:
+            if ln.startswith("#") or not ln.strip():
+                continue
+            t = ln.split()
+            if t[0] == "meta":
+                meta = {t[i]: float(t[i + 1]) for i in range(1, len(t), 2)}
+            elif t[0] == "norm":
+                norms[t[1]] = float(t[2])
+            elif t[0] == "array":
+                cur = ([], [])
+                arrays[t[1]] = cur
+            else:
+                cur[0].append(int(t[0]))
+                cur[1].append(float(t[1]))
+    return meta, norms, {k: (np.array(i, dtype=np.int64), np.array(v)) for k, (i, v) in arrays.items()}
+
+
+@pytest.mark.parametrize("config,n", [("chamber", 128), ("gate", 256)])
+def test_projection_matches_oracle_golden_samples(torch, api, config, n):
+    """The library's forward + adjoint projection at full size against values the oracle computed alone
+    (tests/golden/make_gate_golden.py): 2048 sampled entries per array and the 2-norm of every full array."""
+    meta, norms, arrs = _load_golden("%s%d_oracle_samples.txt" % (config, n))
+    assert int(meta["n"]) == n and meta["tol"] <= 1e-9
+    P, U0, phi, us, gin = _case(config, n)
+    got = _gpu_projection(torch, api, P, U0, phi, us, gin)
+
+    def samp(names):
+        return [got[k].ravel()[arrs[k][0]] for k in names], [arrs[k][1] for k in names]
+
+    # sampled entries, scaled by the rms of the full reference array (so a sparse array's samples are judged fairly)
+    def rel_samples(names):
+        a, b = samp(names)
+        num = sum(np.sum((x - y) ** 2) / x.size for x, y in zip(a, b))
+        den = sum(norms[k] ** 2 / got[k].size for k in names)
+        return np.sqrt(num / den)
+
+    assert rel_samples(["p"]) <= TOL_FIELD
+    assert rel_samples(["u", "v", "w"]) <= TOL_FIELD
+    assert rel_samples(["y"]) <= TOL_FIELD
+    assert rel_samples(["guhat_u", "guhat_v", "guhat_w"]) <= TOL_FIELD
+    assert rel_samples(["galpha_u"]) <= TOL_GRAD
+    assert rel_samples(["gus_u"]) <= TOL_GRAD
+    # the 2-norms of the full arrays
+    for k, tol in (("p", TOL_FIELD), ("u", TOL_FIELD), ("v", TOL_FIELD), ("w", TOL_FIELD), ("y", TOL_FIELD),
+                   ("guhat_u", TOL_FIELD), ("guhat_v", TOL_FIELD), ("guhat_w", TOL_FIELD), ("galpha_u", TOL_GRAD),
+                   ("gus_u", TOL_GRAD)):
+        assert abs(np.linalg.norm(got[k]) - norms[k]) <= tol * norms[k], k
+    assert max(got["iters"]) <= 60, got["iters"]
