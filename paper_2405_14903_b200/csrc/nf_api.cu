@@ -23,7 +23,7 @@ static void free_all(nf_grid *g) {
     cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.code); cudaFree(L.idg); cudaFree(L.pk); cudaFree(L.z); cudaFree(L.r);
   }
   cudaFree(g->us); cudaFree(g->vs); cudaFree(g->ws); cudaFree(g->sdf);
-  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->b0); cudaFree(g->ecorr); cudaFree(g->r_alt); cudaFree(g->tailpack);
+  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->b0); cudaFree(g->ecorr); cudaFree(g->r_alt); cudaFree(g->tailpack); cudaFree(g->tailinv);
   cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
   cudaFree(g->st); cudaFree(g->d_counts); cudaFree(g->geom_par); cudaFree(g->geom_grad);
   if (g->hst) cudaFreeHost((void *)g->hst);
@@ -80,13 +80,16 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     // 2-D mode (nz == 1): x and y coarsen, z stays one layer
     const bool flat = nz == 1;
     L.fz = flat ? 1 : 2;
+    // extents stay >= 4 -- except that a level with more than 128 cells (too many for the direct coarsest solve of
+    // nf_mg.cu) is halved once more if it can be: 48^3 ends at 3^3 instead of 6^3, 256^3 at 4^3 as before
+    const int lim = L.ncell > 128 ? 2 : 4;
     if (flat) {
       if ((lx | ly) & 1) break;
-      if (lx / 2 < 4 || ly / 2 < 4) break;
+      if (lx / 2 < lim || ly / 2 < lim) break;
       lx /= 2; ly /= 2;
     } else {
       if ((lx | ly | lz) & 1) break;
-      if (lx / 2 < 4 || ly / 2 < 4 || lz / 2 < 4) break;
+      if (lx / 2 < lim || ly / 2 < lim || lz / 2 < lim) break;
       lx /= 2; ly /= 2; lz /= 2;
     }
     c *= 0.25f;
@@ -99,6 +102,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     size_t tc = 0;
     for (int l = g->tail; l < nl; ++l) tc += (size_t)g->lv[l].ncell;
     ok = ok && dalloc(&g->tailpack, 8 * tc) == cudaSuccess;
+    ok = ok && dalloc(&g->tailinv, 128 * 128 + 4) == cudaSuccess;
   }
   const size_t nc = nf_nc(g);
   ok = ok && dalloc(&g->us, nf_nu(g)) == cudaSuccess && dalloc(&g->vs, nf_nv(g)) == cudaSuccess &&

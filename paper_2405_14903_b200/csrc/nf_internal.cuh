@@ -121,6 +121,7 @@ struct nf_grid {
   float *b0;  // the prepared right-hand side (kept for the true-residual refresh, nf_solver.cu)
   float *p, *p2, *q, *xtmp;  // p / p2: the search direction ping-pongs between two buffers (k_papply4)
   float *tailpack;  // 8 floats per cell of the tail levels (nf_mg.cu)
+  float *tailinv;   // inverse of the coarsest level's operator (n <= 128 cells: n^2 floats; k_coarse_inverse)
   // scratch face arrays (advection copy / adjoint staging)
   float *fu, *fv, *fw;
   NfSolveState *st;      // device

@@ -22,7 +22,7 @@
 namespace cg = cooperative_groups;
 
 #define NF_VEC_BLOCKS (148 * 8)
-#define NF_TAIL_MAX_CELLS 5632  // 10 floats per cell of shared memory: 225,280 B <= 227 KB
+#define NF_TAIL_MAX_CELLS 2048  // largest level of the shared-memory tail: a 12^3 level is cheaper inside the one-CTA tail, a 16^3 level as four grid phases (measured)
 #define NF_TAIL_THREADS 1024
 
 // ------------------------------------------------------------------------------------------------------------
@@ -489,12 +489,23 @@ __global__ void __launch_bounds__(256) k_dot_rz(const float *__restrict__ a, con
 // ------------------------------------------------------------------------------------------------------------
 // Per level the hierarchy build packs (k_tail_pack): idg[n] = 1/(c diag) (0 inactive), wg[f][n] = c alpha_f with
 // faces towards the outside of the grid zeroed, col[n] = (i+j+k) & 1 as float.  8n floats per level.
+// The coarsest level (<= NF_DIRECT_MAX cells: the hierarchy halves down to extents of 2 or 3) is solved DIRECTLY with
+// the inverse of its operator, computed in fp64 when the weights change (k_coarse_inverse) -- one small matrix-vector
+// product instead of 2 x 8 symmetric Gauss-Seidel sweeps by one warp (measured: 6.8 us of a 20 us tail at 256^3, 9.8 us
+// of 15 us at 48^3, whose coarsest level was 6^3).
+#define NF_DIRECT_MAX 128
 struct NfTailK {
   int nlev, sweeps;
   int singular;  // the system has the constant null vector (R12): the coarsest solve works in its complement
+  int direct;    // 1: the coarsest level is solved with the precomputed inverse
   int n[NF_MAX_LEVELS], nx[NF_MAX_LEVELS], ny[NF_MAX_LEVELS], nz[NF_MAX_LEVELS];
-  int off[NF_MAX_LEVELS];  // offset (in cells) of the level in the packed arrays
-  int fz[NF_MAX_LEVELS];   // z-coarsening factor towards the next level (1 in 2-D mode)
+  int np[NF_MAX_LEVELS];    // n rounded up to a multiple of 4 (16-byte alignment of every block in shared memory)
+  int soff[NF_MAX_LEVELS];  // float offset of the level in shared memory: z[np], r[np], pack[8 n]
+  int goff[NF_MAX_LEVELS];  // float offset of the level's pack in the global pack array
+  int fz[NF_MAX_LEVELS];    // z-coarsening factor towards the next level (1 in 2-D mode)
+  int minv_soff;            // float offset of the coarsest inverse (n^2 floats, padded to a multiple of 4)
+  int scratch_soff;         // 1024 floats of scratch (partial sums of the matrix-vector product)
+  int total_floats;         // dynamic shared memory, in floats
 };
 
 __global__ void __launch_bounds__(256) k_tail_pack(const float *__restrict__ ax, const float *__restrict__ ay,
@@ -516,7 +527,77 @@ __global__ void __launch_bounds__(256) k_tail_pack(const float *__restrict__ ax,
   pack[7 * n + id] = (float)((i + j + k) & 1);
 }
 
-// smem per level (offset 10*off[l] floats): z[n], r[n], pack[8n]
+// Inverse of the coarsest operator A_c (n <= NF_DIRECT_MAX cells) from its pack, in fp64, by in-place Gauss-Jordan
+// elimination without pivoting (A_c is symmetric positive definite on the active cells; inactive cells are decoupled
+// identity rows whose rows / columns of the result are zeroed).  Singular system (R12, constant null vector on the
+// active cells): A_c + sigma u u^T with u = e / sqrt(#active) is inverted instead, and (1/sigma) u u^T subtracted
+// again, which leaves the pseudo-inverse.  One CTA; runs when the weights change (nf_build_hierarchy).
+__global__ void __launch_bounds__(1024) k_coarse_inverse(const float *__restrict__ pack, int n, int nx, int ny,
+                                                          const double *__restrict__ counts,
+                                                          float *__restrict__ minv) {
+  const bool singular = !(counts[1] > 0.0);  // no open face on a Dirichlet domain face (k_encode, level 0)
+  extern __shared__ double sa[];
+  double *a = sa, *rowk = sa + n * n, *colk = rowk + n;
+  __shared__ double s_sigma, s_pivot;
+  __shared__ int s_nact;
+  const int tid = threadIdx.x, nthr = blockDim.x;
+  const int off[6] = {-1, 1, -nx, nx, -nx * ny, nx * ny};
+  for (int e = tid; e < n * n; e += nthr) a[e] = 0.0;
+  __syncthreads();
+  for (int i = tid; i < n; i += nthr) {
+    const float idg = pack[i];
+    if (idg > 0.0f) {
+      a[i * n + i] = 1.0 / (double)idg;
+      for (int f = 0; f < 6; ++f) {
+        const float w = pack[(1 + f) * n + i];
+        if (w != 0.0f) a[i * n + i + off[f]] = -(double)w;
+      }
+    } else {
+      a[i * n + i] = 1.0;
+    }
+  }
+  if (tid == 0) {
+    int na = 0;
+    double sd = 0.0;
+    for (int i = 0; i < n; ++i)
+      if (pack[i] > 0.0f) { na += 1; sd += 1.0 / (double)pack[i]; }
+    s_nact = na;
+    s_sigma = na > 0 ? sd / na : 1.0;
+  }
+  __syncthreads();
+  const double shift = (singular && s_nact > 0) ? s_sigma / s_nact : 0.0;
+  if (shift != 0.0) {
+    for (int e = tid; e < n * n; e += nthr) {
+      const int i = e / n, j = e - i * n;
+      if (pack[i] > 0.0f && pack[j] > 0.0f) a[e] += shift;
+    }
+    __syncthreads();
+  }
+  for (int k = 0; k < n; ++k) {
+    if (tid == 0) s_pivot = a[k * n + k];
+    __syncthreads();
+    const double ip = 1.0 / s_pivot;
+    for (int j = tid; j < n; j += nthr) {
+      rowk[j] = (j == k ? 1.0 : a[k * n + j]) * ip;
+      colk[j] = a[j * n + k];
+    }
+    __syncthreads();
+    for (int e = tid; e < n * n; e += nthr) {
+      const int i = e / n, j = e - i * n;
+      if (i == k) a[e] = rowk[j];
+      else a[e] = (j == k ? 0.0 : a[e]) - colk[i] * rowk[j];
+    }
+    __syncthreads();
+  }
+  const double back = (singular && s_nact > 0) ? 1.0 / (s_sigma * s_nact) : 0.0;
+  for (int e = tid; e < n * n; e += nthr) {
+    const int i = e / n, j = e - i * n;
+    const bool act = pack[i] > 0.0f && pack[j] > 0.0f;
+    minv[e] = act ? (float)(0.5 * (a[e] + a[j * n + i]) - back) : 0.0f;
+  }
+}
+
+// smem per level (float offset soff[l]): z[np], r[np], pack[8n]
 __device__ __forceinline__ void nf_tail_half(float *__restrict__ z, const float *__restrict__ r,
                                              const float *__restrict__ pk, int n, int nx, int sy, int sz, float color,
                                              bool zero) {
@@ -566,79 +647,32 @@ __device__ __forceinline__ void nf_tail_project_warp(float *v, const float *pk, 
   __syncwarp();
 }
 
-// Coarsest level (n <= 64 cells) by ONE warp with its operator in registers: lane l owns cells l and l + 32; `sweeps`
-// red->black sweeps from a zero guess, then `sweeps` black->red sweeps (symmetric), warp barriers only.
-__device__ __forceinline__ void nf_tail_coarsest_warp(float *z, const float *r, const float *pk, int n, int sy, int sz,
-                                                      int sweeps) {
-  const int lane = threadIdx.x;
-  float w[2][6], dg[2], rr[2], col[2];
-  int nb[2][6];
-  bool has[2];
-#pragma unroll
-  for (int c = 0; c < 2; ++c) {
-    const int id = lane + 32 * c;
-    has[c] = id < n;
-    const int ic = has[c] ? id : 0;
-    dg[c] = pk[ic];
-    rr[c] = r[ic];
-    col[c] = pk[7 * n + ic];
-#pragma unroll
-    for (int f = 0; f < 6; ++f) w[c][f] = pk[(1 + f) * n + ic];
-    nb[c][0] = max(ic - 1, 0); nb[c][1] = min(ic + 1, n - 1);
-    nb[c][2] = max(ic - sy, 0); nb[c][3] = min(ic + sy, n - 1);
-    nb[c][4] = max(ic - sz, 0); nb[c][5] = min(ic + sz, n - 1);
-  }
-  auto half = [&](float color, bool zero) {
-#pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      if (has[c] && col[c] == color) {
-        float a = rr[c];
-        if (!zero) {
-#pragma unroll
-          for (int f = 0; f < 6; ++f) a += w[c][f] * z[nb[c][f]];
-        }
-        z[lane + 32 * c] = a * dg[c];
-      }
-    }
-    __syncwarp();
-  };
-  for (int s = 0; s < sweeps; ++s) {
-    half(0.0f, s == 0);
-    half(1.0f, false);
-  }
-  for (int s = 0; s < sweeps; ++s) {
-    half(1.0f, false);
-    half(0.0f, false);
+// Packed operator of the tail levels (and the coarsest inverse), global -> shared, by the bulk-copy engine
+// (cp.async.bulk + mbarrier): one thread issues it, no registers are staged, and in k_vcoarse it overlaps the whole
+// down sweep of the levels above.  Every block is 16-byte aligned on both sides (np, goff: NfTailK).
+__device__ __forceinline__ void nf_tail_bulk(unsigned dst, const char *src, unsigned bytes, unsigned bar) {
+  for (unsigned o = 0; o < bytes; o += 32768u) {
+    const unsigned b = min(32768u, bytes - o);
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst + o),
+                 "l"(src + o), "r"(b), "r"(bar)
+                 : "memory");
   }
 }
-
-// Packed operator of the tail levels, global -> shared, by the bulk-copy engine (cp.async.bulk + mbarrier): one
-// thread issues it, no registers are staged, and in k_vcoarse it overlaps the whole down sweep of the levels above.
-// Needs every level's cell count to be a multiple of 4 (16-byte chunks); otherwise nf_tail_run loads with plain loops.
-__device__ __forceinline__ bool nf_tail_bulk_ok(const NfTailK &T) {
-  bool ok = true;
-  for (int l = 0; l < T.nlev; ++l) ok = ok && (T.n[l] & 3) == 0;
-  return ok;
-}
-__device__ __forceinline__ void nf_tail_prefetch(const NfTailK &T, const float *__restrict__ pack_g, float *sm,
+__device__ __forceinline__ void nf_tail_prefetch(const NfTailK &T, const float *__restrict__ pack_g,
+                                                 const float *__restrict__ minv_g, float *sm,
                                                  unsigned long long *mbar) {  // called by ONE thread
   const unsigned bar = (unsigned)__cvta_generic_to_shared(mbar);
   asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  unsigned total = 0;
+  const int nc = T.n[T.nlev - 1];
+  const unsigned mbytes = T.direct ? 4u * (unsigned)((nc * nc + 3) & ~3) : 0u;
+  unsigned total = mbytes;
   for (int l = 0; l < T.nlev; ++l) total += 32u * (unsigned)T.n[l];
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(total) : "memory");
-  for (int l = 0; l < T.nlev; ++l) {
-    const unsigned n = (unsigned)T.n[l];
-    const unsigned dst = (unsigned)__cvta_generic_to_shared(sm + 10 * (size_t)T.off[l] + 2 * n);
-    const char *src = (const char *)(pack_g + 8 * (size_t)T.off[l]);
-    for (unsigned o = 0; o < 32u * n; o += 32768u) {
-      const unsigned bytes = min(32768u, 32u * n - o);
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst + o),
-                   "l"(src + o), "r"(bytes), "r"(bar)
-                   : "memory");
-    }
-  }
+  for (int l = 0; l < T.nlev; ++l)
+    nf_tail_bulk((unsigned)__cvta_generic_to_shared(sm + T.soff[l] + 2 * T.np[l]), (const char *)(pack_g + T.goff[l]),
+                 32u * (unsigned)T.n[l], bar);
+  if (mbytes) nf_tail_bulk((unsigned)__cvta_generic_to_shared(sm + T.minv_soff), (const char *)minv_g, mbytes, bar);
 }
 __device__ __forceinline__ void nf_tail_wait(unsigned long long *mbar) {
   const unsigned bar = (unsigned)__cvta_generic_to_shared(mbar);
@@ -655,33 +689,38 @@ __device__ __forceinline__ void nf_tail_wait(unsigned long long *mbar) {
 // The sub-V-cycle of the tail levels by ONE CTA (all of its threads must call it); rg / zg: right-hand side and
 // result of the first tail level in global memory (plain loads: rg may have been written in this very kernel).
 // mbar != nullptr: the packs are arriving through nf_tail_prefetch -- wait for them instead of loading.
-__device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__restrict__ pack_g, const float *rg,
-                                            float *zg, float *sm, unsigned long long *mbar) {
+__device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__restrict__ pack_g,
+                                            const float *__restrict__ minv_g, const float *rg, float *zg, float *sm,
+                                            unsigned long long *mbar) {
   const int nl = T.nlev;
   // the first level's right-hand side, zero every z (and the packs unless prefetched)
   for (int l = 0; l < nl; ++l) {
-    const int n = T.n[l];
-    float *base = sm + 10 * (size_t)T.off[l];
+    const int n = T.n[l], np = T.np[l];
+    float *base = sm + T.soff[l];
     if (!mbar) {
-      const float *src = pack_g + 8 * (size_t)T.off[l];
-      for (int t = threadIdx.x; t < 8 * n; t += blockDim.x) base[2 * n + t] = src[t];
+      const float *src = pack_g + T.goff[l];
+      for (int t = threadIdx.x; t < 8 * n; t += blockDim.x) base[2 * np + t] = src[t];
     }
     for (int t = threadIdx.x; t < n; t += blockDim.x) {
       base[t] = 0.0f;
-      base[n + t] = l == 0 ? rg[t] : 0.0f;
+      base[np + t] = l == 0 ? rg[t] : 0.0f;
     }
+  }
+  if (!mbar && T.direct) {
+    const int nc = T.n[nl - 1];
+    for (int t = threadIdx.x; t < nc * nc; t += blockDim.x) sm[T.minv_soff + t] = minv_g[t];
   }
   if (mbar) nf_tail_wait(mbar);
   __syncthreads();
   // down
   for (int l = 0; l + 1 < nl; ++l) {
     const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
-    float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
+    float *z = sm + T.soff[l], *r = z + T.np[l], *pk = z + 2 * T.np[l];
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, true);
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
     // residual + restriction: r_c = 1/8 sum children (r - A z), A z = z/idg - sum wg z_nb on active cells
     const int cn = T.n[l + 1], cnx = T.nx[l + 1], cny = T.ny[l + 1], fz = T.fz[l];
-    float *rc = sm + 10 * (size_t)T.off[l + 1] + cn;
+    float *rc = sm + T.soff[l + 1] + T.np[l + 1];
     const int sy = nx, sz = nx * ny;
     for (int cidx = threadIdx.x; cidx < cn; cidx += blockDim.x) {
       const int I = cidx % cnx, J = (cidx / cnx) % cny, K = cidx / (cnx * cny);
@@ -698,39 +737,47 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
             const float s = pk[1 * n + id] * z[max(id - 1, 0)] + pk[2 * n + id] * z[min(id + 1, n - 1)] +
                       pk[3 * n + id] * z[max(id - sy, 0)] + pk[4 * n + id] * z[min(id + sy, n - 1)] +
                       pk[5 * n + id] * z[max(id - sz, 0)] + pk[6 * n + id] * z[min(id + sz, n - 1)];
-            const float idg = pk[id];
-            // c*diag = 1/idg on active cells (includes faces towards Dirichlet ghosts); inactive: r = 0, z = 0
-            if (idg > 0.0f) acc += r[id] - (z[id] / idg - s);
+            // (a red cell holds z = r idg exactly, so r - A z = c sum alpha z_nb there; inactive: weights 0)
+            acc += s;
           }
       rc[cidx] = (fz == 2 ? 0.125f : 0.25f) * acc;
     }
     __syncthreads();
   }
-  // coarsest level: `sweeps` red->black sweeps from a zero guess, then `sweeps` black->red sweeps (symmetric)
+  // coarsest level
   {
     const int l = nl - 1;
     const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
-    float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
+    float *z = sm + T.soff[l], *r = z + T.np[l], *pk = z + 2 * T.np[l];
     // Singular system: the restricted residual is compatible (zero sum over the active cells) only up to rounding,
-    // and the many sweeps below would amplify what is left into a huge constant in z (which, prolonged, ends up
+    // and an (almost) exact solve would amplify what is left into a huge constant in z (which, prolonged, ends up
     // dominating the search direction: PCG then stalls near 1e-5 and diverges).  Solve in the complement of the
     // constant: project r before and z after (P M_c P stays symmetric).
     if (T.singular) {
       if (threadIdx.x < 32) nf_tail_project_warp(r, pk, n);
       __syncthreads();
     }
-    if (n > 256) {  // (a one-level tail: the CTA-wide sweeps)
-      for (int s = 0; s < T.sweeps; ++s) {
-        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, s == 0);
-        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+    if (T.direct) {
+      // z = A_c^{-1} r with the precomputed (symmetric) inverse: thread (part, i) sums a slice of column i -- read as
+      // row-major mi[j n + i], conflict-free across i -- and the slices are added through the scratch block
+      const float *mi = sm + T.minv_soff;
+      float *scr = sm + T.scratch_soff;
+      const int parts = min((int)blockDim.x / n, 8);
+      const int part = threadIdx.x / n, i = threadIdx.x - part * n;
+      if (part < parts) {
+        const int j0 = part * n / parts, j1 = (part + 1) * n / parts;
+        float acc = 0.0f;
+        for (int j = j0; j < j1; ++j) acc += mi[j * n + i] * r[j];
+        scr[part * n + i] = acc;
       }
-      for (int s = 0; s < T.sweeps; ++s) {
-        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
-        nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
+      __syncthreads();
+      if (threadIdx.x < n) {
+        float acc = 0.0f;
+        for (int p = 0; p < parts; ++p) acc += scr[p * n + threadIdx.x];
+        z[threadIdx.x] = acc;
       }
-    } else if (n <= 64) {
-      if (threadIdx.x < 32) nf_tail_coarsest_warp(z, r, pk, n, nx, nx * ny, T.sweeps);
-    } else {
+      __syncthreads();
+    } else {  // (a coarsest level with more than NF_DIRECT_MAX cells -- odd extents high up: symmetric sweeps)
       for (int s = 0; s < T.sweeps; ++s) {
         nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, s == 0);
         nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
@@ -740,7 +787,6 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
         nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
       }
     }
-    __syncthreads();
     if (T.singular) {
       if (threadIdx.x < 32) nf_tail_project_warp(z, pk, n);
       __syncthreads();
@@ -749,9 +795,9 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
   // up
   for (int l = nl - 2; l >= 0; --l) {
     const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
-    float *z = sm + 10 * (size_t)T.off[l], *r = z + n, *pk = z + 2 * n;
+    float *z = sm + T.soff[l], *r = z + T.np[l], *pk = z + 2 * T.np[l];
     const int cnx = T.nx[l + 1], cny = T.ny[l + 1], fz = T.fz[l];
-    const float *zc = sm + 10 * (size_t)T.off[l + 1];
+    const float *zc = sm + T.soff[l + 1];
     for (int id = threadIdx.x; id < n; id += blockDim.x) {
       const int i = id % nx, j = (id / nx) % ny, k = id / (nx * ny);
       z[id] += zc[((fz == 2 ? k >> 1 : k) * cny + (j >> 1)) * cnx + (i >> 1)];
@@ -760,19 +806,19 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
   }
-  for (int t = threadIdx.x; t < T.n[0]; t += blockDim.x) zg[t] = sm[t];
+  for (int t = threadIdx.x; t < T.n[0]; t += blockDim.x) zg[t] = sm[T.soff[0] + t];
 }
 
 __global__ void __launch_bounds__(NF_TAIL_THREADS) k_tail(NfTailK T, const float *__restrict__ pack_g,
+                                                           const float *__restrict__ minv_g,
                                                            const float *__restrict__ rg, float *__restrict__ zg,
                                                            const NfSolveState *st) {
   if (st && st->done) return;
   extern __shared__ __align__(16) float sm[];
   __shared__ unsigned long long mbar;
-  const bool bulk = nf_tail_bulk_ok(T);
-  if (bulk && threadIdx.x == 0) nf_tail_prefetch(T, pack_g, sm, &mbar);
+  if (threadIdx.x == 0) nf_tail_prefetch(T, pack_g, minv_g, sm, &mbar);
   __syncthreads();
-  nf_tail_run(T, pack_g, rg, zg, sm, bulk ? &mbar : nullptr);
+  nf_tail_run(T, pack_g, minv_g, rg, zg, sm, &mbar);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -867,6 +913,7 @@ struct NfCoarseK {
   float *z[NF_MAX_LEVELS], *r[NF_MAX_LEVELS];
   NfTailK T;
   const float *pack;
+  const float *minv;  // inverse of the coarsest operator (k_coarse_inverse)
 };
 
 __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_constant__ NfCoarseK P,
@@ -874,8 +921,7 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
   if (st && st->done) return;  // (uniform over the grid: written by an earlier kernel)
   extern __shared__ __align__(16) float sm[];
   __shared__ unsigned long long mbar;
-  const bool bulk = P.has_tail && nf_tail_bulk_ok(P.T);
-  if (bulk && blockIdx.x == 0 && threadIdx.x == 0) nf_tail_prefetch(P.T, P.pack, sm, &mbar);
+  if (P.has_tail && blockIdx.x == 0 && threadIdx.x == 0) nf_tail_prefetch(P.T, P.pack, P.minv, sm, &mbar);
   cg::grid_group grid = cg::this_grid();
   // task index: warps are dealt round-robin over the CTAs so that a small level still spreads over every SM
   const int gn = gridDim.x * blockDim.x;  // (tasks < 2^31)
@@ -929,7 +975,7 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
     grid.sync();
   }
   if (P.has_tail) {
-    if (blockIdx.x == 0) nf_tail_run(P.T, P.pack, P.r[P.nb], P.z[P.nb], sm, bulk ? &mbar : nullptr);
+    if (blockIdx.x == 0) nf_tail_run(P.T, P.pack, P.minv, P.r[P.nb], P.z[P.nb], sm, &mbar);
     grid.sync();
   }
   for (int l = P.nb - 1; l >= P.first; --l) {
@@ -944,10 +990,19 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
     } else {
       for (int t = gt; t < nx4 * ny * nz; t += gn) {
         const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
-        if ((j + k) & 1)
-          (L.fz == 2 ? nf_up1_body<1, 2> : nf_up1_body<1, 1>)(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
-        else
-          (L.fz == 2 ? nf_up1_body<0, 2> : nf_up1_body<0, 1>)(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+        // (explicit branches: selecting the body through a conditional expression made it an indirect call --
+        // un-inlined, with a stack frame; this phase took 15 us at the 128^3 level against 5 us for k_up2's)
+        if (L.fz == 2) {
+          if ((j + k) & 1)
+            nf_up1_body<1, 2>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+          else
+            nf_up1_body<0, 2>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+        } else {
+          if ((j + k) & 1)
+            nf_up1_body<1, 1>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+          else
+            nf_up1_body<0, 1>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+        }
       }
     }
     grid.sync();
@@ -969,20 +1024,48 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
 // ------------------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------------------
+#define NF_TAIL_SMEM_MAX 231424  // dynamic shared memory of k_tail / k_vcoarse (226 KB of the 227 KB a CTA may use)
+
+// Shared-memory layout of a tail that starts at level `first` (NfTailK); T.total_floats is what it needs.
+static void tail_desc(const nf_grid *g, int first, NfTailK *T) {
+  const int nl = g->nlev;
+  T->nlev = nl - first;
+  int so = 0, go = 0, m = 1;
+  for (int l = first; l < nl; ++l) {
+    const NfLevel &L = g->lv[l];
+    const int t = l - first, n = (int)L.ncell, np = (n + 3) & ~3;
+    T->n[t] = n; T->np[t] = np; T->nx[t] = L.nx; T->ny[t] = L.ny; T->nz[t] = L.nz; T->fz[t] = L.fz;
+    T->soff[t] = so; T->goff[t] = go;
+    so += 2 * np + 8 * n;
+    so = (so + 3) & ~3;
+    go += 8 * n;
+    if (l == nl - 1) m = std::max(L.nx, std::max(L.ny, L.nz));
+  }
+  const int nc = nl > first ? (int)g->lv[nl - 1].ncell : 0;
+  T->direct = (nc > 0 && nc <= NF_DIRECT_MAX) ? 1 : 0;
+  T->minv_soff = so;
+  if (T->direct) so += (nc * nc + 3) & ~3;
+  T->scratch_soff = so;
+  so += 1024;
+  T->total_floats = so;
+  T->sweeps = 2 * m;
+  T->singular = g->singular;
+}
 static size_t tail_smem_bytes(const nf_grid *g) {
-  size_t cells = 0;
-  for (int l = g->tail; l < g->nlev; ++l) cells += (size_t)g->lv[l].ncell;
-  return cells * 10 * sizeof(float);
+  NfTailK T;
+  tail_desc(g, g->tail, &T);
+  return (size_t)T.total_floats * sizeof(float);
 }
 
 // Decide which levels form the shared-memory tail and which run the vec kernels (called from nf_grid_create).
 void nf_mg_plan(nf_grid *g) {
   const int nl = g->nlev;
-  long long cells = 0;
   int tail = nl;
   for (int l = nl - 1; l >= 0; --l) {
-    if (cells + g->lv[l].ncell > NF_TAIL_MAX_CELLS) break;
-    cells += g->lv[l].ncell;
+    if (g->lv[l].ncell > NF_TAIL_MAX_CELLS) break;
+    NfTailK T;
+    tail_desc(g, l, &T);
+    if ((size_t)T.total_floats * sizeof(float) > NF_TAIL_SMEM_MAX) break;
     tail = l;
   }
   g->tail = tail;
@@ -996,9 +1079,11 @@ void nf_mg_plan(nf_grid *g) {
 }
 
 int nf_mg_init(nf_grid *g) {
-  const int smem = NF_TAIL_MAX_CELLS * 10 * (int)sizeof(float);
+  const int smem = NF_TAIL_SMEM_MAX;
   NF_CUDA(g, cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_coarse_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (NF_DIRECT_MAX * NF_DIRECT_MAX + 2 * NF_DIRECT_MAX) * (int)sizeof(double)));
   // the cooperative coarse kernel: one CTA per SM; needs a tail, at least one vec level below the finest one, and
   // every level between the finest one and the tail to be a vec level
   g->coarse_ctas = 0;
@@ -1037,6 +1122,8 @@ int nf_mg_pack_tail(nf_grid *g) {
     NfLevel &L = g->lv[l];
     const int n = (int)L.ncell;
     NF_LAUNCH(g, NFK_COARSEN, k_tail_pack<<<(n + 255) / 256, 256, 0, g->stream>>>(L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->tailpack + 8 * off));
+    if (l == g->nlev - 1 && n <= NF_DIRECT_MAX)  // the coarsest operator's inverse (fp64 Gauss-Jordan, one CTA)
+      NF_LAUNCH(g, NFK_COARSEN, k_coarse_inverse<<<1, 1024, (size_t)(n * n + 2 * n) * sizeof(double), g->stream>>>(g->tailpack + 8 * off, n, L.nx, L.ny, g->d_counts, g->tailinv));
     off += (size_t)n;
   }
   NF_CUDA(g, cudaGetLastError());
@@ -1107,36 +1194,17 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
       P.pk[l] = g->lv[l].pk;
       if (l >= 2 && l < nb && g->lv[l].pk && P.dense_from == NF_MAX_LEVELS) P.dense_from = l;
     }
-    int off = 0, m = 1;
-    P.T.nlev = nl - g->tail;
-    for (int l = g->tail; l < nl; ++l) {
-      const NfLevel &L = g->lv[l];
-      const int t = l - g->tail;
-      P.T.n[t] = (int)L.ncell; P.T.nx[t] = L.nx; P.T.ny[t] = L.ny; P.T.nz[t] = L.nz; P.T.off[t] = off; P.T.fz[t] = L.fz;
-      off += (int)L.ncell;
-      if (l == nl - 1) m = L.nx > L.ny ? (L.nx > L.nz ? L.nx : L.nz) : (L.ny > L.nz ? L.ny : L.nz);
-    }
-    P.T.sweeps = 2 * m;
-    P.T.singular = g->singular;
+    tail_desc(g, g->tail, &P.T);
+    P.minv = g->tailinv;
     P.pack = g->tailpack;
     const NfSolveState *stc = st;
     void *args[] = {(void *)&P, (void *)&stc};
     NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel((void *)k_vcoarse, dim3(g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
   } else if (has_tail) {
     NfTailK T;
-    T.nlev = nl - g->tail;
-    int off = 0, m = 1;
-    for (int l = g->tail; l < nl; ++l) {
-      const NfLevel &L = g->lv[l];
-      const int t = l - g->tail;
-      T.n[t] = (int)L.ncell; T.nx[t] = L.nx; T.ny[t] = L.ny; T.nz[t] = L.nz; T.off[t] = off; T.fz[t] = L.fz;
-      off += (int)L.ncell;
-      if (l == nl - 1) m = L.nx > L.ny ? (L.nx > L.nz ? L.nx : L.nz) : (L.ny > L.nz ? L.ny : L.nz);
-    }
-    T.sweeps = 2 * m;
-    T.singular = g->singular;
+    tail_desc(g, g->tail, &T);
     NfLevel &F = g->lv[g->tail];
-    NF_LAUNCH(g, NFK_BOTTOM, k_tail<<<1, NF_TAIL_THREADS, tail_smem_bytes(g), g->stream>>>(T, g->tailpack, F.r, F.z, st));
+    NF_LAUNCH(g, NFK_BOTTOM, k_tail<<<1, NF_TAIL_THREADS, tail_smem_bytes(g), g->stream>>>(T, g->tailpack, g->tailinv, F.r, F.z, st));
   } else {  // coarsest level too large for one CTA (odd extents): a few symmetric sweeps in global memory
     NfLevel &B = g->lv[nl - 1];
     const int nsw = 4;

@@ -31,7 +31,7 @@ def test_reference_arm_line_has_contract_keys(capsys):
     import types
     b = _bench()
     b._oracle_case = lambda n: _small_case()  # (a 12^3 sample keeps the CPU suite fast)
-    args = types.SimpleNamespace(steps=1, warmup=0)
+    args = types.SimpleNamespace(steps=1, warmup=0, cpu_n=0, cpu_n_forced=False)
     b.run_reference(args)
     line = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
     for k in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
@@ -48,4 +48,5 @@ def _small_case():
     phi, us = wl.config4_solid(P, 1)
     rng = np.random.default_rng(77)
     gin = [rng.standard_normal(a.shape).astype(np.float32) for a in U]
-    return P, U, phi, us, gin
+    bc = orc.BC(P["bc_types"], P["bc_values"])
+    return P, U, orc.face_weights(phi, bc), us, gin, bc

@@ -6,8 +6,9 @@ check the CUDA V-cycle kernels (fused 4-launch levels, cooperative coarse kernel
 shared-memory tail) against something that carries no fp32 rounding: V(1,1), red-black Gauss-Seidel (pre: red then
 black from a zero guess; post: black then red), piecewise-constant prolongation P, restriction P^T / 8,
 rediscretised coarse operators with c_l = c / 4^l on weights that are the mean of the four coincident fine face
-weights, levels halving while every extent is even and stays >= 4, coarsest level: 2 * (largest extent) symmetric
-sweeps (red-black from zero, then black-red), in the complement of the constant on singular systems.
+weights, levels halving while every extent is even and stays >= 4 (>= 2 while the level has more than 128 cells), coarsest level (<= 128 cells): exact solve (the
+pseudo-inverse in the complement of the constant on singular systems); a larger coarsest level: 2 * (largest extent)
+symmetric sweeps (red-black from zero, then black-red).
 3-D grids only."""
 import numpy as np
 
@@ -27,7 +28,7 @@ def hierarchy(alpha):
     lv = [[np.asarray(x, dtype=np.float32) for x in alpha]]
     while True:
         nz, ny, nx = lv[-1][0].shape[0], lv[-1][0].shape[1], lv[-1][0].shape[2] - 1
-        if (nx | ny | nz) & 1 or min(nx, ny, nz) // 2 < 4:
+        if (nx | ny | nz) & 1 or min(nx, ny, nz) // 2 < (2 if nx * ny * nz > 128 else 4):
             break
         lv.append(_coarsen(lv[-1]))
     return lv
@@ -70,11 +71,25 @@ def vcycle(r, alpha, c, singular):
         if l == len(levels) - 1:
             if singular:
                 r = np.where(act, r - r[act].sum() / max(int(act.sum()), 1), r)
-            sweeps = 2 * max(nx, ny, nz)
-            for _ in range(sweeps):
-                half(red); half(~red)
-            for _ in range(sweeps):
-                half(~red); half(red)
+            if r.size <= 128:  # direct solve with the (pseudo-)inverse of the coarsest operator on the active cells
+                n = r.size
+                A = np.zeros((n, n))
+                for col in range(n):
+                    e = np.zeros(n); e[col] = 1.0
+                    e3 = e.reshape(r.shape)
+                    A[:, col] = (d * e3 - c * _nbsum(e3, a)).ravel()
+                ia = np.flatnonzero(act.ravel())
+                sol = np.zeros(n)
+                if ia.size:
+                    sol[ia] = np.linalg.pinv(A[np.ix_(ia, ia)], hermitian=True) @ r.ravel()[ia] if singular else \
+                        np.linalg.solve(A[np.ix_(ia, ia)], r.ravel()[ia])
+                z = sol.reshape(r.shape)
+            else:
+                sweeps = 2 * max(nx, ny, nz)
+                for _ in range(sweeps):
+                    half(red); half(~red)
+                for _ in range(sweeps):
+                    half(~red); half(red)
             if singular:
                 z = np.where(act, z - z[act].sum() / max(int(act.sum()), 1), z)
             return z
