@@ -176,10 +176,53 @@ def active_cells(alpha):
 
 
 def is_singular(alpha, bc):
-    """True when no Dirichlet domain face carries an open face weight (R12, global form)."""
+    """True when no Dirichlet domain face carries an open face weight: EVERY fluid component is singular (R12)."""
     au, av, aw = alpha
     planes = [au[:, :, 0], au[:, :, -1], av[:, 0, :], av[:, -1, :], aw[0], aw[-1]]
     return not any(bc.types[f] == 1 and np.any(planes[f] > 0) for f in range(6))
+
+
+def components(alpha, bc):
+    """Fluid components (R12): the connected components of the active cells, two cells being connected when the face
+    between them is open (alpha > 0).  Returns (labels, singular): labels[k, j, i] in 1..K on active cells and 0 on
+    inactive ones; singular[c] (c = 0..K, entry 0 unused) is True when component c touches no open face of a Dirichlet
+    domain boundary -- A restricted to it then has the constant null vector.  The labelling itself is a library
+    primitive (scipy.ndimage.label with its default face connectivity) applied to the doubled lattice whose odd sites
+    are the cells and whose sites between two cells are the faces; pinned by a brute-force flood fill."""
+    from scipy import ndimage
+    au, av, aw = (np.asarray(a) for a in alpha)
+    nz, ny, nx = au.shape[0], au.shape[1], au.shape[2] - 1
+    act = active_cells([au, av, aw])
+    lat = np.zeros((2 * nz + 1, 2 * ny + 1, 2 * nx + 1), dtype=bool)
+    lat[1::2, 1::2, 1::2] = act
+    lat[1::2, 1::2, 2:-1:2] = au[:, :, 1:-1] > 0   # interior faces only: a boundary face connects to no second cell
+    lat[1::2, 2:-1:2, 1::2] = av[:, 1:-1, :] > 0
+    lat[2:-1:2, 1::2, 1::2] = aw[1:-1] > 0
+    lab, _ = ndimage.label(lat)
+    cl = lab[1::2, 1::2, 1::2]
+    ids = np.unique(cl[act])
+    remap = np.zeros(int(lab.max()) + 1, dtype=np.int64)
+    remap[ids] = np.arange(1, ids.size + 1)
+    labels = np.where(act, remap[cl], 0)
+    K = int(ids.size)
+    singular = np.ones(K + 1, dtype=bool)
+    planes = [(au[:, :, 0], labels[:, :, 0]), (au[:, :, -1], labels[:, :, -1]), (av[:, 0, :], labels[:, 0, :]),
+              (av[:, -1, :], labels[:, -1, :]), (aw[0], labels[0]), (aw[-1], labels[-1])]
+    for f in range(6):
+        if bc.types[f] == 1:
+            w, l = planes[f]
+            singular[np.unique(l[w > 0])] = False
+    singular[0] = False
+    return labels, singular
+
+
+def remove_component_means(x, labels, singular):
+    """x minus, on every singular component, its mean over that component (R12: compatibility of b, gauge of p)."""
+    K = singular.size - 1
+    sums = np.bincount(labels.ravel(), weights=x.ravel(), minlength=K + 1)
+    cnt = np.maximum(np.bincount(labels.ravel(), minlength=K + 1), 1)
+    mean = np.where(singular, sums / cnt, 0.0)
+    return x - mean[labels]
 
 
 def effective_solid_velocity(us, shapes, bc):
@@ -212,14 +255,15 @@ def rhs(uhat, alpha, us, c, bc):
 def solve(b, alpha, c, bc, tol=1e-12, maxit=200000, info=None):
     """Solve A p = b.  MGPCG is only a fast way to reach this; the oracle uses
     Jacobi-preconditioned CG in fp64 to a relative residual `tol` (R11: ||r||_2 <= tol ||b||_2, x0 = 0).
-    Inactive cells (diag 0) get p = 0 and b = 0.  On a singular system (R12) the mean of b over active
-    cells is removed and the solution has zero mean over active cells."""
+    Inactive cells (diag 0) get p = 0 and b = 0.  A is block diagonal over the fluid components (R12); on every
+    component without an open Dirichlet face the block has the constant null vector: the mean of b over that
+    component is removed (compatibility) and the solution has zero mean over it (gauge)."""
     act = active_cells(alpha)
-    sing = is_singular(alpha, bc)
+    labels, singc = components(alpha, bc)
+    sing = bool(singc.any())
     b = np.where(act, b, 0.0)
-    nact = max(int(act.sum()), 1)
     if sing:
-        b = np.where(act, b - b.sum() / nact, 0.0)
+        b = remove_component_means(b, labels, singc)
     d = diag_A(alpha, c)
     dinv = np.where(act, 1.0 / np.where(act, d, 1.0), 0.0)
     x = np.zeros_like(b)
@@ -243,7 +287,7 @@ def solve(b, alpha, c, bc, tol=1e-12, maxit=200000, info=None):
             p = z + (rz_new / rz) * p
             rz = rz_new
     if sing:
-        x = np.where(act, x - x[act].sum() / nact, 0.0)
+        x = remove_component_means(x, labels, singc)
     if info is not None:
         info["iters"] = it
         info["relres"] = float(np.linalg.norm(b - apply_A(x, alpha, c)) / np.sqrt(bb)) if bb > 0 else 0.0
@@ -261,15 +305,11 @@ def solve_dense(b, alpha, c, bc):
         e[col] = 1.0
         Am[:, col] = apply_A(e.reshape(shape), alpha, c).ravel()
         e[col] = 0.0
+    # the pseudo-inverse IS the per-component definition: it drops the part of b in the null space (the mean over
+    # every singular component) and returns the solution orthogonal to the null space (zero mean over each of them)
     bb = np.where(act, b, 0.0)
-    sing = is_singular(alpha, bc)
-    if sing:
-        bb = np.where(act, bb - bb.sum() / act.sum(), 0.0)
-    x = (np.linalg.pinv(Am, hermitian=True) @ bb.ravel()).reshape(shape)
-    x = np.where(act, x, 0.0)
-    if sing:
-        x = np.where(act, x - x[act].sum() / act.sum(), 0.0)
-    return x
+    x = (np.linalg.pinv(Am, rcond=1e-12, hermitian=True) @ bb.ravel()).reshape(shape)
+    return np.where(act, x, 0.0)
 
 
 # ----------------------------------------------------------------------------------------------------

@@ -538,3 +538,101 @@ def test_keep_largest_component():
     assert ncomp == 2
     act = O.active_cells([au, av, aw])
     assert not act[:, :, :2].any() and act[:, :, 2:].all()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# R12 per fluid component: labels, compatibility and gauge of every singular component
+# ---------------------------------------------------------------------------------------------------------
+def _flood_fill_labels(alpha):
+    """Brute force: breadth-first search over cells, stepping through faces with alpha > 0 (pure Python)."""
+    au, av, aw = alpha
+    nz, ny, nx = au.shape[0], au.shape[1], au.shape[2] - 1
+    act = O.active_cells(alpha)
+    lab = np.zeros((nz, ny, nx), dtype=int)
+    cur = 0
+    for k0 in range(nz):
+        for j0 in range(ny):
+            for i0 in range(nx):
+                if not act[k0, j0, i0] or lab[k0, j0, i0]:
+                    continue
+                cur += 1
+                lab[k0, j0, i0] = cur
+                todo = [(k0, j0, i0)]
+                while todo:
+                    k, j, i = todo.pop()
+                    nbs = []
+                    if i > 0 and au[k, j, i] > 0: nbs.append((k, j, i - 1))
+                    if i + 1 < nx and au[k, j, i + 1] > 0: nbs.append((k, j, i + 1))
+                    if j > 0 and av[k, j, i] > 0: nbs.append((k, j - 1, i))
+                    if j + 1 < ny and av[k, j + 1, i] > 0: nbs.append((k, j + 1, i))
+                    if k > 0 and aw[k, j, i] > 0: nbs.append((k - 1, j, i))
+                    if k + 1 < nz and aw[k + 1, j, i] > 0: nbs.append((k + 1, j, i))
+                    for c in nbs:
+                        if not lab[c]:
+                            lab[c] = cur
+                            todo.append(c)
+    return lab
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_components_equal_brute_force_flood_fill(seed):
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = 7, 6, 5
+    alpha = [np.where(rng.uniform(size=s) < 0.55, 0.0, rng.uniform(0.1, 1, s)) for s in
+             [(nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)]]
+    bc = O.BC((1, 0, 0, 0, 0, 1))
+    O.apply_wall_bc(*alpha, bc)
+    lab, sing = O.components(alpha, bc)
+    ref = _flood_fill_labels(alpha)
+    assert np.array_equal(lab > 0, ref > 0) and lab.max() == ref.max() and lab.max() >= 2
+    # same partition: the pairs (label, reference label) are one to one
+    pairs = set(zip(lab[lab > 0].tolist(), ref[ref > 0].tolist()))
+    assert len(pairs) == lab.max()
+    # singular flag by hand: a component is regular iff one of its cells has an open face on a Dirichlet boundary
+    for c in range(1, lab.max() + 1):
+        m = lab == c
+        touches = bool(np.any(alpha[0][:, :, 0][m[:, :, 0]] > 0) or np.any(alpha[2][-1][m[-1]] > 0))
+        assert sing[c] == (not touches)
+
+
+def test_solve_two_pockets_matches_pseudo_inverse():
+    """A wall of closed faces splits an 8 x 6 x 5 box into a pocket with a Dirichlet face and a closed pocket (its
+    block of A has the constant null vector): the CG solve with per-component compatibility and gauge (R12) equals
+    the pseudo-inverse solution of the dense matrix; the regular pocket keeps its mean, the closed one has none."""
+    rng = np.random.default_rng(5)
+    nx, ny, nz = 8, 6, 5
+    alpha = [rng.uniform(0.2, 1, s) for s in [(nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)]]
+    alpha[0][:, :, 4] = 0.0
+    bc = O.BC((1, 0, 0, 0, 0, 0), (0.3, 0, 0, 0, 0, 0))
+    O.apply_wall_bc(*alpha, bc)
+    lab, sing = O.components(alpha, bc)
+    assert lab.max() == 2 and sing.tolist() == [False, False, True]
+    assert O.is_singular(alpha, bc) is False      # (the global flag says "regular": not enough for the closed pocket)
+    b = rng.standard_normal((nz, ny, nx))
+    x = O.solve(b, alpha, 1.7, bc, tol=1e-13)
+    xd = O.solve_dense(b, alpha, 1.7, bc)
+    assert np.max(np.abs(x - xd)) <= 1e-9 * np.max(np.abs(xd))
+    assert abs(x[lab == 2].mean()) <= 1e-12 and abs(x[lab == 1].mean()) > 1e-3
+    # the residual that is left is exactly the incompatible part of b: its mean over the closed pocket
+    res = b - O.apply_A(x, alpha, 1.7)
+    assert np.max(np.abs(res[lab == 1])) <= 1e-10
+    assert np.max(np.abs(res[lab == 2] - b[lab == 2].mean())) <= 1e-10
+
+
+def test_projection_with_closed_pocket_is_divergence_free_where_it_can_be():
+    """Projection on the two-pocket box with a solid velocity: zero weighted divergence in the pocket with the outlet;
+    in the closed pocket the divergence that remains is the constant the incompatible boundary flux forces."""
+    rng = np.random.default_rng(6)
+    nx, ny, nz = 8, 6, 5
+    shp = [(nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)]
+    alpha = [rng.uniform(0.2, 1, s) for s in shp]
+    alpha[0][:, :, 4] = 0.0
+    bc = O.BC((1, 0, 0, 0, 0, 0))
+    O.apply_wall_bc(*alpha, bc)
+    U = [rng.standard_normal(s) for s in shp]
+    us = [0.1 * rng.standard_normal(s) for s in shp]
+    Un, p = O.project(U, alpha, us, 0.125, 0.9, bc)
+    lab, _ = O.components(alpha, bc)
+    div = O.weighted_divergence(Un, alpha, us, bc)
+    assert np.max(np.abs(div[lab == 1])) <= 1e-9
+    assert np.max(np.abs(div[lab == 2] - div[lab == 2].mean())) <= 1e-9
