@@ -107,8 +107,8 @@ int nf_set_solid_velocity(nf_grid *g, const float *us, const float *vs, const fl
 
 /* a-3..a-5  Solve A p = rhs with MGPCG, A = c G^T S G with homogeneous ghosts.
  * Convergence (R11): ||r||_2 <= tol ||rhs||_2, x0 = 0.  rhs is taken as 0 on inactive cells (sum of the 6
- * face weights = 0), where p = 0.  If no Dirichlet domain face carries an open weight the system is
- * singular (R12): the mean of rhs over active cells is removed and p has zero mean over active cells.
+ * face weights = 0), where p = 0.  On every fluid component without an open Dirichlet face the system is
+ * singular (R12): the mean of rhs over that component is removed and p has zero mean over it.
  * rhs is not modified.  p may not alias rhs. */
 int nf_solve(nf_grid *g, const float *rhs, float *p, float tol, int maxit);
 
@@ -231,8 +231,15 @@ int nf_host_sync(nf_grid *g);
 /* Info about the last solve on this handle.  Synchronises the handle's stream.
  * relres = ||r||_2/||rhs||_2 as tracked by the solver; ms = device time of the solve (CUDA events). */
 int nf_last_solve_info(nf_grid *g, int *iters, float *relres, float *ms);
-/* Number of multigrid levels; number of active cells; 1 if the current system is singular (R12). */
+/* Number of multigrid levels; number of active cells; 1 if no Dirichlet domain face carries an open weight (every
+ * component is then singular, R12; nf_grid_components gives the per-component count). */
 int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, int *singular);
+/* Fluid components of the current weights (R12): A = c G^T S G is block diagonal over the connected components of the
+ * active cells (cells joined by faces with alpha > 0; found on the device by nf_set_solid / nf_set_weights).  A
+ * component without an open face on a Dirichlet domain boundary is singular: every solve removes the mean of the
+ * right-hand side over it (compatibility) and returns a pressure with zero mean over it (gauge) -- the paper is silent;
+ * SURVEY.md 8c.1.  *components = number of components, *singular_components = those that are singular. */
+int nf_grid_components(nf_grid *g, int *components, int *singular_components);
 /* Per-kernel-class device timing (CUDA events around every launch on the handle's stream; adds launch overhead, so
  * use it on extra steps, not on timed ones).  nf_profile_enable(g,1) clears the counters and starts recording;
  * nf_profile_get synchronises the stream and returns the accumulated milliseconds and launch count of class idx

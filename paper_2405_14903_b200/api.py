@@ -56,6 +56,7 @@ _SIGNATURES = {
                                           ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]),
     "nf_grid_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_int),
                                     ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_int)]),
+    "nf_grid_components": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int)]),
     "nf_profile_enable": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "nf_profile_get": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_char_p),
                                       ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)]),
@@ -417,6 +418,12 @@ class Grid:
         lv, na, sg = ctypes.c_int(), ctypes.c_longlong(), ctypes.c_int()
         self._check(self.lib.nf_grid_info(self.h, ctypes.byref(lv), ctypes.byref(na), ctypes.byref(sg)), "nf_grid_info")
         return dict(levels=lv.value, active_cells=na.value, singular=sg.value)
+
+    def components(self):
+        """(number of fluid components, number of singular ones) of the current weights (R12)."""
+        nc, ns = ctypes.c_int(), ctypes.c_int()
+        self._check(self.lib.nf_grid_components(self.h, ctypes.byref(nc), ctypes.byref(ns)), "nf_grid_components")
+        return nc.value, ns.value
 
     def profile_enable(self, on=True):
         self._check(self.lib.nf_profile_enable(self.h, 1 if on else 0), "nf_profile_enable")

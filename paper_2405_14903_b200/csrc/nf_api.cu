@@ -26,6 +26,7 @@ static void free_all(nf_grid *g) {
   cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->b0); cudaFree(g->ecorr); cudaFree(g->r_alt); cudaFree(g->tailpack); cudaFree(g->tailinv);
   cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
   cudaFree(g->st); cudaFree(g->d_counts); cudaFree(g->geom_par); cudaFree(g->geom_grad);
+  nf_components_free(g);
   if (g->hst) cudaFreeHost((void *)g->hst);
   if (g->h_counts) cudaFreeHost(g->h_counts);
   if (g->ev0) cudaEventDestroy(g->ev0);
@@ -52,7 +53,8 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->stream = 0;
   g->nu_pre = 1; g->nu_post = 1; g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
   g->weights_set = g->have_sdf = g->have_us = false;
-  g->singular = 1; g->nact = 0;
+  g->singular = 1; g->singular_info = 1; g->nact = 0; g->ncomp = 0; g->nsing = 0; g->gauge_mode = 1;
+  g->comp = nullptr; g->cc_cnt = nullptr; g->cc_regular = nullptr; g->cc_sums = nullptr; g->cc_meta = nullptr; g->h_cc_meta = nullptr;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
   g->prof_on = false;
   for (int c = 0; c < NFK_COUNT; ++c) { g->prof_ms[c] = 0.0; g->prof_n[c] = 0; }
@@ -102,7 +104,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     size_t tc = 0;
     for (int l = g->tail; l < nl; ++l) tc += (size_t)g->lv[l].ncell;
     ok = ok && dalloc(&g->tailpack, 8 * tc) == cudaSuccess;
-    ok = ok && dalloc(&g->tailinv, 128 * 128 + 4) == cudaSuccess;
+    ok = ok && dalloc(&g->tailinv, 128 * 128 + 4 + 136) == cudaSuccess;  // the inverse + component labels (nf_mg.cu)
   }
   const size_t nc = nf_nc(g);
   ok = ok && dalloc(&g->us, nf_nu(g)) == cudaSuccess && dalloc(&g->vs, nf_nv(g)) == cudaSuccess &&
@@ -113,6 +115,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   ok = ok && dalloc(&g->fu, nf_nu(g)) == cudaSuccess && dalloc(&g->fv, nf_nv(g)) == cudaSuccess &&
        dalloc(&g->fw, nf_nw(g)) == cudaSuccess;
   ok = ok && dalloc(&g->st, 1) == cudaSuccess && dalloc(&g->d_counts, 2) == cudaSuccess;
+  ok = ok && nf_components_alloc(g) == NF_OK;
   ok = ok && dalloc(&g->geom_par, 2 * (size_t)NF_GEOM_MAXP) == cudaSuccess && dalloc(&g->geom_grad, (size_t)NF_GEOM_MAXP) == cudaSuccess;
   ok = ok && cudaHostAlloc((void **)&g->hst, NF_RING * sizeof(NfHostStatus), cudaHostAllocMapped) == cudaSuccess;
   ok = ok && cudaHostGetDevicePointer((void **)&g->hst_dev, (void *)g->hst, 0) == cudaSuccess;
@@ -448,7 +451,15 @@ extern "C" int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, in
   NF_CHECK_HANDLE(g);
   if (levels) *levels = g->nlev;
   if (active_cells) *active_cells = g->weights_set ? g->nact : -1;
-  if (singular) *singular = g->weights_set ? g->singular : -1;
+  if (singular) *singular = g->weights_set ? g->singular_info : -1;
+  return NF_OK;
+}
+
+extern "C" int nf_grid_components(nf_grid *g, int *components, int *singular_components) {
+  NF_CHECK_HANDLE(g);
+  if (!g->weights_set) return NF_ERR_STATE;
+  if (components) *components = g->ncomp;
+  if (singular_components) *singular_components = g->nsing;
   return NF_OK;
 }
 

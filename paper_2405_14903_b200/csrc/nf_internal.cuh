@@ -107,7 +107,13 @@ struct nf_grid {
   int tail;  // first level of the shared-memory tail of the V-cycle (levels tail .. nlev-1 run in one CTA); nlev if none
   NfLevel lv[NF_MAX_LEVELS];
   bool weights_set, have_sdf, have_us;
-  int singular;
+  int singular;  // 1: ONE component and it is singular -- the global mean is removed (R12); see gauge_mode
+  int singular_info;  // no open face on any Dirichlet domain boundary (what nf_grid_info reports)
+  // fluid components (nf_components.cu): labels, per-component cell counts / "has a Dirichlet face" flags / sums
+  int *comp, *cc_cnt, *cc_regular, *cc_meta, *h_cc_meta;
+  double *cc_sums;
+  int ncomp, nsing;  // components of the current weights; those without an open Dirichlet face
+  int gauge_mode;    // 0: no singular component; 1: a single, singular component (global path); 2: per component
   long long nact;
   int nu_pre, nu_post;
   bool warm;     // flag 8 of nf_set_solver_options: caller-provided solution arrays hold the initial guess
@@ -237,6 +243,11 @@ int nf_weights_to_user(nf_grid *g, float *au, float *av, float *aw);
 int nf_build_hierarchy(nf_grid *g);  // coarse weights + active count + singular flag
 int nf_store_solid_velocity(nf_grid *g, const float *us, const float *vs, const float *ws);
 int nf_weights_adjoint_impl(nf_grid *g, const float *gau, const float *gav, const float *gaw, float *gsdf);
+// nf_components.cu
+int nf_components_alloc(nf_grid *g);
+void nf_components_free(nf_grid *g);
+int nf_components_build(nf_grid *g);
+int nf_components_center(nf_grid *g, float *x, float *dst2, double *sq);
 // nf_solver.cu
 int nf_apply_A_impl(nf_grid *g, const float *p, float *q);
 // nf_mg.cu

@@ -529,20 +529,33 @@ __global__ void __launch_bounds__(256) k_tail_pack(const float *__restrict__ ax,
 
 // Inverse of the coarsest operator A_c (n <= NF_DIRECT_MAX cells) from its pack, in fp64, by in-place Gauss-Jordan
 // elimination without pivoting (A_c is symmetric positive definite on the active cells; inactive cells are decoupled
-// identity rows whose rows / columns of the result are zeroed).  Singular system (R12, constant null vector on the
-// active cells): A_c + sigma u u^T with u = e / sqrt(#active) is inverted instead, and (1/sigma) u u^T subtracted
-// again, which leaves the pseudo-inverse.  One CTA; runs when the weights change (nf_build_hierarchy).
-__global__ void __launch_bounds__(1024) k_coarse_inverse(const float *__restrict__ pack, int n, int nx, int ny,
-                                                          const double *__restrict__ counts,
+// identity rows whose rows / columns of the result are zeroed).  Null spaces (R12, per component): the coarse cells
+// are labelled by connected component (min-label propagation in shared memory); a component none of whose cells has an
+// open face on a Dirichlet domain boundary has the constant null vector u = e / sqrt(#cells): A_c + sigma u u^T is
+// inverted instead and (1/sigma) u u^T subtracted again, which leaves the pseudo-inverse.  Behind the n^2 floats of the
+// inverse the kernel writes, as ints, the singular-component number of every cell (-1: none) and their count: the
+// tail projects its right-hand side and its result on the complement of those null vectors.  One CTA; runs when the
+// weights change (nf_build_hierarchy).
+struct NfDir6 {
+  int dir[6];
+};
+__global__ void __launch_bounds__(1024) k_coarse_inverse(const float *__restrict__ pack, int n, NfLvK Lc, NfDir6 bc,
                                                           float *__restrict__ minv) {
-  const bool singular = !(counts[1] > 0.0);  // no open face on a Dirichlet domain face (k_encode, level 0)
   extern __shared__ double sa[];
   double *a = sa, *rowk = sa + n * n, *colk = rowk + n;
-  __shared__ double s_sigma, s_pivot;
-  __shared__ int s_nact;
+  __shared__ double s_pivot, s_sig[NF_DIRECT_MAX];
+  __shared__ int s_lab[NF_DIRECT_MAX], s_reg[NF_DIRECT_MAX], s_cnt[NF_DIRECT_MAX], s_id[NF_DIRECT_MAX], s_kc;
+  const int nx = Lc.nx, ny = Lc.ny, nz = Lc.nz;
   const int tid = threadIdx.x, nthr = blockDim.x;
   const int off[6] = {-1, 1, -nx, nx, -nx * ny, nx * ny};
   for (int e = tid; e < n * n; e += nthr) a[e] = 0.0;
+  for (int i = tid; i < n; i += nthr) {
+    s_lab[i] = pack[i] > 0.0f ? i : -1;
+    s_reg[i] = 0;
+    s_cnt[i] = 0;
+    s_sig[i] = 0.0;
+    s_id[i] = -1;
+  }
   __syncthreads();
   for (int i = tid; i < n; i += nthr) {
     const float idg = pack[i];
@@ -556,20 +569,52 @@ __global__ void __launch_bounds__(1024) k_coarse_inverse(const float *__restrict
       a[i * n + i] = 1.0;
     }
   }
-  if (tid == 0) {
-    int na = 0;
-    double sd = 0.0;
-    for (int i = 0; i < n; ++i)
-      if (pack[i] > 0.0f) { na += 1; sd += 1.0 / (double)pack[i]; }
-    s_nact = na;
-    s_sigma = na > 0 ? sd / na : 1.0;
+  // components: min-label propagation through the open faces
+  for (;;) {
+    int changed = 0;
+    for (int i = tid; i < n; i += nthr) {
+      int m = s_lab[i];
+      if (m < 0) continue;
+      for (int f = 0; f < 6; ++f)
+        if (pack[(1 + f) * n + i] != 0.0f) m = min(m, s_lab[i + off[f]]);
+      if (m < s_lab[i]) { s_lab[i] = m; changed = 1; }
+    }
+    if (!__syncthreads_or(changed)) break;
+  }
+  // a component with an open face on a Dirichlet domain boundary is regular
+  for (int i = tid; i < n; i += nthr) {
+    if (s_lab[i] < 0) continue;
+    const int ci = i % nx, cj = (i / nx) % ny, ck = i / (nx * ny);
+    const bool edge = (ci == 0 && bc.dir[0]) || (ci == nx - 1 && bc.dir[1]) || (cj == 0 && bc.dir[2]) ||
+                      (cj == ny - 1 && bc.dir[3]) || (ck == 0 && bc.dir[4]) || (ck == nz - 1 && bc.dir[5]);
+    if (edge) {
+      const NfW6 w = nf_load_w6(Lc.ax, Lc.ay, Lc.az, ci, cj, ck, nx, ny, Lc.pax);
+      const bool open = (ci == 0 && bc.dir[0] && w.xl > 0.0f) || (ci == nx - 1 && bc.dir[1] && w.xh > 0.0f) ||
+                        (cj == 0 && bc.dir[2] && w.yl > 0.0f) || (cj == ny - 1 && bc.dir[3] && w.yh > 0.0f) ||
+                        (ck == 0 && bc.dir[4] && w.zl > 0.0f) || (ck == nz - 1 && bc.dir[5] && w.zh > 0.0f);
+      if (open) s_reg[s_lab[i]] = 1;
+    }
   }
   __syncthreads();
-  const double shift = (singular && s_nact > 0) ? s_sigma / s_nact : 0.0;
-  if (shift != 0.0) {
+  if (tid == 0) {  // number the singular components; sigma = mean diagonal of the component
+    int kc = 0;
+    for (int i = 0; i < n; ++i) {
+      const int r = s_lab[i];
+      if (r < 0 || s_reg[r]) continue;
+      if (s_id[r] < 0) s_id[r] = kc++;
+      s_cnt[r] += 1;
+      s_sig[r] += 1.0 / (double)pack[i];
+    }
+    for (int r = 0; r < n; ++r)
+      if (s_cnt[r] > 0) s_sig[r] /= s_cnt[r];
+    s_kc = kc;
+  }
+  __syncthreads();
+  if (s_kc > 0) {
     for (int e = tid; e < n * n; e += nthr) {
       const int i = e / n, j = e - i * n;
-      if (pack[i] > 0.0f && pack[j] > 0.0f) a[e] += shift;
+      const int r = s_lab[i];
+      if (r >= 0 && r == s_lab[j] && s_id[r] >= 0) a[e] += s_sig[r] / s_cnt[r];
     }
     __syncthreads();
   }
@@ -589,12 +634,17 @@ __global__ void __launch_bounds__(1024) k_coarse_inverse(const float *__restrict
     }
     __syncthreads();
   }
-  const double back = (singular && s_nact > 0) ? 1.0 / (s_sigma * s_nact) : 0.0;
   for (int e = tid; e < n * n; e += nthr) {
     const int i = e / n, j = e - i * n;
-    const bool act = pack[i] > 0.0f && pack[j] > 0.0f;
-    minv[e] = act ? (float)(0.5 * (a[e] + a[j * n + i]) - back) : 0.0f;
+    const int r = s_lab[i];
+    const bool act = r >= 0 && s_lab[j] >= 0;
+    double v = 0.5 * (a[e] + a[j * n + i]);
+    if (act && r == s_lab[j] && s_id[r] >= 0) v -= 1.0 / (s_sig[r] * s_cnt[r]);
+    minv[e] = act ? (float)v : 0.0f;
   }
+  int *lab_out = reinterpret_cast<int *>(minv + ((n * n + 3) & ~3));
+  for (int i = tid; i < n; i += nthr) lab_out[i] = s_lab[i] >= 0 ? s_id[s_lab[i]] : -1;
+  if (tid == 0) lab_out[n] = s_kc;
 }
 
 // smem per level (float offset soff[l]): z[np], r[np], pack[8n]
@@ -647,6 +697,29 @@ __device__ __forceinline__ void nf_tail_project_warp(float *v, const float *pk, 
   __syncwarp();
 }
 
+// v -= its mean over every singular component of the coarsest level (clab[id] = component number or -1; kc of them).
+// Warp 0 only; caller syncs around it.
+__device__ __forceinline__ void nf_tail_project_comps(float *v, const int *clab, int n, int kc) {
+  const int lane = threadIdx.x;
+  for (int c = 0; c < kc; ++c) {
+    float s = 0.0f, m = 0.0f;
+    for (int id = lane; id < n; id += 32)
+      if (clab[id] == c) {
+        s += v[id];
+        m += 1.0f;
+      }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      s += __shfl_xor_sync(0xffffffffu, s, o);
+      m += __shfl_xor_sync(0xffffffffu, m, o);
+    }
+    const float mean = m > 0.0f ? s / m : 0.0f;
+    for (int id = lane; id < n; id += 32)
+      if (clab[id] == c) v[id] -= mean;
+  }
+  __syncwarp();
+}
+
 // Packed operator of the tail levels (and the coarsest inverse), global -> shared, by the bulk-copy engine
 // (cp.async.bulk + mbarrier): one thread issues it, no registers are staged, and in k_vcoarse it overlaps the whole
 // down sweep of the levels above.  Every block is 16-byte aligned on both sides (np, goff: NfTailK).
@@ -665,7 +738,7 @@ __device__ __forceinline__ void nf_tail_prefetch(const NfTailK &T, const float *
   asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   const int nc = T.n[T.nlev - 1];
-  const unsigned mbytes = T.direct ? 4u * (unsigned)((nc * nc + 3) & ~3) : 0u;
+  const unsigned mbytes = T.direct ? 4u * (unsigned)(((nc * nc + 3) & ~3) + ((nc + 1 + 3) & ~3)) : 0u;
   unsigned total = mbytes;
   for (int l = 0; l < T.nlev; ++l) total += 32u * (unsigned)T.n[l];
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(total) : "memory");
@@ -708,7 +781,8 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
   }
   if (!mbar && T.direct) {
     const int nc = T.n[nl - 1];
-    for (int t = threadIdx.x; t < nc * nc; t += blockDim.x) sm[T.minv_soff + t] = minv_g[t];
+    const int mfl = ((nc * nc + 3) & ~3) + ((nc + 1 + 3) & ~3);  // the inverse and, behind it, the component labels
+    for (int t = threadIdx.x; t < mfl; t += blockDim.x) sm[T.minv_soff + t] = minv_g[t];
   }
   if (mbar) nf_tail_wait(mbar);
   __syncthreads();
@@ -753,8 +827,13 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
     // and an (almost) exact solve would amplify what is left into a huge constant in z (which, prolonged, ends up
     // dominating the search direction: PCG then stalls near 1e-5 and diverges).  Solve in the complement of the
     // constant: project r before and z after (P M_c P stays symmetric).
-    if (T.singular) {
-      if (threadIdx.x < 32) nf_tail_project_warp(r, pk, n);
+    const int *clab = reinterpret_cast<const int *>(sm + T.minv_soff + ((n * n + 3) & ~3));
+    const int kc = T.direct ? clab[n] : 0;  // singular components of the coarsest level (k_coarse_inverse)
+    if (T.direct ? kc > 0 : T.singular != 0) {
+      if (threadIdx.x < 32) {
+        if (T.direct) nf_tail_project_comps(r, clab, n, kc);
+        else nf_tail_project_warp(r, pk, n);
+      }
       __syncthreads();
     }
     if (T.direct) {
@@ -787,8 +866,11 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
         nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
       }
     }
-    if (T.singular) {
-      if (threadIdx.x < 32) nf_tail_project_warp(z, pk, n);
+    if (T.direct ? kc > 0 : T.singular != 0) {
+      if (threadIdx.x < 32) {
+        if (T.direct) nf_tail_project_comps(z, clab, n, kc);
+        else nf_tail_project_warp(z, pk, n);
+      }
       __syncthreads();
     }
   }
@@ -1044,12 +1126,12 @@ static void tail_desc(const nf_grid *g, int first, NfTailK *T) {
   const int nc = nl > first ? (int)g->lv[nl - 1].ncell : 0;
   T->direct = (nc > 0 && nc <= NF_DIRECT_MAX) ? 1 : 0;
   T->minv_soff = so;
-  if (T->direct) so += (nc * nc + 3) & ~3;
+  if (T->direct) so += ((nc * nc + 3) & ~3) + ((nc + 1 + 3) & ~3);
   T->scratch_soff = so;
   so += 1024;
   T->total_floats = so;
   T->sweeps = 2 * m;
-  T->singular = g->singular;
+  T->singular = g->singular_info;  // (only read when the coarsest level is too large for the direct solve)
 }
 static size_t tail_smem_bytes(const nf_grid *g) {
   NfTailK T;
@@ -1123,7 +1205,11 @@ int nf_mg_pack_tail(nf_grid *g) {
     const int n = (int)L.ncell;
     NF_LAUNCH(g, NFK_COARSEN, k_tail_pack<<<(n + 255) / 256, 256, 0, g->stream>>>(L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->tailpack + 8 * off));
     if (l == g->nlev - 1 && n <= NF_DIRECT_MAX)  // the coarsest operator's inverse (fp64 Gauss-Jordan, one CTA)
-      NF_LAUNCH(g, NFK_COARSEN, k_coarse_inverse<<<1, 1024, (size_t)(n * n + 2 * n) * sizeof(double), g->stream>>>(g->tailpack + 8 * off, n, L.nx, L.ny, g->d_counts, g->tailinv));
+    {
+      NfDir6 bc;
+      for (int f = 0; f < 6; ++f) bc.dir[f] = g->bc_type[f] == NF_BC_DIRICHLET ? 1 : 0;
+      NF_LAUNCH(g, NFK_COARSEN, k_coarse_inverse<<<1, 1024, (size_t)(n * n + 2 * n) * sizeof(double), g->stream>>>(g->tailpack + 8 * off, n, nf_lvk(L), bc, g->tailinv));
+    }
     off += (size_t)n;
   }
   NF_CUDA(g, cudaGetLastError());

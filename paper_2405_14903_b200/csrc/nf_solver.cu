@@ -560,7 +560,16 @@ int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit) {
   const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
   const float *in = src ? src : L.r;
   const size_t n = (size_t)L.ncell;
-  if (!g->force_generic && vec_ok(in, L.r, g->b0, g->b0, n)) {
+  if (g->gauge_mode == 2) {
+    // several fluid components, some without a Dirichlet face: compatibility per component (nf_components.cu)
+    if (!g->force_generic && vec_ok(in, L.r, g->b0, g->b0, n)) {
+      NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(in, L.r, nullptr, L.code, n >> 2, nullptr, nullptr));
+    } else {
+      NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<d.grid, d.block, 0, g->stream>>>(in, L.r, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum));
+    }
+    NF_TRY(nf_components_center(g, L.r, g->b0, &g->st->bb));
+    NF_LAUNCH(g, NFK_SETUP, k_start_state<<<1, 32, 0, g->stream>>>(g->st));
+  } else if (!g->force_generic && vec_ok(in, L.r, g->b0, g->b0, n)) {
     if (!g->singular) {
       NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(in, L.r, g->b0, L.code, n >> 2, nullptr, &g->st->bb));
     } else {
@@ -742,8 +751,10 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
     if (rc != NF_OK) return rc;
   }
   g->last_iters = ph.iters;
-  // gauge: zero mean over active cells on a singular system (R12)
-  if (g->singular && !g->force_generic && vec_ok(x, x, x, x, n)) {
+  // gauge: zero mean over active cells on a singular system (R12) -- per component when there are several
+  if (g->gauge_mode == 2) {
+    NF_TRY(nf_components_center(g, x, nullptr, nullptr));
+  } else if (g->singular && !g->force_generic && vec_ok(x, x, x, x, n)) {
     NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, x, nullptr, L.code, n >> 2, &g->st->sum, nullptr));
     const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
     NF_LAUNCH(g, NFK_SETUP, k_center4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, nullptr, L.code, n >> 2, &g->st->sum, inv, nullptr));

@@ -399,6 +399,7 @@ int nf_build_hierarchy(nf_grid *g) {
     if (L.vec) NF_LAUNCH(g, NFK_CLASSIFY, k_encode_deep<<<d.grid, d.block, 0, g->stream>>>(L.code, L.nx, L.ny, L.nz));
   }
   NF_CUDA(g, cudaGetLastError());
+  NF_TRY(nf_components_build(g));  // fluid components of level 0 (R12 per component, nf_components.cu)
   {
     int rc = nf_mg_pack_tail(g);
     if (rc != NF_OK) return rc;
@@ -407,7 +408,18 @@ int nf_build_hierarchy(nf_grid *g) {
   NF_CUDA(g, cudaStreamSynchronize(g->stream));
   const double *hc = g->h_counts;
   g->nact = (long long)hc[0];
-  g->singular = hc[1] > 0.0 ? 0 : 1;
+  g->singular_info = hc[1] > 0.0 ? 0 : 1;
+  // null-space handling (R12): none / one global mean / per component
+  if (g->comp && g->h_cc_meta[0] > 1) {
+    g->ncomp = g->h_cc_meta[0];
+    g->nsing = g->h_cc_meta[2];
+    g->gauge_mode = g->nsing > 0 ? 2 : 0;
+  } else {
+    g->ncomp = g->nact > 0 ? 1 : 0;
+    g->nsing = g->singular_info ? g->ncomp : 0;
+    g->gauge_mode = g->singular_info ? 1 : 0;
+  }
+  g->singular = g->gauge_mode == 1 ? 1 : 0;
   g->weights_set = true;
   return NF_OK;
 }

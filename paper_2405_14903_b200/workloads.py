@@ -256,6 +256,39 @@ def config5_rhs(n, active, seed=1005):
     return b.astype(np.float32)
 
 
+def fluid_components(au, av, aw):
+    """Labels (1..K, 0 = inactive) of the face-connected sets of active cells, and K.  Graph utility only (labels the
+    doubled lattice: cells at odd sites, open interior faces between them): used to draw right-hand sides that are
+    compatible on every closed fluid pocket (BASELINE.json configs[4]: 'RHS i.i.d. N(0,1) with its mean removed')."""
+    from scipy import ndimage
+    nz, ny, nx = au.shape[0], au.shape[1], au.shape[2] - 1
+    act = (au[:, :, :-1] + au[:, :, 1:] + av[:, :-1, :] + av[:, 1:, :] + aw[:-1] + aw[1:]) > 0
+    lat = np.zeros((2 * nz + 1, 2 * ny + 1, 2 * nx + 1), dtype=bool)
+    lat[1::2, 1::2, 1::2] = act
+    lat[1::2, 1::2, 2:-1:2] = au[:, :, 1:-1] > 0
+    lat[1::2, 2:-1:2, 1::2] = av[:, 1:-1, :] > 0
+    lat[2:-1:2, 1::2, 1::2] = aw[1:-1] > 0
+    lab, _ = ndimage.label(lat)
+    cl = np.where(act, lab[1::2, 1::2, 1::2], 0)
+    ids = np.unique(cl[act])
+    remap = np.zeros(int(lab.max()) + 1, dtype=np.int64)
+    remap[ids] = np.arange(1, ids.size + 1)
+    return remap[cl], int(ids.size)
+
+
+def config5_rhs_per_component(n, labels, seed=1005):
+    """N(0,1) on the active cells with the mean over every fluid component removed (closed walls: every component is
+    singular, so this is the compatible right-hand side of configs[4] without discarding any pocket)."""
+    rng = np.random.default_rng(seed + 7 * n)
+    b = np.where(labels > 0, rng.standard_normal((n, n, n)).astype(np.float32), 0).astype(np.float64)
+    K = int(labels.max())
+    sums = np.bincount(labels.ravel(), weights=b.ravel(), minlength=K + 1)
+    cnt = np.maximum(np.bincount(labels.ravel(), minlength=K + 1), 1)
+    mean = sums / cnt
+    mean[0] = 0.0
+    return (b - mean[labels]).astype(np.float32)
+
+
 def keep_largest_component(au, av, aw):
     """Zero every face weight that does not touch the largest face-connected set of active cells
     (R12: the library removes the null space globally, so inputs must have one fluid component).

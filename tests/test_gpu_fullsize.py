@@ -154,12 +154,13 @@ def test_pressure_solve_sweep_residual(torch, api, n):
     phi = wl.config5_phi(n)
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
     g = api.Grid(n, n, n, 1.0 / n)
-    g.set_solid(d(phi))
-    au, av, aw, _ = wl.keep_largest_component(*[a.cpu().numpy() for a in g.get_weights()])
-    active = (au[:, :, :-1] + au[:, :, 1:] + av[:, :-1, :] + av[:, 1:, :] + aw[:-1] + aw[1:]) > 0
-    rhs = wl.config5_rhs(n, active)
-    g.set_weights(d(au), d(av), d(aw))
-    p = torch.empty(g.shape_p, dtype=torch.float32, device="cuda")
+    g.set_solid(d(phi))                      # nf_set_solid alone (per-component null spaces, R12)
+    au, av, aw = [a.cpu().numpy() for a in g.get_weights()]
+    labels, ncomp = wl.fluid_components(au, av, aw)
+    assert g.components() == (ncomp, ncomp)  # closed walls: every component is singular
+    active = labels > 0
+    rhs = wl.config5_rhs_per_component(n, labels)
+    p = torch.zeros(g.shape_p, dtype=torch.float32, device="cuda")
     rc = g.solve(d(rhs), p, tol=1e-6, maxit=400)
     info = g.last_solve_info()
     assert rc == 0 and info["iters"] < 100, info
@@ -167,7 +168,6 @@ def test_pressure_solve_sweep_residual(torch, api, n):
     a64 = [a.astype(np.float64) for a in (au, av, aw)]
     res = rhs.astype(np.float64) - orc.apply_A(p.cpu().numpy().astype(np.float64), a64, c)
     res[~active] = 0.0
-    res[active] -= res[active].mean()
     g.close()
     assert np.linalg.norm(res) <= 5e-6 * np.linalg.norm(rhs)
 
