@@ -551,3 +551,61 @@ def loss_sum_u2(lo, hi):
         g[0][lo:hi, lo:hi, lo:hi] = 2.0 * blk
         return float(np.sum(blk * blk)), g
     return fn
+
+
+def cfl_dt(U, t_left, dx, cfl, max_substeps=64):
+    """Sub-step size under the CFL condition the paper says it adopts ("adopts CFL condition", L403-410
+    Table 4: the steps simulated exceed the frames; no constant or formula is given -- reading R24): the remaining
+    frame time t_left is cut into n equal sub-steps, n the smallest integer with dt = t_left / n <= cfl dx / max|U|
+    (at most max_substeps); re-evaluated after every sub-step because the velocity changes."""
+    vmax = max_speed(U)
+    if not (vmax > 0.0) or not np.isfinite(vmax):
+        return t_left
+    n = max(1, min(max_substeps, int(np.ceil(t_left * vmax / (cfl * dx) - 1e-9))))
+    return t_left / n
+
+
+def rollout_substepped(U0, solid_fn_t, nframes, dt_frame, dx, rho, bc, loss_fn, cfl=1.0, dts=None, tol=1e-12,
+                       advect_on=True, nu=0.0, max_substeps=64):
+    """N frames of length dt_frame, each advanced by CFL sub-steps (cfl_dt, R24): per sub-step of size dt
+    "advect -> viscosity -> geometry at the sub-step's end time -> project" with dt/rho in Eqs. 4-5 (PAPER.md:L78, L103,
+    L151), and the backward pass in reversed order over the SUB-steps (L111); dt is a constant of the backward pass
+    (R24: the sub-step sizes are not differentiated).
+
+    solid_fn_t(t) -> (phi, us, dphi_dtheta, dus_dtheta) at physical time t; loss_fn(U) -> (J, dJ/dU).
+    dts: replay these sub-step sizes (a list of lists, one per frame) instead of choosing them -- what a
+    finite-difference check of the gradient needs, and what the CUDA path is compared on.
+    Returns (J, dJ/dtheta, dJ/dU0, dts_used)."""
+    U = [np.asarray(a, dtype=np.float64) for a in U0]
+    tape, used = [], []
+    for f in range(nframes):
+        t, t_end = f * dt_frame, (f + 1) * dt_frame
+        frame_dts = []
+        k = 0
+        while t_end - t > 1e-12 * dt_frame:
+            dt = dts[f][k] if dts is not None else cfl_dt(U, t_end - t, dx, cfl, max_substeps)
+            Uprev = U
+            Ut = advect(U, dt, dx) if advect_on else [a.copy() for a in U]
+            if nu != 0.0:
+                Ut = viscosity(Ut, nu, dt, dx)
+            t = t + dt
+            phi, us, dphi, dus = solid_fn_t(t)
+            alpha = face_weights(phi, bc)
+            U, p = project(Ut, alpha, us, dx, dt / rho, bc, tol=tol)
+            tape.append((Uprev, Ut, phi, us, dphi, dus, alpha, p, dt))
+            frame_dts.append(dt)
+            k += 1
+            if dts is not None and k >= len(dts[f]):
+                break
+        used.append(frame_dts)
+    J, g = loss_fn(U)
+    g = [np.asarray(a, dtype=np.float64) for a in g]
+    dtheta = 0.0
+    for Uprev, Ut, phi, us, dphi, dus, alpha, p, dt in reversed(tape):
+        g_ut, g_alpha, g_us, _ = project_adjoint(g, alpha, p, Ut, us, dx, dt / rho, bc, tol=tol)
+        g_phi = weights_adjoint(phi, g_alpha[0], g_alpha[1], g_alpha[2], bc)
+        dtheta += float(np.sum(g_phi * dphi)) + sum(float(np.sum(a * b)) for a, b in zip(g_us, dus))
+        if nu != 0.0:
+            g_ut = viscosity(g_ut, nu, dt, dx)
+        g = advect_adjoint(Uprev, g_ut, dt, dx) if advect_on else g_ut
+    return J, dtheta, g, used
