@@ -681,6 +681,91 @@ def run_envs(args):
                       "dtype": "f32", "rows": rows}))
 
 
+def run_config(args):
+    """BASELINE.json configs[1] / configs[2] at their stated size and length through the C ABI (rollout.py sequences the
+    calls): 64^3 x 10 full steps with two oscillating plates, gradient of the centre-block loss w.r.t. the plate
+    amplitude; 128^3 x 50 steps of the chamber pump (static chamber, 16 Gaussian wall bumps modulated by sin(2 pi t/50),
+    Dirichlet outlet), loss 1/2 sum u^2 on the outlet faces, gradient w.r.t. the 16 amplitudes, with the per-step state
+    (U^n, Uhat, p: "checkpointed pressures") kept on the device.  Reports ms per step (forward + backward), the PCG
+    iterations per step and the bytes of the tape."""
+    import numpy as np
+    import torch
+    from paper_2405_14903_b200 import api, rollout as ro, workloads as wl
+    api.load_library()
+    torch.cuda.set_device(0)
+    d = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    cfg = args.config
+    if cfg == 2:
+        n = args.n if args.n_forced else 64
+        P = wl.config2_params(n)
+        nsteps = P["steps"]
+        geom = {}
+        for st in range(1, nsteps + 1):
+            v = wl.config2_solid(P, st, P["theta"])
+            geom[st] = (d(v[0]), [d(a) for a in v[1]], d(v[2]), [d(a) for a in v[3]])
+        solid = lambda st: geom[st]
+        lo, hi = P["loss_lo"], P["loss_hi"]
+
+        def loss(U):
+            blk = U[0][lo:hi, lo:hi, lo:hi].double()
+            G = [torch.zeros_like(a) for a in U]
+            G[0][lo:hi, lo:hi, lo:hi] = (2.0 * blk).float()
+            return (blk * blk).sum(), G
+        name = "configs[1] two oscillating plates %d^3 x %d steps, dJ/d(amplitude)" % (n, nsteps)
+    else:
+        n = args.n if args.n_forced else 128
+        P = wl.config3_params(n)
+        nsteps = P["steps"]
+        phi, us1 = wl.config3_solid(P, P["period"] / 4.0)              # modulation sin(pi/2) = 1: the unit wall field
+        dphi_ = d(phi)
+        unit = [d(a) for a in us1]
+        basis = [[d(a) for a in wl.config3_us_basis(P, P["period"] / 4.0, k)] for k in range(16)]
+
+        def solid(st):
+            mod = float(np.sin(2 * np.pi * st / P["period"]))
+            return dphi_, [mod * a for a in unit], None, {"basis": basis, "scale": mod}
+
+        def loss(U):
+            G = [torch.zeros_like(a) for a in U]
+            out = U[0][:, :, -1].double()
+            G[0][:, :, -1] = out.float()
+            return 0.5 * (out * out).sum(), G
+        name = "configs[2] chamber pump %d^3 x %d steps, dJ/d(16 bump amplitudes)" % (n, nsteps)
+    g = api.Grid(n, n, n, P["dx"])
+    g.set_dt_rho(P["dt_over_rho"])
+    for f in range(6):
+        g.set_domain_bc(f, P["bc_types"][f], P["bc_values"][f])
+    U0 = [torch.zeros(sh, dtype=torch.float32, device="cuda") for sh in (g.shape_u, g.shape_v, g.shape_w)]
+    run = lambda stats=None: ro.rollout(g, U0, solid, nsteps, P["dt"], loss, tol=TOL, maxit=MAXIT, stats=stats)
+    for _ in range(max(1, min(args.warmup, 2))):
+        run()
+    torch.cuda.synchronize()
+    reps = max(1, min(args.steps, 3))
+    l0 = g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.reset_peak_memory_stats()
+    e0.record()
+    for _ in range(reps):
+        J, dJ, _ = run()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    launches = (g.launch_count() - l0) // reps
+    stats = {}
+    run(stats)
+    print(json.dumps({"workload": name, "dtype": "f32", "tol": TOL, "grid": [n, n, n], "steps": nsteps,
+                      "ms_total_fwd_bwd": round(ms, 3), "ms_per_step_fwd_bwd": round(ms / nsteps, 3),
+                      "iters_fwd_mean": round(float(np.mean(stats["iters_fwd"])), 1),
+                      "iters_adj_mean": round(float(np.mean(stats["iters_adj"])), 1),
+                      "iters_fwd_max": int(max(stats["iters_fwd"])), "iters_adj_max": int(max(stats["iters_adj"])),
+                      "tape_bytes": ro.tape_bytes(g, nsteps),
+                      "torch_peak_bytes": int(torch.cuda.max_memory_allocated()),
+                      "gpu_launches_per_rollout": int(launches), "loss": J,
+                      "dJ_dtheta": dJ if isinstance(dJ, list) else [dJ],
+                      "paper_context": "RTX A6000, whole step at 64^3: 0.105 s forward / 0.117-0.301 s backward "
+                                       "(PAPER.md Tables 2-3); memory 405 MB at 64^3 (Table 3)"}))
+
+
 def run_karman(args):
     """the paper's 2-D validation case (appendix D: flow past a cylinder on a
     512 x 1024 grid with viscosity) as a timing workload -- nz = 1 grid of 1024 x 512 cells, inflow p = 1 / outflow p = 0,
@@ -747,10 +832,16 @@ def main():
     ap.add_argument("--envs", default="", help="comma-separated environment counts: aggregate throughput of concurrent "
                                                 "small grids of size --n (e.g. --envs 1,4,8 --n 48) instead of the headline step")
     ap.add_argument("--karman", action="store_true", help="time the 2-D cylinder-in-channel case (1024 x 512, nz = 1)")
+    ap.add_argument("--config", type=int, default=0, choices=[0, 2, 3],
+                    help="2: BASELINE configs[1] (64^3 x 10 steps fwd + backprop); 3: configs[2] (128^3 x 50 steps chamber pump)")
     args = ap.parse_args()
+    args.n_forced = "--n" in sys.argv
     args.cpu_n_forced = args.cpu_n > 0
     if not args.cpu_n_forced:
         args.cpu_n = 96
+    if args.config:
+        run_config(args)
+        return
     if args.karman:
         run_karman(args)
         return

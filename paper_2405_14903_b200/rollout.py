@@ -6,13 +6,20 @@ chain rule only: every step of the path runs in the library's kernels."""
 import torch
 
 
-def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect_on=True, nu=0.0):
+def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect_on=True, nu=0.0, stats=None):
     """solid_fn(step) -> (phi, (us, vs, ws), dphi_dtheta, (dus, dvs, dws)) as CUDA float32 tensors (the derivative
     tensors may be None); loss_fn(U) -> (J tensor, [dJ/du, dJ/dv, dJ/dw]).
+    Several control parameters on which U_s depends linearly (BASELINE.json configs[2]: 16 bump amplitudes): pass
+    dus = {"basis": [(bu, bv, bw) per parameter], "scale": s} -- dJ/dtheta then is a list, dJ/dtheta_k = sum over the
+    steps of s <dJ/dU_s, basis_k> (Eq. 9b in the derived form R10).
+    stats (optional dict): filled with the PCG iteration counts per step ("iters_fwd", "iters_adj"; synchronises).
     Returns (J, dJ/dtheta, dJ/dU0) -- J and dJ/dtheta as Python floats."""
     g = grid
     U = [a.clone() for a in U0]
     tape = []
+    if stats is not None:
+        stats["iters_fwd"], stats["iters_adj"] = [], []
+    dvec = None
     for n in range(1, nsteps + 1):
         Uprev = [a.clone() for a in U]
         if advect_on:
@@ -24,6 +31,8 @@ def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect
         Uhat = [a.clone() for a in U]
         p = torch.zeros(g.shape_p, dtype=torch.float32, device=U[0].device)  # (zeros: a valid guess under the warm-start option)
         g.project(*U, p, tol=tol, maxit=maxit)
+        if stats is not None:
+            stats["iters_fwd"].append(g.last_solve_info()["iters"])
         tape.append((Uprev, Uhat, p, phi, us, dphi, dus))
     J, G = loss_fn(U)
     G = [a.clone() for a in G]
@@ -35,10 +44,17 @@ def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect
         Uprev, Uhat, p, phi, us, dphi, dus = tape[n - 1]
         g.set_solid(phi, *us)  # the hierarchy of step n (the handle holds one geometry at a time)
         g.project_adjoint(*G, p_saved=p, uhat=Uhat, galpha=ga, gus=gs, tol=tol, maxit=maxit)
-        g.weights_adjoint(*ga, gphi)
+        if stats is not None:
+            stats["iters_adj"].append(g.last_solve_info()["iters"])
         if dphi is not None:
+            g.weights_adjoint(*ga, gphi)
             dtheta += (gphi.double() * dphi.double()).sum()
-        if dus is not None:
+        if isinstance(dus, dict):
+            if dvec is None:
+                dvec = torch.zeros(len(dus["basis"]), dtype=torch.float64, device=U[0].device)
+            for k, bk in enumerate(dus["basis"]):
+                dvec[k] += dus["scale"] * sum((a.double() * b.double()).sum() for a, b in zip(gs, bk))
+        elif dus is not None:
             for a, b in zip(gs, dus):
                 if b is not None:
                     dtheta += (a.double() * b.double()).sum()
@@ -46,6 +62,8 @@ def rollout(grid, U0, solid_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect
             g.viscosity(*G, nu, dt)  # Eq. 8: the same symmetric matrix
         if advect_on:
             g.advect_adjoint(*Uprev, *G, dt)
+    if dvec is not None:
+        return float(J), [float(x) for x in dvec.cpu()], G
     return float(J), float(dtheta), G
 
 
@@ -60,6 +78,73 @@ def cfl_substeps(grid, U, dt_frame, cfl=1.0, max_substeps=64):
         return dt_frame, 1
     n = max(1, min(max_substeps, int(math.ceil(dt_frame * vmax / (cfl * grid.dx) - 1e-9))))
     return dt_frame / n, n
+
+
+def rollout_substepped(grid, U0, solid_fn_t, nframes, dt_frame, rho, loss_fn, cfl=1.0, dts=None, tol=1e-6, maxit=400,
+                       advect_on=True, nu=0.0, max_substeps=64):
+    """N frames of length dt_frame, each advanced by CFL sub-steps ("adopts CFL condition", L403-410
+    Table 4: 11 / 54 / 58 solver steps per cycle; R24): per sub-step of size dt  nf_set_dt_rho(dt / rho) -> nf_advect ->
+    [nf_viscosity] -> nf_set_solid(geometry at the sub-step's end time) -> nf_project, and the backward pass over the
+    sub-steps in reverse with the same dt (a constant of the backward pass).  dt comes from cfl_substeps (nf_max_speed
+    on the device) unless `dts` (one list of sub-step sizes per frame) is given, which replays them.
+    solid_fn_t(t) -> (phi, (us, vs, ws), dphi_dtheta, (dus, dvs, dws)) at physical time t, CUDA float32 tensors.
+    Returns (J, dJ/dtheta, dJ/dU0, dts_used).  Sequencing of C-ABI calls only."""
+    g = grid
+    U = [a.clone() for a in U0]
+    tape, used = [], []
+    for f in range(nframes):
+        t, t_end = f * dt_frame, (f + 1) * dt_frame
+        frame, k = [], 0
+        while t_end - t > 1e-12 * dt_frame:
+            dt = dts[f][k] if dts is not None else cfl_substeps(g, U, t_end - t, cfl, max_substeps)[0]
+            Uprev = [a.clone() for a in U]
+            g.set_dt_rho(dt / rho)
+            if advect_on:
+                g.advect(*U, dt)
+            if nu != 0.0:
+                g.viscosity(*U, nu, dt)
+            t = t + dt
+            phi, us, dphi, dus = solid_fn_t(t)
+            g.set_solid(phi, *us)
+            Uhat = [a.clone() for a in U]
+            p = torch.zeros(g.shape_p, dtype=torch.float32, device=U[0].device)
+            g.project(*U, p, tol=tol, maxit=maxit)
+            tape.append((Uprev, Uhat, p, phi, us, dphi, dus, dt))
+            frame.append(dt)
+            k += 1
+            if dts is not None and k >= len(dts[f]):
+                break
+        used.append(frame)
+    J, G = loss_fn(U)
+    G = [a.clone() for a in G]
+    dtheta = torch.zeros((), dtype=torch.float64, device=U[0].device)
+    ga = [torch.empty_like(a) for a in U]
+    gs = [torch.empty_like(a) for a in U]
+    gphi = torch.empty(g.shape_sdf, dtype=torch.float32, device=U[0].device)
+    for Uprev, Uhat, p, phi, us, dphi, dus, dt in reversed(tape):
+        g.set_dt_rho(dt / rho)
+        g.set_solid(phi, *us)
+        g.project_adjoint(*G, p_saved=p, uhat=Uhat, galpha=ga, gus=gs, tol=tol, maxit=maxit)
+        g.weights_adjoint(*ga, gphi)
+        if dphi is not None:
+            dtheta += (gphi.double() * dphi.double()).sum()
+        if dus is not None:
+            for a, b in zip(gs, dus):
+                if b is not None:
+                    dtheta += (a.double() * b.double()).sum()
+        if nu != 0.0:
+            g.viscosity(*G, nu, dt)
+        if advect_on:
+            g.advect_adjoint(*Uprev, *G, dt)
+    return float(J), float(dtheta), G, used
+
+
+def tape_bytes(grid, nsteps):
+    """Device memory of the per-step state kept for the backward pass instead of an autodiff graph:
+    U^n, Uhat (3 face arrays each) and p per step, float32."""
+    nu_, nv_, nw_ = [int(torch.tensor(s).prod()) for s in (grid.shape_u, grid.shape_v, grid.shape_w)]
+    np_ = int(torch.tensor(grid.shape_p).prod())
+    return 4 * nsteps * (2 * (nu_ + nv_ + nw_) + np_)
 
 
 def rollout_parametric(grid, U0, prims_fn, nsteps, dt, loss_fn, tol=1e-6, maxit=400, advect_on=True, band=float("inf")):

@@ -249,3 +249,53 @@ def test_max_speed_and_cfl_substeps(torch, api):
     Z = [torch.zeros_like(a) for a in dU]
     assert g.max_speed(*Z) == 0.0 and ro.cfl_substeps(g, Z, 0.3) == (0.3, 1)
     g.close()
+
+
+def test_substepped_rollout_matches_oracle(torch, api):
+    """CFL sub-stepped frames forward + backward (R24) through the C ABI against the oracle:
+    the library's own sub-step choice (nf_max_speed) gives the oracle's sub-step sizes, and on those sizes the loss
+    (1e-4), dJ/dtheta (1e-3) and dJ/dU0 (1e-3) agree."""
+    from paper_2405_14903_b200 import rollout as ro
+    n, nframes = 24, 2
+    P = wl.config2_params(n)
+    bc = orc.BC(P["bc_types"], P["bc_values"])
+    rng = np.random.default_rng(8)
+    U0 = [(1.5 * rng.standard_normal(s)).astype(np.float32) for s in wl.face_shapes(n, n, n)]
+    dt_frame, rho, theta = 1.0 / n, 2.0, 0.5
+    lo, hi = P["loss_lo"], P["loss_hi"]
+    cache = {}
+
+    def solid(t):
+        key = round(t / P["dt"], 9)
+        if key not in cache:
+            cache[key] = wl.config2_solid(P, t / P["dt"], theta)     # fp32 phi / u_s: the same arrays on both sides
+        return cache[key]
+
+    Jo, dJo, gU0o, used = orc.rollout_substepped(U0, solid, nframes, dt_frame, P["dx"], rho, bc,
+                                                 orc.loss_sum_u2(lo, hi), cfl=1.0)
+    assert all(len(d) >= 2 for d in used)
+    d = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    g = api.Grid(n, n, n, P["dx"])
+
+    def solid_dev(t):
+        v = solid(t)
+        return d(v[0]), [d(a) for a in v[1]], d(v[2]), [d(a) for a in v[3]]
+
+    def loss(U):
+        blk = U[0][lo:hi, lo:hi, lo:hi].double()
+        G = [torch.zeros_like(a) for a in U]
+        G[0][lo:hi, lo:hi, lo:hi] = (2.0 * blk).float()
+        return (blk * blk).sum(), G
+
+    # the library's own CFL choice from the initial velocity
+    dt0, n0 = ro.cfl_substeps(g, [d(a) for a in U0], dt_frame, cfl=1.0)
+    assert n0 == len(used[0]) + 0 * 1 or abs(dt0 - used[0][0]) <= 1e-6 * dt_frame
+    Jg, dJg, gU0g, used_g = ro.rollout_substepped(g, [d(a) for a in U0], solid_dev, nframes, dt_frame, rho, loss,
+                                                  dts=used, tol=1e-6, maxit=200)
+    g.close()
+    assert [len(x) for x in used_g] == [len(x) for x in used]
+    assert abs(Jg - Jo) <= 1e-4 * abs(Jo), (Jg, Jo)
+    assert abs(dJg - dJo) <= 1e-3 * abs(dJo), (dJg, dJo)
+    num = np.sqrt(sum(np.sum((a.cpu().numpy().astype(np.float64) - b) ** 2) for a, b in zip(gU0g, gU0o)))
+    den = np.sqrt(sum(np.sum(b ** 2) for b in gU0o))
+    assert num <= 1e-3 * den, num / den
