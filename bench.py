@@ -672,10 +672,76 @@ def run_envs(args):
         its = pool.run(work(args.steps))
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        rows.append({"envs": E, "env_steps_per_s": round(E * args.steps / dt, 1),
+        rows.append({"mode": "threads (one handle + stream + host thread per environment)", "envs": E,
+                     "env_steps_per_s": round(E * args.steps / dt, 1),
                      "ms_per_env_step": round(1e3 * dt / args.steps, 3),
                      "iters_per_solve": round(sum(its) / (2.0 * E * args.steps), 1)})
         pool.close()
+        # the same work through the batched entry points: ONE host thread, one launch per solver pass for all E
+        grids = [api.Grid(n, n, n, 1.0 / n) for _ in range(E)]
+        for g in grids:
+            g.set_domain_bc(0, 1, 1.0)
+            g.set_domain_bc(1, 1, 0.0)
+        ps = [torch.zeros(g.shape_p, dtype=torch.float32, device="cuda") for g in grids]
+        ys = [torch.zeros(g.shape_p, dtype=torch.float32, device="cuda") for g in grids]
+
+        def batched(reps, lo=0, hi=None):
+            hi = E if hi is None else hi
+            gg, its = grids[lo:hi], 0
+            for _ in range(reps):
+                V = [[a.clone() for a in U0[e]] for e in range(lo, hi)]
+                for g in gg:
+                    g.set_solid(phi)
+                api.project_batch(gg, V, ps[lo:hi], tol=TOL, maxit=MAXIT)
+                its += sum(g.last_solve_info()["iters"] for g in gg)
+                api.project_adjoint_batch(gg, V, ys[lo:hi], p_saved=ps[lo:hi], uhat=U0[lo:hi], tol=TOL, maxit=MAXIT)
+                its += sum(g.last_solve_info()["iters"] for g in gg)
+            torch.cuda.current_stream().synchronize()
+            return its
+        batched(max(args.warmup, 3))
+        l0 = sum(g.launch_count() for g in grids)
+        t0 = time.perf_counter()
+        its = batched(args.steps)
+        dt = time.perf_counter() - t0
+        rows.append({"mode": "batched (nf_project_batch / nf_project_adjoint_batch, one host thread)", "envs": E,
+                     "env_steps_per_s": round(E * args.steps / dt, 1),
+                     "ms_per_env_step": round(1e3 * dt / args.steps, 3),
+                     "iters_per_solve": round(its / (2.0 * E * args.steps), 1),
+                     "launches_per_env_step": round((sum(g.launch_count() for g in grids) - l0) / (E * args.steps), 1)})
+        # groups of batched environments on their own streams / host threads: one group's nf_set_solid passes overlap
+        # another group's solver passes
+        for per in (2, 4, 8):
+            if E < 2 * per:
+                continue
+            import threading
+            T = E // per
+            streams = [torch.cuda.Stream() for _ in range(T)]
+
+            def grouped(reps):
+                out = [0] * T
+
+                def work(t):
+                    with torch.cuda.stream(streams[t]):
+                        out[t] = batched(reps, t * per, (t + 1) * per)
+                th = [threading.Thread(target=work, args=(t,)) for t in range(T)]
+                for x in th:
+                    x.start()
+                for x in th:
+                    x.join()
+                return sum(out)
+            torch.cuda.synchronize()
+            grouped(max(args.warmup, 3))
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            its = grouped(args.steps)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            rows.append({"mode": "batched groups of %d, one stream + host thread per group" % per, "envs": T * per,
+                         "env_steps_per_s": round(T * per * args.steps / dt, 1),
+                         "ms_per_env_step": round(1e3 * dt / args.steps, 3),
+                         "iters_per_solve": round(its / (2.0 * T * per * args.steps), 1)})
+        for g in grids:
+            g.close()
     print(json.dumps({"workload": "NEXT-4 concurrent environments, %d^3 sphere-in-channel, forward + adjoint projection "
                                   "to %g (wall clock over all environments, host threads included)" % (n, TOL),
                       "dtype": "f32", "rows": rows}))

@@ -129,6 +129,27 @@ int nf_project_adjoint(nf_grid *g, float *gu, float *gv, float *gw, const float 
                        float *galpha_u, float *galpha_v, float *galpha_w,
                        float *gus_u, float *gus_v, float *gus_w, float *y_out, float tol, int maxit);
 
+/* ---- NEXT-4  Batched small grids (Table 1: the paper's tasks are 40^3-48^3 grids,
+ * far too small to fill a B200 one at a time; L145 "gym-like" environments) --------------------------------------------
+ * n handles of EQUAL extents on ONE stream, each with its own solid, boundary values and fields: nf_solve /
+ * nf_project / nf_project_adjoint for all of them, with every pass of a PCG iteration issued as ONE kernel launch for
+ * the whole batch (blockIdx.z = environment x z-chunk; one cooperative coarse-level launch, barriers per environment).
+ * The PCG scalars, the convergence test (R11, relative to each environment's own ||b||) and the early exit stay per
+ * environment; the host loop ends when all have converged.  x0 = 0, single-phase PCG on the recursive residual (no
+ * fp64 refresh: these grids are far above the fp32 storage floor of DESIGN.md section 7).  Handles the batched kernels
+ * cannot take (unequal extents, ragged levels, test hooks, more cooperative CTAs than SMs) are solved one at a time
+ * inside the same call -- same results.  Arguments are HOST arrays of n device pointers, meanings as in the
+ * single-handle calls; y (the adjoint variable, n cell arrays) is required.  status (may be NULL): NF_OK /
+ * NF_NOT_CONVERGED per environment; the return value is the worst of them, or a negative error. */
+int nf_solve_batch(nf_grid *const *g, int n, const float *const *rhs, float *const *p, float tol, int maxit, int *status);
+int nf_project_batch(nf_grid *const *g, int n, float *const *u, float *const *v, float *const *w, float *const *p,
+                     float tol, int maxit, int *status);
+int nf_project_adjoint_batch(nf_grid *const *g, int n, float *const *gu, float *const *gv, float *const *gw,
+                             const float *const *p_saved, const float *const *uhat_u, const float *const *uhat_v,
+                             const float *const *uhat_w, float *const *galpha_u, float *const *galpha_v,
+                             float *const *galpha_w, float *const *gus_u, float *const *gus_v, float *const *gus_w,
+                             float *const *y, float tol, int maxit, int *status);
+
 /* a-8  Semi-Lagrangian advection (Eq. 2; L353-357 Eqs. 11-12; R14, R20): for every face
  * position x of component c: v0 = U(x); x_m = x - dt/2 v0; v_m = U(x_m); x_b = x - dt v_m;
  * out_c = U_c(x_b), U(.) = per-component trilinear interpolation, positions clamped to the lattice.

@@ -32,6 +32,12 @@ _SIGNATURES = {
     "nf_solve": (ctypes.c_int, [ctypes.c_void_p, _c_float_p, _c_float_p, ctypes.c_float, ctypes.c_int]),
     "nf_project": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4 + [ctypes.c_float, ctypes.c_int]),
     "nf_project_adjoint": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 14 + [ctypes.c_float, ctypes.c_int]),
+    "nf_solve_batch": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_float,
+                                      ctypes.c_int, ctypes.POINTER(ctypes.c_int)]),
+    "nf_project_batch": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 4 +
+                         [ctypes.c_float, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]),
+    "nf_project_adjoint_batch": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 14 +
+                                 [ctypes.c_float, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]),
     "nf_advect": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.c_float]),
     "nf_max_speed": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.POINTER(ctypes.c_float)]),
     "nf_viscosity": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3 + [ctypes.c_float, ctypes.c_float]),
@@ -442,3 +448,55 @@ class Grid:
 
     def launch_count(self):
         return int(self.lib.nf_launch_count(self.h))
+
+
+# ---- batched entry points (include/nf.h "NEXT-4"): n grids of equal extents on one stream ---------------------------------
+def _ptr_array(tensors):
+    """HOST array of device addresses (None -> NULL array)."""
+    if tensors is None:
+        return None
+    arr = (ctypes.c_void_p * len(tensors))()
+    for i, t in enumerate(tensors):
+        arr[i] = _ptr(t).value if t is not None else None
+    return arr
+
+
+def _batch_prologue(grids):
+    import torch
+    g0 = grids[0]
+    if any(g.device != g0.device for g in grids):
+        raise ValueError("a batch lives on one device")
+    for g in grids:
+        g._bind_stream()  # every handle of the batch on the current torch stream
+    h = (ctypes.c_void_p * len(grids))(*[g.h for g in grids])
+    return g0, h, (ctypes.c_int * len(grids))()
+
+
+def solve_batch(grids, rhs, p, tol=1e-6, maxit=200):
+    """nf_solve_batch: rhs, p = lists of n cell tensors.  Returns the list of per-grid status codes."""
+    g0, h, st = _batch_prologue(grids)
+    rc = g0.lib.nf_solve_batch(h, len(grids), _ptr_array(rhs), _ptr_array(p), float(tol), int(maxit), st)
+    g0._check(rc, "nf_solve_batch")
+    return list(st)
+
+
+def project_batch(grids, U, p, tol=1e-6, maxit=200):
+    """nf_project_batch: U = list of n (u, v, w) triples (in place), p = list of n cell tensors."""
+    g0, h, st = _batch_prologue(grids)
+    rc = g0.lib.nf_project_batch(h, len(grids), _ptr_array([a[0] for a in U]), _ptr_array([a[1] for a in U]),
+                                 _ptr_array([a[2] for a in U]), _ptr_array(p), float(tol), int(maxit), st)
+    g0._check(rc, "nf_project_batch")
+    return list(st)
+
+
+def project_adjoint_batch(grids, G, y, p_saved=None, uhat=None, galpha=None, gus=None, tol=1e-6, maxit=200):
+    """nf_project_adjoint_batch: G = list of n (gu, gv, gw) triples (in place: dJ/dU -> dJ/dUhat), y = list of n cell
+    tensors (the adjoint variable, required); p_saved / uhat / galpha / gus: lists as in Grid.project_adjoint or None."""
+    g0, h, st = _batch_prologue(grids)
+    col = lambda L, c: None if L is None else _ptr_array([a[c] for a in L])
+    rc = g0.lib.nf_project_adjoint_batch(h, len(grids), col(G, 0), col(G, 1), col(G, 2), _ptr_array(p_saved),
+                                         col(uhat, 0), col(uhat, 1), col(uhat, 2), col(galpha, 0), col(galpha, 1),
+                                         col(galpha, 2), col(gus, 0), col(gus, 1), col(gus, 2), _ptr_array(y),
+                                         float(tol), int(maxit), st)
+    g0._check(rc, "nf_project_adjoint_batch")
+    return list(st)

@@ -119,3 +119,68 @@ def project(grid, u, v, w, phi, us=None, vs=None, ws=None, tol=1e-6, maxit=400):
 def geom_sdf(grid, params, K, N, M, complement=False):
     """phi on the nodes from a parameter tensor (any device; the gradient comes back on the same device / dtype)."""
     return _GeomSdf.apply(grid, K, N, M, complement, params)
+
+
+class _ProjectBatch(torch.autograd.Function):
+    """nf_set_solid per environment + nf_project_batch; backward: nf_project_adjoint_batch + nf_weights_adjoint.
+    Flat argument list: for every environment u, v, w, phi, us, vs, ws (the solid velocities may be None)."""
+
+    @staticmethod
+    def forward(ctx, grids, tol, maxit, *flat):
+        from . import api
+        n = len(grids)
+        ctx.grids, ctx.tol, ctx.maxit = grids, float(tol), int(maxit)
+        envs = [flat[7 * e: 7 * e + 7] for e in range(n)]
+        outs, ps, saved, has_us = [], [], [], []
+        for g, (u, v, w, phi, us, vs, ws) in zip(grids, envs):
+            solid = [None if a is None else a.detach().contiguous() for a in (us, vs, ws)]
+            phi_c = phi.detach().contiguous()
+            g.set_solid(phi_c, *solid)
+            uhat = [a.detach().contiguous() for a in (u, v, w)]
+            outs.append([a.clone() for a in uhat])
+            ps.append(torch.zeros(g.shape_p, dtype=torch.float32, device=uhat[0].device))
+            has_us.append([a is not None for a in solid])
+            saved += [phi_c] + uhat + [a for a in solid if a is not None]
+        api.project_batch(grids, outs, ps, tol=ctx.tol, maxit=ctx.maxit)
+        ctx.has_us = has_us
+        ctx.save_for_backward(*(ps + saved))
+        ctx.mark_non_differentiable(*ps)
+        return tuple(a for o in outs for a in o) + tuple(ps)
+
+    @staticmethod
+    def backward(ctx, *grads):
+        from . import api
+        grids, n = ctx.grids, len(ctx.grids)
+        saved = list(ctx.saved_tensors)
+        ps, rest = saved[:n], saved[n:]
+        phis, uhats, solids = [], [], []
+        for e in range(n):
+            phis.append(rest.pop(0))
+            uhats.append([rest.pop(0) for _ in range(3)])
+            solids.append([rest.pop(0) if h else None for h in ctx.has_us[e]])
+        G, ga, gs, ys = [], [], [], []
+        for e, g in enumerate(grids):
+            g.set_solid(phis[e], *solids[e])  # (a handle holds one geometry at a time: the one of this step)
+            G.append([_dense(grads[3 * e + c], uhats[e][c]) for c in range(3)])
+            ga.append([torch.empty_like(a) for a in uhats[e]])
+            gs.append([torch.empty_like(a) for a in uhats[e]])
+            ys.append(torch.zeros_like(ps[e]))
+        api.project_adjoint_batch(grids, G, ys, p_saved=ps, uhat=uhats, galpha=ga, gus=gs, tol=ctx.tol, maxit=ctx.maxit)
+        out = []
+        for e, g in enumerate(grids):
+            gphi = torch.empty_like(phis[e])
+            g.weights_adjoint(*ga[e], gphi)
+            out += G[e] + [gphi] + [b if h else None for b, h in zip(gs[e], ctx.has_us[e])]
+        return (None, None, None) + tuple(out)
+
+
+def project_batch(grids, U, phi, us=None, tol=1e-6, maxit=400):
+    """Batched projection of n environments (include/nf.h nf_project_batch): U = list of (u, v, w), phi = list of node
+    SDFs, us = list of (us, vs, ws) triples / None.  -> (list of (u, v, w), list of p); differentiable like project()."""
+    n = len(grids)
+    flat = []
+    for e in range(n):
+        s = (None, None, None) if us is None or us[e] is None else tuple(us[e])
+        flat += list(U[e]) + [phi[e]] + list(s)
+    out = _ProjectBatch.apply(list(grids), tol, maxit, *flat)
+    return [tuple(out[3 * e: 3 * e + 3]) for e in range(n)], list(out[3 * n:])

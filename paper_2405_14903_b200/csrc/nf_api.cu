@@ -1,5 +1,6 @@
 // nf_api.cu -- the C ABI (include/nf.h): handle management, argument checking, and the composition of the
 // hot-path calls from the kernels in nf_weights.cu / nf_solver.cu / nf_project.cu / nf_advect.cu.
+#include <algorithm>
 #include <new>
 
 #include "nf_internal.cuh"
@@ -27,10 +28,12 @@ static void free_all(nf_grid *g) {
   cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
   cudaFree(g->st); cudaFree(g->d_counts); cudaFree(g->geom_par); cudaFree(g->geom_grad);
   nf_components_free(g);
+  nf_mg_free_batch(g);
   if (g->hst) cudaFreeHost((void *)g->hst);
   if (g->h_counts) cudaFreeHost(g->h_counts);
   if (g->ev0) cudaEventDestroy(g->ev0);
   if (g->ev1) cudaEventDestroy(g->ev1);
+  if (g->ev_meta) cudaEventDestroy(g->ev_meta);
   for (cudaEvent_t e : g->prof_pool) cudaEventDestroy(e);
   if (g->hs_u) {
     cudaStreamDestroy(g->s_h2d); cudaStreamDestroy(g->s_d2h);
@@ -54,6 +57,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->nu_pre = 1; g->nu_post = 1; g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->singular_info = 1; g->nact = 0; g->ncomp = 0; g->nsing = 0; g->gauge_mode = 1;
+  g->d_coarse = nullptr; g->h_coarse = nullptr; g->cbar = nullptr; g->cbar_count = 0; g->meta_pending = false;
   g->comp = nullptr; g->cc_cnt = nullptr; g->cc_regular = nullptr; g->cc_sums = nullptr; g->cc_meta = nullptr; g->h_cc_meta = nullptr;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
   g->prof_on = false;
@@ -121,6 +125,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   ok = ok && cudaHostGetDevicePointer((void **)&g->hst_dev, (void *)g->hst, 0) == cudaSuccess;
   ok = ok && cudaHostAlloc((void **)&g->h_counts, 2 * sizeof(double), cudaHostAllocDefault) == cudaSuccess;
   ok = ok && cudaEventCreate(&g->ev0) == cudaSuccess && cudaEventCreate(&g->ev1) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&g->ev_meta, cudaEventDisableTiming) == cudaSuccess;
   if (ok) {
     for (int s = 0; s < NF_RING; ++s) { g->hst[s].seq = 0; g->hst[s].done = 0; g->hst[s].converged = 0; }
     ok = nf_solver_init(g) == NF_OK;
@@ -204,6 +209,7 @@ extern "C" int nf_set_solid_velocity(nf_grid *g, const float *us, const float *v
 
 static int solve_timed(nf_grid *g, const float *src, float *x, float tol, int maxit, bool warm) {
   if (!(tol > 0.0f) || maxit < 1) return NF_ERR_INVALID;
+  NF_TRY(nf_meta_sync(g));
   NF_CUDA(g, cudaEventRecord(g->ev0, g->stream));
   NF_TRY(nf_solve_prepare_from(g, src, tol, maxit));
   int rc = nf_solve_run(g, x, tol, maxit, warm);
@@ -249,6 +255,101 @@ extern "C" int nf_project_adjoint(nf_grid *g, float *gu, float *gv, float *gw, c
   NF_TRY(nf_adjoint_finish_impl(g, gu, gv, gw, y, p_saved, uhat_u, uhat_v, uhat_w, galpha_u, galpha_v, galpha_w,
                                 gus_u, gus_v, gus_w));
   return rc;
+}
+
+// ---- batched entry points ------------------------------------------------------------------
+// Groups of environments the batched kernels can take (equal extents, one stream, fused path, cooperative grid resident);
+// anything else is solved one handle at a time -- the results are the same, only the number of launches differs.
+template <class PRE, class POST>
+static int batch_drive(nf_grid *const *gs, int n, float *const *x, float tol, int maxit, int *status, PRE pre, POST post) {
+  if (!gs || n < 1 || !x || !(tol > 0.0f) || maxit < 1) return NF_ERR_INVALID;
+  for (int e = 0; e < n; ++e) {
+    if (!gs[e] || !x[e]) return NF_ERR_INVALID;
+    gs[e]->err.clear();
+    if (!gs[e]->weights_set) return NF_ERR_STATE;
+  }
+  for (int e = 0; e < n; ++e) NF_TRY(nf_meta_sync(gs[e]));
+  int worst = NF_OK;
+  int sms = 148, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  int e0 = 0;
+  while (e0 < n) {
+    int cnt = std::min(n - e0, NF_BATCH_MAX);
+    if (gs[e0]->coarse_ctas > 0) cnt = std::min(cnt, std::max(1, sms / gs[e0]->coarse_ctas));
+    nf_grid *G[NF_BATCH_MAX];
+    float *X[NF_BATCH_MAX];
+    int st[NF_BATCH_MAX];
+    for (int e = 0; e < cnt; ++e) { G[e] = gs[e0 + e]; X[e] = x[e0 + e]; st[e] = NF_OK; }
+    for (int e = 0; e < cnt; ++e) NF_TRY(pre(e0 + e));  // right-hand sides into lv[0].r
+    if (cnt > 1 && nf_batch_ok(G, cnt)) {
+      NF_TRY(nf_solve_batch_impl(G, cnt, nullptr, X, tol, maxit, st));
+    } else {
+      for (int e = 0; e < cnt; ++e) {
+        NF_TRY(nf_solve_prepare_from(G[e], nullptr, tol, maxit));
+        int rc = nf_solve_run(G[e], X[e], tol, maxit, false);
+        if (rc < 0) return rc;
+        st[e] = rc;
+      }
+    }
+    for (int e = 0; e < cnt; ++e) {
+      NF_TRY(post(e0 + e));
+      if (status) status[e0 + e] = st[e];
+      worst = std::max(worst, st[e]);
+    }
+    e0 += cnt;
+  }
+  return worst;
+}
+
+extern "C" int nf_solve_batch(nf_grid *const *g, int n, const float *const *rhs, float *const *p, float tol, int maxit,
+                              int *status) {
+  if (!rhs) return NF_ERR_INVALID;
+  return batch_drive(g, n, p, tol, maxit, status,
+                     [&](int e) -> int {
+                       if (!rhs[e] || rhs[e] == p[e]) return NF_ERR_INVALID;
+                       nf_grid *h = g[e];
+                       NF_CUDA(h, cudaMemcpyAsync(h->lv[0].r, rhs[e], nf_nc(h) * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+                       return NF_OK;
+                     },
+                     [&](int) -> int { return NF_OK; });
+}
+
+extern "C" int nf_project_batch(nf_grid *const *g, int n, float *const *u, float *const *v, float *const *w,
+                                float *const *p, float tol, int maxit, int *status) {
+  if (!u || !v || !w) return NF_ERR_INVALID;
+  return batch_drive(g, n, p, tol, maxit, status,
+                     [&](int e) -> int {
+                       if (!u[e] || !v[e] || !w[e]) return NF_ERR_INVALID;
+                       return nf_rhs_impl(g[e], u[e], v[e], w[e]);
+                     },
+                     [&](int e) -> int { return nf_grad_subtract_impl(g[e], u[e], v[e], w[e], p[e]); });
+}
+
+extern "C" int nf_project_adjoint_batch(nf_grid *const *g, int n, float *const *gu, float *const *gv, float *const *gw,
+                                        const float *const *p_saved, const float *const *uhat_u,
+                                        const float *const *uhat_v, const float *const *uhat_w, float *const *galpha_u,
+                                        float *const *galpha_v, float *const *galpha_w, float *const *gus_u,
+                                        float *const *gus_v, float *const *gus_w, float *const *y, float tol, int maxit,
+                                        int *status) {
+  if (!gu || !gv || !gw || !y) return NF_ERR_INVALID;
+  const bool want_ga = galpha_u || galpha_v || galpha_w;
+  if (want_ga && !(galpha_u && galpha_v && galpha_w && p_saved && uhat_u && uhat_v && uhat_w)) return NF_ERR_INVALID;
+  const bool want_gs = gus_u || gus_v || gus_w;
+  if (want_gs && !(gus_u && gus_v && gus_w)) return NF_ERR_INVALID;
+  return batch_drive(g, n, y, tol, maxit, status,
+                     [&](int e) -> int {
+                       if (!gu[e] || !gv[e] || !gw[e]) return NF_ERR_INVALID;
+                       return nf_adjoint_rhs_impl(g[e], gu[e], gv[e], gw[e]);
+                     },
+                     [&](int e) -> int {
+                       return nf_adjoint_finish_impl(g[e], gu[e], gv[e], gw[e], y[e], want_ga ? p_saved[e] : nullptr,
+                                                     want_ga ? uhat_u[e] : nullptr, want_ga ? uhat_v[e] : nullptr,
+                                                     want_ga ? uhat_w[e] : nullptr, want_ga ? galpha_u[e] : nullptr,
+                                                     want_ga ? galpha_v[e] : nullptr, want_ga ? galpha_w[e] : nullptr,
+                                                     want_gs ? gus_u[e] : nullptr, want_gs ? gus_v[e] : nullptr,
+                                                     want_gs ? gus_w[e] : nullptr);
+                     });
 }
 
 extern "C" int nf_viscosity(nf_grid *g, float *u, float *v, float *w, float nu, float dt) {
@@ -336,6 +437,7 @@ extern "C" int nf_vcycle(nf_grid *g, const float *r, float *z) {
   NF_CHECK_HANDLE(g);
   if (!r || !z) return NF_ERR_INVALID;
   if (!g->weights_set) return NF_ERR_STATE;
+  NF_TRY(nf_meta_sync(g));
   const size_t bytes = nf_nc(g) * sizeof(float);
   NF_CUDA(g, cudaMemcpyAsync(g->lv[0].r, r, bytes, cudaMemcpyDeviceToDevice, g->stream));
   NF_TRY(nf_vcycle_impl(g, false, 0));
@@ -449,6 +551,7 @@ extern "C" int nf_last_solve_info(nf_grid *g, int *iters, float *relres, float *
 
 extern "C" int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, int *singular) {
   NF_CHECK_HANDLE(g);
+  if (g->weights_set) NF_TRY(nf_meta_sync(g));
   if (levels) *levels = g->nlev;
   if (active_cells) *active_cells = g->weights_set ? g->nact : -1;
   if (singular) *singular = g->weights_set ? g->singular_info : -1;
@@ -458,6 +561,7 @@ extern "C" int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, in
 extern "C" int nf_grid_components(nf_grid *g, int *components, int *singular_components) {
   NF_CHECK_HANDLE(g);
   if (!g->weights_set) return NF_ERR_STATE;
+  NF_TRY(nf_meta_sync(g));
   if (components) *components = g->ncomp;
   if (singular_components) *singular_components = g->nsing;
   return NF_OK;

@@ -82,6 +82,25 @@ struct NfHostStatus {  // written by the device into mapped pinned memory
   volatile float relres;
 };
 
+// One environment of a batched PCG iteration (nf_solver.cu: nf_solve_batch_run): the level-0
+// operator, its CG vectors and scalars, and the first coarse level's r / z.  p[s], r[s]: the buffer that iteration
+// parity s WRITES (the search direction and the residual ping-pong between two buffers each).
+#define NF_BATCH_MAX 16
+struct NfEnvK {
+  NfLvK L;
+  float *z, *q, *x;
+  float *p[2], *r[2];
+  float *rc, *zc;
+  NfSolveState *st;
+  NfHostStatus *hs;
+};
+struct NfBatchK {
+  int n;    // environments in this launch (<= NF_BATCH_MAX)
+  int nzc;  // z-chunks (CTAs along blockIdx.z) per environment
+  int cnx, cny, cnz;  // extents of the first coarse level
+  NfEnvK e[NF_BATCH_MAX];
+};
+
 // limits of the parametric geometry (nf_geom.cu): K key sections, N curves per section, N*M polygon edges
 #define NF_GEOM_MAXK 64
 #define NF_GEOM_MAXN 64
@@ -127,6 +146,12 @@ struct nf_grid {
   float *b0;  // the prepared right-hand side (kept for the true-residual refresh, nf_solver.cu)
   float *p, *p2, *q, *xtmp;  // p / p2: the search direction ping-pongs between two buffers (k_papply4)
   float *tailpack;  // 8 floats per cell of the tail levels (nf_mg.cu)
+  bool meta_pending;     // the counts of the last hierarchy build have not been read yet (nf_meta_sync)
+  cudaEvent_t ev_meta, ev_coarse;
+  void *h_coarse;        // pinned staging of d_coarse
+  void *d_coarse;        // device copy of the coarse kernel's level table (batched launches, nf_mg.cu)
+  unsigned *cbar;        // per-environment barrier counter of k_vcoarse_b
+  unsigned cbar_count;   // its value after everything enqueued so far
   float *tailinv;   // inverse of the coarsest level's operator (n <= 128 cells: n^2 floats; k_coarse_inverse)
   // scratch face arrays (advection copy / adjoint staging)
   float *fu, *fv, *fw;
@@ -241,6 +266,7 @@ int nf_weights_from_sdf(nf_grid *g, const float *sdf);
 int nf_weights_from_user(nf_grid *g, const float *au, const float *av, const float *aw);
 int nf_weights_to_user(nf_grid *g, float *au, float *av, float *aw);
 int nf_build_hierarchy(nf_grid *g);  // coarse weights + active count + singular flag
+int nf_meta_sync(nf_grid *g);        // wait for / read the counts of the last hierarchy build
 int nf_store_solid_velocity(nf_grid *g, const float *us, const float *vs, const float *ws);
 int nf_weights_adjoint_impl(nf_grid *g, const float *gau, const float *gav, const float *gaw, float *gsdf);
 // nf_components.cu
@@ -254,6 +280,10 @@ int nf_apply_A_impl(nf_grid *g, const float *p, float *q);
 void nf_mg_plan(nf_grid *g);      // choose the shared-memory tail and the vec levels (after the level extents are known)
 int nf_mg_init(nf_grid *g);       // kernel attributes
 int nf_mg_pack_tail(nf_grid *g);  // packed operator of the tail levels from the current weights
+int nf_mg_upload_coarse(nf_grid *g);  // device copy of the coarse kernel's level table (after every hierarchy build)
+void nf_mg_free_batch(nf_grid *g);
+int nf_vcycle_batch(nf_grid **G, int n, const NfBatchK &B, int slot);
+int nf_update_down1_batch(nf_grid **G, int n, const NfBatchK &B, int slot, int seq);
 int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1 = false);  // z = M^{-1} r on lv[0].r -> lv[0].z
 // fused r' = r - a q + pre-smoother of level 0 (r' into g->r_alt, then the two buffers swap); false if not applicable
 bool nf_update_down1_ok(const nf_grid *g);
@@ -263,6 +293,8 @@ int nf_solver_init(nf_grid *g);                          // kernel attributes (o
 int nf_solve_prepare(nf_grid *g, float tol, int maxit);  // from lv[0].r: mask, mean removal, bb
 int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit);
 int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm);  // warm: x holds the initial guess
+bool nf_batch_ok(nf_grid **G, int n);  // the n handles can be solved by the batched kernels
+int nf_solve_batch_impl(nf_grid **G, int n, const float *const *src, float *const *x, float tol, int maxit, int *status);
 // nf_project.cu
 int nf_rhs_impl(nf_grid *g, const float *u, const float *v, const float *w);  // -> lv[0].r
 int nf_grad_subtract_impl(nf_grid *g, float *u, float *v, float *w, const float *p);

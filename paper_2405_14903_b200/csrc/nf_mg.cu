@@ -16,6 +16,7 @@
 //   * k_tail: all levels that fit one CTA's shared memory (<= 5632 cells in total), whole sub-V-cycle in one launch.
 #include <cooperative_groups.h>
 #include <algorithm>
+#include <cstring>
 
 #include "nf_stencil.cuh"
 
@@ -117,13 +118,14 @@ __device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, fl
 // and its neighbour rows, ||r'||^2, and the pre-smoother z = smooth(r') in the same pass: 17 B/cell (r, q, code in;
 // r', z out) instead of 12 + 9, and one kernel's fixed cost less per iteration.  r' goes to a second buffer (the
 // neighbours' threads still read r).  The last CTA to finish runs the convergence check (nf_cg_check).
-__global__ void __launch_bounds__(256, 4) k_update_down1(NfLvK L, const float *__restrict__ rold,
-                                                      const float *__restrict__ q, float *__restrict__ rnew,
-                                                      float *__restrict__ z, int kch, NfSolveState *st, int slot,
-                                                      NfHostStatus *hs, int seq) {
-  nf_pdl_enter();
+// (bz, nzc: this CTA's z-chunk and the number of z-chunks of ITS grid -- blockIdx.z / gridDim.z, or the environment's
+// share of them in a batched launch)
+__device__ __forceinline__ void nf_update_down1_body(const NfLvK &L, const float *__restrict__ rold,
+                                                     const float *__restrict__ q, float *__restrict__ rnew,
+                                                     float *__restrict__ z, int kch, NfSolveState *st, int slot,
+                                                     NfHostStatus *hs, int seq, int bz, int nzc) {
   if (st->done) {  // (uniform: done is only ever set by the last CTA of an earlier launch)
-    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0 && threadIdx.y == 0)
+    if (blockIdx.x == 0 && blockIdx.y == 0 && bz == 0 && threadIdx.x == 0 && threadIdx.y == 0)
       nf_cg_check(st, slot, hs, seq);
     return;
   }
@@ -140,7 +142,7 @@ __global__ void __launch_bounds__(256, 4) k_update_down1(NfLvK L, const float *_
       return v;
     };
     auto R1 = [&](nf_idx at, bool ok) { return nf_ld1(rold, at, ok) - a * nf_ld1(q, at, ok); };
-    const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, L.nz);
+    const int k0 = bz * kch, k1 = min(k0 + kch, L.nz);
     for (int k = k0; k < k1; ++k) {
       const float4 c = ((j + k) & 1) ? nf_down1_core<1>(L, R4, R1, z, i0, j, k) : nf_down1_core<0>(L, R4, R1, z, i0, j, k);
       *reinterpret_cast<float4 *>(rnew + ((nf_idx)k * L.ny + j) * L.nx + i0) = c;
@@ -150,7 +152,7 @@ __global__ void __launch_bounds__(256, 4) k_update_down1(NfLvK L, const float *_
   nf_block_atomic_add((double)part, &st->rr[slot]);
   if (threadIdx.x == 0 && threadIdx.y == 0) {
     __threadfence();
-    const unsigned total = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned total = gridDim.x * gridDim.y * (unsigned)nzc;
     const unsigned t = atomicAdd(&st->ticket, 1u);
     if (t == total - 1) {
       st->ticket = 0;
@@ -158,6 +160,21 @@ __global__ void __launch_bounds__(256, 4) k_update_down1(NfLvK L, const float *_
       nf_cg_check(st, slot, hs, seq);
     }
   }
+}
+__global__ void __launch_bounds__(256, 4) k_update_down1(NfLvK L, const float *__restrict__ rold,
+                                                      const float *__restrict__ q, float *__restrict__ rnew,
+                                                      float *__restrict__ z, int kch, NfSolveState *st, int slot,
+                                                      NfHostStatus *hs, int seq) {
+  nf_pdl_enter();
+  nf_update_down1_body(L, rold, q, rnew, z, kch, st, slot, hs, seq, (int)blockIdx.z, (int)gridDim.z);
+}
+// Batched launches: blockIdx.z = env * nzc + z-chunk; see k_papply4_b (nf_solver.cu)
+__global__ void __launch_bounds__(256, 4) k_update_down1_b(const __grid_constant__ NfBatchK B, int kch, int slot,
+                                                        int seq) {
+  nf_pdl_enter();
+  const int e = (int)blockIdx.z / B.nzc, bz = (int)blockIdx.z - e * B.nzc;
+  const NfEnvK &E = B.e[e];
+  nf_update_down1_body(E.L, E.r[0], E.q, E.r[1], E.z, kch, E.st, slot, E.hs, seq, bz, B.nzc);
 }
 
 __global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restrict__ r, float *__restrict__ z, int kch,
@@ -244,6 +261,18 @@ __global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restri
   } else {
     for (int K = K0; K < K1; ++K) nf_down2_body<1>(L, z, rc, cnx, cny, i0, J, K);
   }
+}
+
+__global__ void __launch_bounds__(256, 4) k_down2_b(const __grid_constant__ NfBatchK B) {
+  nf_pdl_enter();
+  const int e = (int)blockIdx.z / B.nzc, K = (int)blockIdx.z - e * B.nzc;  // (one coarse plane per CTA: nzc = cnz)
+  const NfEnvK &E = B.e[e];
+  if (E.st->done) return;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int J = blockIdx.y * blockDim.y + threadIdx.y;
+  if (i0 >= E.L.nx || J >= B.cny) return;
+  if (E.L.fz == 2) nf_down2_body<2>(E.L, E.z, E.rc, B.cnx, B.cny, i0, J, K);
+  else nf_down2_body<1>(E.L, E.z, E.rc, B.cnx, B.cny, i0, J, K);
 }
 
 // z + P z_coarse on a row of 4 fine cells
@@ -335,6 +364,27 @@ __global__ void __launch_bounds__(256, 4) k_up1(NfLvK L, float *z, const float *
   }
 }
 
+__global__ void __launch_bounds__(256, 4) k_up1_b(const __grid_constant__ NfBatchK B, int kch) {
+  nf_pdl_enter();
+  const int e = (int)blockIdx.z / B.nzc, bz = (int)blockIdx.z - e * B.nzc;
+  const NfEnvK &E = B.e[e];
+  if (E.st->done) return;
+  const NfLvK &L = E.L;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  if (i0 >= L.nx || j >= L.ny) return;
+  const int k0 = bz * kch, k1 = min(k0 + kch, L.nz);
+  for (int k = k0; k < k1; ++k) {
+    if (L.fz == 2) {
+      if ((j + k) & 1) nf_up1_body<1, 2>(L, E.z, E.r[0], E.zc, B.cnx, B.cny, i0, j, k);
+      else nf_up1_body<0, 2>(L, E.z, E.r[0], E.zc, B.cnx, B.cny, i0, j, k);
+    } else {
+      if ((j + k) & 1) nf_up1_body<1, 1>(L, E.z, E.r[0], E.zc, B.cnx, B.cny, i0, j, k);
+      else nf_up1_body<0, 1>(L, E.z, E.r[0], E.zc, B.cnx, B.cny, i0, j, k);
+    }
+  }
+}
+
 // Red half sweep in place (black neighbours are final); returns r.z over the 4 cells.
 template <int PAR>
 __device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const float *r, int i0, int j, int k) {
@@ -391,6 +441,22 @@ __global__ void __launch_bounds__(256, 4) k_up2(NfLvK L, float *z, const float *
       dot += ((j + k) & 1) ? nf_up2_body<1>(L, z, r, i0, j, k) : nf_up2_body<0>(L, z, r, i0, j, k);
   }
   if (DOT) nf_block_atomic_add((double)dot, &st->rz[slot]);
+}
+__global__ void __launch_bounds__(256, 4) k_up2_b(const __grid_constant__ NfBatchK B, int kch, int slot) {
+  nf_pdl_enter();
+  const int e = (int)blockIdx.z / B.nzc, bz = (int)blockIdx.z - e * B.nzc;
+  const NfEnvK &E = B.e[e];
+  if (E.st->done) return;  // (uniform over the environment's CTAs)
+  const NfLvK &L = E.L;
+  const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  float dot = 0.0f;
+  if (i0 < L.nx && j < L.ny) {
+    const int k0 = bz * kch, k1 = min(k0 + kch, L.nz);
+    for (int k = k0; k < k1; ++k)
+      dot += ((j + k) & 1) ? nf_up2_body<1>(L, E.z, E.r[0], i0, j, k) : nf_up2_body<0>(L, E.z, E.r[0], i0, j, k);
+  }
+  nf_block_atomic_add((double)dot, &E.st->rz[slot]);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -998,16 +1064,14 @@ struct NfCoarseK {
   const float *minv;  // inverse of the coarsest operator (k_coarse_inverse)
 };
 
-__global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_constant__ NfCoarseK P,
-                                                                 const NfSolveState *st) {
-  if (st && st->done) return;  // (uniform over the grid: written by an earlier kernel)
-  extern __shared__ __align__(16) float sm[];
-  __shared__ unsigned long long mbar;
-  if (P.has_tail && blockIdx.x == 0 && threadIdx.x == 0) nf_tail_prefetch(P.T, P.pack, P.minv, sm, &mbar);
-  cg::grid_group grid = cg::this_grid();
+// The body: `cta` of `nctas` CTAs work on one environment's coarse levels; SYNC() is the barrier among exactly those.
+template <class SYNC>
+__device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int nctas, float *sm,
+                                                unsigned long long *mbar, SYNC sync) {
+  if (P.has_tail && cta == 0 && threadIdx.x == 0) nf_tail_prefetch(P.T, P.pack, P.minv, sm, mbar);
   // task index: warps are dealt round-robin over the CTAs so that a small level still spreads over every SM
-  const int gn = gridDim.x * blockDim.x;  // (tasks < 2^31)
-  const int gt = ((threadIdx.x >> 5) * gridDim.x + blockIdx.x) * 32 + (threadIdx.x & 31);
+  const int gn = nctas * blockDim.x;  // (tasks < 2^31)
+  const int gt = ((threadIdx.x >> 5) * nctas + cta) * 32 + (threadIdx.x & 31);
   // The static data of the small levels (codes, inverse diagonals, fp32 weights) was evicted from L2 by the fine
   // level's streaming passes: pull it back with L2 prefetches now, off the critical path of the phases below.
   for (int l = P.first; l < P.nb; ++l) {
@@ -1042,7 +1106,7 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
           nf_down1_body<0>(L, P.r[l], P.z[l], i0, j, k);
       }
     }
-    grid.sync();
+    sync();
     if (dense) {
       for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t);
     } else {
@@ -1054,11 +1118,11 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
           nf_down2_body<1>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
       }
     }
-    grid.sync();
+    sync();
   }
   if (P.has_tail) {
-    if (blockIdx.x == 0) nf_tail_run(P.T, P.pack, P.minv, P.r[P.nb], P.z[P.nb], sm, &mbar);
-    grid.sync();
+    if (cta == 0) nf_tail_run(P.T, P.pack, P.minv, P.r[P.nb], P.z[P.nb], sm, mbar);
+    sync();
   }
   for (int l = P.nb - 1; l >= P.first; --l) {
     const NfLvK &L = P.lv[l];
@@ -1087,7 +1151,7 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
         }
       }
     }
-    grid.sync();
+    sync();
     if (dense) {
       for (int t = gt; t < D.n; t += gn) nf_dense_up2(D, t);
     } else {
@@ -1099,8 +1163,61 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_con
           nf_up2_body<0>(L, P.z[l], P.r[l], i0, j, k);
       }
     }
-    if (l > P.first) grid.sync();
+    if (l > P.first) sync();
   }
+}
+
+__global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_constant__ NfCoarseK P,
+                                                                 const NfSolveState *st) {
+  if (st && st->done) return;  // (uniform over the grid: written by an earlier kernel)
+  extern __shared__ __align__(16) float sm[];
+  __shared__ unsigned long long mbar;
+  cg::grid_group grid = cg::this_grid();
+  nf_vcoarse_body(P, (int)blockIdx.x, (int)gridDim.x, sm, &mbar, [&]() { grid.sync(); });
+}
+
+// Batched: ONE cooperative launch runs the coarse levels of up to NF_BATCH_MAX equally sized
+// environments, `nctas` CTAs each (CTA = env * nctas + cta).  The barrier is per environment: an epoch counter in the
+// environment's own word (arrive with one atomic, spin until all nctas have): environments never wait for one another,
+// and one that has converged leaves at once -- after adding the arrivals it skips, so that the counter stays in step
+// with the host's count of barriers per launch.
+struct NfCoarseBatchK {
+  int n, nctas, nbar;  // environments, CTAs per environment, barriers of one launch
+  unsigned base[NF_BATCH_MAX];  // value of the environment's counter when the launch starts
+  unsigned *bar[NF_BATCH_MAX];
+  const NfSolveState *st[NF_BATCH_MAX];
+  const NfCoarseK *P[NF_BATCH_MAX];  // (device copies: one NfCoarseK is ~1.7 KB, sixteen would not fit the parameters)
+};
+__global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_constant__ NfCoarseBatchK B) {
+  const int e = (int)blockIdx.x / B.nctas, cta = (int)blockIdx.x - e * B.nctas;
+  unsigned *bar = B.bar[e];
+  if (B.st[e] && B.st[e]->done) {
+    if (threadIdx.x == 0) atomicAdd(bar, (unsigned)B.nbar);
+    return;
+  }
+  extern __shared__ __align__(16) float sm[];
+  __shared__ unsigned long long mbar;
+  __shared__ NfCoarseK sP;
+  {  // the environment's level table: global -> shared (one round trip)
+    const int *src = reinterpret_cast<const int *>(B.P[e]);
+    int *dst = reinterpret_cast<int *>(&sP);
+    for (int t = threadIdx.x; t < (int)(sizeof(NfCoarseK) / sizeof(int)); t += blockDim.x) dst[t] = src[t];
+  }
+  __syncthreads();
+  unsigned target = B.base[e];
+  const unsigned nctas = (unsigned)B.nctas;
+  nf_vcoarse_body(sP, cta, B.nctas, sm, &mbar, [&]() {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      __threadfence();
+      atomicAdd(bar, 1u);
+      target += nctas;
+      while ((int)(*reinterpret_cast<volatile unsigned *>(bar) - target) < 0) {
+      }
+      __threadfence();
+    }
+    __syncthreads();
+  });
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -1164,6 +1281,7 @@ int nf_mg_init(nf_grid *g) {
   const int smem = NF_TAIL_SMEM_MAX;
   NF_CUDA(g, cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
   NF_CUDA(g, cudaFuncSetAttribute(k_coarse_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (NF_DIRECT_MAX * NF_DIRECT_MAX + 2 * NF_DIRECT_MAX) * (int)sizeof(double)));
   // the cooperative coarse kernel: one CTA per SM; needs a tail, at least one vec level below the finest one, and
@@ -1227,6 +1345,105 @@ static void smooth_half(nf_grid *g, NfLevel &L, int color, bool zero, bool dot, 
     NF_LAUNCH(g, cls, k_rbgs<false, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot));
 }
 
+// The level table of the cooperative coarse kernel (levels 1 .. tail-1 as grid phases, then the tail)
+static void fill_coarse(const nf_grid *g, NfCoarseK *P) {
+  const int nl = g->nlev, nb = g->tail < nl ? g->tail : nl - 1;
+  memset(P, 0, sizeof(*P));
+  P->first = 1; P->nb = nb; P->has_tail = 1;
+  P->dense_from = NF_MAX_LEVELS;
+  for (int l = 0; l < nl; ++l) {
+    P->lv[l] = nf_lvk(g->lv[l]);
+    P->z[l] = g->lv[l].z;
+    P->r[l] = g->lv[l].r;
+    P->pk[l] = g->lv[l].pk;
+    if (l >= 2 && l < nb && g->lv[l].pk && P->dense_from == NF_MAX_LEVELS) P->dense_from = l;
+  }
+  tail_desc(g, g->tail, &P->T);
+  P->minv = g->tailinv;
+  P->pack = g->tailpack;
+}
+// Device copy of that table for the batched kernel (k_vcoarse_b); refreshed whenever the hierarchy is rebuilt.
+int nf_mg_upload_coarse(nf_grid *g) {
+  if (g->coarse_ctas <= 0) return NF_OK;
+  if (!g->d_coarse) NF_CUDA(g, cudaMalloc((void **)&g->d_coarse, sizeof(NfCoarseK)));
+  if (!g->cbar) {
+    NF_CUDA(g, cudaMalloc((void **)&g->cbar, 128));
+    NF_CUDA(g, cudaMemset(g->cbar, 0, 128));
+    g->cbar_count = 0;
+  }
+  if (!g->h_coarse) {
+    NF_CUDA(g, cudaHostAlloc((void **)&g->h_coarse, sizeof(NfCoarseK), cudaHostAllocDefault));
+    NF_CUDA(g, cudaEventCreateWithFlags(&g->ev_coarse, cudaEventDisableTiming));
+  } else {
+    NF_CUDA(g, cudaEventSynchronize(g->ev_coarse));  // (the previous upload has read the pinned buffer)
+  }
+  NfCoarseK *P = static_cast<NfCoarseK *>(g->h_coarse);
+  // (the table's only host-read input is the global "singular" flag of a tail too large for the direct coarsest solve)
+  if (!(g->lv[g->nlev - 1].ncell <= NF_DIRECT_MAX)) NF_TRY(nf_meta_sync(g));
+  fill_coarse(g, P);
+  NF_CUDA(g, cudaMemcpyAsync(g->d_coarse, P, sizeof(*P), cudaMemcpyHostToDevice, g->stream));
+  NF_CUDA(g, cudaEventRecord(g->ev_coarse, g->stream));
+  return NF_OK;
+}
+void nf_mg_free_batch(nf_grid *g) {
+  cudaFree(g->d_coarse);
+  cudaFree(g->cbar);
+  if (g->h_coarse) {
+    cudaFreeHost(g->h_coarse);
+    cudaEventDestroy(g->ev_coarse);
+  }
+}
+
+// One batched PCG iteration's V-cycle part for n environments (equal extents, same stream; checked by the caller):
+// k_down2_b, k_vcoarse_b, k_up1_b, k_up2_b -- four launches for all of them.  B: filled by the caller (r[0] = the
+// current residual).  slot: parity slot that receives r.z.
+int nf_vcycle_batch(nf_grid **G, int n, const NfBatchK &Bin, int slot) {
+  nf_grid *g = G[0];
+  NfLevel &L = g->lv[0], &C = g->lv[1];
+  NfBatchK B = Bin;
+  const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+  NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
+  NfDims d2 = nf_vdims(L.nx / 4, C.ny, C.nz, 1);
+  B.nzc = (int)d2.grid.z;
+  d2.grid.z *= n;
+  NF_LAUNCH(g, NFK_DOWN2_0, nf_launch_pdl(k_down2_b, d2.grid, d2.block, g->stream, B));
+  {
+    NfCoarseBatchK CB;
+    memset(&CB, 0, sizeof(CB));
+    CB.n = n; CB.nctas = g->coarse_ctas;
+    const int nb = g->tail;
+    CB.nbar = 4 * (nb - 1) - 1 + 1;  // four phases per level 1 .. nb-1 (none after the last), one after the tail
+    for (int e = 0; e < n; ++e) {
+      CB.base[e] = G[e]->cbar_count;
+      CB.bar[e] = G[e]->cbar;
+      CB.st[e] = G[e]->st;
+      CB.P[e] = static_cast<const NfCoarseK *>(G[e]->d_coarse);
+    }
+    for (int e = 0; e < n; ++e) G[e]->cbar_count += (unsigned)(CB.nbar * CB.nctas);
+    void *args[] = {(void *)&CB};
+    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel((void *)k_vcoarse_b, dim3(n * g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
+  }
+  B.nzc = (int)d.grid.z;
+  dim3 gb = d.grid;
+  gb.z *= n;
+  NF_LAUNCH(g, NFK_UP1_0, nf_launch_pdl(k_up1_b, gb, d.block, g->stream, B, kch));
+  NF_LAUNCH(g, NFK_UP2_0, nf_launch_pdl(k_up2_b, gb, d.block, g->stream, B, kch, slot));
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+int nf_update_down1_batch(nf_grid **G, int n, const NfBatchK &Bin, int slot, int seq) {
+  nf_grid *g = G[0];
+  NfLevel &L = g->lv[0];
+  NfBatchK B = Bin;
+  const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
+  NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
+  B.nzc = (int)d.grid.z;
+  d.grid.z *= n;
+  NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_update_down1_b, d.grid, d.block, g->stream, B, kch, slot, seq));
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
 // z = M^{-1} r on level 0 (lv[0].r -> lv[0].z).  with_dot: accumulate r.z into st->rz[slot] and honour st->done.
 bool nf_update_down1_ok(const nf_grid *g) {
   return g->nu_pre == 1 && g->nu_post == 1 && !g->force_generic && g->lv[0].vec && g->nlev > 1;
@@ -1271,18 +1488,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
   }
   if (coop) {
     NfCoarseK P;
-    P.first = 1; P.nb = nb; P.has_tail = 1;
-    P.dense_from = NF_MAX_LEVELS;
-    for (int l = 0; l < nl; ++l) {
-      P.lv[l] = nf_lvk(g->lv[l]);
-      P.z[l] = g->lv[l].z;
-      P.r[l] = g->lv[l].r;
-      P.pk[l] = g->lv[l].pk;
-      if (l >= 2 && l < nb && g->lv[l].pk && P.dense_from == NF_MAX_LEVELS) P.dense_from = l;
-    }
-    tail_desc(g, g->tail, &P.T);
-    P.minv = g->tailinv;
-    P.pack = g->tailpack;
+    fill_coarse(g, &P);
     const NfSolveState *stc = st;
     void *args[] = {(void *)&P, (void *)&stc};
     NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel((void *)k_vcoarse, dim3(g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));

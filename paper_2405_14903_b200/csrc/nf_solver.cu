@@ -3,6 +3,7 @@
 // Everything the paper leaves open (smoother, transfers, coarse weights, coarse solve; R13) is described in
 // DESIGN.md section 6.
 #include <chrono>
+#include <cstring>
 #include <thread>
 
 #include "nf_stencil.cuh"
@@ -89,10 +90,10 @@ __global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restr
 // for the cell's own row and its neighbour rows, q = A p', p.q partial sums.  17 B/cell (z, p, code in; p', q out)
 // instead of 12 + 9 for the two separate passes.  p' goes to a second buffer: the neighbours' threads still read p.
 template <bool FIRST>
-__global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__restrict__ z, const float *__restrict__ pold,
-                                                 float *__restrict__ pnew, float *__restrict__ q, float *__restrict__ x,
-                                                 int kch, NfSolveState *st, int slot) {
-  nf_pdl_enter();
+__device__ __forceinline__ void nf_papply4_body(const NfLvK &L, const float *__restrict__ z,
+                                                const float *__restrict__ pold, float *__restrict__ pnew,
+                                                float *__restrict__ q, float *__restrict__ x, int kch,
+                                                NfSolveState *st, int slot, int bz) {
   if (st->done) return;
   float beta = 0.0f, aprev = 0.0f;
   if (!FIRST) {
@@ -108,7 +109,7 @@ __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__rest
   if (i0 < L.nx && j < L.ny) {
     const int nx = L.nx, ny = L.ny, nz = L.nz;
     const nf_idx sy = nx, sz = (nf_idx)nx * ny;
-    const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, nz);
+    const int k0 = bz * kch, k1 = min(k0 + kch, nz);
     nf_idx id = ((nf_idx)k0 * ny + j) * nx + i0;
     auto row4 = [&](nf_idx at, bool ok) -> float4 {
       float4 a = nf_ld4(z, at, ok);
@@ -170,6 +171,22 @@ __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__rest
     }
   }
   nf_block_atomic_add((double)part, &st->pq[slot]);
+}
+template <bool FIRST>
+__global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__restrict__ z, const float *__restrict__ pold,
+                                                 float *__restrict__ pnew, float *__restrict__ q, float *__restrict__ x,
+                                                 int kch, NfSolveState *st, int slot) {
+  nf_pdl_enter();
+  nf_papply4_body<FIRST>(L, z, pold, pnew, q, x, kch, st, slot, (int)blockIdx.z);
+}
+// The same pass for a batch of equally sized environments in ONE launch: blockIdx.z = env * nzc +
+// z-chunk, every environment with its own vectors and its own PCG scalars (an environment that has converged exits).
+template <bool FIRST>
+__global__ void __launch_bounds__(256, 3) k_papply4_b(const __grid_constant__ NfBatchK B, int kch, int slot) {
+  nf_pdl_enter();
+  const int e = (int)blockIdx.z / B.nzc, bz = (int)blockIdx.z - e * B.nzc;
+  const NfEnvK &E = B.e[e];
+  nf_papply4_body<FIRST>(E.L, E.z, E.p[1 - slot], E.p[slot], E.q, E.x, kch, E.st, slot, bz);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -692,6 +709,146 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
   return NF_OK;
 }
 
+// gauge of a singular system (R12): zero mean over the active cells, or per fluid component
+static int apply_gauge(nf_grid *g, float *x) {
+  NfLevel &L = g->lv[0];
+  const size_t n = (size_t)L.ncell;
+  NfDims dc = nf_dims(L.nx, L.ny, L.nz);
+  const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
+  if (g->gauge_mode == 2) {
+    NF_TRY(nf_components_center(g, x, nullptr, nullptr));
+  } else if (g->singular && !g->force_generic && vec_ok(x, x, x, x, n)) {
+    NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, x, nullptr, L.code, n >> 2, &g->st->sum, nullptr));
+    NF_LAUNCH(g, NFK_SETUP, k_center4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, nullptr, L.code, n >> 2, &g->st->sum, inv, nullptr));
+  } else if (g->singular) {
+    NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<dc.grid, dc.block, 0, g->stream>>>(x, x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum));
+    NF_LAUNCH(g, NFK_SETUP, k_sub_mean<<<dc.grid, dc.block, 0, g->stream>>>(x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv, 1,
+                                                    nullptr));
+  }
+  NF_CUDA(g, cudaGetLastError());
+  return NF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// batched solves: n equally sized environments advance through PCG in lockstep, every pass of an
+// iteration is ONE launch for all of them (k_papply4_b, k_update_down1_b, k_down2_b, k_vcoarse_b, k_up1_b, k_up2_b);
+// scalars, convergence and early exit stay per environment.
+// ------------------------------------------------------------------------------------------------------------
+bool nf_batch_ok(nf_grid **G, int n) {
+  if (n < 1 || n > NF_BATCH_MAX) return false;
+  nf_grid *a = G[0];
+  for (int e = 0; e < n; ++e) {
+    nf_grid *g = G[e];
+    NfLevel &L = g->lv[0];
+    const size_t nc = (size_t)L.ncell;
+    if (!g || g->nx != a->nx || g->ny != a->ny || g->nz != a->nz || g->stream != a->stream) return false;
+    if (!g->weights_set || g->force_generic || g->coarse_ctas <= 0 || g->coarse_ctas != a->coarse_ctas) return false;
+    if (!nf_update_down1_ok(g) || !apply_vec_ok(L, g->p, g->q) || !apply_vec_ok(L, g->p2, L.z) || (nc & 3)) return false;
+    if (!vec_ok(g->r_alt, L.r, g->b0, g->b0, nc) || !g->d_coarse) return false;
+    for (int f = 0; f < e; ++f)
+      if (G[f] == g) return false;
+  }
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  return n * a->coarse_ctas <= sms;  // (the cooperative launch must be resident as a whole)
+}
+
+static void fill_batch(nf_grid **G, int n, float *const *x, int it, NfBatchK *B) {
+  memset(B, 0, sizeof(*B));
+  B->n = n;
+  B->cnx = G[0]->lv[1].nx; B->cny = G[0]->lv[1].ny; B->cnz = G[0]->lv[1].nz;
+  for (int e = 0; e < n; ++e) {
+    nf_grid *g = G[e];
+    NfEnvK &E = B->e[e];
+    E.L = nf_lvk(g->lv[0]);
+    E.z = g->lv[0].z; E.q = g->q; E.x = x[e];
+    E.p[0] = g->p; E.p[1] = g->p2;
+    E.r[0] = g->lv[0].r; E.r[1] = g->r_alt;
+    E.rc = g->lv[1].r; E.zc = g->lv[1].z;
+    E.st = g->st;
+    E.hs = &g->hst_dev[it & (NF_RING - 1)];
+  }
+}
+
+// PCG on the prepared residuals (lv[0].r of every environment; st->bb, tol2, maxit set): x[e] accumulates.
+// status[e]: NF_OK / NF_NOT_CONVERGED.
+int nf_solve_batch_run(nf_grid **G, int n, float *const *x, int maxit, int *status) {
+  nf_grid *g0 = G[0];
+  NfLevel &L0 = g0->lv[0];
+  const size_t nc = (size_t)L0.ncell;
+  for (int e = 0; e < n; ++e) {
+    for (int s = 0; s < NF_RING; ++s) G[e]->hst[s].seq = 0;
+    NF_TRY(nf_vcycle_impl(G[e], true, 0));  // z = M^{-1} r and r.z of iteration 0 (per environment: once per solve)
+  }
+  const int kch = nf_kch(L0.nx / 4, L0.ny, L0.nz, NF_KCH_AP);
+  NfDims da = nf_vdims(L0.nx / 4, L0.ny, L0.nz, kch);
+  const int nzc = (int)da.grid.z;
+  dim3 gba = da.grid;
+  gba.z *= n;
+  int it = 0, last_seen = -1;
+  bool all_done = false;
+  if (maxit < 1) maxit = 1;
+  NfBatchK B;
+  for (it = 0; it < maxit && !all_done; ++it) {
+    const int slot = it & 1;
+    fill_batch(G, n, x, it, &B);
+    B.nzc = nzc;
+    if (it == 0)
+      NF_LAUNCH(g0, NFK_APPLY, nf_launch_pdl(k_papply4_b<true>, gba, da.block, g0->stream, B, kch, slot));
+    else
+      NF_LAUNCH(g0, NFK_APPLY, nf_launch_pdl(k_papply4_b<false>, gba, da.block, g0->stream, B, kch, slot));
+    NF_TRY(nf_update_down1_batch(G, n, B, slot, it + 1));
+    for (int e = 0; e < n; ++e) {  // r' was written to r_alt: the two buffers swap roles
+      float *t = G[e]->lv[0].r;
+      G[e]->lv[0].r = G[e]->r_alt;
+      G[e]->r_alt = t;
+    }
+    if (it + 1 < maxit) {
+      fill_batch(G, n, x, it, &B);
+      NF_TRY(nf_vcycle_batch(G, n, B, 1 - slot));
+    }
+    NF_CUDA(g0, cudaGetLastError());
+    const int look = it - NF_LOOKAHEAD;
+    if (look >= 0) {
+      all_done = true;
+      for (int e = 0; e < n; ++e) {
+        NF_TRY(wait_seq(G[e], look, look + 1));
+        NfHostStatus *h = &G[e]->hst[look & (NF_RING - 1)];
+        all_done = all_done && h->done;
+        h->seq = 0;
+      }
+      last_seen = look;
+    }
+  }
+  const int enq = it;
+  for (int e = 0; e < n; ++e) {
+    nf_grid *g = G[e];
+    NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x[e], g->p, g->p2, nc, g->st));
+    for (int s = last_seen + 1; s < enq; ++s) NF_TRY(wait_seq(g, s, s + 1));
+    const NfHostStatus *h = &g->hst[(enq - 1) & (NF_RING - 1)];
+    g->last_iters = h->iter;
+    g->last_relres = h->relres;
+    g->last_timed = false;
+    if (status) status[e] = h->converged ? NF_OK : NF_NOT_CONVERGED;
+    NF_TRY(apply_gauge(g, x[e]));
+  }
+  return NF_OK;
+}
+
+// A x[e] = lv[0].r of environment e (raw right-hand sides already there, or src[e] given): prepare each, then iterate
+// all of them together.  Single-phase PCG on the recursive residual (no fp64 refresh, x0 = 0): the small grids this
+// path is for sit well above the fp32 storage floor of DESIGN.md section 7.
+int nf_solve_batch_impl(nf_grid **G, int n, const float *const *src, float *const *x, float tol, int maxit, int *status) {
+  for (int e = 0; e < n; ++e) {
+    nf_grid *g = G[e];
+    NF_TRY(nf_solve_prepare_from(g, src ? src[e] : nullptr, tol, maxit));
+    NF_CUDA(g, cudaMemsetAsync(x[e], 0, (size_t)g->lv[0].ncell * sizeof(float), g->stream));
+    NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)tol, 1));
+  }
+  return nf_solve_batch_run(G, n, x, maxit, status);
+}
+
 // MGPCG on A x = lv[0].r (prepared; a copy of it is in g->b0).  x is overwritten.
 int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
   NfLevel &L = g->lv[0];
@@ -751,20 +908,7 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
     if (rc != NF_OK) return rc;
   }
   g->last_iters = ph.iters;
-  // gauge: zero mean over active cells on a singular system (R12) -- per component when there are several
-  if (g->gauge_mode == 2) {
-    NF_TRY(nf_components_center(g, x, nullptr, nullptr));
-  } else if (g->singular && !g->force_generic && vec_ok(x, x, x, x, n)) {
-    NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, x, nullptr, L.code, n >> 2, &g->st->sum, nullptr));
-    const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
-    NF_LAUNCH(g, NFK_SETUP, k_center4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, nullptr, L.code, n >> 2, &g->st->sum, inv, nullptr));
-  } else if (g->singular) {
-    NF_LAUNCH(g, NFK_SETUP, k_mask_sum<<<dc.grid, dc.block, 0, g->stream>>>(x, x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum));
-    const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
-    NF_LAUNCH(g, NFK_SETUP, k_sub_mean<<<dc.grid, dc.block, 0, g->stream>>>(x, L.ax, L.ay, L.az, L.nx, L.ny, L.nz, L.pax, &g->st->sum, inv, 1,
-                                                    nullptr));
-  }
-  NF_CUDA(g, cudaGetLastError());
+  NF_TRY(apply_gauge(g, x));
   g->last_relres = ph.relres;
   return ph.converged ? NF_OK : NF_NOT_CONVERGED;
 }

@@ -405,7 +405,20 @@ int nf_build_hierarchy(nf_grid *g) {
     if (rc != NF_OK) return rc;
   }
   NF_CUDA(g, cudaMemcpyAsync(g->h_counts, cnt, 2 * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
-  NF_CUDA(g, cudaStreamSynchronize(g->stream));
+  // The counts (active cells, Dirichlet faces, components) are read lazily: nf_meta_sync waits for this event the
+  // first time a call needs them, so that nf_set_solid itself does not drain the stream (many small environments on
+  // one stream: their hierarchy builds queue up back to back).
+  NF_CUDA(g, cudaEventRecord(g->ev_meta, g->stream));
+  g->meta_pending = true;
+  g->weights_set = true;
+  return nf_mg_upload_coarse(g);
+}
+
+// Host copies of the device-side counts of the last hierarchy build (blocks until that build has run).
+int nf_meta_sync(nf_grid *g) {
+  if (!g->meta_pending) return NF_OK;
+  NF_CUDA(g, cudaEventSynchronize(g->ev_meta));
+  g->meta_pending = false;
   const double *hc = g->h_counts;
   g->nact = (long long)hc[0];
   g->singular_info = hc[1] > 0.0 ? 0 : 1;
@@ -420,7 +433,6 @@ int nf_build_hierarchy(nf_grid *g) {
     g->gauge_mode = g->singular_info ? 1 : 0;
   }
   g->singular = g->gauge_mode == 1 ? 1 : 0;
-  g->weights_set = true;
   return NF_OK;
 }
 

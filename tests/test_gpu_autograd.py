@@ -98,3 +98,47 @@ def test_control_gradient_with_viscosity_through_autograd_matches_oracle(torch, 
     assert abs(float(J.detach()) - Jr) < 1e-4 * Jr
     assert abs(float(theta.grad) - dth) < 1e-3 * abs(dth)
     g.close()
+
+
+def test_vectorised_env_rewards_and_action_gradients_match_oracle(torch, api):
+    """FluidVecEnv (gym-style reset / step over the batched C-ABI calls): three environments with different control
+    amplitudes run two steps; every environment's reward and its gradient w.r.t. its action equal the oracle's rollout
+    (loss 1e-4, gradient 1e-3) -- the action enters through the solid velocity (Eq. 9b) with the shape frozen."""
+    from paper_2405_14903_b200 import env as envmod
+    n, nsteps = 24, 2
+    P = wl.config2_params(n)
+    bc = orc.BC(P["bc_types"], P["bc_values"])
+    lo, hi = P["loss_lo"], P["loss_hi"]
+    thetas = [0.3, 0.5, -0.8]
+    rng = np.random.default_rng(5)
+    U0 = [[(0.2 * rng.standard_normal(s)).astype(np.float32) for s in wl.face_shapes(n, n, n)] for _ in thetas]
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    frozen = {s: wl.config2_solid(P, s, 0.5) for s in range(1, nsteps + 1)}       # shape of theta = 0.5, frozen
+    unit = {s: [d(a) for a in wl.config2_solid(P, s, 1.0)[1]] for s in frozen}     # u_s per unit amplitude
+    phid = {s: d(v[0]) for s, v in frozen.items()}
+
+    def geometry(e, t, action):
+        s = int(round(t / P["dt"]))
+        return phid[s], tuple(action * a for a in unit[s])
+
+    def reward(e, U):
+        blk = U[0][lo:hi, lo:hi, lo:hi].double()
+        return (blk * blk).sum()
+
+    venv = envmod.FluidVecEnv(len(thetas), n, n, n, P["dx"], P["dt"], geometry, reward, rho=P["dt"] / P["dt_over_rho"],
+                              horizon=nsteps, bc_types=P["bc_types"], bc_values=P["bc_values"], tol=1e-6, maxit=200)
+    acts = [torch.tensor(th, dtype=torch.float32, device="cuda", requires_grad=True) for th in thetas]
+    venv.reset([[d(a) for a in U] for U in U0])
+    for _ in range(nsteps):
+        obs, rew, done, info = venv.step(acts)
+    assert done == [True] * len(thetas) and len(info["iters"]) == len(thetas)
+    sum(rew).backward()
+    for e, th in enumerate(thetas):
+        def sf(step, th=th):
+            phi = frozen[step][0]
+            _, us, _, dus = wl.config2_solid(P, step, th)
+            return phi, us, np.zeros(phi.shape), dus
+        Jo, dJo, _ = orc.rollout(U0[e], sf, nsteps, P["dt"], P["dx"], P["dt_over_rho"], bc, orc.loss_sum_u2(lo, hi))
+        assert abs(float(rew[e].detach()) - Jo) <= 1e-4 * abs(Jo), (e, float(rew[e].detach()), Jo)
+        assert abs(float(acts[e].grad) - dJo) <= 1e-3 * abs(dJo), (e, float(acts[e].grad), dJo)
+    venv.close()

@@ -664,3 +664,94 @@ def test_projection_with_closed_pocket_matches_oracle(torch, api):
     assert rel(host(y), yref) < TOL_FIELD
     assert rel3([host(a) for a in Gd], gU) < TOL_FIELD
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-4: batched small grids -- one launch per pass for all environments
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,nenv,bt", [(32, 5, (0,) * 6), (48, 16, (1, 1, 0, 0, 0, 0)), (40, 3, (0, 1, 0, 0, 0, 0)),
+                                       (64, 18, (0, 0, 0, 0, 1, 0))])
+def test_batched_projection_matches_oracle_and_single(torch, api, n, nenv, bt):
+    """nf_project_batch / nf_project_adjoint_batch on environments with DIFFERENT solids, velocities and Dirichlet
+    values: every environment against the oracle (1e-4 on p, U, y, dJ/dUhat; 1e-3 on dJ/dalpha, dJ/dU_s) and against
+    the single-handle calls (same kernels, one launch each: agreement to rounding); iteration counts are per
+    environment (18 environments at 64^3 exceed one cooperative launch: the call splits them)."""
+    rng = np.random.default_rng(100 + n)
+    dx, dtr = 1.0 / n, 0.7
+    bvs = [tuple(float(v) if t else 0.0 for v, t in zip(rng.uniform(-1, 1, 6), bt)) for _ in range(nenv)]
+    grids, phis, Us, Gs, uss = [], [], [], [], []
+    for e in range(nenv):
+        g = make_grid(api, n, n, n, dx, dtr, bt, bvs[e])
+        phi = blob_sdf(n, n, n, 200 + e, nblobs=3 + e % 4)
+        us = [0.2 * a for a in wl.random_velocity(rng, n, n, n, "uniform")]
+        g.set_solid(dev(torch, phi), *[dev(torch, a) for a in us])
+        grids.append(g); phis.append(phi); uss.append(us)
+        Us.append(wl.random_velocity(rng, n, n, n, "uniform"))
+        Gs.append(wl.random_velocity(rng, n, n, n, "normal"))
+    Ud = [[dev(torch, a) for a in U] for U in Us]
+    Uhat = [[a.clone() for a in U] for U in Ud]
+    pd = [torch.zeros(g.shape_p, dtype=torch.float32, device="cuda") for g in grids]
+    st = api.project_batch(grids, Ud, pd, tol=1e-6, maxit=200)
+    assert st == [0] * nenv
+    iters_f = [g.last_solve_info()["iters"] for g in grids]
+    Gd = [[dev(torch, a) for a in G] for G in Gs]
+    yd = [torch.zeros_like(p) for p in pd]
+    ga = [[torch.empty_like(a) for a in G] for G in Gd]
+    gs = [[torch.empty_like(a) for a in G] for G in Gd]
+    st = api.project_adjoint_batch(grids, Gd, yd, p_saved=pd, uhat=Uhat, galpha=ga, gus=gs, tol=1e-6, maxit=200)
+    assert st == [0] * nenv
+    assert all(0 < i <= 60 for i in iters_f), iters_f
+    check = range(nenv) if n <= 40 else (0, nenv // 2, nenv - 1)   # (the oracle is slow: three environments at 48^3+)
+    for e in check:
+        bc = orc.BC(bt, bvs[e])
+        alpha = [host(a) for a in grids[e].get_weights()]
+        Uref, pref = orc.project(Us[e], alpha, uss[e], dx, dtr, bc, tol=1e-12)
+        gU, gA, gS, yref = orc.project_adjoint(Gs[e], alpha, pref, Us[e], uss[e], dx, dtr, bc, tol=1e-12)
+        assert rel(host(pd[e]), pref) < TOL_FIELD
+        assert rel3([host(a) for a in Ud[e]], Uref) < TOL_FIELD
+        assert rel(host(yd[e]), yref) < TOL_FIELD
+        assert rel3([host(a) for a in Gd[e]], gU) < TOL_FIELD
+        assert rel3([host(a) for a in ga[e]], gA) < TOL_GRAD
+        assert rel3([host(a) for a in gs[e]], gS) < TOL_GRAD
+    # against the single-handle path (two-phase solve with the fp64 refresh: a few 1e-6 apart at most)
+    for e in (0, nenv - 1):
+        U1 = [dev(torch, a) for a in Us[e]]
+        p1 = torch.zeros_like(pd[e])
+        assert grids[e].project(*U1, p1, tol=1e-6, maxit=200) == 0
+        assert rel(host(pd[e]), host(p1)) < 2e-5
+        assert rel3([host(a) for a in Ud[e]], [host(a) for a in U1]) < 2e-5
+    for g in grids:
+        g.close()
+
+
+def test_batched_solve_mixed_and_singular(torch, api):
+    """nf_solve_batch: closed-wall (singular) environments with fluid pockets, zero right-hand sides and a maxit that
+    only some environments reach -- status and results per environment."""
+    n, nenv = 32, 6
+    grids, rhs, refs = [], [], []
+    rng = np.random.default_rng(7)
+    for e in range(nenv):
+        g = make_grid(api, n, n, n, 1.0 / n, 0.5)
+        phi = blob_sdf(n, n, n, 300 + e, nblobs=8)
+        g.set_solid(dev(torch, phi))
+        alpha = [host(a) for a in g.get_weights()]
+        act = orc.active_cells(alpha)
+        b = np.where(act, rng.standard_normal((n, n, n)), 0.0).astype(np.float32)
+        if e == 2:
+            b[:] = 0.0
+        grids.append(g); rhs.append(b)
+        refs.append(orc.solve(b.astype(np.float64), alpha, 0.5 * n, orc.BC(), tol=1e-12))
+    pd = [torch.full(g.shape_p, 3.0, dtype=torch.float32, device="cuda") for g in grids]
+    st = api.solve_batch(grids, [dev(torch, b) for b in rhs], pd, tol=1e-6, maxit=200)
+    assert st == [0] * nenv
+    assert grids[2].last_solve_info()["iters"] == 0 and float(pd[2].abs().max()) == 0.0
+    for e in range(nenv):
+        if e != 2:
+            assert rel(host(pd[e]), refs[e]) < TOL_FIELD
+    import warnings
+    with warnings.catch_warnings():
+        warnings.simplefilter("ignore")
+        st = api.solve_batch(grids, [dev(torch, b) for b in rhs], pd, tol=1e-7, maxit=3)
+    assert st[2] == 0 and all(s == api.NF_NOT_CONVERGED for i, s in enumerate(st) if i != 2)
+    for g in grids:
+        g.close()
