@@ -91,6 +91,14 @@ int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value);
  *                  ||b||.  Never applied to the library's internal scratch (adjoint without y_out). */
 int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags);
 
+/* The low-order part of the pressure.  A solve to 1e-6 ends with a correction e
+ * of a fp32 pressure x = O(1): rounding x + e back to fp32 alone leaves a TRUE residual of ~7e-6 at 256^3 (the storage
+ * floor of p).  With a cell array installed here, nf_solve / nf_project / nf_project_adjoint also write
+ * lo = (x + e) - fl(x + e), evaluated in fp64: the solution is p + lo (its fp64 true residual is the 1e-6 the
+ * solver stopped at), and nf_project subtracts the gradient of p + lo.  lo is zeroed when a solve needs no correction.
+ * NULL (the default) switches it off.  The array must stay valid until it is replaced. */
+int nf_set_pressure_lo(nf_grid *g, float *lo_cells);
+
 /* a-1  Face weights from the solid SDF: per face, the fluid area fraction alpha from
  * the 4 node values at its corners (marching-squares area; the printed one-fluid-corner formula
  * 1/2 * phi_A/(phi_A-phi_B) * phi_A/(phi_A-phi_D) and its companions, R3; alpha < 1e-4 -> 0, R4); closed

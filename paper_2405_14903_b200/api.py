@@ -25,6 +25,7 @@ _SIGNATURES = {
     "nf_set_dt_rho": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
     "nf_set_domain_bc": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_float]),
     "nf_set_solver_options": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "nf_set_pressure_lo": (ctypes.c_int, [ctypes.c_void_p, _c_float_p]),
     "nf_set_solid": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
     "nf_set_weights": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3),
     "nf_get_weights": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3),
@@ -225,6 +226,12 @@ class Grid:
 
     def set_solver_options(self, nu_pre=1, nu_post=1, flags=0):
         self._check(self.lib.nf_set_solver_options(self.h, nu_pre, nu_post, flags), "nf_set_solver_options")
+
+    def set_pressure_lo(self, lo):
+        """Install (or remove with None) the cell array that receives the low-order part of the next pressures."""
+        self._expect(lo, self.shape_p, "lo")
+        self._lo_keepalive = lo
+        self._check(self.lib.nf_set_pressure_lo(self.h, _ptr(lo)), "nf_set_pressure_lo")
 
     @_bound
     def set_solid(self, sdf, us=None, vs=None, ws=None):

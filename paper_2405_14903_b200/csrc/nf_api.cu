@@ -57,6 +57,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->nu_pre = 1; g->nu_post = 1; g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->singular_info = 1; g->nact = 0; g->ncomp = 0; g->nsing = 0; g->gauge_mode = 1;
+  g->plo = nullptr; g->lo_valid = false;
   g->d_coarse = nullptr; g->h_coarse = nullptr; g->cbar = nullptr; g->cbar_count = 0; g->meta_pending = false;
   g->comp = nullptr; g->cc_cnt = nullptr; g->cc_regular = nullptr; g->cc_sums = nullptr; g->cc_meta = nullptr; g->h_cc_meta = nullptr;
   g->last_iters = 0; g->last_relres = 0.0f; g->last_timed = false; g->launches = 0;
@@ -178,6 +179,13 @@ extern "C" int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int fl
   NF_CHECK_HANDLE(g);
   if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || flags < 0 || flags > 15) return NF_ERR_INVALID;
   g->nu_pre = nu_pre; g->nu_post = nu_post; g->force_generic = (flags & 2) != 0; g->refresh = (flags & 4) == 0; g->warm = (flags & 8) != 0;
+  return NF_OK;
+}
+
+extern "C" int nf_set_pressure_lo(nf_grid *g, float *lo_cells) {
+  NF_CHECK_HANDLE(g);
+  g->plo = lo_cells;
+  g->lo_valid = false;
   return NF_OK;
 }
 

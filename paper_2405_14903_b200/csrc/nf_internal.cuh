@@ -146,6 +146,8 @@ struct nf_grid {
   float *b0;  // the prepared right-hand side (kept for the true-residual refresh, nf_solver.cu)
   float *p, *p2, *q, *xtmp;  // p / p2: the search direction ping-pongs between two buffers (k_papply4)
   float *tailpack;  // 8 floats per cell of the tail levels (nf_mg.cu)
+  float *plo;      // caller's array for the low-order part of the next solutions (nf_set_pressure_lo), or NULL
+  bool lo_valid;   // the last solve wrote it
   bool meta_pending;     // the counts of the last hierarchy build have not been read yet (nf_meta_sync)
   cudaEvent_t ev_meta, ev_coarse;
   void *h_coarse;        // pinned staging of d_coarse

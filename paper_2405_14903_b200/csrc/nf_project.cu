@@ -70,7 +70,8 @@ __global__ void __launch_bounds__(256) k_grad_subtract(float *__restrict__ u, fl
                                                        const float *__restrict__ us, const float *__restrict__ vs,
                                                        const float *__restrict__ ws, const float *__restrict__ ax,
                                                        const float *__restrict__ ay, const float *__restrict__ az,
-                                                       float c, int nx, int ny, int nz, int pax, NfBcv bc) {
+                                                       float c, int nx, int ny, int nz, int pax, NfBcv bc,
+                                                       const float *__restrict__ plo) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z * blockDim.z + threadIdx.z;
@@ -78,11 +79,12 @@ __global__ void __launch_bounds__(256) k_grad_subtract(float *__restrict__ u, fl
   const size_t sy = nx, sz = (size_t)nx * ny;
   // cell id of (i,j,k) clipped into range is only dereferenced when the corresponding index is in range
   const size_t idc = ((size_t)k * ny + j) * nx + i;
+  // (plo: the low-order part of the pressure, nf_set_pressure_lo -- the pressure is p + plo, the ghosts belong to p)
   if (j < ny && k < nz) {
     const size_t f = ((size_t)k * ny + j) * (nx + 1) + i;
     const float a = ax[((size_t)k * ny + j) * pax + i];
     if (a > 0.0f)
-      u[f] = u[f] - c * nf_face_grad(p, idc, 1, i, nx, bc.v[0], bc.v[1]);
+      u[f] = u[f] - c * (nf_face_grad(p, idc, 1, i, nx, bc.v[0], bc.v[1]) + (plo ? nf_face_grad(plo, idc, 1, i, nx, 0.0f, 0.0f) : 0.0f));
     else
       u[f] = us ? us[f] : 0.0f;
   }
@@ -90,7 +92,7 @@ __global__ void __launch_bounds__(256) k_grad_subtract(float *__restrict__ u, fl
     const size_t f = ((size_t)k * (ny + 1) + j) * nx + i;
     const float a = ay[f];
     if (a > 0.0f)
-      v[f] = v[f] - c * nf_face_grad(p, idc, sy, j, ny, bc.v[2], bc.v[3]);
+      v[f] = v[f] - c * (nf_face_grad(p, idc, sy, j, ny, bc.v[2], bc.v[3]) + (plo ? nf_face_grad(plo, idc, sy, j, ny, 0.0f, 0.0f) : 0.0f));
     else
       v[f] = vs ? vs[f] : 0.0f;
   }
@@ -98,7 +100,7 @@ __global__ void __launch_bounds__(256) k_grad_subtract(float *__restrict__ u, fl
     const size_t f = ((size_t)k * ny + j) * nx + i;
     const float a = az[f];
     if (a > 0.0f)
-      w[f] = w[f] - c * nf_face_grad(p, idc, sz, k, nz, bc.v[4], bc.v[5]);
+      w[f] = w[f] - c * (nf_face_grad(p, idc, sz, k, nz, bc.v[4], bc.v[5]) + (plo ? nf_face_grad(plo, idc, sz, k, nz, 0.0f, 0.0f) : 0.0f));
     else
       w[f] = ws ? ws[f] : 0.0f;
   }
@@ -192,7 +194,7 @@ int nf_grad_subtract_impl(nf_grid *g, float *u, float *v, float *w, const float 
   const bool hu = g->have_us;
   NF_LAUNCH(g, NFK_GRADSUB, k_grad_subtract<<<d.grid, d.block, 0, g->stream>>>(u, v, w, p, hu ? g->us : nullptr, hu ? g->vs : nullptr,
                                                      hu ? g->ws : nullptr, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz,
-                                                     L.pax, bcv(g)));
+                                                     L.pax, bcv(g), g->lo_valid ? g->plo : nullptr));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }

@@ -511,6 +511,17 @@ __global__ void __launch_bounds__(256) k_add(float *__restrict__ x, const float 
   const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
   for (size_t t = tid; t < n; t += nth) x[t] += e[t];
 }
+// x + e in fp64, split into the fp32 pressure and its rounding remainder: x = fl(s), lo = fl(s - x) (nf_set_pressure_lo)
+__global__ void __launch_bounds__(256) k_add_hilo(float *__restrict__ x, const float *__restrict__ e,
+                                                  float *__restrict__ lo, size_t n) {
+  const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = tid; t < n; t += nth) {
+    const double s = (double)x[t] + (double)e[t];
+    const float hi = (float)s;
+    x[t] = hi;
+    lo[t] = (float)(s - (double)hi);
+  }
+}
 // decide from the TRUE residual in rr[0] whether the solve is finished at tolerance `tol`; publish; clear rr[0]
 __global__ void k_phase_check(NfSolveState *st, double tol, NfHostStatus *hs, int seq) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
@@ -865,6 +876,8 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
   NfPhaseOut ph;
   ph.converged = 0; ph.iters = 0; ph.relres = 0.0f;
   int rc = NF_OK;
+  g->lo_valid = false;
+  if (g->plo) NF_CUDA(g, cudaMemsetAsync(g->plo, 0, n * sizeof(float), g->stream));
   // r = b - A x afresh (fp64 evaluation); decide at `tol`; if not done run PCG on it (phase tolerance tolp) for a
   // correction e accumulated on its own, x += e once.  Used for the refresh and for a warm start.
   auto correct = [&](float tolp) -> int {
@@ -887,7 +900,12 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
       const bool fusede = fusedp && apply_vec_ok(L, g->ecorr, g->ecorr);
       rcc = run_pcg_phase(g, g->ecorr, maxit - ph.iters, fusede, v4, &ph);
       if (rcc != NF_OK) return rcc;
-      NF_LAUNCH(g, NFK_SETUP, k_add<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->ecorr, n));
+      if (g->plo) {
+        NF_LAUNCH(g, NFK_SETUP, k_add_hilo<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->ecorr, g->plo, n));
+        g->lo_valid = true;
+      } else {
+        NF_LAUNCH(g, NFK_SETUP, k_add<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->ecorr, n));
+      }
     }
     return NF_OK;
   };

@@ -228,3 +228,28 @@ def test_parametric_geometry_full_size(torch, api):
     sure_in = rw[3] < band - 1e-5
     assert np.max(np.abs(gotw - rw[2])[sure_in]) < 1e-6 and np.any(rw[2][sure_in] != 0)
     g.close()
+
+
+def test_pressure_lo_gives_the_residual_the_solver_stopped_at(torch, gate):
+    """nf_set_pressure_lo at 256^3 (the metric's '1e-6 resid'): the fp32 pressure alone sits on its storage floor (true
+    residual 7e-6, test above); with the low-order part the library also returns, p + lo has the fp64 TRUE residual
+    the solve stopped at, the velocity's weighted divergence drops accordingly, and p itself is unchanged."""
+    g, P, bc, d = gate["g"], gate["P"], gate["bc"], gate["d"]
+    c = P["dt_over_rho"] / P["dx"]
+    U = [d(a) for a in gate["U0"]]
+    p = torch.zeros(g.shape_p, dtype=torch.float32, device="cuda")
+    lo = torch.full(g.shape_p, 9.0, dtype=torch.float32, device="cuda")
+    g.set_pressure_lo(lo)
+    try:
+        assert g.project(*U, p, tol=1e-6, maxit=400) == 0
+    finally:
+        g.set_pressure_lo(None)
+    alpha = [a.cpu().numpy().astype(np.float64) for a in g.get_weights()]
+    us_eff = orc.effective_solid_velocity(gate["us"], [a.shape for a in gate["U0"]], bc)
+    b = orc.rhs([a.astype(np.float64) for a in gate["U0"]], alpha, us_eff, c, bc)
+    ph, pl = p.cpu().numpy().astype(np.float64), lo.cpu().numpy().astype(np.float64)
+    assert 0 < np.abs(pl).max() <= 1e-6 * np.abs(ph).max()          # a rounding remainder, not a second pressure
+    r_hi = np.linalg.norm(b - orc.apply_A(ph, alpha, c)) / np.linalg.norm(b)
+    r_full = np.linalg.norm(b - orc.apply_A(ph + pl, alpha, c)) / np.linalg.norm(b)
+    assert r_full <= 1.5e-6 and r_full < 0.5 * r_hi, (r_hi, r_full)
+    assert float((p - gate["p"]).abs().max()) == 0.0                 # same fp32 pressure as without the option
