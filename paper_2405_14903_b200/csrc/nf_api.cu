@@ -87,18 +87,15 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     // 2-D mode (nz == 1): x and y coarsen, z stays one layer
     const bool flat = nz == 1;
     L.fz = flat ? 1 : 2;
-    // extents stay >= 4 -- except that a level with more than 128 cells (too many for the direct coarsest solve of
-    // nf_mg.cu) is halved once more if it can be: 48^3 ends at 3^3 instead of 6^3, 256^3 at 4^3 as before
+    // Extents halve, rounding UP (a coarse cell at an odd edge has one child along that axis; the absent children
+    // count as solid), while every coarse extent stays >= 4 -- except that a level with more than 128 cells (too many
+    // for the direct coarsest solve of nf_mg.cu) is halved once more if it can be: 48^3 ends at 3^3 instead of 6^3,
+    // 256^3 at 4^3, 250^3 goes 125, 63, 32, 16, 8, 4 (before: it stopped at 125^3 and needed 175 iterations).
     const int lim = L.ncell > 128 ? 2 : 4;
-    if (flat) {
-      if ((lx | ly) & 1) break;
-      if (lx / 2 < lim || ly / 2 < lim) break;
-      lx /= 2; ly /= 2;
-    } else {
-      if ((lx | ly | lz) & 1) break;
-      if (lx / 2 < lim || ly / 2 < lim || lz / 2 < lim) break;
-      lx /= 2; ly /= 2; lz /= 2;
-    }
+    const int hx = (lx + 1) / 2, hy = (ly + 1) / 2, hz = flat ? 1 : (lz + 1) / 2;
+    if (hx < lim || hy < lim || (!flat && hz < lim)) break;
+    if (hx == lx && hy == ly && hz == lz) break;
+    lx = hx; ly = hy; lz = hz;
     c *= 0.25f;
   }
   g->nlev = nl;

@@ -523,6 +523,7 @@ __global__ void __launch_bounds__(256) k_residual_restrict(const float *__restri
       for (int di = 0; di < 2; ++di) {
         if (dk >= fz) continue;  // (2-D mode: the children are the 2 x 2 x 1 cells)
         const int i = 2 * I + di, j = 2 * J + dj, k = fz * K + dk;
+        if (i >= nx || j >= ny || k >= nz) continue;  // (odd extent: this child does not exist)
         const NfW6 w = nf_load_w6(ax, ay, az, i, j, k, nx, ny, pax);
         const size_t id = ((size_t)k * ny + j) * nx + i;
         acc += r[id] - c * (nf_w6_sum(w) * z[id] - nf_nb_sum(z, w, i, j, k, nx, ny, nz));
@@ -873,6 +874,7 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
           for (int di = 0; di < 2; ++di) {
             // (the residual is zero on the black cells: the black half sweep has just solved their equations)
             if (((di + dj + dk) & 1) || dk >= fz) continue;
+            if (2 * I + di >= nx || 2 * J + dj >= ny || fz * K + dk >= T.nz[l]) continue;  // (odd extent: no such child)
             const int id = ((fz * K + dk) * ny + (2 * J + dj)) * nx + 2 * I + di;
             const float s = pk[1 * n + id] * z[max(id - 1, 0)] + pk[2 * n + id] * z[min(id + 1, n - 1)] +
                       pk[3 * n + id] * z[max(id - sy, 0)] + pk[4 * n + id] * z[min(id + sy, n - 1)] +
@@ -1273,7 +1275,8 @@ void nf_mg_plan(nf_grid *g) {
     const NfLevel &L = g->lv[l];
     const double slots = (double)(L.nz + 1) * (L.ny + 1) * (L.pax + 4);  // largest face array of the level
     g->lv[l].vec_idx32 = slots < 4.0e9 ? 1 : 0;
-    g->lv[l].vec = (l < nb && (L.nx & 3) == 0 && g->lv[l].vec_idx32) ? 1 : 0;
+    // (the 4-cells-per-thread kernels work on whole 2 x 2 x 2 families: every extent even, x a multiple of 4)
+    g->lv[l].vec = (l < nb && (L.nx & 3) == 0 && (L.ny & 1) == 0 && (L.fz == 1 || (L.nz & 1) == 0) && g->lv[l].vec_idx32) ? 1 : 0;
   }
 }
 

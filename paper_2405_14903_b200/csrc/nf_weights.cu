@@ -243,24 +243,26 @@ __global__ void __launch_bounds__(256) k_coarsen_weights(const float *__restrict
   const int J = blockIdx.y * blockDim.y + threadIdx.y;
   const int K = blockIdx.z * blockDim.z + threadIdx.z;
   if (I > cnx || J > cny || K > cnz) return;
+  // Coarse face weight = mean of the (up to) four coincident fine faces; fine faces beyond an odd extent do not exist
+  // and count as closed.  The coarse boundary face of an odd axis coincides with the fine boundary face.
   const int i = 2 * I, j = 2 * J, k = fz * K;
-  if (J < cny && K < cnz) {
-    const float *b = fax + ((size_t)k * fny + j) * fpax + i;
-    const size_t sj = fpax, sk = (size_t)fny * fpax;
-    cax[((size_t)K * cny + J) * cpax + I] =
-        fz == 2 ? 0.25f * ((b[0] + b[sj]) + (b[sk] + b[sk + sj])) : 0.5f * (b[0] + b[sj]);
-  }
-  if (I < cnx && K < cnz) {
-    const float *b = fay + ((size_t)k * (fny + 1) + j) * fnx + i;
-    const size_t sk = (size_t)(fny + 1) * fnx;
-    cay[((size_t)K * (cny + 1) + J) * cnx + I] =
-        fz == 2 ? 0.25f * ((b[0] + b[1]) + (b[sk] + b[sk + 1])) : 0.5f * (b[0] + b[1]);
-  }
-  if (I < cnx && J < cny) {
-    const float *b = faz + ((size_t)k * fny + j) * fnx + i;
-    const size_t sj = fnx;
-    caz[((size_t)K * cny + J) * cnx + I] = 0.25f * ((b[0] + b[1]) + (b[sj] + b[sj + 1]));
-  }
+  auto fx = [&](int ii, int jj, int kk) -> float {
+    return (jj < fny && kk < fnz) ? fax[((size_t)kk * fny + jj) * fpax + min(ii, fnx)] : 0.0f;
+  };
+  auto fy = [&](int ii, int jj, int kk) -> float {
+    return (ii < fnx && kk < fnz) ? fay[((size_t)kk * (fny + 1) + min(jj, fny)) * fnx + ii] : 0.0f;
+  };
+  auto fzf = [&](int ii, int jj, int kk) -> float {
+    return (ii < fnx && jj < fny) ? faz[((size_t)min(kk, fnz) * fny + jj) * fnx + ii] : 0.0f;
+  };
+  if (J < cny && K < cnz)
+    cax[((size_t)K * cny + J) * cpax + I] = fz == 2 ? 0.25f * ((fx(i, j, k) + fx(i, j + 1, k)) + (fx(i, j, k + 1) + fx(i, j + 1, k + 1)))
+                                                    : 0.5f * (fx(i, j, k) + fx(i, j + 1, k));
+  if (I < cnx && K < cnz)
+    cay[((size_t)K * (cny + 1) + J) * cnx + I] = fz == 2 ? 0.25f * ((fy(i, j, k) + fy(i + 1, j, k)) + (fy(i, j, k + 1) + fy(i + 1, j, k + 1)))
+                                                         : 0.5f * (fy(i, j, k) + fy(i + 1, j, k));
+  if (I < cnx && J < cny)
+    caz[((size_t)K * cny + J) * cnx + I] = 0.25f * ((fzf(i, j, k) + fzf(i + 1, j, k)) + (fzf(i, j + 1, k) + fzf(i + 1, j + 1, k)));
 }
 
 // Cell codes of one level from its fp32 weights: bits 0..5 = face is fully open, bit 6 = the

@@ -266,7 +266,11 @@ def test_vcycle_fused_equals_generic(torch, api, shape, bt):
 
 @pytest.mark.parametrize("shape,bt,seed", [((32, 32, 32), (0,) * 6, 9), ((64, 64, 64), (1, 1, 0, 0, 0, 0), 9),
                                             ((40, 36, 28), (0, 0, 1, 0, 0, 0), 9), ((96, 96, 96), (0, 1, 0, 0, 0, 0), 9),
-                                            ((128, 128, 128), (1, 1, 0, 0, 0, 0), 9), ((128, 128, 128), (0,) * 6, 2)])
+                                            ((128, 128, 128), (1, 1, 0, 0, 0, 0), 9), ((128, 128, 128), (0,) * 6, 2),
+                                            # odd extents on coarse levels (ceil-coarsening): 100 -> 50, 25, 13, 7, 4;
+                                            # 50 x 30 x 22 -> 25 x 15 x 11 ...; odd from the start
+                                            ((100, 100, 100), (0, 1, 0, 0, 0, 0), 9), ((50, 30, 22), (0,) * 6, 9),
+                                            ((37, 29, 23), (1, 0, 0, 0, 0, 0), 9)])
 def test_vcycle_matches_fp64_reference(torch, api, shape, bt, seed):
     """The CUDA V-cycle (fused fine-level kernels, cooperative coarse kernel incl. its packed per-cell phases at
     >= 96^3, shared-memory tail) against tests/vcycle_ref.py, the same documented preconditioner in NumPy fp64 on the
@@ -755,3 +759,17 @@ def test_batched_solve_mixed_and_singular(torch, api):
     assert st[2] == 0 and all(s == api.NF_NOT_CONVERGED for i, s in enumerate(st) if i != 2)
     for g in grids:
         g.close()
+
+
+@pytest.mark.parametrize("n", [100, 120, 250])
+def test_non_power_of_two_grids_converge_like_the_others(torch, api, n):
+    """Ceil-coarsening keeps the hierarchy going through odd extents (250 -> 125, 63, 32, 16, 8, 4): iteration counts
+    stay at the level of the power-of-two grids (before: 44 / 33 / 175 iterations at 100^3 / 120^3 / 250^3)."""
+    g = make_grid(api, n, n, n, 1.0 / n, bc_types=(0, 1, 0, 0, 0, 0))
+    g.set_solid(dev(torch, blob_sdf(n, n, n, 5)))
+    assert g.info()["levels"] >= 5
+    b = torch.randn(g.shape_p, device="cuda")
+    p = torch.zeros_like(b)
+    assert g.solve(b, p, tol=1e-6, maxit=200) == 0
+    assert g.last_solve_info()["iters"] <= 30, g.last_solve_info()
+    g.close()

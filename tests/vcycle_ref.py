@@ -6,7 +6,8 @@ check the CUDA V-cycle kernels (fused 4-launch levels, cooperative coarse kernel
 shared-memory tail) against something that carries no fp32 rounding: V(1,1), red-black Gauss-Seidel (pre: red then
 black from a zero guess; post: black then red), piecewise-constant prolongation P, restriction P^T / 8,
 rediscretised coarse operators with c_l = c / 4^l on weights that are the mean of the four coincident fine face
-weights, levels halving while every extent is even and stays >= 4 (>= 2 while the level has more than 128 cells), coarsest level (<= 128 cells): exact solve (the
+weights (absent fine faces of an odd edge count as closed), extents halving -- rounding up -- while they stay >= 4
+(>= 2 while the level has more than 128 cells), coarsest level (<= 128 cells): exact solve (the
 pseudo-inverse in the complement of the constant on singular systems); a larger coarsest level: 2 * (largest extent)
 symmetric sweeps (red-black from zero, then black-red).
 3-D grids only."""
@@ -14,12 +15,25 @@ import numpy as np
 
 
 def _coarsen(a):
-    """Coarse face weights in float32 with the library's summation order (so both hierarchies hold identical numbers)."""
+    """Coarse face weights in float32 with the library's summation order (so both hierarchies hold identical numbers).
+    Extents halve rounding up: fine faces beyond an odd extent do not exist and count as closed, and the coarse
+    boundary face of an odd axis coincides with the fine boundary face."""
     au, av, aw = [x.astype(np.float32) for x in a]
+    nz, ny, nx = au.shape[0], au.shape[1], au.shape[2] - 1
+    ez, ey, ex = nz + (nz & 1), ny + (ny & 1), nx + (nx & 1)
     q = np.float32(0.25)
-    cu = q * ((au[0::2, 0::2, 0::2] + au[0::2, 1::2, 0::2]) + (au[1::2, 0::2, 0::2] + au[1::2, 1::2, 0::2]))
-    cv = q * ((av[0::2, 0::2, 0::2] + av[0::2, 0::2, 1::2]) + (av[1::2, 0::2, 0::2] + av[1::2, 0::2, 1::2]))
-    cw = q * ((aw[0::2, 0::2, 0::2] + aw[0::2, 0::2, 1::2]) + (aw[0::2, 1::2, 0::2] + aw[0::2, 1::2, 1::2]))
+    xi = list(range(0, nx, 2)) + [nx]   # fine x-faces under the coarse ones (the last one: the boundary face)
+    yi = list(range(0, ny, 2)) + [ny]
+    zi = list(range(0, nz, 2)) + [nz]
+    pu = np.zeros((ez, ey, nx + 1), np.float32); pu[:nz, :ny] = au
+    pu = pu[:, :, xi]
+    cu = q * ((pu[0::2, 0::2] + pu[0::2, 1::2]) + (pu[1::2, 0::2] + pu[1::2, 1::2]))
+    pv = np.zeros((ez, ny + 1, ex), np.float32); pv[:nz, :, :nx] = av
+    pv = pv[:, yi, :]
+    cv = q * ((pv[0::2, :, 0::2] + pv[0::2, :, 1::2]) + (pv[1::2, :, 0::2] + pv[1::2, :, 1::2]))
+    pw = np.zeros((nz + 1, ey, ex), np.float32); pw[:, :ny, :nx] = aw
+    pw = pw[zi]
+    cw = q * ((pw[:, 0::2, 0::2] + pw[:, 0::2, 1::2]) + (pw[:, 1::2, 0::2] + pw[:, 1::2, 1::2]))
     return [cu, cv, cw]
 
 
@@ -28,7 +42,9 @@ def hierarchy(alpha):
     lv = [[np.asarray(x, dtype=np.float32) for x in alpha]]
     while True:
         nz, ny, nx = lv[-1][0].shape[0], lv[-1][0].shape[1], lv[-1][0].shape[2] - 1
-        if (nx | ny | nz) & 1 or min(nx, ny, nz) // 2 < (2 if nx * ny * nz > 128 else 4):
+        lim = 2 if nx * ny * nz > 128 else 4
+        h = [(nx + 1) // 2, (ny + 1) // 2, (nz + 1) // 2]
+        if min(h) < lim or h == [nx, ny, nz]:
             break
         lv.append(_coarsen(lv[-1]))
     return lv
@@ -95,9 +111,11 @@ def vcycle(r, alpha, c, singular):
             return z
         half(red); half(~red)
         res = np.where(act, r - (d * z - c * _nbsum(z, a)), 0.0)
-        rc = 0.125 * res.reshape(nz // 2, 2, ny // 2, 2, nx // 2, 2).sum(axis=(1, 3, 5))
+        ez, ey, ex = nz + (nz & 1), ny + (ny & 1), nx + (nx & 1)
+        rp = np.zeros((ez, ey, ex)); rp[:nz, :ny, :nx] = res          # (absent children of an odd edge contribute 0)
+        rc = 0.125 * rp.reshape(ez // 2, 2, ey // 2, 2, ex // 2, 2).sum(axis=(1, 3, 5))
         zc = rec(l + 1, rc, 0.25 * c)
-        z += np.repeat(np.repeat(np.repeat(zc, 2, axis=0), 2, axis=1), 2, axis=2)
+        z += np.repeat(np.repeat(np.repeat(zc, 2, axis=0), 2, axis=1), 2, axis=2)[:nz, :ny, :nx]
         half(~red); half(red)
         return z
 
