@@ -97,12 +97,20 @@ __global__ void __launch_bounds__(256) k_cc_merge(NfLvK L, unsigned *comp, unsig
   }
 }
 
-// comp[id] = root of id; counts the roots in meta[0]
+// comp[id] = root of id; counts the roots in meta[0].  The walk to the root is READ-ONLY here: with path halving a
+// thread passing through cell x could overwrite the root x's own thread has just stored with an intermediate parent it
+// read earlier, and the labelling pass below relies on every entry pointing at a root.  (A stale read of comp[x] by
+// a passing thread is harmless: old parent and root are both ancestors.)
 __global__ void __launch_bounds__(256) k_cc_flatten(unsigned *comp, unsigned n, int *meta) {
   const unsigned id = blockIdx.x * blockDim.x + threadIdx.x;
   if (id >= n) return;
   if (comp[id] == 0xffffffffu) return;
-  const unsigned r = nf_cc_find(comp, id);
+  unsigned r = id;
+  for (;;) {
+    const unsigned pr = *reinterpret_cast<volatile unsigned *>(comp + r);
+    if (pr == r) break;
+    r = pr;
+  }
   comp[id] = r;
   if (r == id) atomicAdd(meta, 1);
 }

@@ -773,3 +773,34 @@ def test_non_power_of_two_grids_converge_like_the_others(torch, api, n):
     assert g.solve(b, p, tol=1e-6, maxit=200) == 0
     assert g.last_solve_info()["iters"] <= 30, g.last_solve_info()
     g.close()
+
+
+@pytest.mark.parametrize("n,nblobs,seed", [(128, 0, 0), (96, 60, 1), (72, 90, 2)])
+def test_component_labels_through_the_gauge_at_larger_sizes(torch, api, n, nblobs, seed):
+    """The device labelling (union-find with path halving, one union per run overlap) checked where the oracle's solve
+    is too slow: the number of components equals a host flood fill's, and after a solve with an INCOMPATIBLE right-hand
+    side the pressure has zero mean over every host-labelled component while the fp64 residual is exactly the part of
+    b the definition drops (its component means).  nblobs = 0: the configs[4] sphere field at 128^3, whose 2-cell
+    pocket beside a 1.8 M-cell component exposed a race in the flatten pass."""
+    phi = wl.config5_phi(n) if nblobs == 0 else blob_sdf(n, n, n, 40 + seed, nblobs=nblobs)
+    g = make_grid(api, n, n, n, 1.0 / n)
+    g.set_solid(dev(torch, phi))
+    alpha = [host(a) for a in g.get_weights()]
+    labels, ncomp = wl.fluid_components(*[a.astype(np.float32) for a in alpha])
+    assert g.components() == (ncomp, ncomp) and ncomp >= 2
+    rng = np.random.default_rng(seed)
+    b = np.where(labels > 0, rng.standard_normal((n, n, n)), 0.0).astype(np.float32)
+    p = torch.zeros(g.shape_p, dtype=torch.float32, device="cuda")
+    assert g.solve(dev(torch, b), p, tol=1e-6, maxit=200) == 0
+    assert g.last_solve_info()["iters"] <= 60
+    ph = host(p)
+    K = ncomp
+    cnt = np.maximum(np.bincount(labels.ravel(), minlength=K + 1), 1)
+    pm = np.bincount(labels.ravel(), weights=ph.ravel(), minlength=K + 1) / cnt
+    assert np.max(np.abs(pm[1:])) <= 1e-5 * max(1.0, np.abs(ph).max())
+    bm = np.bincount(labels.ravel(), weights=b.astype(np.float64).ravel(), minlength=K + 1) / cnt
+    bm[0] = 0.0
+    bc_ = b.astype(np.float64) - bm[labels]
+    res = bc_ - orc.apply_A(ph, alpha, 1.0 * n)
+    assert np.linalg.norm(res) <= 5e-6 * np.linalg.norm(bc_)
+    g.close()
