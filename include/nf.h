@@ -77,8 +77,9 @@ int nf_set_dt_rho(nf_grid *g, float dt_over_rho);
 int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value);
 
 /* Solver options (PAPER.md:L230 names only "MGPCG"; every parameter is this library's choice, R13):
- *   nu_pre / nu_post: red-black Gauss-Seidel sweeps before / after the coarse correction (default 1, 1; the fused
- *     4-cells-per-thread V-cycle kernels exist for (1, 1) only, other values run the generic kernels);
+ *   nu_pre / nu_post: red-black Gauss-Seidel sweeps before / after the coarse correction on the FINEST level
+ *     (default 1, 1; PCG needs a symmetric preconditioner, i.e. nu_pre == nu_post -- unequal values are accepted for
+ *     stand-alone V-cycles and run the generic kernels).  The levels below take nf_set_coarse_sweeps;
  *   flags: bit 0 = reserved,
  *          bit 1 = test hook: force the generic kernels (fp32 weights, one colour per launch) on every level,
  *          bit 2 = switch OFF the true-residual refresh.  By default a solve with tol < 3e-4 runs PCG to 30 tol,
@@ -90,6 +91,13 @@ int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value);
  *                  step (the paper is silent on x0, R11; default x0 = 0).  The stopping criterion stays relative to
  *                  ||b||.  Never applied to the library's internal scratch (adjoint without y_out). */
 int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags);
+
+/* Red-black Gauss-Seidel sweeps before AND after the coarse correction on level 1 (the first level below the finest
+ * one) and on every level below that (1..8 each, default 2, 2; R13: the paper names only "MGPCG").  Those levels hold
+ * 1/8 + 1/64 + ... of the cells and run inside one cooperative kernel, so a second sweep there costs ~20 % of a PCG
+ * iteration at 256^3 and saves 40 % of the iterations on the channel-gate workload.  May be called
+ * at any time between solves; handles solved together by the *_batch calls must agree. */
+int nf_set_coarse_sweeps(nf_grid *g, int nu_level1, int nu_deeper);
 
 /* The low-order part of the pressure.  A solve to 1e-6 ends with a correction e
  * of a fp32 pressure x = O(1): rounding x + e back to fp32 alone leaves a TRUE residual of ~7e-6 at 256^3 (the storage

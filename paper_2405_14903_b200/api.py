@@ -25,6 +25,7 @@ _SIGNATURES = {
     "nf_set_dt_rho": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
     "nf_set_domain_bc": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_float]),
     "nf_set_solver_options": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "nf_set_coarse_sweeps": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
     "nf_set_pressure_lo": (ctypes.c_int, [ctypes.c_void_p, _c_float_p]),
     "nf_set_solid": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
     "nf_set_weights": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3),
@@ -226,6 +227,11 @@ class Grid:
 
     def set_solver_options(self, nu_pre=1, nu_post=1, flags=0):
         self._check(self.lib.nf_set_solver_options(self.h, nu_pre, nu_post, flags), "nf_set_solver_options")
+
+    @_bound
+    def set_coarse_sweeps(self, nu_level1=2, nu_deeper=None):
+        nd = nu_level1 if nu_deeper is None else nu_deeper
+        self._check(self.lib.nf_set_coarse_sweeps(self.h, int(nu_level1), int(nd)), "nf_set_coarse_sweeps")
 
     def set_pressure_lo(self, lo):
         """Install (or remove with None) the cell array that receives the low-order part of the next pressures."""

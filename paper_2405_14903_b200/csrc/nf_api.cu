@@ -54,7 +54,19 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   g->nx = nx; g->ny = ny; g->nz = nz; g->dx = dx; g->dt_over_rho = 1.0f;
   for (int f = 0; f < 6; ++f) { g->bc_type[f] = NF_BC_CLOSED; g->bc_val[f] = 0.0f; }
   g->stream = 0;
-  g->nu_pre = 1; g->nu_post = 1; g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
+  g->nu_pre = 1; g->nu_post = 1;
+  // Sweeps on the coarse levels (nf_set_coarse_sweeps overrides): chosen from measurements on the channel-gate
+  // workload.  The extra sweeps run as phases of the cooperative coarse kernel, whose cost is
+  // latency and does not shrink with the grid, while the fine level's cost does: large grids afford more of them.
+  //   256^3, forward + adjoint solve, ms: (1,1) 22.8  (1,2) 18.1  (2,2) 17.7  (2,3) 16.8  (3,3) 16.9
+  //   128^3:                              (1,1) 4.94  (1,2) 4.68  (2,2) 4.71  (2,3) 5.13
+  //    64^3:                              (1,1) 2.58  (1,2) 2.63  (2,2) 2.86
+  {
+    const bool large = (long long)nx * ny * nz >= 6000000LL;
+    g->nu_l1 = large ? 2 : 1;
+    g->nu_deep = large ? 3 : 2;
+  }
+  g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
   g->weights_set = g->have_sdf = g->have_us = false;
   g->singular = 1; g->singular_info = 1; g->nact = 0; g->ncomp = 0; g->nsing = 0; g->gauge_mode = 1;
   g->plo = nullptr; g->lo_valid = false;
@@ -177,6 +189,13 @@ extern "C" int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int fl
   if (nu_pre < 1 || nu_post < 1 || nu_pre > 8 || nu_post > 8 || flags < 0 || flags > 15) return NF_ERR_INVALID;
   g->nu_pre = nu_pre; g->nu_post = nu_post; g->force_generic = (flags & 2) != 0; g->refresh = (flags & 4) == 0; g->warm = (flags & 8) != 0;
   return NF_OK;
+}
+
+extern "C" int nf_set_coarse_sweeps(nf_grid *g, int nu_level1, int nu_deeper) {
+  NF_CHECK_HANDLE(g);
+  if (nu_level1 < 1 || nu_level1 > 8 || nu_deeper < 1 || nu_deeper > 8) return NF_ERR_INVALID;
+  g->nu_l1 = nu_level1; g->nu_deep = nu_deeper;
+  return g->weights_set ? nf_mg_upload_coarse(g) : NF_OK;  // (the batched kernel reads the sweep count from the device table)
 }
 
 extern "C" int nf_set_pressure_lo(nf_grid *g, float *lo_cells) {
@@ -577,7 +596,7 @@ static const char *kClassNames[NFK_COUNT] = {
     "apply_A", "cg_update", "cg_check", "cg_pupdate", "down1_fine", "down2_fine", "up1_fine", "up2_fine", "vec_coarse",
     "rbgs_fine", "rbgs_coarse", "restrict_fine", "restrict_coarse", "prolong_fine", "prolong_coarse", "tail",
     "solve_setup", "rhs", "grad_subtract", "adjoint_rhs", "adjoint_finish", "weights", "coarsen", "encode", "store_us",
-    "advect", "advect_adjoint", "weights_adjoint", "geometry", "misc"};
+    "advect", "advect_adjoint", "weights_adjoint", "geometry", "misc", "sweep_fine"};
 
 void nf_prof_begin(nf_grid *g, int cls) {
   const size_t r = g->prof_cls.size();

@@ -98,6 +98,7 @@ struct NfBatchK {
   int n;    // environments in this launch (<= NF_BATCH_MAX)
   int nzc;  // z-chunks (CTAs along blockIdx.z) per environment
   int cnx, cny, cnz;  // extents of the first coarse level
+  int gen;  // k_down2_b: general residual (the pre-smoother ran more than one sweep)
   NfEnvK e[NF_BATCH_MAX];
 };
 
@@ -112,7 +113,7 @@ enum {
   NFK_APPLY = 0, NFK_UPDATE, NFK_CHECK, NFK_PUPDATE, NFK_DOWN1_0, NFK_DOWN2_0, NFK_UP1_0, NFK_UP2_0, NFK_VEC_C,
   NFK_RBGS0, NFK_RBGS_C, NFK_RESTRICT0, NFK_RESTRICT_C, NFK_PROLONG0, NFK_PROLONG_C, NFK_BOTTOM, NFK_SETUP, NFK_RHS,
   NFK_GRADSUB, NFK_ADJ_RHS, NFK_ADJ_FINISH, NFK_WEIGHTS, NFK_COARSEN, NFK_CLASSIFY, NFK_STORE_US, NFK_ADVECT,
-  NFK_ADVECT_ADJ, NFK_WEIGHTS_ADJ, NFK_GEOM, NFK_MISC, NFK_COUNT
+  NFK_ADVECT_ADJ, NFK_WEIGHTS_ADJ, NFK_GEOM, NFK_MISC, NFK_SWEEP_0, NFK_COUNT
 };
 
 struct nf_grid {
@@ -134,7 +135,8 @@ struct nf_grid {
   int ncomp, nsing;  // components of the current weights; those without an open Dirichlet face
   int gauge_mode;    // 0: no singular component; 1: a single, singular component (global path); 2: per component
   long long nact;
-  int nu_pre, nu_post;
+  int nu_pre, nu_post;  // red-black sweeps before / after the coarse correction on the FINEST level
+  int nu_l1, nu_deep;   // ... on level 1 / on every level below that (pre = post; nf_set_coarse_sweeps)
   bool warm;     // flag 8 of nf_set_solver_options: caller-provided solution arrays hold the initial guess
   bool refresh;  // true-residual refresh between two PCG phases (default on; flag 4 of nf_set_solver_options: off)
   bool force_generic;  // test hook: run the generic (fp32-weight, one colour per launch) kernels everywhere

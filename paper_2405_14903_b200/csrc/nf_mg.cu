@@ -195,9 +195,11 @@ __global__ void __launch_bounds__(256, 4) k_down1(NfLvK L, const float *__restri
 
 // One thread per pair of coarse cells (I0, I0+1) = fine cells i0..i0+3 of the rows (2J+dj, FZ K+dk).  FZ = 2, or 1 in
 // 2-D mode (one layer: 2 x 2 x 1 children, R = P^T / 4).
-template <int FZ>
+// GEN: the pre-smoother ran more than one sweep, so a red cell no longer holds z = r / diag: its residual is
+// (r - diag z) + c sum a z_black (r is read as well).
+template <int FZ, bool GEN = false>
 __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, float *rc, int cnx, int cny, int i0,
-                                              int J, int K) {
+                                              int J, int K, const float *r = nullptr) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const nf_idx sy = nx, sz = (nf_idx)nx * ny;
   const int j0 = 2 * J, k0 = FZ * K;
@@ -228,6 +230,8 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
         zo[0] = zo[1] = zo[2] = zo[3] = 0.0f;  // (one layer between closed walls: both z neighbours are ghosts)
       const float xe = par == 0 ? nf_ld1(z, id - 1, i0 > 0) : nf_ld1(z, id + 4, i0 + 4 < nx);
       const bool open4 = (cc[dk][dj] & 0x7f7f7f7fu) == 0x3f3f3f3fu;  // all four cells: six open faces
+      float rr[4];
+      if (GEN) nf_unpack4(nf_ld4(r, id, true), rr);
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         if (((q + par) & 1) != 0) continue;  // red children only
@@ -237,9 +241,14 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
         float s;
         if (open4) {
           s = ((xl + xh) + (yl + yh)) + (zl + zh);
+          if (GEN) s += rr[q] * L.ic - 6.0f * zc[dk][dj][q];
         } else {
           const NfW6 w = nf_code_w6(L, nf_code_at(cc[dk][dj], q), i0 + q, j, k);
           s = ((w.xl * xl + w.xh * xh) + (w.yl * yl + w.yh * yh)) + (w.zl * zl + w.zh * zh);
+          if (GEN) {
+            const float d = nf_w6_sum(w);
+            s = d > 0.0f ? s + (rr[q] * L.ic - d * zc[dk][dj][q]) : 0.0f;
+          }
         }
         if (q < 2) acc0 += s; else acc1 += s;
       }
@@ -248,15 +257,23 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
   *reinterpret_cast<float2 *>(rc + ((nf_idx)K * cny + J) * cnx + (i0 >> 1)) = make_float2(f * acc0, f * acc1);
 }
 
+// (r != nullptr: the general residual, after more than one pre-smoothing sweep)
 __global__ void __launch_bounds__(256, 4) k_down2(NfLvK L, const float *__restrict__ z, float *__restrict__ rc, int cnx,
-                                               int cny, int cnz, int kch, const NfSolveState *st) {
+                                               int cny, int cnz, int kch, const NfSolveState *st,
+                                               const float *__restrict__ r) {
   nf_pdl_enter();
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int J = blockIdx.y * blockDim.y + threadIdx.y;
   if (i0 >= L.nx || J >= cny) return;
   const int K0 = blockIdx.z * kch, K1 = min(K0 + kch, cnz);
-  if (L.fz == 2) {
+  if (r) {
+    if (L.fz == 2) {
+      for (int K = K0; K < K1; ++K) nf_down2_body<2, true>(L, z, rc, cnx, cny, i0, J, K, r);
+    } else {
+      for (int K = K0; K < K1; ++K) nf_down2_body<1, true>(L, z, rc, cnx, cny, i0, J, K, r);
+    }
+  } else if (L.fz == 2) {
     for (int K = K0; K < K1; ++K) nf_down2_body<2>(L, z, rc, cnx, cny, i0, J, K);
   } else {
     for (int K = K0; K < K1; ++K) nf_down2_body<1>(L, z, rc, cnx, cny, i0, J, K);
@@ -271,7 +288,10 @@ __global__ void __launch_bounds__(256, 4) k_down2_b(const __grid_constant__ NfBa
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int J = blockIdx.y * blockDim.y + threadIdx.y;
   if (i0 >= E.L.nx || J >= B.cny) return;
-  if (E.L.fz == 2) nf_down2_body<2>(E.L, E.z, E.rc, B.cnx, B.cny, i0, J, K);
+  if (B.gen) {
+    if (E.L.fz == 2) nf_down2_body<2, true>(E.L, E.z, E.rc, B.cnx, B.cny, i0, J, K, E.r[0]);
+    else nf_down2_body<1, true>(E.L, E.z, E.rc, B.cnx, B.cny, i0, J, K, E.r[0]);
+  } else if (E.L.fz == 2) nf_down2_body<2>(E.L, E.z, E.rc, B.cnx, B.cny, i0, J, K);
   else nf_down2_body<1>(E.L, E.z, E.rc, B.cnx, B.cny, i0, J, K);
 }
 
@@ -427,9 +447,10 @@ __device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const flo
   return dot;
 }
 
+// flip = 0: the red half sweep; 1: the black one (the same body on the other colour of every row)
 template <bool DOT>
 __global__ void __launch_bounds__(256, 4) k_up2(NfLvK L, float *z, const float *__restrict__ r, int kch,
-                                             NfSolveState *st, int slot) {
+                                             NfSolveState *st, int slot, int flip) {
   nf_pdl_enter();
   if (st && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
@@ -438,11 +459,12 @@ __global__ void __launch_bounds__(256, 4) k_up2(NfLvK L, float *z, const float *
   if (i0 < L.nx && j < L.ny) {
     const int k0 = blockIdx.z * kch, k1 = min(k0 + kch, L.nz);
     for (int k = k0; k < k1; ++k)
-      dot += ((j + k) & 1) ? nf_up2_body<1>(L, z, r, i0, j, k) : nf_up2_body<0>(L, z, r, i0, j, k);
+      dot += ((j + k + flip) & 1) ? nf_up2_body<1>(L, z, r, i0, j, k) : nf_up2_body<0>(L, z, r, i0, j, k);
   }
   if (DOT) nf_block_atomic_add((double)dot, &st->rz[slot]);
 }
-__global__ void __launch_bounds__(256, 4) k_up2_b(const __grid_constant__ NfBatchK B, int kch, int slot) {
+// (slot < 0: no r.z)
+__global__ void __launch_bounds__(256, 4) k_up2_b(const __grid_constant__ NfBatchK B, int kch, int slot, int flip) {
   nf_pdl_enter();
   const int e = (int)blockIdx.z / B.nzc, bz = (int)blockIdx.z - e * B.nzc;
   const NfEnvK &E = B.e[e];
@@ -454,9 +476,9 @@ __global__ void __launch_bounds__(256, 4) k_up2_b(const __grid_constant__ NfBatc
   if (i0 < L.nx && j < L.ny) {
     const int k0 = bz * kch, k1 = min(k0 + kch, L.nz);
     for (int k = k0; k < k1; ++k)
-      dot += ((j + k) & 1) ? nf_up2_body<1>(L, E.z, E.r[0], i0, j, k) : nf_up2_body<0>(L, E.z, E.r[0], i0, j, k);
+      dot += ((j + k + flip) & 1) ? nf_up2_body<1>(L, E.z, E.r[0], i0, j, k) : nf_up2_body<0>(L, E.z, E.r[0], i0, j, k);
   }
-  nf_block_atomic_add((double)dot, &E.st->rz[slot]);
+  if (slot >= 0) nf_block_atomic_add((double)dot, &E.st->rz[slot]);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -563,6 +585,7 @@ __global__ void __launch_bounds__(256) k_dot_rz(const float *__restrict__ a, con
 #define NF_DIRECT_MAX 128
 struct NfTailK {
   int nlev, sweeps;
+  int npre[NF_MAX_LEVELS], npost[NF_MAX_LEVELS];  // red-black sweeps before / after the coarse correction, per level
   int singular;  // the system has the constant null vector (R12): the coarsest solve works in its complement
   int direct;    // 1: the coarsest level is solved with the precomputed inverse
   int n[NF_MAX_LEVELS], nx[NF_MAX_LEVELS], ny[NF_MAX_LEVELS], nz[NF_MAX_LEVELS];
@@ -859,6 +882,11 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
     float *z = sm + T.soff[l], *r = z + T.np[l], *pk = z + 2 * T.np[l];
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, true);
     nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+    for (int s = 1; s < T.npre[l]; ++s) {
+      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
+      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+    }
+    const bool first_only = T.npre[l] == 1;
     // residual + restriction: r_c = 1/8 sum children (r - A z), A z = z/idg - sum wg z_nb on active cells
     const int cn = T.n[l + 1], cnx = T.nx[l + 1], cny = T.ny[l + 1], fz = T.fz[l];
     float *rc = sm + T.soff[l + 1] + T.np[l + 1];
@@ -879,8 +907,10 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
             const float s = pk[1 * n + id] * z[max(id - 1, 0)] + pk[2 * n + id] * z[min(id + 1, n - 1)] +
                       pk[3 * n + id] * z[max(id - sy, 0)] + pk[4 * n + id] * z[min(id + sy, n - 1)] +
                       pk[5 * n + id] * z[max(id - sz, 0)] + pk[6 * n + id] * z[min(id + sz, n - 1)];
-            // (a red cell holds z = r idg exactly, so r - A z = c sum alpha z_nb there; inactive: weights 0)
-            acc += s;
+            // (after ONE sweep a red cell holds z = r idg exactly, so r - A z = c sum alpha z_nb there; inactive:
+            // weights 0.  After more sweeps the red value has been updated: the full expression)
+            const float g = pk[id];
+            acc += first_only ? s : (g > 0.0f ? s + (r[id] - z[id] / g) : 0.0f);
           }
       rc[cidx] = (fz == 2 ? 0.125f : 0.25f) * acc;
     }
@@ -953,8 +983,10 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
       z[id] += zc[((fz == 2 ? k >> 1 : k) * cny + (j >> 1)) * cnx + (i >> 1)];
     }
     __syncthreads();
-    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
-    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
+    for (int s = 0; s < T.npost[l]; ++s) {
+      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
+    }
   }
   for (int t = threadIdx.x; t < T.n[0]; t += blockDim.x) zg[t] = sm[T.soff[0] + t];
 }
@@ -1007,7 +1039,7 @@ __device__ __forceinline__ void nf_dense_down1(const NfDenseLv &D, int id) {
   D.z[id] = a * idg;
 }
 // residual + restriction of the coarse cell cid: red children only (the black residual is zero)
-__device__ __forceinline__ void nf_dense_down2(const NfDenseLv &D, float *rc, int cnx, int cny, int cid) {
+__device__ __forceinline__ void nf_dense_down2(const NfDenseLv &D, float *rc, int cnx, int cny, int cid, bool gen) {
   const int I = cid % cnx, J = (cid / cnx) % cny, K = cid / (cnx * cny);
   float acc = 0.0f;
 #pragma unroll
@@ -1023,7 +1055,9 @@ __device__ __forceinline__ void nf_dense_down2(const NfDenseLv &D, float *rc, in
         float s = 0.0f;
 #pragma unroll
         for (int f = 0; f < 6; ++f) s += D.pk[(1 + f) * D.n + id] * D.z[nb[f]];
-        if (D.pk[id] > 0.0f) acc += s;  // (r - A z = c sum alpha z_nb on a red cell: z = r / diag there)
+        // (after ONE sweep r - A z = c sum alpha z_nb on a red cell: z = r / diag there; after more, the full expression)
+        const float g = D.pk[id];
+        if (g > 0.0f) acc += gen ? s + (D.r[id] - D.z[id] / g) : s;
       }
   rc[cid] = 0.125f * acc;
 }
@@ -1043,10 +1077,10 @@ __device__ __forceinline__ void nf_dense_up1(const NfDenseLv &D, const float *zc
   }
   D.z[id] = a * D.pk[id];
 }
-// red half sweep (its black neighbours are final)
-__device__ __forceinline__ void nf_dense_up2(const NfDenseLv &D, int id) {
+// half sweep on the cells of one colour (0 = red, 1 = black)
+__device__ __forceinline__ void nf_dense_up2(const NfDenseLv &D, int id, int color = 0) {
   const int i = id % D.nx, j = (id / D.nx) % D.ny, k = id / (D.nx * D.ny);
-  if ((i + j + k) & 1) return;
+  if (((i + j + k) & 1) != color) return;
   int nb[6];
   nf_dense_nb(D, id, nb);
   float a = D.r[id];
@@ -1058,6 +1092,7 @@ __device__ __forceinline__ void nf_dense_up2(const NfDenseLv &D, int id) {
 struct NfCoarseK {
   int first, nb, has_tail;
   int dense_from;  // levels >= dense_from (and < nb) run the per-cell phases
+  int nu[NF_MAX_LEVELS];  // red-black sweeps before and after the coarse correction, per level
   const float *pk[NF_MAX_LEVELS];
   NfLvK lv[NF_MAX_LEVELS];
   float *z[NF_MAX_LEVELS], *r[NF_MAX_LEVELS];
@@ -1090,6 +1125,24 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
       for (size_t o = (size_t)gt * 32; o < nzf; o += (size_t)gn * 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(L.az + o));
     }
   }
+  // one half sweep of level l as a phase: color 0 = red, 1 = black
+  auto half = [&](int l, int color) {
+    const NfLvK &L = P.lv[l];
+    if (l >= P.dense_from) {
+      NfDenseLv D;
+      D.pk = P.pk[l]; D.z = P.z[l]; D.r = P.r[l]; D.nx = L.nx; D.ny = L.ny; D.nz = L.nz; D.n = L.nx * L.ny * L.nz;
+      for (int t = gt; t < D.n; t += gn) nf_dense_up2(D, t, color);
+    } else {
+      const int nx4 = L.nx >> 2, ny = L.ny, nz = L.nz;
+      for (int t = gt; t < nx4 * ny * nz; t += gn) {
+        const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
+        if ((j + k + color) & 1)
+          nf_up2_body<1>(L, P.z[l], P.r[l], i0, j, k);
+        else
+          nf_up2_body<0>(L, P.z[l], P.r[l], i0, j, k);
+      }
+    }
+  };
   for (int l = P.first; l < P.nb; ++l) {
     const NfLvK &L = P.lv[l];
     const int nx4 = L.nx >> 2, ny = L.ny, nz = L.nz;
@@ -1109,12 +1162,24 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
       }
     }
     sync();
+    for (int s = 1; s < P.nu[l]; ++s) {  // further pre-smoothing sweeps: red, black
+      half(l, 0);
+      sync();
+      half(l, 1);
+      sync();
+    }
+    const bool gen = P.nu[l] > 1;
     if (dense) {
-      for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t);
+      for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t, gen);
     } else {
       for (int t = gt; t < nx4 * cny * cnz; t += gn) {
         const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
-        if (L.fz == 2)
+        if (gen) {
+          if (L.fz == 2)
+            nf_down2_body<2, true>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
+          else
+            nf_down2_body<1, true>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
+        } else if (L.fz == 2)
           nf_down2_body<2>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
         else
           nf_down2_body<1>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
@@ -1154,16 +1219,12 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
       }
     }
     sync();
-    if (dense) {
-      for (int t = gt; t < D.n; t += gn) nf_dense_up2(D, t);
-    } else {
-      for (int t = gt; t < nx4 * ny * nz; t += gn) {
-        const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
-        if ((j + k) & 1)
-          nf_up2_body<1>(L, P.z[l], P.r[l], i0, j, k);
-        else
-          nf_up2_body<0>(L, P.z[l], P.r[l], i0, j, k);
-      }
+    half(l, 0);
+    for (int s = 1; s < P.nu[l]; ++s) {  // further post-smoothing sweeps: black, red
+      sync();
+      half(l, 1);
+      sync();
+      half(l, 0);
     }
     if (l > P.first) sync();
   }
@@ -1225,6 +1286,7 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_c
 // ------------------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------------------
+static inline int nf_nu_coarse(const nf_grid *g, int l) { return l <= 1 ? g->nu_l1 : g->nu_deep; }
 #define NF_TAIL_SMEM_MAX 231424  // dynamic shared memory of k_tail / k_vcoarse (226 KB of the 227 KB a CTA may use)
 
 // Shared-memory layout of a tail that starts at level `first` (NfTailK); T.total_floats is what it needs.
@@ -1250,6 +1312,10 @@ static void tail_desc(const nf_grid *g, int first, NfTailK *T) {
   so += 1024;
   T->total_floats = so;
   T->sweeps = 2 * m;
+  for (int l = first; l < nl; ++l) {
+    T->npre[l - first] = l == 0 ? g->nu_pre : nf_nu_coarse(g, l);
+    T->npost[l - first] = l == 0 ? g->nu_post : nf_nu_coarse(g, l);
+  }
   T->singular = g->singular_info;  // (only read when the coarsest level is too large for the direct solve)
 }
 static size_t tail_smem_bytes(const nf_grid *g) {
@@ -1353,6 +1419,7 @@ static void fill_coarse(const nf_grid *g, NfCoarseK *P) {
   const int nl = g->nlev, nb = g->tail < nl ? g->tail : nl - 1;
   memset(P, 0, sizeof(*P));
   P->first = 1; P->nb = nb; P->has_tail = 1;
+  for (int l = 0; l < NF_MAX_LEVELS; ++l) P->nu[l] = nf_nu_coarse(g, l);
   P->dense_from = NF_MAX_LEVELS;
   for (int l = 0; l < nl; ++l) {
     P->lv[l] = nf_lvk(g->lv[l]);
@@ -1409,13 +1476,24 @@ int nf_vcycle_batch(nf_grid **G, int n, const NfBatchK &Bin, int slot) {
   NfDims d2 = nf_vdims(L.nx / 4, C.ny, C.nz, 1);
   B.nzc = (int)d2.grid.z;
   d2.grid.z *= n;
+  B.gen = g->nu_pre > 1 ? 1 : 0;
+  if (g->nu_pre > 1) {  // further pre-smoothing sweeps on the finest level: red, black
+    B.nzc = (int)d.grid.z;
+    dim3 gs = d.grid;
+    gs.z *= n;
+    for (int s = 1; s < g->nu_pre; ++s)
+      for (int color = 0; color < 2; ++color)
+        NF_LAUNCH(g, NFK_SWEEP_0, nf_launch_pdl(k_up2_b, gs, d.block, g->stream, B, kch, -1, color));
+    B.nzc = (int)(d2.grid.z / n);
+  }
   NF_LAUNCH(g, NFK_DOWN2_0, nf_launch_pdl(k_down2_b, d2.grid, d2.block, g->stream, B));
   {
     NfCoarseBatchK CB;
     memset(&CB, 0, sizeof(CB));
     CB.n = n; CB.nctas = g->coarse_ctas;
     const int nb = g->tail;
-    CB.nbar = 4 * (nb - 1) - 1 + 1;  // four phases per level 1 .. nb-1 (none after the last), one after the tail
+    CB.nbar = 0;  // 4 nu phases per level 1 .. nb-1 (no barrier after the last), one after the tail
+    for (int l = 1; l < nb; ++l) CB.nbar += 4 * nf_nu_coarse(g, l);
     for (int e = 0; e < n; ++e) {
       CB.base[e] = G[e]->cbar_count;
       CB.bar[e] = G[e]->cbar;
@@ -1430,7 +1508,10 @@ int nf_vcycle_batch(nf_grid **G, int n, const NfBatchK &Bin, int slot) {
   dim3 gb = d.grid;
   gb.z *= n;
   NF_LAUNCH(g, NFK_UP1_0, nf_launch_pdl(k_up1_b, gb, d.block, g->stream, B, kch));
-  NF_LAUNCH(g, NFK_UP2_0, nf_launch_pdl(k_up2_b, gb, d.block, g->stream, B, kch, slot));
+  for (int s = 1; s < g->nu_post; ++s)
+    for (int color = 0; color < 2; ++color)
+      NF_LAUNCH(g, NFK_SWEEP_0, nf_launch_pdl(k_up2_b, gb, d.block, g->stream, B, kch, -1, color));
+  NF_LAUNCH(g, NFK_UP2_0, nf_launch_pdl(k_up2_b, gb, d.block, g->stream, B, kch, slot, 0));
   NF_CUDA(g, cudaGetLastError());
   return NF_OK;
 }
@@ -1449,7 +1530,7 @@ int nf_update_down1_batch(nf_grid **G, int n, const NfBatchK &Bin, int slot, int
 
 // z = M^{-1} r on level 0 (lv[0].r -> lv[0].z).  with_dot: accumulate r.z into st->rz[slot] and honour st->done.
 bool nf_update_down1_ok(const nf_grid *g) {
-  return g->nu_pre == 1 && g->nu_post == 1 && !g->force_generic && g->lv[0].vec && g->nlev > 1;
+  return g->nu_pre == g->nu_post && !g->force_generic && g->lv[0].vec && g->nlev > 1;
 }
 int nf_update_down1(nf_grid *g, int slot, NfHostStatus *hs, int seq) {
   NfLevel &L = g->lv[0];
@@ -1468,7 +1549,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
   const int nl = g->nlev;
   const bool has_tail = g->tail < nl;
   const int nb = has_tail ? g->tail : nl - 1;
-  const bool fused = g->nu_pre == 1 && g->nu_post == 1 && !g->force_generic;
+  const bool fused = g->nu_pre == g->nu_post && !g->force_generic;
   bool dot_done = false;
   const bool coop = fused && g->coarse_ctas > 0 && g->lv[0].vec;
   for (int l = 0; l < (coop ? 1 : nb); ++l) {
@@ -1476,12 +1557,16 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
     if (L.vec && fused) {
       const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
+      const int nu = l == 0 ? g->nu_pre : nf_nu_coarse(g, l);
       if (!(l == 0 && skip_down1))
         NF_LAUNCH(g, (l == 0 ? NFK_DOWN1_0 : NFK_VEC_C), nf_launch_pdl(k_down1, d.grid, d.block, g->stream, nf_lvk(L), L.r, L.z, kch, (const NfSolveState *)st));
+      for (int s = 1; s < nu; ++s)  // further sweeps: red, black
+        for (int color = 0; color < 2; ++color)
+          NF_LAUNCH(g, (l == 0 ? NFK_SWEEP_0 : NFK_VEC_C), nf_launch_pdl(k_up2<false>, d.grid, d.block, g->stream, nf_lvk(L), L.z, (const float *)L.r, kch, st, slot, color));
       NfDims d2 = nf_vdims(L.nx / 4, C.ny, C.nz, 1);
-      NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), nf_launch_pdl(k_down2, d2.grid, d2.block, g->stream, nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, 1, (const NfSolveState *)st));
+      NF_LAUNCH(g, (l == 0 ? NFK_DOWN2_0 : NFK_VEC_C), nf_launch_pdl(k_down2, d2.grid, d2.block, g->stream, nf_lvk(L), L.z, C.r, C.nx, C.ny, C.nz, 1, (const NfSolveState *)st, (const float *)(nu > 1 ? L.r : nullptr)));
     } else {
-      for (int s = 0; s < g->nu_pre; ++s) {
+      for (int s = 0; s < (l == 0 ? g->nu_pre : nf_nu_coarse(g, l)); ++s) {
         smooth_half(g, L, 0, s == 0, false, st, slot);
         smooth_half(g, L, 1, false, false, st, slot);
       }
@@ -1517,18 +1602,23 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
     if (L.vec && fused) {
       const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
+      const int nu = l == 0 ? g->nu_post : nf_nu_coarse(g, l);
       NF_LAUNCH(g, (l == 0 ? NFK_UP1_0 : NFK_VEC_C), nf_launch_pdl(k_up1, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, C.z, C.nx, C.ny, kch, (const NfSolveState *)st));
+      for (int s = 1; s < nu; ++s)  // (up1 was the first black half sweep) red, then the next black one
+        for (int color = 0; color < 2; ++color)
+          NF_LAUNCH(g, (l == 0 ? NFK_SWEEP_0 : NFK_VEC_C), nf_launch_pdl(k_up2<false>, d.grid, d.block, g->stream, nf_lvk(L), L.z, (const float *)L.r, kch, st, slot, color));
       if (l == 0 && with_dot) {
-        NF_LAUNCH(g, NFK_UP2_0, nf_launch_pdl(k_up2<true>, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, kch, g->st, slot));
+        NF_LAUNCH(g, NFK_UP2_0, nf_launch_pdl(k_up2<true>, d.grid, d.block, g->stream, nf_lvk(L), L.z, (const float *)L.r, kch, g->st, slot, 0));
         dot_done = true;
       } else {
-        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), nf_launch_pdl(k_up2<false>, d.grid, d.block, g->stream, nf_lvk(L), L.z, L.r, kch, st, slot));
+        NF_LAUNCH(g, (l == 0 ? NFK_UP2_0 : NFK_VEC_C), nf_launch_pdl(k_up2<false>, d.grid, d.block, g->stream, nf_lvk(L), L.z, (const float *)L.r, kch, st, slot, 0));
       }
     } else {
       NfDims d = nf_dims(L.nx, L.ny, L.nz);
       NF_LAUNCH(g, (l == 0 ? NFK_PROLONG0 : NFK_PROLONG_C), k_prolong_add<<<d.grid, d.block, 0, g->stream>>>(L.z, C.z, L.nx, L.ny, L.nz, C.nx, C.ny, L.fz, st));
-      for (int s = 0; s < g->nu_post; ++s) {
-        const bool dot = with_dot && l == 0 && s == g->nu_post - 1;
+      const int nu = l == 0 ? g->nu_post : nf_nu_coarse(g, l);
+      for (int s = 0; s < nu; ++s) {
+        const bool dot = with_dot && l == 0 && s == nu - 1;
         smooth_half(g, L, 1, false, false, st, slot);
         smooth_half(g, L, 0, false, dot, st, slot);
         dot_done = dot_done || dot;

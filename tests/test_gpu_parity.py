@@ -287,14 +287,20 @@ def test_vcycle_matches_fp64_reference(torch, api, shape, bt, seed):
     alpha = [a.cpu().numpy() for a in g.get_weights()]
     act = orc.active_cells([a.astype(np.float64) for a in alpha])
     r = (np.random.default_rng(4).standard_normal((nz, ny, nx)) * act).astype(np.float32)
-    ref = vc_ref(r, alpha, 0.5 * nx, bool(g.info()["singular"]))
     z1, z2 = torch.empty(g.shape_p, device="cuda"), torch.empty(g.shape_p, device="cuda")
-    g.vcycle(dev(torch, r), z1)
-    g.set_solver_options(1, 1, 2)
-    g.vcycle(dev(torch, r), z2)
+    # sweeps on (level 1, the levels below): the default of grids this size, the default of large grids, V(1,1)
+    for nu_l1, nu_deep in ((1, 2), (2, 3), (1, 1)):
+        ref = vc_ref(r, alpha, 0.5 * nx, bool(g.info()["singular"]), nu_fine=1, nu_l1=nu_l1, nu_deep=nu_deep)
+        g.set_coarse_sweeps(nu_l1, nu_deep)
+        g.set_solver_options(1, 1, 0)
+        g.vcycle(dev(torch, r), z1)
+        g.set_solver_options(1, 1, 2)
+        g.vcycle(dev(torch, r), z2)
+        assert rel(host(z1), ref) < 2e-5, (nu_l1, nu_deep)
+        # (the generic path's cancellation noise passes through every further sweep of the weakly connected cell:
+        # 2.0e-3 at (2, 3) on blob field 9 at 128^3 against 1.4e-3 at (1, 1); the fused path stays below 2e-5)
+        assert rel(host(z2), ref) < (2e-3 if (nu_l1, nu_deep) == (1, 1) else 4e-3), (nu_l1, nu_deep)
     g.close()
-    assert rel(host(z1), ref) < 2e-5
-    assert rel(host(z2), ref) < 2e-3
 
 
 @pytest.mark.parametrize("shape", [(24, 20, 16), (64, 64, 64), (16, 16, 16)])

@@ -3,8 +3,9 @@
 NOT the oracle (the paper defines the projection's RESULT, not the preconditioner: every multigrid parameter is this
 library's own choice, DESIGN.md section 6 / R13) -- a slow third implementation of that documented choice, used to
 check the CUDA V-cycle kernels (fused 4-launch levels, cooperative coarse kernel with its packed per-cell phases,
-shared-memory tail) against something that carries no fp32 rounding: V(1,1), red-black Gauss-Seidel (pre: red then
-black from a zero guess; post: black then red), piecewise-constant prolongation P, restriction P^T / 8,
+shared-memory tail) against something that carries no fp32 rounding: V(nu, nu) with nu chosen per level (the finest
+level, level 1, every level below: 1, 1, 2 by default -- the library's choice for grids below 6 M cells), red-black Gauss-Seidel (pre: red then black, the first sweep from a zero
+guess; post: black then red), piecewise-constant prolongation P, restriction P^T / 8,
 rediscretised coarse operators with c_l = c / 4^l on weights that are the mean of the four coincident fine face
 weights (absent fine faces of an odd edge count as closed), extents halving -- rounding up -- while they stay >= 4
 (>= 2 while the level has more than 128 cells), coarsest level (<= 128 cells): exact solve (the
@@ -67,7 +68,9 @@ def _diag(a):
     return au[:, :, :-1] + au[:, :, 1:] + av[:, :-1, :] + av[:, 1:, :] + aw[:-1] + aw[1:]
 
 
-def vcycle(r, alpha, c, singular):
+def vcycle(r, alpha, c, singular, nu_fine=1, nu_l1=1, nu_deep=2):
+    """nu_fine / nu_l1 / nu_deep: red-black sweeps before and after the coarse correction on the finest level / on
+    level 1 / on every level below that (the library's defaults: nf_set_solver_options, nf_set_coarse_sweeps)."""
     levels = [[x.astype(np.float64) for x in a] for a in hierarchy(alpha)]
 
     def rec(l, r, c):
@@ -109,14 +112,17 @@ def vcycle(r, alpha, c, singular):
             if singular:
                 z = np.where(act, z - z[act].sum() / max(int(act.sum()), 1), z)
             return z
-        half(red); half(~red)
+        nu = nu_fine if l == 0 else (nu_l1 if l == 1 else nu_deep)
+        for _ in range(nu):
+            half(red); half(~red)
         res = np.where(act, r - (d * z - c * _nbsum(z, a)), 0.0)
         ez, ey, ex = nz + (nz & 1), ny + (ny & 1), nx + (nx & 1)
         rp = np.zeros((ez, ey, ex)); rp[:nz, :ny, :nx] = res          # (absent children of an odd edge contribute 0)
         rc = 0.125 * rp.reshape(ez // 2, 2, ey // 2, 2, ex // 2, 2).sum(axis=(1, 3, 5))
         zc = rec(l + 1, rc, 0.25 * c)
         z += np.repeat(np.repeat(np.repeat(zc, 2, axis=0), 2, axis=1), 2, axis=2)[:nz, :ny, :nx]
-        half(~red); half(red)
+        for _ in range(nu):
+            half(~red); half(red)
         return z
 
     return rec(0, np.asarray(r, dtype=np.float64), float(c))
