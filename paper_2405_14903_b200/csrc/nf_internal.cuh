@@ -68,9 +68,16 @@ struct alignas(128) NfSolveState {
   double bb;    // ||b||^2 after masking / mean removal
   double tol2;  // (tolerance of the current phase)^2
   double relres;  // sqrt(rr/bb) at the last executed iteration
+  // Singular system with ONE fluid component (gauge mode 1): the residual is kept compatible -- zero mean over the
+  // active cells -- in every iteration (k_update_down1), not only at the start: fp32 cannot remove a mean of 5e-9 |b|
+  // from b itself (it is below the rounding of the entries), the mean stays while the residual falls by 1e-6, and
+  // the V-cycle amplifies the constant mode: PCG then stalled near 1e-6 and DIVERGED.
+  double inv_nact;  // 1 / #active cells when that projection is on, else 0
+  double sb;        // sum of the prepared right-hand side b0 as stored (what the true residual's mean is)
   alignas(128) double pq[2];
   alignas(128) double rr[2];
   alignas(128) double rz[2];
+  alignas(128) double sr[2];  // sum of the residual written in iteration parity s (or sr[1]: at the start of a phase)
   alignas(128) double sum;   // scratch: sum over active cells
 };
 
@@ -391,6 +398,7 @@ __device__ __forceinline__ void nf_cg_check(NfSolveState *st, int slot, NfHostSt
     st->pq[1 - slot] = 0.0;
     st->rr[1 - slot] = 0.0;
     st->rz[1 - slot] = 0.0;
+    st->sr[1 - slot] = 0.0;
     st->relres = st->bb > 0.0 ? sqrt(rr / st->bb) : 0.0;
   }
   hs->relres = (float)st->relres;

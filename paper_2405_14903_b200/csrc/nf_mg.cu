@@ -45,7 +45,8 @@ __device__ __forceinline__ NfRow4 nf_row(const float *f, const uint8_t *__restri
 // R4(at, ok) / R1(at, ok): the right-hand side r on a row of 4 cells / one cell (0 when !ok).  k_down1 reads it from
 // memory; k_update_down1 evaluates r - a q on the fly.  Returns the row of r of the thread's own 4 cells.
 template <int PAR, class F4, class F1>
-__device__ __forceinline__ float4 nf_down1_core(const NfLvK &L, F4 R4, F1 R1, float *z, int i0, int j, int k) {
+__device__ __forceinline__ float4 nf_down1_core(const NfLvK &L, F4 R4, F1 R1, float *z, int i0, int j, int k,
+                                                unsigned *c4_out = nullptr) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const nf_idx sy = nx, sz = (nf_idx)nx * ny;
   const nf_idx id = ((nf_idx)k * ny + j) * nx + i0;
@@ -54,6 +55,7 @@ __device__ __forceinline__ float4 nf_down1_core(const NfLvK &L, F4 R4, F1 R1, fl
   const float4 crow = R4(id, true);
   nf_unpack4(crow, C.v);
   C.c4 = nf_ldc4(L.code, id, true);
+  if (c4_out) *c4_out = C.c4;
   float out[4], yl[4], yh[4], zl[4], zh[4];
   nf_unpack4(R4(id - sy, j > 0), yl);
   nf_unpack4(R4(id + sy, j + 1 < ny), yh);
@@ -131,25 +133,40 @@ __device__ __forceinline__ void nf_update_down1_body(const NfLvK &L, const float
   }
   const double pq = st->pq[slot];
   const float a = (pq > 0.0) ? (float)(st->rz[slot] / pq) : 0.0f;
+  // singular system: mu = mean of the residual being read (measured when it was written), taken off on the fly, so
+  // that the residual stays compatible while it shrinks (NfSolveState::inv_nact; 0 = off)
+  const bool proj = st->inv_nact != 0.0;
+  const float mu = proj ? (float)(st->sr[1 - slot] * st->inv_nact) : 0.0f;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   float part = 0.0f;
+  double sum = 0.0;
   if (i0 < L.nx && j < L.ny) {
+    // (rows outside the grid: ghosts, 0.  Inactive cells inside it get -mu here; every use of a neighbour's value
+    // multiplies it by that cell's inverse diagonal -- 0 when inactive -- or sits on the all-open fast path.)
     auto R4 = [&](nf_idx at, bool ok) {
       float4 v = nf_ld4(rold, at, ok);
       const float4 w = nf_ld4(q, at, ok);
-      v.x -= a * w.x; v.y -= a * w.y; v.z -= a * w.z; v.w -= a * w.w;
+      const float m = ok ? mu : 0.0f;
+      v.x = (v.x - m) - a * w.x; v.y = (v.y - m) - a * w.y; v.z = (v.z - m) - a * w.z; v.w = (v.w - m) - a * w.w;
       return v;
     };
-    auto R1 = [&](nf_idx at, bool ok) { return nf_ld1(rold, at, ok) - a * nf_ld1(q, at, ok); };
+    auto R1 = [&](nf_idx at, bool ok) { return (nf_ld1(rold, at, ok) - (ok ? mu : 0.0f)) - a * nf_ld1(q, at, ok); };
     const int k0 = bz * kch, k1 = min(k0 + kch, L.nz);
     for (int k = k0; k < k1; ++k) {
-      const float4 c = ((j + k) & 1) ? nf_down1_core<1>(L, R4, R1, z, i0, j, k) : nf_down1_core<0>(L, R4, R1, z, i0, j, k);
+      unsigned c4;
+      float4 c = ((j + k) & 1) ? nf_down1_core<1>(L, R4, R1, z, i0, j, k, &c4) : nf_down1_core<0>(L, R4, R1, z, i0, j, k, &c4);
+      if (proj) {  // the residual of an inactive cell stays 0
+        c.x = (c4 & 0xffu) ? c.x : 0.0f; c.y = (c4 & 0xff00u) ? c.y : 0.0f;
+        c.z = (c4 & 0xff0000u) ? c.z : 0.0f; c.w = (c4 & 0xff000000u) ? c.w : 0.0f;
+        sum += (double)((c.x + c.y) + (c.z + c.w));
+      }
       *reinterpret_cast<float4 *>(rnew + ((nf_idx)k * L.ny + j) * L.nx + i0) = c;
       part += (c.x * c.x + c.y * c.y) + (c.z * c.z + c.w * c.w);
     }
   }
   nf_block_atomic_add((double)part, &st->rr[slot]);
+  if (proj) nf_block_atomic_add(sum, &st->sr[slot]);
   if (threadIdx.x == 0 && threadIdx.y == 0) {
     __threadfence();
     const unsigned total = gridDim.x * gridDim.y * (unsigned)nzc;

@@ -366,10 +366,11 @@ __global__ void __launch_bounds__(256) k_mask4(const float *src, float *dst, flo
   if (sum) nf_block_atomic_add(s, sum);
   if (sq) nf_block_atomic_add(q, sq);
 }
+// (sout: the sum of the centred values AS STORED -- fp32 cannot take a mean of a few 1e-9 |b| off entries of size |b|)
 __global__ void __launch_bounds__(256) k_center4(float *dst, float *dst2, const uint8_t *__restrict__ code, size_t n4,
-                                                 const double *sum, double inv_nact, double *sq) {
+                                                 const double *sum, double inv_nact, double *sq, double *sout = nullptr) {
   const float m = (float)((*sum) * inv_nact);
-  double q = 0.0;
+  double q = 0.0, so = 0.0;
   const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
   for (size_t t = tid; t < n4; t += nth) {
     float4 v = reinterpret_cast<const float4 *>(dst)[t];
@@ -379,17 +380,22 @@ __global__ void __launch_bounds__(256) k_center4(float *dst, float *dst2, const 
     reinterpret_cast<float4 *>(dst)[t] = v;
     if (dst2) reinterpret_cast<float4 *>(dst2)[t] = v;
     q += ((double)v.x * v.x + (double)v.y * v.y) + ((double)v.z * v.z + (double)v.w * v.w);
+    so += ((double)v.x + v.y) + ((double)v.z + v.w);
   }
   if (sq) nf_block_atomic_add(q, sq);
+  if (sout) nf_block_atomic_add(so, sout);
 }
 
-__global__ void k_init_state(NfSolveState *st, double tol, int maxit) {
+__global__ void k_init_state(NfSolveState *st, double tol, int maxit, double inv_nact_proj) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   st->pq[0] = st->pq[1] = 0.0;
   st->rr[0] = st->rr[1] = 0.0;
   st->rz[0] = st->rz[1] = 0.0;
   st->bb = 0.0;
   st->sum = 0.0;
+  st->sr[0] = st->sr[1] = 0.0;
+  st->sb = 0.0;
+  st->inv_nact = inv_nact_proj;
   st->tol2 = tol * tol;
   st->relres = 0.0;
   st->iter = 0;
@@ -403,6 +409,7 @@ __global__ void k_init_state(NfSolveState *st, double tol, int maxit) {
 __global__ void k_start_state(NfSolveState *st) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   st->sum = 0.0;
+  st->sr[1] = st->sb;  // (the first iteration has parity 0 and reads the sum of the residual it starts from in sr[1])
   if (!(st->bb > 0.0)) {
     st->done = 1;
     st->converged = (st->bb == 0.0) ? 1 : 0;
@@ -424,6 +431,8 @@ __global__ void k_phase_begin(NfSolveState *st, double tol, int keep_done) {
   st->pq[0] = st->pq[1] = 0.0;
   st->rr[0] = st->rr[1] = 0.0;
   st->rz[0] = st->rz[1] = 0.0;
+  st->sr[0] = 0.0;
+  if (!keep_done) st->sr[1] = 0.0;  // (keep_done: the first phase, whose sr[1] k_start_state has just set)
   st->ticket = 0;
   st->last_slot = -1;
   if (!keep_done) {
@@ -465,7 +474,10 @@ __global__ void __launch_bounds__(256, 4) k_true_residual4(NfLvK L, float *__res
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z * blockDim.z + threadIdx.z;
-  double part = 0.0;
+  double part = 0.0, sum = 0.0;
+  // singular system (NfSolveState::inv_nact): b0 as stored has the mean sb / #active, A x has none -- taken off here,
+  // in fp64, where the subtraction is exact; what the fp32 rounding of r leaves is measured into sr[1]
+  const double mb = st->sb * st->inv_nact;
   if (i0 < L.nx && j < L.ny && k < L.nz) {
     const int nx = L.nx, ny = L.ny, nz = L.nz;
     const nf_idx sy = nx, sz = (nf_idx)nx * ny, id = ((nf_idx)k * ny + j) * nx + i0;
@@ -486,13 +498,15 @@ __global__ void __launch_bounds__(256, 4) k_true_residual4(NfLvK L, float *__res
       const double s = (((double)w.xl * (c0 - l) + (double)w.xh * (c0 - h)) +
                         ((double)w.yl * (c0 - (double)yl[t]) + (double)w.yh * (c0 - (double)yh[t]))) +
                        ((double)w.zl * (c0 - (double)zl[t]) + (double)w.zh * (c0 - (double)zh[t]));
-      const double v = code ? (double)bb[t] - (double)L.c * s : 0.0;
+      const double v = code ? ((double)bb[t] - mb) - (double)L.c * s : 0.0;
       out[t] = (float)v;
       part += v * v;
+      sum += (double)out[t];
     }
     *reinterpret_cast<float4 *>(r + id) = make_float4(out[0], out[1], out[2], out[3]);
   }
   nf_block_atomic_add(part, &st->rr[0]);
+  if (st->inv_nact != 0.0) nf_block_atomic_add(sum, &st->sr[1]);
 }
 // warm start: the initial guess on the active cells only (0 elsewhere), and 0 everywhere when b = 0 (done is then
 // already set by k_start_state: the answer is x = 0).  NaN, inf and absurdly large entries (an uninitialised array
@@ -584,10 +598,13 @@ int nf_apply_A_impl(nf_grid *g, const float *p, float *q) {
 int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit) {
   NfLevel &L = g->lv[0];
   NfDims d = nf_dims(L.nx, L.ny, L.nz);
-  NF_LAUNCH(g, NFK_SETUP, k_init_state<<<1, 32, 0, g->stream>>>(g->st, (double)tol, maxit));
   const double inv = g->nact > 0 ? 1.0 / (double)g->nact : 0.0;
   const float *in = src ? src : L.r;
   const size_t n = (size_t)L.ncell;
+  // the per-iteration compatibility projection of the residual (NfSolveState::inv_nact): one singular component, on
+  // the float4 / cell-code path
+  const bool projr = g->gauge_mode != 2 && g->singular && !g->force_generic && vec_ok(in, L.r, g->b0, g->b0, n);
+  NF_LAUNCH(g, NFK_SETUP, k_init_state<<<1, 32, 0, g->stream>>>(g->st, (double)tol, maxit, projr ? inv : 0.0));
   if (g->gauge_mode == 2) {
     // several fluid components, some without a Dirichlet face: compatibility per component (nf_components.cu)
     if (!g->force_generic && vec_ok(in, L.r, g->b0, g->b0, n)) {
@@ -602,7 +619,7 @@ int nf_solve_prepare_from(nf_grid *g, const float *src, float tol, int maxit) {
       NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(in, L.r, g->b0, L.code, n >> 2, nullptr, &g->st->bb));
     } else {
       NF_LAUNCH(g, NFK_SETUP, k_mask4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(in, L.r, nullptr, L.code, n >> 2, &g->st->sum, nullptr));
-      NF_LAUNCH(g, NFK_SETUP, k_center4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(L.r, g->b0, L.code, n >> 2, &g->st->sum, inv, &g->st->bb));
+      NF_LAUNCH(g, NFK_SETUP, k_center4<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(L.r, g->b0, L.code, n >> 2, &g->st->sum, inv, &g->st->bb, &g->st->sb));
     }
     NF_LAUNCH(g, NFK_SETUP, k_start_state<<<1, 32, 0, g->stream>>>(g->st));
   } else {
@@ -926,6 +943,8 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
     rc = correct(tol);
     if (rc != NF_OK) return rc;
   }
+  // (phase 1 met its own 30 tol on the very last iteration allowed: that is not the caller's tolerance)
+  if (two_phase && ph.converged && ph.iters >= maxit && !(ph.relres <= tol)) ph.converged = 0;
   g->last_iters = ph.iters;
   NF_TRY(apply_gauge(g, x));
   g->last_relres = ph.relres;
