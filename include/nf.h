@@ -288,6 +288,25 @@ long long nf_launch_count(nf_grid *g);
 /* Last error message of this handle (static storage inside the handle; "" if none). */
 const char *nf_last_error(nf_grid *g);
 
+/* The reduction of nf_max_speed (R24) for callers that must not allocate -- code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc.  No handle (nf_grid_create allocates), no
+ * cudaMalloc / cudaFree / allocating library call, no stream synchronisation: two kernels are enqueued on cuda_stream
+ * (a cudaStream_t; NULL = legacy stream 0) of the CURRENT device and *max_abs_dev -- a DEVICE pointer to one float,
+ * owned by the caller -- receives max over all faces of |u|, |v|, |w| (a NaN propagates) when they have run.
+ * u, v, w: DEVICE arrays in the MAC layout of this header, (nx+1) ny nz, nx (ny+1) nz, nx ny (nz+1) floats, read only.
+ * Scratch: a fixed 64 KB array in the library's device image (one per GPU that loads the library, held until the
+ * process exits): one partial maximum per 16384 faces, so u + v + w faces <= 268 435 456 (cubes up to about 440^3;
+ * 256^3 uses 3 084 of the 16 384 partials).  Larger grids, NULL pointers and non-positive extents return
+ * NF_ERR_INVALID; NF_ERR_CUDA if the array's address cannot be resolved or a launch fails; nf_static_last_error()
+ * (thread-local static storage) says which.  The array's address is resolved on the first call on each device
+ * (cudaGetSymbolAddress: make that call outside a capture).  All calls on a device SHARE the array and it keeps the
+ * last call's contents: nothing in it needs clearing (a call reads only the partials it has just written), calls on
+ * one stream are ordered, but calls that OVERLAP on the GPU -- different streams, concurrently replayed graphs -- race
+ * on it and must be serialised by the caller. */
+int nf_max_speed_static(const float *u, const float *v, const float *w, int nx, int ny, int nz, void *cuda_stream,
+                        float *max_abs_dev);
+const char *nf_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

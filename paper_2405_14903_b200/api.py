@@ -70,6 +70,8 @@ _SIGNATURES = {
                                       ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)]),
     "nf_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
     "nf_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
+    "nf_max_speed_static": (ctypes.c_int, [_c_float_p] * 3 + [ctypes.c_int] * 3 + [ctypes.c_void_p, _c_float_p]),
+    "nf_static_last_error": (ctypes.c_char_p, []),
 }
 EXPORTED_SYMBOLS = tuple(_SIGNATURES)
 
@@ -513,3 +515,27 @@ def project_adjoint_batch(grids, G, y, p_saved=None, uhat=None, galpha=None, gus
                                          float(tol), int(maxit), st)
     g0._check(rc, "nf_project_adjoint_batch")
     return list(st)
+
+
+def max_speed_static(u, v, w, out, stream=None):
+    """nf_max_speed_static: max over all faces of |u|, |v|, |w| into the one-element DEVICE tensor `out`, without a
+    handle and without any allocation (fixed scratch inside the library, include/nf.h).  Enqueued on `stream`
+    (default: torch's current stream of the tensors' device); no synchronisation.  Calls that overlap on the GPU race
+    on the shared scratch.  Raises NfError for sizes beyond the scratch (u + v + w faces > 268 435 456)."""
+    import torch
+    lib = load_library()
+    nz, ny, nx = u.shape[0], u.shape[1], u.shape[2] - 1
+    if tuple(v.shape) != (nz, ny + 1, nx) or tuple(w.shape) != (nz + 1, ny, nx):
+        raise ValueError("u, v, w must be (nz, ny, nx+1), (nz, ny+1, nx), (nz+1, ny, nx)")
+    for t in (u, v, w, out):
+        if not t.is_cuda or t.device != u.device:
+            raise ValueError("nf_max_speed_static takes device tensors on one device")
+    if out.numel() != 1:
+        raise ValueError("out must hold one float32")
+    with torch.cuda.device(u.device):
+        s = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.nf_max_speed_static(_ptr(u), _ptr(v), _ptr(w), int(nx), int(ny), int(nz),
+                                     ctypes.c_void_p(s.cuda_stream), _ptr(out))
+    if rc != 0:
+        raise NfError("nf_max_speed_static failed (%d): %s" % (rc, lib.nf_static_last_error().decode()))
+    return out

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libnf_b200.so")
-SOURCES = ["nf_api.cu", "nf_weights.cu", "nf_solver.cu", "nf_mg.cu", "nf_project.cu", "nf_advect.cu", "nf_geom.cu", "nf_components.cu"]
+SOURCES = ["nf_api.cu", "nf_weights.cu", "nf_solver.cu", "nf_mg.cu", "nf_project.cu", "nf_advect.cu", "nf_geom.cu", "nf_components.cu", "nf_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2,-Wall", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 
