@@ -38,7 +38,17 @@ TOL, MAXIT = 1e-6, 400
 # algorithmic bytes per FINE cell per launch of each kernel class of the PCG iteration
 BYTES = {"apply_A": 25.0, "cg_update": 17.0, "cg_pupdate": 12.0, "down1_fine": 9.0, "down2_fine": 5.5,
          "up1_fine": 13.5, "up2_fine": 13.0, "vec_coarse": 41.0 / 7.0, "rbgs_fine": 24.0, "restrict_fine": 20.5,
-         "prolong_fine": 8.5}
+         "prolong_fine": 8.5, "sweep_fine": 13.0}
+
+
+def coarse_bytes_per_fine_cell(nu_l1, nu_deep):
+    """Algorithmic bytes of the cooperative coarse kernel per FINE cell.  One level with nu sweeps
+    before and after the coarse correction moves, per cell of that level: pre-smoother from zero 9 (r, code in; z
+    out), every further half sweep 13 (z, r, code in; z out), residual + restriction 5.5 (+ 4 for r once nu > 1),
+    prolongation + black half sweep 13.5, red half sweep 13 -> 41 for nu = 1, 41 + 52 (nu - 1) + 4 otherwise.
+    Level 1 holds 1/8 of the fine cells, the deeper ones 1/64 + 1/512 + ... = 1/56."""
+    per = lambda nu: 41.0 + (52.0 * (nu - 1) + 4.0 if nu > 1 else 0.0)
+    return per(nu_l1) / 8.0 + per(nu_deep) / 56.0
 
 
 def _peaks():
@@ -254,12 +264,15 @@ def run_ours(args):
     KNAME = {"apply_A": "k_papply4", "cg_update": "k_update_down1", "down1_fine": "k_down1", "down2_fine": "k_down2",
              "up1_fine": "k_up1", "up2_fine": "k_up2", "vec_coarse": "k_vcoarse"}
     kern = {}
+    sweeps = g.sweeps()
+    bytes_of = dict(BYTES)
+    bytes_of["vec_coarse"] = coarse_bytes_per_fine_cell(sweeps[2], sweeps[3])
     for name, (ms, cnt) in prof.items():
         if cnt == 0:
             continue
         kk = {"ms_total": round(ms, 4), "launches": cnt, "us_per_launch": round(1e3 * ms / cnt, 2)}
-        if name in BYTES:
-            kk["gbs"] = round(BYTES[name] * ncell / (ms / cnt * 1e-3) / 1e9, 1)
+        if name in bytes_of:
+            kk["gbs"] = round(bytes_of[name] * ncell / (ms / cnt * 1e-3) / 1e9, 1)
             kk["frac_of_peak"] = round(kk["gbs"] / peak, 3)
         kern[name] = kk
     tot_ms = sum(v["ms_total"] for v in kern.values())
@@ -275,7 +288,7 @@ def run_ours(args):
         traffic = None
     roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom].get("gbs"), "peak": peak, "unit": "GB/s",
             "frac": round(kern[dom]["gbs"] / peak, 4) if "gbs" in kern[dom] else None, "traffic": traffic,
-            "peak_source": peak_src, "algorithmic_bytes_per_cell": round(BYTES.get(dom, 0.0), 2),
+            "peak_source": peak_src, "algorithmic_bytes_per_cell": round(bytes_of.get(dom, 0.0), 2),
             "cells_per_launch": ncell, "share_of_step": round(kern[dom]["ms_total"] / tot_ms, 3)}
     if "vec_coarse" in kern:
         # the cooperative coarse kernel works on L2-resident levels (ncu: ~25 MB of DRAM traffic per launch for 98 MB of
@@ -292,7 +305,7 @@ def run_ours(args):
     it_names = ["apply_A", "cg_update", "down2_fine", "vec_coarse", "up1_fine", "up2_fine"]
     if all(k_ in kern for k_ in it_names):
         it_us = sum(kern[k_]["us_per_launch"] for k_ in it_names)
-        it_b = sum(BYTES[k_] for k_ in it_names)
+        it_b = sum(bytes_of[k_] for k_ in it_names)
         roof["iteration"] = {"launches": len(it_names), "bytes_per_cell": round(it_b, 1), "us": round(it_us, 1),
                              "gbs": round(it_b * ncell / (it_us * 1e-6) / 1e9, 1),
                              "frac": round(it_b * ncell / (it_us * 1e-6) / 1e9 / peak, 3)}
@@ -364,6 +377,7 @@ def run_ours(args):
                                        "project, project_adjoint, weights_adjoint, advect_adjoint" % n,
                            "grid": [n, n, n], "tol": TOL, "l2_policy": "inputs exceed L2 (>1 GB working set per step)",
                            "parallelism": "replicas x%d" % world, "levels": ninfo["levels"],
+                           "sweeps_fine_l1_deeper": [sweeps[0], sweeps[2], sweeps[3]],
                            "x0": "previous pressure (forward solve)" if args.warm_start else "zero",
                            "active_cells": ninfo["active_cells"]},
                 "projection_ms": round(proj_ms, 3), "iters_fwd_adj": its, "mcell_iters_per_s": round(mcell_it, 1),
@@ -520,16 +534,19 @@ def run_sweep(args):
         prof = g.profile()
         g.profile_enable(False)
         per_kernel = {}
+        sw = g.sweeps()
+        bytes_of = dict(BYTES)
+        bytes_of["vec_coarse"] = coarse_bytes_per_fine_cell(sw[2], sw[3])
         for name, (kms, cnt) in prof.items():
-            if cnt and name in BYTES:
+            if cnt and name in bytes_of:
                 us = 1e3 * kms / cnt
                 per_kernel[name] = {"us_per_launch": round(us, 2), "launches": cnt,
-                                    "gbs": round(BYTES[name] * n ** 3 / (us * 1e-6) / 1e9, 1)}
+                                    "gbs": round(bytes_of[name] * n ** 3 / (us * 1e-6) / 1e9, 1)}
         res = rhs.astype(np.float64) - _apply_A_fp64(p.cpu().numpy().astype(np.float64), au, av, aw, float(n))
         res[~active] = 0.0
         rows.append({"n": n, "rc": int(rc), "iters": info["iters"], "ms": round(ms, 3), "active_cells": nact,
                      "fluid_components": int(ncomp), "components_found_by_library": [ncomp_lib, nsing_lib],
-                     "levels": g.info()["levels"],
+                     "levels": g.info()["levels"], "sweeps_fine_l1_deeper": [sw[0], sw[2], sw[3]],
                      "mcell_iters_per_s": round(nact * info["iters"] / (ms * 1e-3) / 1e6, 1),
                      "us_per_iter": round(1e3 * ms / max(info["iters"], 1), 1),
                      "recursive_relres": float(info["relres"]),

@@ -98,6 +98,10 @@ int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags);
  * iteration at 256^3 and saves 40 % of the iterations on the channel-gate workload.  May be called
  * at any time between solves; handles solved together by the *_batch calls must agree. */
 int nf_set_coarse_sweeps(nf_grid *g, int nu_level1, int nu_deeper);
+/* The smoothing sweeps in force: finest level before / after the coarse correction, level 1, every deeper level
+ * (the defaults depend on the grid size: nf_grid_create picks 1, 1 and 1, 2 below 6 M cells, 2, 3 from there on).
+ * Any pointer may be NULL. */
+int nf_get_sweeps(nf_grid *g, int *nu_fine_pre, int *nu_fine_post, int *nu_level1, int *nu_deeper);
 
 /* The low-order part of the pressure.  A solve to 1e-6 ends with a correction e
  * of a fp32 pressure x = O(1): rounding x + e back to fp32 alone leaves a TRUE residual of ~7e-6 at 256^3 (the storage

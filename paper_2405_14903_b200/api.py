@@ -26,6 +26,7 @@ _SIGNATURES = {
     "nf_set_domain_bc": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_float]),
     "nf_set_solver_options": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
     "nf_set_coarse_sweeps": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
+    "nf_get_sweeps": (ctypes.c_int, [ctypes.c_void_p] + [ctypes.POINTER(ctypes.c_int)] * 4),
     "nf_set_pressure_lo": (ctypes.c_int, [ctypes.c_void_p, _c_float_p]),
     "nf_set_solid": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
     "nf_set_weights": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3),
@@ -234,6 +235,12 @@ class Grid:
     def set_coarse_sweeps(self, nu_level1=2, nu_deeper=None):
         nd = nu_level1 if nu_deeper is None else nu_deeper
         self._check(self.lib.nf_set_coarse_sweeps(self.h, int(nu_level1), int(nd)), "nf_set_coarse_sweeps")
+
+    def sweeps(self):
+        """(nu_fine_pre, nu_fine_post, nu_level1, nu_deeper) in force."""
+        v = [ctypes.c_int() for _ in range(4)]
+        self._check(self.lib.nf_get_sweeps(self.h, *[ctypes.byref(x) for x in v]), "nf_get_sweeps")
+        return tuple(x.value for x in v)
 
     def set_pressure_lo(self, lo):
         """Install (or remove with None) the cell array that receives the low-order part of the next pressures."""

@@ -582,6 +582,15 @@ extern "C" int nf_grid_info(nf_grid *g, int *levels, long long *active_cells, in
   return NF_OK;
 }
 
+extern "C" int nf_get_sweeps(nf_grid *g, int *nu_fine_pre, int *nu_fine_post, int *nu_level1, int *nu_deeper) {
+  NF_CHECK_HANDLE(g);
+  if (nu_fine_pre) *nu_fine_pre = g->nu_pre;
+  if (nu_fine_post) *nu_fine_post = g->nu_post;
+  if (nu_level1) *nu_level1 = g->nu_l1;
+  if (nu_deeper) *nu_deeper = g->nu_deep;
+  return NF_OK;
+}
+
 extern "C" int nf_grid_components(nf_grid *g, int *components, int *singular_components) {
   NF_CHECK_HANDLE(g);
   if (!g->weights_set) return NF_ERR_STATE;
