@@ -675,6 +675,22 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
   if (!fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_cg_pupdate<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(g->p, L.z, n, v4, g->st, 0, 1));
   int it = 0, last_seen = -1, done = 0;
   if (maxit < 1) maxit = 1;
+  // Under nf_profile_enable the host reads an iteration's status right after its update kernel, before it enqueues the
+  // V-cycle of the next one: no launch then returns at once on `done`, and the per-class averages are those of launches
+  // that did their work.  (With the look-ahead of the normal path two iterations' worth of launches per phase exit
+  // early; they diluted the averages of round 1 by 8 launches in 60.)
+  bool stop_now = false;
+  auto prof_check = [&](int i) -> int {
+    if (!g->prof_on) return NF_OK;
+    NF_CUDA(g, cudaGetLastError());
+    const int rcw = wait_seq(g, i, i + 1);
+    if (rcw != NF_OK) return rcw;
+    NfHostStatus *h = &g->hst[i & (NF_RING - 1)];
+    last_seen = i;
+    stop_now = h->done != 0;
+    h->seq = 0;
+    return NF_OK;
+  };
   for (it = 0; it < maxit && !done; ++it) {
     const int slot = it & 1;
     NfHostStatus *hs = &g->hst_dev[it & (NF_RING - 1)];
@@ -690,12 +706,16 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
         // r' = r - a q, ||r'||^2, the check and the pre-smoother of level 0 in one pass; the V-cycle skips its down1
         rc = nf_update_down1(g, slot, hs, it + 1);
         if (rc != NF_OK) return rc;
+        if ((rc = prof_check(it)) != NF_OK) return rc;
+        if (stop_now) { ++it; break; }
         if (it + 1 < maxit) {
           rc = nf_vcycle_impl(g, true, 1 - slot, true);
           if (rc != NF_OK) return rc;
         }
       } else {
         NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_cg_update<false>, dim3(NF_VEC_BLOCKS), dim3(256), g->stream, x, L.r, (const float *)pnew, (const float *)g->q, n, v4, g->st, slot, hs, it + 1));
+        if ((rc = prof_check(it)) != NF_OK) return rc;
+        if (stop_now) { ++it; break; }
         if (it + 1 < maxit) {
           rc = nf_vcycle_impl(g, true, 1 - slot);
           if (rc != NF_OK) return rc;
@@ -704,6 +724,8 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
     } else {
       launch_apply(g, g->p, g->q, true, slot);
       NF_LAUNCH(g, NFK_UPDATE, k_cg_update<true><<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, L.r, g->p, g->q, n, v4, g->st, slot, hs, it + 1));
+      if ((rc = prof_check(it)) != NF_OK) return rc;
+      if (stop_now) { ++it; break; }
       if (it + 1 < maxit) {
         rc = nf_vcycle_impl(g, true, 1 - slot);
         if (rc != NF_OK) return rc;
@@ -712,7 +734,7 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
     }
     NF_CUDA(g, cudaGetLastError());
     const int look = it - NF_LOOKAHEAD;
-    if (look >= 0) {
+    if (look >= 0 && !g->prof_on) {
       rc = wait_seq(g, look, look + 1);
       if (rc != NF_OK) return rc;
       NfHostStatus *h = &g->hst[look & (NF_RING - 1)];
@@ -838,7 +860,7 @@ int nf_solve_batch_run(nf_grid **G, int n, float *const *x, int maxit, int *stat
       NF_TRY(nf_vcycle_batch(G, n, B, 1 - slot));
     }
     NF_CUDA(g0, cudaGetLastError());
-    const int look = it - NF_LOOKAHEAD;
+    const int look = it - (g0->prof_on ? 0 : NF_LOOKAHEAD);
     if (look >= 0) {
       all_done = true;
       for (int e = 0; e < n; ++e) {
