@@ -733,7 +733,10 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
       }
     }
     NF_CUDA(g, cudaGetLastError());
-    const int look = it - NF_LOOKAHEAD;
+    // look-ahead: the host enqueues this many iterations beyond the last one whose status it has read.  Launches made
+    // after convergence return at once but are not free (~4 us each, 6 per iteration): large grids, whose iteration
+    // lasts far longer than its six launches take to enqueue, look ahead by one
+    const int look = it - (n >= (size_t)2000000 ? 1 : NF_LOOKAHEAD);
     if (look >= 0 && !g->prof_on) {
       rc = wait_seq(g, look, look + 1);
       if (rc != NF_OK) return rc;
