@@ -55,16 +55,17 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   for (int f = 0; f < 6; ++f) { g->bc_type[f] = NF_BC_CLOSED; g->bc_val[f] = 0.0f; }
   g->stream = 0;
   g->nu_pre = 1; g->nu_post = 1;
-  // Sweeps on the coarse levels (nf_set_coarse_sweeps overrides): chosen from measurements on the channel-gate
-  // workload.  The extra sweeps run as phases of the cooperative coarse kernel, whose cost is
-  // latency and does not shrink with the grid, while the fine level's cost does: large grids afford more of them.
-  //   256^3, forward + adjoint solve, ms: (1,1) 22.8  (1,2) 18.1  (2,2) 17.7  (2,3) 16.8  (3,3) 16.9
-  //   128^3:                              (1,1) 4.94  (1,2) 4.68  (2,2) 4.71  (2,3) 5.13
-  //    64^3:                              (1,1) 2.58  (1,2) 2.63  (2,2) 2.86
+  // Sweeps on the coarse levels (nf_set_coarse_sweeps overrides): chosen from measurements.  The
+  // extra sweeps run as phases of the cooperative coarse kernel, whose cost is latency and does not shrink with the
+  // grid, while the fine level's cost does: only large grids afford them.  Forward + adjoint solve, ms, sweeps on
+  // (level 1, the levels below):
+  //   channel-gate 256^3: (1,1) 22.8  (1,2) 18.1  (2,2) 17.7  (2,3) 16.5  (3,3) 16.9;  sphere field 384^3 / 512^3: -10 % / -8 %
+  //   channel-gate 128^3: (1,1) 4.94  (1,2) 4.68;  64^3: 2.58 / 2.63;  but chamber 128^3 x 50 steps 7.09 -> 7.44 ms per
+  //   step, plates 64^3 2.75 -> 3.05, sphere field 64^3 / 128^3 + 10 % / + 13 % with (1,2): small grids keep V(1,1)
   {
     const bool large = (long long)nx * ny * nz >= 6000000LL;
     g->nu_l1 = large ? 2 : 1;
-    g->nu_deep = large ? 3 : 2;
+    g->nu_deep = large ? 3 : 1;
   }
   g->force_generic = false; g->refresh = true; g->warm = false; g->host_async = false;
   g->weights_set = g->have_sdf = g->have_us = false;

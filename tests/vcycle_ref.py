@@ -4,7 +4,8 @@ NOT the oracle (the paper defines the projection's RESULT, not the preconditione
 library's own choice, DESIGN.md section 6 / R13) -- a slow third implementation of that documented choice, used to
 check the CUDA V-cycle kernels (fused 4-launch levels, cooperative coarse kernel with its packed per-cell phases,
 shared-memory tail) against something that carries no fp32 rounding: V(nu, nu) with nu chosen per level (the finest
-level, level 1, every level below: 1, 1, 2 by default -- the library's choice for grids below 6 M cells), red-black Gauss-Seidel (pre: red then black, the first sweep from a zero
+level, level 1, every level below: 1, 1, 1 by default -- the library's choice for grids below 6 M cells; 1, 2, 3
+from there on), red-black Gauss-Seidel (pre: red then black, the first sweep from a zero
 guess; post: black then red), piecewise-constant prolongation P, restriction P^T / 8,
 rediscretised coarse operators with c_l = c / 4^l on weights that are the mean of the four coincident fine face
 weights (absent fine faces of an odd edge count as closed), extents halving -- rounding up -- while they stay >= 4
@@ -68,7 +69,7 @@ def _diag(a):
     return au[:, :, :-1] + au[:, :, 1:] + av[:, :-1, :] + av[:, 1:, :] + aw[:-1] + aw[1:]
 
 
-def vcycle(r, alpha, c, singular, nu_fine=1, nu_l1=1, nu_deep=2):
+def vcycle(r, alpha, c, singular, nu_fine=1, nu_l1=1, nu_deep=1):
     """nu_fine / nu_l1 / nu_deep: red-black sweeps before and after the coarse correction on the finest level / on
     level 1 / on every level below that (the library's defaults: nf_set_solver_options, nf_set_coarse_sweeps)."""
     levels = [[x.astype(np.float64) for x in a] for a in hierarchy(alpha)]
