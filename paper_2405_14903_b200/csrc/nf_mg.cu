@@ -1119,7 +1119,9 @@ struct NfCoarseK {
 };
 
 // The body: `cta` of `nctas` CTAs work on one environment's coarse levels; SYNC() is the barrier among exactly those.
-template <class SYNC>
+// MULTI: some level runs more than one sweep (P.nu).  The V(1,1) instance carries none of that code: unused, it still
+// cost 2 - 8 us per launch (register allocation and a colder instruction cache: 91 -> 99 us at 256^3, 53 -> 57 at 128^3).
+template <bool MULTI, class SYNC>
 __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int nctas, float *sm,
                                                 unsigned long long *mbar, SYNC sync) {
   if (P.has_tail && cta == 0 && threadIdx.x == 0) nf_tail_prefetch(P.T, P.pack, P.minv, sm, mbar);
@@ -1179,27 +1181,24 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
       }
     }
     sync();
-    for (int s = 1; s < P.nu[l]; ++s) {  // further pre-smoothing sweeps: red, black
-      half(l, 0);
-      sync();
-      half(l, 1);
-      sync();
+    if (MULTI) {  // further pre-smoothing sweeps: red, black, red, ... (one call site: one copy of the code)
+      for (int q = 0; q < 2 * (P.nu[l] - 1); ++q) {
+        half(l, q & 1);
+        sync();
+      }
     }
-    const bool gen = P.nu[l] > 1;
+    // (the general residual is right after one sweep as well -- r - diag z is then a rounding zero on the red cells --
+    // so the MULTI instance carries that form only)
+    const bool gen = MULTI;
     if (dense) {
       for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t, gen);
     } else {
       for (int t = gt; t < nx4 * cny * cnz; t += gn) {
         const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
-        if (gen) {
-          if (L.fz == 2)
-            nf_down2_body<2, true>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
-          else
-            nf_down2_body<1, true>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
-        } else if (L.fz == 2)
-          nf_down2_body<2>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
+        if (L.fz == 2)
+          nf_down2_body<2, MULTI>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
         else
-          nf_down2_body<1>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K);
+          nf_down2_body<1, MULTI>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
       }
     }
     sync();
@@ -1236,24 +1235,23 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
       }
     }
     sync();
-    half(l, 0);
-    for (int s = 1; s < P.nu[l]; ++s) {  // further post-smoothing sweeps: black, red
-      sync();
-      half(l, 1);
-      sync();
-      half(l, 0);
+    // the red half sweep, then (black, red) once more per further sweep -- one call site
+    for (int q = 0; q < (MULTI ? 2 * P.nu[l] - 1 : 1); ++q) {
+      if (q) sync();
+      half(l, q & 1);
     }
     if (l > P.first) sync();
   }
 }
 
+template <bool MULTI>
 __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_constant__ NfCoarseK P,
                                                                  const NfSolveState *st) {
   if (st && st->done) return;  // (uniform over the grid: written by an earlier kernel)
   extern __shared__ __align__(16) float sm[];
   __shared__ unsigned long long mbar;
   cg::grid_group grid = cg::this_grid();
-  nf_vcoarse_body(P, (int)blockIdx.x, (int)gridDim.x, sm, &mbar, [&]() { grid.sync(); });
+  nf_vcoarse_body<MULTI>(P, (int)blockIdx.x, (int)gridDim.x, sm, &mbar, [&]() { grid.sync(); });
 }
 
 // Batched: ONE cooperative launch runs the coarse levels of up to NF_BATCH_MAX equally sized
@@ -1268,6 +1266,7 @@ struct NfCoarseBatchK {
   const NfSolveState *st[NF_BATCH_MAX];
   const NfCoarseK *P[NF_BATCH_MAX];  // (device copies: one NfCoarseK is ~1.7 KB, sixteen would not fit the parameters)
 };
+template <bool MULTI>
 __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_constant__ NfCoarseBatchK B) {
   const int e = (int)blockIdx.x / B.nctas, cta = (int)blockIdx.x - e * B.nctas;
   unsigned *bar = B.bar[e];
@@ -1286,7 +1285,7 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_c
   __syncthreads();
   unsigned target = B.base[e];
   const unsigned nctas = (unsigned)B.nctas;
-  nf_vcoarse_body(sP, cta, B.nctas, sm, &mbar, [&]() {
+  nf_vcoarse_body<MULTI>(sP, cta, B.nctas, sm, &mbar, [&]() {
     __syncthreads();
     if (threadIdx.x == 0) {
       __threadfence();
@@ -1304,6 +1303,8 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_c
 // host side
 // ------------------------------------------------------------------------------------------------------------
 static inline int nf_nu_coarse(const nf_grid *g, int l) { return l <= 1 ? g->nu_l1 : g->nu_deep; }
+// some grid-phase level of the coarse kernel runs more than one sweep
+static inline bool nf_coarse_multi(const nf_grid *g) { return g->nu_l1 > 1 || (g->nu_deep > 1 && g->tail > 2); }
 #define NF_TAIL_SMEM_MAX 231424  // dynamic shared memory of k_tail / k_vcoarse (226 KB of the 227 KB a CTA may use)
 
 // Shared-memory layout of a tail that starts at level `first` (NfTailK); T.total_floats is what it needs.
@@ -1366,8 +1367,10 @@ void nf_mg_plan(nf_grid *g) {
 int nf_mg_init(nf_grid *g) {
   const int smem = NF_TAIL_SMEM_MAX;
   NF_CUDA(g, cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
   NF_CUDA(g, cudaFuncSetAttribute(k_coarse_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (NF_DIRECT_MAX * NF_DIRECT_MAX + 2 * NF_DIRECT_MAX) * (int)sizeof(double)));
   // the cooperative coarse kernel: one CTA per SM; needs a tail, at least one vec level below the finest one, and
@@ -1381,7 +1384,7 @@ int nf_mg_init(nf_grid *g) {
     NF_CUDA(g, cudaGetDevice(&dev));
     NF_CUDA(g, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     NF_CUDA(g, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
-    NF_CUDA(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_vcoarse, NF_TAIL_THREADS, tail_smem_bytes(g)));
+    NF_CUDA(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_vcoarse<true>, NF_TAIL_THREADS, tail_smem_bytes(g)));
     if (all_vec && coop && per_sm >= 1) {
       // One CTA per 4096 cells of the first coarse level, at least 8, at most one per SM.  A cooperative grid is
       // resident as a whole: sized for the level instead of for the machine, the coarse kernels of several small
@@ -1519,7 +1522,7 @@ int nf_vcycle_batch(nf_grid **G, int n, const NfBatchK &Bin, int slot) {
     }
     for (int e = 0; e < n; ++e) G[e]->cbar_count += (unsigned)(CB.nbar * CB.nctas);
     void *args[] = {(void *)&CB};
-    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel((void *)k_vcoarse_b, dim3(n * g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
+    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel(nf_coarse_multi(g) ? (void *)k_vcoarse_b<true> : (void *)k_vcoarse_b<false>, dim3(n * g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
   }
   B.nzc = (int)d.grid.z;
   dim3 gb = d.grid;
@@ -1596,7 +1599,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
     fill_coarse(g, &P);
     const NfSolveState *stc = st;
     void *args[] = {(void *)&P, (void *)&stc};
-    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel((void *)k_vcoarse, dim3(g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
+    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel(nf_coarse_multi(g) ? (void *)k_vcoarse<true> : (void *)k_vcoarse<false>, dim3(g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
   } else if (has_tail) {
     NfTailK T;
     tail_desc(g, g->tail, &T);
