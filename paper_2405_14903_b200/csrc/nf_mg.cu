@@ -1121,7 +1121,8 @@ struct NfCoarseK {
 // The body: `cta` of `nctas` CTAs work on one environment's coarse levels; SYNC() is the barrier among exactly those.
 // MULTI: some level runs more than one sweep (P.nu).  The V(1,1) instance carries none of that code: unused, it still
 // cost 2 - 8 us per launch (register allocation and a colder instruction cache: 91 -> 99 us at 256^3, 53 -> 57 at 128^3).
-template <bool MULTI, class SYNC>
+// FLAT: 2-D mode (nz == 1: 2 x 2 x 1 children); the 3-D instance carries none of those bodies either.
+template <bool MULTI, bool FLAT, class SYNC>
 __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int nctas, float *sm,
                                                 unsigned long long *mbar, SYNC sync) {
   if (P.has_tail && cta == 0 && threadIdx.x == 0) nf_tail_prefetch(P.T, P.pack, P.minv, sm, mbar);
@@ -1195,10 +1196,7 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
     } else {
       for (int t = gt; t < nx4 * cny * cnz; t += gn) {
         const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
-        if (L.fz == 2)
-          nf_down2_body<2, MULTI>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
-        else
-          nf_down2_body<1, MULTI>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
+        nf_down2_body<FLAT ? 1 : 2, MULTI>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
       }
     }
     sync();
@@ -1221,17 +1219,10 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
         const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
         // (explicit branches: selecting the body through a conditional expression made it an indirect call --
         // un-inlined, with a stack frame; this phase took 15 us at the 128^3 level against 5 us for k_up2's)
-        if (L.fz == 2) {
-          if ((j + k) & 1)
-            nf_up1_body<1, 2>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
-          else
-            nf_up1_body<0, 2>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
-        } else {
-          if ((j + k) & 1)
-            nf_up1_body<1, 1>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
-          else
-            nf_up1_body<0, 1>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
-        }
+        if ((j + k) & 1)
+          nf_up1_body<1, FLAT ? 1 : 2>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
+        else
+          nf_up1_body<0, FLAT ? 1 : 2>(L, P.z[l], P.r[l], P.z[l + 1], cnx, cny, i0, j, k);
       }
     }
     sync();
@@ -1244,14 +1235,14 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
   }
 }
 
-template <bool MULTI>
+template <bool MULTI, bool FLAT>
 __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_constant__ NfCoarseK P,
                                                                  const NfSolveState *st) {
   if (st && st->done) return;  // (uniform over the grid: written by an earlier kernel)
   extern __shared__ __align__(16) float sm[];
   __shared__ unsigned long long mbar;
   cg::grid_group grid = cg::this_grid();
-  nf_vcoarse_body<MULTI>(P, (int)blockIdx.x, (int)gridDim.x, sm, &mbar, [&]() { grid.sync(); });
+  nf_vcoarse_body<MULTI, FLAT>(P, (int)blockIdx.x, (int)gridDim.x, sm, &mbar, [&]() { grid.sync(); });
 }
 
 // Batched: ONE cooperative launch runs the coarse levels of up to NF_BATCH_MAX equally sized
@@ -1285,7 +1276,7 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_c
   __syncthreads();
   unsigned target = B.base[e];
   const unsigned nctas = (unsigned)B.nctas;
-  nf_vcoarse_body<MULTI>(sP, cta, B.nctas, sm, &mbar, [&]() {
+  nf_vcoarse_body<MULTI, false>(sP, cta, B.nctas, sm, &mbar, [&]() {
     __syncthreads();
     if (threadIdx.x == 0) {
       __threadfence();
@@ -1367,8 +1358,10 @@ void nf_mg_plan(nf_grid *g) {
 int nf_mg_init(nf_grid *g) {
   const int smem = NF_TAIL_SMEM_MAX;
   NF_CUDA(g, cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
   NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
   NF_CUDA(g, cudaFuncSetAttribute(k_coarse_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1384,7 +1377,7 @@ int nf_mg_init(nf_grid *g) {
     NF_CUDA(g, cudaGetDevice(&dev));
     NF_CUDA(g, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     NF_CUDA(g, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
-    NF_CUDA(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_vcoarse<true>, NF_TAIL_THREADS, tail_smem_bytes(g)));
+    NF_CUDA(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_vcoarse<true, false>, NF_TAIL_THREADS, tail_smem_bytes(g)));
     if (all_vec && coop && per_sm >= 1) {
       // One CTA per 4096 cells of the first coarse level, at least 8, at most one per SM.  A cooperative grid is
       // resident as a whole: sized for the level instead of for the machine, the coarse kernels of several small
@@ -1599,7 +1592,10 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
     fill_coarse(g, &P);
     const NfSolveState *stc = st;
     void *args[] = {(void *)&P, (void *)&stc};
-    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel(nf_coarse_multi(g) ? (void *)k_vcoarse<true> : (void *)k_vcoarse<false>, dim3(g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
+    const bool multi = nf_coarse_multi(g), flat = g->nz == 1;
+    void *kfun = flat ? (multi ? (void *)k_vcoarse<true, true> : (void *)k_vcoarse<false, true>)
+                      : (multi ? (void *)k_vcoarse<true, false> : (void *)k_vcoarse<false, false>);
+    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel(kfun, dim3(g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
   } else if (has_tail) {
     NfTailK T;
     tail_desc(g, g->tail, &T);
