@@ -50,3 +50,14 @@ def _small_case():
     gin = [rng.standard_normal(a.shape).astype(np.float32) for a in U]
     bc = orc.BC(P["bc_types"], P["bc_values"])
     return P, U, orc.face_weights(phi, bc), us, gin, bc
+
+
+def test_coarse_kernel_bytes_follow_the_sweep_counts():
+    """bench.coarse_bytes_per_fine_cell: the V(1,1) figure is the 41/7 B per fine cell of DESIGN.md 8.1 (41 B per cell of
+    a level, levels of 1/8 + 1/64 + ... of the fine cells); every further sweep adds four half sweeps of 13 B per cell
+    and, once, the 4 B of the right-hand side that the general residual reads."""
+    import bench
+    assert abs(bench.coarse_bytes_per_fine_cell(1, 1) - 41.0 / 7.0) < 1e-12
+    assert abs(bench.coarse_bytes_per_fine_cell(2, 1) - (97.0 / 8.0 + 41.0 / 56.0)) < 1e-12
+    assert abs(bench.coarse_bytes_per_fine_cell(2, 3) - (97.0 / 8.0 + 149.0 / 56.0)) < 1e-12
+    assert abs(bench.coarse_bytes_per_fine_cell(1, 2) - (41.0 / 8.0 + 97.0 / 56.0)) < 1e-12

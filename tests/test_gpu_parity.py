@@ -810,3 +810,37 @@ def test_component_labels_through_the_gauge_at_larger_sizes(torch, api, n, nblob
     res = bc_ - orc.apply_A(ph, alpha, 1.0 * n)
     assert np.linalg.norm(res) <= 5e-6 * np.linalg.norm(bc_)
     g.close()
+
+
+def test_sweep_settings_api_and_solution_independence(torch, api):
+    """nf_set_coarse_sweeps / nf_get_sweeps: defaults by grid size (V(1,1) below 6 M cells), range checks, and -- the
+    preconditioner changes the iteration count, never the answer -- the same pressure within the solver tolerance at
+    every setting, through the fused and the generic kernels."""
+    nx, ny, nz = 64, 48, 40
+    g = make_grid(api, nx, ny, nz, 1.0 / nx, dt_over_rho=0.5, bc_types=(1, 0, 0, 0, 0, 0))
+    assert g.sweeps() == (1, 1, 1, 1)
+    lib = api.load_library()
+    for bad in ((0, 1), (1, 0), (9, 1), (1, 9)):
+        assert lib.nf_set_coarse_sweeps(g.h, bad[0], bad[1]) == -1
+    assert g.sweeps() == (1, 1, 1, 1)
+    g.set_solid(dev(torch, blob_sdf(nx, ny, nz, 3)))
+    act = orc.active_cells([a.cpu().numpy().astype(np.float64) for a in g.get_weights()])
+    rhs = (np.random.default_rng(8).standard_normal((nz, ny, nx)) * act).astype(np.float32)
+    ref, its = None, {}
+    for flags in (0, 2):
+        for nu in ((1, 1), (1, 2), (2, 3), (3, 1)):
+            g.set_solver_options(1, 1, flags)
+            g.set_coarse_sweeps(*nu)
+            assert g.sweeps() == (1, 1) + nu
+            p = torch.zeros(g.shape_p, device="cuda")
+            assert g.solve(dev(torch, rhs), p, tol=1e-7, maxit=200) == 0
+            its[(flags, nu)] = g.last_solve_info()["iters"]
+            if ref is None:
+                ref = host(p)
+            assert rel(host(p), ref) < 2e-5, (flags, nu)
+    assert its[(0, (2, 3))] <= its[(0, (1, 1))]
+    assert its[(0, (1, 1))] == its[(2, (1, 1))] or abs(its[(0, (1, 1))] - its[(2, (1, 1))]) <= 1
+    g.close()
+    big = api.Grid(192, 192, 192, 1.0 / 192)   # 7.1 M cells: the large-grid default
+    assert big.sweeps() == (1, 1, 2, 3)
+    big.close()
