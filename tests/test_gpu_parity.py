@@ -844,3 +844,40 @@ def test_sweep_settings_api_and_solution_independence(torch, api):
     big = api.Grid(192, 192, 192, 1.0 / 192)   # 7.1 M cells: the large-grid default
     assert big.sweeps() == (1, 1, 2, 3)
     big.close()
+
+
+@pytest.mark.parametrize("n,nu", [(32, (2, 2)), (48, (2, 3)), (64, (1, 2))])
+def test_batched_solve_with_several_coarse_sweeps(torch, api, n, nu):
+    """The batched coarse kernel (k_vcoarse_b, per-environment epoch barrier) with more than one sweep per level: the
+    host's count of barriers per launch has to follow the sweep counts or the environments deadlock or race -- same
+    answers as the oracle, same iteration counts as the one-handle path; environments whose sweep settings differ are
+    not batched together but still solved."""
+    nenv = 4
+    grids, rhs, refs = [], [], []
+    rng = np.random.default_rng(11)
+    for e in range(nenv):
+        g = make_grid(api, n, n, n, 1.0 / n, 0.5, bc_types=(1, 0, 0, 0, 0, 0))
+        g.set_solid(dev(torch, blob_sdf(n, n, n, 400 + e, nblobs=5)))
+        g.set_coarse_sweeps(*nu)
+        alpha = [host(a) for a in g.get_weights()]
+        act = orc.active_cells(alpha)
+        b = np.where(act, rng.standard_normal((n, n, n)), 0.0).astype(np.float32)
+        grids.append(g); rhs.append(b)
+        refs.append(orc.solve(b.astype(np.float64), alpha, 0.5 * n, orc.BC((1, 0, 0, 0, 0, 0), (0.0,) * 6), tol=1e-12))
+    pd = [torch.zeros(g.shape_p, dtype=torch.float32, device="cuda") for g in grids]
+    assert api.solve_batch(grids, [dev(torch, b) for b in rhs], pd, tol=1e-6, maxit=200) == [0] * nenv
+    its_b = [g.last_solve_info()["iters"] for g in grids]
+    for e in range(nenv):
+        assert rel(host(pd[e]), refs[e]) < TOL_FIELD
+        p1 = torch.zeros_like(pd[e])
+        grids[e].set_solver_options(1, 1, 4)   # (the batched path has no refresh phase)
+        assert grids[e].solve(dev(torch, rhs[e]), p1, tol=1e-6, maxit=200) == 0
+        grids[e].set_solver_options(1, 1, 0)
+        assert abs(grids[e].last_solve_info()["iters"] - its_b[e]) <= 1
+    grids[1].set_coarse_sweeps(1, 1)           # no longer batchable with the others
+    pd2 = [torch.zeros_like(p) for p in pd]
+    assert api.solve_batch(grids, [dev(torch, b) for b in rhs], pd2, tol=1e-6, maxit=200) == [0] * nenv
+    for e in range(nenv):
+        assert rel(host(pd2[e]), refs[e]) < TOL_FIELD
+    for g in grids:
+        g.close()
