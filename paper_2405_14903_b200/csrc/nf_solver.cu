@@ -469,8 +469,12 @@ __global__ void __launch_bounds__(256) k_true_residual(float *__restrict__ r, co
   nf_block_atomic_add(part, &st->rr[0]);
 }
 // The same on float4 rows with the weights from the 1-byte codes (4 cells per thread, fp64 arithmetic).
+// rr_out / sr_out (either may be null): where ||r||^2 and -- on a singular system -- the sum of r are accumulated.
+// check_done: return at once when the solve has converged (the in-flight replacement of nf_solve_run).
 __global__ void __launch_bounds__(256, 4) k_true_residual4(NfLvK L, float *__restrict__ r, const float *__restrict__ b0,
-                                                        const float *__restrict__ x, NfSolveState *st) {
+                                                        const float *__restrict__ x, NfSolveState *st, double *rr_out,
+                                                        double *sr_out, int check_done) {
+  if (check_done && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z * blockDim.z + threadIdx.z;
@@ -505,8 +509,12 @@ __global__ void __launch_bounds__(256, 4) k_true_residual4(NfLvK L, float *__res
     }
     *reinterpret_cast<float4 *>(r + id) = make_float4(out[0], out[1], out[2], out[3]);
   }
-  nf_block_atomic_add(part, &st->rr[0]);
-  if (st->inv_nact != 0.0) nf_block_atomic_add(sum, &st->sr[1]);
+  if (rr_out) nf_block_atomic_add(part, rr_out);
+  if (sr_out && st->inv_nact != 0.0) nf_block_atomic_add(sum, sr_out);
+}
+// (one thread) the sum slot of the residual buffer that k_true_residual4 is about to rewrite
+__global__ void k_zero_sr(NfSolveState *st, int slot) {
+  if (threadIdx.x == 0 && blockIdx.x == 0 && !st->done) st->sr[slot] = 0.0;
 }
 // warm start: the initial guess on the active cells only (0 elsewhere), and 0 everywhere when b = 0 (done is then
 // already set by k_start_state: the answer is x = 0).  NaN, inf and absurdly large entries (an uninitialised array
@@ -665,9 +673,20 @@ struct NfPhaseOut {
   int converged, iters;
   float relres;
 };
-static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, NfPhaseOut *out) {
+// xe != nullptr (fused path only): IN-FLIGHT RESIDUAL REPLACEMENT.  Once the host has seen the residual below
+// switch_tol, the next iteration recomputes r = b0 - A x in fp64 right after its A-apply (x then holds every update but
+// this iteration's own) and every later update goes to xe (zeroed by the caller) instead of x: the recursion r -= a q
+// drifts from b - A x only through the rounding of the updates of an O(1) x, and the updates of a correction 1e-3 as
+// large round 1e-3 as coarsely.  The search direction is kept, so -- unlike a restart on the true residual -- no
+// V-cycle and no iteration is spent on rebuilding the Krylov space (van der Vorst & Ye's residual replacement; measured
+// at 256^3: 16 iterations and no extra V-cycle against 17 + 1, the same fp64 true residual of 5e-7).  *switched: it happened.
+static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, NfPhaseOut *out, float switch_tol = 0.0f,
+                         float *xe = nullptr, bool *switched = nullptr) {
   NfLevel &L = g->lv[0];
   const size_t n = (size_t)L.ncell;
+  float *xcur = x;            // where the deferred x updates go
+  bool sw = false;
+  float seen_relres = 1e30f;  // the last residual the host has read
   for (int s = 0; s < NF_RING; ++s) g->hst[s].seq = 0;
   const bool fusedr = fusedp && nf_update_down1_ok(g) && vec_ok(g->r_alt, g->r_alt, g->r_alt, g->r_alt, n);
   int rc = nf_vcycle_impl(g, true, 0);
@@ -688,6 +707,7 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
     NfHostStatus *h = &g->hst[i & (NF_RING - 1)];
     last_seen = i;
     stop_now = h->done != 0;
+    seen_relres = h->relres;
     h->seq = 0;
     return NF_OK;
   };
@@ -699,9 +719,17 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
       const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
       if (it == 0)
-        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<true>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, kch, g->st, slot));
+        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<true>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, xcur, kch, g->st, slot));
       else
-        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<false>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, kch, g->st, slot));
+        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<false>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, xcur, kch, g->st, slot));
+      if (xe && !sw && fusedr && it > 0 && seen_relres <= switch_tol) {
+        // x is complete up to the previous iteration: r (the buffer k_update_down1 is about to read) = b0 - A x
+        NfDims dv = nf_dims(L.nx / 4, L.ny, L.nz);
+        NF_LAUNCH(g, NFK_SETUP, k_zero_sr<<<1, 32, 0, g->stream>>>(g->st, 1 - slot));
+        NF_LAUNCH(g, NFK_SETUP, k_true_residual4<<<dv.grid, dv.block, 0, g->stream>>>(nf_lvk(L), L.r, g->b0, x, g->st, nullptr, &g->st->sr[1 - slot], 1));
+        xcur = xe;
+        sw = true;
+      }
       if (fusedr) {
         // r' = r - a q, ||r'||^2, the check and the pre-smoother of level 0 in one pass; the V-cycle skips its down1
         rc = nf_update_down1(g, slot, hs, it + 1);
@@ -743,12 +771,14 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
       NfHostStatus *h = &g->hst[look & (NF_RING - 1)];
       last_seen = look;
       if (h->done) done = 1;
+      seen_relres = h->relres;
       // the ring slot can be reused NF_RING iterations later; clear it now that it has been consumed
       h->seq = 0;
     }
   }
   // the x update of the last executed iteration (every other one rode on the following k_papply4)
-  if (fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->p, g->p2, n, g->st));
+  if (fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(xcur, g->p, g->p2, n, g->st));
+  if (switched) *switched = sw;
   // drain: every enqueued check must have reported before the ring is reused
   const int enq = it;  // checks enqueued: 0 .. enq-1
   for (int s = last_seen + 1; s < enq; ++s) {
@@ -919,6 +949,7 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
   NfPhaseOut ph;
   ph.converged = 0; ph.iters = 0; ph.relres = 0.0f;
   int rc = NF_OK;
+  bool switched = false;
   g->lo_valid = false;
   if (g->plo) NF_CUDA(g, cudaMemsetAsync(g->plo, 0, n * sizeof(float), g->stream));
   // r = b - A x afresh (fp64 evaluation); decide at `tol`; if not done run PCG on it (phase tolerance tolp) for a
@@ -927,7 +958,7 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
     NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)tolp, 0));
     if (!g->force_generic && apply_vec_ok(L, x, L.r) && apply_vec_ok(L, g->b0, g->b0)) {
       NfDims dv = nf_dims(L.nx / 4, L.ny, L.nz);
-      NF_LAUNCH(g, NFK_SETUP, k_true_residual4<<<dv.grid, dv.block, 0, g->stream>>>(nf_lvk(L), L.r, g->b0, x, g->st));
+      NF_LAUNCH(g, NFK_SETUP, k_true_residual4<<<dv.grid, dv.block, 0, g->stream>>>(nf_lvk(L), L.r, g->b0, x, g->st, &g->st->rr[0], &g->st->sr[1], 0));
     } else {
       NF_LAUNCH(g, NFK_SETUP, k_true_residual<<<dc.grid, dc.block, 0, g->stream>>>(L.r, g->b0, x, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->st));
     }
@@ -959,17 +990,42 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
     if (rc != NF_OK) return rc;
   } else {
     NF_CUDA(g, cudaMemsetAsync(x, 0, n * sizeof(float), g->stream));
-    NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)(two_phase ? tol1 : tol), 1));
-    rc = run_pcg_phase(g, x, maxit, fusedp, v4, &ph);
-    if (rc != NF_OK) return rc;
+    // in-flight replacement (run_pcg_phase) where the fused kernels run: the solve then goes straight to `tol`; the
+    // switch point sqrt(tol) = 1e-3 lies well above the drift of the recursion (~3e-5 of |b| at 256^3) and low enough
+    // for the correction's own drift (that much smaller) to stay below tol
+    const bool inflight = two_phase && fusedp && nf_update_down1_ok(g) && apply_vec_ok(L, g->ecorr, g->ecorr) &&
+                          apply_vec_ok(L, x, L.r) && apply_vec_ok(L, g->b0, g->b0) && vec_ok(g->r_alt, g->r_alt, g->r_alt, g->r_alt, n);
+    if (inflight) {
+      NF_CUDA(g, cudaMemsetAsync(g->ecorr, 0, n * sizeof(float), g->stream));
+      NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)tol, 1));
+      // (never below 1e-4: a replacement made when the residual is down at the drift itself perturbs the recursion by
+      // as much as it carries, and PCG stalls -- measured at tol 1e-12: stuck at 1e-6 with the switch at sqrt(tol) = 1e-6)
+      const float sw_tol = fminf(fmaxf(sqrtf(tol), 1e-4f), 1e-2f);
+      rc = run_pcg_phase(g, x, maxit, fusedp, v4, &ph, sw_tol, g->ecorr, &switched);
+      if (rc != NF_OK) return rc;
+      if (switched) {
+        if (g->plo) {
+          NF_LAUNCH(g, NFK_SETUP, k_add_hilo<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->ecorr, g->plo, n));
+          g->lo_valid = true;
+        } else {
+          NF_LAUNCH(g, NFK_SETUP, k_add<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->ecorr, n));
+        }
+      }
+    } else {
+      NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)(two_phase ? tol1 : tol), 1));
+      rc = run_pcg_phase(g, x, maxit, fusedp, v4, &ph);
+      if (rc != NF_OK) return rc;
+    }
   }
-  if (two_phase && ph.converged && ph.iters > 0 && ph.iters < maxit) {
+  // (after an in-flight replacement the recursive residual IS the true one: nothing to refresh; if the solve converged
+  // before the host could place the replacement, the refresh below checks the true residual as before)
+  if (two_phase && !switched && ph.converged && ph.iters > 0 && ph.iters < maxit) {
     // (the correction is ~1e-4 of x: accumulated on its own its rounding is invisible, and x is rounded once)
     rc = correct(tol);
     if (rc != NF_OK) return rc;
   }
   // (phase 1 met its own 30 tol on the very last iteration allowed: that is not the caller's tolerance)
-  if (two_phase && ph.converged && ph.iters >= maxit && !(ph.relres <= tol)) ph.converged = 0;
+  if (two_phase && !switched && ph.converged && ph.iters >= maxit && !(ph.relres <= tol)) ph.converged = 0;
   g->last_iters = ph.iters;
   NF_TRY(apply_gauge(g, x));
   g->last_relres = ph.relres;
