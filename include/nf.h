@@ -94,13 +94,13 @@ int nf_set_solver_options(nf_grid *g, int nu_pre, int nu_post, int flags);
 
 /* Red-black Gauss-Seidel sweeps before AND after the coarse correction on level 1 (the first level below the finest
  * one) and on every level below that (1..8 each; R13: the paper names only "MGPCG").  Default: 2 and 3 on grids of
- * 6 M cells and more, 1 and 1 below.  Those levels hold 1/8 + 1/64 + ... of the cells and run inside one cooperative
+ * 3 M cells and more, 1 and 1 below.  Those levels hold 1/8 + 1/64 + ... of the cells and run inside one cooperative
  * kernel: at 256^3 the extra sweeps double that kernel's time (+ 27 % on a PCG iteration) and save 45 % of the
  * iterations on the channel-gate workload.  May be called at any time between solves; handles
  * solved together by the *_batch calls must agree. */
 int nf_set_coarse_sweeps(nf_grid *g, int nu_level1, int nu_deeper);
 /* The smoothing sweeps in force: finest level before / after the coarse correction, level 1, every deeper level
- * (the defaults depend on the grid size: nf_grid_create picks 1, 1 and 1, 1 below 6 M cells, 2, 3 from there on).
+ * (the defaults depend on the grid size: nf_grid_create picks 1, 1 and 1, 1 below 3 M cells, 2, 3 from there on).
  * Any pointer may be NULL. */
 int nf_get_sweeps(nf_grid *g, int *nu_fine_pre, int *nu_fine_post, int *nu_level1, int *nu_deeper);
 

@@ -62,8 +62,9 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
   //   channel-gate 256^3: (1,1) 22.8  (1,2) 18.1  (2,2) 17.7  (2,3) 16.5  (3,3) 16.9;  sphere field 384^3 / 512^3: -10 % / -8 %
   //   channel-gate 128^3: (1,1) 4.94  (1,2) 4.68;  64^3: 2.58 / 2.63;  but chamber 128^3 x 50 steps 7.09 -> 7.44 ms per
   //   step, plates 64^3 2.75 -> 3.05, sphere field 64^3 / 128^3 + 10 % / + 13 % with (1,2): small grids keep V(1,1)
+  //   channel-gate 128^3 / 160^3 / 192^3 (final kernels): (1,1) 4.26 / 7.08 / 10.15, (2,3) 4.78 / 6.78 / 8.57: the switch sits at 3 M cells
   {
-    const bool large = (long long)nx * ny * nz >= 6000000LL;
+    const bool large = (long long)nx * ny * nz >= 3000000LL;
     g->nu_l1 = large ? 2 : 1;
     g->nu_deep = large ? 3 : 1;
   }

@@ -813,7 +813,7 @@ def test_component_labels_through_the_gauge_at_larger_sizes(torch, api, n, nblob
 
 
 def test_sweep_settings_api_and_solution_independence(torch, api):
-    """nf_set_coarse_sweeps / nf_get_sweeps: defaults by grid size (V(1,1) below 6 M cells), range checks, and -- the
+    """nf_set_coarse_sweeps / nf_get_sweeps: defaults by grid size (V(1,1) below 3 M cells), range checks, and -- the
     preconditioner changes the iteration count, never the answer -- the same pressure within the solver tolerance at
     every setting, through the fused and the generic kernels."""
     nx, ny, nz = 64, 48, 40

@@ -4,7 +4,7 @@ NOT the oracle (the paper defines the projection's RESULT, not the preconditione
 library's own choice, DESIGN.md section 6 / R13) -- a slow third implementation of that documented choice, used to
 check the CUDA V-cycle kernels (fused 4-launch levels, cooperative coarse kernel with its packed per-cell phases,
 shared-memory tail) against something that carries no fp32 rounding: V(nu, nu) with nu chosen per level (the finest
-level, level 1, every level below: 1, 1, 1 by default -- the library's choice for grids below 6 M cells; 1, 2, 3
+level, level 1, every level below: 1, 1, 1 by default -- the library's choice for grids below 3 M cells; 1, 2, 3
 from there on), red-black Gauss-Seidel (pre: red then black, the first sweep from a zero
 guess; post: black then red), piecewise-constant prolongation P, restriction P^T / 8,
 rediscretised coarse operators with c_l = c / 4^l on weights that are the mean of the four coincident fine face
