@@ -24,7 +24,7 @@ static void free_all(nf_grid *g) {
     cudaFree(L.ax); cudaFree(L.ay); cudaFree(L.az); cudaFree(L.code); cudaFree(L.idg); cudaFree(L.pk); cudaFree(L.z); cudaFree(L.r);
   }
   cudaFree(g->us); cudaFree(g->vs); cudaFree(g->ws); cudaFree(g->sdf);
-  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->b0); cudaFree(g->ecorr); cudaFree(g->r_alt); cudaFree(g->tailpack); cudaFree(g->tailinv);
+  cudaFree(g->p); cudaFree(g->q); cudaFree(g->xtmp); cudaFree(g->p2); cudaFree(g->b0); cudaFree(g->ecorr); cudaFree(g->rtrue); cudaFree(g->r_alt); cudaFree(g->tailpack); cudaFree(g->tailinv);
   cudaFree(g->fu); cudaFree(g->fv); cudaFree(g->fw);
   cudaFree(g->st); cudaFree(g->d_counts); cudaFree(g->geom_par); cudaFree(g->geom_grad);
   nf_components_free(g);
@@ -127,7 +127,7 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
        dalloc(&g->ws, nf_nw(g)) == cudaSuccess && dalloc(&g->sdf, nf_nn(g)) == cudaSuccess;
   ok = ok && dalloc(&g->p, nc) == cudaSuccess && dalloc(&g->q, nc) == cudaSuccess &&
        dalloc(&g->xtmp, nc) == cudaSuccess && dalloc(&g->p2, nc) == cudaSuccess &&
-       dalloc(&g->b0, nc) == cudaSuccess && dalloc(&g->ecorr, nc) == cudaSuccess && dalloc(&g->r_alt, nc) == cudaSuccess;
+       dalloc(&g->b0, nc) == cudaSuccess && dalloc(&g->ecorr, nc) == cudaSuccess && dalloc(&g->rtrue, nc) == cudaSuccess && dalloc(&g->r_alt, nc) == cudaSuccess;
   ok = ok && dalloc(&g->fu, nf_nu(g)) == cudaSuccess && dalloc(&g->fv, nf_nv(g)) == cudaSuccess &&
        dalloc(&g->fw, nf_nw(g)) == cudaSuccess;
   ok = ok && dalloc(&g->st, 1) == cudaSuccess && dalloc(&g->d_counts, 2) == cudaSuccess;

@@ -72,6 +72,12 @@ struct alignas(128) NfSolveState {
   // active cells -- in every iteration (k_update_down1), not only at the start: fp32 cannot remove a mean of 5e-9 |b|
   // from b itself (it is below the rounding of the entries), the mean stays while the residual falls by 1e-6, and
   // the V-cycle amplifies the constant mode: PCG then stalled near 1e-6 and DIVERGED.
+  // in-flight residual replacement (nf_solver.cu: run_pcg_phase): 0 not tried, 1 accepted (the iteration read the true
+  // residual, later x updates go to the correction array), -1 rejected (the true residual differed from the recursive
+  // one by more than 10 % of its norm: PCG goes on undisturbed to the phase-1 tolerance and the solve restarts on the
+  // true residual as in round 1)
+  int switched;
+  double dev2, rrt, srt;  // ||r_true - r||^2, ||r_true||^2, sum r_true of the attempt
   double inv_nact;  // 1 / #active cells when that projection is on, else 0
   double sb;        // sum of the prepared right-hand side b0 as stored (what the true residual's mean is)
   alignas(128) double pq[2];
@@ -87,6 +93,7 @@ struct NfHostStatus {  // written by the device into mapped pinned memory
   volatile int done;
   volatile int converged;
   volatile float relres;
+  volatile int switched;  // NfSolveState::switched
 };
 
 // One environment of a batched PCG iteration (nf_solver.cu: nf_solve_batch_run): the level-0
@@ -151,7 +158,8 @@ struct nf_grid {
   float *us, *vs, *ws, *sdf;
   // CG vectors on level 0 (r and z live in lv[0])
   float *r_alt;  // the residual ping-pongs between lv[0].r and this buffer (k_update_down1); both owned by the handle
-  float *ecorr;  // correction vector of the second PCG phase
+  float *ecorr;  // correction vector of the second PCG phase / after an in-flight replacement
+  float *rtrue;  // the true residual of an in-flight replacement attempt (read by ONE k_update_down1 if accepted)
   float *b0;  // the prepared right-hand side (kept for the true-residual refresh, nf_solver.cu)
   float *p, *p2, *q, *xtmp;  // p / p2: the search direction ping-pongs between two buffers (k_papply4)
   float *tailpack;  // 8 floats per cell of the tail levels (nf_mg.cu)
@@ -298,7 +306,7 @@ int nf_update_down1_batch(nf_grid **G, int n, const NfBatchK &B, int slot, int s
 int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1 = false);  // z = M^{-1} r on lv[0].r -> lv[0].z
 // fused r' = r - a q + pre-smoother of level 0 (r' into g->r_alt, then the two buffers swap); false if not applicable
 bool nf_update_down1_ok(const nf_grid *g);
-int nf_update_down1(nf_grid *g, int slot, NfHostStatus *hs, int seq);
+int nf_update_down1(nf_grid *g, int slot, NfHostStatus *hs, int seq, const float *rtrue = nullptr);
 // Solve A x = lv[0].r (already masked; mean removed if singular; st->bb set by nf_solve_prepare).
 int nf_solver_init(nf_grid *g);                          // kernel attributes (once per process)
 int nf_solve_prepare(nf_grid *g, float tol, int maxit);  // from lv[0].r: mask, mean removal, bb
@@ -405,6 +413,7 @@ __device__ __forceinline__ void nf_cg_check(NfSolveState *st, int slot, NfHostSt
   hs->iter = st->iter;
   hs->done = st->done;
   hs->converged = st->converged;
+  hs->switched = st->switched;
   __threadfence_system();
   hs->seq = seq;
   __threadfence_system();

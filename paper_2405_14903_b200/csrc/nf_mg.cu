@@ -122,15 +122,18 @@ __device__ __forceinline__ void nf_down1_body(const NfLvK &L, const float *r, fl
 // neighbours' threads still read r).  The last CTA to finish runs the convergence check (nf_cg_check).
 // (bz, nzc: this CTA's z-chunk and the number of z-chunks of ITS grid -- blockIdx.z / gridDim.z, or the environment's
 // share of them in a batched launch)
-__device__ __forceinline__ void nf_update_down1_body(const NfLvK &L, const float *__restrict__ rold,
+__device__ __forceinline__ void nf_update_down1_body(const NfLvK &L, const float *rold,
                                                      const float *__restrict__ q, float *__restrict__ rnew,
                                                      float *__restrict__ z, int kch, NfSolveState *st, int slot,
-                                                     NfHostStatus *hs, int seq, int bz, int nzc) {
+                                                     NfHostStatus *hs, int seq, int bz, int nzc,
+                                                     const float *rtrue = nullptr) {
   if (st->done) {  // (uniform: done is only ever set by the last CTA of an earlier launch)
     if (blockIdx.x == 0 && blockIdx.y == 0 && bz == 0 && threadIdx.x == 0 && threadIdx.y == 0)
       nf_cg_check(st, slot, hs, seq);
     return;
   }
+  // (an accepted in-flight replacement: this iteration reads the true residual instead of the recursive one)
+  if (rtrue && st->switched == 1) rold = rtrue;
   const double pq = st->pq[slot];
   const float a = (pq > 0.0) ? (float)(st->rz[slot] / pq) : 0.0f;
   // singular system: mu = mean of the residual being read (measured when it was written), taken off on the fly, so
@@ -181,9 +184,9 @@ __device__ __forceinline__ void nf_update_down1_body(const NfLvK &L, const float
 __global__ void __launch_bounds__(256, 4) k_update_down1(NfLvK L, const float *__restrict__ rold,
                                                       const float *__restrict__ q, float *__restrict__ rnew,
                                                       float *__restrict__ z, int kch, NfSolveState *st, int slot,
-                                                      NfHostStatus *hs, int seq) {
+                                                      NfHostStatus *hs, int seq, const float *rtrue) {
   nf_pdl_enter();
-  nf_update_down1_body(L, rold, q, rnew, z, kch, st, slot, hs, seq, (int)blockIdx.z, (int)gridDim.z);
+  nf_update_down1_body(L, rold, q, rnew, z, kch, st, slot, hs, seq, (int)blockIdx.z, (int)gridDim.z, rtrue);
 }
 // Batched launches: blockIdx.z = env * nzc + z-chunk; see k_papply4_b (nf_solver.cu)
 __global__ void __launch_bounds__(256, 4) k_update_down1_b(const __grid_constant__ NfBatchK B, int kch, int slot,
@@ -1545,11 +1548,11 @@ int nf_update_down1_batch(nf_grid **G, int n, const NfBatchK &Bin, int slot, int
 bool nf_update_down1_ok(const nf_grid *g) {
   return g->nu_pre == g->nu_post && !g->force_generic && g->lv[0].vec && g->nlev > 1;
 }
-int nf_update_down1(nf_grid *g, int slot, NfHostStatus *hs, int seq) {
+int nf_update_down1(nf_grid *g, int slot, NfHostStatus *hs, int seq, const float *rtrue) {
   NfLevel &L = g->lv[0];
   const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
   NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
-  NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_update_down1, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.r, (const float *)g->q, g->r_alt, L.z, kch, g->st, slot, hs, seq));
+  NF_LAUNCH(g, NFK_UPDATE, nf_launch_pdl(k_update_down1, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.r, (const float *)g->q, g->r_alt, L.z, kch, g->st, slot, hs, seq, rtrue));
   float *t = L.r;
   L.r = g->r_alt;
   g->r_alt = t;

@@ -89,12 +89,14 @@ __global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restr
 // a-4 + a-3 fused: p' = z + beta p (beta = rz_new / rz_old from device memory; FIRST: p' = z) evaluated on the fly
 // for the cell's own row and its neighbour rows, q = A p', p.q partial sums.  17 B/cell (z, p, code in; p', q out)
 // instead of 12 + 9 for the two separate passes.  p' goes to a second buffer: the neighbours' threads still read p.
+// xe (may be null): after an accepted in-flight replacement the deferred x update goes there instead of to x.
 template <bool FIRST>
 __device__ __forceinline__ void nf_papply4_body(const NfLvK &L, const float *__restrict__ z,
                                                 const float *__restrict__ pold, float *__restrict__ pnew,
-                                                float *__restrict__ q, float *__restrict__ x, int kch,
-                                                NfSolveState *st, int slot, int bz) {
+                                                float *__restrict__ q, float *x, int kch,
+                                                NfSolveState *st, int slot, int bz, float *xe = nullptr) {
   if (st->done) return;
+  if (xe && st->switched == 1) x = xe;
   float beta = 0.0f, aprev = 0.0f;
   if (!FIRST) {
     const double rz_old = st->rz[1 - slot];
@@ -174,10 +176,10 @@ __device__ __forceinline__ void nf_papply4_body(const NfLvK &L, const float *__r
 }
 template <bool FIRST>
 __global__ void __launch_bounds__(256, 3) k_papply4(NfLvK L, const float *__restrict__ z, const float *__restrict__ pold,
-                                                 float *__restrict__ pnew, float *__restrict__ q, float *__restrict__ x,
-                                                 int kch, NfSolveState *st, int slot) {
+                                                 float *__restrict__ pnew, float *__restrict__ q, float *x,
+                                                 int kch, NfSolveState *st, int slot, float *xe) {
   nf_pdl_enter();
-  nf_papply4_body<FIRST>(L, z, pold, pnew, q, x, kch, st, slot, (int)blockIdx.z);
+  nf_papply4_body<FIRST>(L, z, pold, pnew, q, x, kch, st, slot, (int)blockIdx.z, xe);
 }
 // The same pass for a batch of equally sized environments in ONE launch: blockIdx.z = env * nzc +
 // z-chunk, every environment with its own vectors and its own PCG scalars (an environment that has converged exits).
@@ -247,10 +249,12 @@ __global__ void __launch_bounds__(256) k_cg_update(float *__restrict__ x, float 
 
 // The x update of the LAST executed iteration (fused path: every other one rode on the next k_papply4).
 // p0 / p1: the ping-pong buffers; the iteration with parity slot s wrote p' into p_s and its scalars into slot s.
-__global__ void __launch_bounds__(256) k_x_final(float *__restrict__ x, const float *__restrict__ p0,
-                                                 const float *__restrict__ p1, size_t n, const NfSolveState *st) {
+__global__ void __launch_bounds__(256) k_x_final(float *x, const float *__restrict__ p0,
+                                                 const float *__restrict__ p1, size_t n, const NfSolveState *st,
+                                                 float *xe) {
   const int slot = st->last_slot;
   if (slot < 0) return;
+  if (xe && st->switched == 1) x = xe;
   const double pq = st->pq[slot];
   const float a = pq > 0.0 ? (float)(st->rz[slot] / pq) : 0.0f;
   const float4 *p4 = (const float4 *)(slot ? p1 : p0);
@@ -396,6 +400,8 @@ __global__ void k_init_state(NfSolveState *st, double tol, int maxit, double inv
   st->sr[0] = st->sr[1] = 0.0;
   st->sb = 0.0;
   st->inv_nact = inv_nact_proj;
+  st->switched = 0;
+  st->dev2 = st->rrt = st->srt = 0.0;
   st->tol2 = tol * tol;
   st->relres = 0.0;
   st->iter = 0;
@@ -438,6 +444,7 @@ __global__ void k_phase_begin(NfSolveState *st, double tol, int keep_done) {
   if (!keep_done) {
     st->done = 0;
     st->converged = 0;
+    st->switched = 0;
   }
 }
 // r = b0 - A x evaluated in fp64 from the fp32 data (one pass per solve: the fp32 evaluation of A x cancels
@@ -473,12 +480,13 @@ __global__ void __launch_bounds__(256) k_true_residual(float *__restrict__ r, co
 // check_done: return at once when the solve has converged (the in-flight replacement of nf_solve_run).
 __global__ void __launch_bounds__(256, 4) k_true_residual4(NfLvK L, float *__restrict__ r, const float *__restrict__ b0,
                                                         const float *__restrict__ x, NfSolveState *st, double *rr_out,
-                                                        double *sr_out, int check_done) {
+                                                        double *sr_out, int check_done, const float *__restrict__ rcmp,
+                                                        double *dev_out) {
   if (check_done && st->done) return;
   const int i0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z * blockDim.z + threadIdx.z;
-  double part = 0.0, sum = 0.0;
+  double part = 0.0, sum = 0.0, dev = 0.0;
   // singular system (NfSolveState::inv_nact): b0 as stored has the mean sb / #active, A x has none -- taken off here,
   // in fp64, where the subtraction is exact; what the fp32 rounding of r leaves is measured into sr[1]
   const double mb = st->sb * st->inv_nact;
@@ -508,13 +516,32 @@ __global__ void __launch_bounds__(256, 4) k_true_residual4(NfLvK L, float *__res
       sum += (double)out[t];
     }
     *reinterpret_cast<float4 *>(r + id) = make_float4(out[0], out[1], out[2], out[3]);
+    if (rcmp) {  // how far the recursive residual has drifted from this one
+      float ro[4];
+      nf_unpack4(nf_ld4(rcmp, id, true), ro);
+#pragma unroll
+      for (int t = 0; t < 4; ++t) dev += ((double)out[t] - (double)ro[t]) * ((double)out[t] - (double)ro[t]);
+    }
   }
+  if (dev_out) nf_block_atomic_add(dev, dev_out);
   if (rr_out) nf_block_atomic_add(part, rr_out);
   if (sr_out && st->inv_nact != 0.0) nf_block_atomic_add(sum, sr_out);
 }
-// (one thread) the sum slot of the residual buffer that k_true_residual4 is about to rewrite
-__global__ void k_zero_sr(NfSolveState *st, int slot) {
-  if (threadIdx.x == 0 && blockIdx.x == 0 && !st->done) st->sr[slot] = 0.0;
+// (one thread) accept or reject an in-flight replacement attempt: accepted when the true residual differs from the
+// recursive one by at most 10 % of its norm (then the perturbation of the recursion is harmless -- the channel-gate:
+// 2 % -- otherwise PCG stalls: the chamber pump's first steps, whose pressure is 1e4 times larger relative to b, showed
+// 400 iterations).  Rejected: the iteration reads the recursive residual as if nothing had happened and the solve
+// stops at the phase-1 tolerance for the restart on the true residual.
+__global__ void k_switch_decide(NfSolveState *st, int slot, double tol1) {
+  if (threadIdx.x != 0 || blockIdx.x != 0 || st->done) return;
+  if (st->dev2 <= 0.01 * st->rrt) {
+    st->switched = 1;
+    st->sr[1 - slot] = st->srt;  // (the mean k_update_down1 takes off belongs to the buffer it reads)
+  } else {
+    st->switched = -1;
+    st->tol2 = tol1 * tol1;
+  }
+  st->dev2 = st->rrt = st->srt = 0.0;
 }
 // warm start: the initial guess on the active cells only (0 elsewhere), and 0 everywhere when b = 0 (done is then
 // already set by k_start_state: the answer is x = 0).  NaN, inf and absurdly large entries (an uninitialised array
@@ -674,17 +701,20 @@ struct NfPhaseOut {
   float relres;
 };
 // xe != nullptr (fused path only): IN-FLIGHT RESIDUAL REPLACEMENT.  Once the host has seen the residual below
-// switch_tol, the next iteration recomputes r = b0 - A x in fp64 right after its A-apply (x then holds every update but
-// this iteration's own) and every later update goes to xe (zeroed by the caller) instead of x: the recursion r -= a q
-// drifts from b - A x only through the rounding of the updates of an O(1) x, and the updates of a correction 1e-3 as
-// large round 1e-3 as coarsely.  The search direction is kept, so -- unlike a restart on the true residual -- no
-// V-cycle and no iteration is spent on rebuilding the Krylov space (van der Vorst & Ye's residual replacement; measured
-// at 256^3: 16 iterations and no extra V-cycle against 17 + 1, the same fp64 true residual of 5e-7).  *switched: it happened.
+// switch_tol, the next iteration evaluates r_true = b0 - A x in fp64 right after its A-apply (x then holds every update
+// but this iteration's own) and, if that differs from the recursive residual by no more than 10 % of its norm
+// (k_switch_decide, on the device), reads it instead; every later update then goes to xe (zeroed by the caller) instead
+// of x.  The recursion r -= a q drifts from b - A x only through the rounding of the updates of an O(1) x, and the
+// updates of a correction 1e-3 as large round 1e-3 as coarsely.  The search direction is kept, so -- unlike a restart
+// on the true residual -- no V-cycle and no iteration is spent on rebuilding the Krylov space (van der Vorst & Ye's
+// residual replacement; measured at 256^3: 16 iterations and no extra V-cycle against 17 + 1, the same fp64 true
+// residual of 5e-7).  A rejected attempt costs the one evaluation: PCG goes on to tol1 and the caller restarts as before.
+// *switched: 1 accepted, -1 rejected, 0 not tried.
 static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, NfPhaseOut *out, float switch_tol = 0.0f,
-                         float *xe = nullptr, bool *switched = nullptr) {
+                         float *xe = nullptr, int *switched = nullptr, float tol1 = 0.0f) {
   NfLevel &L = g->lv[0];
   const size_t n = (size_t)L.ncell;
-  float *xcur = x;            // where the deferred x updates go
+  float *xalt = nullptr;      // handed to the kernels once an attempt has been enqueued: they pick x or xe themselves
   bool sw = false;
   float seen_relres = 1e30f;  // the last residual the host has read
   for (int s = 0; s < NF_RING; ++s) g->hst[s].seq = 0;
@@ -719,20 +749,23 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
       const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_AP);
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
       if (it == 0)
-        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<true>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, xcur, kch, g->st, slot));
+        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<true>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, kch, g->st, slot, xalt));
       else
-        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<false>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, xcur, kch, g->st, slot));
+        NF_LAUNCH(g, NFK_APPLY, nf_launch_pdl(k_papply4<false>, d.grid, d.block, g->stream, nf_lvk(L), (const float *)L.z, (const float *)pold, pnew, g->q, x, kch, g->st, slot, xalt));
+      const float *rtrue = nullptr;
       if (xe && !sw && fusedr && it > 0 && seen_relres <= switch_tol) {
-        // x is complete up to the previous iteration: r (the buffer k_update_down1 is about to read) = b0 - A x
+        // x is complete up to the previous iteration: r_true = b0 - A x into its own array, compared with the
+        // recursive residual k_update_down1 is about to read; the device decides which of the two it reads
         NfDims dv = nf_dims(L.nx / 4, L.ny, L.nz);
-        NF_LAUNCH(g, NFK_SETUP, k_zero_sr<<<1, 32, 0, g->stream>>>(g->st, 1 - slot));
-        NF_LAUNCH(g, NFK_SETUP, k_true_residual4<<<dv.grid, dv.block, 0, g->stream>>>(nf_lvk(L), L.r, g->b0, x, g->st, nullptr, &g->st->sr[1 - slot], 1));
-        xcur = xe;
+        NF_LAUNCH(g, NFK_SETUP, k_true_residual4<<<dv.grid, dv.block, 0, g->stream>>>(nf_lvk(L), g->rtrue, g->b0, x, g->st, &g->st->rrt, &g->st->srt, 1, (const float *)L.r, &g->st->dev2));
+        NF_LAUNCH(g, NFK_SETUP, k_switch_decide<<<1, 32, 0, g->stream>>>(g->st, slot, (double)tol1));
+        rtrue = g->rtrue;
+        xalt = xe;
         sw = true;
       }
       if (fusedr) {
         // r' = r - a q, ||r'||^2, the check and the pre-smoother of level 0 in one pass; the V-cycle skips its down1
-        rc = nf_update_down1(g, slot, hs, it + 1);
+        rc = nf_update_down1(g, slot, hs, it + 1, rtrue);
         if (rc != NF_OK) return rc;
         if ((rc = prof_check(it)) != NF_OK) return rc;
         if (stop_now) { ++it; break; }
@@ -777,8 +810,7 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
     }
   }
   // the x update of the last executed iteration (every other one rode on the following k_papply4)
-  if (fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(xcur, g->p, g->p2, n, g->st));
-  if (switched) *switched = sw;
+  if (fusedp) NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->p, g->p2, n, g->st, xalt));
   // drain: every enqueued check must have reported before the ring is reused
   const int enq = it;  // checks enqueued: 0 .. enq-1
   for (int s = last_seen + 1; s < enq; ++s) {
@@ -789,6 +821,7 @@ static int run_pcg_phase(nf_grid *g, float *x, int maxit, bool fusedp, int v4, N
   out->converged = h->converged;
   out->relres = h->relres;
   out->iters = h->iter;
+  if (switched) *switched = sw ? h->switched : 0;
   return NF_OK;
 }
 
@@ -908,7 +941,7 @@ int nf_solve_batch_run(nf_grid **G, int n, float *const *x, int maxit, int *stat
   const int enq = it;
   for (int e = 0; e < n; ++e) {
     nf_grid *g = G[e];
-    NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x[e], g->p, g->p2, nc, g->st));
+    NF_LAUNCH(g, NFK_PUPDATE, k_x_final<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x[e], g->p, g->p2, nc, g->st, nullptr));
     for (int s = last_seen + 1; s < enq; ++s) NF_TRY(wait_seq(g, s, s + 1));
     const NfHostStatus *h = &g->hst[(enq - 1) & (NF_RING - 1)];
     g->last_iters = h->iter;
@@ -949,7 +982,7 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
   NfPhaseOut ph;
   ph.converged = 0; ph.iters = 0; ph.relres = 0.0f;
   int rc = NF_OK;
-  bool switched = false;
+  int switched = 0;  // in-flight replacement: 1 accepted, -1 rejected, 0 not tried
   g->lo_valid = false;
   if (g->plo) NF_CUDA(g, cudaMemsetAsync(g->plo, 0, n * sizeof(float), g->stream));
   // r = b - A x afresh (fp64 evaluation); decide at `tol`; if not done run PCG on it (phase tolerance tolp) for a
@@ -958,7 +991,7 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
     NF_LAUNCH(g, NFK_SETUP, k_phase_begin<<<1, 32, 0, g->stream>>>(g->st, (double)tolp, 0));
     if (!g->force_generic && apply_vec_ok(L, x, L.r) && apply_vec_ok(L, g->b0, g->b0)) {
       NfDims dv = nf_dims(L.nx / 4, L.ny, L.nz);
-      NF_LAUNCH(g, NFK_SETUP, k_true_residual4<<<dv.grid, dv.block, 0, g->stream>>>(nf_lvk(L), L.r, g->b0, x, g->st, &g->st->rr[0], &g->st->sr[1], 0));
+      NF_LAUNCH(g, NFK_SETUP, k_true_residual4<<<dv.grid, dv.block, 0, g->stream>>>(nf_lvk(L), L.r, g->b0, x, g->st, &g->st->rr[0], &g->st->sr[1], 0, nullptr, nullptr));
     } else {
       NF_LAUNCH(g, NFK_SETUP, k_true_residual<<<dc.grid, dc.block, 0, g->stream>>>(L.r, g->b0, x, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, g->st));
     }
@@ -1001,9 +1034,9 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
       // (never below 1e-4: a replacement made when the residual is down at the drift itself perturbs the recursion by
       // as much as it carries, and PCG stalls -- measured at tol 1e-12: stuck at 1e-6 with the switch at sqrt(tol) = 1e-6)
       const float sw_tol = fminf(fmaxf(sqrtf(tol), 1e-4f), 1e-2f);
-      rc = run_pcg_phase(g, x, maxit, fusedp, v4, &ph, sw_tol, g->ecorr, &switched);
+      rc = run_pcg_phase(g, x, maxit, fusedp, v4, &ph, sw_tol, g->ecorr, &switched, tol1);
       if (rc != NF_OK) return rc;
-      if (switched) {
+      if (switched == 1) {
         if (g->plo) {
           NF_LAUNCH(g, NFK_SETUP, k_add_hilo<<<NF_VEC_BLOCKS, 256, 0, g->stream>>>(x, g->ecorr, g->plo, n));
           g->lo_valid = true;
@@ -1019,13 +1052,13 @@ int nf_solve_run(nf_grid *g, float *x, float tol, int maxit, bool warm) {
   }
   // (after an in-flight replacement the recursive residual IS the true one: nothing to refresh; if the solve converged
   // before the host could place the replacement, the refresh below checks the true residual as before)
-  if (two_phase && !switched && ph.converged && ph.iters > 0 && ph.iters < maxit) {
+  if (two_phase && switched != 1 && ph.converged && ph.iters > 0 && ph.iters < maxit) {
     // (the correction is ~1e-4 of x: accumulated on its own its rounding is invisible, and x is rounded once)
     rc = correct(tol);
     if (rc != NF_OK) return rc;
   }
   // (phase 1 met its own 30 tol on the very last iteration allowed: that is not the caller's tolerance)
-  if (two_phase && !switched && ph.converged && ph.iters >= maxit && !(ph.relres <= tol)) ph.converged = 0;
+  if (two_phase && switched != 1 && ph.converged && ph.iters >= maxit && !(ph.relres <= tol)) ph.converged = 0;
   g->last_iters = ph.iters;
   NF_TRY(apply_gauge(g, x));
   g->last_relres = ph.relres;
