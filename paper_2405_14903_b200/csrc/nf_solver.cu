@@ -93,10 +93,10 @@ __global__ void __launch_bounds__(256, 4) k_apply4(NfLvK L, const float *__restr
 template <bool FIRST>
 __device__ __forceinline__ void nf_papply4_body(const NfLvK &L, const float *__restrict__ z,
                                                 const float *__restrict__ pold, float *__restrict__ pnew,
-                                                float *__restrict__ q, float *x, int kch,
+                                                float *__restrict__ q, float *xa, int kch,
                                                 NfSolveState *st, int slot, int bz, float *xe = nullptr) {
   if (st->done) return;
-  if (xe && st->switched == 1) x = xe;
+  float *__restrict__ x = (xe && st->switched == 1) ? xe : xa;
   float beta = 0.0f, aprev = 0.0f;
   if (!FIRST) {
     const double rz_old = st->rz[1 - slot];
