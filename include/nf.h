@@ -85,7 +85,11 @@ int nf_set_domain_bc(nf_grid *g, int face, int type, float p_value);
  *          bit 2 = switch OFF the true-residual refresh.  By default a solve with tol < 3e-4 runs PCG to 30 tol,
  *                  re-evaluates r = b - A x in fp64 (the fp32 recursion r -= a q drifts: at 256^3 a recursive 1e-6
  *                  was a true 4e-5), and runs PCG on that residual for a correction down to tol; the true residual
- *                  then sits at the storage rounding of the fp32 pressure,
+ *                  then sits at the storage rounding of the fp32 pressure.  Where the fused
+ *                  kernels run, the refresh happens IN FLIGHT instead: PCG runs straight to tol, one iteration
+ *                  evaluates b - A x in fp64 once the residual is below sqrt(tol) and -- if that differs from the
+ *                  recursive residual by no more than 10 % (decided on the device) -- continues from it with the
+ *                  search direction kept and the later updates in a separate correction; otherwise as above,
  *          bit 3 = warm start: the solution array the caller passes (p of nf_project / nf_solve, y_out of
  *                  nf_project_adjoint) holds the initial guess on entry, e.g. the pressure of the previous time
  *                  step (the paper is silent on x0, R11; default x0 = 0).  The stopping criterion stays relative to
