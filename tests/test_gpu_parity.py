@@ -255,12 +255,16 @@ def test_vcycle_fused_equals_generic(torch, api, shape, bt):
     act = (au[:, :, :-1] + au[:, :, 1:] + av[:, :-1] + av[:, 1:] + aw[:-1] + aw[1:]) > 0
     r = torch.randn(g.shape_p, device="cuda") * act
     z1, z2 = torch.empty_like(r), torch.empty_like(r)
-    g.vcycle(r, z1)
-    g.set_solver_options(1, 1, 2)
-    g.vcycle(r, z2)
-    assert float(z2.abs().max()) > 0
-    assert rel(host(z1), host(z2)) < 2e-5
-    assert float((z1 * (~act)).abs().max()) == 0.0  # inactive cells stay 0
+    # V(1,1) and several sweeps on the coarse levels (the multi-sweep instances of the coarse kernel, 2-D ones included)
+    for nu in ((1, 1), (2, 3)):
+        g.set_coarse_sweeps(*nu)
+        g.set_solver_options(1, 1, 0)
+        g.vcycle(r, z1)
+        g.set_solver_options(1, 1, 2)
+        g.vcycle(r, z2)
+        assert float(z2.abs().max()) > 0
+        assert rel(host(z1), host(z2)) < 2e-5, nu
+        assert float((z1 * (~act)).abs().max()) == 0.0  # inactive cells stay 0
     g.close()
 
 
