@@ -27,6 +27,8 @@ _SIGNATURES = {
     "nf_set_solver_options": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
     "nf_set_coarse_sweeps": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
     "nf_get_sweeps": (ctypes.c_int, [ctypes.c_void_p] + [ctypes.POINTER(ctypes.c_int)] * 4),
+    "nf_set_coarse_relaxation": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
+    "nf_get_coarse_relaxation": (ctypes.c_float, [ctypes.c_void_p]),
     "nf_set_pressure_lo": (ctypes.c_int, [ctypes.c_void_p, _c_float_p]),
     "nf_set_solid": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 4),
     "nf_set_weights": (ctypes.c_int, [ctypes.c_void_p] + [_c_float_p] * 3),
@@ -235,6 +237,13 @@ class Grid:
     def set_coarse_sweeps(self, nu_level1=2, nu_deeper=None):
         nd = nu_level1 if nu_deeper is None else nu_deeper
         self._check(self.lib.nf_set_coarse_sweeps(self.h, int(nu_level1), int(nd)), "nf_set_coarse_sweeps")
+
+    @_bound
+    def set_coarse_relaxation(self, omega=1.0):
+        self._check(self.lib.nf_set_coarse_relaxation(self.h, float(omega)), "nf_set_coarse_relaxation")
+
+    def coarse_relaxation(self):
+        return float(self.lib.nf_get_coarse_relaxation(self.h))
 
     def sweeps(self):
         """(nu_fine_pre, nu_fine_post, nu_level1, nu_deeper) in force."""

@@ -511,7 +511,8 @@ template <bool ZERO, bool DOT>
 __global__ void __launch_bounds__(256) k_rbgs(float *__restrict__ z, const float *__restrict__ r,
                                               const float *__restrict__ ax, const float *__restrict__ ay,
                                               const float *__restrict__ az, float c, int nx, int ny, int nz, int pax,
-                                              int color, NfSolveState *st, int slot) {
+                                              int color, NfSolveState *st, int slot, float om = 1.0f,
+                                              int old_is_zero = 0) {
   if (st && st->done) return;
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -530,6 +531,9 @@ __global__ void __launch_bounds__(256) k_rbgs(float *__restrict__ z, const float
         float s = rv;
         if (!ZERO) s += c * nf_nb_sum(z, w, i, j, k, nx, ny, nz);
         zn = s / (c * d);
+        // over-relaxation (om = 1: plain Gauss-Seidel).  ZERO / old_is_zero: the cell's old value is the zero guess --
+        // the array itself still holds the previous cycle's result on the cells no sweep has written yet
+        if (om != 1.0f) zn = (ZERO || old_is_zero) ? om * zn : (1.0f - om) * z[id] + om * zn;
       }
       z[id] = zn;
       if (DOT) part = (double)rv * (double)zn;
@@ -606,6 +610,7 @@ __global__ void __launch_bounds__(256) k_dot_rz(const float *__restrict__ a, con
 struct NfTailK {
   int nlev, sweeps;
   int npre[NF_MAX_LEVELS], npost[NF_MAX_LEVELS];  // red-black sweeps before / after the coarse correction, per level
+  float om[NF_MAX_LEVELS];  // over-relaxation factor of the sweeps, per level (1 = Gauss-Seidel)
   int singular;  // the system has the constant null vector (R12): the coarsest solve works in its complement
   int direct;    // 1: the coarsest level is solved with the precomputed inverse
   int n[NF_MAX_LEVELS], nx[NF_MAX_LEVELS], ny[NF_MAX_LEVELS], nz[NF_MAX_LEVELS];
@@ -760,7 +765,7 @@ __global__ void __launch_bounds__(1024) k_coarse_inverse(const float *__restrict
 // smem per level (float offset soff[l]): z[np], r[np], pack[8n]
 __device__ __forceinline__ void nf_tail_half(float *__restrict__ z, const float *__restrict__ r,
                                              const float *__restrict__ pk, int n, int nx, int sy, int sz, float color,
-                                             bool zero) {
+                                             bool zero, float om = 1.0f) {
   // nx even: the cells 2h, 2h+1 lie in one row and have different colours -- every thread updates one cell of the
   // wanted colour (no idle half); nx odd: scan all cells
   const bool pairs = (nx & 1) == 0;
@@ -782,7 +787,9 @@ __device__ __forceinline__ void nf_tail_half(float *__restrict__ z, const float 
       a += pk[5 * n + id] * z[max(id - sz, 0)];
       a += pk[6 * n + id] * z[min(id + sz, n - 1)];
     }
-    z[id] = a * pk[id];
+    // (over-relaxed: z = (1 - om) z + om GS; an inactive cell -- pk[id] = 0 -- stays 0 whatever the prolongation left)
+    const float g = pk[id];
+    z[id] = g > 0.0f ? (zero ? om * (a * g) : (1.0f - om) * z[id] + om * (a * g)) : 0.0f;
   }
   __syncthreads();
 }
@@ -900,13 +907,16 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
   for (int l = 0; l + 1 < nl; ++l) {
     const int n = T.n[l], nx = T.nx[l], ny = T.ny[l];
     float *z = sm + T.soff[l], *r = z + T.np[l], *pk = z + 2 * T.np[l];
-    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, true);
-    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+    const float om = T.om[l];
+    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, true, om);
+    nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false, om);
     for (int s = 1; s < T.npre[l]; ++s) {
-      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
-      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
+      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false, om);
+      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false, om);
     }
-    const bool first_only = T.npre[l] == 1;
+    // (plain Gauss-Seidel, one sweep: the black residual is zero and a red cell holds r / diag exactly; several sweeps:
+    // the red residual needs the full expression; over-relaxed: so does every child)
+    const bool first_only = T.npre[l] == 1 && om == 1.0f, allc = om != 1.0f;
     // residual + restriction: r_c = 1/8 sum children (r - A z), A z = z/idg - sum wg z_nb on active cells
     const int cn = T.n[l + 1], cnx = T.nx[l + 1], cny = T.ny[l + 1], fz = T.fz[l];
     float *rc = sm + T.soff[l + 1] + T.np[l + 1];
@@ -921,7 +931,7 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
 #pragma unroll
           for (int di = 0; di < 2; ++di) {
             // (the residual is zero on the black cells: the black half sweep has just solved their equations)
-            if (((di + dj + dk) & 1) || dk >= fz) continue;
+            if ((!allc && ((di + dj + dk) & 1)) || dk >= fz) continue;
             if (2 * I + di >= nx || 2 * J + dj >= ny || fz * K + dk >= T.nz[l]) continue;  // (odd extent: no such child)
             const int id = ((fz * K + dk) * ny + (2 * J + dj)) * nx + 2 * I + di;
             const float s = pk[1 * n + id] * z[max(id - 1, 0)] + pk[2 * n + id] * z[min(id + 1, n - 1)] +
@@ -1004,8 +1014,8 @@ __device__ __forceinline__ void nf_tail_run(const NfTailK &T, const float *__res
     }
     __syncthreads();
     for (int s = 0; s < T.npost[l]; ++s) {
-      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false);
-      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false);
+      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 1.0f, false, T.om[l]);
+      nf_tail_half(z, r, pk, n, nx, nx, nx * ny, 0.0f, false, T.om[l]);
     }
   }
   for (int t = threadIdx.x; t < T.n[0]; t += blockDim.x) zg[t] = sm[T.soff[0] + t];
@@ -1046,7 +1056,8 @@ __device__ __forceinline__ void nf_dense_nb(const NfDenseLv &D, int id, int nb[6
   nb[4] = max(id - sz, 0); nb[5] = min(id + sz, D.n - 1);
 }
 // pre-smooth from a zero guess, both colours in one phase: red z = r idg; black from its red neighbours' r idg
-__device__ __forceinline__ void nf_dense_down1(const NfDenseLv &D, int id) {
+// (om: over-relaxation factor; from the zero guess both colours are om times the Gauss-Seidel value)
+__device__ __forceinline__ void nf_dense_down1(const NfDenseLv &D, int id, float om) {
   const int i = id % D.nx, j = (id / D.nx) % D.ny, k = id / (D.nx * D.ny);
   const float idg = D.pk[id], rv = D.r[id];
   float a = rv;
@@ -1054,12 +1065,14 @@ __device__ __forceinline__ void nf_dense_down1(const NfDenseLv &D, int id) {
     int nb[6];
     nf_dense_nb(D, id, nb);
 #pragma unroll
-    for (int f = 0; f < 6; ++f) a += D.pk[(1 + f) * D.n + id] * (D.r[nb[f]] * D.pk[nb[f]]);
+    for (int f = 0; f < 6; ++f) a += D.pk[(1 + f) * D.n + id] * (om * (D.r[nb[f]] * D.pk[nb[f]]));
   }
-  D.z[id] = a * idg;
+  D.z[id] = om * (a * idg);
 }
 // residual + restriction of the coarse cell cid: red children only (the black residual is zero)
-__device__ __forceinline__ void nf_dense_down2(const NfDenseLv &D, float *rc, int cnx, int cny, int cid, bool gen) {
+// (allc: over-relaxed sweeps leave a residual on the black cells too -- all eight children, full expression)
+__device__ __forceinline__ void nf_dense_down2(const NfDenseLv &D, float *rc, int cnx, int cny, int cid, bool gen,
+                                               bool allc = false) {
   const int I = cid % cnx, J = (cid / cnx) % cny, K = cid / (cnx * cny);
   float acc = 0.0f;
 #pragma unroll
@@ -1068,7 +1081,7 @@ __device__ __forceinline__ void nf_dense_down2(const NfDenseLv &D, float *rc, in
     for (int dj = 0; dj < 2; ++dj)
 #pragma unroll
       for (int di = 0; di < 2; ++di) {
-        if ((di + dj + dk) & 1) continue;
+        if (!allc && ((di + dj + dk) & 1)) continue;
         const int id = ((2 * K + dk) * D.ny + (2 * J + dj)) * D.nx + 2 * I + di;
         int nb[6];
         nf_dense_nb(D, id, nb);
@@ -1082,7 +1095,7 @@ __device__ __forceinline__ void nf_dense_down2(const NfDenseLv &D, float *rc, in
   rc[cid] = 0.125f * acc;
 }
 // black half sweep on z + P zc (red cells keep the un-prolonged value; the red sweep does not read it)
-__device__ __forceinline__ void nf_dense_up1(const NfDenseLv &D, const float *zc, int cnx, int cny, int id) {
+__device__ __forceinline__ void nf_dense_up1(const NfDenseLv &D, const float *zc, int cnx, int cny, int id, float om) {
   const int i = id % D.nx, j = (id / D.nx) % D.ny, k = id / (D.nx * D.ny);
   if (((i + j + k) & 1) == 0) return;
   int nb[6];
@@ -1095,10 +1108,16 @@ __device__ __forceinline__ void nf_dense_up1(const NfDenseLv &D, const float *zc
               kk = min(max(k + dk[f], 0), D.nz - 1);
     a += D.pk[(1 + f) * D.n + id] * (D.z[nb[f]] + zc[((kk >> 1) * cny + (jj >> 1)) * cnx + (ii >> 1)]);
   }
-  D.z[id] = a * D.pk[id];
+  const float g = D.pk[id];
+  // (over-relaxed: the old value is the PROLONGED one; an inactive cell stays 0)
+  const float zo = om != 1.0f ? D.z[id] + zc[((k >> 1) * cny + (j >> 1)) * cnx + (i >> 1)] : 0.0f;
+  D.z[id] = g > 0.0f ? (1.0f - om) * zo + om * (a * g) : 0.0f;
 }
 // half sweep on the cells of one colour (0 = red, 1 = black)
-__device__ __forceinline__ void nf_dense_up2(const NfDenseLv &D, int id, int color = 0) {
+// (om: over-relaxation; zc != nullptr: the cell's old value has not been prolonged yet -- the first red half sweep
+// after nf_dense_up1, which leaves the red cells alone)
+__device__ __forceinline__ void nf_dense_up2(const NfDenseLv &D, int id, int color, float om, const float *zc, int cnx,
+                                             int cny) {
   const int i = id % D.nx, j = (id / D.nx) % D.ny, k = id / (D.nx * D.ny);
   if (((i + j + k) & 1) != color) return;
   int nb[6];
@@ -1106,13 +1125,17 @@ __device__ __forceinline__ void nf_dense_up2(const NfDenseLv &D, int id, int col
   float a = D.r[id];
 #pragma unroll
   for (int f = 0; f < 6; ++f) a += D.pk[(1 + f) * D.n + id] * D.z[nb[f]];
-  D.z[id] = a * D.pk[id];
+  const float g = D.pk[id];
+  float zo = 0.0f;
+  if (om != 1.0f) zo = D.z[id] + (zc ? zc[((k >> 1) * cny + (j >> 1)) * cnx + (i >> 1)] : 0.0f);
+  D.z[id] = g > 0.0f ? (1.0f - om) * zo + om * (a * g) : 0.0f;
 }
 
 struct NfCoarseK {
   int first, nb, has_tail;
   int dense_from;  // levels >= dense_from (and < nb) run the per-cell phases
   int nu[NF_MAX_LEVELS];  // red-black sweeps before and after the coarse correction, per level
+  float om[NF_MAX_LEVELS];  // over-relaxation factor of the per-cell (dense) levels' sweeps; 1 elsewhere
   const float *pk[NF_MAX_LEVELS];
   NfLvK lv[NF_MAX_LEVELS];
   float *z[NF_MAX_LEVELS], *r[NF_MAX_LEVELS];
@@ -1149,12 +1172,12 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
     }
   }
   // one half sweep of level l as a phase: color 0 = red, 1 = black
-  auto half = [&](int l, int color) {
+  auto half = [&](int l, int color, const float *zcp) {
     const NfLvK &L = P.lv[l];
     if (l >= P.dense_from) {
       NfDenseLv D;
       D.pk = P.pk[l]; D.z = P.z[l]; D.r = P.r[l]; D.nx = L.nx; D.ny = L.ny; D.nz = L.nz; D.n = L.nx * L.ny * L.nz;
-      for (int t = gt; t < D.n; t += gn) nf_dense_up2(D, t, color);
+      for (int t = gt; t < D.n; t += gn) nf_dense_up2(D, t, color, P.om[l], zcp, P.lv[l + 1].nx, P.lv[l + 1].ny);
     } else {
       const int nx4 = L.nx >> 2, ny = L.ny, nz = L.nz;
       for (int t = gt; t < nx4 * ny * nz; t += gn) {
@@ -1174,7 +1197,7 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
     NfDenseLv D;
     D.pk = P.pk[l]; D.z = P.z[l]; D.r = P.r[l]; D.nx = L.nx; D.ny = ny; D.nz = nz; D.n = L.nx * ny * nz;
     if (dense) {
-      for (int t = gt; t < D.n; t += gn) nf_dense_down1(D, t);
+      for (int t = gt; t < D.n; t += gn) nf_dense_down1(D, t, P.om[l]);
     } else {
       for (int t = gt; t < nx4 * ny * nz; t += gn) {
         const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
@@ -1187,7 +1210,7 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
     sync();
     if (MULTI) {  // further pre-smoothing sweeps: red, black, red, ... (one call site: one copy of the code)
       for (int q = 0; q < 2 * (P.nu[l] - 1); ++q) {
-        half(l, q & 1);
+        half(l, q & 1, nullptr);
         sync();
       }
     }
@@ -1195,7 +1218,7 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
     // so the MULTI instance carries that form only)
     const bool gen = MULTI;
     if (dense) {
-      for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t, gen);
+      for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t, gen, MULTI && P.om[l] != 1.0f);
     } else {
       for (int t = gt; t < nx4 * cny * cnz; t += gn) {
         const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
@@ -1216,7 +1239,7 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
     NfDenseLv D;
     D.pk = P.pk[l]; D.z = P.z[l]; D.r = P.r[l]; D.nx = L.nx; D.ny = ny; D.nz = nz; D.n = L.nx * ny * nz;
     if (dense) {
-      for (int t = gt; t < D.n; t += gn) nf_dense_up1(D, P.z[l + 1], cnx, cny, t);
+      for (int t = gt; t < D.n; t += gn) nf_dense_up1(D, P.z[l + 1], cnx, cny, t, P.om[l]);
     } else {
       for (int t = gt; t < nx4 * ny * nz; t += gn) {
         const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
@@ -1232,7 +1255,7 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
     // the red half sweep, then (black, red) once more per further sweep -- one call site
     for (int q = 0; q < (MULTI ? 2 * P.nu[l] - 1 : 1); ++q) {
       if (q) sync();
-      half(l, q & 1);
+      half(l, q & 1, q == 0 ? P.z[l + 1] : nullptr);  // (the first red half sweep prolongs its own old value)
     }
     if (l > P.first) sync();
   }
@@ -1297,8 +1320,13 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_c
 // host side
 // ------------------------------------------------------------------------------------------------------------
 static inline int nf_nu_coarse(const nf_grid *g, int l) { return l <= 1 ? g->nu_l1 : g->nu_deep; }
+// over-relaxation of the red-black sweeps: the levels from 2 down (their bodies carry the old value and the full
+// residual; the finest level's and level 1's fused bodies are plain Gauss-Seidel), never in 2-D mode
+static inline float nf_omega(const nf_grid *g, int l) { return (l >= 2 && g->nz != 1) ? g->omega_deep : 1.0f; }
 // some grid-phase level of the coarse kernel runs more than one sweep
-static inline bool nf_coarse_multi(const nf_grid *g) { return g->nu_l1 > 1 || (g->nu_deep > 1 && g->tail > 2); }
+static inline bool nf_coarse_multi(const nf_grid *g) {
+  return g->nu_l1 > 1 || ((g->nu_deep > 1 || (g->omega_deep != 1.0f && g->nz != 1)) && g->tail > 2);
+}
 #define NF_TAIL_SMEM_MAX 231424  // dynamic shared memory of k_tail / k_vcoarse (226 KB of the 227 KB a CTA may use)
 
 // Shared-memory layout of a tail that starts at level `first` (NfTailK); T.total_floats is what it needs.
@@ -1327,6 +1355,7 @@ static void tail_desc(const nf_grid *g, int first, NfTailK *T) {
   for (int l = first; l < nl; ++l) {
     T->npre[l - first] = l == 0 ? g->nu_pre : nf_nu_coarse(g, l);
     T->npost[l - first] = l == 0 ? g->nu_post : nf_nu_coarse(g, l);
+    T->om[l - first] = nf_omega(g, l);
   }
   T->singular = g->singular_info;  // (only read when the coarsest level is too large for the direct solve)
 }
@@ -1419,15 +1448,18 @@ int nf_mg_pack_tail(nf_grid *g) {
   return NF_OK;
 }
 
-static void smooth_half(nf_grid *g, NfLevel &L, int color, bool zero, bool dot, NfSolveState *st, int slot) {
+static void smooth_half(nf_grid *g, NfLevel &L, int color, bool zero, bool dot, NfSolveState *st, int slot,
+                        bool old_is_zero = false) {
+  const float om = nf_omega(g, (int)(&L - &g->lv[0]));
+  const int oz = old_is_zero ? 1 : 0;
   NfDims d = nf_dims((L.nx + 1) / 2, L.ny, L.nz);
   const int cls = (&L == &g->lv[0]) ? NFK_RBGS0 : NFK_RBGS_C;
   if (zero)
-    NF_LAUNCH(g, cls, k_rbgs<true, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot));
+    NF_LAUNCH(g, cls, k_rbgs<true, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot, om, oz));
   else if (dot)
-    NF_LAUNCH(g, cls, k_rbgs<false, true><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot));
+    NF_LAUNCH(g, cls, k_rbgs<false, true><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot, om, oz));
   else
-    NF_LAUNCH(g, cls, k_rbgs<false, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot));
+    NF_LAUNCH(g, cls, k_rbgs<false, false><<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, color, st, slot, om, oz));
 }
 
 // The level table of the cooperative coarse kernel (levels 1 .. tail-1 as grid phases, then the tail)
@@ -1435,7 +1467,10 @@ static void fill_coarse(const nf_grid *g, NfCoarseK *P) {
   const int nl = g->nlev, nb = g->tail < nl ? g->tail : nl - 1;
   memset(P, 0, sizeof(*P));
   P->first = 1; P->nb = nb; P->has_tail = 1;
-  for (int l = 0; l < NF_MAX_LEVELS; ++l) P->nu[l] = nf_nu_coarse(g, l);
+  for (int l = 0; l < NF_MAX_LEVELS; ++l) {
+    P->nu[l] = nf_nu_coarse(g, l);
+    P->om[l] = nf_omega(g, l);
+  }
   P->dense_from = NF_MAX_LEVELS;
   for (int l = 0; l < nl; ++l) {
     P->lv[l] = nf_lvk(g->lv[l]);
@@ -1570,7 +1605,8 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
   const bool coop = fused && g->coarse_ctas > 0 && g->lv[0].vec;
   for (int l = 0; l < (coop ? 1 : nb); ++l) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
-    if (L.vec && fused) {
+    // (the 4-cell bodies are plain Gauss-Seidel: an over-relaxed level outside the cooperative kernel runs the generic ones)
+    if (L.vec && fused && nf_omega(g, l) == 1.0f) {
       const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
       const int nu = l == 0 ? g->nu_pre : nf_nu_coarse(g, l);
@@ -1584,7 +1620,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
     } else {
       for (int s = 0; s < (l == 0 ? g->nu_pre : nf_nu_coarse(g, l)); ++s) {
         smooth_half(g, L, 0, s == 0, false, st, slot);
-        smooth_half(g, L, 1, false, false, st, slot);
+        smooth_half(g, L, 1, false, false, st, slot, s == 0);  // (first black half sweep: its own old value is the zero guess)
       }
       NfDims d = nf_dims(C.nx, C.ny, C.nz);
       NF_LAUNCH(g, (l == 0 ? NFK_RESTRICT0 : NFK_RESTRICT_C), k_residual_restrict<<<d.grid, d.block, 0, g->stream>>>(L.z, L.r, L.ax, L.ay, L.az, L.c, L.nx, L.ny, L.nz, L.pax, C.r, C.nx, C.ny, C.nz, L.fz, st));
@@ -1618,7 +1654,7 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
   }
   for (int l = (coop ? 0 : nb - 1); l >= 0; --l) {
     NfLevel &L = g->lv[l], &C = g->lv[l + 1];
-    if (L.vec && fused) {
+    if (L.vec && fused && nf_omega(g, l) == 1.0f) {
       const int kch = nf_kch(L.nx / 4, L.ny, L.nz, NF_KCH_MG);
       NfDims d = nf_vdims(L.nx / 4, L.ny, L.nz, kch);
       const int nu = l == 0 ? g->nu_post : nf_nu_coarse(g, l);

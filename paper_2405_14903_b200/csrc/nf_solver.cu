@@ -861,7 +861,7 @@ bool nf_batch_ok(nf_grid **G, int n) {
     if (!g->weights_set || g->force_generic || g->coarse_ctas <= 0 || g->coarse_ctas != a->coarse_ctas) return false;
     if (!nf_update_down1_ok(g) || !apply_vec_ok(L, g->p, g->q) || !apply_vec_ok(L, g->p2, L.z) || (nc & 3)) return false;
     if (!vec_ok(g->r_alt, L.r, g->b0, g->b0, nc) || !g->d_coarse) return false;
-    if (g->nu_pre != a->nu_pre || g->nu_post != a->nu_post || g->nu_l1 != a->nu_l1 || g->nu_deep != a->nu_deep) return false;
+    if (g->nu_pre != a->nu_pre || g->nu_post != a->nu_post || g->nu_l1 != a->nu_l1 || g->nu_deep != a->nu_deep || g->omega_deep != a->omega_deep) return false;
     for (int f = 0; f < e; ++f)
       if (G[f] == g) return false;
   }

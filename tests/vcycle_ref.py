@@ -69,9 +69,10 @@ def _diag(a):
     return au[:, :, :-1] + au[:, :, 1:] + av[:, :-1, :] + av[:, 1:, :] + aw[:-1] + aw[1:]
 
 
-def vcycle(r, alpha, c, singular, nu_fine=1, nu_l1=1, nu_deep=1):
+def vcycle(r, alpha, c, singular, nu_fine=1, nu_l1=1, nu_deep=1, omega_deep=1.4):
     """nu_fine / nu_l1 / nu_deep: red-black sweeps before and after the coarse correction on the finest level / on
-    level 1 / on every level below that (the library's defaults: nf_set_solver_options, nf_set_coarse_sweeps)."""
+    level 1 / on every level below that (the library's defaults: nf_set_solver_options, nf_set_coarse_sweeps);
+    omega_deep: over-relaxation factor of the sweeps on the levels from 2 down (nf_set_coarse_relaxation)."""
     levels = [[x.astype(np.float64) for x in a] for a in hierarchy(alpha)]
 
     def rec(l, r, c):
@@ -84,9 +85,12 @@ def vcycle(r, alpha, c, singular, nu_fine=1, nu_l1=1, nu_deep=1):
         red = ((i + j + k) & 1) == 0
         z = np.zeros_like(r)
 
+        om = omega_deep if l >= 2 else 1.0   # over-relaxation of the sweeps on the levels from 2 down (SOR)
+
         def half(mask):
-            zn = (r + c * _nbsum(z, a)) * dinv
-            z[mask] = zn[mask]
+            zn = (1.0 - om) * z + om * (r + c * _nbsum(z, a)) * dinv
+            z[mask & act] = zn[mask & act]
+            z[mask & ~act] = 0.0
 
         if l == len(levels) - 1:
             if singular:
