@@ -1145,10 +1145,12 @@ struct NfCoarseK {
 };
 
 // The body: `cta` of `nctas` CTAs work on one environment's coarse levels; SYNC() is the barrier among exactly those.
-// MULTI: some level runs more than one sweep (P.nu).  The V(1,1) instance carries none of that code: unused, it still
-// cost 2 - 8 us per launch (register allocation and a colder instruction cache: 91 -> 99 us at 256^3, 53 -> 57 at 128^3).
+// MODE 2: some level runs more than one sweep (P.nu).  MODE 1: one sweep everywhere, but over-relaxed on the per-cell
+// levels (general residual of all children, no sweep loops).  MODE 0: V(1,1) Gauss-Seidel, which carries none of that
+// code: unused, it still cost 2 - 8 us per launch (register allocation and a colder instruction cache: 91 -> 99 us at
+// 256^3, 53 -> 57 at 128^3; the over-relaxed V(1,1) of a 128^3 grid ran 14 us slower inside the MODE 2 instance).
 // FLAT: 2-D mode (nz == 1: 2 x 2 x 1 children); the 3-D instance carries none of those bodies either.
-template <bool MULTI, bool FLAT, class SYNC>
+template <int MODE, bool FLAT, class SYNC>
 __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int nctas, float *sm,
                                                 unsigned long long *mbar, SYNC sync) {
   if (P.has_tail && cta == 0 && threadIdx.x == 0) nf_tail_prefetch(P.T, P.pack, P.minv, sm, mbar);
@@ -1208,21 +1210,21 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
       }
     }
     sync();
-    if (MULTI) {  // further pre-smoothing sweeps: red, black, red, ... (one call site: one copy of the code)
+    if (MODE == 2) {  // further pre-smoothing sweeps: red, black, red, ... (one call site: one copy of the code)
       for (int q = 0; q < 2 * (P.nu[l] - 1); ++q) {
         half(l, q & 1, nullptr);
         sync();
       }
     }
     // (the general residual is right after one sweep as well -- r - diag z is then a rounding zero on the red cells --
-    // so the MULTI instance carries that form only)
-    const bool gen = MULTI;
+    // so the MODE 1 / 2 instances carry that form only)
+    const bool gen = MODE != 0;
     if (dense) {
-      for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t, gen, MULTI && P.om[l] != 1.0f);
+      for (int t = gt; t < cnx * cny * cnz; t += gn) nf_dense_down2(D, P.r[l + 1], cnx, cny, t, gen, MODE != 0 && P.om[l] != 1.0f);
     } else {
       for (int t = gt; t < nx4 * cny * cnz; t += gn) {
         const int i0 = 4 * (t % nx4), J = (t / nx4) % cny, K = t / (nx4 * cny);
-        nf_down2_body<FLAT ? 1 : 2, MULTI>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
+        nf_down2_body<FLAT ? 1 : 2, MODE != 0>(L, P.z[l], P.r[l + 1], cnx, cny, i0, J, K, P.r[l]);
       }
     }
     sync();
@@ -1253,7 +1255,7 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
     }
     sync();
     // the red half sweep, then (black, red) once more per further sweep -- one call site
-    for (int q = 0; q < (MULTI ? 2 * P.nu[l] - 1 : 1); ++q) {
+    for (int q = 0; q < (MODE == 2 ? 2 * P.nu[l] - 1 : 1); ++q) {
       if (q) sync();
       half(l, q & 1, q == 0 ? P.z[l + 1] : nullptr);  // (the first red half sweep prolongs its own old value)
     }
@@ -1261,14 +1263,14 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
   }
 }
 
-template <bool MULTI, bool FLAT>
+template <int MODE, bool FLAT>
 __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse(const __grid_constant__ NfCoarseK P,
                                                                  const NfSolveState *st) {
   if (st && st->done) return;  // (uniform over the grid: written by an earlier kernel)
   extern __shared__ __align__(16) float sm[];
   __shared__ unsigned long long mbar;
   cg::grid_group grid = cg::this_grid();
-  nf_vcoarse_body<MULTI, FLAT>(P, (int)blockIdx.x, (int)gridDim.x, sm, &mbar, [&]() { grid.sync(); });
+  nf_vcoarse_body<MODE, FLAT>(P, (int)blockIdx.x, (int)gridDim.x, sm, &mbar, [&]() { grid.sync(); });
 }
 
 // Batched: ONE cooperative launch runs the coarse levels of up to NF_BATCH_MAX equally sized
@@ -1283,7 +1285,7 @@ struct NfCoarseBatchK {
   const NfSolveState *st[NF_BATCH_MAX];
   const NfCoarseK *P[NF_BATCH_MAX];  // (device copies: one NfCoarseK is ~1.7 KB, sixteen would not fit the parameters)
 };
-template <bool MULTI>
+template <int MODE>
 __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_constant__ NfCoarseBatchK B) {
   const int e = (int)blockIdx.x / B.nctas, cta = (int)blockIdx.x - e * B.nctas;
   unsigned *bar = B.bar[e];
@@ -1302,7 +1304,7 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_c
   __syncthreads();
   unsigned target = B.base[e];
   const unsigned nctas = (unsigned)B.nctas;
-  nf_vcoarse_body<MULTI, false>(sP, cta, B.nctas, sm, &mbar, [&]() {
+  nf_vcoarse_body<MODE, false>(sP, cta, B.nctas, sm, &mbar, [&]() {
     __syncthreads();
     if (threadIdx.x == 0) {
       __threadfence();
@@ -1324,8 +1326,9 @@ static inline int nf_nu_coarse(const nf_grid *g, int l) { return l <= 1 ? g->nu_
 // residual; the finest level's and level 1's fused bodies are plain Gauss-Seidel), never in 2-D mode
 static inline float nf_omega(const nf_grid *g, int l) { return (l >= 2 && g->nz != 1) ? g->omega_deep : 1.0f; }
 // some grid-phase level of the coarse kernel runs more than one sweep
-static inline bool nf_coarse_multi(const nf_grid *g) {
-  return g->nu_l1 > 1 || ((g->nu_deep > 1 || (g->omega_deep != 1.0f && g->nz != 1)) && g->tail > 2);
+static inline int nf_coarse_mode(const nf_grid *g) {  // the instance of the coarse kernel (nf_vcoarse_body's MODE)
+  if (g->nu_l1 > 1 || (g->nu_deep > 1 && g->tail > 2)) return 2;
+  return (g->omega_deep != 1.0f && g->nz != 1 && g->tail > 2) ? 1 : 0;
 }
 #define NF_TAIL_SMEM_MAX 231424  // dynamic shared memory of k_tail / k_vcoarse (226 KB of the 227 KB a CTA may use)
 
@@ -1390,12 +1393,14 @@ void nf_mg_plan(nf_grid *g) {
 int nf_mg_init(nf_grid *g) {
   const int smem = NF_TAIL_SMEM_MAX;
   NF_CUDA(g, cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
-  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
+  NF_CUDA(g, cudaFuncSetAttribute(k_vcoarse_b<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem - 4096));
   NF_CUDA(g, cudaFuncSetAttribute(k_coarse_inverse, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (NF_DIRECT_MAX * NF_DIRECT_MAX + 2 * NF_DIRECT_MAX) * (int)sizeof(double)));
   // the cooperative coarse kernel: one CTA per SM; needs a tail, at least one vec level below the finest one, and
@@ -1409,7 +1414,7 @@ int nf_mg_init(nf_grid *g) {
     NF_CUDA(g, cudaGetDevice(&dev));
     NF_CUDA(g, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     NF_CUDA(g, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
-    NF_CUDA(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_vcoarse<true, false>, NF_TAIL_THREADS, tail_smem_bytes(g)));
+    NF_CUDA(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_vcoarse<2, false>, NF_TAIL_THREADS, tail_smem_bytes(g)));
     if (all_vec && coop && per_sm >= 1) {
       // One CTA per 4096 cells of the first coarse level, at least 8, at most one per SM.  A cooperative grid is
       // resident as a whole: sized for the level instead of for the machine, the coarse kernels of several small
@@ -1553,7 +1558,7 @@ int nf_vcycle_batch(nf_grid **G, int n, const NfBatchK &Bin, int slot) {
     }
     for (int e = 0; e < n; ++e) G[e]->cbar_count += (unsigned)(CB.nbar * CB.nctas);
     void *args[] = {(void *)&CB};
-    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel(nf_coarse_multi(g) ? (void *)k_vcoarse_b<true> : (void *)k_vcoarse_b<false>, dim3(n * g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
+    NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel(nf_coarse_mode(g) == 2 ? (void *)k_vcoarse_b<2> : (nf_coarse_mode(g) == 1 ? (void *)k_vcoarse_b<1> : (void *)k_vcoarse_b<0>), dim3(n * g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
   }
   B.nzc = (int)d.grid.z;
   dim3 gb = d.grid;
@@ -1631,9 +1636,11 @@ int nf_vcycle_impl(nf_grid *g, bool with_dot, int slot, bool skip_down1) {
     fill_coarse(g, &P);
     const NfSolveState *stc = st;
     void *args[] = {(void *)&P, (void *)&stc};
-    const bool multi = nf_coarse_multi(g), flat = g->nz == 1;
-    void *kfun = flat ? (multi ? (void *)k_vcoarse<true, true> : (void *)k_vcoarse<false, true>)
-                      : (multi ? (void *)k_vcoarse<true, false> : (void *)k_vcoarse<false, false>);
+    const int mode = nf_coarse_mode(g);
+    const bool flat = g->nz == 1;  // (2-D grids are never over-relaxed: mode 0 or 2)
+    void *kfun = flat ? (mode == 2 ? (void *)k_vcoarse<2, true> : (void *)k_vcoarse<0, true>)
+                      : (mode == 2 ? (void *)k_vcoarse<2, false>
+                                   : (mode == 1 ? (void *)k_vcoarse<1, false> : (void *)k_vcoarse<0, false>));
     NF_LAUNCH(g, NFK_VEC_C, cudaLaunchCooperativeKernel(kfun, dim3(g->coarse_ctas), dim3(NF_TAIL_THREADS), args, tail_smem_bytes(g), g->stream));
   } else if (has_tail) {
     NfTailK T;
