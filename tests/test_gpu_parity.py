@@ -830,23 +830,28 @@ def test_sweep_settings_api_and_solution_independence(torch, api):
     for bad in ((0, 1), (1, 0), (9, 1), (1, 9)):
         assert lib.nf_set_coarse_sweeps(g.h, bad[0], bad[1]) == -1
     assert g.sweeps() == (1, 1, 1, 1)
+    assert abs(g.coarse_relaxation() - 1.4) < 1e-6
+    for bad in (0.9, 2.0, float("nan")):
+        assert lib.nf_set_coarse_relaxation(g.h, bad) == -1
+    assert abs(g.coarse_relaxation() - 1.4) < 1e-6
     g.set_solid(dev(torch, blob_sdf(nx, ny, nz, 3)))
     act = orc.active_cells([a.cpu().numpy().astype(np.float64) for a in g.get_weights()])
     rhs = (np.random.default_rng(8).standard_normal((nz, ny, nx)) * act).astype(np.float32)
     ref, its = None, {}
     for flags in (0, 2):
-        for nu in ((1, 1), (1, 2), (2, 3), (3, 1)):
+        for nu, om in (((1, 1), 1.0), ((1, 2), 1.4), ((2, 3), 1.0), ((3, 1), 1.7), ((1, 1), 1.4)):
             g.set_solver_options(1, 1, flags)
             g.set_coarse_sweeps(*nu)
+            g.set_coarse_relaxation(om)
             assert g.sweeps() == (1, 1) + nu
             p = torch.zeros(g.shape_p, device="cuda")
             assert g.solve(dev(torch, rhs), p, tol=1e-7, maxit=200) == 0
-            its[(flags, nu)] = g.last_solve_info()["iters"]
+            its[(flags, nu, om)] = g.last_solve_info()["iters"]
             if ref is None:
                 ref = host(p)
-            assert rel(host(p), ref) < 2e-5, (flags, nu)
-    assert its[(0, (2, 3))] <= its[(0, (1, 1))]
-    assert its[(0, (1, 1))] == its[(2, (1, 1))] or abs(its[(0, (1, 1))] - its[(2, (1, 1))]) <= 1
+            assert rel(host(p), ref) < 2e-5, (flags, nu, om)
+    assert its[(0, (2, 3), 1.0)] <= its[(0, (1, 1), 1.0)]
+    assert abs(its[(0, (1, 1), 1.0)] - its[(2, (1, 1), 1.0)]) <= 1 and abs(its[(0, (1, 1), 1.4)] - its[(2, (1, 1), 1.4)]) <= 1
     g.close()
     big = api.Grid(192, 192, 192, 1.0 / 192)   # 7.1 M cells: the large-grid default
     assert big.sweeps() == (1, 1, 2, 3)
