@@ -48,12 +48,14 @@ struct NfLvK {
   float c, ic;
   int nx, ny, nz, pax;
   int fz;  // z coarsening factor towards the next level: 2, or 1 in 2-D mode (nz == 1)
+  float om;  // over-relaxation factor of the level's sweeps in the 4-cell bodies (1 outside the cooperative kernel)
 };
 static inline NfLvK nf_lvk(const NfLevel &L) {
   NfLvK K;
   K.ax = L.ax; K.ay = L.ay; K.az = L.az; K.code = L.code; K.idg = L.idg;
   K.c = L.c; K.ic = 1.0f / L.c; K.nx = L.nx; K.ny = L.ny; K.nz = L.nz; K.pax = L.pax;
   K.fz = L.fz;
+  K.om = 1.0f;
   return K;
 }
 

@@ -65,7 +65,9 @@ __device__ __forceinline__ float4 nf_down1_core(const NfLvK &L, F4 R4, F1 R1, fl
   if ((C.c4 & 0x80808080u) == 0x80808080u) {
     // all four cells are deep interior (NF_CODE_DEEP): every diagonal involved is 6c, every weight is 1, and no
     // neighbour code is needed
-    const float g6 = L.ic * (1.0f / 6.0f);
+    // (L.om: over-relaxation, 1 on the finest level -- from the zero guess a red cell gets om r / diag, a black one
+    // om (r + c sum of those) / diag)
+    const float g6 = L.om * (L.ic * (1.0f / 6.0f));
     const float te = re;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
@@ -74,7 +76,7 @@ __device__ __forceinline__ float4 nf_down1_core(const NfLvK &L, F4 R4, F1 R1, fl
       } else {
         const float tl = q > 0 ? C.v[q - 1] : te, th = q < 3 ? C.v[q + 1] : te;
         const float sum = ((tl + th) + (yl[q] + yh[q])) + (zl[q] + zh[q]);
-        out[q] = (C.v[q] + (1.0f / 6.0f) * sum) * g6;
+        out[q] = (C.v[q] + (L.om * (1.0f / 6.0f)) * sum) * g6;
       }
     }
     *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
@@ -89,9 +91,9 @@ __device__ __forceinline__ float4 nf_down1_core(const NfLvK &L, F4 R4, F1 R1, fl
   nf_unpack4(nf_ld4(L.idg, id + sz, k + 1 < nz), gzh);
   nf_unpack4(nf_ld4(L.idg, id, true), idg);
 #pragma unroll
-  for (int q = 0; q < 4; ++q) t[q] = C.v[q] * idg[q];
+  for (int q = 0; q < 4; ++q) t[q] = L.om * (C.v[q] * idg[q]);
   // the x-neighbour outside the segment that a black cell needs: left of q = 0 (PAR = 1) or right of q = 3 (PAR = 0)
-  const float te = re * (PAR ? nf_ld1(L.idg, id - 1, i0 > 0) : nf_ld1(L.idg, id + 4, i0 + 4 < nx));
+  const float te = L.om * (re * (PAR ? nf_ld1(L.idg, id - 1, i0 > 0) : nf_ld1(L.idg, id + 4, i0 + 4 < nx)));
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     if (((q + PAR) & 1) == 0) {
@@ -100,11 +102,11 @@ __device__ __forceinline__ float4 nf_down1_core(const NfLvK &L, F4 R4, F1 R1, fl
       const NfW6 w = nf_code_w6(L, nf_code_at(C.c4, q), i0 + q, j, k);
       const float tl = q > 0 ? t[q - 1] : te, th = q < 3 ? t[q + 1] : te;
       float s = w.xl * tl + w.xh * th;
-      s += w.yl * (yl[q] * gyl[q]);
-      s += w.yh * (yh[q] * gyh[q]);
-      s += w.zl * (zl[q] * gzl[q]);
-      s += w.zh * (zh[q] * gzh[q]);
-      out[q] = (C.v[q] + L.c * s) * idg[q];
+      s += w.yl * (L.om * (yl[q] * gyl[q]));
+      s += w.yh * (L.om * (yh[q] * gyh[q]));
+      s += w.zl * (L.om * (zl[q] * gzl[q]));
+      s += w.zh * (L.om * (zh[q] * gzh[q]));
+      out[q] = L.om * ((C.v[q] + L.c * s) * idg[q]);
     }
   }
   *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
@@ -248,14 +250,22 @@ __device__ __forceinline__ void nf_down2_body(const NfLvK &L, const float *z, fl
         nf_unpack4(dk == 0 ? nf_ld4(z, id - sz, k > 0) : nf_ld4(z, id + sz, k + 1 < nz), zo);
       else
         zo[0] = zo[1] = zo[2] = zo[3] = 0.0f;  // (one layer between closed walls: both z neighbours are ghosts)
-      const float xe = par == 0 ? nf_ld1(z, id - 1, i0 > 0) : nf_ld1(z, id + 4, i0 + 4 < nx);
+      // (over-relaxed level, L.om != 1: the black children carry a residual too -- all four cells, both x-edges)
+      const bool allc = GEN && L.om != 1.0f;
+      float xel, xer;
+      if (allc) {
+        xel = nf_ld1(z, id - 1, i0 > 0);
+        xer = nf_ld1(z, id + 4, i0 + 4 < nx);
+      } else {
+        xel = xer = par == 0 ? nf_ld1(z, id - 1, i0 > 0) : nf_ld1(z, id + 4, i0 + 4 < nx);
+      }
       const bool open4 = (cc[dk][dj] & 0x7f7f7f7fu) == 0x3f3f3f3fu;  // all four cells: six open faces
       float rr[4];
       if (GEN) nf_unpack4(nf_ld4(r, id, true), rr);
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
-        if (((q + par) & 1) != 0) continue;  // red children only
-        const float xl = q > 0 ? zc[dk][dj][q - 1] : xe, xh = q < 3 ? zc[dk][dj][q + 1] : xe;
+        if (!allc && ((q + par) & 1) != 0) continue;  // red children only
+        const float xl = q > 0 ? zc[dk][dj][q - 1] : xel, xh = q < 3 ? zc[dk][dj][q + 1] : xer;
         const float yl = dj == 0 ? yo[q] : zc[dk][0][q], yh = dj == 0 ? zc[dk][1][q] : yo[q];
         const float zl = dk == 0 ? zo[q] : zc[0][dj][q], zh = (FZ == 2 && dk == 0) ? zc[FZ - 1][dj][q] : zo[q];
         float s;
@@ -367,14 +377,17 @@ __device__ __forceinline__ void nf_up1_body(const NfLvK &L, float *z, const floa
   for (int q = 0; q < 4; ++q) {
     if (((q + PAR) & 1) == 0) continue;
     const float xl = q > 0 ? zp[q - 1] : xe, xh = q < 3 ? zp[q + 1] : xe;
+    // (over-relaxed, L.om != 1: the old value is the PROLONGED one; an inactive cell stays 0)
     if (open4) {
       const float s = ((xl + xh) + (yl[q] + yh[q])) + (zl[q] + zh[q]);
       out[q] = (rr[q] + L.c * s) * g6;
+      if (L.om != 1.0f) out[q] = (1.0f - L.om) * zp[q] + L.om * out[q];
     } else {
       const unsigned code = nf_code_at(c4, q);
       const NfW6 w = nf_code_w6(L, code, i0 + q, j, k);
       const float s = ((w.xl * xl + w.xh * xh) + (w.yl * yl[q] + w.yh * yh[q])) + (w.zl * zl[q] + w.zh * zh[q]);
       out[q] = (rr[q] + L.c * s) * ig[q];
+      if (L.om != 1.0f) out[q] = ig[q] > 0.0f ? (1.0f - L.om) * zp[q] + L.om * out[q] : 0.0f;
     }
   }
   *reinterpret_cast<float4 *>(z + id) = make_float4(out[0], out[1], out[2], out[3]);
@@ -426,8 +439,11 @@ __global__ void __launch_bounds__(256, 4) k_up1_b(const __grid_constant__ NfBatc
 }
 
 // Red half sweep in place (black neighbours are final); returns r.z over the 4 cells.
+// zcp != nullptr (over-relaxed levels only): the cells' old values have not been prolonged yet -- the first red half sweep
+// after nf_up1_body, which leaves the red cells alone; cnx, cny: the coarse level's extents.
 template <int PAR>
-__device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const float *r, int i0, int j, int k) {
+__device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const float *r, int i0, int j, int k,
+                                             const float *zcp = nullptr, int cnx = 0, int cny = 0) {
   const int nx = L.nx, ny = L.ny, nz = L.nz;
   const nf_idx sy = nx, sz = (nf_idx)nx * ny;
   const nf_idx id = ((nf_idx)k * ny + j) * nx + i0;
@@ -446,18 +462,26 @@ __device__ __forceinline__ float nf_up2_body(const NfLvK &L, float *z, const flo
   const float g6 = L.ic * (1.0f / 6.0f);
   float ig[4];
   nf_unpack4(nf_ld4(L.idg, id, !open4), ig);
+  float pz[2] = {0.0f, 0.0f};  // the coarse values under cells 0,1 / 2,3 (over-relaxed first red sweep)
+  if (zcp) {
+    const float2 b = *reinterpret_cast<const float2 *>(zcp + ((nf_idx)(L.fz == 2 ? k >> 1 : k) * cny + (j >> 1)) * cnx + (i0 >> 1));
+    pz[0] = b.x; pz[1] = b.y;
+  }
 #pragma unroll
   for (int q = 0; q < 4; ++q) {
     if (((q + PAR) & 1) == 0) {
       const float xl = q > 0 ? zc[q - 1] : xe, xh = q < 3 ? zc[q + 1] : xe;
+      const float zo = zc[q] + pz[q >> 1];
       if (open4) {
         const float s = ((xl + xh) + (yl[q] + yh[q])) + (zl[q] + zh[q]);
         zc[q] = (rr[q] + L.c * s) * g6;
+        if (L.om != 1.0f) zc[q] = (1.0f - L.om) * zo + L.om * zc[q];
       } else {
         const unsigned code = nf_code_at(c4, q);
         const NfW6 w = nf_code_w6(L, code, i0 + q, j, k);
         const float s = ((w.xl * xl + w.xh * xh) + (w.yl * yl[q] + w.yh * yh[q])) + (w.zl * zl[q] + w.zh * zh[q]);
         zc[q] = (rr[q] + L.c * s) * ig[q];
+        if (L.om != 1.0f) zc[q] = ig[q] > 0.0f ? (1.0f - L.om) * zo + L.om * zc[q] : 0.0f;
       }
     }
   }
@@ -1185,9 +1209,9 @@ __device__ __forceinline__ void nf_vcoarse_body(const NfCoarseK &P, int cta, int
       for (int t = gt; t < nx4 * ny * nz; t += gn) {
         const int i0 = 4 * (t % nx4), j = (t / nx4) % ny, k = t / (nx4 * ny);
         if ((j + k + color) & 1)
-          nf_up2_body<1>(L, P.z[l], P.r[l], i0, j, k);
+          nf_up2_body<1>(L, P.z[l], P.r[l], i0, j, k, zcp, P.lv[l + 1].nx, P.lv[l + 1].ny);
         else
-          nf_up2_body<0>(L, P.z[l], P.r[l], i0, j, k);
+          nf_up2_body<0>(L, P.z[l], P.r[l], i0, j, k, zcp, P.lv[l + 1].nx, P.lv[l + 1].ny);
       }
     }
   };
@@ -1322,13 +1346,13 @@ __global__ void __launch_bounds__(NF_TAIL_THREADS, 1) k_vcoarse_b(const __grid_c
 // host side
 // ------------------------------------------------------------------------------------------------------------
 static inline int nf_nu_coarse(const nf_grid *g, int l) { return l <= 1 ? g->nu_l1 : g->nu_deep; }
-// over-relaxation of the red-black sweeps: the levels from 2 down (their bodies carry the old value and the full
-// residual; the finest level's and level 1's fused bodies are plain Gauss-Seidel), never in 2-D mode
-static inline float nf_omega(const nf_grid *g, int l) { return (l >= 2 && g->nz != 1) ? g->omega_deep : 1.0f; }
+// over-relaxation of the red-black sweeps: every level below the finest (their bodies carry the old value and the full
+// residual; the finest level's fused kernels are plain Gauss-Seidel), never in 2-D mode
+static inline float nf_omega(const nf_grid *g, int l) { return (l >= 1 && g->nz != 1) ? g->omega_deep : 1.0f; }
 // some grid-phase level of the coarse kernel runs more than one sweep
 static inline int nf_coarse_mode(const nf_grid *g) {  // the instance of the coarse kernel (nf_vcoarse_body's MODE)
   if (g->nu_l1 > 1 || (g->nu_deep > 1 && g->tail > 2)) return 2;
-  return (g->omega_deep != 1.0f && g->nz != 1 && g->tail > 2) ? 1 : 0;
+  return (g->omega_deep != 1.0f && g->nz != 1) ? 1 : 0;
 }
 #define NF_TAIL_SMEM_MAX 231424  // dynamic shared memory of k_tail / k_vcoarse (226 KB of the 227 KB a CTA may use)
 
@@ -1479,6 +1503,7 @@ static void fill_coarse(const nf_grid *g, NfCoarseK *P) {
   P->dense_from = NF_MAX_LEVELS;
   for (int l = 0; l < nl; ++l) {
     P->lv[l] = nf_lvk(g->lv[l]);
+    P->lv[l].om = P->om[l];  // (the 4-cell bodies of level 1 read it from the level's own table)
     P->z[l] = g->lv[l].z;
     P->r[l] = g->lv[l].r;
     P->pk[l] = g->lv[l].pk;

@@ -72,7 +72,7 @@ def _diag(a):
 def vcycle(r, alpha, c, singular, nu_fine=1, nu_l1=1, nu_deep=1, omega_deep=1.4):
     """nu_fine / nu_l1 / nu_deep: red-black sweeps before and after the coarse correction on the finest level / on
     level 1 / on every level below that (the library's defaults: nf_set_solver_options, nf_set_coarse_sweeps);
-    omega_deep: over-relaxation factor of the sweeps on the levels from 2 down (nf_set_coarse_relaxation)."""
+    omega_deep: over-relaxation factor of the sweeps on every level below the finest (nf_set_coarse_relaxation)."""
     levels = [[x.astype(np.float64) for x in a] for a in hierarchy(alpha)]
 
     def rec(l, r, c):
@@ -85,7 +85,7 @@ def vcycle(r, alpha, c, singular, nu_fine=1, nu_l1=1, nu_deep=1, omega_deep=1.4)
         red = ((i + j + k) & 1) == 0
         z = np.zeros_like(r)
 
-        om = omega_deep if l >= 2 else 1.0   # over-relaxation of the sweeps on the levels from 2 down (SOR)
+        om = omega_deep if l >= 1 else 1.0   # over-relaxation of the sweeps on every level below the finest (SOR)
 
         def half(mask):
             zn = (1.0 - om) * z + om * (r + c * _nbsum(z, a)) * dinv
