@@ -107,13 +107,13 @@ int nf_set_coarse_sweeps(nf_grid *g, int nu_level1, int nu_deeper);
  * (the defaults depend on the grid size: nf_grid_create picks 1, 1 and 1, 1 below 3 M cells, 2, 3 from there on).
  * Any pointer may be NULL. */
 int nf_get_sweeps(nf_grid *g, int *nu_fine_pre, int *nu_fine_post, int *nu_level1, int *nu_deeper);
-/* Over-relaxation factor omega of the red-black sweeps on the levels from 2 down (SOR: z <- (1 - omega) z + omega GS(z);
- * 1 <= omega < 2, NF_ERR_INVALID otherwise; 1 = Gauss-Seidel).  Pre- and post-smoother use the same factor in mirrored
- * order, so the V-cycle stays symmetric positive definite for PCG.  Costs no phase and no pass: those levels' bodies
- * carry the old value and restrict the full residual of all eight children (the finest level and level 1 run their
- * fused 4-cell bodies, which are plain Gauss-Seidel, whatever this says; 2-D grids ignore it).  Default 1.4 (measured
- * on the channel-gate, sphere-field and chamber workloads).  May be called at any time between
- * solves; handles solved together by the *_batch calls must agree. */
+/* Over-relaxation factor omega of the red-black sweeps on every level below the finest (SOR: z <- (1 - omega) z +
+ * omega GS(z); 1 <= omega < 2, NF_ERR_INVALID otherwise; 1 = Gauss-Seidel).  Pre- and post-smoother use the same factor
+ * in mirrored order, so the V-cycle stays symmetric positive definite for PCG.  Costs no phase and no pass: those
+ * levels' bodies carry the old value and restrict the full residual of all eight children (the finest level's fused
+ * kernels are plain Gauss-Seidel whatever this says; 2-D grids ignore it).  Default 1.4 (measured on the channel-gate,
+ * sphere-field and chamber workloads).  May be called at any time between solves; handles solved
+ * together by the *_batch calls must agree. */
 int nf_set_coarse_relaxation(nf_grid *g, float omega);
 float nf_get_coarse_relaxation(nf_grid *g);
 

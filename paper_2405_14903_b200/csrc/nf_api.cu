@@ -68,8 +68,8 @@ extern "C" int nf_grid_create(int nx, int ny, int nz, float dx, nf_grid **out) {
     g->nu_l1 = large ? 2 : 1;
     g->nu_deep = large ? 3 : 1;
   }
-  // Over-relaxation of the sweeps on the levels from 2 down (nf_set_coarse_relaxation overrides): free of phases and
-  // passes.  Forward + adjoint solve, ms, omega = 1 / 1.3 / 1.4 / 1.5 / 1.6: channel-gate 256^3 15.7 / 15.5 / 14.3 / 14.3 /
+  // Over-relaxation of the sweeps on every level below the finest (nf_set_coarse_relaxation overrides): free of phases
+  // and passes.  Forward + adjoint solve, ms, omega = 1 / 1.3 / 1.4 / 1.5 / 1.6 on the levels from 2 down (level 1 added later): channel-gate 256^3 15.7 / 15.5 / 14.3 / 14.3 /
   // 15.0, 128^3 4.36 / 4.20 / 4.09 / 3.96 / 3.96, 64^3 2.42 / 2.32 / 2.30 / 2.18 / 2.23; sphere field 128^3 2.34 / 2.25 / 2.26 /
   // 2.42 / 2.57 (256^3: 6.1 throughout); chamber 128^3 4.01 / 4.05 / 3.91 / 4.17 / 4.30.
   g->omega_deep = 1.4f;

@@ -153,7 +153,7 @@ struct nf_grid {
   long long nact;
   int nu_pre, nu_post;  // red-black sweeps before / after the coarse correction on the FINEST level
   int nu_l1, nu_deep;   // ... on level 1 / on every level below that (pre = post; nf_set_coarse_sweeps)
-  float omega_deep;     // over-relaxation factor of the sweeps on the levels from 2 down (nf_set_coarse_relaxation)
+  float omega_deep;     // over-relaxation factor of the sweeps on every level below the finest (nf_set_coarse_relaxation)
   bool warm;     // flag 8 of nf_set_solver_options: caller-provided solution arrays hold the initial guess
   bool refresh;  // true-residual refresh between two PCG phases (default on; flag 4 of nf_set_solver_options: off)
   bool force_generic;  // test hook: run the generic (fp32-weight, one colour per launch) kernels everywhere
